@@ -1,0 +1,268 @@
+"""ctypes shim over oracle/tridsk_oracle.c -- the plain fp64 CPU oracle.
+
+TEST INFRASTRUCTURE: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+``--impl reference`` legs may import this.  It never imports the CUDA package and shares no
+code with it.  Argument marshalling only; every number is computed in tridsk_oracle.c, except
+O13 (top-k = a lexicographic sort, done here with numpy.lexsort) and E_screen.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tridsk_oracle.c")
+_SO = os.path.join(_HERE, "_tridsk_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2, no -ffast-math."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _SO, _SRC, "-lm"])
+    return _SO
+
+
+class Params(C.Structure):
+    _fields_ = [(n, C.c_double) for n in (
+        "w_long", "w_clash", "w_hbond", "long_mu", "long_two_sigma2", "long_dmax",
+        "hb_mu", "hb_sigma", "hb_dmax", "hb_dclash", "d_floor", "k_wall",
+        "beta", "lr", "adam_b1", "adam_b2", "adam_eps", "pert_trans", "pert_rot", "w_tor")] + [
+        ("n_refine", C.c_int), ("clash_literal", C.c_int)]
+
+
+class _Types(C.Structure):
+    _fields_ = [("n_types", C.c_int), ("radius", C.c_void_p), ("role", C.c_void_p)]
+
+
+class _Grid(C.Structure):
+    _fields_ = [("g", C.c_void_p), ("n_types", C.c_int), ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("origin", C.c_double * 3), ("spacing", C.c_double)]
+
+
+class _Ligand(C.Structure):
+    _fields_ = [("n", C.c_int), ("T", C.c_int), ("P", C.c_int), ("ref", C.c_void_p), ("type", C.c_void_p),
+                ("frag", C.c_void_p), ("tor_a", C.c_void_p), ("tor_b", C.c_void_p), ("tor_parent", C.c_void_p),
+                ("pairs", C.c_void_p)]
+
+
+class StepRec(C.Structure):
+    _fields_ = [("e_prop", C.c_double), ("e_cur", C.c_double), ("u", C.c_double), ("accept", C.c_int),
+                ("entity", C.c_int), ("min_abs_g", C.c_double), ("p_accept", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_field_brute.restype = C.c_double
+        _lib.orc_derive_pairs.restype = C.c_int
+        assert _lib.orc_sizeof_params() == C.sizeof(Params)
+        assert _lib.orc_sizeof_step_rec() == C.sizeof(StepRec)
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _d3(v):
+    return (C.c_double * 3)(*[float(x) for x in v])
+
+
+def default_params(**kw) -> Params:
+    p = Params()
+    lib().orc_default_params(C.byref(p))
+    for k, v in kw.items():
+        setattr(p, k, v)
+    return p
+
+
+class Types:
+    def __init__(self, radius, role):
+        self.radius = np.ascontiguousarray(radius, dtype=np.float64)
+        self.role = np.ascontiguousarray(role, dtype=np.uint8)
+        self.c = _Types(len(self.radius), _p(self.radius).value, _p(self.role).value)
+
+
+class Grid:
+    """Wraps an fp32 [n_types][nz][ny][nx] array (O4); the hot-path oracle reads it as handed."""
+
+    def __init__(self, g, origin, spacing):
+        self.g = np.ascontiguousarray(g, dtype=np.float32)
+        nt, nz, ny, nx = self.g.shape
+        self.origin = np.asarray(origin, dtype=np.float64)
+        self.spacing = float(spacing)
+        self.c = _Grid(_p(self.g).value, nt, nx, ny, nz, _d3(origin), float(spacing))
+
+
+class Ligand:
+    def __init__(self, ref_xyz, atom_type, atom_frag, tor_a, tor_b, tor_parent, bond_ab=None, pairs=None):
+        self.ref = np.ascontiguousarray(ref_xyz, dtype=np.float64)
+        self.type = np.ascontiguousarray(atom_type, dtype=np.uint8)
+        self.frag = np.ascontiguousarray(atom_frag, dtype=np.uint8)
+        self.tor_a = np.ascontiguousarray(tor_a, dtype=np.uint8)
+        self.tor_b = np.ascontiguousarray(tor_b, dtype=np.uint8)
+        self.tor_parent = np.ascontiguousarray(tor_parent, dtype=np.int8)
+        self.n, self.T = len(self.type), len(self.tor_a)
+        if pairs is None:
+            pairs = derive_pairs(self.frag, bond_ab)
+        self.pairs = np.ascontiguousarray(pairs, dtype=np.uint8).reshape(-1, 2)
+        self.P = len(self.pairs)
+        self.c = _Ligand(self.n, self.T, self.P, _p(self.ref).value, _p(self.type).value, _p(self.frag).value,
+                         _p(self.tor_a).value, _p(self.tor_b).value, _p(self.tor_parent).value,
+                         _p(self.pairs).value)
+
+
+def ligand_from_batch(batch, i) -> Ligand:
+    """batch: workloads.synth.LigandBatch (plain arrays)."""
+    d = batch.one(i)
+    return Ligand(d["ref_xyz"], d["atom_type"], d["atom_frag"], d["tor_a"], d["tor_b"], d["tor_parent"],
+                  bond_ab=d["bond_ab"])
+
+
+# ------------------------------------------------------------------------------ O2..O5
+def pair(p: Params, rad_s, role_s, rad_t, role_t, d):
+    e, de = C.c_double(), C.c_double()
+    lib().orc_pair(C.byref(p), C.c_double(rad_s), C.c_ubyte(role_s), C.c_double(rad_t), C.c_ubyte(role_t),
+                   C.c_double(d), C.byref(e), C.byref(de))
+    return e.value, de.value
+
+
+def field_brute(p, ty: Types, rec_xyz, rec_type, t, x):
+    rx = np.ascontiguousarray(rec_xyz, dtype=np.float64)
+    rt = np.ascontiguousarray(rec_type, dtype=np.int32)
+    return lib().orc_field_brute(C.byref(p), C.byref(ty.c), _p(rx), _p(rt), C.c_int(len(rt)), C.c_int(t), _d3(x))
+
+
+def build_grid(p, ty: Types, rec_xyz, rec_type, origin, dims, spacing) -> Grid:
+    rx = np.ascontiguousarray(rec_xyz, dtype=np.float64)
+    rt = np.ascontiguousarray(rec_type, dtype=np.int32)
+    nx, ny, nz = dims
+    out = np.zeros((ty.c.n_types, nz, ny, nx), np.float32)
+    lib().orc_build_grid(C.byref(p), C.byref(ty.c), _p(rx), _p(rt), C.c_int(len(rt)), _d3(origin),
+                         C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(spacing), _p(out))
+    return Grid(out, origin, spacing)
+
+
+def interp(p, G: Grid, t, x):
+    e = C.c_double()
+    g = (C.c_double * 3)()
+    lib().orc_interp(C.byref(p), C.byref(G.c), C.c_int(t), _d3(x), C.byref(e), g)
+    return e.value, np.array(g[:])
+
+
+# ------------------------------------------------------------------------------ O6, O8, O9
+def derive_pairs(frag, bond_ab):
+    frag = np.ascontiguousarray(frag, dtype=np.uint8)
+    bonds = np.ascontiguousarray(bond_ab, dtype=np.uint8).reshape(-1, 2)
+    n = len(frag)
+    cap = n * (n - 1) // 2 + 1
+    out = np.zeros((cap, 2), np.uint8)
+    P = lib().orc_derive_pairs(C.c_int(n), _p(frag), _p(bonds), C.c_int(len(bonds)), _p(out), C.c_int(cap))
+    return out[:P].copy()
+
+
+def fk(L: Ligand, pose):
+    pose = np.ascontiguousarray(pose, dtype=np.float64)
+    x = np.zeros((L.n, 3))
+    lib().orc_fk(C.byref(L.c), _p(pose), _p(x))
+    return x
+
+
+def score_grad(p, ty: Types, G: Grid, L: Ligand, pose, want_grad=True):
+    """-> energy[3] (total, inter, intra), grad[6+T], coords[n,3], gatom[n,3]."""
+    pose = np.ascontiguousarray(pose, dtype=np.float64)
+    e = np.zeros(3)
+    g = np.zeros(6 + L.T)
+    x = np.zeros((L.n, 3))
+    ga = np.zeros((L.n, 3))
+    lib().orc_score_grad(C.byref(p), C.byref(ty.c), C.byref(G.c), C.byref(L.c), _p(pose), _p(e),
+                         _p(g) if want_grad else None, _p(x), _p(ga))
+    return e, g, x, ga
+
+
+def score_grad_batch(p, ty: Types, G: Grid, L: Ligand, poses):
+    poses = np.ascontiguousarray(poses, dtype=np.float64)
+    n, stride = poses.shape
+    e = np.zeros((n, 3))
+    g = np.zeros((n, 6 + L.T))
+    x = np.zeros((n, L.n, 3))
+    lib().orc_score_grad_batch(C.byref(p), C.byref(ty.c), C.byref(G.c), C.byref(L.c), _p(poses), C.c_int(n),
+                               C.c_int(stride), _p(e), _p(g), C.c_int(6 + L.T), _p(x), C.c_int(L.n))
+    return e, g, x
+
+
+# ------------------------------------------------------------------------------ O10..O12
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*ctr)
+    k = (C.c_uint32 * 2)(*key)
+    o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, o)
+    return list(o)
+
+
+def uniform4(seed, chain, step, ligand, purpose):
+    u = (C.c_double * 4)()
+    lib().orc_uniform4(C.c_uint64(seed), C.c_uint32(chain), C.c_uint32(step), C.c_uint32(ligand),
+                       C.c_uint32(purpose), u)
+    return np.array(u[:])
+
+
+def init_pose(L: Ligand, seed, chain, ligand, centre, radius):
+    pose = np.zeros(7 + L.T)
+    lib().orc_init_pose(C.byref(L.c), C.c_uint64(seed), C.c_uint32(chain), C.c_uint32(ligand), _d3(centre),
+                        C.c_double(radius), _p(pose))
+    return pose
+
+
+def mc_step(p, ty, G, L, seed, chain, step, ligand, box_min, box_max, pose, e_cur):
+    """One MC step from (pose, e_cur).  -> new pose, new e_cur, StepRec."""
+    pose = np.array(pose, dtype=np.float64)
+    ec = C.c_double(e_cur)
+    rec = StepRec()
+    lib().orc_mc_step(C.byref(p), C.byref(ty.c), C.byref(G.c), C.byref(L.c), C.c_uint64(seed), C.c_uint32(chain),
+                      C.c_uint32(step), C.c_uint32(ligand), _d3(box_min), _d3(box_max), _p(pose), C.byref(ec),
+                      C.byref(rec))
+    return pose, ec.value, rec
+
+
+def dock(p, ty, G, L, seed, ligand, n_chains, n_steps, box_min, box_max, centre, radius,
+         init_poses=None, first_step=0, want_trace=False):
+    W = 7 + L.T
+    ip = None
+    if init_poses is not None:
+        ip = np.ascontiguousarray(np.asarray(init_poses, dtype=np.float64)[:, :W])
+        assert ip.shape == (n_chains, W)
+    e_best = np.zeros(n_chains)
+    e_cur = np.zeros(n_chains)
+    pose_best = np.zeros((n_chains, W))
+    pose_cur = np.zeros((n_chains, W))
+    trace = (StepRec * (n_chains * n_steps))() if want_trace else None
+    lib().orc_dock(C.byref(p), C.byref(ty.c), C.byref(G.c), C.byref(L.c), C.c_uint64(seed), C.c_uint32(ligand),
+                   C.c_int(n_chains), C.c_int(first_step), C.c_int(n_steps), _d3(box_min), _d3(box_max),
+                   _d3(centre), C.c_double(radius), _p(ip) if ip is not None else None, C.c_int(W),
+                   _p(e_best), _p(pose_best), _p(e_cur), _p(pose_cur), trace)
+    out = dict(e_best=e_best, pose_best=pose_best, e_cur=e_cur, pose_cur=pose_cur)
+    if want_trace:
+        names = [f[0] for f in StepRec._fields_]
+        out["trace"] = {n: np.array([getattr(r, n) for r in trace]).reshape(n_chains, n_steps) for n in names}
+    return out
+
+
+# ------------------------------------------------------------------------------ O13, E_screen
+def topk(e_best, k):
+    """O13: chains sorted by (E_best, chain id) ascending, first k."""
+    e_best = np.asarray(e_best)
+    order = np.lexsort((np.arange(len(e_best)), e_best))
+    return order[:k]
+
+
+def e_screen(e_dock, n_tor, w_tor=0.01):
+    """Eq.E_screen."""
+    return e_dock / (1.0 + w_tor * n_tor)

@@ -1,0 +1,602 @@
+"""Pins for the fp64 oracle (oracle/) against what the paper and the mathematics fix.
+
+None of these retypes the oracle's own formula: each is a printed constant, a closed form at a
+special point, an invariant, a library routine (scipy / torch), brute force on a tiny input,
+or a published known answer.  CPU only.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.interpolate import RegularGridInterpolator
+from scipy.spatial.transform import Rotation
+
+from workloads import synth
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def paper_constants():
+    out = {}
+    for line in open(os.path.join(GOLD, "paper_constants.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split()[:2]
+        out[k] = float(v)
+    return out
+
+
+# --------------------------------------------------------------------------- defaults = paper's constants
+def test_default_params_are_the_papers(orc):
+    c = paper_constants()
+    p = orc.default_params()
+    assert (p.w_long, p.w_clash, p.w_hbond) == (c["w_long"], c["w_clash"], c["w_Hbond"])
+    assert p.long_dmax == c["d_max"] and p.hb_dclash == c["d_clash_hb"]
+    assert (p.hb_mu, p.hb_sigma, p.hb_dmax) == (c["hb_mu"], c["hb_sigma"], c["hb_dmax"])
+    assert p.w_tor == c["w_tor"] and p.lr == c["adam_lr"] and p.beta == c["beta"]
+    # beta makes P(accept) = 0.5 for dE = 10
+    assert abs(math.exp(-p.beta * 10.0) - c["p_accept_dE10"]) < 2e-3
+    # G2: E_long is Vina's second Gaussian exp(-((d_surf - 3)/2)^2)
+    assert p.long_mu == 3.0 and p.long_two_sigma2 == 4.0
+
+
+# --------------------------------------------------------------------------- O2 pair function, closed forms
+R_NON = (1.7, 0)      # radius, role : plain
+R_DON = (1.6, 1)      # donor
+R_ACC = (1.8, 2)      # acceptor
+
+
+def test_pair_long_closed_forms(orc):
+    p = orc.default_params()
+    dvdw = R_NON[0] + R_NON[0]
+    e, de = orc.pair(p, *R_NON, *R_NON, dvdw + 3.0)          # Gaussian centre: L = -1
+    assert e == pytest.approx(-0.2, abs=1e-15) and de == pytest.approx(0.0, abs=1e-15)
+    # Vina's second Gaussian drops to exp(-1) at surface distance 3 +/- 2
+    for s in (+2.0, -2.0):
+        d = dvdw + 3.0 + s
+        e, _ = orc.pair(p, *R_NON, *R_NON, d)
+        clash = 0.0                                           # d >= dvdw here (3.4+1 = 4.4 > 3.4)
+        assert e - clash == pytest.approx(-0.2 * math.exp(-1.0), rel=1e-14)
+    # cutoff: zero at and beyond d_max = 10, non-zero just inside
+    assert orc.pair(p, *R_NON, *R_NON, 10.0) == (0.0, 0.0)
+    assert orc.pair(p, *R_NON, *R_NON, 25.0) == (0.0, 0.0)
+    assert orc.pair(p, *R_NON, *R_NON, 10.0 - 1e-9)[0] < 0.0
+
+
+def test_pair_clash_closed_forms(orc):
+    p = orc.default_params(w_long=0.0, w_hbond=0.0)
+    dvdw = R_NON[0] + R_NON[0]
+    e, de = orc.pair(p, *R_NON, *R_NON, dvdw / math.e)        # -ln(1/e) = 1 -> 10 * 1
+    assert e == pytest.approx(10.0, rel=1e-14)
+    assert de == pytest.approx(-10.0 / (dvdw / math.e), rel=1e-14)
+    assert orc.pair(p, *R_NON, *R_NON, dvdw)[0] == 0.0         # indicator is strict
+    assert orc.pair(p, *R_NON, *R_NON, dvdw * (1 - 1e-12))[0] == pytest.approx(0.0, abs=1e-10)  # continuous
+    # H-bond pair: d_clash = 2.6; reading G3 -> no penalty for 2.6 <= d < d_vdw
+    assert orc.pair(p, *R_DON, *R_ACC, 2.6 + 1e-9)[0] == 0.0
+    assert orc.pair(p, *R_DON, *R_ACC, 3.0)[0] == 0.0
+    assert orc.pair(p, *R_DON, *R_ACC, 2.6 / math.e)[0] == pytest.approx(10.0, rel=1e-14)
+    # paper-literal indicator [d < d_vdw] (kept as an oracle-only switch): negative "penalty" in (2.6, d_vdw)
+    pl = orc.default_params(w_long=0.0, w_hbond=0.0, clash_literal=1)
+    assert orc.pair(pl, *R_DON, *R_ACC, 3.0)[0] == pytest.approx(-10.0 * math.log(3.0 / 2.6), rel=1e-14)
+    # two donors are not an H-bond pair: d_clash = d_vdw
+    assert orc.pair(p, *R_DON, *R_DON, 3.0)[0] == pytest.approx(-10.0 * math.log(3.0 / 3.2), rel=1e-14)
+    # floor (G4): finite at d -> 0, derivative zero below the floor
+    e0, de0 = orc.pair(p, *R_NON, *R_NON, 0.0)
+    assert e0 == pytest.approx(10.0 * math.log(dvdw / 0.05), rel=1e-14) and de0 == 0.0
+
+
+def test_pair_hbond_closed_forms(orc):
+    p = orc.default_params(w_long=0.0, w_clash=0.0)
+    assert orc.pair(p, *R_DON, *R_ACC, 2.88)[0] == pytest.approx(-0.6, rel=1e-15)          # Gaussian centre
+    assert orc.pair(p, *R_ACC, *R_DON, 2.88)[0] == pytest.approx(-0.6, rel=1e-15)          # symmetric in roles
+    assert orc.pair(p, *R_DON, *R_ACC, 3.4 - 1e-12)[0] == pytest.approx(-0.6 * 0.22263, rel=5e-5)  # SURVEY section 4 (5 digits)
+    assert orc.pair(p, *R_DON, *R_ACC, 3.4)[0] == 0.0
+    assert orc.pair(p, *R_DON, *R_DON, 2.88)[0] == 0.0                                     # donor/donor: none
+    assert orc.pair(p, *R_NON, *R_ACC, 2.88)[0] == 0.0
+    both = (1.7, 3)
+    assert orc.pair(p, *both, *both, 2.88)[0] == pytest.approx(-0.6, rel=1e-15)           # role 3 = donor+acceptor
+
+
+def test_pair_total_is_weighted_sum(orc):
+    """Eq.E_dock: the three terms add linearly with their weights."""
+    d = 2.4
+    full = orc.pair(orc.default_params(), *R_DON, *R_ACC, d)
+    parts = [orc.pair(orc.default_params(**{k: 0.0 for k in ks}), *R_DON, *R_ACC, d)
+             for ks in (("w_clash", "w_hbond"), ("w_long", "w_hbond"), ("w_long", "w_clash"))]
+    assert full[0] == pytest.approx(sum(x[0] for x in parts), rel=1e-14)
+    assert full[1] == pytest.approx(sum(x[1] for x in parts), rel=1e-14)
+
+
+def test_pair_derivative_vs_central_difference(orc):
+    p = orc.default_params()
+    rng = np.random.default_rng(0)
+    edges = [10.0, 3.4, 2.6, 0.05]
+    for a, b in ((R_NON, R_NON), (R_DON, R_ACC), (R_NON, R_ACC), ((2.25, 3), (1.5, 3))):
+        ed = edges + [a[0] + b[0]]
+        for d in rng.uniform(0.2, 11.0, size=200):
+            if min(abs(d - x) for x in ed) < 1e-3:
+                continue
+            h = 1e-6
+            fd = (orc.pair(p, *a, *b, d + h)[0] - orc.pair(p, *a, *b, d - h)[0]) / (2 * h)
+            assert orc.pair(p, *a, *b, d)[1] == pytest.approx(fd, rel=1e-6, abs=1e-7)
+
+
+# --------------------------------------------------------------------------- O3/O4 brute force <-> grid
+@pytest.fixture(scope="module")
+def small_system(orc):
+    rng = np.random.default_rng(7)
+    radius, role = synth.type_table(8)
+    ty = orc.Types(radius, role)
+    rec_xyz = rng.uniform(0, 6.0, size=(40, 3))
+    rec_type = rng.integers(0, 8, size=40)
+    p = orc.default_params()
+    G = orc.build_grid(p, ty, rec_xyz, rec_type, (0.5, 0.25, 0.0), (9, 8, 7), 0.375)
+    return dict(p=p, ty=ty, rec_xyz=rec_xyz, rec_type=rec_type, G=G, radius=radius, role=role)
+
+
+def test_field_of_one_atom_is_the_pair_function(orc):
+    radius, role = synth.type_table(8)
+    ty = orc.Types(radius, role)
+    p = orc.default_params()
+    for s, t, d in ((0, 1, 3.3), (2, 3, 2.9), (6, 6, 2.0), (5, 7, 7.7)):
+        f = orc.field_brute(p, ty, [[1.0, 2.0, 3.0]], [s], t, [1.0, 2.0 + d, 3.0])
+        assert f == pytest.approx(orc.pair(p, radius[s], role[s], radius[t], role[t], d)[0], rel=1e-13)
+
+
+def test_field_is_additive_over_receptor_atoms(orc, small_system):
+    S = small_system
+    x = [2.2, 3.1, 1.7]
+    tot = orc.field_brute(S["p"], S["ty"], S["rec_xyz"], S["rec_type"], 3, x)
+    parts = sum(orc.field_brute(S["p"], S["ty"], S["rec_xyz"][i:i + 1], S["rec_type"][i:i + 1], 3, x)
+                for i in range(40))
+    assert tot == pytest.approx(parts, rel=1e-12)
+
+
+def test_grid_equals_brute_force_at_every_node(orc, small_system):
+    S = small_system
+    G = S["G"]
+    nt, nz, ny, nx = G.g.shape
+    assert (nt, nz, ny, nx) == (8, 7, 8, 9)
+    rng = np.random.default_rng(1)
+    for _ in range(300):
+        t, k, j, i = rng.integers(nt), rng.integers(nz), rng.integers(ny), rng.integers(nx)
+        x = G.origin + G.spacing * np.array([i, j, k])
+        f = orc.field_brute(S["p"], S["ty"], S["rec_xyz"], S["rec_type"], int(t), x)
+        assert G.g[t, k, j, i] == np.float32(f)              # x fastest, rounded once to fp32
+
+
+# --------------------------------------------------------------------------- O5 trilinear interpolation
+def test_trilinear_exact_on_nodes(orc, small_system):
+    S = small_system
+    G = S["G"]
+    nt, nz, ny, nx = G.g.shape
+    for t in range(nt):
+        for (i, j, k) in ((0, 0, 0), (nx - 1, ny - 1, nz - 1), (3, 4, 5), (nx - 1, 0, 2), (1, ny - 1, 0)):
+            x = G.origin + G.spacing * np.array([i, j, k])
+            e, _ = orc.interp(S["p"], G, t, x)
+            assert e == pytest.approx(float(G.g[t, k, j, i]), rel=1e-13, abs=1e-13)
+
+
+def test_trilinear_exact_on_trilinear_fields(orc):
+    """A field a + b x + c y + d z + e xy + f yz + g xz + h xyz is reproduced exactly, gradient analytic."""
+    rng = np.random.default_rng(3)
+    co = rng.normal(size=8)
+    origin, h, n = np.array([-1.0, 2.0, 0.5]), 0.5, (6, 5, 7)         # nx, ny, nz ; h exact in binary
+    X, Y, Z = np.meshgrid(*(origin[c] + h * np.arange(n[c]) for c in range(3)), indexing="ij")
+
+    def F(x, y, z):
+        return co[0] + co[1] * x + co[2] * y + co[3] * z + co[4] * x * y + co[5] * y * z + co[6] * x * z + co[7] * x * y * z
+
+    vals = F(X, Y, Z).transpose(2, 1, 0)[None]                          # [1][z][y][x]
+    G = orc.Grid(vals.astype(np.float32), origin, h)
+    g64 = G.g.astype(np.float64)[0].transpose(2, 1, 0)                  # what the oracle sees (fp32-rounded nodes)
+    rgi = RegularGridInterpolator(tuple(origin[c] + h * np.arange(n[c]) for c in range(3)), g64, method="linear")
+    p = orc.default_params()
+    for _ in range(200):
+        x = origin + rng.uniform(0.0, 1.0, size=3) * h * (np.array(n) - 1)
+        e, g = orc.interp(p, G, 0, x)
+        assert e == pytest.approx(F(*x), rel=2e-6, abs=2e-6)            # fp32 node rounding only
+        assert e == pytest.approx(float(rgi(x)[0]), rel=1e-12, abs=1e-12)   # library pin
+        ga = np.array([co[1] + co[4] * x[1] + co[6] * x[2] + co[7] * x[1] * x[2],
+                       co[2] + co[4] * x[0] + co[5] * x[2] + co[7] * x[0] * x[2],
+                       co[3] + co[5] * x[1] + co[6] * x[0] + co[7] * x[0] * x[1]])
+        assert g == pytest.approx(ga, rel=1e-4, abs=1e-4)
+
+
+def test_trilinear_matches_scipy_and_fd_on_a_real_grid(orc, small_system):
+    S = small_system
+    G = S["G"]
+    nt, nz, ny, nx = G.g.shape
+    axes = tuple(G.origin[c] + G.spacing * np.arange(m) for c, m in enumerate((nx, ny, nz)))
+    rng = np.random.default_rng(5)
+    for t in (0, 2, 6):
+        rgi = RegularGridInterpolator(axes, G.g[t].astype(np.float64).transpose(2, 1, 0), method="linear")
+        for _ in range(100):
+            cell = np.array([rng.integers(nx - 1), rng.integers(ny - 1), rng.integers(nz - 1)])
+            frac = rng.uniform(0.05, 0.95, size=3)                      # strictly inside a cell
+            x = G.origin + G.spacing * (cell + frac)
+            e, g = orc.interp(S["p"], G, t, x)
+            assert e == pytest.approx(float(rgi(x)[0]), rel=1e-12, abs=1e-12)
+            h = 1e-6
+            for c in range(3):
+                dx = np.zeros(3); dx[c] = h
+                fd = (orc.interp(S["p"], G, t, x + dx)[0] - orc.interp(S["p"], G, t, x - dx)[0]) / (2 * h)
+                assert g[c] == pytest.approx(fd, rel=1e-6, abs=1e-6 * max(1.0, abs(e)))
+
+
+def test_wall_outside_the_grid(orc, small_system):
+    """G8: clamp + quadratic wall k (x - x_clamped)^2; the interpolant's own gradient is zeroed on a clamped axis."""
+    S = small_system
+    G = S["G"]
+    nt, nz, ny, nx = G.g.shape
+    hi = G.origin + G.spacing * (np.array([nx, ny, nz]) - 1)
+    x_in = G.origin + G.spacing * np.array([2.3, 3.6, 1.2])
+    for axis, sign, dist in ((0, +1, 0.7), (1, -1, 1.3), (2, +1, 0.01)):
+        x = x_in.copy()
+        edge = hi[axis] if sign > 0 else G.origin[axis]
+        x[axis] = edge + sign * dist
+        xc = x.copy(); xc[axis] = edge
+        e, g = orc.interp(S["p"], G, 1, x)
+        ec, gc = orc.interp(S["p"], G, 1, xc)
+        assert e == pytest.approx(ec + 10.0 * dist ** 2, rel=1e-12)
+        assert g[axis] == pytest.approx(sign * 2 * 10.0 * dist, rel=1e-12)
+        other = [c for c in range(3) if c != axis]
+        assert g[other] == pytest.approx(gc[other], rel=1e-12)
+
+
+# --------------------------------------------------------------------------- O8 forward kinematics
+def hand_ligand(orc):
+    """Butane-like chain along z with one torsion about the z axis, plus an off-axis tail."""
+    ref = np.array([[1.0, 0.0, -1.0], [0.0, 0.0, 0.0], [0.0, 0.0, 1.5], [1.2, 0.3, 2.0], [1.5, -0.7, 3.0]])
+    return orc.Ligand(ref, [0, 1, 2, 3, 4], [0, 0, 1, 1, 1], tor_a=[1], tor_b=[2], tor_parent=[-1],
+                      pairs=np.zeros((0, 2), np.uint8))
+
+
+def test_fk_identity_reproduces_reference(orc):
+    L = hand_ligand(orc)
+    assert orc.fk(L, [0, 0, 0, 1, 0, 0, 0, 0.0]) == pytest.approx(L.ref, abs=1e-15)
+
+
+def test_fk_one_torsion_about_z_is_the_textbook_matrix(orc):
+    L = hand_ligand(orc)
+    th = 0.7
+    x = orc.fk(L, [0, 0, 0, 1, 0, 0, 0, th])
+    Rz = np.array([[math.cos(th), -math.sin(th), 0], [math.sin(th), math.cos(th), 0], [0, 0, 1]])
+    assert x[:3] == pytest.approx(L.ref[:3], abs=1e-15)                 # root side + axis atoms fixed
+    assert x[3:] == pytest.approx((Rz @ L.ref[3:].T).T, abs=1e-14)      # right-handed about a -> b = +z
+
+
+def test_fk_rigid_part_matches_scipy_rotation(orc):
+    rng = np.random.default_rng(11)
+    batch = synth.ligands([20], [0], 8, seed=5)
+    L = orc.ligand_from_batch(batch, 0)
+    assert L.T == 0
+    for _ in range(20):
+        q = rng.normal(size=4); q /= np.linalg.norm(q)
+        t = rng.normal(size=3) * 5
+        x = orc.fk(L, np.concatenate([t, q]))
+        R = Rotation.from_quat([q[1], q[2], q[3], q[0]])                # scipy is scalar-last
+        assert x == pytest.approx(R.apply(L.ref) + t, abs=1e-13)
+        assert orc.fk(L, np.concatenate([t, -q])) == pytest.approx(x, abs=1e-13)       # q and -q
+        assert orc.fk(L, np.concatenate([t, 3.7 * q])) == pytest.approx(x, abs=1e-13)  # input renormalised
+
+
+def _dihedral(p0, p1, p2, p3):
+    b1, b2, b3 = p1 - p0, p2 - p1, p3 - p2
+    n1, n2 = np.cross(b1, b2), np.cross(b2, b3)
+    return math.atan2(np.dot(np.cross(n1, n2), b2 / np.linalg.norm(b2)), np.dot(n1, n2))
+
+
+def test_fk_preserves_internal_coordinates_and_drives_dihedrals(orc):
+    rng = np.random.default_rng(13)
+    batch = synth.ligands([30, 24, 40], [6, 3, 9], 16, seed=9)
+    for li in range(3):
+        L = orc.ligand_from_batch(batch, li)
+        bonds = batch.one(li)["bond_ab"].astype(int)
+        nbr = {a: set() for a in range(L.n)}
+        for a, b in bonds:
+            nbr[a].add(b); nbr[b].add(a)
+        rot = {(int(a), int(b)) for a, b in zip(L.tor_a, L.tor_b)}
+        is_rot = lambda a, b: (a, b) in rot or (b, a) in rot
+        for _ in range(5):
+            pose = np.concatenate([rng.normal(size=3) * 4, rng.normal(size=4), rng.uniform(-np.pi, np.pi, L.T)])
+            x = orc.fk(L, pose)
+            pose2 = pose.copy(); pose2[7:] += 2 * np.pi
+            assert orc.fk(L, pose2) == pytest.approx(x, abs=1e-12)       # theta and theta + 2 pi
+            for a, b in bonds:                                           # bond lengths
+                assert np.linalg.norm(x[a] - x[b]) == pytest.approx(np.linalg.norm(L.ref[a] - L.ref[b]), abs=1e-12)
+            for b in range(L.n):                                         # bond angles
+                nb = sorted(nbr[b])
+                for i in range(len(nb)):
+                    for j in range(i + 1, len(nb)):
+                        a, c = nb[i], nb[j]
+                        assert np.linalg.norm(x[a] - x[c]) == pytest.approx(np.linalg.norm(L.ref[a] - L.ref[c]), abs=1e-12)
+            for b, c in bonds:                                           # dihedrals a-b-c-d
+                for a in nbr[b] - {c}:
+                    for d in nbr[c] - {b}:
+                        phi, phi0 = _dihedral(x[a], x[b], x[c], x[d]), _dihedral(*L.ref[[a, b, c, d]])
+                        delta = (phi - phi0 + np.pi) % (2 * np.pi) - np.pi
+                        if not is_rot(b, c):
+                            assert abs(delta) < 1e-10                    # not driven: unchanged
+                        else:
+                            k = [i for i in range(L.T) if {int(L.tor_a[i]), int(L.tor_b[i])} == {b, c}][0]
+                            th = pose[7 + k] if (int(L.tor_a[k]), int(L.tor_b[k])) == (b, c) else pose[7 + k]
+                            want = (th + np.pi) % (2 * np.pi) - np.pi
+                            assert abs((delta - want + np.pi) % (2 * np.pi) - np.pi) < 1e-10   # driven by exactly theta_k
+
+
+def test_derive_pairs_matches_brute_force_bfs(orc):
+    """O6: pairs = {a<b : graph distance >= 4 and different fragment}; independent BFS in Python."""
+    batch = synth.ligands([12, 30, 50], [2, 6, 10], 8, seed=21)
+    for li in range(3):
+        d = batch.one(li)
+        n = len(d["atom_type"])
+        nbr = {a: [] for a in range(n)}
+        for a, b in d["bond_ab"].astype(int):
+            nbr[a].append(b); nbr[b].append(a)
+        want = []
+        for a in range(n):
+            dist = {a: 0}; frontier = [a]
+            while frontier:
+                nxt = []
+                for u in frontier:
+                    for v in nbr[u]:
+                        if v not in dist:
+                            dist[v] = dist[u] + 1; nxt.append(v)
+                frontier = nxt
+            for b in range(a + 1, n):
+                if dist[b] >= 4 and d["atom_frag"][a] != d["atom_frag"][b]:
+                    want.append((a, b))
+        got = orc.derive_pairs(d["atom_frag"], d["bond_ab"])
+        assert [tuple(x) for x in got.astype(int)] == want
+        assert len(want) > 0
+
+
+# --------------------------------------------------------------------------- O6/O7/O9 score + gradient
+@pytest.fixture(scope="module")
+def dock_system(orc):
+    """Small receptor + grid + 3 ligands, oracle-built grid."""
+    rec = synth.receptor(120, 15.0, 8, seed=31, grid_n=41, pocket_radius=4.0)
+    radius, role = synth.type_table(8)
+    ty = orc.Types(radius, role)
+    p = orc.default_params()
+    G = orc.build_grid(p, ty, rec.xyz, rec.type, rec.origin, rec.dims, rec.spacing)
+    batch = synth.ligands([12, 20, 26], [2, 4, 6], 8, seed=41)
+    return dict(rec=rec, ty=ty, p=p, G=G, batch=batch, L=[orc.ligand_from_batch(batch, i) for i in range(3)])
+
+
+def test_intra_energy_is_rigid_invariant_and_obeys_newton(orc, dock_system):
+    S = dock_system
+    rng = np.random.default_rng(17)
+    zero = orc.Grid(np.zeros((8, 41, 41, 41), np.float32), S["rec"].origin, S["rec"].spacing)
+    for L in S["L"]:
+        th = rng.uniform(-np.pi, np.pi, L.T)
+        ref_e = None
+        for _ in range(6):
+            pose = np.concatenate([7.5 + rng.uniform(-1, 1, 3), rng.normal(size=4), th])
+            e, g, x, ga = orc.score_grad(S["p"], S["ty"], zero, L, pose)
+            assert e[1] == 0.0                                           # zero grid, inside the box: no inter/wall
+            ref_e = e[2] if ref_e is None else ref_e
+            assert e[2] == pytest.approx(ref_e, rel=1e-12, abs=1e-12)    # invariant under (t, q)
+            assert ga.sum(axis=0) == pytest.approx(0.0, abs=1e-10)       # sum of internal forces = 0
+            assert np.cross(x, ga).sum(axis=0) == pytest.approx(0.0, abs=1e-9)   # and of internal torques
+            assert g[:6] == pytest.approx(0.0, abs=1e-9)                 # so no rigid-body gradient
+        assert ref_e != 0.0
+
+
+def test_inter_energy_is_sum_of_per_atom_interpolations(orc, dock_system):
+    S = dock_system
+    L = S["L"][1]
+    pose = np.concatenate([[7.4, 7.7, 7.2], [0.3, -0.5, 0.2, 0.8], [0.5, -1.0, 2.0, 0.1]])
+    e, g, x, ga = orc.score_grad(S["p"], S["ty"], S["G"], L, pose)
+    tot = sum(orc.interp(S["p"], S["G"], int(L.type[a]), x[a])[0] for a in range(L.n))
+    assert e[1] == pytest.approx(tot, rel=1e-13)
+    assert e[0] == pytest.approx(e[1] + e[2], rel=1e-14)
+
+
+def _quat_left_mul_rotvec(q_wxyz, v):
+    r = Rotation.from_rotvec(v) * Rotation.from_quat([q_wxyz[1], q_wxyz[2], q_wxyz[3], q_wxyz[0]])
+    x, y, z, w = r.as_quat()
+    return np.array([w, x, y, z])
+
+
+def _safe_pose(orc, S, L, rng):
+    """A pose with no atom within 1e-3 (grid units) of a cell face and no pair within 1e-3 of an indicator edge."""
+    G = S["G"]
+    for _ in range(200):
+        pose = np.concatenate([7.5 + rng.uniform(-2.5, 2.5, 3), rng.normal(size=4), rng.uniform(-np.pi, np.pi, L.T)])
+        pose[3:7] /= np.linalg.norm(pose[3:7])
+        x = orc.fk(L, pose)
+        u = (x - G.origin) / G.spacing
+        if np.any(u < 0.01) or np.any(u > 39.99) or np.min(np.abs(u - np.rint(u))) < 1e-3:
+            continue
+        ok = True
+        for a, b in L.pairs.astype(int):
+            d = np.linalg.norm(x[a] - x[b])
+            r = S["ty"].radius[L.type[a]] + S["ty"].radius[L.type[b]]
+            if min(abs(d - e) for e in (10.0, 3.4, 2.6, r, 0.05)) < 1e-3:
+                ok = False
+        if ok:
+            return pose
+    raise RuntimeError("no safe pose")
+
+
+def test_gradient_matches_central_differences(orc, dock_system):
+    S = dock_system
+    rng = np.random.default_rng(23)
+    h = 1e-5
+    E = lambda L, pose: orc.score_grad(S["p"], S["ty"], S["G"], L, pose, want_grad=False)[0][0]
+    for L in S["L"]:
+        for _ in range(4):
+            pose = _safe_pose(orc, S, L, rng)
+            e, g, x, ga = orc.score_grad(S["p"], S["ty"], S["G"], L, pose)
+            assert g[:3] == pytest.approx(ga.sum(axis=0), rel=1e-12, abs=1e-12)      # translation row = sum of forces
+            scale = max(1.0, np.abs(g).max())
+            for c in range(3):
+                d = np.zeros_like(pose); d[c] = h
+                assert g[c] == pytest.approx((E(L, pose + d) - E(L, pose - d)) / (2 * h), abs=2e-5 * scale)
+            for c in range(3):                                                         # world-frame rotation about t
+                v = np.zeros(3); v[c] = h
+                pp, pm = pose.copy(), pose.copy()
+                pp[3:7] = _quat_left_mul_rotvec(pose[3:7], v)
+                pm[3:7] = _quat_left_mul_rotvec(pose[3:7], -v)
+                assert g[3 + c] == pytest.approx((E(L, pp) - E(L, pm)) / (2 * h), abs=2e-5 * scale)
+            for k in range(L.T):
+                d = np.zeros_like(pose); d[7 + k] = h
+                assert g[6 + k] == pytest.approx((E(L, pose + d) - E(L, pose - d)) / (2 * h), abs=2e-5 * scale)
+
+
+# --------------------------------------------------------------------------- O10 Philox, uniforms
+def test_philox_known_answers(orc):
+    n = 0
+    for line in open(os.path.join(GOLD, "philox4x32_10_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        w = [int(x, 16) for x in line.split()]
+        assert orc.philox4x32_10(w[0:4], w[4:6]) == w[6:10]
+        n += 1
+    assert n == 3
+
+
+def test_uniform_mapping(orc):
+    """u = ((r >> 9) + 0.5) 2^-23: strictly inside (0,1), exact in fp32, counter = (chain, step, ligand, purpose)."""
+    r = orc.philox4x32_10([5, 6, 7, 1], [0x89abcdef, 0x01234567])
+    u = orc.uniform4(0x0123456789abcdef, 5, 6, 7, 1)
+    for ri, ui in zip(r, u):
+        assert ui == ((ri >> 9) + 0.5) / 2 ** 23
+        assert 0.0 < ui < 1.0 and float(np.float32(ui)) == ui
+    us = np.concatenate([orc.uniform4(3, c, 0, 0, 0) for c in range(5000)])
+    assert abs(us.mean() - 0.5) < 0.01 and abs(us.var() - 1 / 12) < 0.005
+    assert not np.array_equal(orc.uniform4(3, 1, 0, 0, 0), orc.uniform4(3, 0, 1, 0, 0))
+
+
+# --------------------------------------------------------------------------- O11 init
+def test_init_pose_distribution(orc, dock_system):
+    L = dock_system["L"][2]
+    c, R = np.array([7.5, 7.5, 7.5]), 4.0
+    P = np.array([orc.init_pose(L, 0, ch, 3, c, R) for ch in range(4000)])
+    r = np.linalg.norm(P[:, :3] - c, axis=1)
+    assert r.max() <= R
+    assert abs(np.mean((r / R) ** 3) - 0.5) < 0.02                       # uniform in the ball
+    assert np.linalg.norm(P[:, 3:7], axis=1) == pytest.approx(1.0, abs=1e-12)
+    assert np.abs(P[:, 3:7].mean(axis=0)).max() < 0.03                   # uniform on S^3: zero mean ...
+    assert np.mean(P[:, 3:7] ** 2, axis=0) == pytest.approx(0.25, abs=0.01)  # ... and isotropic
+    assert np.all(P[:, 7:] >= -np.pi) and np.all(P[:, 7:] < np.pi)
+    assert np.abs(P[:, 7:].mean(axis=0)).max() < 0.12
+    assert np.array_equal(P[5], orc.init_pose(L, 0, 5, 3, c, R))         # counter-based: reproducible
+
+
+# --------------------------------------------------------------------------- O12 Adam + Metropolis
+def one_atom_system(orc):
+    """One atom outside a zero grid on +x: E = k_wall (x - x_max)^2, a 1-D quadratic in the translation."""
+    L = orc.Ligand(np.zeros((1, 3)), [0], [0], [], [], [], pairs=np.zeros((0, 2), np.uint8))
+    G = orc.Grid(np.zeros((1, 4, 4, 4), np.float32), (0, 0, 0), 1.0)     # x_max = 3
+    ty = orc.Types([1.7], [0])
+    return L, G, ty
+
+
+def test_adam_first_step_and_torch_reference(orc):
+    import torch
+    L, G, ty = one_atom_system(orc)
+    box = ([-100.0] * 3, [100.0] * 3)
+    x0 = 5.0
+    pose0 = [x0, 1.5, 1.5, 1, 0, 0, 0]
+    for n_refine in (1, 2, 5):
+        p = orc.default_params(pert_trans=0.0, pert_rot=0.0, n_refine=n_refine)
+        e0 = orc.score_grad(p, ty, G, L, pose0)[0][0]
+        assert e0 == pytest.approx(10.0 * (x0 - 3.0) ** 2, rel=1e-14)
+        pose, ec, rec = orc.mc_step(p, ty, G, L, 0, 0, 0, 0, *box, pose0, e0)
+        assert rec.accept == 1                                           # downhill: always accepted (G15)
+        xt = torch.tensor([x0], dtype=torch.float64, requires_grad=True)
+        opt = torch.optim.Adam([xt], lr=0.1)                             # PyTorch defaults = G12
+        for _ in range(n_refine):
+            opt.zero_grad()
+            (10.0 * (xt - 3.0) ** 2).sum().backward()
+            opt.step()
+        assert pose[0] == pytest.approx(float(xt.detach()[0]), rel=1e-12)
+        assert pose[1:3] == pytest.approx([1.5, 1.5], abs=0)             # zero gradient -> zero Adam step
+        assert ec == pytest.approx(10.0 * (pose[0] - 3.0) ** 2, rel=1e-13)
+        if n_refine == 1:                                                # hand value: -lr g / (|g| + eps)
+            g = 2 * 10.0 * (x0 - 3.0)
+            assert pose[0] == pytest.approx(x0 - 0.1 * g / (abs(g) + 1e-8), rel=1e-15)
+
+
+def test_metropolis_acceptance_probability(orc):
+    """P(accept | dE = +10) = exp(-0.69) = 0.5016; dE <= 0 always accepts; large beta never goes uphill."""
+    L, G, ty = one_atom_system(orc)
+    box = ([-100.0] * 3, [100.0] * 3)
+    pose0 = [5.0, 1.5, 1.5, 1, 0, 0, 0]
+    p = orc.default_params(pert_trans=0.0, pert_rot=0.0, lr=0.0)         # proposal == current pose
+    e_here = orc.score_grad(p, ty, G, L, pose0)[0][0]
+    n, acc = 20000, 0
+    for i in range(n):
+        _, _, rec = orc.mc_step(p, ty, G, L, 1, i % 100, i // 100, 2, *box, pose0, e_here - 10.0)
+        assert rec.e_prop - rec.e_cur == pytest.approx(10.0, rel=1e-12)
+        assert rec.accept == int(rec.u < math.exp(-0.69))
+        acc += rec.accept
+    assert abs(acc / n - 0.5016) < 4 * math.sqrt(0.25 / n)
+    for i in range(200):
+        _, _, rec = orc.mc_step(p, ty, G, L, 1, i, 0, 0, *box, pose0, e_here)          # dE = 0
+        assert rec.accept == 1
+        _, _, rec = orc.mc_step(p, ty, G, L, 1, i, 0, 0, *box, pose0, e_here + 3.0)    # dE < 0
+        assert rec.accept == 1
+    pb = orc.default_params(pert_trans=0.0, pert_rot=0.0, lr=0.0, beta=1e3)
+    for i in range(200):
+        _, _, rec = orc.mc_step(pb, ty, G, L, 1, i, 0, 0, *box, pose0, e_here - 1.0)
+        assert rec.accept == 0
+
+
+def test_perturbation_entities_and_ranges(orc, dock_system):
+    """G11: entity uniform over {translation, rotation, each torsion}; translation stays in the box."""
+    S = dock_system
+    L = S["L"][1]                                                        # T = 4 -> 6 entities
+    p = orc.default_params(lr=0.0)                                       # isolate the perturbation
+    rec_ = S["rec"]
+    pose0 = np.concatenate([rec_.pocket_center, [1, 0, 0, 0], [0.1, 0.2, 0.3, 0.4]])
+    counts = np.zeros(L.T + 2, int)
+    for i in range(3000):
+        pose, ec, rec = orc.mc_step(p, S["ty"], S["G"], L, 9, i, 0, 0, rec_.box_min, rec_.box_max, pose0, 1e9)
+        assert rec.accept == 1                                           # e_cur huge -> always accepted
+        counts[rec.entity] += 1
+        changed_t = not np.array_equal(pose[:3], pose0[:3])
+        changed_q = not np.allclose(pose[3:7], pose0[3:7], atol=1e-15)
+        changed_th = [k for k in range(L.T) if abs(pose[7 + k] - pose0[7 + k]) > 1e-9]   # wrap() rounds in the last bit
+        assert (changed_t, changed_q, changed_th) == (rec.entity == 0, rec.entity == 1,
+                                                      [rec.entity - 2] if rec.entity >= 2 else [])
+        assert np.all(pose[:3] >= rec_.box_min) and np.all(pose[:3] <= rec_.box_max)
+        assert np.all(np.abs(pose[:3] - pose0[:3]) <= 2.0)
+        assert abs(np.linalg.norm(pose[3:7]) - 1) < 1e-12
+        if rec.entity == 1:
+            ang = 2 * math.acos(min(1.0, abs(pose[3])))
+            assert ang <= 0.5 * math.sqrt(3) + 1e-12
+    assert counts.min() > 3000 / 6 * 0.8
+
+
+# --------------------------------------------------------------------------- whole chain sanity, O13, E_screen
+def test_dock_sanity_and_topk(orc, dock_system):
+    S = dock_system
+    rec_, L = S["rec"], S["L"][0]
+    args = (S["p"], S["ty"], S["G"], L, 0, 0)
+    kw = dict(box_min=rec_.box_min, box_max=rec_.box_max, centre=rec_.pocket_center, radius=rec_.pocket_radius)
+    r0 = orc.dock(*args, 16, 0, **kw)
+    r20 = orc.dock(*args, 16, 20, **kw, want_trace=True)
+    r40 = orc.dock(*args, 16, 40, **kw)
+    assert np.all(r20["e_best"] <= r0["e_best"]) and np.all(r40["e_best"] <= r20["e_best"])   # best never rises
+    assert np.all(r20["e_best"] <= r20["e_cur"])
+    assert r20["e_best"].min() < r0["e_best"].min()
+    for c in range(16):                                                  # stored best pose scores to the stored energy
+        e = orc.score_grad(S["p"], S["ty"], S["G"], L, r20["pose_best"][c], want_grad=False)[0][0]
+        assert e == pytest.approx(r20["e_best"][c], rel=1e-12)
+    tr = r20["trace"]
+    assert np.array_equal(tr["accept"], (tr["u"] < np.exp(-0.069 * (tr["e_prop"] - tr["e_cur"]))).astype(int))
+    # resumability: 20 + 20 steps (first_step = 20, from the saved state) == 40 steps
+    r2 = orc.dock(*args, 16, 20, **kw, init_poses=r20["pose_cur"], first_step=20)
+    assert np.minimum(r2["e_best"], r20["e_best"]) == pytest.approx(r40["e_best"], rel=1e-12)
+    # O13 vs brute force
+    e = np.array([3.0, -1.0, 2.0, -1.0, 5.0, -7.0])
+    assert list(orc.topk(e, 4)) == [5, 1, 3, 2]                          # ties -> lower chain id
+    assert list(orc.topk(r20["e_best"], 3)) == sorted(range(16), key=lambda c: (r20["e_best"][c], c))[:3]
+    # Eq.E_screen
+    assert orc.e_screen(-50.0, 6) == pytest.approx(-50.0 / 1.06)
+    assert orc.e_screen(-50.0, 0) == -50.0

@@ -1,0 +1,286 @@
+"""Seeded synthetic inputs shaped like the paper's workloads (harness, not product).
+
+This module holds NONE of the method's arithmetic: no scoring, kinematics, pair lists,
+RNG-for-the-chains.  It only builds the INPUT arrays that the fp64 oracle (``oracle/``)
+and the CUDA library (``paper_2510_24186_b200``) both consume, so that the two never
+have to share code.  Recipe: SURVEY.md section 8(d) / DESIGN.md section 4; configs C1..C5
+are BASELINE.json ``configs[0..4]``.
+
+The paper's own inputs (PDBbind time-split complexes, DEKOIS 2.0 targets, PAPER.md
+lines 75-79, 270, 297) are not available offline; these seeded receptors/ligands
+stand in for them with the same shapes (pocket-sized receptor, drug-like ligands,
+AutoDock-style 0.375 A grid).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass, field
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "_ligand_gen.so")
+_SRC = os.path.join(_HERE, "ligand_gen.c")
+
+
+def build(force: bool = False) -> str:
+    """Compile the ligand generator (plain C, gcc)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.check_call(
+            ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _SO, _SRC, "-lm"])
+    return _SO
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        _lib.ligand_gen_batch.restype = ctypes.c_int
+    return _lib
+
+
+# ----------------------------------------------------------------------------- types
+def type_table(n_types: int):
+    """Synthetic atom-type table (the paper takes vdW radii and H-bond
+    roles from OpenBabel and never lists them).
+
+    radius[t] = 1.5 + 0.1*(t mod 8) + 0.05*(t div 8)  [A];
+    hb_role[t mod 8] = {0,0,1,2,0,0,3,0}  (bit0 donor, bit1 acceptor)."""
+    t = np.arange(n_types)
+    radius = (1.5 + 0.1 * (t % 8) + 0.05 * (t // 8)).astype(np.float32)
+    role = np.array([0, 0, 1, 2, 0, 0, 3, 0], dtype=np.uint8)[t % 8]
+    return radius, role
+
+
+# -------------------------------------------------------------------------- receptor
+@dataclass
+class Receptor:
+    xyz: np.ndarray          # [n_rec,3] float32
+    type: np.ndarray         # [n_rec] int32
+    n_types: int
+    box_len: float
+    origin: np.ndarray       # [3] float32, grid origin (cube corner)
+    dims: tuple              # (nx, ny, nz)
+    spacing: float
+    pocket_center: np.ndarray
+    pocket_radius: float
+    box_min: np.ndarray
+    box_max: np.ndarray
+    min_sep: float
+
+
+def receptor(n_rec: int, box_len: float, n_types: int, seed: int, grid_n: int,
+             pocket_radius: float = 8.0, spacing: float = 0.375) -> Receptor:
+    """Random sequential addition of n_rec points uniform in [0,L]^3 outside the central
+    pocket sphere, min separation s = min(3 A, 0.8*(V_free/n_rec)^(1/3)) (BASELINE.json's
+    literal 3 A jams before n_rec atoms are placed -- SURVEY 8(d))."""
+    rng = np.random.default_rng(seed)
+    centre = np.full(3, box_len / 2.0)
+    v_free = box_len ** 3 - 4.0 / 3.0 * np.pi * pocket_radius ** 3
+    s = min(3.0, 0.8 * (v_free / n_rec) ** (1.0 / 3.0))
+    ncell = max(1, int(box_len / s))
+    cell = box_len / ncell
+    cells: dict = {}
+    pts = np.empty((n_rec, 3))
+    n = 0
+    trials = 0
+    while n < n_rec:
+        batch = rng.uniform(0.0, box_len, size=(4096, 3))
+        for p in batch:
+            trials += 1
+            if np.sum((p - centre) ** 2) < pocket_radius ** 2:
+                continue
+            ci = tuple(np.minimum((p / cell).astype(int), ncell - 1))
+            ok = True
+            for dx in (-1, 0, 1):
+                for dy in (-1, 0, 1):
+                    for dz in (-1, 0, 1):
+                        for j in cells.get((ci[0] + dx, ci[1] + dy, ci[2] + dz), ()):
+                            if np.sum((pts[j] - p) ** 2) < s * s:
+                                ok = False
+                                break
+                        if not ok:
+                            break
+                    if not ok:
+                        break
+                if not ok:
+                    break
+            if not ok:
+                continue
+            pts[n] = p
+            cells.setdefault(ci, []).append(n)
+            n += 1
+            if n == n_rec:
+                break
+        if trials > 4_000_000:
+            raise RuntimeError("receptor RSA did not converge")
+    types = rng.integers(0, n_types, size=n_rec).astype(np.int32)
+    return Receptor(
+        xyz=pts.astype(np.float32), type=types, n_types=n_types, box_len=box_len,
+        origin=np.zeros(3, np.float32), dims=(grid_n, grid_n, grid_n), spacing=spacing,
+        pocket_center=centre.astype(np.float32), pocket_radius=pocket_radius,
+        box_min=(centre - pocket_radius).astype(np.float32),
+        box_max=(centre + pocket_radius).astype(np.float32), min_sep=s)
+
+
+# --------------------------------------------------------------------------- ligands
+@dataclass
+class LigandBatch:
+    """CSR-packed ligand batch, exactly the arrays of ``tridsk_ligand_batch`` (include/tridsk.h)."""
+    n_lig: int
+    atom_off: np.ndarray     # [n_lig+1] int32
+    ref_xyz: np.ndarray      # [sum n,3] float32, centred on the centroid
+    atom_type: np.ndarray    # [sum n] uint8
+    atom_frag: np.ndarray    # [sum n] uint8   0 = root fragment, k+1 = child fragment of torsion k
+    tor_off: np.ndarray      # [n_lig+1] int32
+    tor_a: np.ndarray        # [sum T] uint8   axis a->b, a on the root side
+    tor_b: np.ndarray        # [sum T] uint8
+    tor_parent: np.ndarray   # [sum T] int8    -1 = root; parents precede children
+    bond_off: np.ndarray     # [n_lig+1] int32
+    bond_ab: np.ndarray      # [sum nb,2] uint8
+
+    def n_atoms(self, i):
+        return int(self.atom_off[i + 1] - self.atom_off[i])
+
+    def n_tor(self, i):
+        return int(self.tor_off[i + 1] - self.tor_off[i])
+
+    def one(self, i) -> dict:
+        """Arrays of ligand i (views)."""
+        a0, a1 = self.atom_off[i], self.atom_off[i + 1]
+        t0, t1 = self.tor_off[i], self.tor_off[i + 1]
+        b0, b1 = self.bond_off[i], self.bond_off[i + 1]
+        return dict(ref_xyz=self.ref_xyz[a0:a1], atom_type=self.atom_type[a0:a1],
+                    atom_frag=self.atom_frag[a0:a1], tor_a=self.tor_a[t0:t1],
+                    tor_b=self.tor_b[t0:t1], tor_parent=self.tor_parent[t0:t1],
+                    bond_ab=self.bond_ab[b0:b1])
+
+    def subset(self, idx) -> "LigandBatch":
+        idx = list(idx)
+        parts = [self.one(i) for i in idx]
+        cat = lambda k, dt, shp: (np.concatenate([p[k] for p in parts]).astype(dt)
+                                  if parts else np.zeros(shp, dt))
+        off = lambda k: np.concatenate([[0], np.cumsum([len(p[k]) for p in parts])]).astype(np.int32)
+        return LigandBatch(
+            n_lig=len(idx), atom_off=off("atom_type"), ref_xyz=cat("ref_xyz", np.float32, (0, 3)),
+            atom_type=cat("atom_type", np.uint8, (0,)), atom_frag=cat("atom_frag", np.uint8, (0,)),
+            tor_off=off("tor_a"), tor_a=cat("tor_a", np.uint8, (0,)), tor_b=cat("tor_b", np.uint8, (0,)),
+            tor_parent=cat("tor_parent", np.int8, (0,)), bond_off=off("bond_ab"),
+            bond_ab=cat("bond_ab", np.uint8, (0, 2)))
+
+
+def ligands(n_atoms, n_tor_req, n_types: int, seed: int, backbone: int = 0) -> LigandBatch:
+    """Grow len(n_atoms) tree ligands (see ligand_gen.c for the recipe)."""
+    lib = _load()
+    n = np.ascontiguousarray(n_atoms, dtype=np.int32)
+    tr = np.ascontiguousarray(n_tor_req, dtype=np.int32)
+    L = len(n)
+    atom_off = np.concatenate([[0], np.cumsum(n)]).astype(np.int32)
+    cap_off = np.concatenate([[0], np.cumsum(tr)]).astype(np.int32)
+    tot, cap = int(atom_off[-1]), int(cap_off[-1])
+    xyz = np.zeros((tot, 3), np.float32)
+    typ = np.zeros(tot, np.uint8)
+    frag = np.zeros(tot, np.uint8)
+    bonds = np.zeros((max(tot - L, 0), 2), np.uint8)
+    ta = np.zeros(max(cap, 1), np.uint8)
+    tb = np.zeros(max(cap, 1), np.uint8)
+    tp = np.zeros(max(cap, 1), np.int8)
+    t_out = np.zeros(L, np.int32)
+    P = lambda a: a.ctypes.data_as(ctypes.c_void_p)
+    rc = lib.ligand_gen_batch(ctypes.c_uint64(seed), ctypes.c_int(L), P(n), P(tr), ctypes.c_int(n_types),
+                              ctypes.c_int(backbone), P(atom_off), P(cap_off), P(xyz), P(typ), P(bonds),
+                              P(frag), P(ta), P(tb), P(tp), P(t_out))
+    if rc != 0:
+        raise RuntimeError("ligand generator failed")
+    # compact the torsion arrays from capacity offsets to actual counts
+    tor_off = np.concatenate([[0], np.cumsum(t_out)]).astype(np.int32)
+    sel = np.zeros(max(cap, 1), bool)
+    for_idx = np.repeat(cap_off[:-1], t_out) + (np.arange(int(tor_off[-1])) - np.repeat(tor_off[:-1], t_out))
+    sel[for_idx] = True
+    bond_off = (atom_off - np.arange(L + 1)).astype(np.int32)
+    return LigandBatch(n_lig=L, atom_off=atom_off, ref_xyz=xyz, atom_type=typ, atom_frag=frag,
+                       tor_off=tor_off, tor_a=ta[sel].copy(), tor_b=tb[sel].copy(), tor_parent=tp[sel].copy(),
+                       bond_off=bond_off, bond_ab=bonds)
+
+
+# --------------------------------------------------------------------------- configs
+@dataclass
+class Config:
+    name: str
+    title: str
+    n_rec: int
+    box_len: float
+    grid_n: int
+    n_types: int
+    n_lig: int
+    n_chains: int
+    n_steps: int
+    top_k: int
+    rec_seed: int
+    lig_seed: int
+    philox_seed: int = 0
+    backbone: int = 0
+    sizes: dict = field(default_factory=dict)
+
+
+CONFIGS = {
+    "C1": Config("C1", "Tiny", 300, 20.0, 54, 8, 1, 64, 100, 1, 1001, 2001),
+    "C2": Config("C2", "Drug-like single dock", 3000, 30.0, 80, 16, 1, 384, 1000, 10, 1002, 2002),
+    "C3": Config("C3", "Screening batch", 3000, 30.0, 80, 16, 4096, 128, 500, 1, 1003, 2003),
+    "C4": Config("C4", "Large flexible ligand", 3000, 40.0, 107, 16, 1, 1024, 2000, 1, 1004, 2004, backbone=24),
+    "C5": Config("C5", "High-throughput screen", 5000, 30.0, 80, 16, 65536, 64, 300, 1, 1005, 2005),
+}
+
+
+def config_sizes(cfg: Config, n_lig: int | None = None):
+    """Per-ligand (n_atoms, n_tor_requested) arrays for a config (BASELINE.json configs)."""
+    L = cfg.n_lig if n_lig is None else n_lig
+    rng = np.random.default_rng(cfg.lig_seed)
+    if cfg.name == "C1":
+        return np.full(L, 12), np.full(L, 2)
+    if cfg.name == "C2":
+        return np.full(L, 30), np.full(L, 6)
+    if cfg.name == "C3":
+        n = rng.integers(15, 51, size=cfg.n_lig)
+        t = np.array([rng.integers(0, min(12, k // 4) + 1) for k in n])
+        return n[:L], t[:L]
+    if cfg.name == "C4":
+        return np.full(L, 80), np.full(L, 20)
+    if cfg.name == "C5":
+        n = np.clip(np.rint(rng.normal(28.0, 8.0, size=cfg.n_lig)), 10, 70).astype(int)
+        t = np.minimum(rng.poisson(5.0, size=cfg.n_lig), 15)
+        return n[:L], t[:L]
+    raise KeyError(cfg.name)
+
+
+def make_receptor(cfg: Config) -> Receptor:
+    return receptor(cfg.n_rec, cfg.box_len, cfg.n_types, cfg.rec_seed, cfg.grid_n)
+
+
+def make_ligands(cfg: Config, n_lig: int | None = None) -> LigandBatch:
+    """First n_lig ligands of the config (ligand i is the same whatever n_lig is)."""
+    n, t = config_sizes(cfg, n_lig)
+    return ligands(n, t, cfg.n_types, cfg.lig_seed, backbone=cfg.backbone)
+
+
+def random_poses(batch: LigandBatch, lig_index, rec: Receptor, seed: int, spread: float = 1.0):
+    """Random test poses [n_pose, 7+Tmax] float32: translation uniform in the search box
+    (scaled by `spread` about the pocket centre), uniform unit quaternion, torsions uniform."""
+    rng = np.random.default_rng(seed)
+    lig_index = np.asarray(lig_index, dtype=np.int32)
+    tmax = int(np.max(np.diff(batch.tor_off))) if batch.n_lig else 0
+    n = len(lig_index)
+    poses = np.zeros((n, 7 + tmax), np.float32)
+    half = (rec.box_max - rec.box_min) / 2 * spread
+    poses[:, 0:3] = rec.pocket_center + rng.uniform(-1, 1, size=(n, 3)) * half
+    q = rng.normal(size=(n, 4))
+    poses[:, 3:7] = q / np.linalg.norm(q, axis=1, keepdims=True)
+    poses[:, 7:] = rng.uniform(-np.pi, np.pi, size=(n, tmax))
+    for i, li in enumerate(lig_index):
+        poses[i, 7 + batch.n_tor(li):] = 0.0
+    return poses
