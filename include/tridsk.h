@@ -1,0 +1,188 @@
+/*
+ * tridsk.h -- C-ABI of libtridsk: batched gradient-guided Monte Carlo conformation sampling
+ * (the hot path of TRIDS, arxiv 2510.24186) as hand-written CUDA for sm_100a, one GPU.
+ *
+ * Citations: P:N = /root/reference/PAPER.md line N.  O1..O13 / G1..G19 = DESIGN.md section 3
+ * (the readings taken where the paper is silent or garbled).  The problem the four main calls
+ * solve is the paper's statement of docking: given a receptor pocket, one or many
+ * ligands with rotatable bonds and a search box, sample pose degrees of freedom (translation,
+ * rotation, torsions) by Metropolis Monte Carlo with gradient refinement (P:143-148,
+ * Fig. 2) under the score E_dock, and return the top-N lowest-score poses.
+ *
+ * Conventions
+ *   - Every function returns TRIDSK_OK (0) or a negative error code and never aborts;
+ *     tridsk_last_error(ctx) gives the text (valid until the next call on that ctx).
+ *   - Pointers marked [host] must be host memory; [host|dev] may be either and are detected with
+ *     cudaPointerGetAttributes.  The caller owns every input buffer (copied or consumed before the
+ *     call returns) and every output buffer; the library owns what the opaque handles point to
+ *     until the matching free.
+ *   - All GPU work is enqueued on the stream given to tridsk_create.  Calls that write HOST
+ *     outputs synchronise that stream before returning; calls that write only DEVICE outputs do not.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with TRIDSK_ECUDA.
+ *   - Pose layout   [tx,ty,tz, qw,qx,qy,qz, theta_0..theta_{T-1}]  (Hamilton, active rotation,
+ *     torsion k right-handed about tor_a[k] -> tor_b[k]; theta = 0, q = 1, t = 0 is ref_xyz; O8/G10).
+ *     Input quaternions are renormalised; a zero quaternion gives NaN energies.
+ *   - Gradient layout [dE/dt (3), dE/domega (3, world-frame rotation vector about t), dE/dtheta (T)] (O9).
+ *   - Limits: n_atoms <= 128, n_torsions <= 31, n_types <= 32 per ligand (TRIDSK_ELIMIT otherwise).
+ */
+#ifndef TRIDSK_H
+#define TRIDSK_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TRIDSK_OK      0
+#define TRIDSK_EINVAL (-1)   /* bad argument or inconsistent ligand topology */
+#define TRIDSK_ENOMEM (-2)
+#define TRIDSK_ECUDA  (-3)   /* CUDA error; text in tridsk_last_error */
+#define TRIDSK_ELIMIT (-4)   /* a size limit above is exceeded */
+
+#define TRIDSK_MAX_ATOMS    128
+#define TRIDSK_MAX_TORSIONS 31
+#define TRIDSK_MAX_TYPES    32
+
+typedef struct tridsk_ctx tridsk_ctx;         /* owns CUDA resources on one device */
+typedef struct tridsk_grid tridsk_grid;       /* owns the fp32 [n_types][nz][ny][nx] device grid */
+typedef struct tridsk_ligands tridsk_ligands; /* owns the packed ligand batch on the device */
+
+/* Every constant of the method; tridsk_default_params fills the paper's values. */
+typedef struct {
+    float w_long, w_clash, w_hbond;             /* 0.2, 10.0, 0.6    Eq.E_dock weights            */
+    float long_mu, long_two_sigma2, long_dmax;  /* 3.0, 4.0, 10.0    Eq.E_long; G2            */
+    float hb_mu, hb_sigma, hb_dmax, hb_dclash;  /* 2.88, 0.3, 3.4, 2.6   Eq.E_Hbond, Eq.E_clash */
+    float d_floor, k_wall;                      /* 0.05 A, 10.0 /A^2  G4, G8                             */
+    float beta, lr, adam_b1, adam_b2, adam_eps; /* 0.069, 0.1, 0.9, 0.999, 1e-8   P:148, G12      */
+    float pert_trans, pert_rot;                 /* 2.0 A, 0.5 rad     G11                                 */
+    float w_tor;                                /* 0.01               Eq.E_screen                  */
+    int   n_refine;                             /* 1                  Adam steps per MC step, G12         */
+} tridsk_params;
+
+/* Atom-type table (O1): per type a vdW radius [A] and an H-bond role (bit0 donor, bit1 acceptor). [host] */
+typedef struct {
+    int n_types;
+    const float* radius;
+    const unsigned char* hb_role;
+} tridsk_types;
+
+/*
+ * CSR-packed ligand batch, all [host], copied during tridsk_load_ligands.
+ *   atom_off[n_lig+1]; ref_xyz[sum n][3] reference conformer (centred on its centroid, G10);
+ *   atom_type[sum n]; atom_frag[sum n]: 0 = root rigid fragment, k+1 = the fragment hanging off
+ *   torsion k (it moves with torsion k and all of k's ancestors);
+ *   tor_off[n_lig+1]; tor_a/tor_b[sum T]: rotation axis a -> b, a on the root side;
+ *   tor_parent[sum T]: parent torsion or -1; parents precede children.
+ *   Intra-ligand pairs (O6): give them as pair_off[n_lig+1] + pair_ab[sum P][2], or pass
+ *   pair_off = NULL and give the bond graph (bond_off[n_lig+1], bond_ab[sum nb][2]); the library
+ *   then derives pairs = {a<b : bond-graph distance >= 4 and atom_frag[a] != atom_frag[b]}.
+ *   Atom / torsion indices inside a ligand are local (0-based) bytes.
+ */
+typedef struct {
+    int n_lig;
+    const int* atom_off;
+    const float* ref_xyz;
+    const unsigned char* atom_type;
+    const unsigned char* atom_frag;
+    const int* tor_off;
+    const unsigned char* tor_a;
+    const unsigned char* tor_b;
+    const signed char* tor_parent;
+    const int* pair_off;
+    const unsigned char* pair_ab;
+    const int* bond_off;
+    const unsigned char* bond_ab;
+} tridsk_ligand_batch;
+
+/* One record of the optional per-step trace of tridsk_dock (parity tests). */
+typedef struct {
+    float e_prop;   /* energy of the refined proposal (E_new, O12)          */
+    float e_cur;    /* energy of the current accepted state before the step */
+    float u;        /* the Metropolis uniform                               */
+    int   flags;    /* bit0 = accepted; bits 8.. = perturbed entity (0 translation, 1 rotation, 2+k torsion k) */
+} tridsk_trace_rec;
+
+/* Optional controls of tridsk_dock; NULL = all zero = defaults. */
+typedef struct {
+    int first_step;            /* Philox step counter of the first MC step of this call (resume)            */
+    const float* init_poses;   /* [host|dev] NULL -> Philox initialisation (O11); else [n_lig][n_chains][pose_stride] */
+    int resume;                /* 1: start from chain_state (as written by an earlier call) instead of initialising   */
+    float* chain_state;        /* [host|dev] NULL, or n_lig*n_chains*(2*pose_stride+2) floats laid out as four arrays
+                                  {pose_cur[n_lig][n_chains][pose_stride], pose_best[same], E_cur[n_lig][n_chains],
+                                  E_best[same]}; read if resume, always written                                       */
+    tridsk_trace_rec* trace;   /* [host|dev] NULL, or [n_lig][n_chains][n_steps]                                      */
+    int steps_per_launch;      /* MC steps per kernel launch; 0 = all n_steps in one launch                           */
+    int no_graph;              /* 1: plain stream launches instead of a captured CUDA graph                           */
+} tridsk_dock_opts;
+
+/* ---- lifetime ------------------------------------------------------------------------------ */
+/* cuda_stream: a cudaStream_t (e.g. torch.cuda.Stream().cuda_stream); NULL -> the ctx creates and owns a
+ * non-blocking stream (the legacy default stream cannot be captured into a CUDA graph). */
+int  tridsk_create(tridsk_ctx** out, int device, void* cuda_stream);
+void tridsk_destroy(tridsk_ctx* ctx);
+const char* tridsk_last_error(const tridsk_ctx* ctx);
+void tridsk_default_params(tridsk_params* p);
+int  tridsk_synchronize(tridsk_ctx* ctx);
+
+/* ---- receptor grid (hot-path step a0; O3/O4) ------------------------------------------------- */
+/*
+ * G[t][k][j][i] = sum over receptor atoms a of e(s_a, t, |origin + spacing*(i,j,k) - r_a|), x fastest,
+ * where e = w_long*L + w_clash*C + w_Hbond*H are the paper's receptor-ligand pair terms
+ * (Eq.E_long, Eq.E_clash, Eq.E_Hbond; they depend on the ligand atom only through
+ * its type, which is what makes the tabulation valid -- G7).  rec_xyz[n_rec][3], rec_type[n_rec]: [host|dev].
+ * origin[3], dims[3] = (nx,ny,nz): [host].
+ */
+int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const int* rec_type, int n_rec,
+                      const tridsk_types* types, const tridsk_params* params,
+                      const float origin[3], const int dims[3], float spacing, tridsk_grid** out);
+/* Adopt a caller-built grid (e.g. the oracle's), copied from `values` [host|dev] [n_types][nz][ny][nx]. */
+int tridsk_grid_from_values(tridsk_ctx* ctx, const float* values, int n_types,
+                            const float origin[3], const int dims[3], float spacing, tridsk_grid** out);
+/* Copy the grid out, dst [host|dev] [n_types][nz][ny][nx]. */
+int tridsk_grid_export(tridsk_ctx* ctx, const tridsk_grid* grid, float* dst);
+void tridsk_free_grid(tridsk_grid* grid);
+
+/* ---- ligands ---------------------------------------------------------------------------------- */
+int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* batch, const tridsk_types* types,
+                        tridsk_ligands** out);
+/* n_pairs_out[n_lig] [host] (may be NULL): number of intra-ligand pairs per ligand (given or derived). */
+int tridsk_ligand_info(const tridsk_ligands* ligs, int* n_lig, int* max_atoms, int* max_torsions, int* n_pairs_out);
+void tridsk_free_ligands(tridsk_ligands* ligs);
+
+/* ---- score + analytic gradient of given poses (steps a3..a6; O5..O9) --------------------------- */
+/*
+ * For pose i of ligand lig_index[i]: forward kinematics, E = sum_a [trilinear G_type(a)(x_a) + wall] + E_intra,
+ * and the hand-derived gradient pushed back through the torsion tree (P:131, P:353 item 3).
+ * lig_index[n_pose], poses[n_pose][pose_stride]: [host|dev], pose_stride >= 7 + max T.
+ * energy[n_pose][3] = {total, receptor (inter), intra}; grad[n_pose][grad_stride] or NULL, grad_stride >= 6 + max T;
+ * coords[n_pose][coord_stride][3] or NULL, coord_stride >= max n, atoms in the caller's order: [host|dev].
+ */
+int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* ligs,
+                      const tridsk_params* params, const int* lig_index, const float* poses, int n_pose,
+                      int pose_stride, float* energy, float* grad, int grad_stride, float* coords, int coord_stride);
+
+/* ---- the docking run (steps a1..a10; O10..O13) ---------------------------------------------------- */
+/*
+ * For every ligand: n_chains independent chains x n_steps MC steps (perturb one entity -> n_refine
+ * Adam steps on the analytic gradient -> Metropolis with a Philox4x32-10 stream keyed by
+ * (seed; chain, step, ligand, purpose)), then the top_k lowest best-energies across chains
+ * (ties -> lower chain id).
+ * box_min/box_max/pocket_center: [host].  Outputs [host|dev]:
+ *   out_energy[n_lig][top_k][2] = {E_dock, E_screen = E_dock/(1 + w_tor*T)};
+ *   out_pose[n_lig][top_k][pose_stride]; out_chain[n_lig][top_k].  top_k <= n_chains.
+ */
+int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* ligs, const tridsk_params* params,
+                const float box_min[3], const float box_max[3], const float pocket_center[3], float pocket_radius,
+                int n_chains, int n_steps, int top_k, unsigned long long seed, int pose_stride,
+                float* out_energy, float* out_pose, int* out_chain, const tridsk_dock_opts* opts);
+
+/* Kernel launches enqueued by this ctx since creation (bench.py's gpu_launches). */
+long long tridsk_launch_count(const tridsk_ctx* ctx);
+
+/* Philox4x32-10 block for the given counter/key, computed ON THE DEVICE by the same routine the chains use
+ * (test hook for O10).  ctr[4], key[2], out[4]: [host]. */
+int tridsk_debug_philox(tridsk_ctx* ctx, const unsigned int ctr[4], const unsigned int key[2], unsigned int out[4]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TRIDSK_H */

@@ -20,8 +20,13 @@ _SO = os.path.join(_HERE, "_tridsk_oracle.so")
 
 def build(force: bool = False) -> str:
     """gcc -O2, no -ffast-math."""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+    import hashlib
+    want = hashlib.sha256(open(_SRC, "rb").read()).hexdigest()
+    stamp = _SO + ".stamp"
+    if force or not os.path.exists(_SO) or not os.path.exists(stamp) or open(stamp).read() != want:
         subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _SO, _SRC, "-lm"])
+        with open(stamp, "w") as f:
+            f.write(want)
     return _SO
 
 

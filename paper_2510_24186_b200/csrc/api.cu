@@ -1,0 +1,653 @@
+// api.cu -- the C-ABI of libtridsk (include/tridsk.h): handles, host-side ligand packing, staging of
+// host buffers, and the CUDA-graph-captured launch series of tridsk_dock (hot-path step a10).
+// No arithmetic of the method runs on the host: every step of the path is in the kernels.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "internal.h"
+
+// ---------------------------------------------------------------------------------------- helpers
+static int fail(tridsk_ctx* ctx, int code, const std::string& msg) {
+    if (ctx) ctx->err = msg;
+    return code;
+}
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA,       \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                       \
+    } while (0)
+
+static bool is_device_ptr(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+static int scratch(tridsk_ctx* ctx, int slot, size_t bytes, void** out) {
+    if (bytes > ctx->scratch_bytes[slot]) {
+        if (ctx->scratch[slot]) { CK(cudaStreamSynchronize(ctx->stream)); CK(cudaFree(ctx->scratch[slot])); }
+        ctx->scratch[slot] = nullptr; ctx->scratch_bytes[slot] = 0;
+        size_t cap = bytes + bytes / 4 + 256;
+        CK(cudaMalloc(&ctx->scratch[slot], cap));
+        ctx->scratch_bytes[slot] = cap;
+    }
+    *out = ctx->scratch[slot];
+    return TRIDSK_OK;
+}
+
+// device view of an input buffer: the pointer itself if it is device memory, else a staged copy
+static int stage_in(tridsk_ctx* ctx, int slot, const void* p, size_t bytes, const void** out) {
+    if (is_device_ptr(p)) { *out = p; return TRIDSK_OK; }
+    void* d;
+    int rc = scratch(ctx, slot, bytes, &d);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(d, p, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    *out = d;
+    return TRIDSK_OK;
+}
+
+static void to_dparams(const tridsk_params* p, DParams* d) {
+    d->w_long = p->w_long; d->w_clash = p->w_clash; d->w_hbond = p->w_hbond;
+    d->long_mu = p->long_mu; d->long_inv_two_sigma2 = 1.0f / p->long_two_sigma2; d->long_dmax = p->long_dmax;
+    d->hb_mu = p->hb_mu; d->hb_inv_two_sigma2 = 1.0f / (2.0f * p->hb_sigma * p->hb_sigma);
+    d->hb_dmax = p->hb_dmax; d->hb_dclash = p->hb_dclash;
+    d->d_floor = p->d_floor; d->k_wall = p->k_wall;
+    d->beta = p->beta; d->lr = p->lr; d->adam_b1 = p->adam_b1; d->adam_b2 = p->adam_b2; d->adam_eps = p->adam_eps;
+    d->pert_trans = p->pert_trans; d->pert_rot = p->pert_rot; d->w_tor = p->w_tor;
+    d->n_refine = p->n_refine;
+}
+
+// ---------------------------------------------------------------------------------------- lifetime
+extern "C" void tridsk_default_params(tridsk_params* p) {
+    p->w_long = 0.2f; p->w_clash = 10.0f; p->w_hbond = 0.6f;
+    p->long_mu = 3.0f; p->long_two_sigma2 = 4.0f; p->long_dmax = 10.0f; /* P:113, G2 */
+    p->hb_mu = 2.88f; p->hb_sigma = 0.3f; p->hb_dmax = 3.4f; p->hb_dclash = 2.6f;
+    p->d_floor = 0.05f; p->k_wall = 10.0f;                              /* G4, G8 */
+    p->beta = 0.069f; p->lr = 0.1f; p->adam_b1 = 0.9f; p->adam_b2 = 0.999f; p->adam_eps = 1e-8f;
+    p->pert_trans = 2.0f; p->pert_rot = 0.5f;                           /* G11 */
+    p->w_tor = 0.01f;
+    p->n_refine = 1;
+}
+
+extern "C" int tridsk_create(tridsk_ctx** out, int device, void* cuda_stream) {
+    if (!out) return TRIDSK_EINVAL;
+    *out = nullptr;
+    tridsk_ctx* ctx = new (std::nothrow) tridsk_ctx();
+    if (!ctx) return TRIDSK_ENOMEM;
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaSetDevice(device);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) {           // no CPU fallback: fail loudly
+        fprintf(stderr, "tridsk_create: %s\n", cudaGetErrorString(e));
+        delete ctx;
+        return TRIDSK_ECUDA;
+    }
+    ctx->sm_count = prop.multiProcessorCount;
+    if (!ctx->stream) {               // the legacy default stream cannot be captured into a graph: own one
+        e = cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) { fprintf(stderr, "tridsk_create: %s\n", cudaGetErrorString(e)); delete ctx; return TRIDSK_ECUDA; }
+        ctx->own_stream = true;
+    }
+    *out = ctx;
+    return TRIDSK_OK;
+}
+
+extern "C" void tridsk_destroy(tridsk_ctx* ctx) {
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
+    for (int i = 0; i < 8; ++i) if (ctx->scratch[i]) cudaFree(ctx->scratch[i]);
+    if (ctx->own_stream) cudaStreamDestroy(ctx->stream);
+    delete ctx;
+}
+
+extern "C" const char* tridsk_last_error(const tridsk_ctx* ctx) { return ctx ? ctx->err.c_str() : "null ctx"; }
+extern "C" long long tridsk_launch_count(const tridsk_ctx* ctx) { return ctx ? ctx->launches : 0; }
+extern "C" int tridsk_synchronize(tridsk_ctx* ctx) {
+    if (!ctx) return TRIDSK_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    return TRIDSK_OK;
+}
+
+// ---------------------------------------------------------------------------------------- grid
+static int check_types(tridsk_ctx* ctx, const tridsk_types* t) {
+    if (!t || !t->radius || !t->hb_role || t->n_types < 1) return fail(ctx, TRIDSK_EINVAL, "bad type table");
+    if (t->n_types > TRIDSK_MAX_TYPES) return fail(ctx, TRIDSK_ELIMIT, "n_types > 32");
+    return TRIDSK_OK;
+}
+
+static int new_grid(tridsk_ctx* ctx, int n_types, const float origin[3], const int dims[3], float spacing, tridsk_grid** out) {
+    if (!origin || !dims || dims[0] < 2 || dims[1] < 2 || dims[2] < 2 || !(spacing > 0.f) || n_types < 1)
+        return fail(ctx, TRIDSK_EINVAL, "bad grid geometry");
+    if (n_types > TRIDSK_MAX_TYPES) return fail(ctx, TRIDSK_ELIMIT, "n_types > 32");
+    tridsk_grid* g = new (std::nothrow) tridsk_grid();
+    if (!g) return fail(ctx, TRIDSK_ENOMEM, "host alloc");
+    g->ctx = ctx;
+    g->d.nx = dims[0]; g->d.ny = dims[1]; g->d.nz = dims[2]; g->d.n_types = n_types;
+    g->d.plane = (size_t)dims[0] * dims[1] * dims[2];
+    g->d.ox = origin[0]; g->d.oy = origin[1]; g->d.oz = origin[2];
+    g->d.h = spacing; g->d.inv_h = 1.0f / spacing;
+    cudaError_t e = cudaMalloc(&g->g, sizeof(float) * g->d.plane * n_types);
+    if (e != cudaSuccess) { delete g; return fail(ctx, TRIDSK_ENOMEM, std::string("grid alloc: ") + cudaGetErrorString(e)); }
+    g->d.g = g->g;
+    *out = g;
+    return TRIDSK_OK;
+}
+
+extern "C" int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const int* rec_type, int n_rec,
+                                 const tridsk_types* types, const tridsk_params* params,
+                                 const float origin[3], const int dims[3], float spacing, tridsk_grid** out) {
+    if (!ctx || !out || !params || !rec_xyz || !rec_type || n_rec < 0) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    *out = nullptr;
+    int rc = check_types(ctx, types);
+    if (rc) return rc;
+    const int nt = types->n_types;
+    // receptor atoms -> float4 {x, y, z, type bits}: layout only (staged on the host; n_rec is a few thousand)
+    std::vector<float> xyz(3 * (size_t)n_rec);
+    std::vector<int> typ(n_rec);
+    if (n_rec) {
+        CK(cudaMemcpyAsync(xyz.data(), rec_xyz, sizeof(float) * 3 * n_rec, cudaMemcpyDefault, ctx->stream));
+        CK(cudaMemcpyAsync(typ.data(), rec_type, sizeof(int) * n_rec, cudaMemcpyDefault, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+    }
+    std::vector<float4> rec(n_rec);
+    for (int a = 0; a < n_rec; ++a) {
+        if (typ[a] < 0 || typ[a] >= nt) return fail(ctx, TRIDSK_EINVAL, "receptor atom type out of range");
+        float tbits;
+        memcpy(&tbits, &typ[a], sizeof(float));
+        rec[a] = make_float4(xyz[3 * a], xyz[3 * a + 1], xyz[3 * a + 2], tbits);
+    }
+    // type-pair table: operands of the pair function, not results
+    std::vector<float> tab(4 * (size_t)nt * nt);
+    float dc_max = params->hb_dmax;
+    for (int s = 0; s < nt; ++s)
+        for (int t = 0; t < nt; ++t) {
+            const unsigned char rs = types->hb_role[s], rt = types->hb_role[t];
+            const bool hb = ((rs & 1) && (rt & 2)) || ((rs & 2) && (rt & 1));
+            const float dvdw = types->radius[s] + types->radius[t];
+            const float dc = hb ? params->hb_dclash : dvdw;
+            float* e = &tab[4 * ((size_t)s * nt + t)];
+            e[0] = dvdw + params->long_mu; e[1] = dc; e[2] = hb ? 1.f : 0.f; e[3] = 1.0f / dc;
+            dc_max = std::max(dc_max, dc);
+        }
+    tridsk_grid* g = nullptr;
+    rc = new_grid(ctx, nt, origin, dims, spacing, &g);
+    if (rc) return rc;
+    void *d_rec, *d_tab;
+    if ((rc = scratch(ctx, 0, sizeof(float4) * std::max(n_rec, 1), &d_rec)) || (rc = scratch(ctx, 1, sizeof(float) * tab.size(), &d_tab))) {
+        tridsk_free_grid(g);
+        return rc;
+    }
+    DParams P;
+    to_dparams(params, &P);
+    cudaError_t e = cudaSuccess;
+    if (n_rec) e = cudaMemcpyAsync(d_rec, rec.data(), sizeof(float4) * n_rec, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_tab, tab.data(), sizeof(float) * tab.size(), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = launch_grid_build(ctx->stream, (const float4*)d_rec, n_rec, (const float*)d_tab, nt, P, g->d, dc_max, g->g);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);     // host staging vectors die at return
+    if (e != cudaSuccess) { tridsk_free_grid(g); return fail(ctx, TRIDSK_ECUDA, std::string("build_grid: ") + cudaGetErrorString(e)); }
+    ctx->launches += 1;
+    *out = g;
+    return TRIDSK_OK;
+}
+
+extern "C" int tridsk_grid_from_values(tridsk_ctx* ctx, const float* values, int n_types,
+                                       const float origin[3], const int dims[3], float spacing, tridsk_grid** out) {
+    if (!ctx || !out || !values) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    *out = nullptr;
+    tridsk_grid* g = nullptr;
+    int rc = new_grid(ctx, n_types, origin, dims, spacing, &g);
+    if (rc) return rc;
+    cudaError_t e = cudaMemcpyAsync(g->g, values, sizeof(float) * g->d.plane * n_types, cudaMemcpyDefault, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) { tridsk_free_grid(g); return fail(ctx, TRIDSK_ECUDA, std::string("grid copy: ") + cudaGetErrorString(e)); }
+    *out = g;
+    return TRIDSK_OK;
+}
+
+extern "C" int tridsk_grid_export(tridsk_ctx* ctx, const tridsk_grid* grid, float* dst) {
+    if (!ctx || !grid || !dst) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    CK(cudaMemcpyAsync(dst, grid->g, sizeof(float) * grid->d.plane * grid->d.n_types, cudaMemcpyDefault, ctx->stream));
+    if (!is_device_ptr(dst)) CK(cudaStreamSynchronize(ctx->stream));
+    return TRIDSK_OK;
+}
+
+extern "C" void tridsk_free_grid(tridsk_grid* g) {
+    if (!g) return;
+    if (g->ctx) cudaStreamSynchronize(g->ctx->stream);
+    if (g->g) cudaFree(g->g);
+    delete g;
+}
+
+// ---------------------------------------------------------------------------------------- ligands
+struct PackedLig {
+    LigHdr h;
+    std::vector<float4> f4;
+    std::vector<int> ai;
+    std::vector<FragRec> fr;
+    std::vector<PairRound> rounds;
+    int err = 0;
+    const char* msg = "";
+};
+
+// Host-side packing of one ligand: validation, depth-first atom order, fragment records, pair schedule.
+static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types, int i, PackedLig& out) {
+    const int a0 = b->atom_off[i], n = b->atom_off[i + 1] - a0;
+    const int t0 = b->tor_off[i], T = b->tor_off[i + 1] - t0;
+    auto bad = [&](int code, const char* m) { out.err = code; out.msg = m; };
+    if (n < 1 || T < 0) return bad(TRIDSK_EINVAL, "ligand with no atoms or negative torsion count");
+    if (n > TRIDSK_MAX_ATOMS) return bad(TRIDSK_ELIMIT, "ligand has more than 128 atoms");
+    if (T > TRIDSK_MAX_TORSIONS) return bad(TRIDSK_ELIMIT, "ligand has more than 31 torsions");
+    const float* ref = b->ref_xyz + 3 * (size_t)a0;
+    const unsigned char* type = b->atom_type + a0;
+    const unsigned char* frag = b->atom_frag + a0;
+    const unsigned char* ta = b->tor_a + t0;
+    const unsigned char* tb = b->tor_b + t0;
+    const signed char* tp = b->tor_parent + t0;
+    for (int a = 0; a < n; ++a) {
+        if (type[a] >= types->n_types) return bad(TRIDSK_EINVAL, "ligand atom type out of range");
+        if (frag[a] > T) return bad(TRIDSK_EINVAL, "atom_frag out of range");
+    }
+    std::vector<int> parent(T + 1, -1), depth(T + 1, 0);
+    for (int k = 0; k < T; ++k) {
+        if (tp[k] < -1 || tp[k] >= k) return bad(TRIDSK_EINVAL, "tor_parent must precede its children");
+        if (ta[k] >= n || tb[k] >= n || ta[k] == tb[k]) return bad(TRIDSK_EINVAL, "torsion axis atoms out of range");
+        if (frag[tb[k]] != k + 1) return bad(TRIDSK_EINVAL, "tor_b[k] must lie in fragment k+1");
+        if (frag[ta[k]] != tp[k] + 1) return bad(TRIDSK_EINVAL, "tor_a[k] must lie in the parent fragment");
+        parent[k + 1] = tp[k] + 1;
+        depth[k + 1] = depth[tp[k] + 1] + 1;
+    }
+    // depth-first preorder over fragments (children in torsion order)
+    std::vector<std::vector<int>> kids(T + 1);
+    for (int f = 1; f <= T; ++f) kids[parent[f]].push_back(f);
+    std::vector<int> order, stack{0};
+    while (!stack.empty()) {
+        int f = stack.back(); stack.pop_back();
+        order.push_back(f);
+        for (int c = (int)kids[f].size() - 1; c >= 0; --c) stack.push_back(kids[f][c]);
+    }
+    std::vector<int> count(T + 1, 0), sub(T + 1, 0), lo(T + 1, 0);
+    for (int a = 0; a < n; ++a) count[frag[a]]++;
+    for (int f = T; f >= 0; --f) { sub[f] += count[f]; if (f > 0) sub[parent[f]] += sub[f]; }
+    std::vector<int> newidx(n), oldidx(n);
+    {
+        int pos = 0;
+        for (int f : order) {
+            lo[f] = pos;
+            for (int a = 0; a < n; ++a) if (frag[a] == f) { newidx[a] = pos; oldidx[pos] = a; ++pos; }
+        }
+    }
+    const int J = (n + 31) / 32, S = (n + J - 1) / J;
+    LigHdr& h = out.h;
+    memset(&h, 0, sizeof(h));
+    h.n = n; h.T = T; h.J = J; h.S = S;
+    h.max_depth = *std::max_element(depth.begin(), depth.end());
+    out.f4.resize(n); out.ai.resize(n);
+    for (int p = 0; p < n; ++p) {
+        const int a = oldidx[p];
+        out.f4[p] = make_float4(ref[3 * a], ref[3 * a + 1], ref[3 * a + 2], types->radius[type[a]]);
+        out.ai[p] = (int)type[a] | ((int)frag[a] << 8) | (a << 16);
+    }
+    out.fr.resize(T + 1);
+    for (int f = 0; f <= T; ++f) {
+        FragRec& r = out.fr[f];
+        memset(&r, 0, sizeof(r));
+        r.ux = 1.f;
+        r.parent = parent[f]; r.depth = depth[f]; r.lo = lo[f]; r.hi = lo[f] + sub[f];
+        if (f > 0) {
+            const float* A = ref + 3 * ta[f - 1];
+            const float* B = ref + 3 * tb[f - 1];
+            const double ux = (double)B[0] - A[0], uy = (double)B[1] - A[1], uz = (double)B[2] - A[2];
+            const double un = sqrt(ux * ux + uy * uy + uz * uz);
+            if (!(un > 1e-6)) return bad(TRIDSK_EINVAL, "torsion axis of zero length");
+            r.ux = (float)(ux / un); r.uy = (float)(uy / un); r.uz = (float)(uz / un);   // layout: unit axis, reference frame
+            r.ox = B[0]; r.oy = B[1]; r.oz = B[2];
+        }
+    }
+    // intra-ligand pair set (internal indices)
+    std::vector<unsigned char> pm((size_t)n * n, 0);
+    int P = 0;
+    if (b->pair_off) {
+        const int p0 = b->pair_off[i], np = b->pair_off[i + 1] - p0;
+        for (int k = 0; k < np; ++k) {
+            const int a = b->pair_ab[2 * (size_t)(p0 + k)], c = b->pair_ab[2 * (size_t)(p0 + k) + 1];
+            if (a >= n || c >= n || a == c) return bad(TRIDSK_EINVAL, "pair index out of range");
+            const int x = newidx[a], y = newidx[c];
+            if (pm[(size_t)x * n + y]) return bad(TRIDSK_EINVAL, "duplicate intra-ligand pair");
+            pm[(size_t)x * n + y] = pm[(size_t)y * n + x] = 1;
+            ++P;
+        }
+    } else {
+        if (!b->bond_off || !b->bond_ab) return bad(TRIDSK_EINVAL, "neither pairs nor bonds given");
+        const int b0 = b->bond_off[i], nb = b->bond_off[i + 1] - b0;
+        std::vector<std::vector<int>> adj(n);
+        for (int k = 0; k < nb; ++k) {
+            const int a = b->bond_ab[2 * (size_t)(b0 + k)], c = b->bond_ab[2 * (size_t)(b0 + k) + 1];
+            if (a >= n || c >= n || a == c) return bad(TRIDSK_EINVAL, "bond index out of range");
+            adj[a].push_back(c); adj[c].push_back(a);
+        }
+        // O6: pairs = {a<b : bond-graph distance >= 4 and different rigid fragment}
+        std::vector<int> dist(n);
+        for (int a = 0; a < n; ++a) {
+            std::fill(dist.begin(), dist.end(), 1 << 20);
+            dist[a] = 0;
+            std::vector<int> cur{a};
+            for (int d = 1; d <= 3 && !cur.empty(); ++d) {
+                std::vector<int> nxt;
+                for (int u : cur) for (int v : adj[u]) if (dist[v] > d) { dist[v] = d; nxt.push_back(v); }
+                cur.swap(nxt);
+            }
+            for (int c = a + 1; c < n; ++c)
+                if (dist[c] > 3 && frag[a] != frag[c]) {
+                    pm[(size_t)newidx[a] * n + newidx[c]] = pm[(size_t)newidx[c] * n + newidx[a]] = 1;
+                    ++P;
+                }
+        }
+    }
+    h.n_pairs = P;
+    // conflict-free schedule: round (j1, j2, k): lane l <-> pair (j1*S + l, j2*S + (l+k) mod S)
+    auto hb = [&](int x, int y) {
+        const unsigned char rs = types->hb_role[out.ai[x] & 0xff], rt = types->hb_role[out.ai[y] & 0xff];
+        return ((rs & 1) && (rt & 2)) || ((rs & 2) && (rt & 1));
+    };
+    int tile = 0, covered = 0;
+    for (int j1 = 0; j1 < J; ++j1)
+        for (int j2 = j1; j2 < J; ++j2, ++tile) {
+            h.tile_off[tile] = (int)out.rounds.size();
+            const int k_lo = (j1 == j2) ? 1 : 0, k_hi = (j1 == j2) ? S / 2 : S - 1;
+            for (int k = k_lo; k <= k_hi; ++k) {
+                PairRound r{0u, 0u, k, 0};
+                const bool half = (j1 == j2) && (S % 2 == 0) && (k == S / 2);
+                for (int l = 0; l < S; ++l) {
+                    if (half && l >= S / 2) break;
+                    const int A = j1 * S + l, B = j2 * S + (l + k) % S;
+                    if (A >= n || B >= n || !pm[(size_t)A * n + B]) continue;
+                    r.mask |= 1u << l;
+                    if (hb(A, B)) r.hb |= 1u << l;
+                    ++covered;
+                }
+                if (r.mask) out.rounds.push_back(r);
+            }
+        }
+    for (int t = tile; t <= TRIDSK_MAX_TILES; ++t) h.tile_off[t] = (int)out.rounds.size();
+    if (covered != P) return bad(TRIDSK_EINVAL, "internal: pair schedule does not cover the pair set");
+}
+
+extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b, const tridsk_types* types,
+                                   tridsk_ligands** out) {
+    if (!ctx || !b || !out) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    *out = nullptr;
+    int rc = check_types(ctx, types);
+    if (rc) return rc;
+    if (b->n_lig < 0 || !b->atom_off || !b->tor_off || (b->n_lig && (!b->ref_xyz || !b->atom_type || !b->atom_frag)))
+        return fail(ctx, TRIDSK_EINVAL, "bad ligand batch");
+    const int L = b->n_lig;
+    std::vector<PackedLig> pk(L);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int i = 0; i < L; ++i) pack_ligand(b, types, i, pk[i]);
+    for (int i = 0; i < L; ++i)
+        if (pk[i].err) return fail(ctx, pk[i].err, std::string("ligand ") + std::to_string(i) + ": " + pk[i].msg);
+
+    tridsk_ligands* lg = new (std::nothrow) tridsk_ligands();
+    if (!lg) return fail(ctx, TRIDSK_ENOMEM, "host alloc");
+    lg->ctx = ctx; lg->n_lig = L;
+    size_t na = 0, nf = 0, nr = 0;
+    lg->hdr_h.resize(L); lg->n_pairs.resize(L);
+    for (int i = 0; i < L; ++i) {
+        LigHdr& h = pk[i].h;
+        h.atom_off = (int)na; h.frag_off = (int)nf; h.round_off = (int)nr;
+        na += pk[i].f4.size(); nf += pk[i].fr.size(); nr += pk[i].rounds.size();
+        lg->hdr_h[i] = h; lg->n_pairs[i] = h.n_pairs;
+        lg->max_atoms = std::max(lg->max_atoms, h.n); lg->max_tor = std::max(lg->max_tor, h.T);
+        lg->bucket[h.J].push_back(i);
+    }
+    std::vector<float4> f4(na);
+    std::vector<int> ai(na);
+    std::vector<FragRec> fr(nf);
+    std::vector<PairRound> rd(std::max<size_t>(nr, 1));
+    for (int i = 0; i < L; ++i) {
+        const LigHdr& h = pk[i].h;
+        std::copy(pk[i].f4.begin(), pk[i].f4.end(), f4.begin() + h.atom_off);
+        std::copy(pk[i].ai.begin(), pk[i].ai.end(), ai.begin() + h.atom_off);
+        std::copy(pk[i].fr.begin(), pk[i].fr.end(), fr.begin() + h.frag_off);
+        std::copy(pk[i].rounds.begin(), pk[i].rounds.end(), rd.begin() + h.round_off);
+    }
+    cudaError_t e = cudaSuccess;
+    auto up = [&](void** d, const void* src, size_t bytes) {
+        if (e != cudaSuccess) return;
+        e = cudaMalloc(d, std::max<size_t>(bytes, 16));
+        if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(*d, src, bytes, cudaMemcpyHostToDevice, ctx->stream);
+    };
+    up((void**)&lg->hdr, lg->hdr_h.data(), sizeof(LigHdr) * L);
+    up((void**)&lg->atom_f4, f4.data(), sizeof(float4) * na);
+    up((void**)&lg->atom_i, ai.data(), sizeof(int) * na);
+    up((void**)&lg->frags, fr.data(), sizeof(FragRec) * nf);
+    up((void**)&lg->rounds, rd.data(), sizeof(PairRound) * rd.size());
+    for (int j = 1; j <= TRIDSK_MAX_J; ++j)
+        if (!lg->bucket[j].empty()) up((void**)&lg->bucket_dev[j], lg->bucket[j].data(), sizeof(int) * lg->bucket[j].size());
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) {
+        tridsk_free_ligands(lg);
+        return fail(ctx, e == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA, std::string("load_ligands: ") + cudaGetErrorString(e));
+    }
+    *out = lg;
+    return TRIDSK_OK;
+}
+
+extern "C" int tridsk_ligand_info(const tridsk_ligands* l, int* n_lig, int* max_atoms, int* max_torsions, int* n_pairs_out) {
+    if (!l) return TRIDSK_EINVAL;
+    if (n_lig) *n_lig = l->n_lig;
+    if (max_atoms) *max_atoms = l->max_atoms;
+    if (max_torsions) *max_torsions = l->max_tor;
+    if (n_pairs_out) std::copy(l->n_pairs.begin(), l->n_pairs.end(), n_pairs_out);
+    return TRIDSK_OK;
+}
+
+extern "C" void tridsk_free_ligands(tridsk_ligands* l) {
+    if (!l) return;
+    if (l->ctx) cudaStreamSynchronize(l->ctx->stream);
+    cudaFree(l->hdr); cudaFree(l->atom_f4); cudaFree(l->atom_i); cudaFree(l->frags); cudaFree(l->rounds);
+    for (int j = 0; j <= TRIDSK_MAX_J; ++j) if (l->bucket_dev[j]) cudaFree(l->bucket_dev[j]);
+    delete l;
+}
+
+// ---------------------------------------------------------------------------------------- score + gradient
+extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* ligs,
+                                 const tridsk_params* params, const int* lig_index, const float* poses, int n_pose,
+                                 int pose_stride, float* energy, float* grad, int grad_stride, float* coords, int coord_stride) {
+    if (!ctx || !grid || !ligs || !params || !lig_index || !poses || !energy || n_pose < 0)
+        return fail(ctx, TRIDSK_EINVAL, "null argument");
+    if (pose_stride < 7 + ligs->max_tor) return fail(ctx, TRIDSK_EINVAL, "pose_stride < 7 + max torsions");
+    if (grad && grad_stride < 6 + ligs->max_tor) return fail(ctx, TRIDSK_EINVAL, "grad_stride < 6 + max torsions");
+    if (coords && coord_stride < ligs->max_atoms) return fail(ctx, TRIDSK_EINVAL, "coord_stride < max atoms");
+    if (n_pose == 0) return TRIDSK_OK;
+    // lig_index must be validated on the host: stage a host copy if it lives on the device
+    std::vector<int> li(n_pose);
+    CK(cudaMemcpyAsync(li.data(), lig_index, sizeof(int) * n_pose, cudaMemcpyDefault, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < n_pose; ++i)
+        if (li[i] < 0 || li[i] >= ligs->n_lig) return fail(ctx, TRIDSK_EINVAL, "lig_index out of range");
+    ScoreLaunch a;
+    a.hdr = ligs->hdr; a.atom_f4 = ligs->atom_f4; a.atom_i = ligs->atom_i; a.frags = ligs->frags; a.rounds = ligs->rounds;
+    a.grid = grid->d;
+    to_dparams(params, &a.P);
+    a.n_pose = n_pose; a.pose_stride = pose_stride; a.grad_stride = grad_stride; a.coord_stride = coord_stride;
+    const size_t b_li = sizeof(int) * n_pose, b_po = sizeof(float) * (size_t)n_pose * pose_stride;
+    const size_t b_e = sizeof(float) * 3 * n_pose, b_g = grad ? sizeof(float) * (size_t)n_pose * grad_stride : 0;
+    const size_t b_c = coords ? sizeof(float) * 3 * (size_t)n_pose * coord_stride : 0;
+    // inputs: slot 7 holds [lig_index | poses] when they come from the host
+    const bool h_li = !is_device_ptr(lig_index), h_po = !is_device_ptr(poses);
+    char* in = nullptr;
+    if (h_li || h_po) { int rc = scratch(ctx, 7, b_li + b_po + 64, (void**)&in); if (rc) return rc; }
+    const size_t o_po = (b_li + 15) / 16 * 16;
+    if (h_li) { CK(cudaMemcpyAsync(in, li.data(), b_li, cudaMemcpyHostToDevice, ctx->stream)); a.lig_index = (const int*)in; }
+    else a.lig_index = lig_index;
+    if (h_po) { CK(cudaMemcpyAsync(in + o_po, poses, b_po, cudaMemcpyHostToDevice, ctx->stream)); a.poses = (const float*)(in + o_po); }
+    else a.poses = poses;
+    // outputs: slot 6 holds device temporaries for host outputs
+    const bool h_e = !is_device_ptr(energy), h_g = grad && !is_device_ptr(grad), h_c = coords && !is_device_ptr(coords);
+    char* ob = nullptr;
+    const size_t o_g = (b_e + 15) / 16 * 16, o_c = o_g + (b_g + 15) / 16 * 16;
+    if (h_e || h_g || h_c) { int rc = scratch(ctx, 6, o_c + b_c + 64, (void**)&ob); if (rc) return rc; }
+    a.energy = h_e ? (float*)ob : energy;
+    a.grad = grad ? (h_g ? (float*)(ob + o_g) : grad) : nullptr;
+    a.coords = coords ? (h_c ? (float*)(ob + o_c) : coords) : nullptr;
+    CK(launch_score(ctx->stream, a));
+    ctx->launches += 1;
+    if (h_e) CK(cudaMemcpyAsync(energy, a.energy, b_e, cudaMemcpyDeviceToHost, ctx->stream));
+    if (h_g) CK(cudaMemcpyAsync(grad, a.grad, b_g, cudaMemcpyDeviceToHost, ctx->stream));
+    if (h_c) CK(cudaMemcpyAsync(coords, a.coords, b_c, cudaMemcpyDeviceToHost, ctx->stream));
+    // li (host vector) was consumed by an async copy: always drain before it goes out of scope
+    if (h_e || h_g || h_c || h_li) CK(cudaStreamSynchronize(ctx->stream));
+    return TRIDSK_OK;
+}
+
+// ---------------------------------------------------------------------------------------- dock
+extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* ligs, const tridsk_params* params,
+                           const float box_min[3], const float box_max[3], const float pocket_center[3], float pocket_radius,
+                           int n_chains, int n_steps, int top_k, unsigned long long seed, int pose_stride,
+                           float* out_energy, float* out_pose, int* out_chain, const tridsk_dock_opts* opts_in) {
+    if (!ctx || !grid || !ligs || !params || !box_min || !box_max || !pocket_center)
+        return fail(ctx, TRIDSK_EINVAL, "null argument");
+    tridsk_dock_opts o;
+    memset(&o, 0, sizeof(o));
+    if (opts_in) o = *opts_in;
+    if (n_chains < 1 || n_steps < 0 || top_k < 0 || top_k > n_chains) return fail(ctx, TRIDSK_EINVAL, "bad n_chains / n_steps / top_k");
+    if (top_k > 0 && (!out_energy || !out_pose || !out_chain)) return fail(ctx, TRIDSK_EINVAL, "null output");
+    if (pose_stride < 7 + ligs->max_tor) return fail(ctx, TRIDSK_EINVAL, "pose_stride < 7 + max torsions");
+    if (params->n_refine < 0 || o.first_step < 0 || o.steps_per_launch < 0) return fail(ctx, TRIDSK_EINVAL, "bad option");
+    if (o.resume && !o.chain_state) return fail(ctx, TRIDSK_EINVAL, "resume needs chain_state");
+    if (o.resume && o.init_poses) return fail(ctx, TRIDSK_EINVAL, "resume and init_poses are exclusive");
+    for (int c = 0; c < 3; ++c) if (!(box_min[c] <= box_max[c])) return fail(ctx, TRIDSK_EINVAL, "box_min > box_max");
+    const int L = ligs->n_lig;
+    if (L == 0) return TRIDSK_OK;
+    const size_t nch = (size_t)L * n_chains, n_pose_f = nch * pose_stride;
+
+    // chain state: {pose_cur, pose_best, e_cur, e_best} -- the caller's device buffer, or ctx scratch
+    const size_t state_floats = 2 * n_pose_f + 2 * nch;
+    float* state = nullptr;
+    const bool state_host = o.chain_state && !is_device_ptr(o.chain_state);
+    if (o.chain_state && !state_host) state = o.chain_state;
+    else { int rc = scratch(ctx, 2, sizeof(float) * state_floats, (void**)&state); if (rc) return rc; }
+    if (o.resume && state_host) CK(cudaMemcpyAsync(state, o.chain_state, sizeof(float) * state_floats, cudaMemcpyHostToDevice, ctx->stream));
+    const void* d_init = nullptr;
+    if (o.init_poses) { int rc = stage_in(ctx, 7, o.init_poses, sizeof(float) * n_pose_f, &d_init); if (rc) return rc; }
+    tridsk_trace_rec* d_trace = nullptr;
+    const size_t trace_bytes = sizeof(tridsk_trace_rec) * nch * (size_t)n_steps;
+    const bool trace_host = o.trace && !is_device_ptr(o.trace);
+    if (o.trace && n_steps > 0) {
+        if (trace_host) { int rc = scratch(ctx, 3, trace_bytes, (void**)&d_trace); if (rc) return rc; }
+        else d_trace = o.trace;
+    }
+    // outputs
+    const size_t b_oe = sizeof(float) * 2 * (size_t)L * top_k, b_op = sizeof(float) * (size_t)L * top_k * pose_stride;
+    const size_t b_oc = sizeof(int) * (size_t)L * top_k;
+    const bool h_oe = top_k && !is_device_ptr(out_energy), h_op = top_k && !is_device_ptr(out_pose), h_oc = top_k && !is_device_ptr(out_chain);
+    char* ob = nullptr;
+    const size_t o_p = (b_oe + 15) / 16 * 16, o_c = o_p + (b_op + 15) / 16 * 16;
+    if (h_oe || h_op || h_oc) { int rc = scratch(ctx, 6, o_c + b_oc + 64, (void**)&ob); if (rc) return rc; }
+
+    McLaunch base;
+    memset(&base, 0, sizeof(base));
+    base.hdr = ligs->hdr; base.atom_f4 = ligs->atom_f4; base.atom_i = ligs->atom_i; base.frags = ligs->frags; base.rounds = ligs->rounds;
+    base.grid = grid->d;
+    to_dparams(params, &base.P);
+    for (int c = 0; c < 3; ++c) { base.box_min[c] = box_min[c]; base.box_max[c] = box_max[c]; base.centre[c] = pocket_center[c]; }
+    base.radius = pocket_radius;
+    base.n_chains = n_chains; base.pose_stride = pose_stride; base.seed = seed;
+    base.init_poses = (const float*)d_init;
+    base.pose_cur = state; base.pose_best = state + n_pose_f; base.e_cur = state + 2 * n_pose_f; base.e_best = state + 2 * n_pose_f + nch;
+    base.trace = d_trace; base.trace_stride = n_steps;
+
+    // launch series: per steps_per_launch slice, one launch per atoms-per-lane bucket J; then top-k
+    std::vector<std::pair<int, McLaunch>> series;
+    const int spl = (o.steps_per_launch > 0) ? o.steps_per_launch : std::max(n_steps, 1);
+    int done = 0;
+    bool first = true;
+    do {
+        const int ns = std::min(spl, n_steps - done);
+        for (int j = 1; j <= TRIDSK_MAX_J; ++j) {
+            if (ligs->bucket[j].empty()) continue;
+            McLaunch a = base;
+            a.lig_list = ligs->bucket_dev[j]; a.n_list = (int)ligs->bucket[j].size();
+            a.first_step = o.first_step + done; a.n_steps = ns; a.trace_off = done;
+            a.init_mode = first ? (o.resume ? 2 : (o.init_poses ? 1 : 0)) : 2;
+            series.push_back({j, a});
+        }
+        done += ns; first = false;
+    } while (done < n_steps);
+    TopkLaunch tk;
+    memset(&tk, 0, sizeof(tk));
+    tk.hdr = ligs->hdr; tk.e_best = base.e_best; tk.pose_best = base.pose_best;
+    tk.n_lig = L; tk.n_chains = n_chains; tk.pose_stride = pose_stride; tk.top_k = top_k; tk.w_tor = params->w_tor;
+    tk.out_energy = h_oe ? (float*)ob : out_energy;
+    tk.out_pose = h_op ? (float*)(ob + o_p) : out_pose;
+    tk.out_chain = h_oc ? (int*)(ob + o_c) : out_chain;
+    const int n_launch = (int)series.size() + (top_k > 0 ? 1 : 0);
+
+    auto enqueue = [&](cudaStream_t s) -> cudaError_t {
+        for (auto& it : series) { cudaError_t e = launch_mc(s, it.first, it.second); if (e != cudaSuccess) return e; }
+        if (top_k > 0) return launch_topk(s, tk);
+        return cudaSuccess;
+    };
+    if (o.no_graph) {
+        CK(enqueue(ctx->stream));
+    } else {
+        // a10: the whole series as one CUDA graph; re-used while the launch parameters are byte-identical
+        std::vector<unsigned char> key;
+        for (auto& it : series) {
+            key.insert(key.end(), (unsigned char*)&it.first, (unsigned char*)&it.first + sizeof(int));
+            key.insert(key.end(), (unsigned char*)&it.second, (unsigned char*)&it.second + sizeof(McLaunch));
+        }
+        key.insert(key.end(), (unsigned char*)&tk, (unsigned char*)&tk + sizeof(tk));
+        if (!ctx->graph_exec || key != ctx->graph_key) {
+            if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; }
+            cudaGraph_t graph = nullptr;
+            CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+            cudaError_t e = enqueue(ctx->stream);
+            cudaError_t e2 = cudaStreamEndCapture(ctx->stream, &graph);
+            if (e != cudaSuccess || e2 != cudaSuccess) {
+                if (graph) cudaGraphDestroy(graph);
+                return fail(ctx, TRIDSK_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e != cudaSuccess ? e : e2));
+            }
+            e = cudaGraphInstantiate(&ctx->graph_exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { ctx->graph_exec = nullptr; return fail(ctx, TRIDSK_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e)); }
+            ctx->graph_key = key;
+        }
+        CK(cudaGraphLaunch(ctx->graph_exec, ctx->stream));
+    }
+    ctx->launches += n_launch;
+
+    bool need_sync = false;
+    if (h_oe) { CK(cudaMemcpyAsync(out_energy, tk.out_energy, b_oe, cudaMemcpyDeviceToHost, ctx->stream)); need_sync = true; }
+    if (h_op) { CK(cudaMemcpyAsync(out_pose, tk.out_pose, b_op, cudaMemcpyDeviceToHost, ctx->stream)); need_sync = true; }
+    if (h_oc) { CK(cudaMemcpyAsync(out_chain, tk.out_chain, b_oc, cudaMemcpyDeviceToHost, ctx->stream)); need_sync = true; }
+    if (state_host) { CK(cudaMemcpyAsync(o.chain_state, state, sizeof(float) * state_floats, cudaMemcpyDeviceToHost, ctx->stream)); need_sync = true; }
+    if (trace_host && d_trace) { CK(cudaMemcpyAsync(o.trace, d_trace, trace_bytes, cudaMemcpyDeviceToHost, ctx->stream)); need_sync = true; }
+    if (need_sync || (o.init_poses && !is_device_ptr(o.init_poses)) || (o.resume && state_host)) CK(cudaStreamSynchronize(ctx->stream));
+    return TRIDSK_OK;
+}
+
+// ---------------------------------------------------------------------------------------- test hook
+extern "C" int tridsk_debug_philox(tridsk_ctx* ctx, const unsigned int ctr[4], const unsigned int key[2], unsigned int out[4]) {
+    if (!ctx || !ctr || !key || !out) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    unsigned int h[6] = {ctr[0], ctr[1], ctr[2], ctr[3], key[0], key[1]};
+    unsigned int* d;
+    int rc = scratch(ctx, 7, 64, (void**)&d);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(d, h, sizeof(h), cudaMemcpyHostToDevice, ctx->stream));
+    CK(launch_philox_debug(ctx->stream, d, d + 8));
+    ctx->launches += 1;
+    CK(cudaMemcpyAsync(out, d + 8, 4 * sizeof(unsigned int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return TRIDSK_OK;
+}
