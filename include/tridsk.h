@@ -112,6 +112,8 @@ typedef struct {
     tridsk_trace_rec* trace;   /* [host|dev] NULL, or [n_lig][n_chains][n_steps]                                      */
     int steps_per_launch;      /* MC steps per kernel launch; 0 = all n_steps in one launch                           */
     int no_graph;              /* 1: plain stream launches instead of a captured CUDA graph                           */
+    int chain_base;            /* Philox chain id of local chain 0 (chain sharding across GPUs; results then do not
+                                  depend on the GPU count)                                                            */
 } tridsk_dock_opts;
 
 /* ---- lifetime ------------------------------------------------------------------------------ */
@@ -174,6 +176,10 @@ int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* 
                 const float box_min[3], const float box_max[3], const float pocket_center[3], float pocket_radius,
                 int n_chains, int n_steps, int top_k, unsigned long long seed, int pose_stride,
                 float* out_energy, float* out_pose, int* out_chain, const tridsk_dock_opts* opts);
+
+/* Device time of the last tridsk_dock on this ctx, from CUDA events recorded on the ctx stream around the fused MC
+ * kernel series and the top-k kernel: ms[0] = MC series, ms[1] = top-k.  Blocks until that dock has finished. [host] */
+int tridsk_last_dock_ms(tridsk_ctx* ctx, float ms[2]);
 
 /* Kernel launches enqueued by this ctx since creation (bench.py's gpu_launches). */
 long long tridsk_launch_count(const tridsk_ctx* ctx);

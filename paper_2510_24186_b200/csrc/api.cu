@@ -104,6 +104,7 @@ extern "C" void tridsk_destroy(tridsk_ctx* ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
     if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
+    for (int i = 0; i < 3; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     for (int i = 0; i < 8; ++i) if (ctx->scratch[i]) cudaFree(ctx->scratch[i]);
     if (ctx->own_stream) cudaStreamDestroy(ctx->stream);
     delete ctx;
@@ -562,7 +563,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     to_dparams(params, &base.P);
     for (int c = 0; c < 3; ++c) { base.box_min[c] = box_min[c]; base.box_max[c] = box_max[c]; base.centre[c] = pocket_center[c]; }
     base.radius = pocket_radius;
-    base.n_chains = n_chains; base.pose_stride = pose_stride; base.seed = seed;
+    base.n_chains = n_chains; base.pose_stride = pose_stride; base.seed = seed; base.chain_base = o.chain_base;
     base.init_poses = (const float*)d_init;
     base.pose_cur = state; base.pose_best = state + n_pose_f; base.e_cur = state + 2 * n_pose_f; base.e_best = state + 2 * n_pose_f + nch;
     base.trace = d_trace; base.trace_stride = n_steps;
@@ -593,10 +594,17 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     tk.out_chain = h_oc ? (int*)(ob + o_c) : out_chain;
     const int n_launch = (int)series.size() + (top_k > 0 ? 1 : 0);
 
+    for (int i = 0; i < 3; ++i) if (!ctx->ev[i]) CK(cudaEventCreate(&ctx->ev[i]));
+    ctx->ev_valid = false;
+    // events are recorded with the External flag so that they stay queryable when captured into the graph
     auto enqueue = [&](cudaStream_t s) -> cudaError_t {
-        for (auto& it : series) { cudaError_t e = launch_mc(s, it.first, it.second); if (e != cudaSuccess) return e; }
-        if (top_k > 0) return launch_topk(s, tk);
-        return cudaSuccess;
+        cudaError_t e = cudaEventRecordWithFlags(ctx->ev[0], s, cudaEventRecordExternal);
+        if (e != cudaSuccess) return e;
+        for (auto& it : series) { e = launch_mc(s, it.first, it.second); if (e != cudaSuccess) return e; }
+        e = cudaEventRecordWithFlags(ctx->ev[1], s, cudaEventRecordExternal);
+        if (e != cudaSuccess) return e;
+        if (top_k > 0) { e = launch_topk(s, tk); if (e != cudaSuccess) return e; }
+        return cudaEventRecordWithFlags(ctx->ev[2], s, cudaEventRecordExternal);
     };
     if (o.no_graph) {
         CK(enqueue(ctx->stream));
@@ -626,6 +634,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         CK(cudaGraphLaunch(ctx->graph_exec, ctx->stream));
     }
     ctx->launches += n_launch;
+    ctx->ev_valid = true;
 
     bool need_sync = false;
     if (h_oe) { CK(cudaMemcpyAsync(out_energy, tk.out_energy, b_oe, cudaMemcpyDeviceToHost, ctx->stream)); need_sync = true; }
@@ -634,6 +643,15 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     if (state_host) { CK(cudaMemcpyAsync(o.chain_state, state, sizeof(float) * state_floats, cudaMemcpyDeviceToHost, ctx->stream)); need_sync = true; }
     if (trace_host && d_trace) { CK(cudaMemcpyAsync(o.trace, d_trace, trace_bytes, cudaMemcpyDeviceToHost, ctx->stream)); need_sync = true; }
     if (need_sync || (o.init_poses && !is_device_ptr(o.init_poses)) || (o.resume && state_host)) CK(cudaStreamSynchronize(ctx->stream));
+    return TRIDSK_OK;
+}
+
+extern "C" int tridsk_last_dock_ms(tridsk_ctx* ctx, float ms[2]) {
+    if (!ctx || !ms) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    if (!ctx->ev_valid) return fail(ctx, TRIDSK_EINVAL, "no dock has run on this ctx");
+    CK(cudaEventSynchronize(ctx->ev[2]));
+    CK(cudaEventElapsedTime(&ms[0], ctx->ev[0], ctx->ev[1]));
+    CK(cudaEventElapsedTime(&ms[1], ctx->ev[1], ctx->ev[2]));
     return TRIDSK_OK;
 }
 

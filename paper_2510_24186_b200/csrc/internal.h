@@ -74,6 +74,7 @@ struct McLaunch {
     DParams P;
     float box_min[3], box_max[3], centre[3], radius;
     int n_chains, pose_stride;
+    int chain_base;               // global id of local chain 0 in the Philox counter (multi-GPU chain sharding)
     unsigned long long seed;
     int first_step, n_steps;
     int init_mode;                // 0 Philox init, 1 from init_poses, 2 resume from state
@@ -125,6 +126,8 @@ struct tridsk_ctx {
     cudaGraphExec_t graph_exec = nullptr;
     std::vector<unsigned char> graph_key;
     int graph_launches = 0;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // dock: before MC series, after MC series, after top-k
+    bool ev_valid = false;
 };
 
 struct tridsk_grid {
