@@ -9,6 +9,7 @@ from __future__ import annotations
 
 import ctypes as C
 import os
+import weakref
 
 import numpy as np
 
@@ -98,6 +99,7 @@ class Grid:
     def __init__(self, eng, handle, n_types, dims, origin, spacing):
         self.eng, self.handle, self.n_types, self.dims = eng, handle, n_types, tuple(dims)
         self.origin, self.spacing = np.asarray(origin, np.float32), float(spacing)
+        eng._children.add(self)
 
     def export(self):
         nx, ny, nz = self.dims
@@ -120,6 +122,7 @@ class Grid:
 class Ligands:
     def __init__(self, eng, handle):
         self.eng, self.handle = eng, handle
+        eng._children.add(self)
         n, na, nt = C.c_int(), C.c_int(), C.c_int()
         lib().tridsk_ligand_info(handle, C.byref(n), C.byref(na), C.byref(nt), None)
         self.n_lig, self.max_atoms, self.max_tor = n.value, na.value, nt.value
@@ -149,6 +152,7 @@ class Engine:
         self.device = torch.device("cuda", device)
         self.stream = torch.cuda.Stream(device=self.device)
         self.ctx = C.c_void_p()
+        self._children = weakref.WeakSet()      # live Grid / Ligands handles: freed before the ctx
         rc = lib().tridsk_create(C.byref(self.ctx), C.c_int(device), C.c_void_p(self.stream.cuda_stream))
         if rc != OK:
             raise TridskError(rc, "tridsk_create failed")
@@ -158,6 +162,8 @@ class Engine:
             raise TridskError(rc, lib().tridsk_last_error(self.ctx).decode())
 
     def close(self):
+        for ch in list(self._children):
+            ch.free()
         if self.ctx:
             lib().tridsk_destroy(self.ctx)
             self.ctx = C.c_void_p()

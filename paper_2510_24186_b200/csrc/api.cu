@@ -223,8 +223,7 @@ extern "C" int tridsk_grid_export(tridsk_ctx* ctx, const tridsk_grid* grid, floa
 
 extern "C" void tridsk_free_grid(tridsk_grid* g) {
     if (!g) return;
-    if (g->ctx) cudaStreamSynchronize(g->ctx->stream);
-    if (g->g) cudaFree(g->g);
+    if (g->g) cudaFree(g->g);       // cudaFree waits for the device; g->ctx may already be destroyed
     delete g;
 }
 
@@ -453,8 +452,7 @@ extern "C" int tridsk_ligand_info(const tridsk_ligands* l, int* n_lig, int* max_
 }
 
 extern "C" void tridsk_free_ligands(tridsk_ligands* l) {
-    if (!l) return;
-    if (l->ctx) cudaStreamSynchronize(l->ctx->stream);
+    if (!l) return;                 // cudaFree waits for the device; l->ctx may already be destroyed
     cudaFree(l->hdr); cudaFree(l->atom_f4); cudaFree(l->atom_i); cudaFree(l->frags); cudaFree(l->rounds);
     for (int j = 0; j <= TRIDSK_MAX_J; ++j) if (l->bucket_dev[j]) cudaFree(l->bucket_dev[j]);
     delete l;
@@ -596,18 +594,20 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
 
     for (int i = 0; i < 3; ++i) if (!ctx->ev[i]) CK(cudaEventCreate(&ctx->ev[i]));
     ctx->ev_valid = false;
-    // events are recorded with the External flag so that they stay queryable when captured into the graph
-    auto enqueue = [&](cudaStream_t s) -> cudaError_t {
-        cudaError_t e = cudaEventRecordWithFlags(ctx->ev[0], s, cudaEventRecordExternal);
+    // inside a capture the events are recorded with the External flag (event-record nodes that stay queryable);
+    // that flag is only legal while capturing
+    auto enqueue = [&](cudaStream_t s, bool capturing) -> cudaError_t {
+        const unsigned fl = capturing ? cudaEventRecordExternal : cudaEventRecordDefault;
+        cudaError_t e = cudaEventRecordWithFlags(ctx->ev[0], s, fl);
         if (e != cudaSuccess) return e;
         for (auto& it : series) { e = launch_mc(s, it.first, it.second); if (e != cudaSuccess) return e; }
-        e = cudaEventRecordWithFlags(ctx->ev[1], s, cudaEventRecordExternal);
+        e = cudaEventRecordWithFlags(ctx->ev[1], s, fl);
         if (e != cudaSuccess) return e;
         if (top_k > 0) { e = launch_topk(s, tk); if (e != cudaSuccess) return e; }
-        return cudaEventRecordWithFlags(ctx->ev[2], s, cudaEventRecordExternal);
+        return cudaEventRecordWithFlags(ctx->ev[2], s, fl);
     };
     if (o.no_graph) {
-        CK(enqueue(ctx->stream));
+        CK(enqueue(ctx->stream, false));
     } else {
         // a10: the whole series as one CUDA graph; re-used while the launch parameters are byte-identical
         std::vector<unsigned char> key;
@@ -620,7 +620,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
             if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; }
             cudaGraph_t graph = nullptr;
             CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
-            cudaError_t e = enqueue(ctx->stream);
+            cudaError_t e = enqueue(ctx->stream, true);
             cudaError_t e2 = cudaStreamEndCapture(ctx->stream, &graph);
             if (e != cudaSuccess || e2 != cudaSuccess) {
                 if (graph) cudaGraphDestroy(graph);
