@@ -177,6 +177,14 @@ int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* 
                 int n_chains, int n_steps, int top_k, unsigned long long seed, int pose_stride,
                 float* out_energy, float* out_pose, int* out_chain, const tridsk_dock_opts* opts);
 
+/*
+ * Chain-to-thread mapping of the fused kernel: 0 = automatic (a warp per chain when chains are few,
+ * a lane per chain when n_lig * n_chains >= 256 per SM), 1 = always a warp per chain, 2 = always a lane per chain.
+ * Applies to tridsk_dock and tridsk_score_grad on this ctx.  Both mappings compute O1..O13; their fp32 summation
+ * orders differ, so chains are bit-reproducible per mapping, not across mappings.
+ */
+int tridsk_set_kernel(tridsk_ctx* ctx, int kernel);
+
 /* Device time of the last tridsk_dock on this ctx, from CUDA events recorded on the ctx stream around the fused MC
  * kernel series and the top-k kernel: ms[0] = MC series, ms[1] = top-k.  Blocks until that dock has finished. [host] */
 int tridsk_last_dock_ms(tridsk_ctx* ctx, float ms[2]);

@@ -177,6 +177,10 @@ class Engine:
     def synchronize(self):
         self._ck(lib().tridsk_synchronize(self.ctx))
 
+    def set_kernel(self, kernel: int):
+        """0 auto, 1 warp per chain, 2 lane per chain (tridsk_set_kernel)."""
+        self._ck(lib().tridsk_set_kernel(self.ctx, C.c_int(kernel)))
+
     def launch_count(self) -> int:
         return int(lib().tridsk_launch_count(self.ctx))
 

@@ -137,8 +137,9 @@ static int new_grid(tridsk_ctx* ctx, int n_types, const float origin[3], const i
     g->d.ox = origin[0]; g->d.oy = origin[1]; g->d.oz = origin[2];
     g->d.h = spacing; g->d.inv_h = 1.0f / spacing;
     cudaError_t e = cudaMalloc(&g->g, sizeof(float) * g->d.plane * n_types);
-    if (e != cudaSuccess) { delete g; return fail(ctx, TRIDSK_ENOMEM, std::string("grid alloc: ") + cudaGetErrorString(e)); }
-    g->d.g = g->g;
+    if (e == cudaSuccess) e = cudaMalloc(&g->gp, sizeof(float4) * g->d.plane * n_types);   // xy-packed copy (DGrid::gp)
+    if (e != cudaSuccess) { cudaFree(g->g); delete g; return fail(ctx, TRIDSK_ENOMEM, std::string("grid alloc: ") + cudaGetErrorString(e)); }
+    g->d.g = g->g; g->d.gp = g->gp;
     *out = g;
     return TRIDSK_OK;
 }
@@ -193,9 +194,10 @@ extern "C" int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const in
     if (n_rec) e = cudaMemcpyAsync(d_rec, rec.data(), sizeof(float4) * n_rec, cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_tab, tab.data(), sizeof(float) * tab.size(), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = launch_grid_build(ctx->stream, (const float4*)d_rec, n_rec, (const float*)d_tab, nt, P, g->d, dc_max, g->g);
+    if (e == cudaSuccess) e = launch_grid_pack(ctx->stream, g->d, g->gp);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);     // host staging vectors die at return
     if (e != cudaSuccess) { tridsk_free_grid(g); return fail(ctx, TRIDSK_ECUDA, std::string("build_grid: ") + cudaGetErrorString(e)); }
-    ctx->launches += 1;
+    ctx->launches += 2;
     *out = g;
     return TRIDSK_OK;
 }
@@ -208,7 +210,9 @@ extern "C" int tridsk_grid_from_values(tridsk_ctx* ctx, const float* values, int
     int rc = new_grid(ctx, n_types, origin, dims, spacing, &g);
     if (rc) return rc;
     cudaError_t e = cudaMemcpyAsync(g->g, values, sizeof(float) * g->d.plane * n_types, cudaMemcpyDefault, ctx->stream);
+    if (e == cudaSuccess) e = launch_grid_pack(ctx->stream, g->d, g->gp);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    ctx->launches += 1;
     if (e != cudaSuccess) { tridsk_free_grid(g); return fail(ctx, TRIDSK_ECUDA, std::string("grid copy: ") + cudaGetErrorString(e)); }
     *out = g;
     return TRIDSK_OK;
@@ -224,6 +228,7 @@ extern "C" int tridsk_grid_export(tridsk_ctx* ctx, const tridsk_grid* grid, floa
 extern "C" void tridsk_free_grid(tridsk_grid* g) {
     if (!g) return;
     if (g->g) cudaFree(g->g);       // cudaFree waits for the device; g->ctx may already be destroyed
+    if (g->gp) cudaFree(g->gp);
     delete g;
 }
 
@@ -234,6 +239,8 @@ struct PackedLig {
     std::vector<int> ai;
     std::vector<FragRec> fr;
     std::vector<PairRound> rounds;
+    std::vector<uint2> lane_pairs;      // lane format: grouped by first atom a < b (internal indices)
+    std::vector<int> lane_pstart;
     int err = 0;
     const char* msg = "";
 };
@@ -302,6 +309,8 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
         memset(&r, 0, sizeof(r));
         r.ux = 1.f;
         r.parent = parent[f]; r.depth = depth[f]; r.lo = lo[f]; r.hi = lo[f] + sub[f];
+        r.own_hi = lo[f] + count[f];
+        if (f > 0) r.axis = newidx[ta[f - 1]] | (newidx[tb[f - 1]] << 8);
         if (f > 0) {
             const float* A = ref + 3 * ta[f - 1];
             const float* B = ref + 3 * tb[f - 1];
@@ -353,6 +362,22 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
         }
     }
     h.n_pairs = P;
+    // lane format: per first atom a the partners b > a, with the pair's operands {donor/acceptor flag, d_vdw}
+    out.lane_pstart.assign(n + 1, 0);
+    out.lane_pairs.reserve(P);
+    for (int x = 0; x < n; ++x) {
+        out.lane_pstart[x] = (int)out.lane_pairs.size();
+        for (int y = x + 1; y < n; ++y) {
+            if (!pm[(size_t)x * n + y]) continue;
+            const unsigned char rs = types->hb_role[out.ai[x] & 0xff], rt = types->hb_role[out.ai[y] & 0xff];
+            const unsigned hbf = (((rs & 1) && (rt & 2)) || ((rs & 2) && (rt & 1))) ? 1u : 0u;
+            const float dvdw = out.f4[x].w + out.f4[y].w;         // same fp32 sum the warp kernel forms
+            unsigned bits;
+            memcpy(&bits, &dvdw, sizeof(bits));
+            out.lane_pairs.push_back(make_uint2((unsigned)y | (hbf << 8), bits));
+        }
+    }
+    out.lane_pstart[n] = (int)out.lane_pairs.size();
     // conflict-free schedule: round (j1, j2, k): lane l <-> pair (j1*S + l, j2*S + (l+k) mod S)
     auto hb = [&](int x, int y) {
         const unsigned char rs = types->hb_role[out.ai[x] & 0xff], rt = types->hb_role[out.ai[y] & 0xff];
@@ -399,12 +424,13 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     tridsk_ligands* lg = new (std::nothrow) tridsk_ligands();
     if (!lg) return fail(ctx, TRIDSK_ENOMEM, "host alloc");
     lg->ctx = ctx; lg->n_lig = L;
-    size_t na = 0, nf = 0, nr = 0;
+    size_t na = 0, nf = 0, nr = 0, nlp = 0, nps = 0;
     lg->hdr_h.resize(L); lg->n_pairs.resize(L);
     for (int i = 0; i < L; ++i) {
         LigHdr& h = pk[i].h;
-        h.atom_off = (int)na; h.frag_off = (int)nf; h.round_off = (int)nr;
+        h.atom_off = (int)na; h.frag_off = (int)nf; h.round_off = (int)nr; h.lp_off = (int)nlp; h.ps_off = (int)nps;
         na += pk[i].f4.size(); nf += pk[i].fr.size(); nr += pk[i].rounds.size();
+        nlp += pk[i].lane_pairs.size(); nps += pk[i].lane_pstart.size();
         lg->hdr_h[i] = h; lg->n_pairs[i] = h.n_pairs;
         lg->max_atoms = std::max(lg->max_atoms, h.n); lg->max_tor = std::max(lg->max_tor, h.T);
         lg->bucket[h.J].push_back(i);
@@ -413,8 +439,12 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     std::vector<int> ai(na);
     std::vector<FragRec> fr(nf);
     std::vector<PairRound> rd(std::max<size_t>(nr, 1));
+    std::vector<uint2> lp(std::max<size_t>(nlp, 1));
+    std::vector<int> ps(std::max<size_t>(nps, 1));
     for (int i = 0; i < L; ++i) {
         const LigHdr& h = pk[i].h;
+        std::copy(pk[i].lane_pairs.begin(), pk[i].lane_pairs.end(), lp.begin() + h.lp_off);
+        std::copy(pk[i].lane_pstart.begin(), pk[i].lane_pstart.end(), ps.begin() + h.ps_off);
         std::copy(pk[i].f4.begin(), pk[i].f4.end(), f4.begin() + h.atom_off);
         std::copy(pk[i].ai.begin(), pk[i].ai.end(), ai.begin() + h.atom_off);
         std::copy(pk[i].fr.begin(), pk[i].fr.end(), fr.begin() + h.frag_off);
@@ -431,6 +461,9 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     up((void**)&lg->atom_i, ai.data(), sizeof(int) * na);
     up((void**)&lg->frags, fr.data(), sizeof(FragRec) * nf);
     up((void**)&lg->rounds, rd.data(), sizeof(PairRound) * rd.size());
+    up((void**)&lg->lane_pairs, lp.data(), sizeof(uint2) * lp.size());
+    up((void**)&lg->lane_pstart, ps.data(), sizeof(int) * ps.size());
+    if (e == cudaSuccess) e = cudaMalloc((void**)&lg->all_ids, sizeof(int) * std::max(L, 1));
     for (int j = 1; j <= TRIDSK_MAX_J; ++j)
         if (!lg->bucket[j].empty()) up((void**)&lg->bucket_dev[j], lg->bucket[j].data(), sizeof(int) * lg->bucket[j].size());
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
@@ -454,6 +487,7 @@ extern "C" int tridsk_ligand_info(const tridsk_ligands* l, int* n_lig, int* max_
 extern "C" void tridsk_free_ligands(tridsk_ligands* l) {
     if (!l) return;                 // cudaFree waits for the device; l->ctx may already be destroyed
     cudaFree(l->hdr); cudaFree(l->atom_f4); cudaFree(l->atom_i); cudaFree(l->frags); cudaFree(l->rounds);
+    cudaFree(l->lane_pairs); cudaFree(l->lane_pstart); cudaFree(l->all_ids);
     for (int j = 0; j <= TRIDSK_MAX_J; ++j) if (l->bucket_dev[j]) cudaFree(l->bucket_dev[j]);
     delete l;
 }
@@ -475,7 +509,9 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
     for (int i = 0; i < n_pose; ++i)
         if (li[i] < 0 || li[i] >= ligs->n_lig) return fail(ctx, TRIDSK_EINVAL, "lig_index out of range");
     ScoreLaunch a;
+    memset(&a, 0, sizeof(a));
     a.hdr = ligs->hdr; a.atom_f4 = ligs->atom_f4; a.atom_i = ligs->atom_i; a.frags = ligs->frags; a.rounds = ligs->rounds;
+    a.lane_pairs = ligs->lane_pairs; a.lane_pstart = ligs->lane_pstart;
     a.grid = grid->d;
     to_dparams(params, &a.P);
     a.n_pose = n_pose; a.pose_stride = pose_stride; a.grad_stride = grad_stride; a.coord_stride = coord_stride;
@@ -499,17 +535,95 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
     a.energy = h_e ? (float*)ob : energy;
     a.grad = grad ? (h_g ? (float*)(ob + o_g) : grad) : nullptr;
     a.coords = coords ? (h_c ? (float*)(ob + o_c) : coords) : nullptr;
-    CK(launch_score(ctx->stream, a));
+    std::vector<int> seg;                                   // lane form: [seg_lig | seg_start | seg_cnt | perm]
+    if (ctx->kernel == 2) {
+        // one lane per pose, one 32-lane CTA per run of <= 32 poses of the same ligand
+        std::vector<int> perm(n_pose);
+        for (int i = 0; i < n_pose; ++i) perm[i] = i;
+        std::stable_sort(perm.begin(), perm.end(), [&](int x, int y) { return li[x] < li[y]; });
+        std::vector<int> s_lig, s_start, s_cnt;
+        size_t smem = 0;
+        for (int i = 0; i < n_pose;) {
+            int j = i;
+            while (j < n_pose && j - i < 32 && li[perm[j]] == li[perm[i]]) ++j;
+            s_lig.push_back(li[perm[i]]); s_start.push_back(i); s_cnt.push_back(j - i);
+            const LigHdr& h = ligs->hdr_h[li[perm[i]]];
+            smem = std::max(smem, lane_topo_bytes(h.n, h.T, h.n_pairs) + 128 * (size_t)(3 * h.n + lane_fslots(h.n, h.T) + h.T));
+            i = j;
+        }
+        if (smem > TRIDSK_SMEM_MAX_CTA) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");
+        const int ns = (int)s_lig.size();
+        seg.insert(seg.end(), s_lig.begin(), s_lig.end());
+        seg.insert(seg.end(), s_start.begin(), s_start.end());
+        seg.insert(seg.end(), s_cnt.begin(), s_cnt.end());
+        seg.insert(seg.end(), perm.begin(), perm.end());
+        int* d_seg;
+        { int rc = scratch(ctx, 5, sizeof(int) * seg.size(), (void**)&d_seg); if (rc) return rc; }
+        CK(cudaMemcpyAsync(d_seg, seg.data(), sizeof(int) * seg.size(), cudaMemcpyHostToDevice, ctx->stream));
+        a.seg_lig = d_seg; a.seg_start = d_seg + ns; a.seg_cnt = d_seg + 2 * ns; a.perm = d_seg + 3 * ns;
+        CK(launch_score_lane(ctx->stream, a, ns, smem));
+    } else {
+        CK(launch_score(ctx->stream, a));
+    }
     ctx->launches += 1;
     if (h_e) CK(cudaMemcpyAsync(energy, a.energy, b_e, cudaMemcpyDeviceToHost, ctx->stream));
     if (h_g) CK(cudaMemcpyAsync(grad, a.grad, b_g, cudaMemcpyDeviceToHost, ctx->stream));
     if (h_c) CK(cudaMemcpyAsync(coords, a.coords, b_c, cudaMemcpyDeviceToHost, ctx->stream));
     // li (host vector) was consumed by an async copy: always drain before it goes out of scope
-    if (h_e || h_g || h_c || h_li) CK(cudaStreamSynchronize(ctx->stream));
+    if (h_e || h_g || h_c || h_li || !seg.empty()) CK(cudaStreamSynchronize(ctx->stream));
     return TRIDSK_OK;
 }
 
 // ---------------------------------------------------------------------------------------- dock
+// Lane-per-chain launch plan: a ligand's CTA needs topology + chains_per_cta * chain_slots * 4 bytes of shared memory;
+// for every ligand pick the (chains per CTA, resident CTAs per SM) that keeps the most warps resident, and give each
+// such class one launch whose dynamic shared memory is that class's share of the SM.
+static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_refine) {
+    const long long key = ((long long)n_chains << 8) | (n_refine > 1 ? 1 : 0);
+    if (lg->lane_plan_key == key) return TRIDSK_OK;
+    const int L = lg->n_lig;
+    const int cmax = std::min(128, (n_chains + 31) / 32 * 32);
+    std::vector<std::pair<int, int>> cls(L);                 // (class = C << 8 | resident CTAs, ligand)
+    for (int i = 0; i < L; ++i) {
+        const LigHdr& h = lg->hdr_h[i];
+        const size_t topo = lane_topo_bytes(h.n, h.T, h.n_pairs);
+        const size_t per_chain = 4 * (size_t)lane_chain_slots(h.n, h.T, n_refine);
+        int best_c = 0, best_r = 0, best_w = -1;
+        for (int c = cmax; c >= 32; c -= 32) {
+            const size_t need = topo + per_chain * c;
+            if (need > TRIDSK_SMEM_MAX_CTA) continue;
+            int r = (int)(TRIDSK_SMEM_PER_SM / (need + TRIDSK_SMEM_RESERVED));
+            r = std::min(r, 16);
+            const int w = std::min(r * c / 32, 24);             // beyond ~24 warps the register file is the limit
+            if (w > best_w) { best_w = w; best_c = c; best_r = r; }
+        }
+        if (best_w < 0) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");
+        cls[i] = {(best_c << 8) | best_r, i};
+    }
+    std::sort(cls.begin(), cls.end());
+    lg->lane_ids_h.resize(L);
+    lg->lane_plan.clear();
+    for (int i = 0; i < L; ++i) {
+        lg->lane_ids_h[i] = cls[i].second;
+        if (i == 0 || cls[i].first != cls[i - 1].first) {
+            const int c = cls[i].first >> 8, r = cls[i].first & 0xff;
+            const size_t smem = std::min<size_t>(TRIDSK_SMEM_PER_SM / r - TRIDSK_SMEM_RESERVED, TRIDSK_SMEM_MAX_CTA) / 16 * 16;
+            lg->lane_plan.push_back({c, smem, i, 0});
+        }
+        lg->lane_plan.back().count++;
+    }
+    CK(cudaStreamSynchronize(ctx->stream));                  // an earlier dock may still read all_ids
+    CK(cudaMemcpyAsync(lg->all_ids, lg->lane_ids_h.data(), sizeof(int) * L, cudaMemcpyHostToDevice, ctx->stream));
+    lg->lane_plan_key = key;
+    return TRIDSK_OK;
+}
+
+extern "C" int tridsk_set_kernel(tridsk_ctx* ctx, int kernel) {
+    if (!ctx || kernel < 0 || kernel > 2) return fail(ctx, TRIDSK_EINVAL, "kernel must be 0 (auto), 1 (warp per chain) or 2 (lane per chain)");
+    ctx->kernel = kernel;
+    return TRIDSK_OK;
+}
+
 extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* ligs, const tridsk_params* params,
                            const float box_min[3], const float box_max[3], const float pocket_center[3], float pocket_radius,
                            int n_chains, int n_steps, int top_k, unsigned long long seed, int pose_stride,
@@ -557,6 +671,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     McLaunch base;
     memset(&base, 0, sizeof(base));
     base.hdr = ligs->hdr; base.atom_f4 = ligs->atom_f4; base.atom_i = ligs->atom_i; base.frags = ligs->frags; base.rounds = ligs->rounds;
+    base.lane_pairs = ligs->lane_pairs; base.lane_pstart = ligs->lane_pstart;
     base.grid = grid->d;
     to_dparams(params, &base.P);
     for (int c = 0; c < 3; ++c) { base.box_min[c] = box_min[c]; base.box_max[c] = box_max[c]; base.centre[c] = pocket_center[c]; }
@@ -566,20 +681,40 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     base.pose_cur = state; base.pose_best = state + n_pose_f; base.e_cur = state + 2 * n_pose_f; base.e_best = state + 2 * n_pose_f + nch;
     base.trace = d_trace; base.trace_stride = n_steps;
 
-    // launch series: per steps_per_launch slice, one launch per atoms-per-lane bucket J; then top-k
-    std::vector<std::pair<int, McLaunch>> series;
+    // Mapping: a warp per chain when chains are few (latency), a lane per chain when they outnumber the machine's
+    // lanes several times over (throughput).  tridsk_set_kernel overrides.
+    const bool lane = ctx->kernel == 2 || (ctx->kernel == 0 && nch >= (size_t)ctx->sm_count * 32 * 8);
+    ctx->last_kernel = lane ? 2 : 1;
+    tridsk_ligands* lg = const_cast<tridsk_ligands*>(ligs);
+    if (lane) { int rc = lane_plan(ctx, lg, n_chains, params->n_refine); if (rc) return rc; }
+
+    // launch series: per steps_per_launch slice, one launch per bucket (atoms per lane J, or shared-memory class); then top-k
+    struct Item { int kind, arg; size_t smem; McLaunch a; };
+    std::vector<Item> series;
     const int spl = (o.steps_per_launch > 0) ? o.steps_per_launch : std::max(n_steps, 1);
     int done = 0;
     bool first = true;
     do {
         const int ns = std::min(spl, n_steps - done);
-        for (int j = 1; j <= TRIDSK_MAX_J; ++j) {
-            if (ligs->bucket[j].empty()) continue;
-            McLaunch a = base;
-            a.lig_list = ligs->bucket_dev[j]; a.n_list = (int)ligs->bucket[j].size();
+        auto fill = [&](McLaunch& a) {
             a.first_step = o.first_step + done; a.n_steps = ns; a.trace_off = done;
             a.init_mode = first ? (o.resume ? 2 : (o.init_poses ? 1 : 0)) : 2;
-            series.push_back({j, a});
+        };
+        if (lane) {
+            for (const auto& b : lg->lane_plan) {
+                McLaunch a = base;
+                a.lig_list = lg->all_ids + b.first; a.n_list = b.count;
+                fill(a);
+                series.push_back({2, b.chains_per_cta, b.smem, a});
+            }
+        } else {
+            for (int j = 1; j <= TRIDSK_MAX_J; ++j) {
+                if (ligs->bucket[j].empty()) continue;
+                McLaunch a = base;
+                a.lig_list = ligs->bucket_dev[j]; a.n_list = (int)ligs->bucket[j].size();
+                fill(a);
+                series.push_back({1, j, 0, a});
+            }
         }
         done += ns; first = false;
     } while (done < n_steps);
@@ -600,7 +735,10 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         const unsigned fl = capturing ? cudaEventRecordExternal : cudaEventRecordDefault;
         cudaError_t e = cudaEventRecordWithFlags(ctx->ev[0], s, fl);
         if (e != cudaSuccess) return e;
-        for (auto& it : series) { e = launch_mc(s, it.first, it.second); if (e != cudaSuccess) return e; }
+        for (auto& it : series) {
+            e = it.kind == 2 ? launch_mc_lane(s, it.a, it.arg, it.smem) : launch_mc(s, it.arg, it.a);
+            if (e != cudaSuccess) return e;
+        }
         e = cudaEventRecordWithFlags(ctx->ev[1], s, fl);
         if (e != cudaSuccess) return e;
         if (top_k > 0) { e = launch_topk(s, tk); if (e != cudaSuccess) return e; }
@@ -612,8 +750,9 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         // a10: the whole series as one CUDA graph; re-used while the launch parameters are byte-identical
         std::vector<unsigned char> key;
         for (auto& it : series) {
-            key.insert(key.end(), (unsigned char*)&it.first, (unsigned char*)&it.first + sizeof(int));
-            key.insert(key.end(), (unsigned char*)&it.second, (unsigned char*)&it.second + sizeof(McLaunch));
+            const long long hd[3] = {it.kind, it.arg, (long long)it.smem};
+            key.insert(key.end(), (const unsigned char*)hd, (const unsigned char*)hd + sizeof(hd));
+            key.insert(key.end(), (unsigned char*)&it.a, (unsigned char*)&it.a + sizeof(McLaunch));
         }
         key.insert(key.end(), (unsigned char*)&tk, (unsigned char*)&tk + sizeof(tk));
         if (!ctx->graph_exec || key != ctx->graph_key) {

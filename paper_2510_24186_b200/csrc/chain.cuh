@@ -151,6 +151,43 @@ __device__ __forceinline__ float grid_interp(const DGrid& G, float k_wall, int t
     return e;
 }
 
+// The same interpolant read from the xy-packed copy of the grid (DGrid::gp): the 8 corners of a cell are two
+// aligned 16-byte records (z and z+1), i.e. 2 load instructions and 2 cache lines per atom instead of 8 and 4.
+// Arithmetic and operation order are those of grid_interp, so both give bit-identical results.
+template <bool GRAD>
+__device__ __forceinline__ float grid_interp_packed(const DGrid& G, float k_wall, int type, float x, float y, float z,
+                                                    float& gx, float& gy, float& gz) {
+    const float ux = (x - G.ox) * G.inv_h, uy = (y - G.oy) * G.inv_h, uz = (z - G.oz) * G.inv_h;
+    const float cx = fminf(fmaxf(ux, 0.f), (float)(G.nx - 1));
+    const float cy = fminf(fmaxf(uy, 0.f), (float)(G.ny - 1));
+    const float cz = fminf(fmaxf(uz, 0.f), (float)(G.nz - 1));
+    const int ix = min((int)cx, G.nx - 2), iy = min((int)cy, G.ny - 2), iz = min((int)cz, G.nz - 2);
+    const float fx = cx - (float)ix, fy = cy - (float)iy, fz = cz - (float)iz;
+    const float4* p = G.gp + (size_t)type * G.plane + ((size_t)iz * G.ny + iy) * G.nx + ix;
+    const float4 lo = __ldg(p), hi = __ldg(p + (size_t)G.nx * G.ny);
+    const float v000 = lo.x, v001 = lo.y, v010 = lo.z, v011 = lo.w, v100 = hi.x, v101 = hi.y, v110 = hi.z, v111 = hi.w;
+    const float d00 = v001 - v000, d01 = v011 - v010, d10 = v101 - v100, d11 = v111 - v110;
+    const float a00 = fmaf(fx, d00, v000), a01 = fmaf(fx, d01, v010), a10 = fmaf(fx, d10, v100), a11 = fmaf(fx, d11, v110);
+    const float e0 = a01 - a00, e1 = a11 - a10;
+    const float b0 = fmaf(fy, e0, a00), b1 = fmaf(fy, e1, a10);
+    float e = fmaf(fz, b1 - b0, b0);
+    const bool clx = (cx != ux), cly = (cy != uy), clz = (cz != uz);
+    float wx = 0.f, wy = 0.f, wz = 0.f;
+    if (clx | cly | clz) {
+        wx = clx ? x - (G.ox + cx * G.h) : 0.f;
+        wy = cly ? y - (G.oy + cy * G.h) : 0.f;
+        wz = clz ? z - (G.oz + cz * G.h) : 0.f;
+        e += k_wall * (wx * wx + wy * wy + wz * wz);
+    }
+    if (GRAD) {
+        const float dx0 = fmaf(fy, d01 - d00, d00), dx1 = fmaf(fy, d11 - d10, d10);
+        gx = (clx ? 0.f : fmaf(fz, dx1 - dx0, dx0) * G.inv_h) + 2.f * k_wall * wx;
+        gy = (cly ? 0.f : fmaf(fz, e1 - e0, e0) * G.inv_h) + 2.f * k_wall * wy;
+        gz = (clz ? 0.f : (b1 - b0) * G.inv_h) + 2.f * k_wall * wz;
+    }
+    return e;
+}
+
 // ------------------------------------------------------------------ O2: pair function e(s,t,d) and (de/dd)/d
 // L = -[d<dmax] exp(-(d-dvdw-mu)^2/(2 sigma^2)) (sign G1); C = -[d<dc] ln(max(d,floor)/dc), dc = 2.6 for
 // donor/acceptor pairs else dvdw (G3, G4); H = -[hb, d<3.4] exp(-(d-2.88)^2/(2*0.3^2)).

@@ -5,6 +5,8 @@
 // change), receptor atoms are staged through shared memory in chunks and read as warp broadcasts, and each
 // type plane is written with unit-stride stores along x.  Receptor atoms are visited in input order, so the
 // fp32 sums are reproducible.  The bound is the XU/FP32 pipes (one ex2 per node-atom-type triple), not memory.
+#include <algorithm>
+
 #include "internal.h"
 
 #define GB_BX 32
@@ -85,5 +87,26 @@ cudaError_t launch_grid_build(cudaStream_t s, const float4* rec, int n_rec, cons
     if (n_types <= 8) grid_build_kernel<8><<<g, block, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, out);
     else if (n_types <= 16) grid_build_kernel<16><<<g, block, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, out);
     else grid_build_kernel<32><<<g, block, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, out);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ xy-packed copy of the grid (DGrid::gp)
+// gp[t][z][y][x] = {g(x,y), g(x+1,y), g(x,y+1), g(x+1,y+1)} at the same (t, z); indices clamped at the upper
+// edges (those records are never the base of a cell: i0 <= n - 2).  The 8 corners of a trilinear cell are then two
+// aligned 16-byte records, which is what the chain kernels gather.
+__global__ void __launch_bounds__(256) grid_pack_kernel(const DGrid G, float4* __restrict__ out) {
+    const size_t total = G.plane * (size_t)G.n_types;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int x = (int)(i % G.nx), y = (int)((i / G.nx) % G.ny);
+        const int dx = (x + 1 < G.nx) ? 1 : 0;
+        const size_t dy = (y + 1 < G.ny) ? (size_t)G.nx : 0;
+        out[i] = make_float4(G.g[i], G.g[i + dx], G.g[i + dy], G.g[i + dy + dx]);
+    }
+}
+
+cudaError_t launch_grid_pack(cudaStream_t s, DGrid grid, float4* out) {
+    const size_t total = grid.plane * (size_t)grid.n_types;
+    const int blocks = (int)std::min<size_t>((total + 255) / 256, 148 * 16);
+    grid_pack_kernel<<<blocks, 256, 0, s>>>(grid, out);
     return cudaGetLastError();
 }

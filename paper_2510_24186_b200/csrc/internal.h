@@ -28,6 +28,7 @@ struct DParams {
 // Receptor grid: fp32 planes [type][z][y][x] (x fastest).
 struct DGrid {
     const float* g;
+    const float4* gp;             // xy-packed copy: gp[t][z][y][x] = {g(x,y), g(x+1,y), g(x,y+1), g(x+1,y+1)} (edges clamped)
     int nx, ny, nz, n_types;
     size_t plane;                 // nx*ny*nz
     float ox, oy, oz, h, inv_h;
@@ -44,13 +45,17 @@ struct LigHdr {
     int max_depth;
     int tile_off[TRIDSK_MAX_TILES + 1];   // round ranges per (j1<=j2) tile, relative to round_off
     int n_pairs;
-    int pad[4];
+    int lp_off;                   // lane format: into lane_pairs (n_pairs records, grouped by first atom)
+    int ps_off;                   // lane format: into lane_pstart (n + 1 entries)
+    int pad[2];
 };
 
 // Per-fragment record; fragment 0 is the root, fragment k+1 hangs off torsion k.
 struct FragRec {
     float ux, uy, uz, ox;         // axis unit vector and axis point (atom b_k), reference frame
-    float oy, oz, pad0, pad1;
+    float oy, oz;
+    int own_hi;                   // the fragment's own atoms are [lo, own_hi) (internal order)
+    int axis;                     // internal indices of the axis atoms: a_k | b_k << 8 (0 for the root)
     int parent, depth, lo, hi;    // parent fragment, depth (root = 0), subtree atom range [lo, hi)
 };
 
@@ -68,7 +73,9 @@ struct McLaunch {
     const int* atom_i;            // type | frag << 8 | original index << 16
     const FragRec* frags;
     const PairRound* rounds;
-    const int* lig_list;          // ligands handled by this launch (one J bucket)
+    const uint2* lane_pairs;      // lane format: {b | hb << 8, d_vdw bits}, grouped by first atom a < b
+    const int* lane_pstart;       // lane format: per ligand n + 1 offsets into its lane_pairs
+    const int* lig_list;          // ligands handled by this launch (one bucket)
     int n_list;
     DGrid grid;
     DParams P;
@@ -93,6 +100,12 @@ struct ScoreLaunch {
     const int* atom_i;
     const FragRec* frags;
     const PairRound* rounds;
+    const uint2* lane_pairs;
+    const int* lane_pstart;
+    const int* seg_lig;           // lane score kernel: per CTA the ligand, and its poses perm[seg_start .. seg_start + seg_cnt)
+    const int* seg_start;
+    const int* seg_cnt;
+    const int* perm;
     DGrid grid;
     DParams P;
     const int* lig_index;
@@ -111,6 +124,22 @@ struct TopkLaunch {
     float* out_energy; float* out_pose; int* out_chain;
 };
 
+// ---------------------------------------------------------------- lane-per-chain kernel: shared-memory budget
+// One CTA = chains_per_cta chains of ONE ligand.  Shared memory = the ligand's topology (staged once per CTA)
+// + per chain: coordinates X[3n], forces F[max(3n, 12(T+1))] (the fragment frames of the forward pass alias F),
+// current and proposed torsions [2T], and the torsion Adam moments [2T] when n_refine > 1.
+#define TRIDSK_SMEM_PER_SM 233472      // 228 KB
+#define TRIDSK_SMEM_RESERVED 1024      // per resident CTA
+#define TRIDSK_SMEM_MAX_CTA 232448     // 227 KB opt-in maximum per CTA
+__host__ __device__ static inline size_t lane_topo_bytes(int n, int T, int P) {
+    const size_t b = 16 * (size_t)n + sizeof(FragRec) * (size_t)(T + 1) + 8 * (size_t)P + 4 * (size_t)(n + 1);
+    return (b + 15) / 16 * 16;
+}
+__host__ __device__ static inline int lane_fslots(int n, int T) { return 3 * n > 12 * (T + 1) ? 3 * n : 12 * (T + 1); }
+__host__ __device__ static inline int lane_chain_slots(int n, int T, int n_refine) {
+    return 3 * n + lane_fslots(n, T) + 2 * T + (n_refine > 1 ? 2 * T : 0);
+}
+
 // ---------------------------------------------------------------- host-side handles
 struct tridsk_ctx {
     int device = 0;
@@ -128,11 +157,14 @@ struct tridsk_ctx {
     int graph_launches = 0;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // dock: before MC series, after MC series, after top-k
     bool ev_valid = false;
+    int kernel = 0;               // tridsk_set_kernel: 0 auto, 1 warp per chain, 2 lane per chain
+    int last_kernel = 0;          // what the last dock used
 };
 
 struct tridsk_grid {
     tridsk_ctx* ctx;
     float* g = nullptr;
+    float4* gp = nullptr;
     DGrid d;
 };
 
@@ -147,6 +179,13 @@ struct tridsk_ligands {
     int* atom_i = nullptr;
     FragRec* frags = nullptr;
     PairRound* rounds = nullptr;
+    uint2* lane_pairs = nullptr;
+    int* lane_pstart = nullptr;
+    int* all_ids = nullptr;       // 0..n_lig-1 re-ordered per lane bucket (refilled when the plan key changes)
+    struct LaneBucket { int chains_per_cta; size_t smem; int first, count; };
+    std::vector<LaneBucket> lane_plan;
+    std::vector<int> lane_ids_h;  // host copy behind all_ids (must outlive the async upload)
+    long long lane_plan_key = -1; // n_chains << 8 | (n_refine > 1)
     int* bucket_dev[TRIDSK_MAX_J + 1] = {nullptr, nullptr, nullptr, nullptr, nullptr};
 };
 
@@ -154,7 +193,11 @@ struct tridsk_ligands {
 cudaError_t launch_grid_build(cudaStream_t s, const float4* rec /* x,y,z,type */, int n_rec,
                               const float* pair_tab /* [n_types][n_types][4] */, int n_types,
                               const DParams& P, DGrid grid, float dc_max, float* out);
+cudaError_t launch_grid_pack(cudaStream_t s, DGrid grid, float4* out);
 cudaError_t launch_mc(cudaStream_t s, int J, const McLaunch& a);
+cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta, size_t smem_bytes);
+cudaError_t launch_score_lane(cudaStream_t s, const ScoreLaunch& a, int n_seg, size_t smem_bytes);
+cudaError_t mc_lane_prepare(size_t max_smem_bytes);
 cudaError_t launch_score(cudaStream_t s, const ScoreLaunch& a);
 cudaError_t launch_topk(cudaStream_t s, const TopkLaunch& a);
 cudaError_t launch_philox_debug(cudaStream_t s, const unsigned int* ctr_key /* dev[6] */, unsigned int* out /* dev[4] */);
