@@ -3,6 +3,7 @@
 // No arithmetic of the method runs on the host: every step of the path is in the kernels.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -105,6 +106,11 @@ extern "C" void tridsk_destroy(tridsk_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
     for (int i = 0; i < 3; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    if (ctx->fork_ev) cudaEventDestroy(ctx->fork_ev);
+    for (int i = 0; i < TRIDSK_BRANCHES; ++i) {
+        if (ctx->join_ev[i]) cudaEventDestroy(ctx->join_ev[i]);
+        if (ctx->side[i]) cudaStreamDestroy(ctx->side[i]);
+    }
     for (int i = 0; i < 8; ++i) if (ctx->scratch[i]) cudaFree(ctx->scratch[i]);
     if (ctx->own_stream) cudaStreamDestroy(ctx->stream);
     delete ctx;
@@ -239,8 +245,8 @@ struct PackedLig {
     std::vector<int> ai;
     std::vector<FragRec> fr;
     std::vector<PairRound> rounds;
-    std::vector<uint2> lane_pairs;      // lane format: grouped by first atom a < b (internal indices)
-    std::vector<int> lane_pstart;
+    std::vector<LaneFrag> lane_frags;   // lane format (internal.h): fragments in pre-order
+    std::vector<uint2> lane_stream;     // lane format: the pair instruction stream
     int err = 0;
     const char* msg = "";
 };
@@ -362,22 +368,67 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
         }
     }
     h.n_pairs = P;
-    // lane format: per first atom a the partners b > a, with the pair's operands {donor/acceptor flag, d_vdw}
-    out.lane_pstart.assign(n + 1, 0);
-    out.lane_pairs.reserve(P);
-    for (int x = 0; x < n; ++x) {
-        out.lane_pstart[x] = (int)out.lane_pairs.size();
-        for (int y = x + 1; y < n; ++y) {
-            if (!pm[(size_t)x * n + y]) continue;
-            const unsigned char rs = types->hb_role[out.ai[x] & 0xff], rt = types->hb_role[out.ai[y] & 0xff];
-            const unsigned hbf = (((rs & 1) && (rt & 2)) || ((rs & 2) && (rt & 1))) ? 1u : 0u;
-            const float dvdw = out.f4[x].w + out.f4[y].w;         // same fp32 sum the warp kernel forms
-            unsigned bits;
-            memcpy(&bits, &dvdw, sizeof(bits));
-            out.lane_pairs.push_back(make_uint2((unsigned)y | (hbf << 8), bits));
+    // lane format (internal.h): fragments in depth-first pre-order, pairs as a stream of (tile x partner-run) blocks
+    {
+        std::vector<int> pre(T + 1);
+        for (int g = 0; g <= T; ++g) pre[order[g]] = g;
+        out.lane_frags.resize(T + 1);
+        for (int g = 0; g <= T; ++g) {
+            const int f = order[g];
+            const FragRec& r = out.fr[f];
+            LaneFrag& q = out.lane_frags[g];
+            q.ux = r.ux; q.uy = r.uy; q.uz = r.uz; q.ox = r.ox; q.oy = r.oy; q.oz = r.oz;
+            q.lo = r.lo; q.own_hi = r.own_hi; q.parent = f > 0 ? pre[parent[f]] : 0; q.depth = depth[f];
+            q.axis = r.axis; q.tor = f - 1;
         }
+        auto hbp = [&](int x, int y) {
+            const unsigned char rs = types->hb_role[out.ai[x] & 0xff], rt = types->hb_role[out.ai[y] & 0xff];
+            return ((rs & 1) && (rt & 2)) || ((rs & 2) && (rt & 1));
+        };
+        std::vector<int> gof(n);                 // pre-order fragment of an internal atom
+        for (int g = 0; g <= T; ++g) for (int a = out.lane_frags[g].lo; a < out.lane_frags[g].own_hi; ++a) gof[a] = g;
+        int covered2 = 0;
+        for (int g = 0; g <= T; ++g) {
+            const int lo_g = out.lane_frags[g].lo, cnt = out.lane_frags[g].own_hi - lo_g;
+            const size_t hdr_at = out.lane_stream.size();
+            out.lane_stream.push_back(make_uint2(0u, 0u));
+            const int nt = (cnt + 3) / 4;
+            unsigned n_tiles = 0;
+            for (int tl = 0, a0 = lo_g; tl < nt; ++tl) {
+                const int w = cnt / nt + (tl < cnt % nt ? 1 : 0);
+                const size_t tile_at = out.lane_stream.size();
+                out.lane_stream.push_back(make_uint2((unsigned)a0 | ((unsigned)w << 8), 0u));
+                unsigned n_runs = 0;
+                for (int fb = g; fb <= T; ++fb) {
+                    const size_t run_at = out.lane_stream.size();
+                    out.lane_stream.push_back(make_uint2((unsigned)fb, 0u));
+                    unsigned nb = 0;
+                    for (int y = out.lane_frags[fb].lo; y < out.lane_frags[fb].own_hi; ++y) {
+                        unsigned excl = (0xfu << w) & 0xfu, hbm = 0, any = 0;   // lanes beyond the tile width never pair
+                        for (int i = 0; i < w; ++i) {
+                            const int x = a0 + i;
+                            if (x < y && pm[(size_t)x * n + y]) { any = 1; ++covered2; if (hbp(x, y)) hbm |= 1u << i; }
+                            else excl |= 1u << i;
+                        }
+                        if (!any) continue;
+                        unsigned bits;
+                        memcpy(&bits, &out.f4[y].w, sizeof(bits));
+                        out.lane_stream.push_back(make_uint2((unsigned)y | (excl << 8) | (hbm << 12), bits));
+                        ++nb;
+                    }
+                    if (nb) { out.lane_stream[run_at].y = nb; ++n_runs; }
+                    else out.lane_stream.pop_back();
+                }
+                if (n_runs) { out.lane_stream[tile_at].y = n_runs; ++n_tiles; }
+                else out.lane_stream.pop_back();
+                a0 += w;
+            }
+            out.lane_stream[hdr_at].x = n_tiles;
+        }
+        (void)gof;
+        if (covered2 != P) return bad(TRIDSK_EINVAL, "internal: lane pair stream does not cover the pair set");
+        h.ls_len = (int)out.lane_stream.size();
     }
-    out.lane_pstart[n] = (int)out.lane_pairs.size();
     // conflict-free schedule: round (j1, j2, k): lane l <-> pair (j1*S + l, j2*S + (l+k) mod S)
     auto hb = [&](int x, int y) {
         const unsigned char rs = types->hb_role[out.ai[x] & 0xff], rt = types->hb_role[out.ai[y] & 0xff];
@@ -424,13 +475,13 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     tridsk_ligands* lg = new (std::nothrow) tridsk_ligands();
     if (!lg) return fail(ctx, TRIDSK_ENOMEM, "host alloc");
     lg->ctx = ctx; lg->n_lig = L;
-    size_t na = 0, nf = 0, nr = 0, nlp = 0, nps = 0;
+    size_t na = 0, nf = 0, nr = 0, nls = 0;
     lg->hdr_h.resize(L); lg->n_pairs.resize(L);
     for (int i = 0; i < L; ++i) {
         LigHdr& h = pk[i].h;
-        h.atom_off = (int)na; h.frag_off = (int)nf; h.round_off = (int)nr; h.lp_off = (int)nlp; h.ps_off = (int)nps;
+        h.atom_off = (int)na; h.frag_off = (int)nf; h.round_off = (int)nr; h.ls_off = (int)nls;
         na += pk[i].f4.size(); nf += pk[i].fr.size(); nr += pk[i].rounds.size();
-        nlp += pk[i].lane_pairs.size(); nps += pk[i].lane_pstart.size();
+        nls += pk[i].lane_stream.size();
         lg->hdr_h[i] = h; lg->n_pairs[i] = h.n_pairs;
         lg->max_atoms = std::max(lg->max_atoms, h.n); lg->max_tor = std::max(lg->max_tor, h.T);
         lg->bucket[h.J].push_back(i);
@@ -439,12 +490,12 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     std::vector<int> ai(na);
     std::vector<FragRec> fr(nf);
     std::vector<PairRound> rd(std::max<size_t>(nr, 1));
-    std::vector<uint2> lp(std::max<size_t>(nlp, 1));
-    std::vector<int> ps(std::max<size_t>(nps, 1));
+    std::vector<LaneFrag> lf(nf);
+    std::vector<uint2> lsv(std::max<size_t>(nls, 1));
     for (int i = 0; i < L; ++i) {
         const LigHdr& h = pk[i].h;
-        std::copy(pk[i].lane_pairs.begin(), pk[i].lane_pairs.end(), lp.begin() + h.lp_off);
-        std::copy(pk[i].lane_pstart.begin(), pk[i].lane_pstart.end(), ps.begin() + h.ps_off);
+        std::copy(pk[i].lane_frags.begin(), pk[i].lane_frags.end(), lf.begin() + h.frag_off);
+        std::copy(pk[i].lane_stream.begin(), pk[i].lane_stream.end(), lsv.begin() + h.ls_off);
         std::copy(pk[i].f4.begin(), pk[i].f4.end(), f4.begin() + h.atom_off);
         std::copy(pk[i].ai.begin(), pk[i].ai.end(), ai.begin() + h.atom_off);
         std::copy(pk[i].fr.begin(), pk[i].fr.end(), fr.begin() + h.frag_off);
@@ -461,8 +512,8 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     up((void**)&lg->atom_i, ai.data(), sizeof(int) * na);
     up((void**)&lg->frags, fr.data(), sizeof(FragRec) * nf);
     up((void**)&lg->rounds, rd.data(), sizeof(PairRound) * rd.size());
-    up((void**)&lg->lane_pairs, lp.data(), sizeof(uint2) * lp.size());
-    up((void**)&lg->lane_pstart, ps.data(), sizeof(int) * ps.size());
+    up((void**)&lg->lane_frags, lf.data(), sizeof(LaneFrag) * nf);
+    up((void**)&lg->lane_stream, lsv.data(), sizeof(uint2) * lsv.size());
     if (e == cudaSuccess) e = cudaMalloc((void**)&lg->all_ids, sizeof(int) * std::max(L, 1));
     for (int j = 1; j <= TRIDSK_MAX_J; ++j)
         if (!lg->bucket[j].empty()) up((void**)&lg->bucket_dev[j], lg->bucket[j].data(), sizeof(int) * lg->bucket[j].size());
@@ -487,7 +538,7 @@ extern "C" int tridsk_ligand_info(const tridsk_ligands* l, int* n_lig, int* max_
 extern "C" void tridsk_free_ligands(tridsk_ligands* l) {
     if (!l) return;                 // cudaFree waits for the device; l->ctx may already be destroyed
     cudaFree(l->hdr); cudaFree(l->atom_f4); cudaFree(l->atom_i); cudaFree(l->frags); cudaFree(l->rounds);
-    cudaFree(l->lane_pairs); cudaFree(l->lane_pstart); cudaFree(l->all_ids);
+    cudaFree(l->lane_frags); cudaFree(l->lane_stream); cudaFree(l->all_ids);
     for (int j = 0; j <= TRIDSK_MAX_J; ++j) if (l->bucket_dev[j]) cudaFree(l->bucket_dev[j]);
     delete l;
 }
@@ -511,7 +562,7 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
     ScoreLaunch a;
     memset(&a, 0, sizeof(a));
     a.hdr = ligs->hdr; a.atom_f4 = ligs->atom_f4; a.atom_i = ligs->atom_i; a.frags = ligs->frags; a.rounds = ligs->rounds;
-    a.lane_pairs = ligs->lane_pairs; a.lane_pstart = ligs->lane_pstart;
+    a.lane_frags = ligs->lane_frags; a.lane_stream = ligs->lane_stream;
     a.grid = grid->d;
     to_dparams(params, &a.P);
     a.n_pose = n_pose; a.pose_stride = pose_stride; a.grad_stride = grad_stride; a.coord_stride = coord_stride;
@@ -548,7 +599,7 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
             while (j < n_pose && j - i < 32 && li[perm[j]] == li[perm[i]]) ++j;
             s_lig.push_back(li[perm[i]]); s_start.push_back(i); s_cnt.push_back(j - i);
             const LigHdr& h = ligs->hdr_h[li[perm[i]]];
-            smem = std::max(smem, lane_topo_bytes(h.n, h.T, h.n_pairs) + 128 * (size_t)(3 * h.n + lane_fslots(h.n, h.T) + h.T));
+            smem = std::max(smem, lane_topo_bytes(h.n, h.T, h.ls_len) + 128 * (size_t)lane_chain_slots(h.n, h.T, h.max_depth, 1));
             i = j;
         }
         if (smem > TRIDSK_SMEM_MAX_CTA) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");
@@ -575,43 +626,46 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
 }
 
 // ---------------------------------------------------------------------------------------- dock
-// Lane-per-chain launch plan: a ligand's CTA needs topology + chains_per_cta * chain_slots * 4 bytes of shared memory;
-// for every ligand pick the (chains per CTA, resident CTAs per SM) that keeps the most warps resident, and give each
-// such class one launch whose dynamic shared memory is that class's share of the SM.
+// Lane-per-chain launch plan.  A CTA holds C chains of one ligand (C = n_chains rounded up to a warp, at most 128, fewer
+// if a big ligand would not fit) and needs topology + C * chain_slots * 4 bytes of shared memory.  Ligands are grouped
+// by (C, resident CTAs per SM) so that small ligands keep their high occupancy; every group is one launch whose dynamic
+// shared memory is the group's largest need, the groups run concurrently as parallel branches of the CUDA graph, and
+// inside a group the costliest ligands go first (short tail).
 static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_refine) {
     const long long key = ((long long)n_chains << 8) | (n_refine > 1 ? 1 : 0);
     if (lg->lane_plan_key == key) return TRIDSK_OK;
     const int L = lg->n_lig;
     const int cmax = std::min(128, (n_chains + 31) / 32 * 32);
-    std::vector<std::pair<int, int>> cls(L);                 // (class = C << 8 | resident CTAs, ligand)
+    struct Ent { int cls; long long cost; int lig; size_t need; };
+    std::vector<Ent> ent(L);
     for (int i = 0; i < L; ++i) {
         const LigHdr& h = lg->hdr_h[i];
-        const size_t topo = lane_topo_bytes(h.n, h.T, h.n_pairs);
-        const size_t per_chain = 4 * (size_t)lane_chain_slots(h.n, h.T, n_refine);
-        int best_c = 0, best_r = 0, best_w = -1;
-        for (int c = cmax; c >= 32; c -= 32) {
-            const size_t need = topo + per_chain * c;
-            if (need > TRIDSK_SMEM_MAX_CTA) continue;
-            int r = (int)(TRIDSK_SMEM_PER_SM / (need + TRIDSK_SMEM_RESERVED));
-            r = std::min(r, 16);
-            const int w = std::min(r * c / 32, 24);             // beyond ~24 warps the register file is the limit
-            if (w > best_w) { best_w = w; best_c = c; best_r = r; }
-        }
-        if (best_w < 0) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");
-        cls[i] = {(best_c << 8) | best_r, i};
+        const size_t topo = lane_topo_bytes(h.n, h.T, h.ls_len);
+        const size_t per_chain = 4 * (size_t)lane_chain_slots(h.n, h.T, h.max_depth, n_refine);
+        int c = cmax;
+        while (c > 32 && topo + per_chain * c > TRIDSK_SMEM_MAX_CTA) c -= 32;
+        const size_t need = (topo + per_chain * c + 15) / 16 * 16;
+        if (need > TRIDSK_SMEM_MAX_CTA) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");
+        int r = (int)(TRIDSK_SMEM_PER_SM / (need + TRIDSK_SMEM_RESERVED));
+        r = std::max(1, std::min(r, 16 * 32 / c));            // 128 registers per thread: at most 16 warps per SM
+        ent[i] = {(c << 8) | r, (long long)h.n_pairs + 6LL * h.n + 8LL * h.T, i, need};
     }
-    std::sort(cls.begin(), cls.end());
+    std::sort(ent.begin(), ent.end(), [](const Ent& x, const Ent& y) {
+        if (x.cls != y.cls) return x.cls < y.cls;
+        if (x.cost != y.cost) return x.cost > y.cost;
+        return x.lig < y.lig;
+    });
     lg->lane_ids_h.resize(L);
     lg->lane_plan.clear();
     for (int i = 0; i < L; ++i) {
-        lg->lane_ids_h[i] = cls[i].second;
-        if (i == 0 || cls[i].first != cls[i - 1].first) {
-            const int c = cls[i].first >> 8, r = cls[i].first & 0xff;
-            const size_t smem = std::min<size_t>(TRIDSK_SMEM_PER_SM / r - TRIDSK_SMEM_RESERVED, TRIDSK_SMEM_MAX_CTA) / 16 * 16;
-            lg->lane_plan.push_back({c, smem, i, 0});
-        }
+        lg->lane_ids_h[i] = ent[i].lig;
+        if (i == 0 || ent[i].cls != ent[i - 1].cls) lg->lane_plan.push_back({ent[i].cls >> 8, 0, i, 0});
         lg->lane_plan.back().count++;
+        lg->lane_plan.back().smem = std::max(lg->lane_plan.back().smem, ent[i].need);
     }
+    if (getenv("TRIDSK_DEBUG"))
+        for (const auto& b : lg->lane_plan)
+            fprintf(stderr, "tridsk lane plan: %d ligands, %d chains per CTA, %zu bytes of shared memory\n", b.count, b.chains_per_cta, b.smem);
     CK(cudaStreamSynchronize(ctx->stream));                  // an earlier dock may still read all_ids
     CK(cudaMemcpyAsync(lg->all_ids, lg->lane_ids_h.data(), sizeof(int) * L, cudaMemcpyHostToDevice, ctx->stream));
     lg->lane_plan_key = key;
@@ -671,7 +725,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     McLaunch base;
     memset(&base, 0, sizeof(base));
     base.hdr = ligs->hdr; base.atom_f4 = ligs->atom_f4; base.atom_i = ligs->atom_i; base.frags = ligs->frags; base.rounds = ligs->rounds;
-    base.lane_pairs = ligs->lane_pairs; base.lane_pstart = ligs->lane_pstart;
+    base.lane_frags = ligs->lane_frags; base.lane_stream = ligs->lane_stream;
     base.grid = grid->d;
     to_dparams(params, &base.P);
     for (int c = 0; c < 3; ++c) { base.box_min[c] = box_min[c]; base.box_max[c] = box_max[c]; base.centre[c] = pocket_center[c]; }
@@ -689,7 +743,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     if (lane) { int rc = lane_plan(ctx, lg, n_chains, params->n_refine); if (rc) return rc; }
 
     // launch series: per steps_per_launch slice, one launch per bucket (atoms per lane J, or shared-memory class); then top-k
-    struct Item { int kind, arg; size_t smem; McLaunch a; };
+    struct Item { int kind, arg; size_t smem; int branch; McLaunch a; };
     std::vector<Item> series;
     const int spl = (o.steps_per_launch > 0) ? o.steps_per_launch : std::max(n_steps, 1);
     int done = 0;
@@ -701,11 +755,12 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
             a.init_mode = first ? (o.resume ? 2 : (o.init_poses ? 1 : 0)) : 2;
         };
         if (lane) {
+            int br = 0;
             for (const auto& b : lg->lane_plan) {
                 McLaunch a = base;
                 a.lig_list = lg->all_ids + b.first; a.n_list = b.count;
                 fill(a);
-                series.push_back({2, b.chains_per_cta, b.smem, a});
+                series.push_back({2, b.chains_per_cta, b.smem, br++ % TRIDSK_BRANCHES, a});
             }
         } else {
             for (int j = 1; j <= TRIDSK_MAX_J; ++j) {
@@ -713,7 +768,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
                 McLaunch a = base;
                 a.lig_list = ligs->bucket_dev[j]; a.n_list = (int)ligs->bucket[j].size();
                 fill(a);
-                series.push_back({1, j, 0, a});
+                series.push_back({1, j, 0, (j - 1) % TRIDSK_BRANCHES, a});
             }
         }
         done += ns; first = false;
@@ -729,14 +784,35 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
 
     for (int i = 0; i < 3; ++i) if (!ctx->ev[i]) CK(cudaEventCreate(&ctx->ev[i]));
     ctx->ev_valid = false;
+    // independent launches (size buckets) run as parallel branches: branch 0 is the ctx stream, the others side streams
+    int n_branch = 1;
+    for (auto& it : series) n_branch = std::max(n_branch, it.branch + 1);
+    if (n_branch > 1) {
+        if (!ctx->fork_ev) CK(cudaEventCreateWithFlags(&ctx->fork_ev, cudaEventDisableTiming));
+        for (int i = 1; i < n_branch; ++i) {
+            if (!ctx->side[i]) CK(cudaStreamCreateWithFlags(&ctx->side[i], cudaStreamNonBlocking));
+            if (!ctx->join_ev[i]) CK(cudaEventCreateWithFlags(&ctx->join_ev[i], cudaEventDisableTiming));
+        }
+    }
     // inside a capture the events are recorded with the External flag (event-record nodes that stay queryable);
     // that flag is only legal while capturing
     auto enqueue = [&](cudaStream_t s, bool capturing) -> cudaError_t {
         const unsigned fl = capturing ? cudaEventRecordExternal : cudaEventRecordDefault;
         cudaError_t e = cudaEventRecordWithFlags(ctx->ev[0], s, fl);
         if (e != cudaSuccess) return e;
+        if (n_branch > 1) {
+            e = cudaEventRecord(ctx->fork_ev, s);
+            for (int i = 1; i < n_branch && e == cudaSuccess; ++i) e = cudaStreamWaitEvent(ctx->side[i], ctx->fork_ev, 0);
+            if (e != cudaSuccess) return e;
+        }
         for (auto& it : series) {
-            e = it.kind == 2 ? launch_mc_lane(s, it.a, it.arg, it.smem) : launch_mc(s, it.arg, it.a);
+            cudaStream_t bs = it.branch == 0 ? s : ctx->side[it.branch];
+            e = it.kind == 2 ? launch_mc_lane(bs, it.a, it.arg, it.smem) : launch_mc(bs, it.arg, it.a);
+            if (e != cudaSuccess) return e;
+        }
+        for (int i = 1; i < n_branch; ++i) {
+            e = cudaEventRecord(ctx->join_ev[i], ctx->side[i]);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(s, ctx->join_ev[i], 0);
             if (e != cudaSuccess) return e;
         }
         e = cudaEventRecordWithFlags(ctx->ev[1], s, fl);
@@ -750,7 +826,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         // a10: the whole series as one CUDA graph; re-used while the launch parameters are byte-identical
         std::vector<unsigned char> key;
         for (auto& it : series) {
-            const long long hd[3] = {it.kind, it.arg, (long long)it.smem};
+            const long long hd[4] = {it.kind, it.arg, (long long)it.smem, it.branch};
             key.insert(key.end(), (const unsigned char*)hd, (const unsigned char*)hd + sizeof(hd));
             key.insert(key.end(), (unsigned char*)&it.a, (unsigned char*)&it.a + sizeof(McLaunch));
         }

@@ -53,7 +53,7 @@ __device__ __forceinline__ void quat_rotate_by(float q[4], float vx, float vy, f
     else {
         const float ainv = rsqrtf(a2), a = a2 * ainv;
         float sn, cs;
-        sincosf(0.5f * a, &sn, &cs);
+        __sincosf(0.5f * a, &sn, &cs);                // |a| is a fraction of a radian: abs error < 5e-7, and q is renormalised
         dw = cs; s = sn * ainv;
     }
     const float dx = s * vx, dy = s * vy, dz = s * vz;

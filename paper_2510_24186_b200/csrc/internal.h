@@ -12,6 +12,7 @@
 #define TRIDSK_WARPS_PER_CTA 4
 #define TRIDSK_MAX_J 4           // atoms per lane (n_atoms <= 32 * MAX_J)
 #define TRIDSK_MAX_TILES 10      // J(J+1)/2 tiles of the pair schedule
+#define TRIDSK_BRANCHES 8        // parallel branches of a dock's launch series (ctx stream + side streams)
 
 // ---------------------------------------------------------------- device-side packed formats
 // Scoring / sampling constants in the form the kernels use (fp32).
@@ -45,10 +46,29 @@ struct LigHdr {
     int max_depth;
     int tile_off[TRIDSK_MAX_TILES + 1];   // round ranges per (j1<=j2) tile, relative to round_off
     int n_pairs;
-    int lp_off;                   // lane format: into lane_pairs (n_pairs records, grouped by first atom)
-    int ps_off;                   // lane format: into lane_pstart (n + 1 entries)
+    int ls_off;                   // lane format: into lane_stream (ls_len uint2 words, see LaneFrag)
+    int ls_len;
     int pad[2];
 };
+
+// Lane format (mc_lane.cu).  Fragments are re-indexed in depth-first PRE-order g = 0..T (0 = root), so that the
+// subtree of g is the contiguous fragment range [g, g_end) and a fragment at depth d finds its parent's frame in
+// frame slot d - 1.  One record per fragment:
+struct LaneFrag {
+    float ux, uy, uz;             // torsion axis (unit) and axis point (atom b_k), reference frame
+    float ox, oy, oz;
+    int lo, own_hi;               // the fragment's own atoms [lo, own_hi), internal order
+    int parent;                   // pre-order index of the parent fragment (0 for the root)
+    int depth;                    // root = 0
+    int axis;                     // internal indices of the axis atoms a_k | b_k << 8
+    int tor;                      // torsion index k of the pose vector (pose[7 + k]); -1 for the root
+};
+// The intra-ligand pair set as a uniform instruction stream of uint2 words.  For every fragment g (pre-order):
+//   {n_tiles, 0}
+//   per tile (1..4 consecutive own atoms of g):   {a0 | width << 8, n_runs}
+//     per run (partners in ONE later fragment fb): {fb, n_b}
+//       per partner atom b:                        {b | excl << 8 | hb << 12, vdW radius of b (float bits)}
+// excl bit i: (a0 + i, b) is NOT a pair; hb bit i: (a0 + i, b) is a donor/acceptor pair.
 
 // Per-fragment record; fragment 0 is the root, fragment k+1 hangs off torsion k.
 struct FragRec {
@@ -73,8 +93,8 @@ struct McLaunch {
     const int* atom_i;            // type | frag << 8 | original index << 16
     const FragRec* frags;
     const PairRound* rounds;
-    const uint2* lane_pairs;      // lane format: {b | hb << 8, d_vdw bits}, grouped by first atom a < b
-    const int* lane_pstart;       // lane format: per ligand n + 1 offsets into its lane_pairs
+    const LaneFrag* lane_frags;   // lane format: T + 1 records per ligand at frag_off, pre-order
+    const uint2* lane_stream;     // lane format: the pair instruction stream
     const int* lig_list;          // ligands handled by this launch (one bucket)
     int n_list;
     DGrid grid;
@@ -100,8 +120,8 @@ struct ScoreLaunch {
     const int* atom_i;
     const FragRec* frags;
     const PairRound* rounds;
-    const uint2* lane_pairs;
-    const int* lane_pstart;
+    const LaneFrag* lane_frags;
+    const uint2* lane_stream;
     const int* seg_lig;           // lane score kernel: per CTA the ligand, and its poses perm[seg_start .. seg_start + seg_cnt)
     const int* seg_start;
     const int* seg_cnt;
@@ -126,18 +146,20 @@ struct TopkLaunch {
 
 // ---------------------------------------------------------------- lane-per-chain kernel: shared-memory budget
 // One CTA = chains_per_cta chains of ONE ligand.  Shared memory = the ligand's topology (staged once per CTA)
-// + per chain: coordinates X[3n], forces F[max(3n, 12(T+1))] (the fragment frames of the forward pass alias F),
-// current and proposed torsions [2T], and the torsion Adam moments [2T] when n_refine > 1.
+// + per chain: coordinates X[3n], a scratch region that holds the fragment frames [12 max_depth] during the forward
+// pass and the per-fragment wrenches [6(T+1)] during the reverse pass, current and proposed torsions [2T], and the
+// torsion Adam moments [2T] when n_refine > 1.
 #define TRIDSK_SMEM_PER_SM 233472      // 228 KB
 #define TRIDSK_SMEM_RESERVED 1024      // per resident CTA
 #define TRIDSK_SMEM_MAX_CTA 232448     // 227 KB opt-in maximum per CTA
-__host__ __device__ static inline size_t lane_topo_bytes(int n, int T, int P) {
-    const size_t b = 16 * (size_t)n + sizeof(FragRec) * (size_t)(T + 1) + 8 * (size_t)P + 4 * (size_t)(n + 1);
-    return (b + 15) / 16 * 16;
+__host__ __device__ static inline size_t lane_topo_bytes(int n, int T, int ls_len) {
+    return (16 * (size_t)n + 16 * (size_t)((n + 3) / 4) + sizeof(LaneFrag) * (size_t)(T + 1) + 8 * (size_t)ls_len + 15) / 16 * 16;
 }
-__host__ __device__ static inline int lane_fslots(int n, int T) { return 3 * n > 12 * (T + 1) ? 3 * n : 12 * (T + 1); }
-__host__ __device__ static inline int lane_chain_slots(int n, int T, int n_refine) {
-    return 3 * n + lane_fslots(n, T) + 2 * T + (n_refine > 1 ? 2 * T : 0);
+__host__ __device__ static inline int lane_wslots(int T, int max_depth) {
+    return 6 * (T + 1) > 12 * max_depth ? 6 * (T + 1) : 12 * max_depth;
+}
+__host__ __device__ static inline int lane_chain_slots(int n, int T, int max_depth, int n_refine) {
+    return 3 * n + lane_wslots(T, max_depth) + 2 * T + (n_refine > 1 ? 2 * T : 0);
 }
 
 // ---------------------------------------------------------------- host-side handles
@@ -157,6 +179,8 @@ struct tridsk_ctx {
     int graph_launches = 0;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // dock: before MC series, after MC series, after top-k
     bool ev_valid = false;
+    cudaStream_t side[TRIDSK_BRANCHES] = {};           // side[0] unused
+    cudaEvent_t fork_ev = nullptr, join_ev[TRIDSK_BRANCHES] = {};
     int kernel = 0;               // tridsk_set_kernel: 0 auto, 1 warp per chain, 2 lane per chain
     int last_kernel = 0;          // what the last dock used
 };
@@ -179,8 +203,8 @@ struct tridsk_ligands {
     int* atom_i = nullptr;
     FragRec* frags = nullptr;
     PairRound* rounds = nullptr;
-    uint2* lane_pairs = nullptr;
-    int* lane_pstart = nullptr;
+    LaneFrag* lane_frags = nullptr;
+    uint2* lane_stream = nullptr;
     int* all_ids = nullptr;       // 0..n_lig-1 re-ordered per lane bucket (refilled when the plan key changes)
     struct LaneBucket { int chains_per_cta; size_t smem; int first, count; };
     std::vector<LaneBucket> lane_plan;
