@@ -246,7 +246,8 @@ struct PackedLig {
     std::vector<FragRec> fr;
     std::vector<PairRound> rounds;
     std::vector<LaneFrag> lane_frags;   // lane format (internal.h): fragments in pre-order
-    std::vector<uint2> lane_stream;     // lane format: the pair instruction stream
+    std::vector<uint4> lane_stream;     // lane format: the pair instruction stream (header units)
+    std::vector<LaneRec> lane_recs;     // lane format: the pair records, in stream order
     int err = 0;
     const char* msg = "";
 };
@@ -391,36 +392,40 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
         for (int g = 0; g <= T; ++g) {
             const int lo_g = out.lane_frags[g].lo, cnt = out.lane_frags[g].own_hi - lo_g;
             const size_t hdr_at = out.lane_stream.size();
-            out.lane_stream.push_back(make_uint2(0u, 0u));
+            out.lane_stream.push_back(make_uint4(0u, 0u, 0u, 0u));
             const int nt = (cnt + 3) / 4;
             unsigned n_tiles = 0;
             for (int tl = 0, a0 = lo_g; tl < nt; ++tl) {
                 const int w = cnt / nt + (tl < cnt % nt ? 1 : 0);
                 const size_t tile_at = out.lane_stream.size();
-                out.lane_stream.push_back(make_uint2((unsigned)a0 | ((unsigned)w << 8), 0u));
+                out.lane_stream.push_back(make_uint4((unsigned)a0, (unsigned)w, 0u, 0u));
                 unsigned n_runs = 0;
-                for (int fb = g; fb <= T; ++fb) {
-                    const size_t run_at = out.lane_stream.size();
-                    out.lane_stream.push_back(make_uint2((unsigned)fb, 0u));
+                for (int fb = g; fb <= T; ++fb) {             // fb == g: only explicit pair lists can pair a fragment with itself
                     unsigned nb = 0;
                     for (int y = out.lane_frags[fb].lo; y < out.lane_frags[fb].own_hi; ++y) {
-                        unsigned excl = (0xfu << w) & 0xfu, hbm = 0, any = 0;   // lanes beyond the tile width never pair
-                        for (int i = 0; i < w; ++i) {
+                        LaneRec rec;
+                        memset(&rec, 0, sizeof(rec));
+                        rec.b = (unsigned)y;
+                        bool any = false;
+                        for (int i = 0; i < 4; ++i) {
                             const int x = a0 + i;
-                            if (x < y && pm[(size_t)x * n + y]) { any = 1; ++covered2; if (hbp(x, y)) hbm |= 1u << i; }
-                            else excl |= 1u << i;
+                            rec.dvdw[i] = -1.f;                               // no pair in this slot
+                            if (i < w && x < y && pm[(size_t)x * n + y]) {
+                                any = true; ++covered2;
+                                rec.dvdw[i] = out.f4[x].w + out.f4[y].w;      // layout: operands of the pair function
+                                if (hbp(x, y)) rec.hbmask |= 1u << i;
+                            }
                         }
                         if (!any) continue;
-                        unsigned bits;
-                        memcpy(&bits, &out.f4[y].w, sizeof(bits));
-                        out.lane_stream.push_back(make_uint2((unsigned)y | (excl << 8) | (hbm << 12), bits));
+                        out.lane_recs.push_back(rec);
                         ++nb;
                     }
-                    if (nb) { out.lane_stream[run_at].y = nb; ++n_runs; }
-                    else out.lane_stream.pop_back();
+                    if (nb) { out.lane_stream.push_back(make_uint4((unsigned)fb, nb, 0u, 0u)); ++n_runs; }
                 }
-                if (n_runs) { out.lane_stream[tile_at].y = n_runs; ++n_tiles; }
-                else out.lane_stream.pop_back();
+                if (n_runs) {
+                    // the run headers were pushed after their records were counted: they already follow the tile header
+                    out.lane_stream[tile_at].z = n_runs; ++n_tiles;
+                } else out.lane_stream.pop_back();
                 a0 += w;
             }
             out.lane_stream[hdr_at].x = n_tiles;
@@ -428,6 +433,7 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
         (void)gof;
         if (covered2 != P) return bad(TRIDSK_EINVAL, "internal: lane pair stream does not cover the pair set");
         h.ls_len = (int)out.lane_stream.size();
+        h.n_rec = (int)out.lane_recs.size();
     }
     // conflict-free schedule: round (j1, j2, k): lane l <-> pair (j1*S + l, j2*S + (l+k) mod S)
     auto hb = [&](int x, int y) {
@@ -475,13 +481,13 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     tridsk_ligands* lg = new (std::nothrow) tridsk_ligands();
     if (!lg) return fail(ctx, TRIDSK_ENOMEM, "host alloc");
     lg->ctx = ctx; lg->n_lig = L;
-    size_t na = 0, nf = 0, nr = 0, nls = 0;
+    size_t na = 0, nf = 0, nr = 0, nls = 0, nrec = 0;
     lg->hdr_h.resize(L); lg->n_pairs.resize(L);
     for (int i = 0; i < L; ++i) {
         LigHdr& h = pk[i].h;
-        h.atom_off = (int)na; h.frag_off = (int)nf; h.round_off = (int)nr; h.ls_off = (int)nls;
+        h.atom_off = (int)na; h.frag_off = (int)nf; h.round_off = (int)nr; h.ls_off = (int)nls; h.rec_off = (int)nrec;
         na += pk[i].f4.size(); nf += pk[i].fr.size(); nr += pk[i].rounds.size();
-        nls += pk[i].lane_stream.size();
+        nls += pk[i].lane_stream.size(); nrec += pk[i].lane_recs.size();
         lg->hdr_h[i] = h; lg->n_pairs[i] = h.n_pairs;
         lg->max_atoms = std::max(lg->max_atoms, h.n); lg->max_tor = std::max(lg->max_tor, h.T);
         lg->bucket[h.J].push_back(i);
@@ -491,11 +497,13 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     std::vector<FragRec> fr(nf);
     std::vector<PairRound> rd(std::max<size_t>(nr, 1));
     std::vector<LaneFrag> lf(nf);
-    std::vector<uint2> lsv(std::max<size_t>(nls, 1));
+    std::vector<uint4> lsv(std::max<size_t>(nls, 1));
+    std::vector<LaneRec> lrv(std::max<size_t>(nrec, 1));
     for (int i = 0; i < L; ++i) {
         const LigHdr& h = pk[i].h;
         std::copy(pk[i].lane_frags.begin(), pk[i].lane_frags.end(), lf.begin() + h.frag_off);
         std::copy(pk[i].lane_stream.begin(), pk[i].lane_stream.end(), lsv.begin() + h.ls_off);
+        std::copy(pk[i].lane_recs.begin(), pk[i].lane_recs.end(), lrv.begin() + h.rec_off);
         std::copy(pk[i].f4.begin(), pk[i].f4.end(), f4.begin() + h.atom_off);
         std::copy(pk[i].ai.begin(), pk[i].ai.end(), ai.begin() + h.atom_off);
         std::copy(pk[i].fr.begin(), pk[i].fr.end(), fr.begin() + h.frag_off);
@@ -513,7 +521,8 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     up((void**)&lg->frags, fr.data(), sizeof(FragRec) * nf);
     up((void**)&lg->rounds, rd.data(), sizeof(PairRound) * rd.size());
     up((void**)&lg->lane_frags, lf.data(), sizeof(LaneFrag) * nf);
-    up((void**)&lg->lane_stream, lsv.data(), sizeof(uint2) * lsv.size());
+    up((void**)&lg->lane_stream, lsv.data(), sizeof(uint4) * lsv.size());
+    up((void**)&lg->lane_recs, lrv.data(), sizeof(LaneRec) * lrv.size());
     if (e == cudaSuccess) e = cudaMalloc((void**)&lg->all_ids, sizeof(int) * std::max(L, 1));
     for (int j = 1; j <= TRIDSK_MAX_J; ++j)
         if (!lg->bucket[j].empty()) up((void**)&lg->bucket_dev[j], lg->bucket[j].data(), sizeof(int) * lg->bucket[j].size());
@@ -538,7 +547,7 @@ extern "C" int tridsk_ligand_info(const tridsk_ligands* l, int* n_lig, int* max_
 extern "C" void tridsk_free_ligands(tridsk_ligands* l) {
     if (!l) return;                 // cudaFree waits for the device; l->ctx may already be destroyed
     cudaFree(l->hdr); cudaFree(l->atom_f4); cudaFree(l->atom_i); cudaFree(l->frags); cudaFree(l->rounds);
-    cudaFree(l->lane_frags); cudaFree(l->lane_stream); cudaFree(l->all_ids);
+    cudaFree(l->lane_frags); cudaFree(l->lane_stream); cudaFree(l->lane_recs); cudaFree(l->all_ids);
     for (int j = 0; j <= TRIDSK_MAX_J; ++j) if (l->bucket_dev[j]) cudaFree(l->bucket_dev[j]);
     delete l;
 }
@@ -562,7 +571,7 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
     ScoreLaunch a;
     memset(&a, 0, sizeof(a));
     a.hdr = ligs->hdr; a.atom_f4 = ligs->atom_f4; a.atom_i = ligs->atom_i; a.frags = ligs->frags; a.rounds = ligs->rounds;
-    a.lane_frags = ligs->lane_frags; a.lane_stream = ligs->lane_stream;
+    a.lane_frags = ligs->lane_frags; a.lane_stream = ligs->lane_stream; a.lane_recs = ligs->lane_recs;
     a.grid = grid->d;
     to_dparams(params, &a.P);
     a.n_pose = n_pose; a.pose_stride = pose_stride; a.grad_stride = grad_stride; a.coord_stride = coord_stride;
@@ -599,7 +608,7 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
             while (j < n_pose && j - i < 32 && li[perm[j]] == li[perm[i]]) ++j;
             s_lig.push_back(li[perm[i]]); s_start.push_back(i); s_cnt.push_back(j - i);
             const LigHdr& h = ligs->hdr_h[li[perm[i]]];
-            smem = std::max(smem, lane_topo_bytes(h.n, h.T, h.ls_len) + 128 * (size_t)lane_chain_slots(h.n, h.T, h.max_depth, 1));
+            smem = std::max(smem, lane_topo_bytes(h.n, h.T, h.ls_len, h.n_rec) + 128 * (size_t)lane_chain_slots(h.n, h.T, h.max_depth, 1));
             i = j;
         }
         if (smem > TRIDSK_SMEM_MAX_CTA) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");
@@ -640,7 +649,7 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
     std::vector<Ent> ent(L);
     for (int i = 0; i < L; ++i) {
         const LigHdr& h = lg->hdr_h[i];
-        const size_t topo = lane_topo_bytes(h.n, h.T, h.ls_len);
+        const size_t topo = lane_topo_bytes(h.n, h.T, h.ls_len, h.n_rec);
         const size_t per_chain = 4 * (size_t)lane_chain_slots(h.n, h.T, h.max_depth, n_refine);
         int c = cmax;
         while (c > 32 && topo + per_chain * c > TRIDSK_SMEM_MAX_CTA) c -= 32;
@@ -725,7 +734,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     McLaunch base;
     memset(&base, 0, sizeof(base));
     base.hdr = ligs->hdr; base.atom_f4 = ligs->atom_f4; base.atom_i = ligs->atom_i; base.frags = ligs->frags; base.rounds = ligs->rounds;
-    base.lane_frags = ligs->lane_frags; base.lane_stream = ligs->lane_stream;
+    base.lane_frags = ligs->lane_frags; base.lane_stream = ligs->lane_stream; base.lane_recs = ligs->lane_recs;
     base.grid = grid->d;
     to_dparams(params, &base.P);
     for (int c = 0; c < 3; ++c) { base.box_min[c] = box_min[c]; base.box_max[c] = box_max[c]; base.centre[c] = pocket_center[c]; }

@@ -46,9 +46,10 @@ struct LigHdr {
     int max_depth;
     int tile_off[TRIDSK_MAX_TILES + 1];   // round ranges per (j1<=j2) tile, relative to round_off
     int n_pairs;
-    int ls_off;                   // lane format: into lane_stream (ls_len uint2 words, see LaneFrag)
+    int ls_off;                   // lane format: into lane_stream (ls_len 16-byte header units, see LaneFrag)
     int ls_len;
-    int pad[2];
+    int rec_off;                  // lane format: into lane_recs (n_rec records, in the order the stream consumes them)
+    int n_rec;
 };
 
 // Lane format (mc_lane.cu).  Fragments are re-indexed in depth-first PRE-order g = 0..T (0 = root), so that the
@@ -63,12 +64,23 @@ struct LaneFrag {
     int axis;                     // internal indices of the axis atoms a_k | b_k << 8
     int tor;                      // torsion index k of the pose vector (pose[7 + k]); -1 for the root
 };
-// The intra-ligand pair set as a uniform instruction stream of uint2 words.  For every fragment g (pre-order):
-//   {n_tiles, 0}
-//   per tile (1..4 consecutive own atoms of g):   {a0 | width << 8, n_runs}
-//     per run (partners in ONE later fragment fb): {fb, n_b}
-//       per partner atom b:                        {b | excl << 8 | hb << 12, vdW radius of b (float bits)}
-// excl bit i: (a0 + i, b) is NOT a pair; hb bit i: (a0 + i, b) is a donor/acceptor pair.
+// The intra-ligand pair set as a uniform instruction stream: 16-byte header units + a record array that the headers
+// consume in order.  For every fragment g (pre-order):
+//   {n_tiles, 0, 0, 0}
+//   per tile (1..4 consecutive own atoms a0 .. a0+w-1 of g):   {a0, w, n_runs, 0}
+//     per run (partner atoms in ONE later fragment fb):          {fb, n_rec, 0, 0}   -> the next n_rec records
+// One record = one partner atom b against the 4 slots of the tile.  In global memory (LaneRec) it holds what depends
+// on the ligand only; lane_stage turns it into the 48-byte shared-memory form that also depends on the parameters:
+//   {c[4]  = dvdw + long_mu,          (slot without a pair -- excluded, or beyond the tile width: -1e15)
+//    dc[4] = clash distance: hb_dclash for a donor/acceptor pair else dvdw,   (slot without a pair: 0)
+//    3 * b, hbmask, 0, 0}
+// so that the pair arithmetic has no topology branch: a slot without a pair evaluates to exactly zero.
+struct LaneRec {
+    float dvdw[4];                // r_a + r_b per slot; < 0 for a slot without a pair
+    uint32_t b, hbmask;           // partner atom (internal index); bit i: slot i is a donor/acceptor pair
+    uint32_t pad[2];
+};
+#define TRIDSK_LANE_REC_SMEM 48
 
 // Per-fragment record; fragment 0 is the root, fragment k+1 hangs off torsion k.
 struct FragRec {
@@ -94,7 +106,8 @@ struct McLaunch {
     const FragRec* frags;
     const PairRound* rounds;
     const LaneFrag* lane_frags;   // lane format: T + 1 records per ligand at frag_off, pre-order
-    const uint2* lane_stream;     // lane format: the pair instruction stream
+    const uint4* lane_stream;     // lane format: the pair instruction stream (header units)
+    const LaneRec* lane_recs;     // lane format: the pair records
     const int* lig_list;          // ligands handled by this launch (one bucket)
     int n_list;
     DGrid grid;
@@ -121,7 +134,8 @@ struct ScoreLaunch {
     const FragRec* frags;
     const PairRound* rounds;
     const LaneFrag* lane_frags;
-    const uint2* lane_stream;
+    const uint4* lane_stream;
+    const LaneRec* lane_recs;
     const int* seg_lig;           // lane score kernel: per CTA the ligand, and its poses perm[seg_start .. seg_start + seg_cnt)
     const int* seg_start;
     const int* seg_cnt;
@@ -152,8 +166,9 @@ struct TopkLaunch {
 #define TRIDSK_SMEM_PER_SM 233472      // 228 KB
 #define TRIDSK_SMEM_RESERVED 1024      // per resident CTA
 #define TRIDSK_SMEM_MAX_CTA 232448     // 227 KB opt-in maximum per CTA
-__host__ __device__ static inline size_t lane_topo_bytes(int n, int T, int ls_len) {
-    return (16 * (size_t)n + 16 * (size_t)((n + 3) / 4) + sizeof(LaneFrag) * (size_t)(T + 1) + 8 * (size_t)ls_len + 15) / 16 * 16;
+__host__ __device__ static inline size_t lane_topo_bytes(int n, int T, int ls_len, int n_rec) {
+    return 16 * (size_t)n + 16 * (size_t)((n + 3) / 4) + sizeof(LaneFrag) * (size_t)(T + 1) + 16 * (size_t)ls_len +
+           TRIDSK_LANE_REC_SMEM * (size_t)n_rec;
 }
 __host__ __device__ static inline int lane_wslots(int T, int max_depth) {
     return 6 * (T + 1) > 12 * max_depth ? 6 * (T + 1) : 12 * max_depth;
@@ -204,7 +219,8 @@ struct tridsk_ligands {
     FragRec* frags = nullptr;
     PairRound* rounds = nullptr;
     LaneFrag* lane_frags = nullptr;
-    uint2* lane_stream = nullptr;
+    uint4* lane_stream = nullptr;
+    LaneRec* lane_recs = nullptr;
     int* all_ids = nullptr;       // 0..n_lig-1 re-ordered per lane bucket (refilled when the plan key changes)
     struct LaneBucket { int chains_per_cta; size_t smem; int first, count; };
     std::vector<LaneBucket> lane_plan;

@@ -25,40 +25,48 @@ struct LaneTopo {
     const float4* ref;      // [n] {ref x, y, z, vdW radius}
     const int* meta;        // [n] type | (first own atom of its fragment) << 8 | pre-order fragment << 16
     const LaneFrag* frag;   // [T + 1]
-    const uint2* stream;    // pair instruction stream (internal.h)
+    const uint4* stream;    // pair instruction stream: header units (internal.h)
+    const uint4* recs;      // pair records, 3 units each: {c[4]}, {dc[4]}, {3 b, hbmask, 0, 0}
     int n, T;
 };
 
 // Constants of the pair function in the form the inner loop wants them.
 struct PairK {
     float nk2;              // -log2(e) / (2 sigma^2) of the long-range Gaussian
-    float dmax, mu, nmu;    // long-range cut-off, mu, -mu
-    float kappa;            // force scale: F = kappa * sum u g rinv d,  kappa = -2 w_long / log2(e)
-    float inv_kappa;
-    float w_long, w_clash, w_hbond, d_floor, hb_dclash, hb_dmax, hb_mu, hb_nk2, hb_k;
+    float dmax;             // long-range cut-off
+    float kappa;            // gradient scale: dE/dx_a = kappa * sum s (x_a - x_b),  kappa = -2 w_long / log2(e)
+    float kc;               // clash gradient in kappa units: w_clash / kappa
+    float inv_floor;        // 1 / d_floor
+    float kh;               // hydrogen-bond gradient in kappa units: 2 w_hbond / (2 sigma_hb^2) / kappa
+    float w_long, w_clash_ln2, w_hbond, hb_dmax, hb_mu, hb_nk2;
 };
 __device__ __forceinline__ PairK make_pairk(const DParams& P) {
     PairK K;
     const float L2E = 1.4426950408889634f;
-    K.nk2 = -P.long_inv_two_sigma2 * L2E; K.dmax = P.long_dmax; K.mu = P.long_mu; K.nmu = -P.long_mu;
-    K.kappa = -2.f * P.w_long / L2E; K.inv_kappa = 1.f / K.kappa;
-    K.w_long = P.w_long; K.w_clash = P.w_clash; K.w_hbond = P.w_hbond; K.d_floor = P.d_floor;
-    K.hb_dclash = P.hb_dclash; K.hb_dmax = P.hb_dmax; K.hb_mu = P.hb_mu;
-    K.hb_nk2 = -P.hb_inv_two_sigma2 * L2E; K.hb_k = P.hb_inv_two_sigma2;
+    K.nk2 = -P.long_inv_two_sigma2 * L2E; K.dmax = P.long_dmax;
+    K.kappa = -2.f * P.w_long / L2E;
+    K.kc = P.w_clash / K.kappa; K.inv_floor = 1.f / P.d_floor;
+    K.kh = 2.f * P.w_hbond * P.hb_inv_two_sigma2 / K.kappa;
+    K.w_long = P.w_long; K.w_clash_ln2 = P.w_clash * 0.6931471805599453f; K.w_hbond = P.w_hbond;
+    K.hb_dmax = P.hb_dmax; K.hb_mu = P.hb_mu; K.hb_nk2 = -P.hb_inv_two_sigma2 * L2E;
     return K;
 }
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
-// Stage one ligand's topology into shared memory; returns the first byte after it (16-byte aligned).
+// Stage one ligand's topology into shared memory; returns the first byte after it (16-byte aligned).  The pair
+// records take their parameter-dependent form here (internal.h): c = dvdw + mu, dc = clash distance, 3 * b.
 __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char* smem, const LigHdr* __restrict__ h,
                                                      const float4* __restrict__ atom_f4, const int* __restrict__ atom_i,
-                                                     const LaneFrag* __restrict__ lane_frags, const uint2* __restrict__ lane_stream) {
-    const int n = h->n, T = h->T, ls = h->ls_len, tid = threadIdx.x, nt = blockDim.x;
+                                                     const LaneFrag* __restrict__ lane_frags, const uint4* __restrict__ lane_stream,
+                                                     const LaneRec* __restrict__ lane_recs, const DParams& P) {
+    const int n = h->n, T = h->T, ls = h->ls_len, nr = h->n_rec, tid = threadIdx.x, nt = blockDim.x;
     float4* ref = reinterpret_cast<float4*>(smem);
     int* meta = reinterpret_cast<int*>(smem + 16 * (size_t)n);
     int* frag = reinterpret_cast<int*>(smem + 16 * (size_t)n + 16 * (size_t)((n + 3) / 4));
-    uint2* stream = reinterpret_cast<uint2*>(reinterpret_cast<unsigned char*>(frag) + sizeof(LaneFrag) * (size_t)(T + 1));
+    uint4* stream = reinterpret_cast<uint4*>(reinterpret_cast<unsigned char*>(frag) + sizeof(LaneFrag) * (size_t)(T + 1));
+    uint4* recs = stream + ls;
     const LaneFrag* fsrc = lane_frags + h->frag_off;
     for (int i = tid; i < n; i += nt) ref[i] = __ldg(atom_f4 + h->atom_off + i);
     for (int i = tid; i < (T + 1) * (int)(sizeof(LaneFrag) / 4); i += nt) frag[i] = __ldg(reinterpret_cast<const int*>(fsrc) + i);
@@ -67,8 +75,23 @@ __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char*
         for (int a = lo; a < hi; ++a) meta[a] = (__ldg(atom_i + h->atom_off + a) & 0xff) | ((a == lo) << 8) | (g << 16);
     }
     for (int i = tid; i < ls; i += nt) stream[i] = __ldg(lane_stream + h->ls_off + i);
-    S.ref = ref; S.meta = meta; S.frag = reinterpret_cast<const LaneFrag*>(frag); S.stream = stream; S.n = n; S.T = T;
-    return smem + lane_topo_bytes(n, T, ls);
+    for (int i = tid; i < nr; i += nt) {
+        const uint4* src = reinterpret_cast<const uint4*>(lane_recs + h->rec_off + i);
+        const uint4 dv = __ldg(src), mt = __ldg(src + 1);
+        const float d[4] = {__uint_as_float(dv.x), __uint_as_float(dv.y), __uint_as_float(dv.z), __uint_as_float(dv.w)};
+        float c[4], dc[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const bool pair = d[k] >= 0.f, hb = (mt.y >> k) & 1u;
+            c[k] = pair ? d[k] + P.long_mu : -1e15f;
+            dc[k] = pair ? (hb ? P.hb_dclash : d[k]) : 0.f;
+        }
+        recs[3 * i] = make_uint4(__float_as_uint(c[0]), __float_as_uint(c[1]), __float_as_uint(c[2]), __float_as_uint(c[3]));
+        recs[3 * i + 1] = make_uint4(__float_as_uint(dc[0]), __float_as_uint(dc[1]), __float_as_uint(dc[2]), __float_as_uint(dc[3]));
+        recs[3 * i + 2] = make_uint4(3u * mt.x, mt.y, 0u, 0u);
+    }
+    S.ref = ref; S.meta = meta; S.frag = reinterpret_cast<const LaneFrag*>(frag); S.stream = stream; S.recs = recs; S.n = n; S.T = T;
+    return smem + lane_topo_bytes(n, T, ls, nr);
 }
 
 // ------------------------------------------------------------------ a3 forward kinematics (O8)
@@ -182,74 +205,80 @@ __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, fl
 }
 
 // ------------------------------------------------------------------ a5 intra-ligand pairs (O2, O6)
-// One pair (a, b); c = r_a + r_b + mu, hb = donor/acceptor pair (warp-uniform).  Accumulates eL += the unweighted
-// long-range Gaussian, eX += the weighted clash / hydrogen-bond energy, and GRAD: (fx, fy, fz) += (de/dd / d)
-// (x_a - x_b) / kappa.  L = -[d<dmax] exp(-(d-dvdw-mu)^2/(2 sigma^2)) (G1); C = -[d<dc] ln(max(d,floor)/dc),
-// dc = 2.6 for donor/acceptor pairs else dvdw (G3, G4); H = -[hb, d<3.4] exp(-(d-2.88)^2/(2*0.3^2))
-// (P:123-125).
+// One record: partner atom b against the 4 slots of a tile, branch-free so that the four evaluations interleave.
+//   L = -[d<dmax] exp(-(d-dvdw-mu)^2/(2 sigma^2))  (G1):  eL += [d<dmax] 2^(nk2 (d-c)^2),  c = dvdw + mu
+//   C = -[d<dc] ln(max(d,floor)/dc)                (G3, G4):  eC += lg2(max(dc / max(d,floor), 1))
+//   H = -[hb, d<3.4] exp(-(d-2.88)^2/(2*0.3^2)):  eH += ..., only in records that hold such a pair
+// GRAD: f_i += s (x_a - x_b) with s = (de/dd) / d / kappa.  A slot without a pair has c = -1e15, dc = 0 and adds 0.
 template <bool GRAD>
-__device__ __forceinline__ void lane_pair(const PairK& K, float ax, float ay, float az, float bx, float by, float bz,
-                                          float c, bool hb, float& eL, float& eX, float& fx, float& fy, float& fz) {
-    const float dx = ax - bx, dy = ay - by, dz = az - bz;
-    const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-    const float rinv = rsqrt_approx(fmaxf(d2, 1e-12f));
-    const float d = d2 * rinv;
-    const float t = d - c;
-    const float u = t * K.nk2;
-    float g = ex2_approx(u * t);
-    g = d < K.dmax ? g : 0.f;
-    eL += g;
-    float s = 0.f;
-    if (GRAD) s = u * g * rinv;
-    const float dvdw = c - K.mu;
-    if (d < (hb ? K.hb_dmax : dvdw)) {                        // rare: clash and / or hydrogen-bond range
-        const float dc = hb ? K.hb_dclash : dvdw;
-        if (d < dc) {
-            eX -= K.w_clash * __logf(fmaxf(d, K.d_floor) * __frcp_rn(dc));
-            if (GRAD && d > K.d_floor) s -= K.w_clash * rinv * rinv * K.inv_kappa;
-        }
-        if (hb) {
-            const float th = d - K.hb_mu;
-            const float gh = ex2_approx(K.hb_nk2 * th * th);
-            eX -= K.w_hbond * gh;
-            if (GRAD) s += K.w_hbond * 2.f * th * K.hb_k * gh * rinv * K.inv_kappa;
-        }
-    }
-    if (GRAD) { fx = fmaf(s, dx, fx); fy = fmaf(s, dy, fy); fz = fmaf(s, dz, fz); }
-}
-
-// One tile: w <= 4 consecutive own atoms a0 .. a0+w-1 of fragment g against n_runs runs of partner atoms.  Returns
-// the stream position after the tile.  GRAD: acc += the wrench the tile's atoms receive; WR[fb] -= each run's wrench.
-// Every flag test is warp-uniform.
-template <bool GRAD>
-__device__ __forceinline__ const uint2* lane_tile(const uint2* sp, int a0, int w, int n_runs, const LaneTopo& S, const PairK& K,
-                                                  const float* __restrict__ X, float* __restrict__ WR, int C,
-                                                  float acc[6], float& eL, float& eX) {
-    float ax[4], ay[4], az[4], ca[4];
+__device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], const float ay[4], const float az[4],
+                                         float bx, float by, float bz, const float4 c4, const float4 dc4, unsigned hbmask,
+                                         float& eL, float& eC, float& eH, float fx[4], float fy[4], float fz[4]) {
+    const float c[4] = {c4.x, c4.y, c4.z, c4.w}, dc[4] = {dc4.x, dc4.y, dc4.z, dc4.w};
+    float dx[4], dy[4], dz[4], d[4], rinv[4], s[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const int a = a0 + (i < w ? i : 0);
-        const float* xa = X + 3 * a * C;
+        dx[i] = ax[i] - bx; dy[i] = ay[i] - by; dz[i] = az[i] - bz;
+        const float d2 = fmaxf(fmaf(dx[i], dx[i], fmaf(dy[i], dy[i], dz[i] * dz[i])), 1e-12f);
+        rinv[i] = rsqrt_approx(d2);
+        d[i] = d2 * rinv[i];
+        const float t = d[i] - c[i];
+        const float u = t * K.nk2;
+        float g = ex2_approx(u * t);
+        g = d[i] < K.dmax ? g : 0.f;
+        eL += g;
+        const float q = dc[i] * fminf(rinv[i], K.inv_floor);         // dc / max(d, floor); > 1 inside the clash range
+        eC += lg2_approx(fmaxf(q, 1.f));
+        if (GRAD) {
+            s[i] = u * g * rinv[i];
+            if (q > 1.f && rinv[i] < K.inv_floor) s[i] = fmaf(-K.kc * rinv[i], rinv[i], s[i]);
+        }
+    }
+    if (hbmask) {                                                    // warp-uniform; about one record in three
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            if ((hbmask >> i) & 1u) {
+                const float th = d[i] - K.hb_mu;
+                float gh = ex2_approx(K.hb_nk2 * th * th);
+                gh = d[i] < K.hb_dmax ? gh : 0.f;
+                eH += gh;
+                if (GRAD) s[i] = fmaf(K.kh * th, gh * rinv[i], s[i]);
+            }
+        }
+    }
+    if (GRAD) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { fx[i] = fmaf(s[i], dx[i], fx[i]); fy[i] = fmaf(s[i], dy[i], fy[i]); fz[i] = fmaf(s[i], dz[i], fz[i]); }
+    }
+}
+
+// One tile: w <= 4 consecutive own atoms a0 .. a0+w-1 of fragment g against n_runs runs of partner atoms; hp / rp walk
+// the header units / the records.  GRAD: acc += the wrench the tile's atoms receive; WR[fb] -= each run's wrench.
+template <bool GRAD>
+__device__ __forceinline__ void lane_tile(const uint4*& hp, const uint4*& rp, int a0, int w, int n_runs, const PairK& K,
+                                          const float* __restrict__ X, float* __restrict__ WR, int C,
+                                          float acc[6], float& eL, float& eC, float& eH) {
+    float ax[4], ay[4], az[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float* xa = X + 3 * (a0 + (i < w ? i : 0)) * C;
         ax[i] = xa[0]; ay[i] = xa[C]; az[i] = xa[2 * C];
-        ca[i] = S.ref[a].w + K.mu;
     }
     for (int run = 0; run < n_runs; ++run) {
-        const uint2 rh = *sp++;
+        const uint4 rh = *hp++;
         const int fb = (int)rh.x, nb = (int)rh.y;
         float fx[4], fy[4], fz[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) fx[i] = fy[i] = fz[i] = 0.f;
-        for (int j = 0; j < nb; ++j) {
-            const uint2 rec = sp[j];
-            const float* xb = X + 3 * (int)(rec.x & 0xffu) * C;
-            const float bx = xb[0], by = xb[C], bz = xb[2 * C], rb = __uint_as_float(rec.y);
-            const unsigned fl = rec.x >> 8;                   // excl bits 0..3, hb bits 4..7
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-                if (!((fl >> i) & 1u))
-                    lane_pair<GRAD>(K, ax[i], ay[i], az[i], bx, by, bz, ca[i] + rb, (fl >> (4 + i)) & 1u, eL, eX, fx[i], fy[i], fz[i]);
+        for (int j = 0; j < nb; ++j, rp += 3) {
+            const uint4 c4 = rp[0], dc4 = rp[1];
+            const uint2 mt = *reinterpret_cast<const uint2*>(rp + 2);
+            const float* xb = X + (int)mt.x * C;
+            lane_rec<GRAD>(K, ax, ay, az, xb[0], xb[C], xb[2 * C],
+                           make_float4(__uint_as_float(c4.x), __uint_as_float(c4.y), __uint_as_float(c4.z), __uint_as_float(c4.w)),
+                           make_float4(__uint_as_float(dc4.x), __uint_as_float(dc4.y), __uint_as_float(dc4.z), __uint_as_float(dc4.w)),
+                           mt.y, eL, eC, eH, fx, fy, fz);
         }
-        sp += nb;
         if (GRAD) {
             float wv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -268,22 +297,22 @@ __device__ __forceinline__ const uint2* lane_tile(const uint2* sp, int a0, int w
             }
         }
     }
-    return sp;
 }
 
 // All pairs of the ligand.  GRAD: WR[g] (initialised by lane_grid) += the pair wrenches.
 template <bool GRAD>
 __device__ __forceinline__ float lane_pairs(const LaneTopo& S, const PairK& K, const float* __restrict__ X,
                                             float* __restrict__ WR, int C) {
-    float eL = 0.f, eX = 0.f;
-    const uint2* sp = S.stream;
+    float eL = 0.f, eC = 0.f, eH = 0.f;
+    const uint4* hp = S.stream;
+    const uint4* rp = S.recs;
     for (int g = 0; g <= S.T; ++g) {
-        const int n_tiles = (int)(*sp++).x;
+        const int n_tiles = (int)(*hp++).x;
         if (n_tiles == 0) continue;
         float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         for (int tl = 0; tl < n_tiles; ++tl) {
-            const uint2 h = *sp++;
-            sp = lane_tile<GRAD>(sp, (int)(h.x & 0xffu), (int)(h.x >> 8), (int)h.y, S, K, X, WR, C, acc, eL, eX);
+            const uint4 h = *hp++;
+            lane_tile<GRAD>(hp, rp, (int)h.x, (int)h.y, (int)h.z, K, X, WR, C, acc, eL, eC, eH);
         }
         if (GRAD) {
             float* wg = WR + 6 * g * C;
@@ -291,7 +320,7 @@ __device__ __forceinline__ float lane_pairs(const LaneTopo& S, const PairK& K, c
             for (int c = 0; c < 6; ++c) wg[c * C] += acc[c];
         }
     }
-    return eX - K.w_long * eL;
+    return fmaf(K.w_clash_ln2, eC, -fmaf(K.w_long, eL, K.w_hbond * eH));
 }
 
 // ------------------------------------------------------------------ a3..a5: one pose evaluation by one lane
@@ -347,7 +376,7 @@ __global__ void __launch_bounds__(128, 4) mc_lane_kernel(const McLaunch a) {
     const int chain = (blockIdx.x % cpl) * C + tid;
     const LigHdr* h = a.hdr + lig;
     LaneTopo S;
-    unsigned char* after = lane_stage(S, lane_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.lane_stream);
+    unsigned char* after = lane_stage(S, lane_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.lane_stream, a.lane_recs, a.P);
     const int max_depth = h->max_depth;
     __syncthreads();
     if (chain >= a.n_chains) return;
@@ -534,7 +563,7 @@ __global__ void __launch_bounds__(32) score_lane_kernel(const ScoreLaunch a) {
     const int lig = a.seg_lig[blockIdx.x];
     const LigHdr* h = a.hdr + lig;
     LaneTopo S;
-    unsigned char* after = lane_stage(S, lane_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.lane_stream);
+    unsigned char* after = lane_stage(S, lane_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.lane_stream, a.lane_recs, a.P);
     __syncthreads();
     if (tid >= a.seg_cnt[blockIdx.x]) return;
     const int i = a.perm[a.seg_start[blockIdx.x] + tid];
