@@ -651,12 +651,18 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
         const LigHdr& h = lg->hdr_h[i];
         const size_t topo = lane_topo_bytes(h.n, h.T, h.ls_len, h.n_rec);
         const size_t per_chain = 4 * (size_t)lane_chain_slots(h.n, h.T, h.max_depth, n_refine);
-        int c = cmax;
-        while (c > 32 && topo + per_chain * c > TRIDSK_SMEM_MAX_CTA) c -= 32;
-        const size_t need = (topo + per_chain * c + 15) / 16 * 16;
-        if (need > TRIDSK_SMEM_MAX_CTA) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");
-        int r = (int)(TRIDSK_SMEM_PER_SM / (need + TRIDSK_SMEM_RESERVED));
-        r = std::max(1, std::min(r, 16 * 32 / c));            // 128 registers per thread: at most 16 warps per SM
+        // chains per CTA: the multiple of a warp that keeps the most warps resident per SM (ties: the larger CTA, which
+        // stages the topology fewer times); 128 registers per thread allow 16 warps per SM
+        int c = 0, r = 0;
+        size_t need = 0;
+        for (int cc = cmax; cc >= 32; cc -= 32) {
+            const size_t nd = (topo + per_chain * cc + 15) / 16 * 16;
+            if (nd > TRIDSK_SMEM_MAX_CTA) continue;
+            int rr = (int)(TRIDSK_SMEM_PER_SM / (nd + TRIDSK_SMEM_RESERVED));
+            rr = std::max(1, std::min(std::min(rr, 32), 16 * 32 / cc));
+            if (rr * cc > r * c) { c = cc; r = rr; need = nd; }
+        }
+        if (c == 0) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");
         ent[i] = {(c << 8) | r, (long long)h.n_pairs + 6LL * h.n + 8LL * h.T, i, need};
     }
     std::sort(ent.begin(), ent.end(), [](const Ent& x, const Ent& y) {

@@ -70,17 +70,16 @@ struct LaneFrag {
 //   per tile (1..4 consecutive own atoms a0 .. a0+w-1 of g):   {a0, w, n_runs, 0}
 //     per run (partner atoms in ONE later fragment fb):          {fb, n_rec, 0, 0}   -> the next n_rec records
 // One record = one partner atom b against the 4 slots of the tile.  In global memory (LaneRec) it holds what depends
-// on the ligand only; lane_stage turns it into the 48-byte shared-memory form that also depends on the parameters:
-//   {c[4]  = dvdw + long_mu,          (slot without a pair -- excluded, or beyond the tile width: -1e15)
-//    dc[4] = clash distance: hb_dclash for a donor/acceptor pair else dvdw,   (slot without a pair: 0)
-//    3 * b, hbmask, 0, 0}
-// so that the pair arithmetic has no topology branch: a slot without a pair evaluates to exactly zero.
+// on the ligand only; lane_stage turns it into the 20-byte shared-memory form (two arrays) that also depends on the
+// parameters:  c[4] = dvdw + long_mu (slot without a pair -- excluded, or beyond the tile width: -1e15), and one word
+// 3 * b | hbmask << 16.  The pair arithmetic then has no topology branch: a slot without a pair evaluates to exactly
+// zero (its clash distance c - mu is negative).
 struct LaneRec {
     float dvdw[4];                // r_a + r_b per slot; < 0 for a slot without a pair
     uint32_t b, hbmask;           // partner atom (internal index); bit i: slot i is a donor/acceptor pair
     uint32_t pad[2];
 };
-#define TRIDSK_LANE_REC_SMEM 48
+#define TRIDSK_LANE_REC_SMEM 20
 
 // Per-fragment record; fragment 0 is the root, fragment k+1 hangs off torsion k.
 struct FragRec {
@@ -168,7 +167,7 @@ struct TopkLaunch {
 #define TRIDSK_SMEM_MAX_CTA 232448     // 227 KB opt-in maximum per CTA
 __host__ __device__ static inline size_t lane_topo_bytes(int n, int T, int ls_len, int n_rec) {
     return 16 * (size_t)n + 16 * (size_t)((n + 3) / 4) + sizeof(LaneFrag) * (size_t)(T + 1) + 16 * (size_t)ls_len +
-           TRIDSK_LANE_REC_SMEM * (size_t)n_rec;
+           (TRIDSK_LANE_REC_SMEM * (size_t)n_rec + 15) / 16 * 16;
 }
 __host__ __device__ static inline int lane_wslots(int T, int max_depth) {
     return 6 * (T + 1) > 12 * max_depth ? 6 * (T + 1) : 12 * max_depth;

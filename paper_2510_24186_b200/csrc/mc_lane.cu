@@ -26,7 +26,8 @@ struct LaneTopo {
     const int* meta;        // [n] type | (first own atom of its fragment) << 8 | pre-order fragment << 16
     const LaneFrag* frag;   // [T + 1]
     const uint4* stream;    // pair instruction stream: header units (internal.h)
-    const uint4* recs;      // pair records, 3 units each: {c[4]}, {dc[4]}, {3 b, hbmask, 0, 0}
+    const float4* rec_c;    // pair records: c[4] per record ...
+    const uint32_t* rec_m;  // ... and 3 b | hbmask << 16
     int n, T;
 };
 
@@ -35,6 +36,8 @@ struct PairK {
     float nk2;              // -log2(e) / (2 sigma^2) of the long-range Gaussian
     float dmax;             // long-range cut-off
     float kappa;            // gradient scale: dE/dx_a = kappa * sum s (x_a - x_b),  kappa = -2 w_long / log2(e)
+    float mu;               // long-range mu: the clash distance of a plain pair is c - mu
+    float hb_dclash;        // clash distance of a donor/acceptor pair
     float kc;               // clash gradient in kappa units: w_clash / kappa
     float inv_floor;        // 1 / d_floor
     float kh;               // hydrogen-bond gradient in kappa units: 2 w_hbond / (2 sigma_hb^2) / kappa
@@ -45,6 +48,7 @@ __device__ __forceinline__ PairK make_pairk(const DParams& P) {
     const float L2E = 1.4426950408889634f;
     K.nk2 = -P.long_inv_two_sigma2 * L2E; K.dmax = P.long_dmax;
     K.kappa = -2.f * P.w_long / L2E;
+    K.mu = P.long_mu; K.hb_dclash = P.hb_dclash;
     K.kc = P.w_clash / K.kappa; K.inv_floor = 1.f / P.d_floor;
     K.kh = 2.f * P.w_hbond * P.hb_inv_two_sigma2 / K.kappa;
     K.w_long = P.w_long; K.w_clash_ln2 = P.w_clash * 0.6931471805599453f; K.w_hbond = P.w_hbond;
@@ -56,7 +60,7 @@ __device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.
 __device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 // Stage one ligand's topology into shared memory; returns the first byte after it (16-byte aligned).  The pair
-// records take their parameter-dependent form here (internal.h): c = dvdw + mu, dc = clash distance, 3 * b.
+// records take their parameter-dependent form here (internal.h): c = dvdw + mu, 3 * b | hbmask << 16.
 __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char* smem, const LigHdr* __restrict__ h,
                                                      const float4* __restrict__ atom_f4, const int* __restrict__ atom_i,
                                                      const LaneFrag* __restrict__ lane_frags, const uint4* __restrict__ lane_stream,
@@ -66,7 +70,8 @@ __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char*
     int* meta = reinterpret_cast<int*>(smem + 16 * (size_t)n);
     int* frag = reinterpret_cast<int*>(smem + 16 * (size_t)n + 16 * (size_t)((n + 3) / 4));
     uint4* stream = reinterpret_cast<uint4*>(reinterpret_cast<unsigned char*>(frag) + sizeof(LaneFrag) * (size_t)(T + 1));
-    uint4* recs = stream + ls;
+    float4* rec_c = reinterpret_cast<float4*>(stream + ls);
+    uint32_t* rec_m = reinterpret_cast<uint32_t*>(rec_c + nr);
     const LaneFrag* fsrc = lane_frags + h->frag_off;
     for (int i = tid; i < n; i += nt) ref[i] = __ldg(atom_f4 + h->atom_off + i);
     for (int i = tid; i < (T + 1) * (int)(sizeof(LaneFrag) / 4); i += nt) frag[i] = __ldg(reinterpret_cast<const int*>(fsrc) + i);
@@ -79,18 +84,13 @@ __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char*
         const uint4* src = reinterpret_cast<const uint4*>(lane_recs + h->rec_off + i);
         const uint4 dv = __ldg(src), mt = __ldg(src + 1);
         const float d[4] = {__uint_as_float(dv.x), __uint_as_float(dv.y), __uint_as_float(dv.z), __uint_as_float(dv.w)};
-        float c[4], dc[4];
+        float c[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const bool pair = d[k] >= 0.f, hb = (mt.y >> k) & 1u;
-            c[k] = pair ? d[k] + P.long_mu : -1e15f;
-            dc[k] = pair ? (hb ? P.hb_dclash : d[k]) : 0.f;
-        }
-        recs[3 * i] = make_uint4(__float_as_uint(c[0]), __float_as_uint(c[1]), __float_as_uint(c[2]), __float_as_uint(c[3]));
-        recs[3 * i + 1] = make_uint4(__float_as_uint(dc[0]), __float_as_uint(dc[1]), __float_as_uint(dc[2]), __float_as_uint(dc[3]));
-        recs[3 * i + 2] = make_uint4(3u * mt.x, mt.y, 0u, 0u);
+        for (int k = 0; k < 4; ++k) c[k] = d[k] >= 0.f ? d[k] + P.long_mu : -1e15f;
+        rec_c[i] = make_float4(c[0], c[1], c[2], c[3]);
+        rec_m[i] = 3u * mt.x | (mt.y << 16);
     }
-    S.ref = ref; S.meta = meta; S.frag = reinterpret_cast<const LaneFrag*>(frag); S.stream = stream; S.recs = recs; S.n = n; S.T = T;
+    S.ref = ref; S.meta = meta; S.frag = reinterpret_cast<const LaneFrag*>(frag); S.stream = stream; S.rec_c = rec_c; S.rec_m = rec_m; S.n = n; S.T = T;
     return smem + lane_topo_bytes(n, T, ls, nr);
 }
 
@@ -207,14 +207,20 @@ __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, fl
 // ------------------------------------------------------------------ a5 intra-ligand pairs (O2, O6)
 // One record: partner atom b against the 4 slots of a tile, branch-free so that the four evaluations interleave.
 //   L = -[d<dmax] exp(-(d-dvdw-mu)^2/(2 sigma^2))  (G1):  eL += [d<dmax] 2^(nk2 (d-c)^2),  c = dvdw + mu
-//   C = -[d<dc] ln(max(d,floor)/dc)                (G3, G4):  eC += lg2(max(dc / max(d,floor), 1))
+//   C = -[d<dc] ln(max(d,floor)/dc)                (G3, G4):  eC += lg2(max(dc / max(d,floor), 1)),
+//       dc = c - mu, or hb_dclash for a donor/acceptor pair
 //   H = -[hb, d<3.4] exp(-(d-2.88)^2/(2*0.3^2)):  eH += ..., only in records that hold such a pair
-// GRAD: f_i += s (x_a - x_b) with s = (de/dd) / d / kappa.  A slot without a pair has c = -1e15, dc = 0 and adds 0.
+// GRAD: f_i += s (x_a - x_b) with s = (de/dd) / d / kappa.  A slot without a pair has c = -1e15 and adds 0.
 template <bool GRAD>
 __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], const float ay[4], const float az[4],
-                                         float bx, float by, float bz, const float4 c4, const float4 dc4, unsigned hbmask,
+                                         float bx, float by, float bz, const float4 c4, unsigned hbmask,
                                          float& eL, float& eC, float& eH, float fx[4], float fy[4], float fz[4]) {
-    const float c[4] = {c4.x, c4.y, c4.z, c4.w}, dc[4] = {dc4.x, dc4.y, dc4.z, dc4.w};
+    const float c[4] = {c4.x, c4.y, c4.z, c4.w};
+    float dc[4] = {c4.x - K.mu, c4.y - K.mu, c4.z - K.mu, c4.w - K.mu};   // clash distance dvdw (negative: no pair)
+    if (hbmask) {                                                    // warp-uniform; about one record in three
+#pragma unroll
+        for (int i = 0; i < 4; ++i) dc[i] = ((hbmask >> i) & 1u) ? K.hb_dclash : dc[i];
+    }
     float dx[4], dy[4], dz[4], d[4], rinv[4], s[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -234,7 +240,7 @@ __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], cons
             if (q > 1.f && rinv[i] < K.inv_floor) s[i] = fmaf(-K.kc * rinv[i], rinv[i], s[i]);
         }
     }
-    if (hbmask) {                                                    // warp-uniform; about one record in three
+    if (hbmask) {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             if ((hbmask >> i) & 1u) {
@@ -253,9 +259,9 @@ __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], cons
 }
 
 // One tile: w <= 4 consecutive own atoms a0 .. a0+w-1 of fragment g against n_runs runs of partner atoms; hp / rp walk
-// the header units / the records.  GRAD: acc += the wrench the tile's atoms receive; WR[fb] -= each run's wrench.
+// the header units / the two record arrays.  GRAD: acc += the wrench the tile's atoms receive; WR[fb] -= each run's wrench.
 template <bool GRAD>
-__device__ __forceinline__ void lane_tile(const uint4*& hp, const uint4*& rp, int a0, int w, int n_runs, const PairK& K,
+__device__ __forceinline__ void lane_tile(const uint4*& hp, const float4*& rc, const uint32_t*& rm, int a0, int w, int n_runs, const PairK& K,
                                           const float* __restrict__ X, float* __restrict__ WR, int C,
                                           float acc[6], float& eL, float& eC, float& eH) {
     float ax[4], ay[4], az[4];
@@ -270,15 +276,13 @@ __device__ __forceinline__ void lane_tile(const uint4*& hp, const uint4*& rp, in
         float fx[4], fy[4], fz[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) fx[i] = fy[i] = fz[i] = 0.f;
-        for (int j = 0; j < nb; ++j, rp += 3) {
-            const uint4 c4 = rp[0], dc4 = rp[1];
-            const uint2 mt = *reinterpret_cast<const uint2*>(rp + 2);
-            const float* xb = X + (int)mt.x * C;
-            lane_rec<GRAD>(K, ax, ay, az, xb[0], xb[C], xb[2 * C],
-                           make_float4(__uint_as_float(c4.x), __uint_as_float(c4.y), __uint_as_float(c4.z), __uint_as_float(c4.w)),
-                           make_float4(__uint_as_float(dc4.x), __uint_as_float(dc4.y), __uint_as_float(dc4.z), __uint_as_float(dc4.w)),
-                           mt.y, eL, eC, eH, fx, fy, fz);
+        for (int j = 0; j < nb; ++j) {
+            const float4 c4 = rc[j];
+            const uint32_t mt = rm[j];
+            const float* xb = X + (int)(mt & 0xffffu) * C;
+            lane_rec<GRAD>(K, ax, ay, az, xb[0], xb[C], xb[2 * C], c4, mt >> 16, eL, eC, eH, fx, fy, fz);
         }
+        rc += nb; rm += nb;
         if (GRAD) {
             float wv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -305,14 +309,15 @@ __device__ __forceinline__ float lane_pairs(const LaneTopo& S, const PairK& K, c
                                             float* __restrict__ WR, int C) {
     float eL = 0.f, eC = 0.f, eH = 0.f;
     const uint4* hp = S.stream;
-    const uint4* rp = S.recs;
+    const float4* rc = S.rec_c;
+    const uint32_t* rm = S.rec_m;
     for (int g = 0; g <= S.T; ++g) {
         const int n_tiles = (int)(*hp++).x;
         if (n_tiles == 0) continue;
         float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         for (int tl = 0; tl < n_tiles; ++tl) {
             const uint4 h = *hp++;
-            lane_tile<GRAD>(hp, rp, (int)h.x, (int)h.y, (int)h.z, K, X, WR, C, acc, eL, eC, eH);
+            lane_tile<GRAD>(hp, rc, rm, (int)h.x, (int)h.y, (int)h.z, K, X, WR, C, acc, eL, eC, eH);
         }
         if (GRAD) {
             float* wg = WR + 6 * g * C;
@@ -540,6 +545,8 @@ cudaError_t mc_lane_prepare(size_t max_smem_bytes) {
     if (g_lane_prepared) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute(mc_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(score_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
+    // residency is bound by shared memory (the chains' coordinates): take the whole 228 KB, the grid gathers live in L2 anyway
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e == cudaSuccess) g_lane_prepared = true;
     return e;
 }
