@@ -97,6 +97,19 @@ extern "C" int tridsk_create(tridsk_ctx** out, int device, void* cuda_stream) {
         if (e != cudaSuccess) { fprintf(stderr, "tridsk_create: %s\n", cudaGetErrorString(e)); delete ctx; return TRIDSK_ECUDA; }
         ctx->own_stream = true;
     }
+    {
+        cudaMemPoolProps pp;
+        memset(&pp, 0, sizeof(pp));
+        pp.allocType = cudaMemAllocationTypePinned;
+        pp.location.type = cudaMemLocationTypeDevice;
+        pp.location.id = device;
+        e = cudaMemPoolCreate(&ctx->pool, &pp);
+        if (e == cudaSuccess) {
+            unsigned long long keep = ~0ULL;
+            e = cudaMemPoolSetAttribute(ctx->pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        if (e != cudaSuccess) { fprintf(stderr, "tridsk_create: %s\n", cudaGetErrorString(e)); tridsk_destroy(ctx); return TRIDSK_ECUDA; }
+    }
     *out = ctx;
     return TRIDSK_OK;
 }
@@ -104,6 +117,8 @@ extern "C" int tridsk_create(tridsk_ctx** out, int device, void* cuda_stream) {
 extern "C" void tridsk_destroy(tridsk_ctx* ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
+    *ctx->alive = false;
+    if (ctx->pool) cudaMemPoolDestroy(ctx->pool);   // outstanding grids keep their memory until they are freed
     if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
     for (int i = 0; i < 3; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     if (ctx->fork_ev) cudaEventDestroy(ctx->fork_ev);
@@ -137,14 +152,19 @@ static int new_grid(tridsk_ctx* ctx, int n_types, const float origin[3], const i
     if (n_types > TRIDSK_MAX_TYPES) return fail(ctx, TRIDSK_ELIMIT, "n_types > 32");
     tridsk_grid* g = new (std::nothrow) tridsk_grid();
     if (!g) return fail(ctx, TRIDSK_ENOMEM, "host alloc");
-    g->ctx = ctx;
+    g->ctx = ctx; g->ctx_alive = ctx->alive;
     g->d.nx = dims[0]; g->d.ny = dims[1]; g->d.nz = dims[2]; g->d.n_types = n_types;
     g->d.plane = (size_t)dims[0] * dims[1] * dims[2];
     g->d.ox = origin[0]; g->d.oy = origin[1]; g->d.oz = origin[2];
     g->d.h = spacing; g->d.inv_h = 1.0f / spacing;
-    cudaError_t e = cudaMalloc(&g->g, sizeof(float) * g->d.plane * n_types);
-    if (e == cudaSuccess) e = cudaMalloc(&g->gp, sizeof(float4) * g->d.plane * n_types);   // xy-packed copy (DGrid::gp)
-    if (e != cudaSuccess) { cudaFree(g->g); delete g; return fail(ctx, TRIDSK_ENOMEM, std::string("grid alloc: ") + cudaGetErrorString(e)); }
+    cudaError_t e = cudaMallocFromPoolAsync((void**)&g->g, sizeof(float) * g->d.plane * n_types, ctx->pool, ctx->stream);
+    if (e == cudaSuccess)                                                                  // xy-packed copy (DGrid::gp)
+        e = cudaMallocFromPoolAsync((void**)&g->gp, sizeof(float4) * g->d.plane * n_types, ctx->pool, ctx->stream);
+    if (e != cudaSuccess) {
+        if (g->g) cudaFreeAsync(g->g, ctx->stream);
+        delete g;
+        return fail(ctx, TRIDSK_ENOMEM, std::string("grid alloc: ") + cudaGetErrorString(e));
+    }
     g->d.g = g->g; g->d.gp = g->gp;
     *out = g;
     return TRIDSK_OK;
@@ -158,21 +178,6 @@ extern "C" int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const in
     int rc = check_types(ctx, types);
     if (rc) return rc;
     const int nt = types->n_types;
-    // receptor atoms -> float4 {x, y, z, type bits}: layout only (staged on the host; n_rec is a few thousand)
-    std::vector<float> xyz(3 * (size_t)n_rec);
-    std::vector<int> typ(n_rec);
-    if (n_rec) {
-        CK(cudaMemcpyAsync(xyz.data(), rec_xyz, sizeof(float) * 3 * n_rec, cudaMemcpyDefault, ctx->stream));
-        CK(cudaMemcpyAsync(typ.data(), rec_type, sizeof(int) * n_rec, cudaMemcpyDefault, ctx->stream));
-        CK(cudaStreamSynchronize(ctx->stream));
-    }
-    std::vector<float4> rec(n_rec);
-    for (int a = 0; a < n_rec; ++a) {
-        if (typ[a] < 0 || typ[a] >= nt) return fail(ctx, TRIDSK_EINVAL, "receptor atom type out of range");
-        float tbits;
-        memcpy(&tbits, &typ[a], sizeof(float));
-        rec[a] = make_float4(xyz[3 * a], xyz[3 * a + 1], xyz[3 * a + 2], tbits);
-    }
     // type-pair table: operands of the pair function, not results
     std::vector<float> tab(4 * (size_t)nt * nt);
     float dc_max = params->hb_dmax;
@@ -189,21 +194,34 @@ extern "C" int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const in
     tridsk_grid* g = nullptr;
     rc = new_grid(ctx, nt, origin, dims, spacing, &g);
     if (rc) return rc;
-    void *d_rec, *d_tab;
-    if ((rc = scratch(ctx, 0, sizeof(float4) * std::max(n_rec, 1), &d_rec)) || (rc = scratch(ctx, 1, sizeof(float) * tab.size(), &d_tab))) {
-        tridsk_free_grid(g);
-        return rc;
-    }
+    // scratch 0: [bad flag (16 B) | float4 rec[n_rec]], scratch 1: table, scratch 4: staged host inputs
+    char* d_rec0; void* d_tab;
+    const void *d_xyz = nullptr, *d_typ = nullptr;
+    if ((rc = scratch(ctx, 0, 16 + sizeof(float4) * std::max(n_rec, 1), (void**)&d_rec0)) ||
+        (rc = scratch(ctx, 1, sizeof(float) * tab.size(), &d_tab))) { tridsk_free_grid(g); return rc; }
+    const size_t b_xyz = (sizeof(float) * 3 * (size_t)n_rec + 15) / 16 * 16;
+    const bool h_xyz = n_rec && !is_device_ptr(rec_xyz), h_typ = n_rec && !is_device_ptr(rec_type);
+    char* stage = nullptr;
+    if ((h_xyz || h_typ) && (rc = scratch(ctx, 4, b_xyz + sizeof(int) * n_rec, (void**)&stage))) { tridsk_free_grid(g); return rc; }
     DParams P;
     to_dparams(params, &P);
-    cudaError_t e = cudaSuccess;
-    if (n_rec) e = cudaMemcpyAsync(d_rec, rec.data(), sizeof(float4) * n_rec, cudaMemcpyHostToDevice, ctx->stream);
+    int* d_bad = (int*)d_rec0;
+    float4* d_rec = (float4*)(d_rec0 + 16);
+    cudaError_t e = cudaMemsetAsync(d_bad, 0, sizeof(int), ctx->stream);
+    if (e == cudaSuccess && h_xyz) e = cudaMemcpyAsync(stage, rec_xyz, sizeof(float) * 3 * n_rec, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess && h_typ) e = cudaMemcpyAsync(stage + b_xyz, rec_type, sizeof(int) * n_rec, cudaMemcpyHostToDevice, ctx->stream);
+    d_xyz = h_xyz ? (const void*)stage : (const void*)rec_xyz;
+    d_typ = h_typ ? (const void*)(stage + b_xyz) : (const void*)rec_type;
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_tab, tab.data(), sizeof(float) * tab.size(), cudaMemcpyHostToDevice, ctx->stream);
-    if (e == cudaSuccess) e = launch_grid_build(ctx->stream, (const float4*)d_rec, n_rec, (const float*)d_tab, nt, P, g->d, dc_max, g->g);
+    if (e == cudaSuccess) e = launch_rec_pack(ctx->stream, (const float*)d_xyz, (const int*)d_typ, n_rec, nt, d_rec, d_bad);
+    if (e == cudaSuccess) e = launch_grid_build(ctx->stream, d_rec, n_rec, (const float*)d_tab, nt, P, g->d, dc_max, g->g);
     if (e == cudaSuccess) e = launch_grid_pack(ctx->stream, g->d, g->gp);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);     // host staging vectors die at return
+    int bad = 0;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);     // host staging (tab, bad) dies at return
     if (e != cudaSuccess) { tridsk_free_grid(g); return fail(ctx, TRIDSK_ECUDA, std::string("build_grid: ") + cudaGetErrorString(e)); }
-    ctx->launches += 2;
+    ctx->launches += 2 + (n_rec > 0 ? 1 : 0);
+    if (bad) { tridsk_free_grid(g); return fail(ctx, TRIDSK_EINVAL, "receptor atom type out of range"); }
     *out = g;
     return TRIDSK_OK;
 }
@@ -233,8 +251,13 @@ extern "C" int tridsk_grid_export(tridsk_ctx* ctx, const tridsk_grid* grid, floa
 
 extern "C" void tridsk_free_grid(tridsk_grid* g) {
     if (!g) return;
-    if (g->g) cudaFree(g->g);       // cudaFree waits for the device; g->ctx may already be destroyed
-    if (g->gp) cudaFree(g->gp);
+    if (g->ctx_alive && *g->ctx_alive) {             // stream-ordered: later work on the ctx stream may reuse the memory
+        if (g->g) cudaFreeAsync(g->g, g->ctx->stream);
+        if (g->gp) cudaFreeAsync(g->gp, g->ctx->stream);
+    } else {                                        // the ctx is gone: cudaFree waits for the device
+        if (g->g) cudaFree(g->g);
+        if (g->gp) cudaFree(g->gp);
+    }
     delete g;
 }
 

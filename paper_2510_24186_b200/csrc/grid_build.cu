@@ -1,45 +1,93 @@
 // grid_build.cu -- hot-path step a0: receptor grid precompute (O3/O4).
 //
 // G[t][k][j][i] = sum_a e(s_a, t, |x_node - r_a|).  One thread per grid node accumulates ALL ligand types in
-// registers (the distance to a receptor atom is type-independent; only d_vdw and the donor/acceptor flag
-// change), receptor atoms are staged through shared memory in chunks and read as warp broadcasts, and each
-// type plane is written with unit-stride stores along x.  Receptor atoms are visited in input order, so the
-// fp32 sums are reproducible.  The bound is the XU/FP32 pipes (one ex2 per node-atom-type triple), not memory.
+// registers (the distance to a receptor atom is type-independent; only d_vdw and the donor/acceptor flag change).
+// A CTA owns a compact brick of 8 x 4 x 4 nodes (a warp: 8 x 2 x 2), so that the atoms within the 10 A cut-off of
+// one lane are nearly those of the whole warp.  Receptor atoms stream through in chunks: the CTA first culls a chunk
+// against the brick's bounding sphere (ordered compaction, so atoms are still visited in input order and the fp32
+// sums are reproducible), then every thread walks the survivors as warp broadcasts from shared memory.
+// The bound is the XU pipe (one ex2 per node-atom-type triple), not memory: the grid is written once.
 #include <algorithm>
 
 #include "internal.h"
 
-#define GB_BX 32
+#define GB_BX 8
 #define GB_BY 4
-#define GB_CHUNK 512
+#define GB_BZ 4
+#define GB_THREADS (GB_BX * GB_BY * GB_BZ)
+#define GB_CHUNK 1024
+
+__device__ __forceinline__ float exp2f_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// {x, y, z, type bits} per receptor atom; *bad is set if a type is out of range (the atom is then skipped)
+__global__ void rec_pack_kernel(const float* __restrict__ xyz, const int* __restrict__ type, int n_rec, int n_types,
+                                float4* __restrict__ out, int* __restrict__ bad) {
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= n_rec) return;
+    int t = type[a];
+    if (t < 0 || t >= n_types) { *bad = 1; t = -1; }
+    out[a] = make_float4(xyz[3 * a], xyz[3 * a + 1], xyz[3 * a + 2], __int_as_float(t));
+}
 
 // pair_tab[s][t] = {d_vdw + mu, d_clash (2.6 for donor/acceptor pairs else d_vdw), hb flag, 1/d_clash}
 template <int NT>
-__global__ void __launch_bounds__(GB_BX * GB_BY) grid_build_kernel(const float4* __restrict__ rec, int n_rec,
-                                                                   const float4* __restrict__ pair_tab, int n_types,
-                                                                   const DParams P, const DGrid G, float dc_max,
-                                                                   float* __restrict__ out) {
+__global__ void __launch_bounds__(GB_THREADS) grid_build_kernel(const float4* __restrict__ rec, int n_rec,
+                                                                const float4* __restrict__ pair_tab, int n_types,
+                                                                const DParams P, const DGrid G, float dc_max,
+                                                                float* __restrict__ out) {
     __shared__ float4 s_atom[GB_CHUNK];
     __shared__ float4 s_tab[TRIDSK_MAX_TYPES * NT];
-    const int tid = threadIdx.y * GB_BX + threadIdx.x;
-    for (int i = tid; i < n_types * NT; i += GB_BX * GB_BY) {
+    __shared__ __align__(16) float s_c[TRIDSK_MAX_TYPES * NT];      // d_vdw + mu alone: what the common case reads
+    __shared__ int s_warp[GB_THREADS / 32 + 1];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int i = tid; i < n_types * NT; i += GB_THREADS) {
         const int s = i / NT, t = i % NT;
-        s_tab[i] = t < n_types ? pair_tab[s * n_types + t] : make_float4(0.f, 0.f, 0.f, 1.f);
+        const float4 e = t < n_types ? pair_tab[s * n_types + t] : make_float4(1e15f, 0.f, 0.f, 1.f);
+        s_tab[i] = e; s_c[i] = e.x;
     }
-    const int ix = blockIdx.x * GB_BX + threadIdx.x, iy = blockIdx.y * GB_BY + threadIdx.y, iz = blockIdx.z;
-    const bool in = ix < G.nx && iy < G.ny;
+    // node of this thread: warp = 8 x 2 x 2 sub-brick, the CTA's 4 warps tile 8 x 4 x 4
+    const int lx = lane & 7, ly = ((lane >> 3) & 1) + 2 * (warp & 1), lz = (lane >> 4) + 2 * (warp >> 1);
+    const int ix = blockIdx.x * GB_BX + lx, iy = blockIdx.y * GB_BY + ly, iz = blockIdx.z * GB_BZ + lz;
+    const bool in = ix < G.nx && iy < G.ny && iz < G.nz;
     const float x = G.ox + G.h * (float)ix, y = G.oy + G.h * (float)iy, z = G.oz + G.h * (float)iz;
-    float acc[NT];
+    // bounding sphere of the brick
+    const float hx = 0.5f * G.h * (float)(GB_BX - 1), hy = 0.5f * G.h * (float)(GB_BY - 1), hz = 0.5f * G.h * (float)(GB_BZ - 1);
+    const float cx = G.ox + G.h * (float)(blockIdx.x * GB_BX) + hx, cy = G.oy + G.h * (float)(blockIdx.y * GB_BY) + hy;
+    const float cz = G.oz + G.h * (float)(blockIdx.z * GB_BZ) + hz;
+    const float rc = P.long_dmax + sqrtf(hx * hx + hy * hy + hz * hz) + 1e-3f;
+    const float rc2 = rc * rc;
+
+    float acc[NT], accx[NT];                       // acc: sum of 2^(...) Gaussians (scaled by -w_long at the end); accx: the rest
 #pragma unroll
-    for (int t = 0; t < NT; ++t) acc[t] = 0.f;
+    for (int t = 0; t < NT; ++t) { acc[t] = 0.f; accx[t] = 0.f; }
     const float dmax2 = P.long_dmax * P.long_dmax;
+    const float nk2 = -P.long_inv_two_sigma2 * 1.4426950408889634f;
 
     for (int base = 0; base < n_rec; base += GB_CHUNK) {
+        // ---- cull this chunk against the brick's sphere, keeping input order
         __syncthreads();
-        for (int i = tid; i < GB_CHUNK && base + i < n_rec; i += GB_BX * GB_BY) s_atom[i] = rec[base + i];
-        __syncthreads();
-        const int cnt = min(GB_CHUNK, n_rec - base);
-        for (int a = 0; a < cnt; ++a) {
+        int n_keep = 0;
+        for (int r0 = 0; r0 < GB_CHUNK && base + r0 < n_rec; r0 += GB_THREADS) {
+            const int a = base + r0 + tid;
+            float4 ra = make_float4(0.f, 0.f, 0.f, 0.f);
+            bool keep = false;
+            if (a < n_rec) {
+                ra = __ldg(rec + a);
+                const float dx = ra.x - cx, dy = ra.y - cy, dz = ra.z - cz;
+                keep = (dx * dx + dy * dy + dz * dz < rc2) && (__float_as_int(ra.w) >= 0);
+            }
+            const unsigned m = __ballot_sync(0xffffffffu, keep);
+            if (lane == 0) s_warp[warp] = __popc(m);
+            __syncthreads();
+            int off = n_keep, total = 0;
+#pragma unroll
+            for (int w = 0; w < GB_THREADS / 32; ++w) { const int c = s_warp[w]; if (w < warp) off += c; total += c; }
+            if (keep) s_atom[off + __popc(m & ((1u << lane) - 1u))] = ra;
+            n_keep += total;
+            __syncthreads();
+        }
+        // ---- every node against the survivors
+        for (int a = 0; a < n_keep; ++a) {
             const float4 ra = s_atom[a];
             const float dx = x - ra.x, dy = y - ra.y, dz = z - ra.z;
             const float d2 = dx * dx + dy * dy + dz * dz;
@@ -47,26 +95,30 @@ __global__ void __launch_bounds__(GB_BX * GB_BY) grid_build_kernel(const float4*
             const float rinv = rsqrtf(fmaxf(d2, 1e-12f));
             const float d = d2 * rinv;
             if (!(d < P.long_dmax)) continue;
-            const float4* row = s_tab + __float_as_int(ra.w) * NT;
-            if (d >= dc_max) {                      // common case: only the long-range Gaussian can act
+            const int s = __float_as_int(ra.w);
+            const float4* crow = reinterpret_cast<const float4*>(s_c + s * NT);
 #pragma unroll
-                for (int t = 0; t < NT; ++t) {
-                    const float u = d - row[t].x;
-                    acc[t] -= P.w_long * __expf(-u * u * P.long_inv_two_sigma2);
-                }
-            } else {
+            for (int t4 = 0; t4 < NT / 4; ++t4) {
+                const float4 c = crow[t4];
+                const float u0 = d - c.x, u1 = d - c.y, u2 = d - c.z, u3 = d - c.w;
+                acc[4 * t4 + 0] += exp2f_approx(u0 * (u0 * nk2));
+                acc[4 * t4 + 1] += exp2f_approx(u1 * (u1 * nk2));
+                acc[4 * t4 + 2] += exp2f_approx(u2 * (u2 * nk2));
+                acc[4 * t4 + 3] += exp2f_approx(u3 * (u3 * nk2));
+            }
+            if (d < dc_max) {                       // rare: clash and / or hydrogen-bond range of some type
+                const float4* row = s_tab + s * NT;
                 const float dfl = fmaxf(d, P.d_floor);
 #pragma unroll
                 for (int t = 0; t < NT; ++t) {
                     const float4 c = row[t];
-                    const float u = d - c.x;
-                    float e = -P.w_long * __expf(-u * u * P.long_inv_two_sigma2);
+                    float e = 0.f;
                     if (d < c.y) e -= P.w_clash * __logf(dfl * c.w);
                     if (c.z != 0.f && d < P.hb_dmax) {
                         const float w = d - P.hb_mu;
                         e -= P.w_hbond * __expf(-w * w * P.hb_inv_two_sigma2);
                     }
-                    acc[t] += e;
+                    accx[t] += e;
                 }
             }
         }
@@ -75,18 +127,24 @@ __global__ void __launch_bounds__(GB_BX * GB_BY) grid_build_kernel(const float4*
         const size_t node = ((size_t)iz * G.ny + iy) * G.nx + ix;
 #pragma unroll
         for (int t = 0; t < NT; ++t)
-            if (t < n_types) out[(size_t)t * G.plane + node] = acc[t];
+            if (t < n_types) out[(size_t)t * G.plane + node] = fmaf(-P.w_long, acc[t], accx[t]);
     }
+}
+
+cudaError_t launch_rec_pack(cudaStream_t s, const float* xyz, const int* type, int n_rec, int n_types, float4* out, int* bad) {
+    if (n_rec <= 0) return cudaSuccess;
+    rec_pack_kernel<<<(n_rec + 255) / 256, 256, 0, s>>>(xyz, type, n_rec, n_types, out, bad);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_grid_build(cudaStream_t s, const float4* rec, int n_rec, const float* pair_tab, int n_types,
                               const DParams& P, DGrid grid, float dc_max, float* out) {
     // dc_max >= every d_clash and hb_dmax: beyond it only the long-range Gaussian can act
-    const dim3 block(GB_BX, GB_BY), g((grid.nx + GB_BX - 1) / GB_BX, (grid.ny + GB_BY - 1) / GB_BY, grid.nz);
+    const dim3 g((grid.nx + GB_BX - 1) / GB_BX, (grid.ny + GB_BY - 1) / GB_BY, (grid.nz + GB_BZ - 1) / GB_BZ);
     const float4* tab = reinterpret_cast<const float4*>(pair_tab);
-    if (n_types <= 8) grid_build_kernel<8><<<g, block, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, out);
-    else if (n_types <= 16) grid_build_kernel<16><<<g, block, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, out);
-    else grid_build_kernel<32><<<g, block, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, out);
+    if (n_types <= 8) grid_build_kernel<8><<<g, GB_THREADS, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, out);
+    else if (n_types <= 16) grid_build_kernel<16><<<g, GB_THREADS, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, out);
+    else grid_build_kernel<32><<<g, GB_THREADS, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, out);
     return cudaGetLastError();
 }
 

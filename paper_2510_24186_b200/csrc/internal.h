@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <memory>
 #include <string>
 #include <vector>
 
@@ -196,11 +197,15 @@ struct tridsk_ctx {
     cudaStream_t side[TRIDSK_BRANCHES] = {};           // side[0] unused
     cudaEvent_t fork_ev = nullptr, join_ev[TRIDSK_BRANCHES] = {};
     int kernel = 0;               // tridsk_set_kernel: 0 auto, 1 warp per chain, 2 lane per chain
+    // grids come from a stream-ordered pool that keeps its memory (a screen rebuilds same-sized grids per receptor)
+    cudaMemPool_t pool = nullptr;
+    std::shared_ptr<bool> alive = std::make_shared<bool>(true);   // handles that outlive the ctx free synchronously
     int last_kernel = 0;          // what the last dock used
 };
 
 struct tridsk_grid {
     tridsk_ctx* ctx;
+    std::shared_ptr<bool> ctx_alive;
     float* g = nullptr;
     float4* gp = nullptr;
     DGrid d;
@@ -229,6 +234,7 @@ struct tridsk_ligands {
 };
 
 // ---------------------------------------------------------------- kernel launchers (one per .cu)
+cudaError_t launch_rec_pack(cudaStream_t s, const float* xyz, const int* type, int n_rec, int n_types, float4* out, int* bad);
 cudaError_t launch_grid_build(cudaStream_t s, const float4* rec /* x,y,z,type */, int n_rec,
                               const float* pair_tab /* [n_types][n_types][4] */, int n_types,
                               const DParams& P, DGrid grid, float dc_max, float* out);
