@@ -178,10 +178,11 @@ int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* 
                 float* out_energy, float* out_pose, int* out_chain, const tridsk_dock_opts* opts);
 
 /*
- * Chain-to-thread mapping of the fused kernel: 0 = automatic (a warp per chain when chains are few,
- * a lane per chain when n_lig * n_chains >= 256 per SM), 1 = always a warp per chain, 2 = always a lane per chain.
- * Applies to tridsk_dock and tridsk_score_grad on this ctx.  Both mappings compute O1..O13; their fp32 summation
- * orders differ, so chains are bit-reproducible per mapping, not across mappings.
+ * Chain-to-thread mapping of the fused kernel: 0 = automatic (a CTA per chain for a single dock with
+ * at most 8 chains per SM, a lane per chain when n_lig * n_chains >= 256 per SM, a warp per chain in between), 1 = always
+ * a warp per chain, 2 = always a lane per chain, 3 = always a CTA per chain (batches of at most 1024 ligands).
+ * Applies to tridsk_dock and tridsk_score_grad on this ctx.  All mappings compute O1..O13; their fp32 summation orders
+ * differ, so chains are bit-reproducible per mapping, not across mappings.
  */
 int tridsk_set_kernel(tridsk_ctx* ctx, int kernel);
 

@@ -271,12 +271,14 @@ struct PackedLig {
     std::vector<LaneFrag> lane_frags;   // lane format (internal.h): fragments in pre-order
     std::vector<uint4> lane_stream;     // lane format: the pair instruction stream (header units)
     std::vector<LaneRec> lane_recs;     // lane format: the pair records, in stream order
+    std::vector<int> cta_rows;          // CTA format (internal.h): n + 1 row offsets
+    std::vector<uint2> cta_recs;        // CTA format: 2 P row records, then P flat records
     int err = 0;
     const char* msg = "";
 };
 
 // Host-side packing of one ligand: validation, depth-first atom order, fragment records, pair schedule.
-static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types, int i, PackedLig& out) {
+static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types, int i, bool want_cta, PackedLig& out) {
     const int a0 = b->atom_off[i], n = b->atom_off[i + 1] - a0;
     const int t0 = b->tor_off[i], T = b->tor_off[i + 1] - t0;
     auto bad = [&](int code, const char* m) { out.err = code; out.msg = m; };
@@ -458,6 +460,28 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
         h.ls_len = (int)out.lane_stream.size();
         h.n_rec = (int)out.lane_recs.size();
     }
+    // CTA format (internal.h): row form (every pair from both ends) + flat form (every pair once), internal indices
+    if (want_cta) {
+        auto hbq = [&](int x, int y) {
+            const unsigned char rs = types->hb_role[out.ai[x] & 0xff], rt = types->hb_role[out.ai[y] & 0xff];
+            return ((rs & 1) && (rt & 2)) || ((rs & 2) && (rt & 1));
+        };
+        auto fbits = [](float v) { unsigned u; memcpy(&u, &v, sizeof(u)); return u; };
+        out.cta_rows.assign(n + 1, 0);
+        for (int x = 0; x < n; ++x) {
+            out.cta_rows[x] = (int)out.cta_recs.size();
+            for (int y = 0; y < n; ++y)
+                if (y != x && pm[(size_t)x * n + y])
+                    out.cta_recs.push_back(make_uint2((unsigned)y | (hbq(x, y) ? 0x100u : 0u), fbits(out.f4[x].w + out.f4[y].w)));
+        }
+        out.cta_rows[n] = (int)out.cta_recs.size();
+        for (int x = 0; x < n; ++x)
+            for (int y = x + 1; y < n; ++y)
+                if (pm[(size_t)x * n + y])
+                    out.cta_recs.push_back(make_uint2((unsigned)x | ((unsigned)y << 8) | (hbq(x, y) ? 0x10000u : 0u),
+                                                      fbits(out.f4[x].w + out.f4[y].w)));
+        if ((int)out.cta_recs.size() != 3 * P) return bad(TRIDSK_EINVAL, "internal: CTA pair records do not cover the pair set");
+    }
     // conflict-free schedule: round (j1, j2, k): lane l <-> pair (j1*S + l, j2*S + (l+k) mod S)
     auto hb = [&](int x, int y) {
         const unsigned char rs = types->hb_role[out.ai[x] & 0xff], rt = types->hb_role[out.ai[y] & 0xff];
@@ -496,24 +520,35 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
         return fail(ctx, TRIDSK_EINVAL, "bad ligand batch");
     const int L = b->n_lig;
     std::vector<PackedLig> pk(L);
+    // the CTA-per-chain format triples the pair storage: it is the single-dock mapping, so screens do not carry it
+    const bool want_cta = L <= TRIDSK_CTA_MAX_LIG;
 #pragma omp parallel for schedule(dynamic, 16)
-    for (int i = 0; i < L; ++i) pack_ligand(b, types, i, pk[i]);
+    for (int i = 0; i < L; ++i) pack_ligand(b, types, i, want_cta, pk[i]);
     for (int i = 0; i < L; ++i)
         if (pk[i].err) return fail(ctx, pk[i].err, std::string("ligand ") + std::to_string(i) + ": " + pk[i].msg);
 
     tridsk_ligands* lg = new (std::nothrow) tridsk_ligands();
     if (!lg) return fail(ctx, TRIDSK_ENOMEM, "host alloc");
-    lg->ctx = ctx; lg->n_lig = L;
-    size_t na = 0, nf = 0, nr = 0, nls = 0, nrec = 0;
+    lg->ctx = ctx; lg->n_lig = L; lg->has_cta = want_cta;
+    size_t na = 0, nf = 0, nr = 0, nls = 0, nrec = 0, ncr = 0, ncc = 0;
     lg->hdr_h.resize(L); lg->n_pairs.resize(L);
     for (int i = 0; i < L; ++i) {
         LigHdr& h = pk[i].h;
         h.atom_off = (int)na; h.frag_off = (int)nf; h.round_off = (int)nr; h.ls_off = (int)nls; h.rec_off = (int)nrec;
+        h.cta_row_off = (int)ncr; h.cta_rec_off = (int)ncc;
         na += pk[i].f4.size(); nf += pk[i].fr.size(); nr += pk[i].rounds.size();
         nls += pk[i].lane_stream.size(); nrec += pk[i].lane_recs.size();
+        ncr += pk[i].cta_rows.size(); ncc += pk[i].cta_recs.size();
         lg->hdr_h[i] = h; lg->n_pairs[i] = h.n_pairs;
         lg->max_atoms = std::max(lg->max_atoms, h.n); lg->max_tor = std::max(lg->max_tor, h.T);
         lg->bucket[h.J].push_back(i);
+        if (want_cta) {
+            int th, lpa;
+            cta_shape(h.n, &th, &lpa);
+            const int k = th == 128 ? 0 : 1;
+            lg->cta_bucket[k].push_back(i);
+            lg->cta_smem[k] = std::max(lg->cta_smem[k], cta_layout(h.n, h.T, h.n_pairs).total);
+        }
     }
     std::vector<float4> f4(na);
     std::vector<int> ai(na);
@@ -522,11 +557,15 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     std::vector<LaneFrag> lf(nf);
     std::vector<uint4> lsv(std::max<size_t>(nls, 1));
     std::vector<LaneRec> lrv(std::max<size_t>(nrec, 1));
+    std::vector<int> crv(std::max<size_t>(ncr, 1));
+    std::vector<uint2> ccv(std::max<size_t>(ncc, 1));
     for (int i = 0; i < L; ++i) {
         const LigHdr& h = pk[i].h;
         std::copy(pk[i].lane_frags.begin(), pk[i].lane_frags.end(), lf.begin() + h.frag_off);
         std::copy(pk[i].lane_stream.begin(), pk[i].lane_stream.end(), lsv.begin() + h.ls_off);
         std::copy(pk[i].lane_recs.begin(), pk[i].lane_recs.end(), lrv.begin() + h.rec_off);
+        std::copy(pk[i].cta_rows.begin(), pk[i].cta_rows.end(), crv.begin() + h.cta_row_off);
+        std::copy(pk[i].cta_recs.begin(), pk[i].cta_recs.end(), ccv.begin() + h.cta_rec_off);
         std::copy(pk[i].f4.begin(), pk[i].f4.end(), f4.begin() + h.atom_off);
         std::copy(pk[i].ai.begin(), pk[i].ai.end(), ai.begin() + h.atom_off);
         std::copy(pk[i].fr.begin(), pk[i].fr.end(), fr.begin() + h.frag_off);
@@ -546,6 +585,10 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     up((void**)&lg->lane_frags, lf.data(), sizeof(LaneFrag) * nf);
     up((void**)&lg->lane_stream, lsv.data(), sizeof(uint4) * lsv.size());
     up((void**)&lg->lane_recs, lrv.data(), sizeof(LaneRec) * lrv.size());
+    up((void**)&lg->cta_rows, crv.data(), sizeof(int) * crv.size());
+    up((void**)&lg->cta_recs, ccv.data(), sizeof(uint2) * ccv.size());
+    for (int k = 0; k < 2; ++k)
+        if (!lg->cta_bucket[k].empty()) up((void**)&lg->cta_bucket_dev[k], lg->cta_bucket[k].data(), sizeof(int) * lg->cta_bucket[k].size());
     if (e == cudaSuccess) e = cudaMalloc((void**)&lg->all_ids, sizeof(int) * std::max(L, 1));
     for (int j = 1; j <= TRIDSK_MAX_J; ++j)
         if (!lg->bucket[j].empty()) up((void**)&lg->bucket_dev[j], lg->bucket[j].data(), sizeof(int) * lg->bucket[j].size());
@@ -570,7 +613,8 @@ extern "C" int tridsk_ligand_info(const tridsk_ligands* l, int* n_lig, int* max_
 extern "C" void tridsk_free_ligands(tridsk_ligands* l) {
     if (!l) return;                 // cudaFree waits for the device; l->ctx may already be destroyed
     cudaFree(l->hdr); cudaFree(l->atom_f4); cudaFree(l->atom_i); cudaFree(l->frags); cudaFree(l->rounds);
-    cudaFree(l->lane_frags); cudaFree(l->lane_stream); cudaFree(l->lane_recs); cudaFree(l->all_ids);
+    cudaFree(l->lane_frags); cudaFree(l->lane_stream); cudaFree(l->lane_recs); cudaFree(l->cta_rows); cudaFree(l->cta_recs); cudaFree(l->all_ids);
+    for (int k = 0; k < 2; ++k) if (l->cta_bucket_dev[k]) cudaFree(l->cta_bucket_dev[k]);
     for (int j = 0; j <= TRIDSK_MAX_J; ++j) if (l->bucket_dev[j]) cudaFree(l->bucket_dev[j]);
     delete l;
 }
@@ -595,6 +639,7 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
     memset(&a, 0, sizeof(a));
     a.hdr = ligs->hdr; a.atom_f4 = ligs->atom_f4; a.atom_i = ligs->atom_i; a.frags = ligs->frags; a.rounds = ligs->rounds;
     a.lane_frags = ligs->lane_frags; a.lane_stream = ligs->lane_stream; a.lane_recs = ligs->lane_recs;
+    a.cta_rows = ligs->cta_rows; a.cta_recs = ligs->cta_recs;
     a.grid = grid->d;
     to_dparams(params, &a.P);
     a.n_pose = n_pose; a.pose_stride = pose_stride; a.grad_stride = grad_stride; a.coord_stride = coord_stride;
@@ -645,6 +690,11 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
         CK(cudaMemcpyAsync(d_seg, seg.data(), sizeof(int) * seg.size(), cudaMemcpyHostToDevice, ctx->stream));
         a.seg_lig = d_seg; a.seg_start = d_seg + ns; a.seg_cnt = d_seg + 2 * ns; a.perm = d_seg + 3 * ns;
         CK(launch_score_lane(ctx->stream, a, ns, smem));
+    } else if (ctx->kernel == 3) {
+        if (!ligs->has_cta) return fail(ctx, TRIDSK_EINVAL, "the CTA-per-chain mapping needs a ligand batch of at most 1024 ligands");
+        const size_t smem = std::max(ligs->cta_smem[0], ligs->cta_smem[1]);
+        if (smem > TRIDSK_SMEM_MAX_CTA) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
+        CK(launch_score_cta(ctx->stream, a, smem));
     } else {
         CK(launch_score(ctx->stream, a));
     }
@@ -711,7 +761,8 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
 }
 
 extern "C" int tridsk_set_kernel(tridsk_ctx* ctx, int kernel) {
-    if (!ctx || kernel < 0 || kernel > 2) return fail(ctx, TRIDSK_EINVAL, "kernel must be 0 (auto), 1 (warp per chain) or 2 (lane per chain)");
+    if (!ctx || kernel < 0 || kernel > 3)
+        return fail(ctx, TRIDSK_EINVAL, "kernel must be 0 (auto), 1 (warp per chain), 2 (lane per chain) or 3 (CTA per chain)");
     ctx->kernel = kernel;
     return TRIDSK_OK;
 }
@@ -764,6 +815,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     memset(&base, 0, sizeof(base));
     base.hdr = ligs->hdr; base.atom_f4 = ligs->atom_f4; base.atom_i = ligs->atom_i; base.frags = ligs->frags; base.rounds = ligs->rounds;
     base.lane_frags = ligs->lane_frags; base.lane_stream = ligs->lane_stream; base.lane_recs = ligs->lane_recs;
+    base.cta_rows = ligs->cta_rows; base.cta_recs = ligs->cta_recs;
     base.grid = grid->d;
     to_dparams(params, &base.P);
     for (int c = 0; c < 3; ++c) { base.box_min[c] = box_min[c]; base.box_max[c] = box_max[c]; base.centre[c] = pocket_center[c]; }
@@ -773,10 +825,22 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     base.pose_cur = state; base.pose_best = state + n_pose_f; base.e_cur = state + 2 * n_pose_f; base.e_best = state + 2 * n_pose_f + nch;
     base.trace = d_trace; base.trace_stride = n_steps;
 
-    // Mapping: a warp per chain when chains are few (latency), a lane per chain when they outnumber the machine's
-    // lanes several times over (throughput).  tridsk_set_kernel overrides.
-    const bool lane = ctx->kernel == 2 || (ctx->kernel == 0 && nch >= (size_t)ctx->sm_count * 32 * 8);
-    ctx->last_kernel = lane ? 2 : 1;
+    // Mapping: a CTA per chain when chains are scarce (a single dock: latency of one evaluation), a lane per chain when
+    // they outnumber the machine's lanes several times over (screens: throughput), a warp per chain in between.
+    // tridsk_set_kernel overrides.
+    int mode = ctx->kernel;
+    if (mode == 0) {
+        if (nch >= (size_t)ctx->sm_count * 32 * 8) mode = 2;
+        else if (ligs->has_cta && nch <= (size_t)ctx->sm_count * 8) mode = 3;
+        else mode = 1;
+    }
+    if (mode == 3) {
+        if (!ligs->has_cta) return fail(ctx, TRIDSK_EINVAL, "the CTA-per-chain mapping needs a ligand batch of at most 1024 ligands");
+        if (std::max(ligs->cta_smem[0], ligs->cta_smem[1]) > TRIDSK_SMEM_MAX_CTA)
+            return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
+    }
+    const bool lane = mode == 2;
+    ctx->last_kernel = mode;
     tridsk_ligands* lg = const_cast<tridsk_ligands*>(ligs);
     if (lane) { int rc = lane_plan(ctx, lg, n_chains, params->n_refine); if (rc) return rc; }
 
@@ -799,6 +863,14 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
                 a.lig_list = lg->all_ids + b.first; a.n_list = b.count;
                 fill(a);
                 series.push_back({2, b.chains_per_cta, b.smem, br++ % TRIDSK_BRANCHES, a});
+            }
+        } else if (mode == 3) {
+            for (int k = 0; k < 2; ++k) {
+                if (ligs->cta_bucket[k].empty()) continue;
+                McLaunch a = base;
+                a.lig_list = ligs->cta_bucket_dev[k]; a.n_list = (int)ligs->cta_bucket[k].size();
+                fill(a);
+                series.push_back({3, k == 0 ? 128 : 256, ligs->cta_smem[k], k, a});
             }
         } else {
             for (int j = 1; j <= TRIDSK_MAX_J; ++j) {
@@ -845,7 +917,8 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         }
         for (auto& it : series) {
             cudaStream_t bs = it.branch == 0 ? s : ctx->side[it.branch];
-            e = it.kind == 2 ? launch_mc_lane(bs, it.a, it.arg, it.smem) : launch_mc(bs, it.arg, it.a);
+            e = it.kind == 2 ? launch_mc_lane(bs, it.a, it.arg, it.smem)
+                : it.kind == 3 ? launch_mc_cta(bs, it.a, it.arg, it.smem) : launch_mc(bs, it.arg, it.a);
             if (e != cudaSuccess) return e;
         }
         for (int i = 1; i < n_branch; ++i) {

@@ -66,6 +66,35 @@ __device__ __forceinline__ void quat_rotate_by(float q[4], float vx, float vy, f
     q[0] = r[0]; q[1] = r[1]; q[2] = r[2]; q[3] = r[3];
 }
 
+// ------------------------------------------------------------------ pair-function constants (lane and CTA kernels)
+// Constants of the pair function in the form the inner loop wants them.
+struct PairK {
+    float nk2;              // -log2(e) / (2 sigma^2) of the long-range Gaussian
+    float dmax;             // long-range cut-off
+    float kappa;            // gradient scale: dE/dx_a = kappa * sum s (x_a - x_b),  kappa = -2 w_long / log2(e)
+    float mu;               // long-range mu: the clash distance of a plain pair is c - mu
+    float hb_dclash;        // clash distance of a donor/acceptor pair
+    float kc;               // clash gradient in kappa units: w_clash / kappa
+    float inv_floor;        // 1 / d_floor
+    float kh;               // hydrogen-bond gradient in kappa units: 2 w_hbond / (2 sigma_hb^2) / kappa
+    float w_long, w_clash_ln2, w_hbond, hb_dmax, hb_mu, hb_nk2;
+};
+__device__ __forceinline__ PairK make_pairk(const DParams& P) {
+    PairK K;
+    const float L2E = 1.4426950408889634f;
+    K.nk2 = -P.long_inv_two_sigma2 * L2E; K.dmax = P.long_dmax;
+    K.kappa = -2.f * P.w_long / L2E;
+    K.mu = P.long_mu; K.hb_dclash = P.hb_dclash;
+    K.kc = P.w_clash / K.kappa; K.inv_floor = 1.f / P.d_floor;
+    K.kh = 2.f * P.w_hbond * P.hb_inv_two_sigma2 / K.kappa;
+    K.w_long = P.w_long; K.w_clash_ln2 = P.w_clash * 0.6931471805599453f; K.w_hbond = P.w_hbond;
+    K.hb_dmax = P.hb_dmax; K.hb_mu = P.hb_mu; K.hb_nk2 = -P.hb_inv_two_sigma2 * L2E;
+    return K;
+}
+__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
 // ------------------------------------------------------------------ per-chain view of one ligand, in registers
 template <int J>
 struct Lig {
@@ -184,6 +213,47 @@ __device__ __forceinline__ float grid_interp_packed(const DGrid& G, float k_wall
         gx = (clx ? 0.f : fmaf(fz, dx1 - dx0, dx0) * G.inv_h) + 2.f * k_wall * wx;
         gy = (cly ? 0.f : fmaf(fz, e1 - e0, e0) * G.inv_h) + 2.f * k_wall * wy;
         gz = (clz ? 0.f : (b1 - b0) * G.inv_h) + 2.f * k_wall * wz;
+    }
+    return e;
+}
+
+// The same interpolant in two halves, so that a caller can issue the two 16-byte loads early and blend late (the CTA
+// kernel hides the L2 latency behind its pair loop).  Arithmetic and operation order are those of grid_interp.
+struct GridCell {
+    const float4* p;
+    float fx, fy, fz, wx, wy, wz;
+    bool clx, cly, clz;
+};
+__device__ __forceinline__ GridCell grid_locate(const DGrid& G, int type, float x, float y, float z) {
+    GridCell c;
+    const float ux = (x - G.ox) * G.inv_h, uy = (y - G.oy) * G.inv_h, uz = (z - G.oz) * G.inv_h;
+    const float cx = fminf(fmaxf(ux, 0.f), (float)(G.nx - 1));
+    const float cy = fminf(fmaxf(uy, 0.f), (float)(G.ny - 1));
+    const float cz = fminf(fmaxf(uz, 0.f), (float)(G.nz - 1));
+    const int ix = min((int)cx, G.nx - 2), iy = min((int)cy, G.ny - 2), iz = min((int)cz, G.nz - 2);
+    c.fx = cx - (float)ix; c.fy = cy - (float)iy; c.fz = cz - (float)iz;
+    c.p = G.gp + (size_t)type * G.plane + ((size_t)iz * G.ny + iy) * G.nx + ix;
+    c.clx = (cx != ux); c.cly = (cy != uy); c.clz = (cz != uz);
+    c.wx = c.clx ? x - (G.ox + cx * G.h) : 0.f;
+    c.wy = c.cly ? y - (G.oy + cy * G.h) : 0.f;
+    c.wz = c.clz ? z - (G.oz + cz * G.h) : 0.f;
+    return c;
+}
+template <bool GRAD>
+__device__ __forceinline__ float grid_blend(const DGrid& G, float k_wall, const GridCell& c, const float4 lo, const float4 hi,
+                                            float& gx, float& gy, float& gz) {
+    const float v000 = lo.x, v001 = lo.y, v010 = lo.z, v011 = lo.w, v100 = hi.x, v101 = hi.y, v110 = hi.z, v111 = hi.w;
+    const float d00 = v001 - v000, d01 = v011 - v010, d10 = v101 - v100, d11 = v111 - v110;
+    const float a00 = fmaf(c.fx, d00, v000), a01 = fmaf(c.fx, d01, v010), a10 = fmaf(c.fx, d10, v100), a11 = fmaf(c.fx, d11, v110);
+    const float e0 = a01 - a00, e1 = a11 - a10;
+    const float b0 = fmaf(c.fy, e0, a00), b1 = fmaf(c.fy, e1, a10);
+    float e = fmaf(c.fz, b1 - b0, b0);
+    if (c.clx | c.cly | c.clz) e += k_wall * (c.wx * c.wx + c.wy * c.wy + c.wz * c.wz);
+    if (GRAD) {
+        const float dx0 = fmaf(c.fy, d01 - d00, d00), dx1 = fmaf(c.fy, d11 - d10, d10);
+        gx = (c.clx ? 0.f : fmaf(c.fz, dx1 - dx0, dx0) * G.inv_h) + 2.f * k_wall * c.wx;
+        gy = (c.cly ? 0.f : fmaf(c.fz, e1 - e0, e0) * G.inv_h) + 2.f * k_wall * c.wy;
+        gz = (c.clz ? 0.f : (b1 - b0) * G.inv_h) + 2.f * k_wall * c.wz;
     }
     return e;
 }

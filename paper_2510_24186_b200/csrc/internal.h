@@ -13,6 +13,7 @@
 #define TRIDSK_WARPS_PER_CTA 4
 #define TRIDSK_MAX_J 4           // atoms per lane (n_atoms <= 32 * MAX_J)
 #define TRIDSK_MAX_TILES 10      // J(J+1)/2 tiles of the pair schedule
+#define TRIDSK_CTA_MAX_LIG 1024  // batches up to this size also carry the CTA-per-chain pair format
 #define TRIDSK_BRANCHES 8        // parallel branches of a dock's launch series (ctx stream + side streams)
 
 // ---------------------------------------------------------------- device-side packed formats
@@ -51,6 +52,8 @@ struct LigHdr {
     int ls_len;
     int rec_off;                  // lane format: into lane_recs (n_rec records, in the order the stream consumes them)
     int n_rec;
+    int cta_row_off;              // CTA format: into cta_rows (n + 1 row offsets, relative to the ligand's records)
+    int cta_rec_off;              // CTA format: into cta_recs (2 n_pairs row records, then n_pairs flat records)
 };
 
 // Lane format (mc_lane.cu).  Fragments are re-indexed in depth-first PRE-order g = 0..T (0 = root), so that the
@@ -82,6 +85,11 @@ struct LaneRec {
 };
 #define TRIDSK_LANE_REC_SMEM 20
 
+// CTA format (mc_cta.cu): the pair set twice over.  Row form, for the gradient: for every atom a (internal order) the
+// partners b of a, {b | hb << 8, dvdw bits}, rows delimited by cta_rows -- every pair appears in both rows, so an atom's
+// force is a sum its own threads own (no scatter, no atomics).  Flat form, for energy-only evaluations: every pair once,
+// {a | b << 8 | hb << 16, dvdw bits}, sorted by (a, b).  Fragments are the LaneFrag records (pre-order).
+
 // Per-fragment record; fragment 0 is the root, fragment k+1 hangs off torsion k.
 struct FragRec {
     float ux, uy, uz, ox;         // axis unit vector and axis point (atom b_k), reference frame
@@ -108,6 +116,8 @@ struct McLaunch {
     const LaneFrag* lane_frags;   // lane format: T + 1 records per ligand at frag_off, pre-order
     const uint4* lane_stream;     // lane format: the pair instruction stream (header units)
     const LaneRec* lane_recs;     // lane format: the pair records
+    const int* cta_rows;          // CTA format
+    const uint2* cta_recs;
     const int* lig_list;          // ligands handled by this launch (one bucket)
     int n_list;
     DGrid grid;
@@ -136,6 +146,8 @@ struct ScoreLaunch {
     const LaneFrag* lane_frags;
     const uint4* lane_stream;
     const LaneRec* lane_recs;
+    const int* cta_rows;
+    const uint2* cta_recs;
     const int* seg_lig;           // lane score kernel: per CTA the ligand, and its poses perm[seg_start .. seg_start + seg_cnt)
     const int* seg_start;
     const int* seg_cnt;
@@ -177,6 +189,32 @@ __host__ __device__ static inline int lane_chain_slots(int n, int T, int max_dep
     return 3 * n + lane_wslots(T, max_depth) + 2 * T + (n_refine > 1 ? 2 * T : 0);
 }
 
+// CTA-per-chain kernel: shared-memory layout (byte offsets) -- topology {ref, meta, fragments, row offsets, records},
+// the chain's coordinates X[3][n], per-atom (force, moment about t) AF[6][n] and a reduction scratch
+struct CtaLayout { size_t ref, meta, frag, rows, recs, X, AF, red, total; };
+#define TRIDSK_AL16(x) (((x) + 15) / 16 * 16)
+__host__ __device__ static inline CtaLayout cta_layout(int n, int T, int n_pairs) {
+    CtaLayout L;
+    size_t o = 0;
+    L.ref = o; o += 16 * (size_t)n;
+    L.meta = o; o = TRIDSK_AL16(o + 4 * (size_t)n);
+    L.frag = o; o += sizeof(LaneFrag) * (size_t)(T + 1);
+    L.rows = o; o = TRIDSK_AL16(o + 4 * (size_t)(n + 1));
+    L.recs = o; o = TRIDSK_AL16(o + 8 * 3 * (size_t)n_pairs);
+    L.X = o; o = TRIDSK_AL16(o + 12 * (size_t)n);
+    L.AF = o; o = TRIDSK_AL16(o + 24 * (size_t)n);
+    L.red = o; o += 4 * 64;
+    L.total = o;
+    return L;
+}
+// threads per chain and lanes per atom of the CTA kernel
+__host__ __device__ static inline void cta_shape(int n, int* threads, int* lpa) {
+    if (n <= 16) { *threads = 128; *lpa = 8; }
+    else if (n <= 32) { *threads = 128; *lpa = 4; }
+    else if (n <= 64) { *threads = 256; *lpa = 4; }
+    else { *threads = 256; *lpa = 2; }
+}
+
 // ---------------------------------------------------------------- host-side handles
 struct tridsk_ctx {
     int device = 0;
@@ -196,7 +234,7 @@ struct tridsk_ctx {
     bool ev_valid = false;
     cudaStream_t side[TRIDSK_BRANCHES] = {};           // side[0] unused
     cudaEvent_t fork_ev = nullptr, join_ev[TRIDSK_BRANCHES] = {};
-    int kernel = 0;               // tridsk_set_kernel: 0 auto, 1 warp per chain, 2 lane per chain
+    int kernel = 0;               // tridsk_set_kernel: 0 auto, 1 warp per chain, 2 lane per chain, 3 CTA per chain
     // grids come from a stream-ordered pool that keeps its memory (a screen rebuilds same-sized grids per receptor)
     cudaMemPool_t pool = nullptr;
     std::shared_ptr<bool> alive = std::make_shared<bool>(true);   // handles that outlive the ctx free synchronously
@@ -225,6 +263,12 @@ struct tridsk_ligands {
     LaneFrag* lane_frags = nullptr;
     uint4* lane_stream = nullptr;
     LaneRec* lane_recs = nullptr;
+    bool has_cta = false;
+    int* cta_rows = nullptr;
+    uint2* cta_recs = nullptr;
+    std::vector<int> cta_bucket[2];              // ligand ids per CTA size (128, 256 threads)
+    int* cta_bucket_dev[2] = {nullptr, nullptr};
+    size_t cta_smem[2] = {0, 0};                 // largest shared-memory need per bucket
     int* all_ids = nullptr;       // 0..n_lig-1 re-ordered per lane bucket (refilled when the plan key changes)
     struct LaneBucket { int chains_per_cta; size_t smem; int first, count; };
     std::vector<LaneBucket> lane_plan;
@@ -244,5 +288,7 @@ cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta
 cudaError_t launch_score_lane(cudaStream_t s, const ScoreLaunch& a, int n_seg, size_t smem_bytes);
 cudaError_t mc_lane_prepare(size_t max_smem_bytes);
 cudaError_t launch_score(cudaStream_t s, const ScoreLaunch& a);
+cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int threads, size_t smem_bytes);
+cudaError_t launch_score_cta(cudaStream_t s, const ScoreLaunch& a, size_t smem_bytes);
 cudaError_t launch_topk(cudaStream_t s, const TopkLaunch& a);
 cudaError_t launch_philox_debug(cudaStream_t s, const unsigned int* ctr_key /* dev[6] */, unsigned int* out /* dev[4] */);

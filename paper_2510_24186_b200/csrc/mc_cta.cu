@@ -1,0 +1,483 @@
+// mc_cta.cu -- the latency form of the fused per-chain Monte Carlo kernel (steps a1..a8, a10): one CTA per chain.
+//
+// A single dock has a few hundred chains, each a serial string of thousands of pose evaluations: the time of a dock is
+// (evaluations per chain) x (latency of one evaluation), and a warp per chain (mc_kernel.cu) leaves that latency at
+// ~2,100 dependent warp instructions.  Here a chain gets 4 or 8 warps:
+//   * every WARP keeps the whole pose and all fragment frames in registers (lane g = fragment g in pre-order) and
+//     repeats the scalar work -- Philox, forward kinematics of the frames, the reverse pass, Adam, Metropolis -- so the
+//     warps never have to exchange pose state and take identical decisions by construction;
+//   * the atoms are spread over the CTA, `lpa` lanes per atom: the gradient evaluation walks the pair set in ROW form
+//     (every atom meets all its partners, each pair is visited from both ends), so an atom's force is accumulated by
+//     its own lanes -- no scatter, no atomics, bit-reproducible; the energy-only evaluation walks the flat pair list;
+//   * the receptor term of an atom is two 16-byte gathers whose L2 latency hides behind the pair loop;
+//   * two __syncthreads per evaluation: coordinates visible, per-atom (force, moment) / energy partials visible.
+//
+// P:N = PAPER.md line N; O*/G* = DESIGN.md section 3.
+#include "chain.cuh"
+
+struct CtaTopo {
+    const float4* ref;      // [n] {ref x, y, z, vdW radius}, internal (depth-first) atom order
+    const int* meta;        // [n] type | pre-order fragment << 8 | original index << 16
+    const LaneFrag* frag;   // [T + 1] pre-order
+    const int* rows;        // [n + 1] row offsets into recs
+    const uint2* recs;      // [2P] row records {b | hb << 8, c}, then [P] flat records {a | b << 8 | hb << 16, c}; c = dvdw + mu
+    float *X, *AF, *red;    // X[3][n], AF[6][n], red[64]
+    int n, T, P, lpa;
+};
+
+// this lane's fragment (lane g = fragment g in pre-order; lanes beyond T are idle copies of the root)
+struct CtaFrag {
+    float ux, uy, uz, ox, oy, oz;
+    int parent, depth, lo, own_hi, tor, g_end;
+    bool valid;
+};
+
+__device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char* smem, const LigHdr* __restrict__ h,
+                                          const float4* __restrict__ atom_f4, const int* __restrict__ atom_i,
+                                          const LaneFrag* __restrict__ lane_frags, const int* __restrict__ cta_rows,
+                                          const uint2* __restrict__ cta_recs, const DParams& P) {
+    const int n = h->n, T = h->T, np = h->n_pairs, tid = threadIdx.x, nt = blockDim.x, lane = tid & 31;
+    const CtaLayout L = cta_layout(n, T, np);
+    float4* ref = reinterpret_cast<float4*>(smem + L.ref);
+    int* meta = reinterpret_cast<int*>(smem + L.meta);
+    int* frag = reinterpret_cast<int*>(smem + L.frag);
+    int* rows = reinterpret_cast<int*>(smem + L.rows);
+    uint2* recs = reinterpret_cast<uint2*>(smem + L.recs);
+    const LaneFrag* fsrc = lane_frags + h->frag_off;
+    for (int i = tid; i < n; i += nt) ref[i] = __ldg(atom_f4 + h->atom_off + i);
+    for (int i = tid; i < (T + 1) * (int)(sizeof(LaneFrag) / 4); i += nt) frag[i] = __ldg(reinterpret_cast<const int*>(fsrc) + i);
+    for (int g = tid; g <= T; g += nt) {
+        const int lo = __ldg(&fsrc[g].lo), hi = __ldg(&fsrc[g].own_hi);
+        for (int a = lo; a < hi; ++a) {
+            const int w = __ldg(atom_i + h->atom_off + a);
+            meta[a] = (w & 0xff) | (g << 8) | (((w >> 16) & 0xff) << 16);
+        }
+    }
+    for (int i = tid; i <= n; i += nt) rows[i] = __ldg(cta_rows + h->cta_row_off + i);
+    for (int i = tid; i < 3 * np; i += nt) {
+        const uint2 r = __ldg(cta_recs + h->cta_rec_off + i);
+        recs[i] = make_uint2(r.x, __float_as_uint(__uint_as_float(r.y) + P.long_mu));
+    }
+    S.ref = ref; S.meta = meta; S.frag = reinterpret_cast<const LaneFrag*>(frag); S.rows = rows; S.recs = recs;
+    S.X = reinterpret_cast<float*>(smem + L.X); S.AF = reinterpret_cast<float*>(smem + L.AF);
+    S.red = reinterpret_cast<float*>(smem + L.red);
+    S.n = n; S.T = T; S.P = np;
+    int threads;
+    cta_shape(n, &threads, &S.lpa);
+    __syncthreads();
+    const LaneFrag& r = S.frag[lane <= T ? lane : 0];
+    F.valid = lane <= T;
+    F.ux = r.ux; F.uy = r.uy; F.uz = r.uz; F.ox = r.ox; F.oy = r.oy; F.oz = r.oz;
+    F.parent = F.valid ? r.parent : 0; F.depth = F.valid ? r.depth : 0;
+    F.lo = r.lo; F.own_hi = F.valid ? r.own_hi : r.lo; F.tor = F.valid ? r.tor : -1;
+    int e = lane + 1;
+    while (F.valid && e <= T && S.frag[e].depth > r.depth) ++e;      // the subtree of g is the fragment range [g, g_end)
+    F.g_end = F.valid ? e : 1;
+}
+
+// ------------------------------------------------------------------ O2: one pair, scalar (same arithmetic as lane_rec)
+template <bool GRAD, bool ENERGY>
+__device__ __forceinline__ void cta_pair(const PairK& K, float dx, float dy, float dz, float c, bool hb,
+                                         float& eL, float& eC, float& eH, float& fx, float& fy, float& fz) {
+    const float d2 = fmaxf(fmaf(dx, dx, fmaf(dy, dy, dz * dz)), 1e-12f);
+    const float rinv = rsqrt_approx(d2);
+    const float d = d2 * rinv;
+    const float t = d - c;
+    const float u = t * K.nk2;
+    float g = ex2_approx(u * t);
+    g = d < K.dmax ? g : 0.f;
+    const float dc = hb ? K.hb_dclash : c - K.mu;
+    const float q = dc * fminf(rinv, K.inv_floor);
+    float s = 0.f;
+    if (ENERGY) { eL += g; eC += lg2_approx(fmaxf(q, 1.f)); }
+    if (GRAD) {
+        s = u * g * rinv;
+        if (q > 1.f && rinv < K.inv_floor) s = fmaf(-K.kc * rinv, rinv, s);
+    }
+    if (hb) {
+        const float th = d - K.hb_mu;
+        float gh = ex2_approx(K.hb_nk2 * th * th);
+        gh = d < K.hb_dmax ? gh : 0.f;
+        if (ENERGY) eH += gh;
+        if (GRAD) s = fmaf(K.kh * th, gh * rinv, s);
+    }
+    if (GRAD) { fx = fmaf(s, dx, fx); fy = fmaf(s, dy, fy); fz = fmaf(s, dz, fz); }
+}
+
+// ------------------------------------------------------------------ a3..a6: one pose evaluation by the whole CTA
+// In : t[3], unit q[4] (uniform), theta (lane g holds the torsion angle of fragment g).
+// Out: ENERGY: e_inter, e_intra (uniform over the CTA); GRAD: g6 = {dE/dt, dE/domega about t} (uniform), gth = dE/dtheta
+//      on lane g (O9); x, y, z = this thread's atom (valid when `active`).
+template <bool GRAD, bool ENERGY>
+__device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
+                                         int max_depth, const float t[3], const float q[4], float theta,
+                                         int atom, int part, bool active, float& x, float& y, float& z,
+                                         float& e_inter, float& e_intra, float g6[6], float& gth) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = S.n;
+
+    // ---- a3 forward kinematics (O8): world frame (R, p) of this lane's fragment, F_g = F_parent o L_g
+    float R[9], p[3];
+    quat_matrix(q, R);
+    p[0] = t[0]; p[1] = t[1]; p[2] = t[2];
+    if (max_depth > 0) {
+        float sn, cs;
+        __sincosf(theta, &sn, &cs);
+        const float oc = 1.f - cs;
+        float Lm[9];
+        Lm[0] = fmaf(oc * F.ux, F.ux, cs);          Lm[1] = fmaf(oc * F.ux, F.uy, -sn * F.uz);  Lm[2] = fmaf(oc * F.ux, F.uz, sn * F.uy);
+        Lm[3] = fmaf(oc * F.uy, F.ux, sn * F.uz);   Lm[4] = fmaf(oc * F.uy, F.uy, cs);          Lm[5] = fmaf(oc * F.uy, F.uz, -sn * F.ux);
+        Lm[6] = fmaf(oc * F.uz, F.ux, -sn * F.uy);  Lm[7] = fmaf(oc * F.uz, F.uy, sn * F.ux);   Lm[8] = fmaf(oc * F.uz, F.uz, cs);
+        const float c0 = F.ox - (Lm[0] * F.ox + Lm[1] * F.oy + Lm[2] * F.oz);
+        const float c1 = F.oy - (Lm[3] * F.ox + Lm[4] * F.oy + Lm[5] * F.oz);
+        const float c2 = F.oz - (Lm[6] * F.ox + Lm[7] * F.oy + Lm[8] * F.oz);
+        for (int d = 1; d <= max_depth; ++d) {
+            float PR[9], pp[3];
+#pragma unroll
+            for (int i = 0; i < 9; ++i) PR[i] = __shfl_sync(FULL_MASK, R[i], F.parent);
+#pragma unroll
+            for (int i = 0; i < 3; ++i) pp[i] = __shfl_sync(FULL_MASK, p[i], F.parent);
+            if (F.depth == d) {
+#pragma unroll
+                for (int r = 0; r < 3; ++r) {
+                    R[3 * r + 0] = PR[3 * r] * Lm[0] + PR[3 * r + 1] * Lm[3] + PR[3 * r + 2] * Lm[6];
+                    R[3 * r + 1] = PR[3 * r] * Lm[1] + PR[3 * r + 1] * Lm[4] + PR[3 * r + 2] * Lm[7];
+                    R[3 * r + 2] = PR[3 * r] * Lm[2] + PR[3 * r + 1] * Lm[5] + PR[3 * r + 2] * Lm[8];
+                    p[r] = PR[3 * r] * c0 + PR[3 * r + 1] * c1 + PR[3 * r + 2] * c2 + pp[r];
+                }
+            }
+        }
+    }
+    // this thread's atom: x_a = R_frag(a) r_a + p_frag(a); the group's first lane publishes it and starts the gathers
+    const int m = active ? S.meta[atom] : 0;
+    {
+        const int fr = (m >> 8) & 0xff;
+        float A[9], b[3];
+#pragma unroll
+        for (int i = 0; i < 9; ++i) A[i] = __shfl_sync(FULL_MASK, R[i], fr);
+#pragma unroll
+        for (int i = 0; i < 3; ++i) b[i] = __shfl_sync(FULL_MASK, p[i], fr);
+        const float4 r = S.ref[active ? atom : 0];
+        x = A[0] * r.x + A[1] * r.y + A[2] * r.z + b[0];
+        y = A[3] * r.x + A[4] * r.y + A[5] * r.z + b[1];
+        z = A[6] * r.x + A[7] * r.y + A[8] * r.z + b[2];
+    }
+    const bool lead = active && part == 0;
+    GridCell cell;
+    float4 glo = make_float4(0.f, 0.f, 0.f, 0.f), ghi = glo;
+    if (lead) {
+        S.X[atom] = x; S.X[n + atom] = y; S.X[2 * n + atom] = z;
+        cell = grid_locate(G, m & 0xff, x, y, z);
+        glo = __ldg(cell.p); ghi = __ldg(cell.p + (size_t)G.nx * G.ny);
+    }
+    __syncthreads();
+
+    // ---- a5 intra-ligand pairs (O6)
+    float eL = 0.f, eC = 0.f, eH = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
+    if (GRAD) {
+        if (active) {
+            const int k1 = S.rows[atom + 1];
+#pragma unroll 2
+            for (int k = S.rows[atom] + part; k < k1; k += S.lpa) {
+                const uint2 rec = S.recs[k];
+                const int b = (int)(rec.x & 0xffu);
+                cta_pair<true, ENERGY>(K, x - S.X[b], y - S.X[n + b], z - S.X[2 * n + b], __uint_as_float(rec.y), (rec.x >> 8) & 1u,
+                                       eL, eC, eH, fx, fy, fz);
+            }
+        }
+        eL *= 0.5f; eC *= 0.5f; eH *= 0.5f;                         // every pair was visited from both ends
+    } else {
+        const uint2* flat = S.recs + 2 * S.P;
+        float f0, f1, f2;
+#pragma unroll 2
+        for (int k = tid; k < S.P; k += blockDim.x) {
+            const uint2 rec = flat[k];
+            const int a = (int)(rec.x & 0xffu), b = (int)((rec.x >> 8) & 0xffu);
+            cta_pair<false, true>(K, S.X[a] - S.X[b], S.X[n + a] - S.X[n + b], S.X[2 * n + a] - S.X[2 * n + b], __uint_as_float(rec.y),
+                                  (rec.x >> 16) & 1u, eL, eC, eH, f0, f1, f2);
+        }
+    }
+    // ---- a4 receptor term of this thread's atom (the gathers were issued before the barrier)
+    float ei = 0.f, gx = 0.f, gy = 0.f, gz = 0.f;
+    if (lead) ei = grid_blend<GRAD>(G, P.k_wall, cell, glo, ghi, gx, gy, gz);
+    if (GRAD) {
+        for (int o = S.lpa >> 1; o > 0; o >>= 1) {                  // the atom's lanes are adjacent: fixed-order tree
+            fx += __shfl_xor_sync(FULL_MASK, fx, o);
+            fy += __shfl_xor_sync(FULL_MASK, fy, o);
+            fz += __shfl_xor_sync(FULL_MASK, fz, o);
+        }
+        if (lead) {
+            const float Fx = fmaf(K.kappa, fx, gx), Fy = fmaf(K.kappa, fy, gy), Fz = fmaf(K.kappa, fz, gz);
+            const float ax = x - t[0], ay = y - t[1], az = z - t[2];
+            float* af = S.AF + atom;
+            af[0] = Fx; af[n] = Fy; af[2 * n] = Fz;
+            af[3 * n] = ay * Fz - az * Fy; af[4 * n] = az * Fx - ax * Fz; af[5 * n] = ax * Fy - ay * Fx;
+        }
+    }
+    if (ENERGY) {
+        const float ea = fmaf(K.w_clash_ln2, eC, -fmaf(K.w_long, eL, K.w_hbond * eH));
+        const float si = warp_sum(ei), sa = warp_sum(ea);
+        if (lane == 0) { S.red[2 * warp] = si; S.red[2 * warp + 1] = sa; }
+    }
+    __syncthreads();
+    if (ENERGY) {
+        e_inter = 0.f; e_intra = 0.f;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { e_inter += S.red[2 * w]; e_intra += S.red[2 * w + 1]; }
+    }
+    if (!GRAD) return;
+
+    // ---- a6 reverse mode through the tree (O9): own-atom sums per fragment, inclusive scan over the pre-order, a
+    // subtree is a contiguous fragment range
+    float v[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    for (int a = F.lo; a < F.own_hi; ++a) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) v[c] += S.AF[c * n + a];
+    }
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) {
+            const float u = __shfl_up_sync(FULL_MASK, v[c], o);
+            if (lane >= o) v[c] += u;
+        }
+    }
+    float s[6];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        const float hi = __shfl_sync(FULL_MASK, v[c], F.g_end - 1);
+        const float lo = __shfl_sync(FULL_MASK, v[c], lane > 0 ? lane - 1 : 0);
+        s[c] = hi - (lane > 0 ? lo : 0.f);
+        g6[c] = __shfl_sync(FULL_MASK, v[c], 31);
+    }
+    gth = 0.f;
+    if (F.valid && lane >= 1) {
+        const float wx = R[0] * F.ux + R[1] * F.uy + R[2] * F.uz;
+        const float wy = R[3] * F.ux + R[4] * F.uy + R[5] * F.uz;
+        const float wz = R[6] * F.ux + R[7] * F.uy + R[8] * F.uz;
+        const float bx = R[0] * F.ox + R[1] * F.oy + R[2] * F.oz + p[0] - t[0];
+        const float by = R[3] * F.ox + R[4] * F.oy + R[5] * F.oz + p[1] - t[1];
+        const float bz = R[6] * F.ox + R[7] * F.oy + R[8] * F.oz + p[2] - t[2];
+        const float tx = s[3] - (by * s[2] - bz * s[1]);             // torque about b = M_t - (b - t) x F
+        const float ty = s[4] - (bz * s[0] - bx * s[2]);
+        const float tz = s[5] - (bx * s[1] - by * s[0]);
+        gth = wx * tx + wy * ty + wz * tz;
+    }
+}
+
+// ------------------------------------------------------------------ chain state I/O: lane g <-> pose[7 + tor(g)]
+__device__ __forceinline__ void cta_load_pose(const float* __restrict__ src, const CtaFrag& F, float t[3], float q[4], float& th) {
+    t[0] = src[0]; t[1] = src[1]; t[2] = src[2];
+    q[0] = src[3]; q[1] = src[4]; q[2] = src[5]; q[3] = src[6];
+    th = F.tor >= 0 ? src[7 + F.tor] : 0.f;
+}
+__device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const CtaFrag& F, int T, int stride, const float t[3],
+                                               const float q[4], float th) {
+    const int lane = threadIdx.x & 31;
+    if (lane == 0) {
+        dst[0] = t[0]; dst[1] = t[1]; dst[2] = t[2];
+        dst[3] = q[0]; dst[4] = q[1]; dst[5] = q[2]; dst[6] = q[3];
+    }
+    if (F.tor >= 0) dst[7 + F.tor] = th;
+    for (int e = 7 + T + lane; e < stride; e += 32) dst[e] = 0.f;
+}
+
+// ------------------------------------------------------------------ the fused MC kernel, one CTA per chain
+__global__ void __launch_bounds__(256) mc_cta_kernel(const McLaunch a) {
+    extern __shared__ __align__(16) unsigned char cta_smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lig = a.lig_list[blockIdx.x / a.n_chains];
+    const int chain = blockIdx.x % a.n_chains;
+    const LigHdr* h = a.hdr + lig;
+    CtaTopo S;
+    CtaFrag F;
+    cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.P);
+    const DParams& P = a.P;
+    const PairK K = make_pairk(P);
+    const int T = S.T, max_depth = h->max_depth;
+    const int atom = tid / S.lpa, part = tid % S.lpa;
+    const bool active = atom < S.n;
+    const size_t cidx = (size_t)lig * a.n_chains + chain;
+    const uint2 key = make_uint2((uint32_t)a.seed, (uint32_t)(a.seed >> 32));
+    const uint32_t gchain = (uint32_t)(a.chain_base + chain);
+
+    float ct[3], cq[4], cth, ecur;          // current accepted state (every warp holds a copy)
+    float bt[3], bq[4], bth, ebest;         // best state seen
+    float x, y, z, g6[6], gth, ei, ea;
+
+    if (a.init_mode == 2) {                 // resume
+        cta_load_pose(a.pose_cur + cidx * a.pose_stride, F, ct, cq, cth);
+        cta_load_pose(a.pose_best + cidx * a.pose_stride, F, bt, bq, bth);
+        ecur = a.e_cur[cidx]; ebest = a.e_best[cidx];
+    } else {
+        if (a.init_mode == 1) {
+            cta_load_pose(a.init_poses + cidx * a.pose_stride, F, ct, cq, cth);
+            quat_normalise(cq);
+        } else {                            // a1 / O11: Philox initialisation; lane l computes block purpose 2 + l
+            const uint4 r = philox4x32_10(make_uint4(gchain, 0u, (uint32_t)lig, 2u + (uint32_t)lane), key);
+            const float u0 = u01(r.x), u1 = u01(r.y), u2 = u01(r.z), u3 = u01(r.w);
+            const float a0 = __shfl_sync(FULL_MASK, u0, 0), a1 = __shfl_sync(FULL_MASK, u1, 0), a2 = __shfl_sync(FULL_MASK, u2, 0);
+            const float b0 = __shfl_sync(FULL_MASK, u0, 1), b1 = __shfl_sync(FULL_MASK, u1, 1), b2 = __shfl_sync(FULL_MASK, u2, 1);
+            const float rr = a.radius * cbrtf(a0), zz = 2.f * a1 - 1.f, sq = sqrtf(fmaxf(1.f - zz * zz, 0.f));
+            float sn, cs;
+            sincosf(2.f * PI_F * a2, &sn, &cs);
+            ct[0] = a.centre[0] + rr * sq * cs; ct[1] = a.centre[1] + rr * sq * sn; ct[2] = a.centre[2] + rr * zz;
+            const float s1 = sqrtf(1.f - b0), s2 = sqrtf(b0);
+            float sn1, cs1, sn2, cs2;
+            sincosf(2.f * PI_F * b1, &sn1, &cs1);
+            sincosf(2.f * PI_F * b2, &sn2, &cs2);
+            cq[0] = s2 * cs2; cq[1] = s1 * sn1; cq[2] = s1 * cs1; cq[3] = s2 * sn2;
+            quat_normalise(cq);
+            // torsion k takes element k % 4 of block 4 + k / 4, i.e. of lane 2 + k / 4
+            const int k = F.tor >= 0 ? F.tor : 0, src = 2 + (k >> 2);
+            const float v0 = __shfl_sync(FULL_MASK, u0, src & 31), v1 = __shfl_sync(FULL_MASK, u1, src & 31);
+            const float v2 = __shfl_sync(FULL_MASK, u2, src & 31), v3 = __shfl_sync(FULL_MASK, u3, src & 31);
+            const float uu = (k & 3) == 0 ? v0 : (k & 3) == 1 ? v1 : (k & 3) == 2 ? v2 : v3;
+            cth = F.tor >= 0 ? PI_F * (2.f * uu - 1.f) : 0.f;
+        }
+        cta_eval<false, true>(S, a.grid, P, K, F, max_depth, ct, cq, cth, atom, part, active, x, y, z, ei, ea, g6, gth);
+        ecur = ei + ea;
+        ebest = ecur;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) bt[i] = ct[i];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) bq[i] = cq[i];
+        bth = cth;
+    }
+
+    for (int s = 0; s < a.n_steps; ++s) {
+        const uint32_t step = (uint32_t)(a.first_step + s);
+        // O10: even lanes draw the perturbation block (purpose 0), odd lanes the Metropolis block (purpose 1)
+        const uint4 r = philox4x32_10(make_uint4(gchain, step, (uint32_t)lig, (uint32_t)(lane & 1)), key);
+        const float u0 = __shfl_sync(FULL_MASK, u01(r.x), 0), u1 = __shfl_sync(FULL_MASK, u01(r.y), 0);
+        const float u2 = __shfl_sync(FULL_MASK, u01(r.z), 0), u3 = __shfl_sync(FULL_MASK, u01(r.w), 0);
+        const float um = __shfl_sync(FULL_MASK, u01(r.x), 1);
+
+        // a2 / O12: perturb one entity of {translation, rotation, torsion k}
+        float pt[3] = {ct[0], ct[1], ct[2]}, pq[4] = {cq[0], cq[1], cq[2], cq[3]}, pth = cth;
+        const int entity = min((int)(u0 * (float)(T + 2)), T + 1);
+        if (entity == 0) {
+            pt[0] = fminf(fmaxf(pt[0] + P.pert_trans * (2.f * u1 - 1.f), a.box_min[0]), a.box_max[0]);
+            pt[1] = fminf(fmaxf(pt[1] + P.pert_trans * (2.f * u2 - 1.f), a.box_min[1]), a.box_max[1]);
+            pt[2] = fminf(fmaxf(pt[2] + P.pert_trans * (2.f * u3 - 1.f), a.box_min[2]), a.box_max[2]);
+        } else if (entity == 1) {
+            quat_rotate_by(pq, P.pert_rot * (2.f * u1 - 1.f), P.pert_rot * (2.f * u2 - 1.f), P.pert_rot * (2.f * u3 - 1.f));
+        } else if (F.tor == entity - 2) {
+            pth = PI_F * (2.f * u1 - 1.f);
+        }
+
+        // a3..a7: n_refine Adam steps on the 6+T tangent components (moments reset every MC step, G12)
+        float m[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        float b1p = 1.f, b2p = 1.f;
+        for (int rf = 0; rf < P.n_refine; ++rf) {
+            cta_eval<true, false>(S, a.grid, P, K, F, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
+            b1p *= P.adam_b1; b2p *= P.adam_b2;
+            const float c1 = 1.f / (1.f - b1p), c2 = 1.f / (1.f - b2p);
+            float g[7] = {g6[0], g6[1], g6[2], g6[3], g6[4], g6[5], gth}, dl[7];
+#pragma unroll
+            for (int i = 0; i < 7; ++i) {
+                m[i] = P.adam_b1 * m[i] + (1.f - P.adam_b1) * g[i];
+                v[i] = P.adam_b2 * v[i] + (1.f - P.adam_b2) * g[i] * g[i];
+                dl[i] = -P.lr * (m[i] * c1) / (sqrtf(v[i] * c2) + P.adam_eps);
+            }
+            pt[0] = fminf(fmaxf(pt[0] + dl[0], a.box_min[0]), a.box_max[0]);
+            pt[1] = fminf(fmaxf(pt[1] + dl[1], a.box_min[1]), a.box_max[1]);
+            pt[2] = fminf(fmaxf(pt[2] + dl[2], a.box_min[2]), a.box_max[2]);
+            quat_rotate_by(pq, dl[3], dl[4], dl[5]);
+            float th = pth + dl[6];
+            if (th >= PI_F) th -= 2.f * PI_F;
+            if (th < -PI_F) th += 2.f * PI_F;
+            pth = F.tor >= 0 ? th : 0.f;
+        }
+
+        // a8: energy of the refined proposal, Metropolis, best tracking
+        cta_eval<false, true>(S, a.grid, P, K, F, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
+        const float enew = ei + ea;
+        const bool accept = isfinite(enew) && (um < expf(-P.beta * (enew - ecur)));
+        if (a.trace != nullptr && tid == 0) {
+            tridsk_trace_rec rec;
+            rec.e_prop = enew; rec.e_cur = ecur; rec.u = um; rec.flags = (accept ? 1 : 0) | (entity << 8);
+            a.trace[cidx * a.trace_stride + a.trace_off + s] = rec;
+        }
+        if (accept) {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) ct[i] = pt[i];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) cq[i] = pq[i];
+            cth = pth; ecur = enew;
+            if (enew < ebest) {
+#pragma unroll
+                for (int i = 0; i < 3; ++i) bt[i] = pt[i];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) bq[i] = pq[i];
+                bth = pth; ebest = enew;
+            }
+        }
+    }
+
+    if (warp == 0) {
+        cta_store_pose(a.pose_cur + cidx * a.pose_stride, F, T, a.pose_stride, ct, cq, cth);
+        cta_store_pose(a.pose_best + cidx * a.pose_stride, F, T, a.pose_stride, bt, bq, bth);
+        if (lane == 0) { a.e_cur[cidx] = ecur; a.e_best[cidx] = ebest; }
+    }
+}
+
+// ------------------------------------------------------------------ tridsk_score_grad, CTA form: one CTA per pose
+__global__ void __launch_bounds__(256) score_cta_kernel(const ScoreLaunch a) {
+    extern __shared__ __align__(16) unsigned char cta_smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int i = blockIdx.x;
+    const int lig = a.lig_index[i];
+    const LigHdr* h = a.hdr + lig;
+    CtaTopo S;
+    CtaFrag F;
+    cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.P);
+    const PairK K = make_pairk(a.P);
+    const int atom = tid / S.lpa, part = tid % S.lpa;
+    const bool active = atom < S.n;
+    float t[3], q[4], th, x, y, z, g6[6], gth = 0.f, ei, ea;
+    cta_load_pose(a.poses + (size_t)i * a.pose_stride, F, t, q, th);
+    quat_normalise(q);
+    if (a.grad != nullptr) cta_eval<true, true>(S, a.grid, a.P, K, F, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
+    else cta_eval<false, true>(S, a.grid, a.P, K, F, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
+    if (tid == 0) { a.energy[3 * (size_t)i] = ei + ea; a.energy[3 * (size_t)i + 1] = ei; a.energy[3 * (size_t)i + 2] = ea; }
+    if (a.grad != nullptr && warp == 0) {
+        float* g = a.grad + (size_t)i * a.grad_stride;
+        if (lane == 0) { g[0] = g6[0]; g[1] = g6[1]; g[2] = g6[2]; g[3] = g6[3]; g[4] = g6[4]; g[5] = g6[5]; }
+        if (F.tor >= 0) g[6 + F.tor] = gth;
+        for (int e = 6 + S.T + lane; e < a.grad_stride; e += 32) g[e] = 0.f;
+    }
+    if (a.coords != nullptr) {
+        float* c = a.coords + (size_t)i * a.coord_stride * 3;
+        if (active && part == 0) {
+            const int orig = (S.meta[atom] >> 16) & 0xff;
+            c[3 * orig] = x; c[3 * orig + 1] = y; c[3 * orig + 2] = z;
+        }
+        for (int e = 3 * S.n + tid; e < 3 * a.coord_stride; e += blockDim.x) c[e] = 0.f;
+    }
+}
+
+static bool g_cta_prepared = false;
+static cudaError_t mc_cta_prepare() {
+    if (g_cta_prepared) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(mc_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(score_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) g_cta_prepared = true;
+    return e;
+}
+
+cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int threads, size_t smem_bytes) {
+    const long long blocks = (long long)a.n_list * a.n_chains;
+    if (blocks <= 0) return cudaSuccess;
+    if (blocks > 0x7fffffffLL || (threads != 128 && threads != 256)) return cudaErrorInvalidValue;
+    cudaError_t e = mc_cta_prepare();
+    if (e != cudaSuccess) return e;
+    mc_cta_kernel<<<(unsigned)blocks, threads, smem_bytes, s>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_score_cta(cudaStream_t s, const ScoreLaunch& a, size_t smem_bytes) {
+    if (a.n_pose <= 0) return cudaSuccess;
+    cudaError_t e = mc_cta_prepare();
+    if (e != cudaSuccess) return e;
+    score_cta_kernel<<<a.n_pose, 256, smem_bytes, s>>>(a);
+    return cudaGetLastError();
+}

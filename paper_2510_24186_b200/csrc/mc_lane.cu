@@ -31,34 +31,6 @@ struct LaneTopo {
     int n, T;
 };
 
-// Constants of the pair function in the form the inner loop wants them.
-struct PairK {
-    float nk2;              // -log2(e) / (2 sigma^2) of the long-range Gaussian
-    float dmax;             // long-range cut-off
-    float kappa;            // gradient scale: dE/dx_a = kappa * sum s (x_a - x_b),  kappa = -2 w_long / log2(e)
-    float mu;               // long-range mu: the clash distance of a plain pair is c - mu
-    float hb_dclash;        // clash distance of a donor/acceptor pair
-    float kc;               // clash gradient in kappa units: w_clash / kappa
-    float inv_floor;        // 1 / d_floor
-    float kh;               // hydrogen-bond gradient in kappa units: 2 w_hbond / (2 sigma_hb^2) / kappa
-    float w_long, w_clash_ln2, w_hbond, hb_dmax, hb_mu, hb_nk2;
-};
-__device__ __forceinline__ PairK make_pairk(const DParams& P) {
-    PairK K;
-    const float L2E = 1.4426950408889634f;
-    K.nk2 = -P.long_inv_two_sigma2 * L2E; K.dmax = P.long_dmax;
-    K.kappa = -2.f * P.w_long / L2E;
-    K.mu = P.long_mu; K.hb_dclash = P.hb_dclash;
-    K.kc = P.w_clash / K.kappa; K.inv_floor = 1.f / P.d_floor;
-    K.kh = 2.f * P.w_hbond * P.hb_inv_two_sigma2 / K.kappa;
-    K.w_long = P.w_long; K.w_clash_ln2 = P.w_clash * 0.6931471805599453f; K.w_hbond = P.w_hbond;
-    K.hb_dmax = P.hb_dmax; K.hb_mu = P.hb_mu; K.hb_nk2 = -P.hb_inv_two_sigma2 * L2E;
-    return K;
-}
-__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-__device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-__device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-
 // Stage one ligand's topology into shared memory; returns the first byte after it (16-byte aligned).  The pair
 // records take their parameter-dependent form here (internal.h): c = dvdw + mu, 3 * b | hbmask << 16.
 __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char* smem, const LigHdr* __restrict__ h,

@@ -28,13 +28,13 @@ def worst(got, want, rtol=RTOL, atol=ATOL, scale=None):
     return float(np.max(np.abs(got - want) / (atol + rtol * ref)))
 
 
-@pytest.fixture(scope="module", params=["warp", "lane"])
+@pytest.fixture(scope="module", params=["warp", "lane", "cta"])
 def eng(request):
-    """Every test runs under both chain-to-thread mappings of the fused kernel: a warp per chain and a
-    lane per chain (tridsk_set_kernel)."""
+    """Every test runs under all three chain-to-thread mappings of the fused kernel: a warp, a lane and
+    a CTA per chain (tridsk_set_kernel)."""
     from paper_2510_24186_b200 import Engine
     e = Engine(0)
-    e.set_kernel({"warp": 1, "lane": 2}[request.param])
+    e.set_kernel({"warp": 1, "lane": 2, "cta": 3}[request.param])
     yield e
     e.close()
 
