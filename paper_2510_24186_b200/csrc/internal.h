@@ -202,7 +202,7 @@ __host__ __device__ static inline CtaLayout cta_layout(int n, int T, int n_pairs
     L.rows = o; o = TRIDSK_AL16(o + 4 * (size_t)(n + 1));
     L.recs = o; o = TRIDSK_AL16(o + 8 * 3 * (size_t)n_pairs);
     L.X = o; o = TRIDSK_AL16(o + 12 * (size_t)n);
-    L.AF = o; o = TRIDSK_AL16(o + 24 * (size_t)n);
+    L.AF = o; o = TRIDSK_AL16(o + 32 * (size_t)n);
     L.red = o; o += 4 * 64;
     L.total = o;
     return L;

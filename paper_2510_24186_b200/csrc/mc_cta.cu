@@ -21,7 +21,7 @@ struct CtaTopo {
     const LaneFrag* frag;   // [T + 1] pre-order
     const int* rows;        // [n + 1] row offsets into recs
     const uint2* recs;      // [2P] row records {b | hb << 8, c}, then [P] flat records {a | b << 8 | hb << 16, c}; c = dvdw + mu
-    float *X, *AF, *red;    // X[3][n], AF[6][n], red[64]
+    float *X, *AF, *red;    // X[3][n], AF[n][8] = {force, 0, moment about t, 0}, red[64]
     int n, T, P, lpa;
 };
 
@@ -208,9 +208,9 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
         if (lead) {
             const float Fx = fmaf(K.kappa, fx, gx), Fy = fmaf(K.kappa, fy, gy), Fz = fmaf(K.kappa, fz, gz);
             const float ax = x - t[0], ay = y - t[1], az = z - t[2];
-            float* af = S.AF + atom;
-            af[0] = Fx; af[n] = Fy; af[2 * n] = Fz;
-            af[3 * n] = ay * Fz - az * Fy; af[4 * n] = az * Fx - ax * Fz; af[5 * n] = ax * Fy - ay * Fx;
+            float4* af = reinterpret_cast<float4*>(S.AF) + 2 * atom;
+            af[0] = make_float4(Fx, Fy, Fz, 0.f);
+            af[1] = make_float4(ay * Fz - az * Fy, az * Fx - ax * Fz, ax * Fy - ay * Fx, 0.f);
         }
     }
     if (ENERGY) {
@@ -229,8 +229,8 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     // subtree is a contiguous fragment range
     float v[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     for (int a = F.lo; a < F.own_hi; ++a) {
-#pragma unroll
-        for (int c = 0; c < 6; ++c) v[c] += S.AF[c * n + a];
+        const float4 f = reinterpret_cast<const float4*>(S.AF)[2 * a], mo = reinterpret_cast<const float4*>(S.AF)[2 * a + 1];
+        v[0] += f.x; v[1] += f.y; v[2] += f.z; v[3] += mo.x; v[4] += mo.y; v[5] += mo.z;
     }
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -281,7 +281,7 @@ __device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const Ct
 }
 
 // ------------------------------------------------------------------ the fused MC kernel, one CTA per chain
-__global__ void __launch_bounds__(256) mc_cta_kernel(const McLaunch a) {
+__global__ void __launch_bounds__(256, 2) mc_cta_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lig = a.lig_list[blockIdx.x / a.n_chains];
@@ -370,13 +370,13 @@ __global__ void __launch_bounds__(256) mc_cta_kernel(const McLaunch a) {
         for (int rf = 0; rf < P.n_refine; ++rf) {
             cta_eval<true, false>(S, a.grid, P, K, F, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
             b1p *= P.adam_b1; b2p *= P.adam_b2;
-            const float c1 = 1.f / (1.f - b1p), c2 = 1.f / (1.f - b2p);
+            const float c1 = __fdividef(1.f, 1.f - b1p), c2 = __fdividef(1.f, 1.f - b2p);
             float g[7] = {g6[0], g6[1], g6[2], g6[3], g6[4], g6[5], gth}, dl[7];
 #pragma unroll
-            for (int i = 0; i < 7; ++i) {
+            for (int i = 0; i < 7; ++i) {                            // division / square root to 2 ulp: far inside the tolerance
                 m[i] = P.adam_b1 * m[i] + (1.f - P.adam_b1) * g[i];
                 v[i] = P.adam_b2 * v[i] + (1.f - P.adam_b2) * g[i] * g[i];
-                dl[i] = -P.lr * (m[i] * c1) / (sqrtf(v[i] * c2) + P.adam_eps);
+                dl[i] = __fdividef(-P.lr * (m[i] * c1), __fsqrt_rn(v[i] * c2) + P.adam_eps);
             }
             pt[0] = fminf(fmaxf(pt[0] + dl[0], a.box_min[0]), a.box_max[0]);
             pt[1] = fminf(fmaxf(pt[1] + dl[1], a.box_min[1]), a.box_max[1]);
