@@ -185,6 +185,8 @@ int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* 
  * differ, so chains are bit-reproducible per mapping, not across mappings.
  */
 int tridsk_set_kernel(tridsk_ctx* ctx, int kernel);
+/* The mapping (1, 2 or 3) the last tridsk_dock on this ctx used; 0 before any dock. */
+int tridsk_last_kernel(const tridsk_ctx* ctx);
 
 /* Device time of the last tridsk_dock on this ctx, from CUDA events recorded on the ctx stream around the fused MC
  * kernel series and the top-k kernel: ms[0] = MC series, ms[1] = top-k.  Blocks until that dock has finished. [host] */

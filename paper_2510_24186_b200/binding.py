@@ -65,6 +65,8 @@ def lib():
         _lib.tridsk_last_error.restype = C.c_char_p
         _lib.tridsk_launch_count.restype = C.c_longlong
         _lib.tridsk_launch_count.argtypes = [C.c_void_p]
+        _lib.tridsk_last_kernel.restype = C.c_int
+        _lib.tridsk_last_kernel.argtypes = [C.c_void_p]
         _lib.tridsk_last_error.argtypes = [C.c_void_p]
         for name in ("tridsk_destroy", "tridsk_free_grid", "tridsk_free_ligands"):
             getattr(_lib, name).restype = None
@@ -180,6 +182,10 @@ class Engine:
     def set_kernel(self, kernel: int):
         """0 auto, 1 warp per chain, 2 lane per chain, 3 CTA per chain (tridsk_set_kernel)."""
         self._ck(lib().tridsk_set_kernel(self.ctx, C.c_int(kernel)))
+
+    def last_kernel(self) -> int:
+        """Mapping the last dock used: 1 warp, 2 lane, 3 CTA per chain (tridsk_last_kernel)."""
+        return int(lib().tridsk_last_kernel(self.ctx))
 
     def launch_count(self) -> int:
         return int(lib().tridsk_launch_count(self.ctx))

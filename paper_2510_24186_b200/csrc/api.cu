@@ -767,6 +767,8 @@ extern "C" int tridsk_set_kernel(tridsk_ctx* ctx, int kernel) {
     return TRIDSK_OK;
 }
 
+extern "C" int tridsk_last_kernel(const tridsk_ctx* ctx) { return ctx ? ctx->last_kernel : 0; }
+
 extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* ligs, const tridsk_params* params,
                            const float box_min[3], const float box_max[3], const float pocket_center[3], float pocket_radius,
                            int n_chains, int n_steps, int top_k, unsigned long long seed, int pose_stride,

@@ -449,3 +449,38 @@ def test_full_size_c2_dock_sampled_against_oracle(orc, eng, gp):
     _, _, _, eb = split_state(r["state"], 1, cfg.n_chains, 7 + L.T)
     assert np.array_equal(r["chain"][0], orc.topk(eb[0], cfg.top_k))
     assert e[0, 0] < -5.0                                                      # the search found a bound pose
+
+
+@pytest.mark.parametrize("name,n_sample", [("C1", 1), ("C3", 24), ("C4", 1), ("C5", 24)])
+def test_full_size_configs_auto_mapping_sampled_against_oracle(orc, gp, name, n_sample):
+    """BASELINE configs C1, C3, C4, C5 at full size, launched as bench.py launches them (automatic chain-to-thread mapping:
+    CTA per chain for the single docks, lane per chain for the screens; one graph launch): the returned top pose of
+    sampled ligands is re-scored by the oracle from the paper's plain receptor sums at the touched nodes, and the
+    returned energies are ordered."""
+    from paper_2510_24186_b200 import Engine
+    cfg = synth.CONFIGS[name]
+    rec = synth.make_receptor(cfg)
+    radius, role = synth.type_table(cfg.n_types)
+    batch = synth.make_ligands(cfg)
+    e = Engine(0)
+    try:
+        grid = e.build_grid(rec.xyz, rec.type, radius, role, gp, rec.origin, rec.dims, rec.spacing)
+        ligs = e.load_ligands(batch, radius, role)
+        r = e.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius,
+                   cfg.n_chains, cfg.n_steps, cfg.top_k, seed=cfg.philox_seed)
+        assert e.last_kernel() == (3 if batch.n_lig == 1 else 2)
+    finally:
+        e.close()
+    en = r["energy"]
+    assert np.all(np.isfinite(en)) and np.all(np.diff(en[:, :, 0], axis=1) >= 0)
+    ty, p = orc.Types(radius, role), orc.default_params()
+    rng = np.random.default_rng(7)
+    for l in sorted(rng.choice(batch.n_lig, size=min(n_sample, batch.n_lig), replace=False)):
+        L = orc.ligand_from_batch(batch, int(l))
+        pose = r["pose"][l, 0, :7 + L.T].astype(np.float64)
+        x = orc.fk(L, pose)
+        G = _sparse_oracle_grid(orc, p, ty, rec, x, L.type)
+        eo = orc.score_grad(p, ty, G, L, pose, want_grad=False)[0][0]
+        assert close(en[l, 0, 0], eo, rtol=2e-4, atol=2e-3), (name, l, en[l, 0, 0], eo)
+        assert close(en[l, 0, 1], eo / (1.0 + 0.01 * L.T), rtol=2e-4, atol=2e-3)          # E_screen (P:135)
+    assert np.median(en[:, 0, 0]) < 0.0                                                       # the search found bound poses
