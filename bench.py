@@ -29,6 +29,10 @@ from workloads import synth  # noqa: E402
 
 METRIC = "score+grad pose evals/sec per B200"
 UNIT = "pose evals/s"
+KERNEL_NAMES = {1: "mc_kernel<J> (warp per chain)", 2: "mc_lane_kernel (lane per chain)", 3: "mc_cta_kernel (CTA per chain)"}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the `ncu --set full` captures
+# summarised under profiles/ (r1b_ncu_full_cta_c2.txt, r1b_ncu_full_lane_c5.txt); None where no capture was made
+NCU_TRAFFIC_BYTES = {"C2": 14.50e6}
 
 
 # ----------------------------------------------------------------------------------------- accounting
@@ -180,7 +184,8 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
         ms_grid_build=float(np.mean(t_grid)), ms_mc_kernels=mc_ms, ms_topk=float(np.mean(t_topk)),
         wall_s=wall, launches=launches, scaling=scaling, clocks=clocks,
         roofline=dict(bound="alu", achieved=ach, peak=pk["alu_tflops"], unit="TFLOP/s", frac=ach / pk["alu_tflops"],
-                      traffic=None, kernel="mc_kernel (fused MC step series)",
+                      traffic=NCU_TRAFFIC_BYTES.get(name) if n_lig is None else None,
+                      kernel=KERNEL_NAMES.get(eng.last_kernel(), "?") + ", fused MC step series",
                       peak_source=f"148 SM x 128 lanes x 2 x {pk['sm_mhz']:.0f} MHz ({pk['source']})",
                       xu_gops=w["xu"] / (mc_ms * 1e-3) / 1e9, xu_frac=w["xu"] / (mc_ms * 1e-3) / 1e9 / pk["xu_gops"],
                       grid_gather_gbs=w["gather_bytes"] / (mc_ms * 1e-3) / 1e9,
@@ -318,6 +323,7 @@ def main():
             r = run_workload(eng, name, 2 if big else 5, 3, do_e2e=False, sample_clocks=False)
             extras[name] = {k: r[k] for k in ("title", "evals", "value", "score_grad_evals_per_s", "ms_per_step", "ms_per_task",
                                               "ms_grid_build", "ms_mc_kernels", "ms_topk", "launches", "best_energy")}
+            extras[name]["kernel"] = r["roofline"]["kernel"]
             extras[name]["roofline_frac"] = r["roofline"]["frac"]
             extras[name]["mc_kernel_evals_per_s"] = r["roofline"]["mc_kernel_evals_per_s"]
     if rank != 0:
