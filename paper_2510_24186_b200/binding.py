@@ -180,7 +180,8 @@ class Engine:
         self._ck(lib().tridsk_synchronize(self.ctx))
 
     def set_kernel(self, kernel: int):
-        """0 auto, 1 warp per chain, 2 lane per chain, 3 CTA per chain (tridsk_set_kernel)."""
+        """0 auto, 1 warp per chain, 2 lane per chain, 3 CTA per chain, 4 lane per chain with coordinates in tensor memory
+        (tridsk_set_kernel)."""
         self._ck(lib().tridsk_set_kernel(self.ctx, C.c_int(kernel)))
 
     def last_kernel(self) -> int:

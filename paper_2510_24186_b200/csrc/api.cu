@@ -664,7 +664,7 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
     a.grad = grad ? (h_g ? (float*)(ob + o_g) : grad) : nullptr;
     a.coords = coords ? (h_c ? (float*)(ob + o_c) : coords) : nullptr;
     std::vector<int> seg;                                   // lane form: [seg_lig | seg_start | seg_cnt | perm]
-    if (ctx->kernel == 2) {
+    if (ctx->kernel == 2 || ctx->kernel == 4) {
         // one lane per pose, one 32-lane CTA per run of <= 32 poses of the same ligand
         std::vector<int> perm(n_pose);
         for (int i = 0; i < n_pose; ++i) perm[i] = i;
@@ -714,11 +714,12 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
 // shared memory is the group's largest need, the groups run concurrently as parallel branches of the CUDA graph, and
 // inside a group the costliest ligands go first (short tail).
 static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_refine) {
-    const long long key = ((long long)n_chains << 8) | (n_refine > 1 ? 1 : 0);
+    const long long key = ((long long)n_chains << 8) | (n_refine > 1 ? 1 : 0) | (ctx->kernel == 4 ? 2 : 0);
     if (lg->lane_plan_key == key) return TRIDSK_OK;
     const int L = lg->n_lig;
     const int cmax = std::min(128, (n_chains + 31) / 32 * 32);
     struct Ent { int cls; long long cost; int lig; size_t need; };
+    const bool use_tm = ctx->kernel == 4;
     std::vector<Ent> ent(L);
     for (int i = 0; i < L; ++i) {
         const LigHdr& h = lg->hdr_h[i];
@@ -735,8 +736,21 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
             rr = std::max(1, std::min(std::min(rr, 32), 16 * 32 / cc));
             if (rr * cc > r * c) { c = cc; r = rr; need = nd; }
         }
-        if (c == 0) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");
-        ent[i] = {(c << 8) | r, (long long)h.n_pairs + 6LL * h.n + 8LL * h.T, i, need};
+        // tensor-memory form (mc_lane_tm_kernel): coordinates in TMEM columns, the rest of the chain state in shared
+        // memory, 4 warps per CTA each with its own topology copy; taken when it keeps more warps resident
+        int tm_cols = 0, tm_r = 0;
+        size_t region = 0;
+        if (use_tm && 3 * h.n + 1 <= 128) {
+            tm_cols = 3 * h.n + 1 <= 32 ? 32 : 3 * h.n + 1 <= 64 ? 64 : 128;
+            region = (topo + 32 * (per_chain - 12 * (size_t)h.n) + 15) / 16 * 16;
+            const size_t cta = (4 * region + 1023) / 1024 * 1024 + TRIDSK_SMEM_RESERVED;
+            tm_r = (int)std::min<size_t>(std::min<size_t>(TRIDSK_SMEM_PER_SM / cta, 512 / tm_cols), 4);
+            if (4 * region > TRIDSK_SMEM_MAX_CTA - 1024) tm_r = 0;
+        }
+        if (c == 0 && tm_r == 0) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");
+        const long long cost = (long long)h.n_pairs + 6LL * h.n + 8LL * h.T;
+        if (4 * tm_r > r * c / 32) ent[i] = {0x40000000 | (tm_cols << 8) | tm_r, cost, i, region};
+        else ent[i] = {(c << 8) | r, cost, i, need};
     }
     std::sort(ent.begin(), ent.end(), [](const Ent& x, const Ent& y) {
         if (x.cls != y.cls) return x.cls < y.cls;
@@ -747,13 +761,17 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
     lg->lane_plan.clear();
     for (int i = 0; i < L; ++i) {
         lg->lane_ids_h[i] = ent[i].lig;
-        if (i == 0 || ent[i].cls != ent[i - 1].cls) lg->lane_plan.push_back({ent[i].cls >> 8, 0, i, 0});
+        if (i == 0 || ent[i].cls != ent[i - 1].cls) {
+            const bool tm = (ent[i].cls & 0x40000000) != 0;
+            lg->lane_plan.push_back({tm ? 32 : ent[i].cls >> 8, 0, i, 0, tm ? (ent[i].cls >> 8) & 0xff : 0});
+        }
         lg->lane_plan.back().count++;
         lg->lane_plan.back().smem = std::max(lg->lane_plan.back().smem, ent[i].need);
     }
     if (getenv("TRIDSK_DEBUG"))
         for (const auto& b : lg->lane_plan)
-            fprintf(stderr, "tridsk lane plan: %d ligands, %d chains per CTA, %zu bytes of shared memory\n", b.count, b.chains_per_cta, b.smem);
+            fprintf(stderr, "tridsk lane plan: %d ligands, %s, %d chains per %s, %zu bytes of shared memory\n", b.count,
+                    b.tm_cols ? "TMEM" : "smem", b.chains_per_cta, b.tm_cols ? "warp" : "CTA", b.smem);
     CK(cudaStreamSynchronize(ctx->stream));                  // an earlier dock may still read all_ids
     CK(cudaMemcpyAsync(lg->all_ids, lg->lane_ids_h.data(), sizeof(int) * L, cudaMemcpyHostToDevice, ctx->stream));
     lg->lane_plan_key = key;
@@ -761,8 +779,8 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
 }
 
 extern "C" int tridsk_set_kernel(tridsk_ctx* ctx, int kernel) {
-    if (!ctx || kernel < 0 || kernel > 3)
-        return fail(ctx, TRIDSK_EINVAL, "kernel must be 0 (auto), 1 (warp per chain), 2 (lane per chain) or 3 (CTA per chain)");
+    if (!ctx || kernel < 0 || kernel > 4)
+        return fail(ctx, TRIDSK_EINVAL, "kernel must be 0 (auto), 1 (warp), 2 (lane), 3 (CTA per chain) or 4 (lane per chain, coordinates in tensor memory)");
     ctx->kernel = kernel;
     return TRIDSK_OK;
 }
@@ -841,7 +859,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         if (std::max(ligs->cta_smem[0], ligs->cta_smem[1]) > TRIDSK_SMEM_MAX_CTA)
             return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
     }
-    const bool lane = mode == 2;
+    const bool lane = mode == 2 || mode == 4;
     ctx->last_kernel = mode;
     tridsk_ligands* lg = const_cast<tridsk_ligands*>(ligs);
     if (lane) { int rc = lane_plan(ctx, lg, n_chains, params->n_refine); if (rc) return rc; }
@@ -864,7 +882,8 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
                 McLaunch a = base;
                 a.lig_list = lg->all_ids + b.first; a.n_list = b.count;
                 fill(a);
-                series.push_back({2, b.chains_per_cta, b.smem, br++ % TRIDSK_BRANCHES, a});
+                a.lane_region = (int)b.smem; a.tm_cols = b.tm_cols;
+                series.push_back({b.tm_cols ? 4 : 2, b.chains_per_cta, b.smem, br++ % TRIDSK_BRANCHES, a});
             }
         } else if (mode == 3) {
             for (int k = 0; k < 2; ++k) {
@@ -919,7 +938,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         }
         for (auto& it : series) {
             cudaStream_t bs = it.branch == 0 ? s : ctx->side[it.branch];
-            e = it.kind == 2 ? launch_mc_lane(bs, it.a, it.arg, it.smem)
+            e = it.kind == 4 ? launch_mc_lane_tm(bs, it.a) : it.kind == 2 ? launch_mc_lane(bs, it.a, it.arg, it.smem)
                 : it.kind == 3 ? launch_mc_cta(bs, it.a, it.arg, it.smem) : launch_mc(bs, it.arg, it.a);
             if (e != cudaSuccess) return e;
         }

@@ -484,3 +484,27 @@ def test_full_size_configs_auto_mapping_sampled_against_oracle(orc, gp, name, n_
         assert close(en[l, 0, 0], eo, rtol=2e-4, atol=2e-3), (name, l, en[l, 0, 0], eo)
         assert close(en[l, 0, 1], eo / (1.0 + 0.01 * L.T), rtol=2e-4, atol=2e-3)          # E_screen
     assert np.median(en[:, 0, 0]) < 0.0                                                       # the search found bound poses
+
+
+def test_tensor_memory_lane_kernel_is_bit_identical_to_shared_memory_lane_kernel(gp):
+    """Mapping 4 keeps the chains' coordinates in tensor memory (tcgen05.st / tcgen05.ld) instead of shared memory; the
+    arithmetic and its order are those of mapping 2, so a screen gives bit-identical energies, poses and chain ids."""
+    from paper_2510_24186_b200 import Engine
+    cfg = synth.CONFIGS["C5"]
+    rec = synth.make_receptor(cfg)
+    radius, role = synth.type_table(cfg.n_types)
+    batch = synth.make_ligands(cfg, 192)
+    out = {}
+    for mode in (2, 4):
+        e = Engine(0)
+        try:
+            e.set_kernel(mode)
+            grid = e.build_grid(rec.xyz, rec.type, radius, role, gp, rec.origin, rec.dims, rec.spacing)
+            ligs = e.load_ligands(batch, radius, role)
+            out[mode] = e.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius,
+                               40, 60, 3, seed=5)                 # 40 chains: a partial second warp per ligand
+            assert e.last_kernel() == mode
+        finally:
+            e.close()
+    for k in ("energy", "pose", "chain"):
+        assert np.array_equal(out[2][k], out[4][k]), k
