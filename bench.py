@@ -295,6 +295,7 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the other configs' short runs")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--n-lig", type=int, default=None, help="first n ligands of a screening config (profiling)")
+    ap.add_argument("--kernel", type=int, default=0, help="force a chain-to-thread mapping (tridsk_set_kernel); 0 = automatic")
     args = ap.parse_args()
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     local = int(os.environ.get("LOCAL_RANK", 0))
@@ -312,6 +313,7 @@ def main():
     if world > 1:
         torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local))
     eng = Engine(local)
+    eng.set_kernel(args.kernel)
     args.warmup = max(args.warmup, 3)
     main_res = run_workload(eng, args.workload, args.steps, args.warmup, rank, world, n_lig=args.n_lig)
     extras = {}

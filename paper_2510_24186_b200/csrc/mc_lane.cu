@@ -280,14 +280,23 @@ __device__ __forceinline__ void lane_tile(const uint4*& hp, const float4*& rc, c
         float fx[4], fy[4], fz[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) fx[i] = fy[i] = fz[i] = 0.f;
+        // software pipeline: the next record (and its partner's coordinates, a dependent load) is fetched while the
+        // current one is evaluated
+        float4 c4 = rc[0];
+        uint32_t mt = rm[0];
+        float bx, by, bz;
+        X.get((int)(mt & 0xffffu), bx, by, bz);
         for (int j = 0; j < nb; ++j) {
-            const float4 c4 = rc[j];
-            const uint32_t mt = rm[j];
-            float bx, by, bz;
-            X.get((int)(mt & 0xffffu), bx, by, bz);
+            const int jn = min(j + 1, nb - 1);
+            const float4 c4n = rc[jn];
+            const uint32_t mtn = rm[jn];
+            float nx, ny, nz;
             X.fence(bx, by, bz);
+            X.get((int)(mtn & 0xffffu), nx, ny, nz);
             lane_rec<GRAD>(K, ax, ay, az, bx, by, bz, c4, mt >> 16, eL, eC, eH, fx, fy, fz);
+            c4 = c4n; mt = mtn; bx = nx; by = ny; bz = nz;
         }
+        X.fence(bx, by, bz);
         rc += nb; rm += nb;
         if (GRAD) {
             float wv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
