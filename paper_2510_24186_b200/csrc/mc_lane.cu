@@ -216,7 +216,7 @@ __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, fl
 //       dc = c - mu, or hb_dclash for a donor/acceptor pair
 //   H = -[hb, d<3.4] exp(-(d-2.88)^2/(2*0.3^2)):  eH += ..., only in records that hold such a pair
 // GRAD: f_i += s (x_a - x_b) with s = (de/dd) / d / kappa.  A slot without a pair has c = -1e15 and adds 0.
-template <bool GRAD>
+template <bool GRAD, bool ENERGY>
 __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], const float ay[4], const float az[4],
                                          float bx, float by, float bz, const float4 c4, unsigned hbmask,
                                          float& eL, float& eC, float& eH, float fx[4], float fy[4], float fz[4]) {
@@ -237,9 +237,8 @@ __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], cons
         const float u = t * K.nk2;
         float g = ex2_approx(u * t);
         g = d[i] < K.dmax ? g : 0.f;
-        eL += g;
         const float q = dc[i] * fminf(rinv[i], K.inv_floor);         // dc / max(d, floor); > 1 inside the clash range
-        eC += lg2_approx(fmaxf(q, 1.f));
+        if (ENERGY) { eL += g; eC += lg2_approx(fmaxf(q, 1.f)); }
         if (GRAD) {
             s[i] = u * g * rinv[i];
             if (q > 1.f && rinv[i] < K.inv_floor) s[i] = fmaf(-K.kc * rinv[i], rinv[i], s[i]);
@@ -252,7 +251,7 @@ __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], cons
                 const float th = d[i] - K.hb_mu;
                 float gh = ex2_approx(K.hb_nk2 * th * th);
                 gh = d[i] < K.hb_dmax ? gh : 0.f;
-                eH += gh;
+                if (ENERGY) eH += gh;
                 if (GRAD) s[i] = fmaf(K.kh * th, gh * rinv[i], s[i]);
             }
         }
@@ -265,7 +264,7 @@ __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], cons
 
 // One tile: w <= 4 consecutive own atoms a0 .. a0+w-1 of fragment g against n_runs runs of partner atoms; hp / rp walk
 // the header units / the two record arrays.  GRAD: acc += the wrench the tile's atoms receive; WR[fb] -= each run's wrench.
-template <bool GRAD, class XS>
+template <bool GRAD, bool ENERGY, class XS>
 __device__ __forceinline__ void lane_tile(const uint4*& hp, const float4*& rc, const uint32_t*& rm, int a0, int w, int n_runs, const PairK& K,
                                           const XS& X, float* __restrict__ WR, int C,
                                           float acc[6], float& eL, float& eC, float& eH) {
@@ -293,7 +292,7 @@ __device__ __forceinline__ void lane_tile(const uint4*& hp, const float4*& rc, c
             float nx, ny, nz;
             X.fence(bx, by, bz);
             X.get((int)(mtn & 0xffffu), nx, ny, nz);
-            lane_rec<GRAD>(K, ax, ay, az, bx, by, bz, c4, mt >> 16, eL, eC, eH, fx, fy, fz);
+            lane_rec<GRAD, ENERGY>(K, ax, ay, az, bx, by, bz, c4, mt >> 16, eL, eC, eH, fx, fy, fz);
             c4 = c4n; mt = mtn; bx = nx; by = ny; bz = nz;
         }
         X.fence(bx, by, bz);
@@ -319,7 +318,7 @@ __device__ __forceinline__ void lane_tile(const uint4*& hp, const float4*& rc, c
 }
 
 // All pairs of the ligand.  GRAD: WR[g] (initialised by lane_grid) += the pair wrenches.
-template <bool GRAD, class XS>
+template <bool GRAD, bool ENERGY, class XS>
 __device__ __forceinline__ float lane_pairs(const LaneTopo& S, const PairK& K, const XS& X, float* __restrict__ WR, int C) {
     float eL = 0.f, eC = 0.f, eH = 0.f;
     const uint4* hp = S.stream;
@@ -331,7 +330,7 @@ __device__ __forceinline__ float lane_pairs(const LaneTopo& S, const PairK& K, c
         float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         for (int tl = 0; tl < n_tiles; ++tl) {
             const uint4 h = *hp++;
-            lane_tile<GRAD, XS>(hp, rc, rm, (int)h.x, (int)h.y, (int)h.z, K, X, WR, C, acc, eL, eC, eH);
+            lane_tile<GRAD, ENERGY, XS>(hp, rc, rm, (int)h.x, (int)h.y, (int)h.z, K, X, WR, C, acc, eL, eC, eH);
         }
         if (GRAD) {
             float* wg = WR + 6 * g * C;
@@ -344,14 +343,15 @@ __device__ __forceinline__ float lane_pairs(const LaneTopo& S, const PairK& K, c
 
 // ------------------------------------------------------------------ a3..a5: one pose evaluation by one lane
 // In : t[3], unit q[4] (registers), th[(g-1)*C] torsion angles (shared), grad (warp-uniform).
-// Out: X (world coordinates), e_inter, e_intra; grad: WR[g] = wrench on the own atoms of fragment g.
-template <class XS>
+// Out: X (world coordinates), e_inter, e_intra (e_intra of a gradient evaluation only if GE); grad: WR[g] = wrench on the
+//      own atoms of fragment g.
+template <bool GE, class XS>
 __device__ __forceinline__ void lane_eval(const LaneTopo& S, const DGrid& G, const DParams& P, const PairK& K, bool grad,
                                           const float t[3], const float q[4], const float* __restrict__ th,
                                           const XS& X, float* __restrict__ WR, int C, float& e_inter, float& e_intra) {
     lane_fk(S, t, q, th, X, WR, C);
     e_inter = lane_grid(S, G, P.k_wall, grad, X, WR, C);
-    e_intra = grad ? lane_pairs<true, XS>(S, K, X, WR, C) : lane_pairs<false, XS>(S, K, X, WR, C);
+    e_intra = grad ? lane_pairs<true, GE, XS>(S, K, X, WR, C) : lane_pairs<false, true, XS>(S, K, X, WR, C);
 }
 
 // ------------------------------------------------------------------ a6 reverse mode through the tree (O9)
@@ -474,7 +474,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
         for (int rf = (s >= 0 ? 0 : P.n_refine); rf <= P.n_refine; ++rf) {
             const bool grad = rf < P.n_refine;
             float ei, ea;
-            lane_eval(S, a.grid, P, K, grad, pt, pq, THP, X, WR, C, ei, ea);
+            lane_eval<false>(S, a.grid, P, K, grad, pt, pq, THP, X, WR, C, ei, ea);   // the Adam steps need no energy
             enew = ei + ea;
             if (!grad) break;
             b1p *= P.adam_b1; b2p *= P.adam_b2;
@@ -678,7 +678,7 @@ __global__ void __launch_bounds__(32) score_lane_kernel(const ScoreLaunch a) {
     quat_normalise(q);
     for (int g = 1; g <= T; ++g) TH[(g - 1) * C] = src[7 + S.frag[g].tor];
     float ei, ea;
-    lane_eval(S, a.grid, a.P, K, a.grad != nullptr, t, q, TH, X, WR, C, ei, ea);
+    lane_eval<true>(S, a.grid, a.P, K, a.grad != nullptr, t, q, TH, X, WR, C, ei, ea);
     a.energy[3 * (size_t)i] = ei + ea; a.energy[3 * (size_t)i + 1] = ei; a.energy[3 * (size_t)i + 2] = ea;
     if (a.grad != nullptr) {
         float* gr = a.grad + (size_t)i * a.grad_stride;
