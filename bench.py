@@ -107,6 +107,7 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
 
     cfg = synth.CONFIGS[name]
     gp = default_params()
+    gp.n_refine = cfg.n_refine
     rec = synth.make_receptor(cfg)
     radius, role = synth.type_table(cfg.n_types)
     batch_all = synth.make_ligands(cfg, n_lig)
@@ -228,7 +229,9 @@ def oracle_setup(name, n_lig):
     rec = synth.make_receptor(cfg)
     radius, role = synth.type_table(cfg.n_types)
     batch = synth.make_ligands(cfg, n_lig)
-    return orc, cfg, rec, orc.Types(radius, role), orc.default_params(), batch
+    p = orc.default_params()
+    p.n_refine = cfg.n_refine
+    return orc, cfg, rec, orc.Types(radius, role), p, batch
 
 
 def oracle_time(name, budget_s=20.0, grid=None):
@@ -272,7 +275,7 @@ def run_reference(args):
         vals.append(oracle_time(name, budget_s=8.0, grid=first["G"]))
     timed = vals[-args.steps:]
     rate = float(np.mean([v["dock_evals_per_s"] for v in timed]))
-    evals_step = cfg.n_lig * cfg.n_chains * (cfg.n_steps * 2 + 1)
+    evals_step = cfg.n_lig * cfg.n_chains * (cfg.n_steps * (cfg.n_refine + 1) + 1)
     t_step = first["t_grid"] + evals_step / rate
     value = evals_step / t_step
     line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
@@ -333,15 +336,15 @@ def main():
     cfg = synth.CONFIGS[args.workload]
     cpu = None
     if not args.no_cpu and args.n_lig is None:
-        cpu = cpu_baseline(args.workload, cfg.n_chains * (cfg.n_steps * 2 + 1), cfg.n_lig)
-    idx = int(args.workload[1]) - 1
+        cpu = cpu_baseline(args.workload, cfg.n_chains * (cfg.n_steps * (cfg.n_refine + 1) + 1), cfg.n_lig)
+    idx = int(args.workload[1]) - 1 if args.workload[0] == "C" else -1
     line = dict(
         metric=METRIC, value=main_res["value"], unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
         ms_per_step=main_res["ms_per_step"], higher_is_better=True, scaling=main_res["scaling"], vs_baseline=None,
         dtype="f32", data="synthetic",
-        config=dict(workload=f"{args.workload} {cfg.title} (BASELINE.json configs[{idx}])", n_ligands=main_res["n_lig"] * world
+        config=dict(workload=f"{args.workload} {cfg.title}" + (f" (BASELINE.json configs[{idx}])" if idx >= 0 else " (not a BASELINE.json config)"), n_ligands=main_res["n_lig"] * world
                     if main_res["scaling"] == "strong" else main_res["n_lig"], n_chains=cfg.n_chains, n_mc_steps=cfg.n_steps,
-                    top_k=cfg.top_k, n_refine=1, l2="flushed between steps (256 MiB memset outside the timed events)",
+                    top_k=cfg.top_k, n_refine=cfg.n_refine, l2="flushed between steps (256 MiB memset outside the timed events)",
                     step="grid build (a0) + init + MC steps + top-k (a1..a10), one CUDA-graph launch"),
         score_grad_evals_per_s=main_res["score_grad_evals_per_s"], ms_per_task=main_res["ms_per_task"],
         ms_grid_build=main_res["ms_grid_build"], ms_mc_kernels=main_res["ms_mc_kernels"], ms_topk=main_res["ms_topk"],

@@ -231,6 +231,7 @@ class Config:
     philox_seed: int = 0
     backbone: int = 0
     sizes: dict = field(default_factory=dict)
+    n_refine: int = 1
 
 
 CONFIGS = {
@@ -239,6 +240,11 @@ CONFIGS = {
     "C3": Config("C3", "Screening batch", 3000, 30.0, 80, 16, 4096, 128, 500, 1, 1003, 2003),
     "C4": Config("C4", "Large flexible ligand", 3000, 40.0, 107, 16, 1, 1024, 2000, 1, 1004, 2004, backbone=24),
     "C5": Config("C5", "High-throughput screen", 5000, 30.0, 80, 16, 65536, 64, 300, 1, 1005, 2005),
+    # Not a BASELINE.json config: the sampling shape the paper states for its own runs (1,024 copies, depth 8,
+    # Adam refinement in every loop; 8 output poses) on the C2 receptor and ligand.  The number of Adam iterations
+    # per loop is not stated in the paper; 32 is this build's choice (G12).
+    "P1": Config("P1", "Paper-shaped run (1,024 copies x 8 loops x 32 Adam steps)", 3000, 30.0, 80, 16, 1, 1024, 8, 8, 1002, 2002,
+                 n_refine=32),
 }
 
 
@@ -248,7 +254,7 @@ def config_sizes(cfg: Config, n_lig: int | None = None):
     rng = np.random.default_rng(cfg.lig_seed)
     if cfg.name == "C1":
         return np.full(L, 12), np.full(L, 2)
-    if cfg.name == "C2":
+    if cfg.name in ("C2", "P1"):
         return np.full(L, 30), np.full(L, 6)
     if cfg.name == "C3":
         n = rng.integers(15, 51, size=cfg.n_lig)
