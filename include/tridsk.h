@@ -114,6 +114,11 @@ typedef struct {
     int no_graph;              /* 1: plain stream launches instead of a captured CUDA graph                           */
     int chain_base;            /* Philox chain id of local chain 0 (chain sharding across GPUs; results then do not
                                   depend on the GPU count)                                                            */
+    float cluster_rmsd;        /* > 0: duplicate removal in the top-k ("clustered to remove the duplicates"; G20):
+                                  chains are walked in (E_best, chain id) order and a pose whose heavy-atom RMSD (same
+                                  atom order, receptor frame) to an already kept pose is below this many Angstrom is
+                                  skipped.  Slots left over get chain -1, energies +inf and a zero pose.  Needs
+                                  top_k * max_atoms <= 4096.  0: plain top-k (O13)                                     */
 } tridsk_dock_opts;
 
 /* ---- lifetime ------------------------------------------------------------------------------ */
@@ -171,6 +176,7 @@ int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_lig
  * box_min/box_max/pocket_center: [host].  Outputs [host|dev]:
  *   out_energy[n_lig][top_k][2] = {E_dock, E_screen = E_dock/(1 + w_tor*T)};
  *   out_pose[n_lig][top_k][pose_stride]; out_chain[n_lig][top_k].  top_k <= n_chains.
+ * opts->cluster_rmsd > 0 replaces the plain top-k by the duplicate-removing one (O14).
  */
 int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* ligs, const tridsk_params* params,
                 const float box_min[3], const float box_max[3], const float pocket_center[3], float pocket_radius,

@@ -268,6 +268,31 @@ def topk(e_best, k):
     return order[:k]
 
 
+def topk_cluster(e_best, pose_best, L: Ligand, k, rmsd_min):
+    """O14 ("ranked ... clustered to remove the duplicates ... top N"; reading G20): walk the chains in the order
+    of O13; a chain's best pose is a duplicate if its heavy-atom RMSD (same atom order, no superposition: poses live in
+    the receptor frame) to an already kept pose is below rmsd_min, otherwise it is kept; stop at k kept.
+    -> (kept chain ids, length <= k; margin = the smallest |RMSD - rmsd_min| met on the way, for tie detection)."""
+    e_best = np.asarray(e_best)
+    order = np.lexsort((np.arange(len(e_best)), e_best))
+    kept, kept_x, margin = [], [], np.inf
+    for c in order:
+        if len(kept) == k:
+            break
+        x = fk(L, np.asarray(pose_best[c], dtype=np.float64)[:7 + L.T])
+        dup = False
+        for kx in kept_x:                                     # plain loop, in kept order; every comparison is made
+            rmsd = float(np.sqrt(np.mean(np.sum((x - kx) ** 2, axis=1))))
+            margin = min(margin, abs(rmsd - rmsd_min))
+            if rmsd < rmsd_min:
+                dup = True
+                break
+        if not dup:
+            kept.append(int(c))
+            kept_x.append(x)
+    return np.array(kept, dtype=np.int64), margin
+
+
 def e_screen(e_dock, n_tor, w_tor=0.01):
     """Eq.E_screen, P:135-137."""
     return e_dock / (1.0 + w_tor * n_tor)

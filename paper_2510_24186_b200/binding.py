@@ -46,7 +46,7 @@ class _Batch(C.Structure):
 class _DockOpts(C.Structure):
     _fields_ = [("first_step", C.c_int), ("init_poses", C.c_void_p), ("resume", C.c_int),
                 ("chain_state", C.c_void_p), ("trace", C.c_void_p), ("steps_per_launch", C.c_int),
-                ("no_graph", C.c_int), ("chain_base", C.c_int)]
+                ("no_graph", C.c_int), ("chain_base", C.c_int), ("cluster_rmsd", C.c_float)]
 
 
 TRACE_DTYPE = np.dtype([("e_prop", np.float32), ("e_cur", np.float32), ("u", np.float32), ("flags", np.int32)])
@@ -277,7 +277,7 @@ class Engine:
     def dock(self, grid: Grid, ligs: Ligands, params, box_min, box_max, pocket_center, pocket_radius,
              n_chains, n_steps, top_k, seed=0, pose_stride=None, device_out=False, init_poses=None,
              first_step=0, resume=False, chain_state=None, want_state=False, want_trace=False,
-             steps_per_launch=0, no_graph=False, chain_base=0, out=None):
+             steps_per_launch=0, no_graph=False, chain_base=0, out=None, cluster_rmsd=0.0):
         """-> dict(energy[n_lig,k,2], pose[n_lig,k,stride], chain[n_lig,k], state?, trace?).
         device_out: outputs are CUDA torch tensors (no D2H, no sync); else numpy (D2H inside the call).
         out: optional pre-allocated (energy, pose, chain) buffers to write into."""
@@ -298,6 +298,7 @@ class Engine:
         o.first_step, o.resume = int(first_step), int(bool(resume))
         o.steps_per_launch, o.no_graph = int(steps_per_launch), int(bool(no_graph))
         o.chain_base = int(chain_base)
+        o.cluster_rmsd = float(cluster_rmsd)
         keep = []
         if init_poses is not None:
             if isinstance(init_poses, np.ndarray):

@@ -802,6 +802,9 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     if (params->n_refine < 0 || o.first_step < 0 || o.steps_per_launch < 0) return fail(ctx, TRIDSK_EINVAL, "bad option");
     if (o.resume && !o.chain_state) return fail(ctx, TRIDSK_EINVAL, "resume needs chain_state");
     if (o.resume && o.init_poses) return fail(ctx, TRIDSK_EINVAL, "resume and init_poses are exclusive");
+    if (!(o.cluster_rmsd >= 0.f)) return fail(ctx, TRIDSK_EINVAL, "cluster_rmsd must be >= 0");
+    if (o.cluster_rmsd > 0.f && (long long)top_k * ligs->max_atoms > 4096)
+        return fail(ctx, TRIDSK_ELIMIT, "duplicate-removing top-k needs top_k * max_atoms <= 4096");
     for (int c = 0; c < 3; ++c) if (!(box_min[c] <= box_max[c])) return fail(ctx, TRIDSK_EINVAL, "box_min > box_max");
     const int L = ligs->n_lig;
     if (L == 0) return TRIDSK_OK;
@@ -908,6 +911,8 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     memset(&tk, 0, sizeof(tk));
     tk.hdr = ligs->hdr; tk.e_best = base.e_best; tk.pose_best = base.pose_best;
     tk.n_lig = L; tk.n_chains = n_chains; tk.pose_stride = pose_stride; tk.top_k = top_k; tk.w_tor = params->w_tor;
+    tk.atom_f4 = ligs->atom_f4; tk.lane_frags = ligs->lane_frags; tk.cluster_rmsd = o.cluster_rmsd;
+    tk.max_atoms = ligs->max_atoms; tk.max_tor = ligs->max_tor;
     tk.out_energy = h_oe ? (float*)ob : out_energy;
     tk.out_pose = h_op ? (float*)(ob + o_p) : out_pose;
     tk.out_chain = h_oc ? (int*)(ob + o_c) : out_chain;

@@ -169,6 +169,10 @@ struct TopkLaunch {
     int n_lig, n_chains, pose_stride, top_k;
     float w_tor;
     float* out_energy; float* out_pose; int* out_chain;
+    // duplicate-removing form (cluster_rmsd > 0): the ligands' reference conformers and fragment records for the FK
+    const float4* atom_f4; const LaneFrag* lane_frags;
+    float cluster_rmsd;
+    int max_atoms, max_tor;
 };
 
 // ---------------------------------------------------------------- lane-per-chain kernel: shared-memory budget
@@ -293,4 +297,5 @@ cudaError_t launch_score(cudaStream_t s, const ScoreLaunch& a);
 cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int threads, size_t smem_bytes);
 cudaError_t launch_score_cta(cudaStream_t s, const ScoreLaunch& a, size_t smem_bytes);
 cudaError_t launch_topk(cudaStream_t s, const TopkLaunch& a);
+size_t topk_cluster_smem(int top_k, int max_atoms, int max_tor);
 cudaError_t launch_philox_debug(cudaStream_t s, const unsigned int* ctr_key /* dev[6] */, unsigned int* out /* dev[4] */);

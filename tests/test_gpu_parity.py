@@ -508,3 +508,43 @@ def test_tensor_memory_lane_kernel_is_bit_identical_to_shared_memory_lane_kernel
             e.close()
     for k in ("energy", "pose", "chain"):
         assert np.array_equal(out[2][k], out[4][k]), k
+
+
+def test_duplicate_removing_topk_matches_oracle(orc, gp, system):
+    """O14 ("clustered to remove the duplicates", G20): the kept chains, their order and the left-over slots of the
+    GPU's duplicate-removing top-k equal the oracle's greedy pass over the same per-chain best poses; decisions within
+    1e-3 A of the threshold (fp32 vs fp64 RMSD) are excluded by construction of the check."""
+    from paper_2510_24186_b200 import Engine, split_state
+    rec, batch = system["rec"], system["batch"]
+    radius, role = system["radius"], system["role"]
+    e = Engine(0)
+    try:
+        grid = e.build_grid(rec.xyz, rec.type, radius, role, gp, rec.origin, rec.dims, rec.spacing)
+        ligs = e.load_ligands(batch, radius, role)
+        n_ch, k = 96, 6
+        checked = 0
+        for thr in (0.5, 2.0, 6.0, 50.0):
+            r = e.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, n_ch, 30, k, seed=3,
+                       want_state=True, cluster_rmsd=thr)
+            _, pb, _, eb = split_state(r["state"], batch.n_lig, n_ch, 7 + ligs.max_tor)
+            for l in range(batch.n_lig):
+                L = orc.ligand_from_batch(batch, l)
+                kept, margin = orc.topk_cluster(eb[l], pb[l], L, k, thr)
+                if margin < 1e-3:
+                    continue
+                checked += 1
+                want = np.full(k, -1)
+                want[:len(kept)] = kept
+                assert np.array_equal(r["chain"][l], want), (thr, l, r["chain"][l], want)
+                assert np.array_equal(r["energy"][l, :len(kept), 0], eb[l][kept])
+                assert np.all(np.isinf(r["energy"][l, len(kept):, 0])) and np.all(r["pose"][l, len(kept):] == 0)
+                for j, c in enumerate(kept):
+                    assert np.array_equal(r["pose"][l, j], pb[l, c])
+        assert checked >= 3 * batch.n_lig
+        # cluster_rmsd = 0 is the plain top-k
+        r0 = e.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, n_ch, 30, k, seed=3)
+        r1 = e.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, n_ch, 30, k, seed=3,
+                    cluster_rmsd=1e-6)
+        assert np.array_equal(r0["chain"], r1["chain"])
+    finally:
+        e.close()

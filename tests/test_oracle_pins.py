@@ -600,3 +600,53 @@ def test_dock_sanity_and_topk(orc, dock_system):
     # Eq.E_screen
     assert orc.e_screen(-50.0, 6) == pytest.approx(-50.0 / 1.06)
     assert orc.e_screen(-50.0, 0) == -50.0
+
+
+# --------------------------------------------------------------------------- O14: duplicate-removing top-k (G20)
+def test_topk_cluster_constructed_cases_and_invariants(orc, dock_system):
+    S = dock_system
+    L = S["L"][1]
+    W = 7 + L.T
+    rng = np.random.default_rng(11)
+    base = np.zeros(W)
+    base[3] = 1.0
+    base[7:] = rng.uniform(-1, 1, L.T)
+    # a rigid translation by v moves every atom by v: RMSD = |v| exactly (closed form)
+    shifts = np.array([0.0, 0.3, 0.9, 1.1, 2.5, 2.6, 4.0])
+    poses = np.tile(base, (len(shifts), 1))
+    poses[:, 0] = shifts
+    x0 = orc.fk(L, poses[0])
+    for i, sh in enumerate(shifts):
+        xi = orc.fk(L, poses[i])
+        assert np.sqrt(np.mean(np.sum((xi - x0) ** 2, axis=1))) == pytest.approx(sh, abs=1e-12)
+    e = np.array([-9.0, -8.0, -7.0, -6.0, -5.0, -4.0, -3.0])
+    kept, margin = orc.topk_cluster(e, poses, L, 4, 1.0)
+    # 0 kept; 0.3, 0.9 are within 1 A of it; 1.1 kept; 2.5 is 1.4 from 1.1 -> kept; 2.6 within 0.1 of 2.5; 4.0 kept
+    assert list(kept) == [0, 3, 4, 6] and margin == pytest.approx(0.1, abs=1e-9)
+    # no threshold -> plain O13; a huge threshold -> one cluster; k larger than the number of clusters -> fewer ids
+    assert list(orc.topk_cluster(e, poses, L, 4, 0.0)[0]) == list(orc.topk(e, 4))
+    assert list(orc.topk_cluster(e, poses, L, 4, 100.0)[0]) == [0]
+    assert list(orc.topk_cluster(e, poses, L, 7, 1.0)[0]) == [0, 3, 4, 6]
+    # the energy order decides who represents a cluster: reverse the energies
+    assert list(orc.topk_cluster(-e, poses, L, 3, 1.0)[0]) == [6, 5, 3]
+    # invariants on random poses: kept poses are pairwise >= thr apart, every skipped better-ranked chain is a duplicate
+    n_ch = 40
+    P = np.zeros((n_ch, W))
+    P[:, 0:3] = rng.normal(0, 0.8, (n_ch, 3))
+    q = rng.normal(size=(n_ch, 4)) * 0.15 + np.array([1, 0, 0, 0])
+    P[:, 3:7] = q / np.linalg.norm(q, axis=1, keepdims=True)
+    P[:, 7:] = base[7:] + rng.normal(0, 0.2, (n_ch, L.T))
+    E = rng.normal(size=n_ch)
+    thr = 1.5
+    kept, _ = orc.topk_cluster(E, P, L, 5, thr)
+    X = [orc.fk(L, P[c]) for c in range(n_ch)]
+    rmsd = lambda a, b: np.sqrt(np.mean(np.sum((X[a] - X[b]) ** 2, axis=1)))
+    assert 1 <= len(kept) <= 5
+    for i in range(len(kept)):
+        for j in range(i):
+            assert rmsd(kept[i], kept[j]) >= thr
+    order = list(orc.topk(E, n_ch))
+    last = order.index(kept[-1])
+    for c in order[:last]:
+        if c not in kept:
+            assert any(rmsd(c, kk) < thr for kk in kept if order.index(kk) < order.index(c))
