@@ -744,7 +744,7 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
             tm_cols = 3 * h.n + 1 <= 32 ? 32 : 3 * h.n + 1 <= 64 ? 64 : 128;
             region = (topo + 32 * (per_chain - 12 * (size_t)h.n) + 15) / 16 * 16;
             const size_t cta = (4 * region + 1023) / 1024 * 1024 + TRIDSK_SMEM_RESERVED;
-            tm_r = (int)std::min<size_t>(std::min<size_t>(TRIDSK_SMEM_PER_SM / cta, 512 / tm_cols), 4);
+            tm_r = (int)std::min<size_t>(std::min<size_t>(TRIDSK_SMEM_PER_SM / cta, 512 / tm_cols), 3);
             if (4 * region > TRIDSK_SMEM_MAX_CTA - 1024) tm_r = 0;
         }
         if (c == 0 && tm_r == 0) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the lane kernel's shared memory");

@@ -572,7 +572,7 @@ __global__ void __launch_bounds__(128, 4) mc_lane_kernel(const McLaunch a) {
 
 // Coordinates in tensor memory: one CTA = 4 warps, every WARP takes its own work item (ligand, block of 32 chains) and
 // stages that ligand's topology into its own quarter of the CTA's shared memory; warp w owns TMEM lanes 32w .. 32w+31.
-__global__ void __launch_bounds__(128, 4) mc_lane_tm_kernel(const McLaunch a) {
+__global__ void __launch_bounds__(128, 3) mc_lane_tm_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char lane_smem[];
     __shared__ uint32_t tm_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, C = 32;
