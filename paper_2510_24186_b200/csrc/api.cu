@@ -413,6 +413,31 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
         };
         std::vector<int> gof(n);                 // pre-order fragment of an internal atom
         for (int g = 0; g <= T; ++g) for (int a = out.lane_frags[g].lo; a < out.lane_frags[g].own_hi; ++a) gof[a] = g;
+        // which of the two fragments of a pair supplies the 4-slot tiles: the one that needs fewer records (a 5-atom
+        // fragment against a 4-atom one is 2 tiles x 4 partners = 8 records one way, 1 tile x 5 partners = 5 the other)
+        auto tiles_of = [&](int g, std::vector<std::pair<int, int>>& tl) {
+            tl.clear();
+            const int lo_g = out.lane_frags[g].lo, cnt = out.lane_frags[g].own_hi - lo_g, nt = (cnt + 3) / 4;
+            for (int t = 0, a0 = lo_g; t < nt; ++t) { const int w = cnt / nt + (t < cnt % nt ? 1 : 0); tl.push_back({a0, w}); a0 += w; }
+        };
+        auto rec_count = [&](int ft, int fp) {
+            std::vector<std::pair<int, int>> tl;
+            tiles_of(ft, tl);
+            int cnt = 0;
+            for (auto& t : tl)
+                for (int y = out.lane_frags[fp].lo; y < out.lane_frags[fp].own_hi; ++y) {
+                    bool any = false;
+                    for (int i = 0; i < t.second; ++i) any = any || pm[(size_t)(t.first + i) * n + y];
+                    cnt += any;
+                }
+            return cnt;
+        };
+        std::vector<unsigned char> tile_side((size_t)(T + 1) * (T + 1), 0);    // [g][fb] = 1: g supplies the tiles of the pair {g, fb}
+        for (int g = 0; g <= T; ++g)
+            for (int fb = g + 1; fb <= T; ++fb) {
+                const bool g_side = rec_count(g, fb) <= rec_count(fb, g);
+                tile_side[(size_t)g * (T + 1) + fb] = g_side; tile_side[(size_t)fb * (T + 1) + g] = !g_side;
+            }
         int covered2 = 0;
         for (int g = 0; g <= T; ++g) {
             const int lo_g = out.lane_frags[g].lo, cnt = out.lane_frags[g].own_hi - lo_g;
@@ -425,7 +450,8 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
                 const size_t tile_at = out.lane_stream.size();
                 out.lane_stream.push_back(make_uint4((unsigned)a0, (unsigned)w, 0u, 0u));
                 unsigned n_runs = 0;
-                for (int fb = g; fb <= T; ++fb) {             // fb == g: only explicit pair lists can pair a fragment with itself
+                for (int fb = 0; fb <= T; ++fb) {             // fb == g: only explicit pair lists can pair a fragment with itself
+                    if (fb != g && !tile_side[(size_t)g * (T + 1) + fb]) continue;
                     unsigned nb = 0;
                     for (int y = out.lane_frags[fb].lo; y < out.lane_frags[fb].own_hi; ++y) {
                         LaneRec rec;
@@ -435,7 +461,7 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
                         for (int i = 0; i < 4; ++i) {
                             const int x = a0 + i;
                             rec.dvdw[i] = -1.f;                               // no pair in this slot
-                            if (i < w && x < y && pm[(size_t)x * n + y]) {
+                            if (i < w && (fb != g || x < y) && pm[(size_t)x * n + y]) {
                                 any = true; ++covered2;
                                 rec.dvdw[i] = out.f4[x].w + out.f4[y].w;      // layout: operands of the pair function
                                 if (hbp(x, y)) rec.hbmask |= 1u << i;
@@ -570,6 +596,12 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
         std::copy(pk[i].ai.begin(), pk[i].ai.end(), ai.begin() + h.atom_off);
         std::copy(pk[i].fr.begin(), pk[i].fr.end(), fr.begin() + h.frag_off);
         std::copy(pk[i].rounds.begin(), pk[i].rounds.end(), rd.begin() + h.round_off);
+    }
+    if (getenv("TRIDSK_DEBUG")) {
+        long long np = 0;
+        for (int i = 0; i < L; ++i) np += pk[i].h.n_pairs;
+        fprintf(stderr, "tridsk load_ligands: %d ligands, %lld pairs in %zu 4-slot records (slot utilisation %.1f %%)\n", L, np, nrec,
+                nrec ? 25.0 * (double)np / (double)nrec : 0.0);
     }
     cudaError_t e = cudaSuccess;
     auto up = [&](void** d, const void* src, size_t bytes) {

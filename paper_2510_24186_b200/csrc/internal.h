@@ -72,7 +72,8 @@ struct LaneFrag {
 // consume in order.  For every fragment g (pre-order):
 //   {n_tiles, 0, 0, 0}
 //   per tile (1..4 consecutive own atoms a0 .. a0+w-1 of g):   {a0, w, n_runs, 0}
-//     per run (partner atoms in ONE later fragment fb):          {fb, n_rec, 0, 0}   -> the next n_rec records
+//     per run (partner atoms in ONE other fragment fb):          {fb, n_rec, 0, 0}   -> the next n_rec records
+// Of the two fragments of a pair, the one that needs fewer records supplies the tiles (api.cu).
 // One record = one partner atom b against the 4 slots of the tile.  In global memory (LaneRec) it holds what depends
 // on the ligand only; lane_stage turns it into the 20-byte shared-memory form (two arrays) that also depends on the
 // parameters:  c[4] = dvdw + long_mu (slot without a pair -- excluded, or beyond the tile width: -1e15), and one word
