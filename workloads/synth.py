@@ -243,6 +243,9 @@ CONFIGS = {
     # Not a BASELINE.json config: the sampling shape the paper states for its own runs (1,024 copies, depth 8,
     # Adam refinement in every loop; 8 output poses) on the C2 receptor and ligand.  The number of Adam iterations
     # per loop is not stated in the paper; 32 is this build's choice (G12).
+    # Not a BASELINE.json config: 32 independent copies of the C2 dock in one batch ("C2 run as 32 concurrent
+    # independent docks to show the kernel's rate when fed")
+    "C2x32": Config("C2x32", "32 concurrent drug-like single docks", 3000, 30.0, 80, 16, 32, 384, 1000, 10, 1002, 2002),
     "P1": Config("P1", "Paper-shaped run (1,024 copies x 8 loops x 32 Adam steps)", 3000, 30.0, 80, 16, 1, 1024, 8, 8, 1002, 2002,
                  n_refine=32),
 }
@@ -254,7 +257,7 @@ def config_sizes(cfg: Config, n_lig: int | None = None):
     rng = np.random.default_rng(cfg.lig_seed)
     if cfg.name == "C1":
         return np.full(L, 12), np.full(L, 2)
-    if cfg.name in ("C2", "P1"):
+    if cfg.name in ("C2", "P1", "C2x32"):
         return np.full(L, 30), np.full(L, 6)
     if cfg.name == "C3":
         n = rng.integers(15, 51, size=cfg.n_lig)
