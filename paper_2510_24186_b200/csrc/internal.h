@@ -197,7 +197,7 @@ __host__ __device__ static inline int lane_chain_slots(int n, int T, int max_dep
 
 // CTA-per-chain kernel: shared-memory layout (byte offsets) -- topology {ref, meta, fragments, row offsets, records},
 // the chain's coordinates X[3][n], per-atom (force, moment about t) AF[6][n] and a reduction scratch
-struct CtaLayout { size_t ref, meta, frag, rows, recs, X, AF, red, total; };
+struct CtaLayout { size_t ref, meta, frag, rows, recs, X, AF, PF, red, total; };
 #define TRIDSK_AL16(x) (((x) + 15) / 16 * 16)
 __host__ __device__ static inline CtaLayout cta_layout(int n, int T, int n_pairs) {
     CtaLayout L;
@@ -209,6 +209,7 @@ __host__ __device__ static inline CtaLayout cta_layout(int n, int T, int n_pairs
     L.recs = o; o = TRIDSK_AL16(o + 8 * 3 * (size_t)n_pairs);
     L.X = o; o = TRIDSK_AL16(o + 12 * (size_t)n);
     L.AF = o; o = TRIDSK_AL16(o + 32 * (size_t)n);
+    L.PF = o; o = TRIDSK_AL16(o + 32 * (size_t)n);
     L.red = o; o += 4 * 64;
     L.total = o;
     return L;

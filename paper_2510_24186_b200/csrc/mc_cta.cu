@@ -21,14 +21,14 @@ struct CtaTopo {
     const LaneFrag* frag;   // [T + 1] pre-order
     const int* rows;        // [n + 1] row offsets into recs
     const uint2* recs;      // [2P] row records {b | hb << 8, c}, then [P] flat records {a | b << 8 | hb << 16, c}; c = dvdw + mu
-    float *X, *AF, *red;    // X[3][n], AF[n][8] = {force, 0, moment about t, 0}, red[64]
+    float *X, *AF, *PF, *red;  // X[3][n], AF[n][8] = {force, 0, moment about t, 0}, PF = its prefix sums, red[64]
     int n, T, P, lpa;
 };
 
 // this lane's fragment (lane g = fragment g in pre-order; lanes beyond T are idle copies of the root)
 struct CtaFrag {
     float ux, uy, uz, ox, oy, oz;
-    int parent, depth, lo, own_hi, tor, g_end;
+    int parent, depth, lo, own_hi, tor, sub_hi;              // sub_hi: end of the subtree's atom range [lo, sub_hi)
     bool valid;
 };
 
@@ -60,6 +60,7 @@ __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char*
     }
     S.ref = ref; S.meta = meta; S.frag = reinterpret_cast<const LaneFrag*>(frag); S.rows = rows; S.recs = recs;
     S.X = reinterpret_cast<float*>(smem + L.X); S.AF = reinterpret_cast<float*>(smem + L.AF);
+    S.PF = reinterpret_cast<float*>(smem + L.PF);
     S.red = reinterpret_cast<float*>(smem + L.red);
     S.n = n; S.T = T; S.P = np;
     int threads;
@@ -72,7 +73,7 @@ __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char*
     F.lo = r.lo; F.own_hi = F.valid ? r.own_hi : r.lo; F.tor = F.valid ? r.tor : -1;
     int e = lane + 1;
     while (F.valid && e <= T && S.frag[e].depth > r.depth) ++e;      // the subtree of g is the fragment range [g, g_end)
-    F.g_end = F.valid ? e : 1;
+    F.sub_hi = F.valid ? S.frag[e - 1].own_hi : 1;
 }
 
 // ------------------------------------------------------------------ O2: one pair, scalar (same arithmetic as lane_rec)
@@ -102,6 +103,54 @@ __device__ __forceinline__ void cta_pair(const PairK& K, float dx, float dy, flo
         if (GRAD) s = fmaf(K.kh * th, gh * rinv, s);
     }
     if (GRAD) { fx = fmaf(s, dx, fx); fy = fmaf(s, dy, fy); fz = fmaf(s, dz, fz); }
+}
+
+// Four pairs at a time, branch-free in the main part so that the four dependency chains interleave (a thread's pairs are
+// otherwise a serial string of shared-memory load -> rsqrt -> ex2 latencies).  A lane without a pair in slot u passes
+// ok[u] = false: its c becomes -1e15 and the slot evaluates to exactly zero.
+template <bool GRAD, bool ENERGY>
+__device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c_in[4],
+                                           const bool hb_in[4], const bool ok[4], float& eL, float& eC, float& eH,
+                                           float& fx, float& fy, float& fz) {
+    float d[4], rinv[4], s[4];
+    bool hb[4], any_hb = false;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const float c = ok[u] ? c_in[u] : -1e15f;
+        hb[u] = ok[u] && hb_in[u];
+        any_hb = any_hb || hb[u];
+        const float d2 = fmaxf(fmaf(dx[u], dx[u], fmaf(dy[u], dy[u], dz[u] * dz[u])), 1e-12f);
+        rinv[u] = rsqrt_approx(d2);
+        d[u] = d2 * rinv[u];
+        const float t = d[u] - c;
+        const float w = t * K.nk2;
+        float g = ex2_approx(w * t);
+        g = d[u] < K.dmax ? g : 0.f;
+        const float dc = hb[u] ? K.hb_dclash : c - K.mu;
+        const float q = dc * fminf(rinv[u], K.inv_floor);
+        s[u] = 0.f;
+        if (ENERGY) { eL += g; eC += lg2_approx(fmaxf(q, 1.f)); }
+        if (GRAD) {
+            s[u] = w * g * rinv[u];
+            if (q > 1.f && rinv[u] < K.inv_floor) s[u] = fmaf(-K.kc * rinv[u], rinv[u], s[u]);
+        }
+    }
+    if (any_hb) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (hb[u]) {
+                const float th = d[u] - K.hb_mu;
+                float gh = ex2_approx(K.hb_nk2 * th * th);
+                gh = d[u] < K.hb_dmax ? gh : 0.f;
+                if (ENERGY) eH += gh;
+                if (GRAD) s[u] = fmaf(K.kh * th, gh * rinv[u], s[u]);
+            }
+        }
+    }
+    if (GRAD) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { fx = fmaf(s[u], dx[u], fx); fy = fmaf(s[u], dy[u], fy); fz = fmaf(s[u], dz[u], fz); }
+    }
 }
 
 // ------------------------------------------------------------------ a3..a6: one pose evaluation by the whole CTA
@@ -176,24 +225,39 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     if (GRAD) {
         if (active) {
             const int k1 = S.rows[atom + 1];
-#pragma unroll 2
-            for (int k = S.rows[atom] + part; k < k1; k += S.lpa) {
-                const uint2 rec = S.recs[k];
-                const int b = (int)(rec.x & 0xffu);
-                cta_pair<true, ENERGY>(K, x - S.X[b], y - S.X[n + b], z - S.X[2 * n + b], __uint_as_float(rec.y), (rec.x >> 8) & 1u,
-                                       eL, eC, eH, fx, fy, fz);
+            for (int k = S.rows[atom] + part; k < k1; k += 4 * S.lpa) {
+                float dx[4], dy[4], dz[4], c[4];
+                bool hb[4], ok[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int kk = k + u * S.lpa;
+                    ok[u] = kk < k1;
+                    const uint2 rec = S.recs[ok[u] ? kk : k];
+                    const int b = (int)(rec.x & 0xffu);
+                    dx[u] = x - S.X[b]; dy[u] = y - S.X[n + b]; dz[u] = z - S.X[2 * n + b];
+                    c[u] = __uint_as_float(rec.y); hb[u] = (rec.x >> 8) & 1u;
+                }
+                cta_pairs4<true, ENERGY>(K, dx, dy, dz, c, hb, ok, eL, eC, eH, fx, fy, fz);
             }
         }
         eL *= 0.5f; eC *= 0.5f; eH *= 0.5f;                         // every pair was visited from both ends
     } else {
         const uint2* flat = S.recs + 2 * S.P;
-        float f0, f1, f2;
-#pragma unroll 2
-        for (int k = tid; k < S.P; k += blockDim.x) {
-            const uint2 rec = flat[k];
-            const int a = (int)(rec.x & 0xffu), b = (int)((rec.x >> 8) & 0xffu);
-            cta_pair<false, true>(K, S.X[a] - S.X[b], S.X[n + a] - S.X[n + b], S.X[2 * n + a] - S.X[2 * n + b], __uint_as_float(rec.y),
-                                  (rec.x >> 16) & 1u, eL, eC, eH, f0, f1, f2);
+        float f0 = 0.f, f1 = 0.f, f2 = 0.f;
+        const int nt = (int)blockDim.x;
+        for (int k = tid; k < S.P; k += 4 * nt) {
+            float dx[4], dy[4], dz[4], c[4];
+            bool hb[4], ok[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int kk = k + u * nt;
+                ok[u] = kk < S.P;
+                const uint2 rec = flat[ok[u] ? kk : k];
+                const int a = (int)(rec.x & 0xffu), b = (int)((rec.x >> 8) & 0xffu);
+                dx[u] = S.X[a] - S.X[b]; dy[u] = S.X[n + a] - S.X[n + b]; dz[u] = S.X[2 * n + a] - S.X[2 * n + b];
+                c[u] = __uint_as_float(rec.y); hb[u] = (rec.x >> 16) & 1u;
+            }
+            cta_pairs4<false, true>(K, dx, dy, dz, c, hb, ok, eL, eC, eH, f0, f1, f2);
         }
     }
     // ---- a4 receptor term of this thread's atom (the gathers were issued before the barrier)
@@ -225,29 +289,44 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     }
     if (!GRAD) return;
 
-    // ---- a6 reverse mode through the tree (O9): own-atom sums per fragment, inclusive scan over the pre-order, a
-    // subtree is a contiguous fragment range
-    float v[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    for (int a = F.lo; a < F.own_hi; ++a) {
-        const float4 f = reinterpret_cast<const float4*>(S.AF)[2 * a], mo = reinterpret_cast<const float4*>(S.AF)[2 * a + 1];
-        v[0] += f.x; v[1] += f.y; v[2] += f.z; v[3] += mo.x; v[4] += mo.y; v[5] += mo.z;
+    // ---- a6 reverse mode through the tree (O9): inclusive prefix sums of the per-atom (force, moment) records over the
+    // depth-first atom order (32 atoms per round, shuffle scan + carry); a fragment's subtree is the contiguous atom range
+    // [lo, sub_hi), so its wrench is a difference of two prefix entries.  Every warp writes the same prefix values to PF.
+    float carry[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    float4* PF = reinterpret_cast<float4*>(S.PF);
+    for (int a0 = 0; a0 < n; a0 += 32) {
+        const int a = a0 + lane;
+        float v[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        if (a < n) {
+            const float4 f = reinterpret_cast<const float4*>(S.AF)[2 * a], mo = reinterpret_cast<const float4*>(S.AF)[2 * a + 1];
+            v[0] = f.x; v[1] = f.y; v[2] = f.z; v[3] = mo.x; v[4] = mo.y; v[5] = mo.z;
+        }
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+#pragma unroll
+            for (int c = 0; c < 6; ++c) {
+                const float u = __shfl_up_sync(FULL_MASK, v[c], o);
+                if (lane >= o) v[c] += u;
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 6; ++c) v[c] += carry[c];
+        if (a < n) { PF[2 * a] = make_float4(v[0], v[1], v[2], 0.f); PF[2 * a + 1] = make_float4(v[3], v[4], v[5], 0.f); }
+#pragma unroll
+        for (int c = 0; c < 6; ++c) carry[c] = __shfl_sync(FULL_MASK, v[c], 31);
     }
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-#pragma unroll
-        for (int c = 0; c < 6; ++c) {
-            const float u = __shfl_up_sync(FULL_MASK, v[c], o);
-            if (lane >= o) v[c] += u;
+    __syncwarp();
+    float s[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (F.valid) {
+        const float4 hf = PF[2 * (F.sub_hi - 1)], hm = PF[2 * (F.sub_hi - 1) + 1];
+        s[0] = hf.x; s[1] = hf.y; s[2] = hf.z; s[3] = hm.x; s[4] = hm.y; s[5] = hm.z;
+        if (F.lo > 0) {
+            const float4 lf = PF[2 * (F.lo - 1)], lm = PF[2 * (F.lo - 1) + 1];
+            s[0] -= lf.x; s[1] -= lf.y; s[2] -= lf.z; s[3] -= lm.x; s[4] -= lm.y; s[5] -= lm.z;
         }
     }
-    float s[6];
 #pragma unroll
-    for (int c = 0; c < 6; ++c) {
-        const float hi = __shfl_sync(FULL_MASK, v[c], F.g_end - 1);
-        const float lo = __shfl_sync(FULL_MASK, v[c], lane > 0 ? lane - 1 : 0);
-        s[c] = hi - (lane > 0 ? lo : 0.f);
-        g6[c] = __shfl_sync(FULL_MASK, v[c], 31);
-    }
+    for (int c = 0; c < 6; ++c) g6[c] = carry[c];
     gth = 0.f;
     if (F.valid && lane >= 1) {
         const float wx = R[0] * F.ux + R[1] * F.uy + R[2] * F.uz;
