@@ -455,7 +455,7 @@ __global__ void __launch_bounds__(256, 2) mc_cta_kernel(const McLaunch a) {
             for (int i = 0; i < 7; ++i) {                            // division / square root to 2 ulp: far inside the tolerance
                 m[i] = P.adam_b1 * m[i] + (1.f - P.adam_b1) * g[i];
                 v[i] = P.adam_b2 * v[i] + (1.f - P.adam_b2) * g[i] * g[i];
-                dl[i] = __fdividef(-P.lr * (m[i] * c1), __fsqrt_rn(v[i] * c2) + P.adam_eps);
+                dl[i] = __fdividef(-P.lr * (m[i] * c1), sqrt_approx(v[i] * c2) + P.adam_eps);
             }
             pt[0] = fminf(fmaxf(pt[0] + dl[0], a.box_min[0]), a.box_max[0]);
             pt[1] = fminf(fmaxf(pt[1] + dl[1], a.box_min[1]), a.box_max[1]);

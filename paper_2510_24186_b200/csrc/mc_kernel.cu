@@ -111,13 +111,14 @@ __global__ void __launch_bounds__(TRIDSK_WARPS_PER_CTA * 32) mc_kernel(const McL
             float ei, ea;
             eval_pose<J, true>(L, a.grid, P, pt, pq, pth, x, y, z, ei, ea, gt, gw, gth, sP);
             b1p *= P.adam_b1; b2p *= P.adam_b2;
-            const float c1 = 1.f / (1.f - b1p), c2 = 1.f / (1.f - b2p);
+            const float c1 = __fdividef(1.f, 1.f - b1p), c2 = __fdividef(1.f, 1.f - b2p);   // 2-ulp division / square root:
+            // far inside the tolerance, and the IEEE forms are slow-path subroutines on the chain's critical path
             float g[7] = {gt[0], gt[1], gt[2], gw[0], gw[1], gw[2], gth}, dl[7];
 #pragma unroll
             for (int i = 0; i < 7; ++i) {
                 m[i] = P.adam_b1 * m[i] + (1.f - P.adam_b1) * g[i];
                 v[i] = P.adam_b2 * v[i] + (1.f - P.adam_b2) * g[i] * g[i];
-                dl[i] = -P.lr * (m[i] * c1) / (sqrtf(v[i] * c2) + P.adam_eps);
+                dl[i] = __fdividef(-P.lr * (m[i] * c1), sqrt_approx(v[i] * c2) + P.adam_eps);
             }
             pt[0] = fminf(fmaxf(pt[0] + dl[0], a.box_min[0]), a.box_max[0]);
             pt[1] = fminf(fmaxf(pt[1] + dl[1], a.box_min[1]), a.box_max[1]);

@@ -478,7 +478,8 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
             enew = ei + ea;
             if (!grad) break;
             b1p *= P.adam_b1; b2p *= P.adam_b2;
-            const float c1 = 1.f / (1.f - b1p), c2 = 1.f / (1.f - b2p);
+            const float c1 = __fdividef(1.f, 1.f - b1p), c2 = __fdividef(1.f, 1.f - b2p);   // 2-ulp division / square root:
+            // far inside the tolerance, and the IEEE forms are slow-path subroutines on the chain's critical path
             const bool keep = rf + 1 < P.n_refine;
             float g6[6];
             lane_backward(S, pt, X, WR, C, g6, [&](int g, float gk) {      // torsion gradients are consumed as produced
@@ -487,7 +488,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
                 mk = P.adam_b1 * mk + (1.f - P.adam_b1) * gk;
                 vk = P.adam_b2 * vk + (1.f - P.adam_b2) * gk * gk;
                 if (keep) { MV[2 * (g - 1) * C] = mk; MV[(2 * (g - 1) + 1) * C] = vk; }
-                float th = THP[(g - 1) * C] - P.lr * (mk * c1) / (sqrtf(vk * c2) + P.adam_eps);
+                float th = THP[(g - 1) * C] - __fdividef(P.lr * (mk * c1), sqrt_approx(vk * c2) + P.adam_eps);
                 if (th >= PI_F) th -= 2.f * PI_F;
                 if (th < -PI_F) th += 2.f * PI_F;
                 THP[(g - 1) * C] = th;
@@ -497,7 +498,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
             for (int i = 0; i < 6; ++i) {
                 m[i] = P.adam_b1 * m[i] + (1.f - P.adam_b1) * g6[i];
                 v[i] = P.adam_b2 * v[i] + (1.f - P.adam_b2) * g6[i] * g6[i];
-                dl[i] = -P.lr * (m[i] * c1) / (sqrtf(v[i] * c2) + P.adam_eps);
+                dl[i] = __fdividef(-P.lr * (m[i] * c1), sqrt_approx(v[i] * c2) + P.adam_eps);
             }
             pt[0] = fminf(fmaxf(pt[0] + dl[0], a.box_min[0]), a.box_max[0]);
             pt[1] = fminf(fmaxf(pt[1] + dl[1], a.box_min[1]), a.box_max[1]);
