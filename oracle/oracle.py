@@ -192,6 +192,21 @@ def score_grad(p, ty: Types, G: Grid, L: Ligand, pose, want_grad=True):
     return e, g, x, ga
 
 
+def score_grad_direct(p, ty: Types, rec_xyz, rec_type, L: Ligand, pose, want_grad=True):
+    """The same evaluation with the receptor term as the paper's direct sums over receptor atoms (no grid, no wall;
+    SURVEY 8(f) NEXT-3).  -> energy[3], grad[6+T], coords[n,3], gatom[n,3]."""
+    pose = np.ascontiguousarray(pose, dtype=np.float64)
+    xyz = np.ascontiguousarray(rec_xyz, dtype=np.float64)
+    typ = np.ascontiguousarray(rec_type, dtype=np.int32)
+    e = np.zeros(3)
+    g = np.zeros(6 + L.T)
+    x = np.zeros((L.n, 3))
+    ga = np.zeros((L.n, 3))
+    lib().orc_score_grad_direct(C.byref(p), C.byref(ty.c), _p(xyz), typ.ctypes.data_as(C.c_void_p), C.c_int(len(typ)),
+                                C.byref(L.c), _p(pose), _p(e), _p(g) if want_grad else None, _p(x), _p(ga))
+    return e, g, x, ga
+
+
 def score_grad_batch(p, ty: Types, G: Grid, L: Ligand, poses):
     poses = np.ascontiguousarray(poses, dtype=np.float64)
     n, stride = poses.shape

@@ -281,6 +281,37 @@ int orc_derive_pairs(int n, const unsigned char* frag, const unsigned char* bond
 }
 
 /* ------------------------------------------------------------------ O7 + O9: score and gradient */
+/* O9: pose gradient from the per-atom gradient g[n][3] by the direct sums (no tree accumulation), O(N*T). */
+static void pose_gradient(const orc_ligand* L, const double* pose, const double* x, const double* g, double* grad) {
+    int n = L->n;
+    for (int c = 0; c < 6 + L->T; ++c) grad[c] = 0.0;
+    for (int a = 0; a < n; ++a) {
+        double r[3] = {x[3 * a] - pose[0], x[3 * a + 1] - pose[1], x[3 * a + 2] - pose[2]};
+        const double* ga = g + 3 * a;
+        grad[0] += ga[0]; grad[1] += ga[1]; grad[2] += ga[2];
+        grad[3] += r[1] * ga[2] - r[2] * ga[1];
+        grad[4] += r[2] * ga[0] - r[0] * ga[2];
+        grad[5] += r[0] * ga[1] - r[1] * ga[0];
+    }
+    for (int k = 0; k < L->T; ++k) {
+        const double* xa = x + 3 * L->tor_a[k];
+        const double* xb = x + 3 * L->tor_b[k];
+        double u[3] = {xb[0] - xa[0], xb[1] - xa[1], xb[2] - xa[2]};
+        double un = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+        u[0] /= un; u[1] /= un; u[2] /= un;
+        double tq[3] = {0, 0, 0};
+        for (int a = 0; a < n; ++a) {
+            if (!in_subtree(L, L->frag[a], k)) continue;
+            double r[3] = {x[3 * a] - xb[0], x[3 * a + 1] - xb[1], x[3 * a + 2] - xb[2]};
+            const double* ga = g + 3 * a;
+            tq[0] += r[1] * ga[2] - r[2] * ga[1];
+            tq[1] += r[2] * ga[0] - r[0] * ga[2];
+            tq[2] += r[0] * ga[1] - r[1] * ga[0];
+        }
+        grad[6 + k] = u[0] * tq[0] + u[1] * tq[1] + u[2] * tq[2];
+    }
+}
+
 /*
  * E = sum_a [interp(a) + wall(a)] + E_intra.  energy[3] = {total, inter, intra}.
  * grad (may be NULL) = [dE/dt (3), dE/domega (3, world-frame rotation vector about t), dE/dtheta (T)]
@@ -313,34 +344,52 @@ void orc_score_grad(const orc_params* p, const orc_types* ty, const orc_grid* G,
             }
     }
     energy[0] = e_inter + e_intra; energy[1] = e_inter; energy[2] = e_intra;
-    if (grad) {
-        for (int c = 0; c < 6 + L->T; ++c) grad[c] = 0.0;
-        for (int a = 0; a < n; ++a) {
-            double r[3] = {x[3 * a] - pose[0], x[3 * a + 1] - pose[1], x[3 * a + 2] - pose[2]};
-            const double* ga = g + 3 * a;
-            grad[0] += ga[0]; grad[1] += ga[1]; grad[2] += ga[2];
-            grad[3] += r[1] * ga[2] - r[2] * ga[1];
-            grad[4] += r[2] * ga[0] - r[0] * ga[2];
-            grad[5] += r[0] * ga[1] - r[1] * ga[0];
-        }
-        for (int k = 0; k < L->T; ++k) {
-            const double* xa = x + 3 * L->tor_a[k];
-            const double* xb = x + 3 * L->tor_b[k];
-            double u[3] = {xb[0] - xa[0], xb[1] - xa[1], xb[2] - xa[2]};
-            double un = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
-            u[0] /= un; u[1] /= un; u[2] /= un;
-            double tq[3] = {0, 0, 0};
-            for (int a = 0; a < n; ++a) {
-                if (!in_subtree(L, L->frag[a], k)) continue;
-                double r[3] = {x[3 * a] - xb[0], x[3 * a + 1] - xb[1], x[3 * a + 2] - xb[2]};
-                const double* ga = g + 3 * a;
-                tq[0] += r[1] * ga[2] - r[2] * ga[1];
-                tq[1] += r[2] * ga[0] - r[0] * ga[2];
-                tq[2] += r[0] * ga[1] - r[1] * ga[0];
-            }
-            grad[6 + k] = u[0] * tq[0] + u[1] * tq[1] + u[2] * tq[2];
+    if (grad) pose_gradient(L, pose, x, g, grad);
+    if (coords) memcpy(coords, x, sizeof(double) * 3 * n);
+    if (gatom) memcpy(gatom, g, sizeof(double) * 3 * n);
+    free(x); free(g);
+}
+
+/*
+ * The same pose evaluation with the receptor term taken the paper's own way (P:103-125, P:353 item 4): direct sums over
+ * the receptor atoms, E_inter = sum_a sum_r e(s_r, t_a, |x_a - r_r|), no grid, no interpolation, no wall.
+ * NEXT-3: it is what the grid tabulates (O3), so the difference to orc_score_grad is the interpolation error.
+ */
+void orc_score_grad_direct(const orc_params* p, const orc_types* ty, const double* rec_xyz, const int* rec_type, int n_rec,
+                           const orc_ligand* L, const double* pose, double energy[3], double* grad, double* coords,
+                           double* gatom) {
+    int n = L->n;
+    double* x = (double*)malloc(sizeof(double) * 3 * n);
+    double* g = (double*)calloc(3 * n, sizeof(double));
+    orc_fk(L, pose, x);
+    double e_inter = 0.0, e_intra = 0.0;
+    for (int a = 0; a < n; ++a) {
+        int ta = L->type[a];
+        for (int r = 0; r < n_rec; ++r) {
+            double dv[3] = {x[3 * a] - rec_xyz[3 * r], x[3 * a + 1] - rec_xyz[3 * r + 1], x[3 * a + 2] - rec_xyz[3 * r + 2]};
+            double d = sqrt(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2]), e, de;
+            int s = rec_type[r];
+            orc_pair(p, ty->radius[s], ty->role[s], ty->radius[ta], ty->role[ta], d, &e, &de);
+            e_inter += e;
+            if (d > 0.0)
+                for (int c = 0; c < 3; ++c) g[3 * a + c] += de * dv[c] / d;
         }
     }
+    for (int k = 0; k < L->P; ++k) {
+        int a = L->pairs[2 * k], b = L->pairs[2 * k + 1];
+        double dv[3] = {x[3 * a] - x[3 * b], x[3 * a + 1] - x[3 * b + 1], x[3 * a + 2] - x[3 * b + 2]};
+        double d = sqrt(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2]), e, de;
+        int ta = L->type[a], tb = L->type[b];
+        orc_pair(p, ty->radius[ta], ty->role[ta], ty->radius[tb], ty->role[tb], d, &e, &de);
+        e_intra += e;
+        if (d > 0.0)
+            for (int c = 0; c < 3; ++c) {
+                g[3 * a + c] += de * dv[c] / d;
+                g[3 * b + c] -= de * dv[c] / d;
+            }
+    }
+    energy[0] = e_inter + e_intra; energy[1] = e_inter; energy[2] = e_intra;
+    if (grad) pose_gradient(L, pose, x, g, grad);
     if (coords) memcpy(coords, x, sizeof(double) * 3 * n);
     if (gatom) memcpy(gatom, g, sizeof(double) * 3 * n);
     free(x); free(g);

@@ -650,3 +650,51 @@ def test_topk_cluster_constructed_cases_and_invariants(orc, dock_system):
     for c in order[:last]:
         if c not in kept:
             assert any(rmsd(c, kk) < thr for kk in kept if order.index(kk) < order.index(c))
+
+
+# --------------------------------------------------------------------------- direct-pair receptor mode (S:8(f) NEXT-3)
+def test_direct_receptor_mode_pins(orc, dock_system):
+    S = dock_system
+    rec_, p, ty, G = S["rec"], S["p"], S["ty"], S["G"]
+    rng = np.random.default_rng(5)
+    # (1) a two-atom rigid "ligand" (atoms at -0.75 / +0.75 A on x = -2 / +2 grid steps) with both atoms exactly on grid
+    #     nodes: the interpolant is exact there (O4/O5), so the grid path and the direct path -- two different routes from
+    #     the paper's sums -- must agree to the grid's fp32 rounding (2 bonded atoms: no intra pair)
+    one = synth.ligands([2], [0], 8, seed=3)
+    assert np.array_equal(one.ref_xyz, np.array([[-0.75, 0, 0], [0.75, 0, 0]], np.float32))
+    L1 = orc.ligand_from_batch(one, 0)
+    for _ in range(12):
+        ijk = rng.integers(4, 36, 3)
+        pose = np.concatenate([rec_.origin + rec_.spacing * ijk, [1.0, 0, 0, 0]])
+        eg = orc.score_grad(p, ty, G, L1, pose, want_grad=False)[0]
+        ed, _, x1, _ = orc.score_grad_direct(p, ty, rec_.xyz, rec_.type, L1, pose, want_grad=False)
+        assert ed[2] == 0.0 and ed[1] == pytest.approx(eg[1], rel=3e-7, abs=1e-5)
+        brute = sum(orc.field_brute(p, ty, rec_.xyz, rec_.type, int(L1.type[a]), x1[a]) for a in range(2))
+        assert ed[1] == pytest.approx(brute, rel=1e-13)
+    # (2) same intra term as the grid path; analytic gradient vs central differences on all 6+T components
+    h = 1e-5
+    E = lambda L, pose: orc.score_grad_direct(p, ty, rec_.xyz, rec_.type, L, pose, want_grad=False)[0][0]
+    for L in S["L"]:
+        for _ in range(2):
+            pose = _safe_pose(orc, S, L, rng)
+            x = orc.fk(L, pose)
+            dmin = np.min(np.linalg.norm(x[:, None, :] - rec_.xyz[None, :, :], axis=2))
+            e, g, _, ga = orc.score_grad_direct(p, ty, rec_.xyz, rec_.type, L, pose)
+            assert e[2] == orc.score_grad(p, ty, G, L, pose, want_grad=False)[0][2]
+            assert g[:3] == pytest.approx(ga.sum(axis=0), rel=1e-12, abs=1e-12)
+            scale = max(1.0, np.abs(g).max())
+            tol = 2e-5 * scale if dmin > 0.06 else None
+            if tol is None:
+                continue
+            for c in range(3):
+                d = np.zeros_like(pose); d[c] = h
+                assert g[c] == pytest.approx((E(L, pose + d) - E(L, pose - d)) / (2 * h), abs=tol)
+            for c in range(3):
+                v = np.zeros(3); v[c] = h
+                pp, pm = pose.copy(), pose.copy()
+                pp[3:7] = _quat_left_mul_rotvec(pose[3:7], v)
+                pm[3:7] = _quat_left_mul_rotvec(pose[3:7], -v)
+                assert g[3 + c] == pytest.approx((E(L, pp) - E(L, pm)) / (2 * h), abs=tol)
+            for k in range(L.T):
+                d = np.zeros_like(pose); d[7 + k] = h
+                assert g[6 + k] == pytest.approx((E(L, pose + d) - E(L, pose - d)) / (2 * h), abs=tol)
