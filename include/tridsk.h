@@ -167,6 +167,18 @@ int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_lig
                       const tridsk_params* params, const int* lig_index, const float* poses, int n_pose,
                       int pose_stride, float* energy, float* grad, int grad_stride, float* coords, int coord_stride);
 
+/*
+ * The same evaluation with the receptor term taken the paper's own way (P:103-125, P:353 item 4):
+ * direct sums over the receptor atoms, E_inter = sum_a sum_r e(s_r, t_a, |x_a - r_r|) -- no grid, no interpolation, no
+ * wall.  It is what the grid tabulates (O3): the difference to tridsk_score_grad is the interpolation error of the hot
+ * path's receptor term.  A measuring tool (O(n_atoms * n_rec) per pose), not part of tridsk_dock.
+ * rec_xyz[n_rec][3], rec_type[n_rec], lig_index, poses, energy[n_pose][3], grad (or NULL): [host|dev] as in
+ * tridsk_score_grad.  Needs a ligand batch of at most 1024 ligands.
+ */
+int tridsk_score_direct(tridsk_ctx* ctx, const float* rec_xyz, const int* rec_type, int n_rec, const tridsk_types* types,
+                        const tridsk_params* params, const tridsk_ligands* ligs, const int* lig_index, const float* poses,
+                        int n_pose, int pose_stride, float* energy, float* grad, int grad_stride);
+
 /* ---- the docking run (steps a1..a10; O10..O13) ---------------------------------------------------- */
 /*
  * For every ligand: n_chains independent chains x n_steps MC steps (perturb one entity -> n_refine

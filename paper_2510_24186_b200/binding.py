@@ -273,6 +273,24 @@ class Engine:
         self._sync_out()
         return energy, grad, coords
 
+    def score_direct(self, rec_xyz, rec_type, radius, role, ligs: Ligands, params, lig_index, poses, want_grad=True):
+        """tridsk_score_direct: receptor term as direct sums over the receptor atoms (no grid).  Host (numpy) buffers.
+        -> energy[n,3], grad[n,6+Tmax]."""
+        ty, keep = self._types(radius, role)
+        rec_xyz = np.ascontiguousarray(rec_xyz, np.float32)
+        rec_type = np.ascontiguousarray(rec_type, np.int32)
+        poses = np.ascontiguousarray(poses, np.float32)
+        lig_index = np.ascontiguousarray(lig_index, np.int32)
+        n, stride, gs = int(poses.shape[0]), int(poses.shape[1]), 6 + ligs.max_tor
+        energy = np.empty((n, 3), np.float32)
+        grad = np.empty((n, gs), np.float32) if want_grad else None
+        self._sync_in()
+        self._ck(lib().tridsk_score_direct(self.ctx, _ptr(rec_xyz), _ptr(rec_type), C.c_int(int(rec_xyz.shape[0])), C.byref(ty),
+                                           C.byref(params), ligs.handle, _ptr(lig_index), _ptr(poses), C.c_int(n), C.c_int(stride),
+                                           _ptr(energy), _ptr(grad), C.c_int(gs)))
+        self._sync_out()
+        return energy, grad
+
     # ------------------------------------------------------------------ dock
     def dock(self, grid: Grid, ligs: Ligands, params, box_min, box_max, pocket_center, pocket_radius,
              n_chains, n_steps, top_k, seed=0, pose_stride=None, device_out=False, init_poses=None,

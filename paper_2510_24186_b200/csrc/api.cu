@@ -739,6 +739,65 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
     return TRIDSK_OK;
 }
 
+// ---------------------------------------------------------------------------------------- score, direct receptor sums
+extern "C" int tridsk_score_direct(tridsk_ctx* ctx, const float* rec_xyz, const int* rec_type, int n_rec, const tridsk_types* types,
+                                   const tridsk_params* params, const tridsk_ligands* ligs, const int* lig_index, const float* poses,
+                                   int n_pose, int pose_stride, float* energy, float* grad, int grad_stride) {
+    if (!ctx || !rec_xyz || !rec_type || n_rec < 0 || !params || !ligs || !lig_index || !poses || !energy || n_pose < 0)
+        return fail(ctx, TRIDSK_EINVAL, "null argument");
+    int rc = check_types(ctx, types);
+    if (rc) return rc;
+    if (!ligs->has_cta) return fail(ctx, TRIDSK_EINVAL, "tridsk_score_direct needs a ligand batch of at most 1024 ligands");
+    if (pose_stride < 7 + ligs->max_tor) return fail(ctx, TRIDSK_EINVAL, "pose_stride < 7 + max torsions");
+    if (grad && grad_stride < 6 + ligs->max_tor) return fail(ctx, TRIDSK_EINVAL, "grad_stride < 6 + max torsions");
+    if (n_pose == 0) return TRIDSK_OK;
+    const int nt = types->n_types;
+    std::vector<int> li(n_pose);
+    CK(cudaMemcpyAsync(li.data(), lig_index, sizeof(int) * n_pose, cudaMemcpyDefault, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < n_pose; ++i)
+        if (li[i] < 0 || li[i] >= ligs->n_lig) return fail(ctx, TRIDSK_EINVAL, "lig_index out of range");
+    // scratch 0: [bad flag (16 B) | float4 rec[n_rec]]; 1: [radius | role]; 4: staged host receptor; 7: inputs; 6: outputs
+    char *d_rec0, *d_ty, *stage = nullptr, *in = nullptr, *ob = nullptr;
+    if ((rc = scratch(ctx, 0, 16 + sizeof(float4) * std::max(n_rec, 1), (void**)&d_rec0)) ||
+        (rc = scratch(ctx, 1, sizeof(float) * nt + nt + 64, (void**)&d_ty))) return rc;
+    const size_t b_xyz = (sizeof(float) * 3 * (size_t)n_rec + 15) / 16 * 16;
+    const bool h_xyz = n_rec && !is_device_ptr(rec_xyz), h_typ = n_rec && !is_device_ptr(rec_type);
+    if ((h_xyz || h_typ) && (rc = scratch(ctx, 4, b_xyz + sizeof(int) * n_rec, (void**)&stage))) return rc;
+    const size_t b_li = sizeof(int) * n_pose, b_po = sizeof(float) * (size_t)n_pose * pose_stride, o_po = (b_li + 15) / 16 * 16;
+    const bool h_li = !is_device_ptr(lig_index), h_po = !is_device_ptr(poses);
+    if ((h_li || h_po) && (rc = scratch(ctx, 7, o_po + b_po + 64, (void**)&in))) return rc;
+    const size_t b_e = sizeof(float) * 3 * n_pose, b_g = grad ? sizeof(float) * (size_t)n_pose * grad_stride : 0, o_g = (b_e + 15) / 16 * 16;
+    const bool h_e = !is_device_ptr(energy), h_g = grad && !is_device_ptr(grad);
+    if ((h_e || h_g) && (rc = scratch(ctx, 6, o_g + b_g + 64, (void**)&ob))) return rc;
+    int* d_bad = (int*)d_rec0;
+    float4* d_rec = (float4*)(d_rec0 + 16);
+    CK(cudaMemsetAsync(d_bad, 0, sizeof(int), ctx->stream));
+    if (h_xyz) CK(cudaMemcpyAsync(stage, rec_xyz, sizeof(float) * 3 * n_rec, cudaMemcpyHostToDevice, ctx->stream));
+    if (h_typ) CK(cudaMemcpyAsync(stage + b_xyz, rec_type, sizeof(int) * n_rec, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(d_ty, types->radius, sizeof(float) * nt, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(d_ty + sizeof(float) * nt, types->hb_role, nt, cudaMemcpyHostToDevice, ctx->stream));
+    CK(launch_rec_pack(ctx->stream, h_xyz ? (const float*)stage : rec_xyz, h_typ ? (const int*)(stage + b_xyz) : rec_type, n_rec, nt, d_rec, d_bad));
+    if (h_li) CK(cudaMemcpyAsync(in, li.data(), b_li, cudaMemcpyHostToDevice, ctx->stream));
+    if (h_po) CK(cudaMemcpyAsync(in + o_po, poses, b_po, cudaMemcpyHostToDevice, ctx->stream));
+    DParams P;
+    to_dparams(params, &P);
+    float* d_e = h_e ? (float*)ob : energy;
+    float* d_g = grad ? (h_g ? (float*)(ob + o_g) : grad) : nullptr;
+    CK(launch_score_direct(ctx->stream, ligs->hdr, ligs->atom_f4, ligs->atom_i, ligs->lane_frags, ligs->cta_rows, ligs->cta_recs, d_rec,
+                           n_rec, (const float*)d_ty, (const unsigned char*)(d_ty + sizeof(float) * nt), P,
+                           h_li ? (const int*)in : lig_index, h_po ? (const float*)(in + o_po) : poses, n_pose, pose_stride, d_e, d_g,
+                           grad_stride, ligs->max_atoms));
+    ctx->launches += 1 + (n_rec > 0 ? 1 : 0);
+    int bad = 0;
+    CK(cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    if (h_e) CK(cudaMemcpyAsync(energy, d_e, b_e, cudaMemcpyDeviceToHost, ctx->stream));
+    if (h_g) CK(cudaMemcpyAsync(grad, d_g, b_g, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));                  // li, bad and the type table are host staging
+    if (bad) return fail(ctx, TRIDSK_EINVAL, "receptor atom type out of range");
+    return TRIDSK_OK;
+}
+
 // ---------------------------------------------------------------------------------------- dock
 // Lane-per-chain launch plan.  A CTA holds C chains of one ligand (C = n_chains rounded up to a warp, at most 128, fewer
 // if a big ligand would not fit) and needs topology + C * chain_slots * 4 bytes of shared memory.  Ligands are grouped

@@ -299,5 +299,9 @@ cudaError_t launch_score(cudaStream_t s, const ScoreLaunch& a);
 cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int threads, size_t smem_bytes);
 cudaError_t launch_score_cta(cudaStream_t s, const ScoreLaunch& a, size_t smem_bytes);
 cudaError_t launch_topk(cudaStream_t s, const TopkLaunch& a);
+cudaError_t launch_score_direct(cudaStream_t s, const LigHdr* hdr, const float4* atom_f4, const int* atom_i, const LaneFrag* lane_frags,
+                                const int* cta_rows, const uint2* cta_recs, const float4* rec, int n_rec, const float* radius,
+                                const unsigned char* role, const DParams& P, const int* lig_index, const float* poses, int n_pose,
+                                int pose_stride, float* energy, float* grad, int grad_stride, int max_atoms);
 size_t topk_cluster_smem(int top_k, int max_atoms, int max_tor);
 cudaError_t launch_philox_debug(cudaStream_t s, const unsigned int* ctr_key /* dev[6] */, unsigned int* out /* dev[4] */);

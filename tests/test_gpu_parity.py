@@ -548,3 +548,46 @@ def test_duplicate_removing_topk_matches_oracle(orc, gp, system):
         assert np.array_equal(r0["chain"], r1["chain"])
     finally:
         e.close()
+
+
+def test_score_direct_matches_oracle_and_bounds_the_interpolation_error(orc, gp, system):
+    """tridsk_score_direct (S:8(f) NEXT-3): receptor term as the paper's direct sums, per pose energy and gradient vs the
+    oracle's direct evaluation at rel 1e-4 / abs 1e-3 -- and, on the same poses, how far the hot path's trilinear grid
+    energy is from it (the interpolation error of G7; printed, loosely bounded)."""
+    from paper_2510_24186_b200 import Engine
+    rec, batch, L, ty, p = system["rec"], system["batch"], system["L"], system["ty"], system["p"]
+    radius, role = system["radius"], system["role"]
+    e = Engine(0)
+    try:
+        ligs = e.load_ligands(batch, radius, role)
+        grid = e.grid_from_values(system["G"].g, rec.origin, rec.spacing)
+        li = np.repeat(np.arange(batch.n_lig, dtype=np.int32), 3)
+        poses = synth.random_poses(batch, li, rec, seed=9, spread=0.6)
+        # relax the poses a little so that they are not all deep clashes: 20 MC steps from them, one chain each
+        ed, gd = e.score_direct(rec.xyz, rec.type, radius, role, ligs, gp, li, poses)
+        eg, _, _ = e.score_grad(grid, ligs, gp, li, poses, want_coords=False)
+        worst_e = worst_g = 0.0
+        for i in range(len(li)):
+            Li = L[int(li[i])]
+            eo, go, _, _ = orc.score_grad_direct(p, ty, rec.xyz, rec.type, Li, poses[i, :7 + Li.T].astype(np.float64))
+            worst_e = max(worst_e, worst(ed[i], eo))
+            worst_g = max(worst_g, worst(gd[i, :6 + Li.T], go, scale=np.abs(go).max()))
+        assert worst_e <= 1.0 and worst_g <= 1.0, (worst_e, worst_g)
+        # interpolation error of the grid path (receptor term only), relative to the spread of the energies
+        inside = np.abs(eg[:, 1] - ed[:, 1])
+        print("grid vs direct receptor energy: median |dE| %.3g, max %.3g, median |E| %.3g" %
+              (np.median(inside), inside.max(), np.median(np.abs(ed[:, 1]))))
+        assert np.median(inside) < 0.05 * np.median(np.abs(ed[:, 1])) + 0.5
+        # the same on docked poses (what the search actually returns): best pose of 64 chains x 150 steps per ligand
+        r = e.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, 64, 150, 1, seed=1)
+        lj = np.arange(batch.n_lig, dtype=np.int32)
+        pj = np.ascontiguousarray(r["pose"][:, 0, :])
+        edj, _ = e.score_direct(rec.xyz, rec.type, radius, role, ligs, gp, lj, pj, want_grad=False)
+        egj, _, _ = e.score_grad(grid, ligs, gp, lj, pj, want_grad=False, want_coords=False)
+        dj = np.abs(egj[:, 1] - edj[:, 1])
+        print("docked poses: receptor energy median %.4g, grid - direct: median |dE| %.3g, max %.3g (relative median %.2g)" %
+              (np.median(edj[:, 1]), np.median(dj), dj.max(), np.median(dj / np.abs(edj[:, 1]))))
+        assert np.array_equal(egj[:, 2], edj[:, 2]) or np.allclose(egj[:, 2], edj[:, 2], rtol=1e-5, atol=1e-4)   # same intra term
+        assert np.median(dj / np.abs(edj[:, 1])) < 0.02
+    finally:
+        e.close()
