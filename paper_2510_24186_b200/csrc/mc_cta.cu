@@ -2,11 +2,11 @@
 //
 // A single dock has a few hundred chains, each a serial string of thousands of pose evaluations: the time of a dock is
 // (evaluations per chain) x (latency of one evaluation), and a warp per chain (mc_kernel.cu) leaves that latency at
-// ~2,100 dependent warp instructions.  Here a chain gets 4 or 8 warps:
+// ~2,100 dependent warp instructions.  Here a chain gets 4 warps:
 //   * every WARP keeps the whole pose and all fragment frames in registers (lane g = fragment g in pre-order) and
 //     repeats the scalar work -- Philox, forward kinematics of the frames, the reverse pass, Adam, Metropolis -- so the
 //     warps never have to exchange pose state and take identical decisions by construction;
-//   * the atoms are spread over the CTA, `lpa` lanes per atom: the gradient evaluation walks the pair set in ROW form
+//   * the atoms are spread over the CTA, `lpa` (8, 4, 2 or 1) lanes per atom: the gradient evaluation walks the pair set in ROW form
 //     (every atom meets all its partners, each pair is visited from both ends), so an atom's force is accumulated by
 //     its own lanes -- no scatter, no atomics, bit-reproducible; the energy-only evaluation walks the flat pair list;
 //   * the receptor term of an atom is two 16-byte gathers whose L2 latency hides behind the pair loop;
@@ -360,7 +360,7 @@ __device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const Ct
 }
 
 // ------------------------------------------------------------------ the fused MC kernel, one CTA per chain
-__global__ void __launch_bounds__(256, 2) mc_cta_kernel(const McLaunch a) {
+__global__ void __launch_bounds__(128, 4) mc_cta_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lig = a.lig_list[blockIdx.x / a.n_chains];
