@@ -591,3 +591,45 @@ def test_score_direct_matches_oracle_and_bounds_the_interpolation_error(orc, gp,
         assert np.median(dj / np.abs(edj[:, 1])) < 0.02
     finally:
         e.close()
+
+
+def test_error_paths_of_the_optional_modes(gp, system):
+    """Argument checks of the round-1 additions: limits of the duplicate-removing top-k, of the CTA / direct modes on
+    large batches, bad receptor types in tridsk_score_direct, bad mapping ids."""
+    from paper_2510_24186_b200 import Engine, TridskError
+    rec, batch, radius, role = system["rec"], system["batch"], system["radius"], system["role"]
+    e = Engine(0)
+    try:
+        grid = e.grid_from_values(system["G"].g, rec.origin, rec.spacing)
+        ligs = e.load_ligands(batch, radius, role)
+        dock = lambda **kw: e.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, 64, 2, **kw)
+        with pytest.raises(TridskError) as ei:                                        # 60 x 80 atoms > 4096
+            dock(top_k=60, cluster_rmsd=1.0)
+        assert ei.value.code == -4
+        with pytest.raises(TridskError) as ei:
+            dock(top_k=2, cluster_rmsd=-1.0)
+        assert ei.value.code == -1
+        with pytest.raises(TridskError):
+            e.set_kernel(5)
+        li = np.zeros(2, np.int32)
+        poses = synth.random_poses(batch, li, rec, seed=1)
+        bad_type = rec.type.copy(); bad_type[5] = 99
+        with pytest.raises(TridskError) as ei:
+            e.score_direct(rec.xyz, bad_type, radius, role, ligs, gp, li, poses)
+        assert ei.value.code == -1
+        with pytest.raises(TridskError):
+            e.score_direct(rec.xyz, rec.type, radius, role, ligs, gp, np.array([0, 999], np.int32), poses)
+        # a batch above 1024 ligands carries no CTA-per-chain format: mapping 3 and the direct mode refuse it
+        many = synth.ligands([12] * 1025, [1] * 1025, 16, seed=8)
+        lm = e.load_ligands(many, radius, role)
+        e.set_kernel(3)
+        with pytest.raises(TridskError) as ei:
+            e.dock(grid, lm, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, 32, 2, 1)
+        assert ei.value.code == -1
+        e.set_kernel(0)
+        with pytest.raises(TridskError):
+            e.score_direct(rec.xyz, rec.type, radius, role, lm, gp, li, poses[:, :8])
+        r = e.dock(grid, lm, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, 32, 2, 1)   # automatic mapping still works
+        assert e.last_kernel() == 2 and np.all(np.isfinite(r["energy"]))
+    finally:
+        e.close()
