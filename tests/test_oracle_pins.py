@@ -698,3 +698,77 @@ def test_direct_receptor_mode_pins(orc, dock_system):
             for k in range(L.T):
                 d = np.zeros_like(pose); d[7 + k] = h
                 assert g[6 + k] == pytest.approx((E(L, pose + d) - E(L, pose - d)) / (2 * h), abs=tol)
+
+
+# --------------------------------------------------------------------------- E_MDN (Eq.E_MDN; S:8(f) NEXT-1 groundwork)
+def test_mdn_energy_pins():
+    from scipy.stats import norm
+    from oracle import mdn
+    rng = np.random.default_rng(3)
+    one = lambda v: np.array([[[v]]], dtype=np.float64)
+    # (1) one residue of one atom, one ligand atom, K = 1: E = -N(d; mu, sigma) (closed form + scipy's density)
+    rec = np.zeros((1, 3)); off = np.array([0, 1])
+    for d, m, s in [(3.0, 3.0, 0.5), (4.2, 3.5, 0.8), (2.0, 4.0, 1.1)]:
+        E, g, dm = mdn.mdn_energy(rec, off, one(1.0), one(m), one(s), np.array([[d, 0.0, 0.0]]))
+        assert dm[0, 0] == pytest.approx(d) and E == pytest.approx(-norm.pdf(d, loc=m, scale=s), rel=1e-13)
+        # dE/dd = N(d) (d - mu) / sigma^2, along +x (the atom sits on the x axis, the receptor atom at the origin)
+        assert g[0] == pytest.approx([norm.pdf(d, m, s) * (d - m) / s ** 2, 0, 0], rel=1e-12, abs=1e-15)
+    E, _, _ = mdn.mdn_energy(rec, off, one(1.0), one(3.0), one(0.5), np.array([[3.0, 0, 0]]))
+    assert E == pytest.approx(-1.0 / (0.5 * np.sqrt(2 * np.pi)), rel=1e-14)          # at d = mu: -1 / (sigma sqrt(2 pi))
+    # (2) the cut-off: d_cut = 5 A, strict
+    assert mdn.mdn_energy(rec, off, one(1.0), one(5.0), one(1.0), np.array([[5.0, 0, 0]]))[0] == 0.0
+    assert mdn.mdn_energy(rec, off, one(1.0), one(5.0), one(1.0), np.array([[4.999, 0, 0]]))[0] < -0.39
+    # (3) mixture weights: two equal components = the mean of the two single-component energies
+    two = lambda a, b: np.array([[[a, b]]], dtype=np.float64)
+    x = np.array([[3.3, 0, 0]])
+    E2 = mdn.mdn_energy(rec, off, two(0.5, 0.5), two(3.0, 4.0), two(0.5, 0.9), x)[0]
+    assert E2 == pytest.approx(0.5 * (-norm.pdf(3.3, 3.0, 0.5)) + 0.5 * (-norm.pdf(3.3, 4.0, 0.9)), rel=1e-13)
+    # (4) d_ij is the MINIMUM over the residue's atoms: the nearer atom decides, the farther is irrelevant
+    rec2 = np.array([[0.0, 0, 0], [0.0, 2.0, 0]]); off2 = np.array([0, 2])
+    xa = np.array([[3.0, 0.0, 0.0]])
+    Ea, ga, dma = mdn.mdn_energy(rec2, off2, one(1.0), one(3.2), one(0.6), xa)
+    assert dma[0, 0] == pytest.approx(3.0) and Ea == pytest.approx(-norm.pdf(3.0, 3.2, 0.6), rel=1e-13)
+    assert ga[0, 1] == 0.0                                                            # the gradient points along x: arg-min atom is atom 0
+    # two residues add up (sum over i), two ligand atoms add up (sum over j)
+    rec3 = np.array([[0.0, 0, 0], [10.0, 0, 0]]); off3 = np.array([0, 1, 2])
+    x2 = np.array([[3.0, 0, 0], [7.5, 0, 0]])
+    pi3 = np.ones((2, 2, 1)); mu3 = np.full((2, 2, 1), 3.0); s3 = np.full((2, 2, 1), 0.7)
+    E3 = mdn.mdn_energy(rec3, off3, pi3, mu3, s3, x2)[0]
+    # residue 0 sees atom 0 at 3.0 (atom 1 at 7.5: cut); residue 1 sees atom 1 at 2.5 (atom 0 at 7: cut)
+    assert E3 == pytest.approx(-norm.pdf(3.0, 3.0, 0.7) - norm.pdf(2.5, 3.0, 0.7), rel=1e-13)
+    # (5) analytic gradient vs central differences on a random system, away from arg-min switches and the cut-off
+    rec_ = synth.receptor(120, 15.0, 8, seed=31, grid_n=41, pocket_radius=4.0)
+    order, res_off = synth.residues(rec_, 8)
+    rxyz = rec_.xyz[order].astype(np.float64)
+    assert sorted(order) == list(range(120)) and res_off[-1] == 120 and np.all(np.diff(res_off) > 0)
+    n, K = 6, 4
+    pi, mu, sg = synth.gmm_params(len(res_off) - 1, n, K, seed=5)
+    assert np.allclose(pi.sum(axis=2), 1.0, atol=1e-6)
+    h, checked = 1e-6, 0
+    for _ in range(40):
+        x = rec_.pocket_center + rng.uniform(-5.0, 5.0, (n, 3))
+        E, g, dm = mdn.mdn_energy(rxyz, res_off, pi, mu, sg, x)
+        if np.min(np.abs(dm - 5.0)) < 1e-3:
+            continue
+        # skip configurations where two atoms of a residue are almost equally near (the arg-min could switch under +-h)
+        near_tie = False
+        for i in range(len(res_off) - 1):
+            for j in range(n):
+                dd = np.sort(np.linalg.norm(x[j] - rxyz[res_off[i]:res_off[i + 1]], axis=1))
+                near_tie |= len(dd) > 1 and dd[1] - dd[0] < 1e-3 and dd[0] < 5.0
+        if near_tie or E == 0.0:
+            continue
+        for j in range(n):
+            for c in range(3):
+                xp, xm = x.copy(), x.copy()
+                xp[j, c] += h; xm[j, c] -= h
+                fd = (mdn.mdn_energy(rxyz, res_off, pi, mu, sg, xp)[0] - mdn.mdn_energy(rxyz, res_off, pi, mu, sg, xm)[0]) / (2 * h)
+                assert g[j, c] == pytest.approx(fd, rel=2e-6, abs=2e-8)
+        checked += 1
+        if checked == 3:
+            break
+    assert checked == 3
+    # (6) invariance: a common rigid translation of receptor and ligand changes nothing
+    t = np.array([1.3, -2.2, 0.7])
+    E0 = mdn.mdn_energy(rxyz, res_off, pi, mu, sg, x)[0]
+    assert mdn.mdn_energy(rxyz + t, res_off, pi, mu, sg, x + t)[0] == pytest.approx(E0, rel=1e-12)

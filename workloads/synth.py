@@ -298,3 +298,29 @@ def random_poses(batch: LigandBatch, lig_index, rec: Receptor, seed: int, spread
     for i, li in enumerate(lig_index):
         poses[i, 7 + batch.n_tor(li):] = 0.0
     return poses
+
+
+# --------------------------------------------------------------------------- inputs of E_MDN
+def residues(rec: "Receptor", size: int = 8):
+    """Group the receptor atoms into spatially compact pseudo-residues of `size` atoms (the paper's residues come from
+    the protein's sequence, which a synthetic point cloud does not have): atoms are ordered by the Morton code of their
+    5 A cell and cut into consecutive groups.  -> (order [n_rec] permutation of the atoms, res_off [n_res+1])."""
+    cell = np.floor((rec.xyz - rec.xyz.min(axis=0)) / 5.0).astype(np.int64)
+    code = np.zeros(len(cell), np.int64)
+    for b in range(6):
+        for c in range(3):
+            code |= ((cell[:, c] >> b) & 1) << (3 * b + c)
+    order = np.lexsort((np.arange(len(code)), code))
+    n_res = (len(order) + size - 1) // size
+    res_off = np.minimum(np.arange(n_res + 1) * size, len(order)).astype(np.int32)
+    return order, res_off
+
+
+def gmm_params(n_res: int, n_atoms: int, K: int, seed: int):
+    """Synthetic mixture parameters standing in for the graph transformer's output (trained weights are not
+    here): pi ~ Dirichlet(1) over K, mu ~ U(2.5, 6.0) A, sigma ~ U(0.3, 1.2) A.  -> pi, mu, sigma float32 [n_res][n_atoms][K]."""
+    rng = np.random.default_rng(seed)
+    pi = rng.dirichlet(np.ones(K), size=(n_res, n_atoms)).astype(np.float32)
+    mu = rng.uniform(2.5, 6.0, size=(n_res, n_atoms, K)).astype(np.float32)
+    sigma = rng.uniform(0.3, 1.2, size=(n_res, n_atoms, K)).astype(np.float32)
+    return pi, mu, sigma
