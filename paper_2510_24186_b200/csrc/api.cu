@@ -858,7 +858,11 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
         }
         lg->lane_plan.back().count++;
         lg->lane_plan.back().smem = std::max(lg->lane_plan.back().smem, ent[i].need);
+        lg->lane_plan.back().work += ent[i].cost;
     }
+    // the buckets run as concurrent graph branches: start the one with the most work first
+    std::stable_sort(lg->lane_plan.begin(), lg->lane_plan.end(),
+                     [](const tridsk_ligands::LaneBucket& x, const tridsk_ligands::LaneBucket& y) { return x.work > y.work; });
     if (getenv("TRIDSK_DEBUG"))
         for (const auto& b : lg->lane_plan)
             fprintf(stderr, "tridsk lane plan: %d ligands, %s, %d chains per %s, %zu bytes of shared memory\n", b.count,

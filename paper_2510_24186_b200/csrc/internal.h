@@ -14,7 +14,7 @@
 #define TRIDSK_MAX_J 4           // atoms per lane (n_atoms <= 32 * MAX_J)
 #define TRIDSK_MAX_TILES 10      // J(J+1)/2 tiles of the pair schedule
 #define TRIDSK_CTA_MAX_LIG 1024  // batches up to this size also carry the CTA-per-chain pair format
-#define TRIDSK_BRANCHES 8        // parallel branches of a dock's launch series (ctx stream + side streams)
+#define TRIDSK_BRANCHES 16       // parallel branches of a dock's launch series (ctx stream + side streams)
 
 // ---------------------------------------------------------------- device-side packed formats
 // Scoring / sampling constants in the form the kernels use (fp32).
@@ -278,7 +278,7 @@ struct tridsk_ligands {
     int* cta_bucket_dev[2] = {nullptr, nullptr};
     size_t cta_smem[2] = {0, 0};                 // largest shared-memory need per bucket
     int* all_ids = nullptr;       // 0..n_lig-1 re-ordered per lane bucket (refilled when the plan key changes)
-    struct LaneBucket { int chains_per_cta; size_t smem; int first, count; int tm_cols; };   // tm_cols > 0: tensor-memory form, smem = bytes per warp
+    struct LaneBucket { int chains_per_cta; size_t smem; int first, count; int tm_cols; long long work = 0; };   // tm_cols > 0: tensor-memory form, smem = bytes per warp
     std::vector<LaneBucket> lane_plan;
     std::vector<int> lane_ids_h;  // host copy behind all_ids (must outlive the async upload)
     long long lane_plan_key = -1; // n_chains << 8 | (n_refine > 1)
