@@ -55,12 +55,17 @@ _lib = None
 
 
 def lib():
-    """Load libtridsk.so; fails loudly if it has not been built (python -m paper_2510_24186_b200.build)."""
+    """Load libtridsk.so, (re)building it with nvcc first if it is missing or older than its sources (content-hash
+    stamp); fails loudly if that is impossible -- there is no CPU fallback."""
     global _lib
     if _lib is None:
-        if not os.path.exists(LIB_PATH):
-            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2510_24186_b200.build` "
-                              "(there is no CPU fallback)")
+        try:
+            from . import build as _build
+            _build.build()
+        except Exception as exc:                              # no nvcc, compile error, ...
+            if not os.path.exists(LIB_PATH):
+                raise ImportError(f"{LIB_PATH} is missing and could not be built ({exc}); build it with "
+                                  "`python -m paper_2510_24186_b200.build` (there is no CPU fallback)") from exc
         _lib = C.CDLL(LIB_PATH)
         _lib.tridsk_last_error.restype = C.c_char_p
         _lib.tridsk_launch_count.restype = C.c_longlong

@@ -271,6 +271,7 @@ struct PackedLig {
     std::vector<LaneFrag> lane_frags;   // lane format (internal.h): fragments in pre-order
     std::vector<uint4> lane_stream;     // lane format: the pair instruction stream (header units)
     std::vector<LaneRec> lane_recs;     // lane format: the pair records, in stream order
+    long long w_hist[5] = {0, 0, 0, 0, 0};
     std::vector<int> cta_rows;          // CTA format (internal.h): n + 1 row offsets
     std::vector<uint2> cta_recs;        // CTA format: 2 P row records, then P flat records
     int err = 0;
@@ -468,6 +469,7 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
                             }
                         }
                         if (!any) continue;
+                        out.w_hist[w]++;
                         out.lane_recs.push_back(rec);
                         ++nb;
                     }
@@ -602,6 +604,9 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
         for (int i = 0; i < L; ++i) np += pk[i].h.n_pairs;
         fprintf(stderr, "tridsk load_ligands: %d ligands, %lld pairs in %zu 4-slot records (slot utilisation %.1f %%)\n", L, np, nrec,
                 nrec ? 25.0 * (double)np / (double)nrec : 0.0);
+        long long wh[5] = {0, 0, 0, 0, 0};
+        for (int i = 0; i < L; ++i) for (int w = 1; w <= 4; ++w) wh[w] += pk[i].w_hist[w];
+        fprintf(stderr, "tridsk load_ligands: records by tile width 1..4: %lld %lld %lld %lld\n", wh[1], wh[2], wh[3], wh[4]);
     }
     cudaError_t e = cudaSuccess;
     auto up = [&](void** d, const void* src, size_t bytes) {
