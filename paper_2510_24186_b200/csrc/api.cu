@@ -198,7 +198,7 @@ extern "C" int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const in
     char* d_rec0; void* d_tab;
     const void *d_xyz = nullptr, *d_typ = nullptr;
     if ((rc = scratch(ctx, 0, 16 + sizeof(float4) * std::max(n_rec, 1), (void**)&d_rec0)) ||
-        (rc = scratch(ctx, 1, sizeof(float) * tab.size(), &d_tab))) { tridsk_free_grid(g); return rc; }
+        (rc = scratch(ctx, 1, sizeof(float) * (tab.size() + nt), &d_tab))) { tridsk_free_grid(g); return rc; }
     const size_t b_xyz = (sizeof(float) * 3 * (size_t)n_rec + 15) / 16 * 16;
     const bool h_xyz = n_rec && !is_device_ptr(rec_xyz), h_typ = n_rec && !is_device_ptr(rec_type);
     char* stage = nullptr;
@@ -213,8 +213,10 @@ extern "C" int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const in
     d_xyz = h_xyz ? (const void*)stage : (const void*)rec_xyz;
     d_typ = h_typ ? (const void*)(stage + b_xyz) : (const void*)rec_type;
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_tab, tab.data(), sizeof(float) * tab.size(), cudaMemcpyHostToDevice, ctx->stream);
+    float* d_rad = (float*)d_tab + tab.size();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_rad, types->radius, sizeof(float) * nt, cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = launch_rec_pack(ctx->stream, (const float*)d_xyz, (const int*)d_typ, n_rec, nt, d_rec, d_bad);
-    if (e == cudaSuccess) e = launch_grid_build(ctx->stream, d_rec, n_rec, (const float*)d_tab, nt, P, g->d, dc_max, g->g);
+    if (e == cudaSuccess) e = launch_grid_build(ctx->stream, d_rec, n_rec, (const float*)d_tab, nt, P, g->d, dc_max, types->radius, d_rad, g->g);
     if (e == cudaSuccess) e = launch_grid_pack(ctx->stream, g->d, g->gp);
     int bad = 0;
     if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);

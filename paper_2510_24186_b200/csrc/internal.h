@@ -289,7 +289,8 @@ struct tridsk_ligands {
 cudaError_t launch_rec_pack(cudaStream_t s, const float* xyz, const int* type, int n_rec, int n_types, float4* out, int* bad);
 cudaError_t launch_grid_build(cudaStream_t s, const float4* rec /* x,y,z,type */, int n_rec,
                               const float* pair_tab /* [n_types][n_types][4] */, int n_types,
-                              const DParams& P, DGrid grid, float dc_max, float* out);
+                              const DParams& P, DGrid grid, float dc_max, const float* radius_h /* host [n_types] */,
+                              const float* rec_radius_dev /* device [n_types] */, float* out);
 cudaError_t launch_grid_pack(cudaStream_t s, DGrid grid, float4* out);
 cudaError_t launch_mc(cudaStream_t s, int J, const McLaunch& a);
 cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta, size_t smem_bytes);
