@@ -633,3 +633,27 @@ def test_error_paths_of_the_optional_modes(gp, system):
         assert e.last_kernel() == 2 and np.all(np.isfinite(r["energy"]))
     finally:
         e.close()
+
+
+def test_grid_build_general_and_lattice_tables(orc, gp):
+    """The grid kernel has two forms of the long-range term: one ex2 per type for a general radius table,
+    and A B^m C_m when the radii lie on a lattice.  Both against the oracle's grid: a jittered (non-lattice) table, a
+    lattice with repeated radii, and the synthetic table."""
+    from paper_2510_24186_b200 import Engine
+    rec = synth.receptor(150, 15.0, 8, seed=5, grid_n=33, pocket_radius=4.0)
+    radius0, role = synth.type_table(8)
+    rng = np.random.default_rng(2)
+    tables = {"lattice": radius0,
+              "general": (radius0 + rng.uniform(-0.03, 0.03, 8)).astype(np.float32),
+              "repeated": np.array([1.5, 1.7, 1.6, 1.7, 1.9, 1.5, 1.8, 1.8], np.float32)}
+    e = Engine(0)
+    try:
+        for name, radius in tables.items():
+            ty = orc.Types(radius, role)
+            G = orc.build_grid(orc.default_params(), ty, rec.xyz, rec.type, rec.origin, rec.dims, rec.spacing)
+            g = e.build_grid(rec.xyz, rec.type, radius, role, gp, rec.origin, rec.dims, rec.spacing)
+            w = worst(g.export(), G.g)
+            assert w <= 1.0, (name, w)
+            g.free()
+    finally:
+        e.close()
