@@ -360,7 +360,7 @@ __device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const Ct
 }
 
 // ------------------------------------------------------------------ the fused MC kernel, one CTA per chain
-__global__ void __launch_bounds__(128, 4) mc_cta_kernel(const McLaunch a) {
+__global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lig = a.lig_list[blockIdx.x / a.n_chains];
