@@ -862,6 +862,10 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
         if (i == 0 || ent[i].cls != ent[i - 1].cls) {
             const bool tm = (ent[i].cls & 0x40000000) != 0;
             lg->lane_plan.push_back({tm ? 32 : ent[i].cls >> 8, 0, i, 0, tm ? (ent[i].cls >> 8) & 0xff : 0});
+            if (!tm) {                                       // resident warps per SM of this class -> register budget
+                const int warps = (ent[i].cls >> 8) * (ent[i].cls & 0xff) / 32;
+                lg->lane_plan.back().minb = getenv("TRIDSK_MINB4") ? 4 : warps <= 8 ? 2 : warps <= 12 ? 3 : 4;
+            }
         }
         lg->lane_plan.back().count++;
         lg->lane_plan.back().smem = std::max(lg->lane_plan.back().smem, ent[i].need);
@@ -987,7 +991,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
                 McLaunch a = base;
                 a.lig_list = lg->all_ids + b.first; a.n_list = b.count;
                 fill(a);
-                a.lane_region = (int)b.smem; a.tm_cols = b.tm_cols;
+                a.lane_region = (int)b.smem; a.tm_cols = b.tm_cols; a.lane_minb = b.minb;
                 series.push_back({b.tm_cols ? 4 : 2, b.chains_per_cta, b.smem, br++ % TRIDSK_BRANCHES, a});
             }
         } else if (mode == 3) {
@@ -1045,7 +1049,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         }
         for (auto& it : series) {
             cudaStream_t bs = it.branch == 0 ? s : ctx->side[it.branch];
-            e = it.kind == 4 ? launch_mc_lane_tm(bs, it.a) : it.kind == 2 ? launch_mc_lane(bs, it.a, it.arg, it.smem)
+            e = it.kind == 4 ? launch_mc_lane_tm(bs, it.a) : it.kind == 2 ? launch_mc_lane(bs, it.a, it.arg, it.smem, it.a.lane_minb)
                 : it.kind == 3 ? launch_mc_cta(bs, it.a, it.arg, it.smem) : launch_mc(bs, it.arg, it.a);
             if (e != cudaSuccess) return e;
         }

@@ -137,6 +137,7 @@ struct McLaunch {
     tridsk_trace_rec* trace;      // [n_lig][n_chains][trace_stride] or NULL
     int trace_stride, trace_off;
     int lane_region, tm_cols;     // tensor-memory lane kernel: shared-memory bytes per warp, TMEM columns per CTA
+    int lane_minb;                // shared-memory lane kernel: register budget class (launch_bounds min blocks)
 };
 
 struct ScoreLaunch {
@@ -278,7 +279,7 @@ struct tridsk_ligands {
     int* cta_bucket_dev[2] = {nullptr, nullptr};
     size_t cta_smem[2] = {0, 0};                 // largest shared-memory need per bucket
     int* all_ids = nullptr;       // 0..n_lig-1 re-ordered per lane bucket (refilled when the plan key changes)
-    struct LaneBucket { int chains_per_cta; size_t smem; int first, count; int tm_cols; long long work = 0; };   // tm_cols > 0: tensor-memory form, smem = bytes per warp
+    struct LaneBucket { int chains_per_cta; size_t smem; int first, count; int tm_cols; long long work = 0; int minb = 4; };   // tm_cols > 0: tensor-memory form, smem = bytes per warp
     std::vector<LaneBucket> lane_plan;
     std::vector<int> lane_ids_h;  // host copy behind all_ids (must outlive the async upload)
     long long lane_plan_key = -1; // n_chains << 8 | (n_refine > 1)
@@ -293,7 +294,7 @@ cudaError_t launch_grid_build(cudaStream_t s, const float4* rec /* x,y,z,type */
                               const float* rec_radius_dev /* device [n_types] */, float* out);
 cudaError_t launch_grid_pack(cudaStream_t s, DGrid grid, float4* out);
 cudaError_t launch_mc(cudaStream_t s, int J, const McLaunch& a);
-cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta, size_t smem_bytes);
+cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta, size_t smem_bytes, int minb);
 cudaError_t launch_mc_lane_tm(cudaStream_t s, const McLaunch& a);
 cudaError_t launch_score_lane(cudaStream_t s, const ScoreLaunch& a, int n_seg, size_t smem_bytes);
 cudaError_t mc_lane_prepare(size_t max_smem_bytes);
