@@ -824,14 +824,14 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
         const size_t topo = lane_topo_bytes(h.n, h.T, h.ls_len, h.n_rec);
         const size_t per_chain = 4 * (size_t)lane_chain_slots(h.n, h.T, h.max_depth, n_refine);
         // chains per CTA: the multiple of a warp that keeps the most warps resident per SM (ties: the larger CTA, which
-        // stages the topology fewer times); 128 registers per thread allow 16 warps per SM
+        // stages the topology fewer times); 168 registers per thread allow 12 warps per SM
         int c = 0, r = 0;
         size_t need = 0;
         for (int cc = cmax; cc >= 32; cc -= 32) {
             const size_t nd = (topo + per_chain * cc + 15) / 16 * 16;
             if (nd > TRIDSK_SMEM_MAX_CTA) continue;
             int rr = (int)(TRIDSK_SMEM_PER_SM / (nd + TRIDSK_SMEM_RESERVED));
-            rr = std::max(1, std::min(std::min(rr, 32), 16 * 32 / cc));
+            rr = std::max(1, std::min(std::min(rr, 32), 12 * 32 / cc));
             if (rr * cc > r * c) { c = cc; r = rr; need = nd; }
         }
         // tensor-memory form (mc_lane_tm_kernel): coordinates in TMEM columns, the rest of the chain state in shared
@@ -864,7 +864,7 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
             lg->lane_plan.push_back({tm ? 32 : ent[i].cls >> 8, 0, i, 0, tm ? (ent[i].cls >> 8) & 0xff : 0});
             if (!tm) {                                       // resident warps per SM of this class -> register budget
                 const int warps = (ent[i].cls >> 8) * (ent[i].cls & 0xff) / 32;
-                lg->lane_plan.back().minb = getenv("TRIDSK_MINB4") ? 4 : warps <= 8 ? 2 : warps <= 12 ? 3 : 4;
+                lg->lane_plan.back().minb = warps <= 8 ? 2 : 3;     // measured: 12 warps at 168 registers beat 16 at 128
             }
         }
         lg->lane_plan.back().count++;

@@ -279,7 +279,7 @@ struct tridsk_ligands {
     int* cta_bucket_dev[2] = {nullptr, nullptr};
     size_t cta_smem[2] = {0, 0};                 // largest shared-memory need per bucket
     int* all_ids = nullptr;       // 0..n_lig-1 re-ordered per lane bucket (refilled when the plan key changes)
-    struct LaneBucket { int chains_per_cta; size_t smem; int first, count; int tm_cols; long long work = 0; int minb = 4; };   // tm_cols > 0: tensor-memory form, smem = bytes per warp
+    struct LaneBucket { int chains_per_cta; size_t smem; int first, count; int tm_cols; long long work = 0; int minb = 3; };   // tm_cols > 0: tensor-memory form, smem = bytes per warp
     std::vector<LaneBucket> lane_plan;
     std::vector<int> lane_ids_h;  // host copy behind all_ids (must outlive the async upload)
     long long lane_plan_key = -1; // n_chains << 8 | (n_refine > 1)

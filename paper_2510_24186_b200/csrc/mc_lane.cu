@@ -548,8 +548,9 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
 
 // ------------------------------------------------------------------ the fused MC kernel, one lane per chain
 // Coordinates in shared memory: one CTA = up to 128 chains of ONE ligand (any ligand size that fits).
-// MINB = resident 128-thread CTAs per SM the register budget must allow (4: 128 registers, 3: 168, 2: 255): the host picks
-// the largest budget that does not lower the residency its shared-memory plan gives a size bucket.
+// MINB = resident 128-thread CTAs per SM the register budget must allow (3: 168 registers, 2: 255): the host picks 255 for
+// the size buckets whose shared-memory need keeps at most 8 warps per SM resident anyway, 168 (12 warps) for the rest --
+// measured: 12 warps at 168 registers beat 16 warps at 128 (C5 1885 -> 1824 ms), 8 warps at 255 do not (1917 ms).
 template <int MINB>
 __global__ void __launch_bounds__(128, MINB) mc_lane_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char lane_smem[];
@@ -626,14 +627,12 @@ __global__ void score_lane_kernel(const ScoreLaunch a);
 
 cudaError_t mc_lane_prepare(size_t max_smem_bytes) {
     if (g_lane_prepared) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(mc_lane_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
+    cudaError_t e = cudaFuncSetAttribute(mc_lane_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<3>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(score_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
     // residency is bound by shared memory (the chains' coordinates): take the whole 228 KB, the grid gathers live in L2 anyway
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_tm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes - 1024);   // it has 16 static bytes
     if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_tm_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e == cudaSuccess) g_lane_prepared = true;
@@ -648,8 +647,7 @@ cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta
     cudaError_t e = mc_lane_prepare(TRIDSK_SMEM_MAX_CTA);
     if (e != cudaSuccess) return e;
     if (minb == 2) mc_lane_kernel<2><<<(unsigned)blocks, chains_per_cta, smem_bytes, s>>>(a);
-    else if (minb == 3) mc_lane_kernel<3><<<(unsigned)blocks, chains_per_cta, smem_bytes, s>>>(a);
-    else mc_lane_kernel<4><<<(unsigned)blocks, chains_per_cta, smem_bytes, s>>>(a);
+    else mc_lane_kernel<3><<<(unsigned)blocks, chains_per_cta, smem_bytes, s>>>(a);
     return cudaGetLastError();
 }
 
