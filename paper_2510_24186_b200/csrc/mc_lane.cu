@@ -170,14 +170,15 @@ __device__ __forceinline__ void lane_fk(const LaneTopo& S, const float t[3], con
 template <class XS>
 __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, float k_wall, bool grad,
                                            const XS& X, float* __restrict__ WR, int C) {
+    constexpr int GA = 2;                                        // atoms in flight
     float e_inter = 0.f;
     float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     int gcur = 0;
-    for (int a0 = 0; a0 < S.n; a0 += 4) {
-        float e[4], gx[4], gy[4], gz[4], x[4], y[4], z[4];
-        int m[4];
+    for (int a0 = 0; a0 < S.n; a0 += GA) {
+        float e[GA], gx[GA], gy[GA], gz[GA], x[GA], y[GA], z[GA];
+        int m[GA];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < GA; ++i) {
             const int a = min(a0 + i, S.n - 1);               // the tail repeats the last atom (result unused)
             m[i] = S.meta[a];
             X.get(3 * a, x[i], y[i], z[i]);
@@ -185,7 +186,7 @@ __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, fl
             e[i] = grid_interp_packed<true>(G, k_wall, m[i] & 0xff, x[i], y[i], z[i], gx[i], gy[i], gz[i]);
         }
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < GA; ++i) {
             if (a0 + i < S.n) {
                 e_inter += e[i];
                 if (grad) {
