@@ -830,7 +830,7 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
         for (int cc = cmax; cc >= 32; cc -= 32) {
             const size_t nd = (topo + per_chain * cc + 15) / 16 * 16;
             if (nd > TRIDSK_SMEM_MAX_CTA) continue;
-            int rr = (int)(TRIDSK_SMEM_PER_SM / (nd + TRIDSK_SMEM_RESERVED));
+            int rr = (int)(TRIDSK_SMEM_PER_SM / ((nd + 1023) / 1024 * 1024 + TRIDSK_SMEM_RESERVED));   // allocated in KB units
             rr = std::max(1, std::min(std::min(rr, 32), 12 * 32 / cc));
             if (rr * cc > r * c) { c = cc; r = rr; need = nd; }
         }
