@@ -827,12 +827,16 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
         // stages the topology fewer times); 168 registers per thread allow 12 warps per SM
         int c = 0, r = 0;
         size_t need = 0;
+        long long best_live = -1;
         for (int cc = cmax; cc >= 32; cc -= 32) {
             const size_t nd = (topo + per_chain * cc + 15) / 16 * 16;
             if (nd > TRIDSK_SMEM_MAX_CTA) continue;
             int rr = (int)(TRIDSK_SMEM_PER_SM / ((nd + 1023) / 1024 * 1024 + TRIDSK_SMEM_RESERVED));   // allocated in KB units
             rr = std::max(1, std::min(std::min(rr, 32), 12 * 32 / cc));
-            if (rr * cc > r * c) { c = cc; r = rr; need = nd; }
+            // live chains resident per SM: a ligand's last CTA may be partly empty (128 chains in CTAs of 96 = 96 + 32)
+            const int cpl_ = (n_chains + cc - 1) / cc;
+            const long long live = (long long)rr * n_chains / cpl_;
+            if (live > best_live) { best_live = live; c = cc; r = rr; need = nd; }
         }
         // tensor-memory form (mc_lane_tm_kernel): coordinates in TMEM columns, the rest of the chain state in shared
         // memory, 4 warps per CTA each with its own topology copy; taken when it keeps more warps resident
