@@ -70,8 +70,8 @@ __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char*
 // Shared memory, slot-major (slot i of this lane's chain is X[i * C]) -- or TENSOR MEMORY: 256 KB per SM that nothing
 // else on this path uses.  A CTA of four warps owns `cols` columns of all 128 TMEM lanes; lane = chain, column 3a + c =
 // coordinate c of atom a, moved with tcgen05.st / tcgen05.ld (32x32b: every thread of a warp touches its own lane).
-// Taking the coordinates (two thirds of a chain's shared memory) out of shared memory is what lets 16 warps stay
-// resident per SM instead of 8-12.  A load is asynchronous: fence() (tcgen05.wait::ld, tied to the destination
+// Taking the coordinates (two thirds of a chain's shared memory) out of shared memory lets 12 warps stay resident per
+// SM where the shared-memory form holds 6-10 (measured: on par overall; an explicit option).  A load is asynchronous: fence() (tcgen05.wait::ld, tied to the destination
 // registers) must sit between get() and the first use.
 struct XShared {
     float* X; int C;
