@@ -71,8 +71,9 @@ __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char*
 // else on this path uses.  A CTA of four warps owns `cols` columns of all 128 TMEM lanes; lane = chain, column 3a + c =
 // coordinate c of atom a, moved with tcgen05.st / tcgen05.ld (32x32b: every thread of a warp touches its own lane).
 // Taking the coordinates (two thirds of a chain's shared memory) out of shared memory lets 12 warps stay resident per
-// SM where the shared-memory form holds 6-10 (measured: on par overall; an explicit option).  A load is asynchronous: fence() (tcgen05.wait::ld, tied to the destination
-// registers) must sit between get() and the first use.
+// SM where the shared-memory form holds 6-10 (measured: on par overall; an explicit option).
+// A load is asynchronous: fence() (tcgen05.wait::ld, tied to the destination registers) must sit between get() and
+// the first use.
 struct XShared {
     float* X; int C;
     __device__ __forceinline__ void put(int a, float x, float y, float z) const { float* xa = X + 3 * a * C; xa[0] = x; xa[C] = y; xa[2 * C] = z; }
