@@ -657,3 +657,40 @@ def test_grid_build_general_and_lattice_tables(orc, gp):
             g.free()
     finally:
         e.close()
+
+
+@pytest.mark.parametrize("mode", [1, 2, 3, 4])
+def test_extreme_ligand_sizes_under_every_mapping(orc, gp, mode):
+    """Ligands from 2 atoms / 0 torsions to the limits (128 atoms, 31 torsions), including the sizes around the 32-atom
+    and 64-atom boundaries of the mappings: per-pose energy and gradient vs the oracle, and the poses a short dock returns
+    re-scored by the oracle."""
+    from paper_2510_24186_b200 import Engine
+    rec = synth.receptor(300, 20.0, 16, seed=1001, grid_n=54)
+    radius, role = synth.type_table(16)
+    ty, p = orc.Types(radius, role), orc.default_params()
+    G = orc.build_grid(p, ty, rec.xyz, rec.type, rec.origin, rec.dims, rec.spacing)
+    ns = [2, 3, 5, 9, 16, 17, 31, 32, 33, 47, 63, 64, 65, 90, 100, 127, 128]
+    ts = [0, 0, 1, 2, 4, 0, 8, 10, 12, 15, 20, 25, 31, 31, 28, 31, 31]
+    batch = synth.ligands(ns, ts, 16, seed=77)
+    e = Engine(0)
+    try:
+        e.set_kernel(mode)
+        grid = e.grid_from_values(G.g, rec.origin, rec.spacing)
+        ligs = e.load_ligands(batch, radius, role)
+        li = np.repeat(np.arange(batch.n_lig, dtype=np.int32), 2)
+        poses = synth.random_poses(batch, li, rec, seed=5, spread=0.5)
+        en, gr, _ = e.score_grad(grid, ligs, gp, li, poses)
+        Ls = [orc.ligand_from_batch(batch, l) for l in range(batch.n_lig)]
+        for i in range(len(li)):
+            L = Ls[int(li[i])]
+            eo, go, _, _ = orc.score_grad(p, ty, G, L, poses[i, :7 + L.T].astype(np.float64))
+            assert worst(en[i], eo) <= 1.0, (mode, L.n, L.T)
+            assert worst(gr[i, :6 + L.T], go, scale=np.abs(go).max()) <= 1.0, (mode, L.n, L.T)
+        r = e.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, 40, 12, 2, seed=9)
+        assert e.last_kernel() == mode
+        for l, L in enumerate(Ls):
+            for k in range(2):
+                eo = orc.score_grad(p, ty, G, L, r["pose"][l, k, :7 + L.T].astype(np.float64), want_grad=False)[0][0]
+                assert close(r["energy"][l, k, 0], eo, rtol=2e-4, atol=2e-3), (mode, L.n, L.T)
+    finally:
+        e.close()
