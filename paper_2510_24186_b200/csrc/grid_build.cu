@@ -47,7 +47,8 @@ struct GridLattice {
     float cm[TRIDSK_MAX_TYPES];   // C_m of sorted position k
 };
 
-template <int NT, bool LAT>
+// LAT: 0 general table, 1 lattice, 2 lattice whose sorted types all step up by one delta (no select per type)
+template <int NT, int LAT>
 __global__ void __launch_bounds__(GB_THREADS) grid_build_kernel(const float4* __restrict__ rec, int n_rec,
                                                                 const float4* __restrict__ pair_tab, int n_types,
                                                                 const DParams P, const DGrid G, float dc_max,
@@ -120,7 +121,7 @@ __global__ void __launch_bounds__(GB_THREADS) grid_build_kernel(const float4* __
                 float pw = exp2f_approx(nk2 * xs * xs);
 #pragma unroll
                 for (int k = 0; k < NT; ++k) {                  // sorted by radius; padding positions have cm = 0
-                    if (k > 0) pw = ((lat.step_mask >> k) & 1u) ? pw * B : pw;
+                    if (k > 0) pw = (LAT == 2 || ((lat.step_mask >> k) & 1u)) ? pw * B : pw;
                     acc[k] = fmaf(pw, lat.cm[k], acc[k]);
                 }
             } else {
@@ -210,13 +211,15 @@ cudaError_t launch_grid_build(cudaStream_t s, const float4* rec, int n_rec, cons
             lat.cm[k] = (float)exp2(nk2 * (m * delta) * (m * delta));
         }
         if (ok && m * delta * 2.0 * fabs(nk2) * 12.0 < 60.0) {       // B^m stays far from overflow for |x| < 12 A
-            lat.on = 1; lat.delta_k = (float)(-2.0 * nk2 * delta); lat.rmin = radius_h[ord[0]];
+            lat.on = lat.step_mask == ((n_types >= 32 ? 0xffffffffu : ((1u << n_types) - 1u)) & ~1u) ? 2 : 1;
+            lat.delta_k = (float)(-2.0 * nk2 * delta); lat.rmin = radius_h[ord[0]];
         }
     }
 #define TRIDSK_GB_LAUNCH(NT)                                                                                              \
     do {                                                                                                                  \
-        if (lat.on) grid_build_kernel<NT, true><<<g, GB_THREADS, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, lat, rec_radius_dev, out); \
-        else grid_build_kernel<NT, false><<<g, GB_THREADS, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, lat, rec_radius_dev, out);       \
+        if (lat.on == 2) grid_build_kernel<NT, 2><<<g, GB_THREADS, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, lat, rec_radius_dev, out);   \
+        else if (lat.on) grid_build_kernel<NT, 1><<<g, GB_THREADS, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, lat, rec_radius_dev, out);  \
+        else grid_build_kernel<NT, 0><<<g, GB_THREADS, 0, s>>>(rec, n_rec, tab, n_types, P, grid, dc_max, lat, rec_radius_dev, out);            \
     } while (0)
     if (n_types <= 8) TRIDSK_GB_LAUNCH(8);
     else if (n_types <= 16) TRIDSK_GB_LAUNCH(16);
