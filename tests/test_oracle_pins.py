@@ -401,21 +401,21 @@ def _quat_left_mul_rotvec(q_wxyz, v):
     return np.array([w, x, y, z])
 
 
-def _safe_pose(orc, S, L, rng):
-    """A pose with no atom within 1e-3 (grid units) of a cell face and no pair within 1e-3 of an indicator edge."""
+def _safe_pose(orc, S, L, rng, margin=1e-3):
+    """A pose with no atom within `margin` (grid units) of a cell face and no pair within `margin` of an indicator edge."""
     G = S["G"]
     for _ in range(200):
         pose = np.concatenate([7.5 + rng.uniform(-2.5, 2.5, 3), rng.normal(size=4), rng.uniform(-np.pi, np.pi, L.T)])
         pose[3:7] /= np.linalg.norm(pose[3:7])
         x = orc.fk(L, pose)
         u = (x - G.origin) / G.spacing
-        if np.any(u < 0.01) or np.any(u > 39.99) or np.min(np.abs(u - np.rint(u))) < 1e-3:
+        if np.any(u < 0.01) or np.any(u > 39.99) or np.min(np.abs(u - np.rint(u))) < margin:
             continue
         ok = True
         for a, b in L.pairs.astype(int):
             d = np.linalg.norm(x[a] - x[b])
             r = S["ty"].radius[L.type[a]] + S["ty"].radius[L.type[b]]
-            if min(abs(d - e) for e in (10.0, 3.4, 2.6, r, 0.05)) < 1e-3:
+            if min(abs(d - e) for e in (10.0, 3.4, 2.6, r, 0.05)) < margin:
                 ok = False
         if ok:
             return pose
@@ -571,6 +571,148 @@ def test_perturbation_entities_and_ranges(orc, dock_system):
             ang = 2 * math.acos(min(1.0, abs(pose[3])))
             assert ang <= 0.5 * math.sqrt(3) + 1e-12
     assert counts.min() > 3000 / 6 * 0.8
+
+
+# --------------------------------------------------------------------------- O12: rotation / torsion branch of the MC step
+def _rigid_entity_counter(orc, L, seed, lig, want):
+    """(chain, step) whose perturbation block picks entity `want` (0 translation, 1 rotation, 2+k torsion k)."""
+    for chain in range(64):
+        for step in range(64):
+            if int(math.floor(orc.uniform4(seed, chain, step, lig, 0)[0] * (L.T + 2))) == want:
+                return chain, step
+    raise RuntimeError("no counter found")
+
+
+def _rot(q_wxyz):
+    return Rotation.from_quat([q_wxyz[1], q_wxyz[2], q_wxyz[3], q_wxyz[0]])
+
+
+def test_adam_step_is_first_order_descent_on_all_components(orc, dock_system):
+    """O12 / G9 / G14.  With zero perturbation amplitudes the proposal is the current pose; the first Adam step is
+    delta_i = -lr g_i / (|g_i| + eps) = -lr sign(g_i) on every one of the 6+T tangent components (translation, WORLD-frame
+    rotation vector about t, torsions).  Two pins that do not retype the update:
+      (a) the descent identity  E(pose') - E(pose) = sum_i g_i delta_i + O(lr^2) = -lr sum_i |g_i|, with g the gradient
+          that test_gradient_matches_central_differences pins against finite differences -- it fails for a body-frame
+          composition q (x) exp(d), a quarter angle in exp_q, a sign or an index slip in the torsion update;
+      (b) the returned pose equals t - lr sign(g_t), Rotation.from_rotvec(-lr sign(g_w)) * Rotation(q) (scipy composes),
+          theta - lr sign(g_theta)."""
+    S = dock_system
+    rng = np.random.default_rng(101)
+    lr = 1e-5
+    p = orc.default_params(pert_trans=0.0, pert_rot=0.0, lr=lr, n_refine=1)
+    rec_ = S["rec"]
+    E = lambda L, pose: orc.score_grad(p, S["ty"], S["G"], L, pose, want_grad=False)[0][0]
+    n_sign_mixed = 0
+    for li, L in enumerate(S["L"]):
+        for trial in range(6):
+            pose0 = _safe_pose(orc, S, L, rng, margin=5e-3)
+            pose0[:3] = np.clip(pose0[:3], rec_.box_min + 0.01, rec_.box_max - 0.01)
+            x = orc.fk(L, pose0)
+            u = (x - S["G"].origin) / S["G"].spacing
+            if np.min(np.abs(u - np.rint(u))) < 5e-3:
+                continue
+            e0, g, _, _ = orc.score_grad(p, S["ty"], S["G"], L, pose0)
+            if np.min(np.abs(g)) < 1e-3:                      # sign(g_i) must be unambiguous
+                continue
+            chain, step = _rigid_entity_counter(orc, L, 5, li, trial % 2)        # entity 0 or 1: amplitudes are zero
+            pose1, e1, rec = orc.mc_step(p, S["ty"], S["G"], L, 5, chain, step, li, rec_.box_min, rec_.box_max, pose0, 1e9)
+            assert rec.accept == 1 and rec.entity == trial % 2
+            assert e1 == pytest.approx(E(L, pose1), rel=1e-13)
+            # (a) first-order descent identity over all 6+T components
+            assert e1 - e0[0] == pytest.approx(-lr * np.abs(g).sum(), rel=2e-3)
+            # (b) the pose itself
+            sg = g / (np.abs(g) + 1e-8)                        # Adam's first step in closed form: -lr g / (|g| + eps)
+            assert pose1[:3] == pytest.approx(pose0[:3] - lr * sg[:3], abs=1e-12)
+            r_exp = Rotation.from_rotvec(-lr * sg[3:6]) * _rot(pose0[3:7])
+            r_got = _rot(pose1[3:7])
+            assert (r_got * r_exp.inv()).magnitude() < 1e-10
+            assert (r_got * (_rot(pose0[3:7]) * Rotation.from_rotvec(-lr * sg[3:6])).inv()).magnitude() > 1e-7 or \
+                np.allclose(sg[3:6], 0)                        # and it is NOT the body-frame composition
+            assert abs(np.linalg.norm(pose1[3:7]) - 1) < 1e-14
+            assert pose1[7:] == pytest.approx(pose0[7:] - lr * sg[6:], abs=1e-12)
+            n_sign_mixed += int(len(set(np.sign(g[6:]))) > 1) if L.T > 1 else 0
+    assert n_sign_mixed >= 3                                   # an index swap among torsions would have shown
+
+
+def test_perturbation_values_and_rotation_composition(orc, dock_system):
+    """O12 / G11: with lr = 0 the accepted pose IS the perturbed pose.  Translation: t + 2 A (2u-1) per axis, clamped;
+    rotation: left-multiplied (world-frame) rotation vector w = 0.5 rad (2u-1): every atom moves by
+    x' - t = Rot(w)(x - t) with scipy's Rotation; torsion k: theta_k = pi (2u_1 - 1).  The uniforms are the Philox block
+    (chain, step, ligand, purpose 0), pinned by the known answers."""
+    S = dock_system
+    rec_ = S["rec"]
+    p = orc.default_params(lr=0.0)
+    rng = np.random.default_rng(77)
+    seen = set()
+    for li, L in enumerate(S["L"]):
+        pose0 = np.concatenate([rec_.pocket_center + rng.uniform(-1, 1, 3), rng.normal(size=4), rng.uniform(-3, 3, L.T)])
+        pose0[3:7] /= np.linalg.norm(pose0[3:7])
+        x0 = orc.fk(L, pose0)
+        for i in range(60):
+            chain, step = i % 7, i // 7
+            u = orc.uniform4(11, chain, step, li, 0)
+            pose1, _, rec = orc.mc_step(p, S["ty"], S["G"], L, 11, chain, step, li, rec_.box_min, rec_.box_max, pose0, 1e9)
+            ent = int(math.floor(u[0] * (L.T + 2)))
+            assert rec.entity == ent and rec.accept == 1
+            seen.add(min(ent, 2))
+            x1 = orc.fk(L, pose1)
+            if ent == 0:
+                assert pose1[:3] == pytest.approx(np.clip(pose0[:3] + 2.0 * (2 * u[1:4] - 1), rec_.box_min, rec_.box_max), abs=1e-13)
+                assert x1 - pose1[:3] == pytest.approx(x0 - pose0[:3], abs=1e-12)
+            elif ent == 1:
+                w = 0.5 * (2 * u[1:4] - 1)
+                assert x1 - pose0[:3] == pytest.approx(Rotation.from_rotvec(w).apply(x0 - pose0[:3]), abs=1e-11)
+                body = (_rot(pose0[3:7]) * Rotation.from_rotvec(w)).apply(L.ref)      # the wrong (body-frame) order differs
+                assert L.T > 0 or np.abs(body + pose0[:3] - x1).max() > 1e-3
+            else:
+                exp = pose0.copy(); exp[7 + ent - 2] = math.pi * (2 * u[1] - 1)
+                assert pose1 == pytest.approx(exp, abs=1e-13)
+    assert seen == {0, 1, 2}
+
+
+def test_torsion_wrap_and_box_clamp_in_the_adam_update(orc, dock_system):
+    """G14: torsions are wrapped into [-pi, pi) (same coordinates as the unwrapped angle), translations clamped to the box."""
+    S = dock_system
+    rec_ = S["rec"]
+    lr = 0.1
+    p = orc.default_params(pert_trans=0.0, pert_rot=0.0, lr=lr, n_refine=1)
+    rng = np.random.default_rng(5)
+    wrapped_up = wrapped_dn = 0
+    for li, L in enumerate(S["L"]):
+        for trial in range(40):
+            pose0 = np.concatenate([rec_.pocket_center + rng.uniform(-1, 1, 3), rng.normal(size=4),
+                                    rng.choice([-1.0, 1.0], L.T) * (math.pi - 0.05 * rng.uniform(0.1, 1.0, L.T))])
+            pose0[3:7] /= np.linalg.norm(pose0[3:7])
+            _, g, _, _ = orc.score_grad(p, S["ty"], S["G"], L, pose0)
+            if np.min(np.abs(g)) < 1e-6:
+                continue
+            chain, step = _rigid_entity_counter(orc, L, 3, li, 0)
+            pose1, _, rec = orc.mc_step(p, S["ty"], S["G"], L, 3, chain, step, li, rec_.box_min - 50, rec_.box_max + 50, pose0, 1e9)
+            raw = pose0[7:] - lr * g[6:] / (np.abs(g[6:]) + 1e-8)         # first Adam step (pinned above)
+            assert np.all(pose1[7:] >= -math.pi) and np.all(pose1[7:] < math.pi)
+            k_wrap = np.rint((raw - pose1[7:]) / (2 * math.pi))
+            assert pose1[7:] == pytest.approx(raw - 2 * math.pi * k_wrap, abs=1e-12)
+            wrapped_up += int(np.sum(k_wrap > 0)); wrapped_dn += int(np.sum(k_wrap < 0))
+            unwrapped = pose1.copy(); unwrapped[7:] = raw
+            assert orc.fk(L, pose1) == pytest.approx(orc.fk(L, unwrapped), abs=1e-9)
+    assert wrapped_up > 5 and wrapped_dn > 5
+    # exactly -pi stays, +pi maps to -pi: the half-open interval
+    L = S["L"][0]
+    p0 = orc.default_params(pert_trans=0.0, pert_rot=0.0, lr=0.0)
+    chain, step = _rigid_entity_counter(orc, L, 3, 0, 0)
+    for th_in, th_out in ((math.pi, -math.pi), (-math.pi, -math.pi), (math.pi - 1e-9, math.pi - 1e-9)):
+        pose0 = np.concatenate([rec_.pocket_center, [1, 0, 0, 0], [th_in] * L.T])
+        pose1, _, _ = orc.mc_step(p0, S["ty"], S["G"], L, 3, chain, step, 0, rec_.box_min, rec_.box_max, pose0, 1e9)
+        assert pose1[7:] == pytest.approx([th_out] * L.T, abs=1e-15)    # (wrap's a + pi rounds in the last bit)
+    # box clamp, closed form: one atom left of a zero grid, E = k_wall x^2, g = 2 k_wall x < 0 -> step +lr, cut at box_max
+    L1, G1, ty1 = one_atom_system(orc)
+    pose0 = [-1.0, 1.5, 1.5, 1, 0, 0, 0]
+    e0 = orc.score_grad(p, ty1, G1, L1, pose0)[0][0]
+    assert e0 == pytest.approx(10.0, rel=1e-14)
+    pose1, e1, rec = orc.mc_step(p, ty1, G1, L1, 0, 0, 0, 0, [-100.0] * 3, [-0.95, 100.0, 100.0], pose0, e0)
+    assert pose1[0] == -0.95 and e1 == pytest.approx(10.0 * 0.95 ** 2, rel=1e-14) and rec.accept == 1
+    pose1, e1, rec = orc.mc_step(p, ty1, G1, L1, 0, 0, 0, 0, [-100.0] * 3, [100.0] * 3, pose0, e0)
+    assert pose1[0] == pytest.approx(-1.0 + 0.1 * 20.0 / (20.0 + 1e-8), rel=1e-14)   # unclamped: the full Adam step
 
 
 # --------------------------------------------------------------------------- whole chain sanity, O13, E_screen
