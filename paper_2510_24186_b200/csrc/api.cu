@@ -92,6 +92,11 @@ extern "C" int tridsk_create(tridsk_ctx** out, int device, void* cuda_stream) {
         return TRIDSK_ECUDA;
     }
     ctx->sm_count = prop.multiProcessorCount;
+    // kernel attributes are per device: opt every kernel in to its shared-memory size on THIS device
+    e = mc_lane_prepare(TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = mc_cta_prepare();
+    if (e == cudaSuccess) e = topk_prepare();
+    if (e != cudaSuccess) { fprintf(stderr, "tridsk_create: %s\n", cudaGetErrorString(e)); delete ctx; return TRIDSK_ECUDA; }
     if (!ctx->stream) {               // the legacy default stream cannot be captured into a graph: own one
         e = cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking);
         if (e != cudaSuccess) { fprintf(stderr, "tridsk_create: %s\n", cudaGetErrorString(e)); delete ctx; return TRIDSK_ECUDA; }

@@ -77,7 +77,7 @@ struct LaneFrag {
 // One record = one partner atom b against the 4 slots of the tile.  In global memory (LaneRec) it holds what depends
 // on the ligand only; lane_stage turns it into the 20-byte shared-memory form (two arrays) that also depends on the
 // parameters:  c[4] = dvdw + long_mu (slot without a pair -- excluded, or beyond the tile width: -1e15), and one word
-// 3 * b | hbmask << 16.  The pair arithmetic then has no topology branch: a slot without a pair evaluates to exactly
+// scale * b | hbmask << 16 (scale * b = where atom b's coordinates start in the chain's coordinate store).  The pair arithmetic then has no topology branch: a slot without a pair evaluates to exactly
 // zero (its clash distance c - mu is negative).
 struct LaneRec {
     float dvdw[4];                // r_a + r_b per slot; < 0 for a slot without a pair
@@ -187,7 +187,7 @@ struct TopkLaunch {
 #define TRIDSK_SMEM_MAX_CTA 232448     // 227 KB opt-in maximum per CTA
 __host__ __device__ static inline size_t lane_topo_bytes(int n, int T, int ls_len, int n_rec) {
     return 16 * (size_t)n + 16 * (size_t)((n + 3) / 4) + sizeof(LaneFrag) * (size_t)(T + 1) + 16 * (size_t)ls_len +
-           (TRIDSK_LANE_REC_SMEM * (size_t)n_rec + 15) / 16 * 16;
+           (TRIDSK_LANE_REC_SMEM * (size_t)(n_rec + 1) + 15) / 16 * 16;   // + the pad record
 }
 __host__ __device__ static inline int lane_wslots(int T, int max_depth) {
     return 6 * (T + 1) > 12 * max_depth ? 6 * (T + 1) : 12 * max_depth;
@@ -297,7 +297,9 @@ cudaError_t launch_mc(cudaStream_t s, int J, const McLaunch& a);
 cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta, size_t smem_bytes, int minb);
 cudaError_t launch_mc_lane_tm(cudaStream_t s, const McLaunch& a);
 cudaError_t launch_score_lane(cudaStream_t s, const ScoreLaunch& a, int n_seg, size_t smem_bytes);
-cudaError_t mc_lane_prepare(size_t max_smem_bytes);
+cudaError_t mc_lane_prepare(size_t max_smem_bytes);   // the *_prepare functions opt the kernels in to large shared memory on the CURRENT device
+cudaError_t mc_cta_prepare();
+cudaError_t topk_prepare();
 cudaError_t launch_score(cudaStream_t s, const ScoreLaunch& a);
 cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int threads, size_t smem_bytes);
 cudaError_t launch_score_cta(cudaStream_t s, const ScoreLaunch& a, size_t smem_bytes);

@@ -534,12 +534,10 @@ __global__ void __launch_bounds__(256) score_cta_kernel(const ScoreLaunch a) {
     }
 }
 
-static bool g_cta_prepared = false;
-static cudaError_t mc_cta_prepare() {
-    if (g_cta_prepared) return cudaSuccess;
+// per device (function attributes are per device): called by tridsk_create
+cudaError_t mc_cta_prepare() {
     cudaError_t e = cudaFuncSetAttribute(mc_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(score_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
-    if (e == cudaSuccess) g_cta_prepared = true;
     return e;
 }
 
@@ -547,16 +545,12 @@ cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int threads, size_t
     const long long blocks = (long long)a.n_list * a.n_chains;
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL || (threads != 128 && threads != 256)) return cudaErrorInvalidValue;
-    cudaError_t e = mc_cta_prepare();
-    if (e != cudaSuccess) return e;
     mc_cta_kernel<<<(unsigned)blocks, threads, smem_bytes, s>>>(a);
     return cudaGetLastError();
 }
 
 cudaError_t launch_score_cta(cudaStream_t s, const ScoreLaunch& a, size_t smem_bytes) {
     if (a.n_pose <= 0) return cudaSuccess;
-    cudaError_t e = mc_cta_prepare();
-    if (e != cudaSuccess) return e;
     score_cta_kernel<<<a.n_pose, 256, smem_bytes, s>>>(a);
     return cudaGetLastError();
 }

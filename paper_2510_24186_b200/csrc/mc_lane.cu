@@ -32,18 +32,22 @@ struct LaneTopo {
 };
 
 // Stage one ligand's topology into shared memory; returns the first byte after it (16-byte aligned).  The pair
-// records take their parameter-dependent form here (internal.h): c = dvdw + mu, 3 * b | hbmask << 16.
+// records take their parameter- and launch-dependent form here (internal.h): c = dvdw + mu, and one word
+// rec_scale * b | hbmask << 16 -- rec_scale * b is where the coordinates of partner atom b start in the chain's
+// coordinate store (3 C floats per atom in shared memory, 3 columns in tensor memory), so the record loop adds it to a
+// base and loads.  One pad record (no pairs, atom 0) follows the last one: the loop always fetches one record ahead.
 __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char* smem, const LigHdr* __restrict__ h,
                                                      const float4* __restrict__ atom_f4, const int* __restrict__ atom_i,
                                                      const LaneFrag* __restrict__ lane_frags, const uint4* __restrict__ lane_stream,
-                                                     const LaneRec* __restrict__ lane_recs, const DParams& P, int tid, int nt) {
+                                                     const LaneRec* __restrict__ lane_recs, const DParams& P, int tid, int nt,
+                                                     uint32_t rec_scale) {
     const int n = h->n, T = h->T, ls = h->ls_len, nr = h->n_rec;
     float4* ref = reinterpret_cast<float4*>(smem);
     int* meta = reinterpret_cast<int*>(smem + 16 * (size_t)n);
     int* frag = reinterpret_cast<int*>(smem + 16 * (size_t)n + 16 * (size_t)((n + 3) / 4));
     uint4* stream = reinterpret_cast<uint4*>(reinterpret_cast<unsigned char*>(frag) + sizeof(LaneFrag) * (size_t)(T + 1));
     float4* rec_c = reinterpret_cast<float4*>(stream + ls);
-    uint32_t* rec_m = reinterpret_cast<uint32_t*>(rec_c + nr);
+    uint32_t* rec_m = reinterpret_cast<uint32_t*>(rec_c + nr + 1);
     const LaneFrag* fsrc = lane_frags + h->frag_off;
     for (int i = tid; i < n; i += nt) ref[i] = __ldg(atom_f4 + h->atom_off + i);
     for (int i = tid; i < (T + 1) * (int)(sizeof(LaneFrag) / 4); i += nt) frag[i] = __ldg(reinterpret_cast<const int*>(fsrc) + i);
@@ -52,7 +56,8 @@ __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char*
         for (int a = lo; a < hi; ++a) meta[a] = (__ldg(atom_i + h->atom_off + a) & 0xff) | ((a == lo) << 8) | (g << 16);
     }
     for (int i = tid; i < ls; i += nt) stream[i] = __ldg(lane_stream + h->ls_off + i);
-    for (int i = tid; i < nr; i += nt) {
+    for (int i = tid; i <= nr; i += nt) {
+        if (i == nr) { rec_c[i] = make_float4(-1e15f, -1e15f, -1e15f, -1e15f); rec_m[i] = 0u; continue; }
         const uint4* src = reinterpret_cast<const uint4*>(lane_recs + h->rec_off + i);
         const uint4 dv = __ldg(src), mt = __ldg(src + 1);
         const float d[4] = {__uint_as_float(dv.x), __uint_as_float(dv.y), __uint_as_float(dv.z), __uint_as_float(dv.w)};
@@ -60,37 +65,44 @@ __device__ __forceinline__ unsigned char* lane_stage(LaneTopo& S, unsigned char*
 #pragma unroll
         for (int k = 0; k < 4; ++k) c[k] = d[k] >= 0.f ? d[k] + P.long_mu : -1e15f;
         rec_c[i] = make_float4(c[0], c[1], c[2], c[3]);
-        rec_m[i] = 3u * mt.x | (mt.y << 16);
+        rec_m[i] = rec_scale * mt.x | (mt.y << 16);
     }
     S.ref = ref; S.meta = meta; S.frag = reinterpret_cast<const LaneFrag*>(frag); S.stream = stream; S.rec_c = rec_c; S.rec_m = rec_m; S.n = n; S.T = T;
     return smem + lane_topo_bytes(n, T, ls, nr);
 }
 
 // ------------------------------------------------------------------ the coordinates of one chain
-// Shared memory, slot-major (slot i of this lane's chain is X[i * C]) -- or TENSOR MEMORY: 256 KB per SM that nothing
-// else on this path uses.  A CTA of four warps owns `cols` columns of all 128 TMEM lanes; lane = chain, column 3a + c =
-// coordinate c of atom a, moved with tcgen05.st / tcgen05.ld (32x32b: every thread of a warp touches its own lane).
-// Taking the coordinates (two thirds of a chain's shared memory) out of shared memory lets 12 warps stay resident per
-// SM where the shared-memory form holds 6-10 (measured: on par overall; an explicit option).
-// A load is asynchronous: fence() (tcgen05.wait::ld, tied to the destination registers) must sit between get() and
-// the first use.
+// Shared memory, slot-major (slot i of this lane's chain is X[i * C], C = chains per CTA, a compile-time constant so
+// that every slot offset is an immediate) -- or TENSOR MEMORY: 256 KB per SM that nothing else on this path uses.  A CTA
+// of four warps owns `cols` columns of all 128 TMEM lanes; lane = chain, column 3a + c = coordinate c of atom a, moved
+// with tcgen05.st / tcgen05.ld (32x32b: every thread of a warp touches its own lane).  Taking the coordinates (two thirds
+// of a chain's shared memory) out of shared memory lets 12 warps stay resident per SM where the shared-memory form holds
+// 6-10 (measured: on par overall; an explicit option).
+// get(off, ...) takes the atom's offset in the store's own unit, off = kScale * a (what the pair records carry).
+// A tensor-memory load is asynchronous: fence() (tcgen05.wait::ld, tied to the destination registers) must sit between
+// get() and the first use.
+template <int C>
 struct XShared {
-    float* X; int C;
+    static constexpr int kC = C;
+    static constexpr uint32_t kScale = 3u * C;
+    float* X;
     __device__ __forceinline__ void put(int a, float x, float y, float z) const { float* xa = X + 3 * a * C; xa[0] = x; xa[C] = y; xa[2 * C] = z; }
-    __device__ __forceinline__ void get(int a3, float& x, float& y, float& z) const { const float* xa = X + a3 * C; x = xa[0]; y = xa[C]; z = xa[2 * C]; }
+    __device__ __forceinline__ void get(uint32_t off, float& x, float& y, float& z) const { const float* xa = X + off; x = xa[0]; y = xa[C]; z = xa[2 * C]; }
     __device__ __forceinline__ void fence(float&, float&, float&) const {}
     __device__ __forceinline__ void flush() const {}
 };
 struct XTensor {
+    static constexpr int kC = 32;
+    static constexpr uint32_t kScale = 3u;
     uint32_t tb;            // TMEM address of column 0 in this warp's lane quarter
     // writes columns 3a .. 3a+3: atoms are placed in ascending order, so the fourth column is rewritten by atom a + 1
     __device__ __forceinline__ void put(int a, float x, float y, float z) const {
         asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
                      :: "r"(tb + 3u * (uint32_t)a), "r"(__float_as_uint(x)), "r"(__float_as_uint(y)), "r"(__float_as_uint(z)), "r"(0u) : "memory");
     }
-    __device__ __forceinline__ void get(int a3, float& x, float& y, float& z) const {
+    __device__ __forceinline__ void get(uint32_t off, float& x, float& y, float& z) const {
         uint32_t r0, r1, r2, r3;
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(tb + (uint32_t)a3) : "memory");
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(tb + off) : "memory");
         x = __uint_as_float(r0); y = __uint_as_float(r1); z = __uint_as_float(r2);
     }
     __device__ __forceinline__ void fence(float& x, float& y, float& z) const {
@@ -113,7 +125,8 @@ __device__ __forceinline__ void lane_place(const LaneTopo& S, const float R[9], 
 }
 template <class XS>
 __device__ __forceinline__ void lane_fk(const LaneTopo& S, const float t[3], const float q[4], const float* __restrict__ th,
-                                        const XS& X, float* __restrict__ FR, int C) {
+                                        const XS& X, float* __restrict__ FR) {
+    constexpr int C = XS::kC;
     float R[9], p[3];
     quat_matrix(q, R);
     p[0] = t[0]; p[1] = t[1]; p[2] = t[2];
@@ -164,88 +177,179 @@ __device__ __forceinline__ void lane_fk(const LaneTopo& S, const float t[3], con
 }
 
 // ------------------------------------------------------------------ a4 receptor energy (O5)
-// Two 16-byte records of the xy-packed grid per atom, four atoms in flight.  grad: WR[g] <- wrench (force, moment
-// about the origin) of the grid forces on the own atoms of fragment g, for every g (this initialises WR).
-// The kernel's code must stay inside the 32 KB instruction cache (B300_MICROARCH.md), so there is ONE copy of the
-// evaluation with a warp-uniform `grad` flag instead of two template instances.
+// Two 16-byte records of the xy-packed grid per atom.  The common case -- the atom lies inside the grid -- takes a short
+// path (u = x * inv_h - origin * inv_h by one FMA, floor, fraction, one unsigned range test per axis); an atom on or
+// beyond the boundary takes the general clamp of O5 and raises c.cl (bit i: axis i clamped), which sends the blend
+// through the wall terms (G8).
+struct LaneCell {
+    const float4* p;
+    float fx, fy, fz;
+    int cl;
+};
+struct LaneGridK { float nox, noy, noz; };        // -origin * inv_h
+__device__ __forceinline__ LaneCell lane_locate(const DGrid& G, const LaneGridK& Q, int type, float x, float y, float z) {
+    LaneCell c;
+    const float ux = fmaf(x, G.inv_h, Q.nox), uy = fmaf(y, G.inv_h, Q.noy), uz = fmaf(z, G.inv_h, Q.noz);
+    int ix = __float2int_rd(ux), iy = __float2int_rd(uy), iz = __float2int_rd(uz);
+    c.fx = ux - (float)ix; c.fy = uy - (float)iy; c.fz = uz - (float)iz;
+    c.cl = 0;
+    if ((unsigned)ix > (unsigned)(G.nx - 2) || (unsigned)iy > (unsigned)(G.ny - 2) || (unsigned)iz > (unsigned)(G.nz - 2)) {
+        const float vx = (x - G.ox) * G.inv_h, vy = (y - G.oy) * G.inv_h, vz = (z - G.oz) * G.inv_h;
+        const float cx = fminf(fmaxf(vx, 0.f), (float)(G.nx - 1));
+        const float cy = fminf(fmaxf(vy, 0.f), (float)(G.ny - 1));
+        const float cz = fminf(fmaxf(vz, 0.f), (float)(G.nz - 1));
+        ix = min((int)cx, G.nx - 2); iy = min((int)cy, G.ny - 2); iz = min((int)cz, G.nz - 2);
+        c.fx = cx - (float)ix; c.fy = cy - (float)iy; c.fz = cz - (float)iz;
+        c.cl = (cx != vx ? 1 : 0) | (cy != vy ? 2 : 0) | (cz != vz ? 4 : 0);
+    }
+    c.p = G.gp + (size_t)type * G.plane + ((size_t)iz * G.ny + iy) * G.nx + ix;
+    return c;
+}
+// value, and (grad, warp-uniform) the gradient in GRID units: the caller multiplies by inv_h
+__device__ __forceinline__ float lane_blend(const DGrid& G, float k_wall, const LaneCell& c, const float4 lo, const float4 hi, bool grad,
+                                            float x, float y, float z, float& gx, float& gy, float& gz) {
+    const float v000 = lo.x, v001 = lo.y, v010 = lo.z, v011 = lo.w, v100 = hi.x, v101 = hi.y, v110 = hi.z, v111 = hi.w;
+    const float d00 = v001 - v000, d01 = v011 - v010, d10 = v101 - v100, d11 = v111 - v110;
+    const float a00 = fmaf(c.fx, d00, v000), a01 = fmaf(c.fx, d01, v010), a10 = fmaf(c.fx, d10, v100), a11 = fmaf(c.fx, d11, v110);
+    const float e0 = a01 - a00, e1 = a11 - a10;
+    const float b0 = fmaf(c.fy, e0, a00), b1 = fmaf(c.fy, e1, a10);
+    float e = fmaf(c.fz, b1 - b0, b0);
+    if (grad) {
+        const float dx0 = fmaf(c.fy, d01 - d00, d00), dx1 = fmaf(c.fy, d11 - d10, d10);
+        gx = fmaf(c.fz, dx1 - dx0, dx0);
+        gy = fmaf(c.fz, e1 - e0, e0);
+        gz = b1 - b0;
+    }
+    if (c.cl) {                                   // rare: outside the grid -- clamped axes have no gradient, quadratic wall
+        const float vx = (x - G.ox) * G.inv_h, vy = (y - G.oy) * G.inv_h, vz = (z - G.oz) * G.inv_h;
+        const float cx = fminf(fmaxf(vx, 0.f), (float)(G.nx - 1));
+        const float cy = fminf(fmaxf(vy, 0.f), (float)(G.ny - 1));
+        const float cz = fminf(fmaxf(vz, 0.f), (float)(G.nz - 1));
+        const float wx = (c.cl & 1) ? x - (G.ox + cx * G.h) : 0.f;
+        const float wy = (c.cl & 2) ? y - (G.oy + cy * G.h) : 0.f;
+        const float wz = (c.cl & 4) ? z - (G.oz + cz * G.h) : 0.f;
+        e += k_wall * (wx * wx + wy * wy + wz * wz);
+        if (grad) {
+            const float kw = 2.f * k_wall * G.h;
+            gx = ((c.cl & 1) ? 0.f : gx) + kw * wx;
+            gy = ((c.cl & 2) ? 0.f : gy) + kw * wy;
+            gz = ((c.cl & 4) ? 0.f : gz) + kw * wz;
+        }
+    }
+    return e;
+}
+
+// All atoms of the ligand, two in flight, software-pipelined: while one atom is blended the other's cell is located
+// and its two records are on their way from L2 (the wait for them was 11 % of the kernel's time when a pair of atoms
+// was fetched and consumed together).  grad (warp-uniform): WR[g] <- wscale * wrench (force, moment about the origin)
+// of the grid forces on the own atoms of fragment g, for every g (this initialises WR); wscale = inv_h / kappa (the
+// reverse pass works in the pair terms' kappa units, lane_backward).
+// The kernel's code must stay small (instruction cache, B300_MICROARCH.md), so there is ONE copy of the evaluation with
+// a warp-uniform `grad` flag instead of two template instances.
 template <class XS>
-__device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, float k_wall, bool grad,
-                                           const XS& X, float* __restrict__ WR, int C) {
-    constexpr int GA = 2;                                        // atoms in flight
+__device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, float k_wall, bool grad, float wscale,
+                                           const XS& X, float* __restrict__ WR) {
+    constexpr int C = XS::kC;
+    const LaneGridK Q = {-G.ox * G.inv_h, -G.oy * G.inv_h, -G.oz * G.inv_h};
     float e_inter = 0.f;
     float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     int gcur = 0;
-    for (int a0 = 0; a0 < S.n; a0 += GA) {
-        float e[GA], gx[GA], gy[GA], gz[GA], x[GA], y[GA], z[GA];
-        int m[GA];
+    const int n = S.n;
+    auto consume = [&](int a, int m, const LaneCell& c, const float4 lo, const float4 hi, float x, float y, float z) {
+        float gx, gy, gz;
+        e_inter += lane_blend(G, k_wall, c, lo, hi, grad, x, y, z, gx, gy, gz);
+        if (grad) {
+            if ((m & 0x100) && a > 0) {            // first own atom of the next fragment: the previous one is complete
 #pragma unroll
-        for (int i = 0; i < GA; ++i) {
-            const int a = min(a0 + i, S.n - 1);               // the tail repeats the last atom (result unused)
-            m[i] = S.meta[a];
-            X.get(3 * a, x[i], y[i], z[i]);
-            X.fence(x[i], y[i], z[i]);
-            e[i] = grid_interp_packed<true>(G, k_wall, m[i] & 0xff, x[i], y[i], z[i], gx[i], gy[i], gz[i]);
-        }
-#pragma unroll
-        for (int i = 0; i < GA; ++i) {
-            if (a0 + i < S.n) {
-                e_inter += e[i];
-                if (grad) {
-                    if ((m[i] & 0x100) && a0 + i > 0) {
-#pragma unroll
-                        for (int c = 0; c < 6; ++c) { WR[(6 * gcur + c) * C] = acc[c]; acc[c] = 0.f; }
-                    }
-                    gcur = m[i] >> 16;
-                    acc[0] += gx[i]; acc[1] += gy[i]; acc[2] += gz[i];
-                    acc[3] += y[i] * gz[i] - z[i] * gy[i];
-                    acc[4] += z[i] * gx[i] - x[i] * gz[i];
-                    acc[5] += x[i] * gy[i] - y[i] * gx[i];
-                }
+                for (int k = 0; k < 6; ++k) { WR[(6 * gcur + k) * C] = acc[k] * wscale; acc[k] = 0.f; }
             }
+            gcur = m >> 16;
+            acc[0] += gx; acc[1] += gy; acc[2] += gz;
+            acc[3] += y * gz - z * gy;
+            acc[4] += z * gx - x * gz;
+            acc[5] += x * gy - y * gx;
         }
+    };
+    float xa, ya, za, xb, yb, zb;
+    int ma, mb;
+    LaneCell ca, cb;
+    float4 la, ha, lb, hb;
+    const size_t zs = (size_t)G.nx * G.ny;
+    ma = S.meta[0];
+    X.get(0u, xa, ya, za);
+    X.fence(xa, ya, za);
+    ca = lane_locate(G, Q, ma & 0xff, xa, ya, za);
+    la = __ldg(ca.p); ha = __ldg(ca.p + zs);
+    for (int a0 = 0; a0 < n; a0 += 2) {
+        const int a1 = min(a0 + 1, n - 1), a2 = min(a0 + 2, n - 1);     // the tail repeats the last atom (result unused)
+        mb = S.meta[a1];
+        X.get(XS::kScale * (uint32_t)a1, xb, yb, zb);
+        X.fence(xb, yb, zb);
+        cb = lane_locate(G, Q, mb & 0xff, xb, yb, zb);
+        lb = __ldg(cb.p); hb = __ldg(cb.p + zs);
+        consume(a0, ma, ca, la, ha, xa, ya, za);
+        ma = S.meta[a2];
+        X.get(XS::kScale * (uint32_t)a2, xa, ya, za);
+        X.fence(xa, ya, za);
+        ca = lane_locate(G, Q, ma & 0xff, xa, ya, za);
+        la = __ldg(ca.p); ha = __ldg(ca.p + zs);
+        if (a0 + 1 < n) consume(a0 + 1, mb, cb, lb, hb, xb, yb, zb);
     }
     if (grad) {
 #pragma unroll
-        for (int c = 0; c < 6; ++c) WR[(6 * gcur + c) * C] = acc[c];
+        for (int k = 0; k < 6; ++k) WR[(6 * gcur + k) * C] = acc[k] * wscale;
     }
     return e_inter;
 }
 
 // ------------------------------------------------------------------ a5 intra-ligand pairs (O2, O6)
 // One record: partner atom b against the 4 slots of a tile, branch-free so that the four evaluations interleave.
-//   L = -[d<dmax] exp(-(d-dvdw-mu)^2/(2 sigma^2))  (G1):  eL += [d<dmax] 2^(nk2 (d-c)^2),  c = dvdw + mu
-//   C = -[d<dc] ln(max(d,floor)/dc)                (G3, G4):  eC += lg2(max(dc / max(d,floor), 1)),
-//       dc = c - mu, or hb_dclash for a donor/acceptor pair
+//   L = -[d<dmax] exp(-(d-dvdw-mu)^2/(2 sigma^2))  (G1):  eL += [d<dmax] 2^(nk2 t^2),  t = d - c,  c = dvdw + mu
+//   C = -[d<dc] ln(max(d,floor)/dc)                (G3, G4):  eC += lg2 of the PRODUCT over the 4 slots of
+//       max(dc / max(d,floor), 1) (one lg2 per record; the product is at most (dc/floor)^4),  dc = c - mu, or hb_dclash for
+//       a donor/acceptor pair.  The force needs no dc: d < dc is t < -mu (t < hb_dclash - c for a donor/acceptor pair).
 //   H = -[hb, d<3.4] exp(-(d-2.88)^2/(2*0.3^2)):  eH += ..., only in records that hold such a pair
 // GRAD: f_i += s (x_a - x_b) with s = (de/dd) / d / kappa.  A slot without a pair has c = -1e15 and adds 0.
+// The 1e-12 inside the squared distance keeps rsqrt finite for coincident atoms (it moves d by < 1e-12 / 2d).
 template <bool GRAD, bool ENERGY>
 __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], const float ay[4], const float az[4],
                                          float bx, float by, float bz, const float4 c4, unsigned hbmask,
                                          float& eL, float& eC, float& eH, float fx[4], float fy[4], float fz[4]) {
     const float c[4] = {c4.x, c4.y, c4.z, c4.w};
-    float dc[4] = {c4.x - K.mu, c4.y - K.mu, c4.z - K.mu, c4.w - K.mu};   // clash distance dvdw (negative: no pair)
+    float thr[4] = {K.neg_mu, K.neg_mu, K.neg_mu, K.neg_mu};            // clash range in terms of t = d - c
+    float dc[4];
+    if (ENERGY) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) dc[i] = c[i] - K.mu;                 // clash distance dvdw (negative: no pair)
+    }
     if (hbmask) {                                                    // warp-uniform; about one record in three
 #pragma unroll
-        for (int i = 0; i < 4; ++i) dc[i] = ((hbmask >> i) & 1u) ? K.hb_dclash : dc[i];
+        for (int i = 0; i < 4; ++i) {
+            if (GRAD) thr[i] = ((hbmask >> i) & 1u) ? K.hb_dclash - c[i] : thr[i];
+            if (ENERGY) dc[i] = ((hbmask >> i) & 1u) ? K.hb_dclash : dc[i];
+        }
     }
-    float dx[4], dy[4], dz[4], d[4], rinv[4], s[4];
+    float dx[4], dy[4], dz[4], d[4], rinv[4], s[4], q[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         dx[i] = ax[i] - bx; dy[i] = ay[i] - by; dz[i] = az[i] - bz;
-        const float d2 = fmaxf(fmaf(dx[i], dx[i], fmaf(dy[i], dy[i], dz[i] * dz[i])), 1e-12f);
+        const float d2 = fmaf(dx[i], dx[i], fmaf(dy[i], dy[i], fmaf(dz[i], dz[i], 1e-12f)));
         rinv[i] = rsqrt_approx(d2);
         d[i] = d2 * rinv[i];
         const float t = d[i] - c[i];
         const float u = t * K.nk2;
         float g = ex2_approx(u * t);
         g = d[i] < K.dmax ? g : 0.f;
-        const float q = dc[i] * fminf(rinv[i], K.inv_floor);         // dc / max(d, floor); > 1 inside the clash range
-        if (ENERGY) { eL += g; eC += lg2_approx(fmaxf(q, 1.f)); }
+        if (ENERGY) {
+            eL += g;
+            q[i] = fmaxf(dc[i] * fminf(rinv[i], K.inv_floor), 1.f);     // dc / max(d, floor); > 1 inside the clash range
+        }
         if (GRAD) {
             s[i] = u * g * rinv[i];
-            if (q > 1.f && rinv[i] < K.inv_floor) s[i] = fmaf(-K.kc * rinv[i], rinv[i], s[i]);
+            if (t < thr[i] && rinv[i] < K.inv_floor) s[i] = fmaf(-K.kc * rinv[i], rinv[i], s[i]);
         }
     }
+    if (ENERGY) eC += lg2_approx((q[0] * q[1]) * (q[2] * q[3]));
     if (hbmask) {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -264,41 +368,44 @@ __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], cons
     }
 }
 
-// One tile: w <= 4 consecutive own atoms a0 .. a0+w-1 of fragment g against n_runs runs of partner atoms; hp / rp walk
-// the header units / the two record arrays.  GRAD: acc += the wrench the tile's atoms receive; WR[fb] -= each run's wrench.
+// The record stream is read one record ahead, across run, tile and fragment boundaries: `mt` / (bx, by, bz) always hold
+// the NEXT record's word and its partner's coordinates (a dependent load), so no run starts with an exposed load.
+struct PairCursor {
+    const uint4* hp;        // header units
+    const float4* rc;       // record c[4]
+    const uint32_t* rm;     // record words; rm[0] is the record in `mt`
+    uint32_t mt;
+    float bx, by, bz;
+};
+
+// One tile: w <= 4 consecutive own atoms a0 .. a0+w-1 of fragment g against n_runs runs of partner atoms.
+// GRAD: acc += the wrench the tile's atoms receive; WR[fb] -= each run's wrench (kappa units).
 template <bool GRAD, bool ENERGY, class XS>
-__device__ __forceinline__ void lane_tile(const uint4*& hp, const float4*& rc, const uint32_t*& rm, int a0, int w, int n_runs, const PairK& K,
-                                          const XS& X, float* __restrict__ WR, int C,
+__device__ __forceinline__ void lane_tile(PairCursor& pc, int a0, int w, int n_runs, const PairK& K,
+                                          const XS& X, float* __restrict__ WR,
                                           float acc[6], float& eL, float& eC, float& eH) {
+    constexpr int C = XS::kC;
     float ax[4], ay[4], az[4];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) X.get(3 * (a0 + (i < w ? i : 0)), ax[i], ay[i], az[i]);
+    for (int i = 0; i < 4; ++i) X.get(XS::kScale * (uint32_t)(a0 + (i < w ? i : 0)), ax[i], ay[i], az[i]);
 #pragma unroll
     for (int i = 0; i < 4; ++i) X.fence(ax[i], ay[i], az[i]);
     for (int run = 0; run < n_runs; ++run) {
-        const uint4 rh = *hp++;
-        const int fb = (int)rh.x, nb = (int)rh.y;
+        const uint4 rh = *pc.hp++;
+        const int fb = (int)rh.x;
+        const uint32_t* const rend = pc.rm + rh.y;
         float fx[4], fy[4], fz[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) fx[i] = fy[i] = fz[i] = 0.f;
-        // software pipeline: the next record (and its partner's coordinates, a dependent load) is fetched while the
-        // current one is evaluated
-        float4 c4 = rc[0];
-        uint32_t mt = rm[0];
-        float bx, by, bz;
-        X.get((int)(mt & 0xffffu), bx, by, bz);
-        for (int j = 0; j < nb; ++j) {
-            const int jn = min(j + 1, nb - 1);
-            const float4 c4n = rc[jn];
-            const uint32_t mtn = rm[jn];
+        do {
+            const float4 c4 = *pc.rc++;
+            const uint32_t mtn = *++pc.rm;
             float nx, ny, nz;
-            X.fence(bx, by, bz);
-            X.get((int)(mtn & 0xffffu), nx, ny, nz);
-            lane_rec<GRAD, ENERGY>(K, ax, ay, az, bx, by, bz, c4, mt >> 16, eL, eC, eH, fx, fy, fz);
-            c4 = c4n; mt = mtn; bx = nx; by = ny; bz = nz;
-        }
-        X.fence(bx, by, bz);
-        rc += nb; rm += nb;
+            X.fence(pc.bx, pc.by, pc.bz);
+            X.get(mtn & 0xffffu, nx, ny, nz);
+            lane_rec<GRAD, ENERGY>(K, ax, ay, az, pc.bx, pc.by, pc.bz, c4, pc.mt >> 16, eL, eC, eH, fx, fy, fz);
+            pc.mt = mtn; pc.bx = nx; pc.by = ny; pc.bz = nz;
+        } while (pc.rm != rend);
         if (GRAD) {
             float wv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -310,60 +417,63 @@ __device__ __forceinline__ void lane_tile(const uint4*& hp, const float4*& rc, c
             }
             float* wb = WR + 6 * fb * C;
 #pragma unroll
-            for (int c = 0; c < 6; ++c) {
-                const float v = K.kappa * wv[c];
-                acc[c] += v;
-                wb[c * C] -= v;
+            for (int k = 0; k < 6; ++k) {
+                acc[k] += wv[k];
+                wb[k * C] -= wv[k];
             }
         }
     }
 }
 
-// All pairs of the ligand.  GRAD: WR[g] (initialised by lane_grid) += the pair wrenches.
+// All pairs of the ligand.  GRAD: WR[g] (initialised by lane_grid, kappa units) += the pair wrenches.
 template <bool GRAD, bool ENERGY, class XS>
-__device__ __forceinline__ float lane_pairs(const LaneTopo& S, const PairK& K, const XS& X, float* __restrict__ WR, int C) {
+__device__ __forceinline__ float lane_pairs(const LaneTopo& S, const PairK& K, const XS& X, float* __restrict__ WR) {
+    constexpr int C = XS::kC;
     float eL = 0.f, eC = 0.f, eH = 0.f;
-    const uint4* hp = S.stream;
-    const float4* rc = S.rec_c;
-    const uint32_t* rm = S.rec_m;
+    PairCursor pc;
+    pc.hp = S.stream; pc.rc = S.rec_c; pc.rm = S.rec_m;
+    pc.mt = pc.rm[0];                                               // the first record (the pad record if there is none)
+    X.get(pc.mt & 0xffffu, pc.bx, pc.by, pc.bz);
     for (int g = 0; g <= S.T; ++g) {
-        const int n_tiles = (int)(*hp++).x;
+        const int n_tiles = (int)(*pc.hp++).x;
         if (n_tiles == 0) continue;
         float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         for (int tl = 0; tl < n_tiles; ++tl) {
-            const uint4 h = *hp++;
-            lane_tile<GRAD, ENERGY, XS>(hp, rc, rm, (int)h.x, (int)h.y, (int)h.z, K, X, WR, C, acc, eL, eC, eH);
+            const uint4 h = *pc.hp++;
+            lane_tile<GRAD, ENERGY, XS>(pc, (int)h.x, (int)h.y, (int)h.z, K, X, WR, acc, eL, eC, eH);
         }
         if (GRAD) {
             float* wg = WR + 6 * g * C;
 #pragma unroll
-            for (int c = 0; c < 6; ++c) wg[c * C] += acc[c];
+            for (int k = 0; k < 6; ++k) wg[k * C] += acc[k];
         }
     }
+    X.fence(pc.bx, pc.by, pc.bz);                                   // the pad record's load is still in flight
     return fmaf(K.w_clash_ln2, eC, -fmaf(K.w_long, eL, K.w_hbond * eH));
 }
 
 // ------------------------------------------------------------------ a3..a5: one pose evaluation by one lane
 // In : t[3], unit q[4] (registers), th[(g-1)*C] torsion angles (shared), grad (warp-uniform).
 // Out: X (world coordinates), e_inter, e_intra (e_intra of a gradient evaluation only if GE); grad: WR[g] = wrench on the
-//      own atoms of fragment g.
+//      own atoms of fragment g in kappa units (1 / K.kappa of the true wrench).
 template <bool GE, class XS>
 __device__ __forceinline__ void lane_eval(const LaneTopo& S, const DGrid& G, const DParams& P, const PairK& K, bool grad,
                                           const float t[3], const float q[4], const float* __restrict__ th,
-                                          const XS& X, float* __restrict__ WR, int C, float& e_inter, float& e_intra) {
-    lane_fk(S, t, q, th, X, WR, C);
-    e_inter = lane_grid(S, G, P.k_wall, grad, X, WR, C);
-    e_intra = grad ? lane_pairs<true, GE, XS>(S, K, X, WR, C) : lane_pairs<false, true, XS>(S, K, X, WR, C);
+                                          const XS& X, float* __restrict__ WR, float& e_inter, float& e_intra) {
+    lane_fk(S, t, q, th, X, WR);
+    e_inter = lane_grid(S, G, P.k_wall, grad, G.inv_h * K.inv_kappa, X, WR);
+    e_intra = grad ? lane_pairs<true, GE, XS>(S, K, X, WR) : lane_pairs<false, true, XS>(S, K, X, WR);
 }
 
 // ------------------------------------------------------------------ a6 reverse mode through the tree (O9)
 // Fragments in reverse pre-order: when g is visited WR[g] already holds the wrench of its whole subtree; its torsion
 // gradient is u_g . (M - x_b x F) with the axis taken from the world coordinates of its two axis atoms, and the
-// wrench moves on to the parent.  `sink(g, dE/dtheta)` consumes the torsion gradients; on return g6 = {dE/dt,
-// dE/domega about t}.
+// wrench moves on to the parent.  WR is in kappa units: `sink(g, dE/dtheta)` and g6 = {dE/dt, dE/domega about t} are
+// multiplied by kappa on the way out.
 template <class XS, class Sink>
 __device__ __forceinline__ void lane_backward(const LaneTopo& S, const float t[3], const XS& X,
-                                              float* __restrict__ WR, int C, float g6[6], Sink sink) {
+                                              float* __restrict__ WR, float kappa, float g6[6], Sink sink) {
+    constexpr int C = XS::kC;
     for (int g = S.T; g >= 1; --g) {
         const LaneFrag& r = S.frag[g];
         float w[6];
@@ -372,18 +482,18 @@ __device__ __forceinline__ void lane_backward(const LaneTopo& S, const float t[3
 #pragma unroll
         for (int c = 0; c < 6; ++c) { w[c] = wg[c * C]; wp[c * C] += w[c]; }
         float ax, ay, az, ox, oy, oz;
-        X.get(3 * (r.axis & 0xff), ax, ay, az);
-        X.get(3 * ((r.axis >> 8) & 0xff), ox, oy, oz);
+        X.get(XS::kScale * (uint32_t)(r.axis & 0xff), ax, ay, az);
+        X.get(XS::kScale * (uint32_t)((r.axis >> 8) & 0xff), ox, oy, oz);
         X.fence(ax, ay, az); X.fence(ox, oy, oz);
         float ux = ox - ax, uy = oy - ay, uz = oz - az;
-        const float un = rsqrtf(ux * ux + uy * uy + uz * uz);
+        const float un = rsqrtf(ux * ux + uy * uy + uz * uz) * kappa;
         const float mx = w[3] - (oy * w[2] - oz * w[1]);
         const float my = w[4] - (oz * w[0] - ox * w[2]);
         const float mz = w[5] - (ox * w[1] - oy * w[0]);
         sink(g, (ux * mx + uy * my + uz * mz) * un);
     }
 #pragma unroll
-    for (int c = 0; c < 6; ++c) g6[c] = WR[c * C];
+    for (int c = 0; c < 6; ++c) g6[c] = WR[c * C] * kappa;
     const float fx = g6[0], fy = g6[1], fz = g6[2];
     g6[3] -= t[1] * fz - t[2] * fy;
     g6[4] -= t[2] * fx - t[0] * fz;
@@ -396,7 +506,8 @@ __device__ __forceinline__ void lane_backward(const LaneTopo& S, const float t[3
 template <class XS>
 __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S, int lig, int chain, bool live, int max_depth,
                                            const XS& X, float* __restrict__ WR, float* __restrict__ THC, float* __restrict__ THP,
-                                           float* __restrict__ MV, int C) {
+                                           float* __restrict__ MV) {
+    constexpr int C = XS::kC;
     const DParams& P = a.P;
     const PairK K = make_pairk(P);
     const int T = S.T;
@@ -476,7 +587,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
         for (int rf = (s >= 0 ? 0 : P.n_refine); rf <= P.n_refine; ++rf) {
             const bool grad = rf < P.n_refine;
             float ei, ea;
-            lane_eval<false>(S, a.grid, P, K, grad, pt, pq, THP, X, WR, C, ei, ea);   // the Adam steps need no energy
+            lane_eval<false>(S, a.grid, P, K, grad, pt, pq, THP, X, WR, ei, ea);   // the Adam steps need no energy
             enew = ei + ea;
             if (!grad) break;
             b1p *= P.adam_b1; b2p *= P.adam_b2;
@@ -484,7 +595,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
             // far inside the tolerance, and the IEEE forms are slow-path subroutines on the chain's critical path
             const bool keep = rf + 1 < P.n_refine;
             float g6[6];
-            lane_backward(S, pt, X, WR, C, g6, [&](int g, float gk) {      // torsion gradients are consumed as produced
+            lane_backward(S, pt, X, WR, K.kappa, g6, [&](int g, float gk) {   // torsion gradients are consumed as produced
                 float mk = 0.f, vk = 0.f;
                 if (rf > 0) { mk = MV[2 * (g - 1) * C]; vk = MV[(2 * (g - 1) + 1) * C]; }
                 mk = P.adam_b1 * mk + (1.f - P.adam_b1) * gk;
@@ -549,32 +660,33 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
 }
 
 // ------------------------------------------------------------------ the fused MC kernel, one lane per chain
-// Coordinates in shared memory: one CTA = up to 128 chains of ONE ligand (any ligand size that fits).
+// Coordinates in shared memory: one CTA = C = 32, 64, 96 or 128 chains of ONE ligand (any ligand size that fits); C is a
+// template parameter so that every slot offset of the chain's shared-memory state is an immediate.
 // MINB = resident 128-thread CTAs per SM the register budget must allow (3: 168 registers, 2: 255): the host picks 255 for
 // the size buckets whose shared-memory need keeps at most 8 warps per SM resident anyway, 168 (12 warps) for the rest --
 // measured: 12 warps at 168 registers beat 16 warps at 128 (C5 1885 -> 1824 ms), 8 warps at 255 do not (1917 ms).
-template <int MINB>
+template <int MINB, int C>
 __global__ void __launch_bounds__(128, MINB) mc_lane_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char lane_smem[];
-    const int C = blockDim.x, tid = threadIdx.x;
+    const int tid = threadIdx.x;
     const int cpl = (a.n_chains + C - 1) / C;                 // CTAs per ligand
     const int lig = a.lig_list[blockIdx.x / cpl];
     const int chain = (blockIdx.x % cpl) * C + tid;
     const LigHdr* h = a.hdr + lig;
     LaneTopo S;
-    unsigned char* after = lane_stage(S, lane_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.lane_stream, a.lane_recs, a.P, tid, C);
+    unsigned char* after = lane_stage(S, lane_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.lane_stream, a.lane_recs, a.P, tid, C,
+                                      XShared<C>::kScale);
     const int max_depth = h->max_depth;
     __syncthreads();
     if (chain >= a.n_chains) return;
     const int n = S.n, T = S.T;
-    XShared X;
+    XShared<C> X;
     X.X = reinterpret_cast<float*>(after) + tid;              // slot-major: slot i of this chain is X[i * C]
-    X.C = C;
     float* WR = X.X + 3 * n * C;                              // frames (forward) / wrenches (reverse)
     float* THC = WR + lane_wslots(T, max_depth) * C;          // current accepted torsions, by pre-order fragment g - 1
     float* THP = THC + T * C;                                 // proposal
     float* MV = THP + T * C;                                  // torsion Adam moments {m, v} (n_refine > 1 only)
-    lane_chain(a, S, lig, chain, true, max_depth, X, WR, THC, THP, MV, C);
+    lane_chain(a, S, lig, chain, true, max_depth, X, WR, THC, THP, MV);
 }
 
 // Coordinates in tensor memory: one CTA = 4 warps, every WARP takes its own work item (ligand, block of 32 chains) and
@@ -582,7 +694,8 @@ __global__ void __launch_bounds__(128, MINB) mc_lane_kernel(const McLaunch a) {
 __global__ void __launch_bounds__(128, 3) mc_lane_tm_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char lane_smem[];
     __shared__ uint32_t tm_base;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, C = 32;
+    constexpr int C = 32;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (warp == 0) {                                          // one warp allocates the CTA's columns
         const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&tm_base);
         if (a.tm_cols == 32) asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 32;" :: "r"(dst) : "memory");
@@ -600,7 +713,7 @@ __global__ void __launch_bounds__(128, 3) mc_lane_tm_kernel(const McLaunch a) {
     const LigHdr* h = a.hdr + lig;
     LaneTopo S;
     unsigned char* after = lane_stage(S, lane_smem + (size_t)warp * a.lane_region, h, a.atom_f4, a.atom_i, a.lane_frags, a.lane_stream,
-                                      a.lane_recs, a.P, lane, 32);
+                                      a.lane_recs, a.P, lane, 32, XTensor::kScale);
     const int max_depth = h->max_depth;
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -613,7 +726,7 @@ __global__ void __launch_bounds__(128, 3) mc_lane_tm_kernel(const McLaunch a) {
         float* THC = WR + lane_wslots(T, max_depth) * C;
         float* THP = THC + T * C;
         float* MV = THP + T * C;
-        lane_chain(a, S, lig, chain, live, max_depth, X, WR, THC, THP, MV, C);
+        lane_chain(a, S, lig, chain, live, max_depth, X, WR, THC, THP, MV);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -624,32 +737,47 @@ __global__ void __launch_bounds__(128, 3) mc_lane_tm_kernel(const McLaunch a) {
     }
 }
 
-static bool g_lane_prepared = false;
 __global__ void score_lane_kernel(const ScoreLaunch a);
 
-cudaError_t mc_lane_prepare(size_t max_smem_bytes) {
-    if (g_lane_prepared) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(mc_lane_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<3>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(score_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
+// Opt-in shared-memory sizes are per device and per function: done once per device (tridsk_create -> mc_lane_prepare).
+template <int MINB, int C>
+static cudaError_t lane_prepare_one(size_t max_smem_bytes) {
+    cudaError_t e = cudaFuncSetAttribute(mc_lane_kernel<MINB, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
     // residency is bound by shared memory (the chains' coordinates): take the whole 228 KB, the grid gathers live in L2 anyway
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<MINB, C>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    return e;
+}
+cudaError_t mc_lane_prepare(size_t max_smem_bytes) {
+    cudaError_t e = lane_prepare_one<3, 32>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<3, 64>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<3, 96>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<3, 128>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 32>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 64>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 96>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 128>(max_smem_bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(score_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_tm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes - 1024);   // it has 16 static bytes
     if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_tm_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e == cudaSuccess) g_lane_prepared = true;
     return e;
 }
 
+template <int MINB>
+static void lane_launch_c(cudaStream_t s, const McLaunch& a, unsigned blocks, int c, size_t smem_bytes) {
+    switch (c) {
+        case 32: mc_lane_kernel<MINB, 32><<<blocks, 32, smem_bytes, s>>>(a); break;
+        case 64: mc_lane_kernel<MINB, 64><<<blocks, 64, smem_bytes, s>>>(a); break;
+        case 96: mc_lane_kernel<MINB, 96><<<blocks, 96, smem_bytes, s>>>(a); break;
+        default: mc_lane_kernel<MINB, 128><<<blocks, 128, smem_bytes, s>>>(a); break;
+    }
+}
 cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta, size_t smem_bytes, int minb) {
     const int cpl = (a.n_chains + chains_per_cta - 1) / chains_per_cta;
     const long long blocks = (long long)a.n_list * cpl;
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL || chains_per_cta < 32 || chains_per_cta > 128 || (chains_per_cta & 31)) return cudaErrorInvalidValue;
-    cudaError_t e = mc_lane_prepare(TRIDSK_SMEM_MAX_CTA);
-    if (e != cudaSuccess) return e;
-    if (minb == 2) mc_lane_kernel<2><<<(unsigned)blocks, chains_per_cta, smem_bytes, s>>>(a);
-    else mc_lane_kernel<3><<<(unsigned)blocks, chains_per_cta, smem_bytes, s>>>(a);
+    if (minb == 2) lane_launch_c<2>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);
+    else lane_launch_c<3>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);
     return cudaGetLastError();
 }
 
@@ -658,8 +786,6 @@ cudaError_t launch_mc_lane_tm(cudaStream_t s, const McLaunch& a) {
     const long long items = (long long)a.n_list * wpl, blocks = (items + 3) / 4;
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL || (a.tm_cols != 32 && a.tm_cols != 64 && a.tm_cols != 128) || a.lane_region % 16) return cudaErrorInvalidValue;
-    cudaError_t e = mc_lane_prepare(TRIDSK_SMEM_MAX_CTA);
-    if (e != cudaSuccess) return e;
     mc_lane_tm_kernel<<<(unsigned)blocks, 128, 4 * (size_t)a.lane_region, s>>>(a);
     return cudaGetLastError();
 }
@@ -668,19 +794,20 @@ cudaError_t launch_mc_lane_tm(cudaStream_t s, const McLaunch& a) {
 // One 32-thread CTA takes up to 32 poses of one ligand (the host groups poses by ligand: seg_*, perm).
 __global__ void __launch_bounds__(32) score_lane_kernel(const ScoreLaunch a) {
     extern __shared__ __align__(16) unsigned char lane_smem[];
-    const int C = 32, tid = threadIdx.x;
+    constexpr int C = 32;
+    const int tid = threadIdx.x;
     const int lig = a.seg_lig[blockIdx.x];
     const LigHdr* h = a.hdr + lig;
     LaneTopo S;
-    unsigned char* after = lane_stage(S, lane_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.lane_stream, a.lane_recs, a.P, tid, 32);
+    unsigned char* after = lane_stage(S, lane_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.lane_stream, a.lane_recs, a.P, tid, 32,
+                                      XShared<32>::kScale);
     __syncthreads();
     if (tid >= a.seg_cnt[blockIdx.x]) return;
     const int i = a.perm[a.seg_start[blockIdx.x] + tid];
     const int n = S.n, T = S.T;
     const PairK K = make_pairk(a.P);
-    XShared X;
+    XShared<32> X;
     X.X = reinterpret_cast<float*>(after) + tid;
-    X.C = C;
     float* WR = X.X + 3 * n * C;
     float* TH = WR + lane_wslots(T, h->max_depth) * C;
     const float* src = a.poses + (size_t)i * a.pose_stride;
@@ -688,13 +815,13 @@ __global__ void __launch_bounds__(32) score_lane_kernel(const ScoreLaunch a) {
     quat_normalise(q);
     for (int g = 1; g <= T; ++g) TH[(g - 1) * C] = src[7 + S.frag[g].tor];
     float ei, ea;
-    lane_eval<true>(S, a.grid, a.P, K, a.grad != nullptr, t, q, TH, X, WR, C, ei, ea);
+    lane_eval<true>(S, a.grid, a.P, K, a.grad != nullptr, t, q, TH, X, WR, ei, ea);
     a.energy[3 * (size_t)i] = ei + ea; a.energy[3 * (size_t)i + 1] = ei; a.energy[3 * (size_t)i + 2] = ea;
     if (a.grad != nullptr) {
         float* gr = a.grad + (size_t)i * a.grad_stride;
         for (int e = 6; e < a.grad_stride; ++e) gr[e] = 0.f;
         float g6[6];
-        lane_backward(S, t, X, WR, C, g6, [&](int g, float gk) { gr[6 + S.frag[g].tor] = gk; });
+        lane_backward(S, t, X, WR, K.kappa, g6, [&](int g, float gk) { gr[6 + S.frag[g].tor] = gk; });
 #pragma unroll
         for (int c = 0; c < 6; ++c) gr[c] = g6[c];
     }
@@ -710,8 +837,6 @@ __global__ void __launch_bounds__(32) score_lane_kernel(const ScoreLaunch a) {
 
 cudaError_t launch_score_lane(cudaStream_t s, const ScoreLaunch& a, int n_seg, size_t smem_bytes) {
     if (n_seg <= 0) return cudaSuccess;
-    cudaError_t e = mc_lane_prepare(TRIDSK_SMEM_MAX_CTA);
-    if (e != cudaSuccess) return e;
     score_lane_kernel<<<n_seg, 32, smem_bytes, s>>>(a);
     return cudaGetLastError();
 }

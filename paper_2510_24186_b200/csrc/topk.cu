@@ -185,16 +185,15 @@ size_t topk_cluster_smem(int top_k, int max_atoms, int max_tor) {
     return sizeof(float) * 3 * (size_t)max_atoms * ((size_t)top_k + 1);
 }
 
+// per device (function attributes are per device): called by tridsk_create
+cudaError_t topk_prepare() {
+    return cudaFuncSetAttribute(topk_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA - 2048);
+}
+
 cudaError_t launch_topk(cudaStream_t s, const TopkLaunch& a) {
     if (a.n_lig <= 0 || a.top_k <= 0) return cudaSuccess;
     if (a.cluster_rmsd > 0.f) {
         const size_t smem = topk_cluster_smem(a.top_k, a.max_atoms, a.max_tor);
-        static bool prepared = false;
-        if (!prepared) {
-            cudaError_t e = cudaFuncSetAttribute(topk_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA - 2048);
-            if (e != cudaSuccess) return e;
-            prepared = true;
-        }
         if (smem > TRIDSK_SMEM_MAX_CTA - 2048) return cudaErrorInvalidValue;
         topk_cluster_kernel<<<a.n_lig, TOPK_THREADS, smem, s>>>(a);
     } else {
