@@ -78,7 +78,7 @@ struct PairK {
     float inv_floor;        // 1 / d_floor
     float kh;               // hydrogen-bond gradient in kappa units: 2 w_hbond / (2 sigma_hb^2) / kappa
     float w_long, w_clash_ln2, w_hbond, hb_dmax, hb_mu, hb_nk2;
-    float neg_mu, inv_kappa;
+    float neg_mu, inv_kappa, nkc;   // nkc = -kc
 };
 __device__ __forceinline__ PairK make_pairk(const DParams& P) {
     PairK K;
@@ -92,7 +92,7 @@ __device__ __forceinline__ PairK make_pairk(const DParams& P) {
     K.kh = 2.f * P.w_hbond * P.hb_inv_two_sigma2 / K.kappa;
     K.w_long = P.w_long; K.w_clash_ln2 = P.w_clash * 0.6931471805599453f; K.w_hbond = P.w_hbond;
     K.hb_dmax = P.hb_dmax; K.hb_mu = P.hb_mu; K.hb_nk2 = -P.hb_inv_two_sigma2 * L2E;
-    K.neg_mu = -P.long_mu; K.inv_kappa = 1.f / K.kappa;
+    K.neg_mu = -P.long_mu; K.inv_kappa = 1.f / K.kappa; K.nkc = -K.kc;
     return K;
 }
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }

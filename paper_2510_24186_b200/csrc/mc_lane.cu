@@ -239,13 +239,17 @@ __device__ __forceinline__ float lane_blend(const DGrid& G, float k_wall, const 
     return e;
 }
 
-// All atoms of the ligand, two in flight, software-pipelined: while one atom is blended the other's cell is located
-// and its two records are on their way from L2 (the wait for them was 11 % of the kernel's time when a pair of atoms
-// was fetched and consumed together).  grad (warp-uniform): WR[g] <- wscale * wrench (force, moment about the origin)
-// of the grid forces on the own atoms of fragment g, for every g (this initialises WR); wscale = inv_h / kappa (the
-// reverse pass works in the pair terms' kappa units, lane_backward).
+// All atoms of the ligand, software-pipelined LANE_GD deep: an atom's cell is located and its two records are requested
+// LANE_GD - 1 atoms before it is blended, so that the L2 round trip (the wait for it was 11-15 % of the kernel's time
+// when an atom was consumed one blend after its request) is covered by the blends of the atoms before it.
+// grad (warp-uniform): WR[g] <- wscale * wrench (force, moment about the origin) of the grid forces on the own atoms
+// of fragment g, for every g (this initialises WR); wscale = inv_h / kappa (the reverse pass works in the pair terms'
+// kappa units, lane_backward).
 // The kernel's code must stay small (instruction cache, B300_MICROARCH.md), so there is ONE copy of the evaluation with
 // a warp-uniform `grad` flag instead of two template instances.
+#ifndef LANE_GD
+#define LANE_GD 2     // measured on C5: 2 in flight 225 ms, 3: 238 ms, 4: 245 ms (8,192 ligands) -- the unrolled copies cost more
+#endif                // instruction-cache misses than the deeper prefetch saves
 template <class XS>
 __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, float k_wall, bool grad, float wscale,
                                            const XS& X, float* __restrict__ WR) {
@@ -255,49 +259,53 @@ __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, fl
     float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     int gcur = 0;
     const int n = S.n;
-    auto consume = [&](int a, int m, const LaneCell& c, const float4 lo, const float4 hi, float x, float y, float z) {
-        float gx, gy, gz;
-        e_inter += lane_blend(G, k_wall, c, lo, hi, grad, x, y, z, gx, gy, gz);
-        if (grad) {
-            if ((m & 0x100) && a > 0) {            // first own atom of the next fragment: the previous one is complete
-#pragma unroll
-                for (int k = 0; k < 6; ++k) { WR[(6 * gcur + k) * C] = acc[k] * wscale; acc[k] = 0.f; }
-            }
-            gcur = m >> 16;
-            acc[0] += gx; acc[1] += gy; acc[2] += gz;
-            acc[3] += y * gz - z * gy;
-            acc[4] += z * gx - x * gz;
-            acc[5] += x * gy - y * gx;
-        }
-    };
-    float xa, ya, za, xb, yb, zb;
-    int ma, mb;
-    LaneCell ca, cb;
-    float4 la, ha, lb, hb;
     const size_t zs = (size_t)G.nx * G.ny;
-    ma = S.meta[0];
-    X.get(0u, xa, ya, za);
-    X.fence(xa, ya, za);
-    ca = lane_locate(G, Q, ma & 0xff, xa, ya, za);
-    la = __ldg(ca.p); ha = __ldg(ca.p + zs);
-    for (int a0 = 0; a0 < n; a0 += 2) {
-        const int a1 = min(a0 + 1, n - 1), a2 = min(a0 + 2, n - 1);     // the tail repeats the last atom (result unused)
-        mb = S.meta[a1];
-        X.get(XS::kScale * (uint32_t)a1, xb, yb, zb);
-        X.fence(xb, yb, zb);
-        cb = lane_locate(G, Q, mb & 0xff, xb, yb, zb);
-        lb = __ldg(cb.p); hb = __ldg(cb.p + zs);
-        consume(a0, ma, ca, la, ha, xa, ya, za);
-        ma = S.meta[a2];
-        X.get(XS::kScale * (uint32_t)a2, xa, ya, za);
-        X.fence(xa, ya, za);
-        ca = lane_locate(G, Q, ma & 0xff, xa, ya, za);
-        la = __ldg(ca.p); ha = __ldg(ca.p + zs);
-        if (a0 + 1 < n) consume(a0 + 1, mb, cb, lb, hb, xb, yb, zb);
+    float x[LANE_GD], y[LANE_GD], z[LANE_GD];
+    int m[LANE_GD];
+    LaneCell c[LANE_GD];
+    float4 lo[LANE_GD], hi[LANE_GD];
+#pragma unroll
+    for (int k = 0; k < LANE_GD - 1; ++k) {                    // prologue: atoms 0 .. LANE_GD-2 (the tail repeats the last atom)
+        const int a = min(k, n - 1);
+        m[k] = S.meta[a];
+        X.get(XS::kScale * (uint32_t)a, x[k], y[k], z[k]);
+        X.fence(x[k], y[k], z[k]);
+        c[k] = lane_locate(G, Q, m[k] & 0xff, x[k], y[k], z[k]);
+        lo[k] = __ldg(c[k].p); hi[k] = __ldg(c[k].p + zs);
+    }
+    for (int a0 = 0; a0 < n; a0 += LANE_GD) {
+#pragma unroll
+        for (int k = 0; k < LANE_GD; ++k) {
+            {                                                   // request atom a0 + k + LANE_GD - 1 into the slot freed last
+                constexpr int D1 = LANE_GD - 1;
+                const int sl = (k + D1) % LANE_GD;
+                const int a = min(a0 + k + D1, n - 1);
+                m[sl] = S.meta[a];
+                X.get(XS::kScale * (uint32_t)a, x[sl], y[sl], z[sl]);
+                X.fence(x[sl], y[sl], z[sl]);
+                c[sl] = lane_locate(G, Q, m[sl] & 0xff, x[sl], y[sl], z[sl]);
+                lo[sl] = __ldg(c[sl].p); hi[sl] = __ldg(c[sl].p + zs);
+            }
+            if (a0 + k < n) {                                   // blend atom a0 + k
+                float gx, gy, gz;
+                e_inter += lane_blend(G, k_wall, c[k], lo[k], hi[k], grad, x[k], y[k], z[k], gx, gy, gz);
+                if (grad) {
+                    if ((m[k] & 0x100) && a0 + k > 0) {        // first own atom of the next fragment: the previous one is complete
+#pragma unroll
+                        for (int j = 0; j < 6; ++j) { WR[(6 * gcur + j) * C] = acc[j] * wscale; acc[j] = 0.f; }
+                    }
+                    gcur = m[k] >> 16;
+                    acc[0] += gx; acc[1] += gy; acc[2] += gz;
+                    acc[3] += y[k] * gz - z[k] * gy;
+                    acc[4] += z[k] * gx - x[k] * gz;
+                    acc[5] += x[k] * gy - y[k] * gx;
+                }
+            }
+        }
     }
     if (grad) {
 #pragma unroll
-        for (int k = 0; k < 6; ++k) WR[(6 * gcur + k) * C] = acc[k] * wscale;
+        for (int j = 0; j < 6; ++j) WR[(6 * gcur + j) * C] = acc[j] * wscale;
     }
     return e_inter;
 }
@@ -316,37 +324,34 @@ __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], cons
                                          float bx, float by, float bz, const float4 c4, unsigned hbmask,
                                          float& eL, float& eC, float& eH, float fx[4], float fy[4], float fz[4]) {
     const float c[4] = {c4.x, c4.y, c4.z, c4.w};
-    float thr[4] = {K.neg_mu, K.neg_mu, K.neg_mu, K.neg_mu};            // clash range in terms of t = d - c
     float dc[4];
     if (ENERGY) {
 #pragma unroll
         for (int i = 0; i < 4; ++i) dc[i] = c[i] - K.mu;                 // clash distance dvdw (negative: no pair)
-    }
-    if (hbmask) {                                                    // warp-uniform; about one record in three
+        if (hbmask) {                                                // warp-uniform; about one record in three
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            if (GRAD) thr[i] = ((hbmask >> i) & 1u) ? K.hb_dclash - c[i] : thr[i];
-            if (ENERGY) dc[i] = ((hbmask >> i) & 1u) ? K.hb_dclash : dc[i];
+            for (int i = 0; i < 4; ++i) dc[i] = ((hbmask >> i) & 1u) ? K.hb_dclash : dc[i];
         }
     }
-    float dx[4], dy[4], dz[4], d[4], rinv[4], s[4], q[4];
+    float dx[4], dy[4], dz[4], d[4], rinv[4], s[4], q[4], t[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         dx[i] = ax[i] - bx; dy[i] = ay[i] - by; dz[i] = az[i] - bz;
         const float d2 = fmaf(dx[i], dx[i], fmaf(dy[i], dy[i], fmaf(dz[i], dz[i], 1e-12f)));
         rinv[i] = rsqrt_approx(d2);
         d[i] = d2 * rinv[i];
-        const float t = d[i] - c[i];
-        const float u = t * K.nk2;
-        float g = ex2_approx(u * t);
+        t[i] = d[i] - c[i];
+        const float u = t[i] * K.nk2;
+        float g = ex2_approx(u * t[i]);
         g = d[i] < K.dmax ? g : 0.f;
         if (ENERGY) {
             eL += g;
             q[i] = fmaxf(dc[i] * fminf(rinv[i], K.inv_floor), 1.f);     // dc / max(d, floor); > 1 inside the clash range
         }
         if (GRAD) {
-            s[i] = u * g * rinv[i];
-            if (t < thr[i] && rinv[i] < K.inv_floor) s[i] = fmaf(-K.kc * rinv[i], rinv[i], s[i]);
+            // s = rinv (u g - [floor < d < dvdw] kc rinv); a donor/acceptor slot is corrected below
+            const float in = (t[i] < K.neg_mu && rinv[i] < K.inv_floor) ? 1.f : 0.f;    // one FSET, no select / predicate chain
+            s[i] = rinv[i] * fmaf(in, K.nkc * rinv[i], u * g);
         }
     }
     if (ENERGY) eC += lg2_approx((q[0] * q[1]) * (q[2] * q[3]));
@@ -358,7 +363,12 @@ __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], cons
                 float gh = ex2_approx(K.hb_nk2 * th * th);
                 gh = d[i] < K.hb_dmax ? gh : 0.f;
                 if (ENERGY) eH += gh;
-                if (GRAD) s[i] = fmaf(K.kh * th, gh * rinv[i], s[i]);
+                if (GRAD) {
+                    s[i] = fmaf(K.kh * th, gh * rinv[i], s[i]);
+                    // the clash range of a donor/acceptor pair ends at hb_dclash, not at dvdw: put the term right
+                    const bool plain = t[i] < K.neg_mu, hb = d[i] < K.hb_dclash;
+                    if (plain != hb && rinv[i] < K.inv_floor) s[i] = fmaf(hb ? K.nkc : -K.nkc, rinv[i] * rinv[i], s[i]);
+                }
             }
         }
     }
@@ -560,8 +570,17 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
         const uint32_t step = (uint32_t)(a.first_step + s);
         float pt[3] = {ct[0], ct[1], ct[2]}, pq[4] = {cq[0], cq[1], cq[2], cq[3]};
         int entity = 0;
+        float um = 0.f;
         if (s >= 0) {
-            const uint4 r = philox4x32_10(make_uint4(gchain, step, (uint32_t)lig, 0u), key);  // O10: perturbation block
+            // O10: the Metropolis block (purpose 1) and the perturbation block (purpose 0) of this step, drawn by ONE copy of
+            // the generator (a loop that is not unrolled: the hot code must stay inside the instruction cache)
+            uint4 r = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll 1
+            for (uint32_t pz = 0; pz < 2; ++pz) {
+                const uint4 v = philox4x32_10(make_uint4(gchain, step, (uint32_t)lig, 1u - pz), key);
+                if (pz == 0) um = u01(v.x);
+                else r = v;
+            }
             const float u0 = u01(r.x), u1 = u01(r.y), u2 = u01(r.z), u3 = u01(r.w);
             // a2 / O12: perturb one entity of {translation, rotation, torsion k}
             entity = min((int)(u0 * (float)(T + 2)), T + 1);
@@ -622,8 +641,6 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
         // a8: Metropolis and best tracking; the initial pose is always "accepted"
         bool accept = true;
         if (s >= 0) {
-            const uint4 rm = philox4x32_10(make_uint4(gchain, step, (uint32_t)lig, 1u), key); // Metropolis block
-            const float um = u01(rm.x);
             accept = isfinite(enew) && (um < expf(-P.beta * (enew - ecur)));
             if (a.trace != nullptr && live) {
                 tridsk_trace_rec rec;
