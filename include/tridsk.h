@@ -21,7 +21,10 @@
  *   - There is no CPU fallback: without a CUDA device every compute call fails with TRIDSK_ECUDA.
  *   - Pose layout   [tx,ty,tz, qw,qx,qy,qz, theta_0..theta_{T-1}]  (Hamilton, active rotation,
  *     torsion k right-handed about tor_a[k] -> tor_b[k]; theta = 0, q = 1, t = 0 is ref_xyz; O8/G10).
- *     Input quaternions are renormalised; a zero quaternion gives NaN energies.
+ *     Input quaternions are renormalised; a pose whose quaternion has zero or non-finite norm is rejected with
+ *     TRIDSK_EINVAL when the poses are HOST memory (tridsk_score_grad, tridsk_score_direct, tridsk_dock init_poses).
+ *     Poses handed over in DEVICE memory are never read by the host (the call stays asynchronous): there such a pose
+ *     gets NaN energies (tridsk_score_grad) or a chain that rejects every proposal (tridsk_dock).
  *   - Gradient layout [dE/dt (3), dE/domega (3, world-frame rotation vector about t), dE/dtheta (T)] (O9).
  *   - Limits: n_atoms <= 128, n_torsions <= 31, n_types <= 32 per ligand (TRIDSK_ELIMIT otherwise).
  */
@@ -218,6 +221,22 @@ long long tridsk_launch_count(const tridsk_ctx* ctx);
 /* Philox4x32-10 block for the given counter/key, computed ON THE DEVICE by the same routine the chains use
  * (test hook for O10).  ctr[4], key[2], out[4]: [host]. */
 int tridsk_debug_philox(tridsk_ctx* ctx, const unsigned int ctr[4], const unsigned int key[2], unsigned int out[4]);
+
+/*
+ * The roofline denominators of the fused MC step, measured on this device: one launch of
+ * microbenchmark `which` on the ctx stream, timed with CUDA events.  ms [host]: device time of the launch; work [host]:
+ * what it did -- flops (TRIDSK_MB_FFMA, TRIDSK_MB_FFMA2: independent FP32 FMA chains, plain and packed f32x2), MUFU
+ * operations (TRIDSK_MB_MUFU: ex2.approx chains), bytes read (TRIDSK_MB_L2_READ: coalesced 16-byte loads over a buffer of
+ * `bytes`, `iters` passes; below the L2 size the buffer is L2-resident after the first pass), bytes of 32-byte sectors
+ * touched (TRIDSK_MB_GATHER: per lane one 16-byte load from a pseudo-random sector of a buffer of `bytes`, the access a
+ * trilinear lookup in the xy-packed grid makes twice per atom).  Not on the docking path.
+ */
+#define TRIDSK_MB_FFMA    0
+#define TRIDSK_MB_FFMA2   1
+#define TRIDSK_MB_MUFU    2
+#define TRIDSK_MB_L2_READ 3
+#define TRIDSK_MB_GATHER  4
+int tridsk_debug_microbench(tridsk_ctx* ctx, int which, unsigned long long bytes, int iters, float* ms, double* work);
 
 #ifdef __cplusplus
 }

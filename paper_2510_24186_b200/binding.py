@@ -357,6 +357,12 @@ class Engine:
         self._ck(lib().tridsk_last_dock_ms(self.ctx, ms))
         return float(ms[0]), float(ms[1])
 
+    def microbench(self, which, nbytes=0, iters=1):
+        """One launch of a roofline microbenchmark (tridsk_debug_microbench): returns (ms, work)."""
+        ms, work = C.c_float(), C.c_double()
+        self._ck(lib().tridsk_debug_microbench(self.ctx, int(which), C.c_ulonglong(int(nbytes)), int(iters), C.byref(ms), C.byref(work)))
+        return float(ms.value), float(work.value)
+
     def philox(self, ctr, key):
         out = (C.c_uint * 4)()
         self._ck(lib().tridsk_debug_philox(self.ctx, (C.c_uint * 4)(*ctr), (C.c_uint * 2)(*key), out))

@@ -7,11 +7,28 @@
 #include <string.h>
 
 #include <algorithm>
+#include <cmath>
 #include <new>
+
+#include <nvtx3/nvToolsExt.h>
 
 #include "internal.h"
 
 // ---------------------------------------------------------------------------------------- helpers
+// NVTX range around a C-ABI call: captures under nsys / ncu name the four hot-path calls.
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
+// Every entry point makes the ctx's device current: handles of several devices can live in one process.
+#define ENTER(ctx)                                                                                 \
+    do {                                                                                           \
+        int dev_ = -1;                                                                             \
+        if (cudaGetDevice(&dev_) != cudaSuccess || dev_ != (ctx)->device) {                        \
+            cudaError_t e_ = cudaSetDevice((ctx)->device);                                         \
+            if (e_ != cudaSuccess) return fail((ctx), TRIDSK_ECUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e_)); \
+        }                                                                                          \
+    } while (0)
 static int fail(tridsk_ctx* ctx, int code, const std::string& msg) {
     if (ctx) ctx->err = msg;
     return code;
@@ -53,6 +70,16 @@ static int stage_in(tridsk_ctx* ctx, int slot, const void* p, size_t bytes, cons
     return TRIDSK_OK;
 }
 
+// host poses: the quaternion of every pose must have a finite, non-zero norm (tridsk.h conventions)
+static bool host_quats_ok(const float* poses, size_t n_pose, int pose_stride) {
+    for (size_t i = 0; i < n_pose; ++i) {
+        const float* q = poses + i * pose_stride + 3;
+        const float n2 = q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3];
+        if (!(n2 > 0.f) || !std::isfinite(n2)) return false;
+    }
+    return true;
+}
+
 static void to_dparams(const tridsk_params* p, DParams* d) {
     d->w_long = p->w_long; d->w_clash = p->w_clash; d->w_hbond = p->w_hbond;
     d->long_mu = p->long_mu; d->long_inv_two_sigma2 = 1.0f / p->long_two_sigma2; d->long_dmax = p->long_dmax;
@@ -62,6 +89,18 @@ static void to_dparams(const tridsk_params* p, DParams* d) {
     d->beta = p->beta; d->lr = p->lr; d->adam_b1 = p->adam_b1; d->adam_b2 = p->adam_b2; d->adam_eps = p->adam_eps;
     d->pert_trans = p->pert_trans; d->pert_rot = p->pert_rot; d->w_tor = p->w_tor;
     d->n_refine = p->n_refine;
+}
+
+// the constants every kernel divides by or takes a logarithm / square root of
+static int check_params(tridsk_ctx* ctx, const tridsk_params* p) {
+    const float pos[] = {p->long_two_sigma2, p->hb_sigma, p->d_floor, p->hb_dclash, p->lr};
+    for (float v : pos) if (!(v > 0.f) || !std::isfinite(v)) return fail(ctx, TRIDSK_EINVAL, "long_two_sigma2, hb_sigma, d_floor, hb_dclash and lr must be > 0");
+    const float fin[] = {p->w_long, p->w_clash, p->w_hbond, p->long_mu, p->long_dmax, p->hb_mu, p->hb_dmax, p->k_wall, p->beta,
+                         p->adam_b1, p->adam_b2, p->adam_eps, p->pert_trans, p->pert_rot, p->w_tor};
+    for (float v : fin) if (!std::isfinite(v)) return fail(ctx, TRIDSK_EINVAL, "non-finite parameter");
+    if (!(p->adam_b1 >= 0.f && p->adam_b1 < 1.f && p->adam_b2 >= 0.f && p->adam_b2 < 1.f)) return fail(ctx, TRIDSK_EINVAL, "adam_b1, adam_b2 must lie in [0, 1)");
+    if (p->n_refine < 0) return fail(ctx, TRIDSK_EINVAL, "n_refine < 0");
+    return TRIDSK_OK;
 }
 
 // ---------------------------------------------------------------------------------------- lifetime
@@ -131,7 +170,7 @@ extern "C" void tridsk_destroy(tridsk_ctx* ctx) {
         if (ctx->join_ev[i]) cudaEventDestroy(ctx->join_ev[i]);
         if (ctx->side[i]) cudaStreamDestroy(ctx->side[i]);
     }
-    for (int i = 0; i < 8; ++i) if (ctx->scratch[i]) cudaFree(ctx->scratch[i]);
+    for (int i = 0; i < TRIDSK_SCRATCH; ++i) if (ctx->scratch[i]) cudaFree(ctx->scratch[i]);
     if (ctx->own_stream) cudaStreamDestroy(ctx->stream);
     delete ctx;
 }
@@ -140,6 +179,7 @@ extern "C" const char* tridsk_last_error(const tridsk_ctx* ctx) { return ctx ? c
 extern "C" long long tridsk_launch_count(const tridsk_ctx* ctx) { return ctx ? ctx->launches : 0; }
 extern "C" int tridsk_synchronize(tridsk_ctx* ctx) {
     if (!ctx) return TRIDSK_EINVAL;
+    ENTER(ctx);
     CK(cudaStreamSynchronize(ctx->stream));
     return TRIDSK_OK;
 }
@@ -179,6 +219,9 @@ extern "C" int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const in
                                  const tridsk_types* types, const tridsk_params* params,
                                  const float origin[3], const int dims[3], float spacing, tridsk_grid** out) {
     if (!ctx || !out || !params || !rec_xyz || !rec_type || n_rec < 0) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    NvtxRange nvtx_("tridsk_build_grid");
+    if (int prc = check_params(ctx, params)) return prc;
     *out = nullptr;
     int rc = check_types(ctx, types);
     if (rc) return rc;
@@ -236,6 +279,7 @@ extern "C" int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const in
 extern "C" int tridsk_grid_from_values(tridsk_ctx* ctx, const float* values, int n_types,
                                        const float origin[3], const int dims[3], float spacing, tridsk_grid** out) {
     if (!ctx || !out || !values) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
     *out = nullptr;
     tridsk_grid* g = nullptr;
     int rc = new_grid(ctx, n_types, origin, dims, spacing, &g);
@@ -251,6 +295,7 @@ extern "C" int tridsk_grid_from_values(tridsk_ctx* ctx, const float* values, int
 
 extern "C" int tridsk_grid_export(tridsk_ctx* ctx, const tridsk_grid* grid, float* dst) {
     if (!ctx || !grid || !dst) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
     CK(cudaMemcpyAsync(dst, grid->g, sizeof(float) * grid->d.plane * grid->d.n_types, cudaMemcpyDefault, ctx->stream));
     if (!is_device_ptr(dst)) CK(cudaStreamSynchronize(ctx->stream));
     return TRIDSK_OK;
@@ -548,12 +593,20 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
 extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b, const tridsk_types* types,
                                    tridsk_ligands** out) {
     if (!ctx || !b || !out) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    NvtxRange nvtx_("tridsk_load_ligands");
     *out = nullptr;
     int rc = check_types(ctx, types);
     if (rc) return rc;
     if (b->n_lig < 0 || !b->atom_off || !b->tor_off || (b->n_lig && (!b->ref_xyz || !b->atom_type || !b->atom_frag)))
         return fail(ctx, TRIDSK_EINVAL, "bad ligand batch");
     const int L = b->n_lig;
+    // offsets must be non-decreasing, and every array an offset table indexes must be there
+    auto mono = [&](const int* off) { for (int i = 0; i < L; ++i) if (off[i + 1] < off[i] || off[0] < 0) return false; return true; };
+    if (!mono(b->atom_off) || !mono(b->tor_off)) return fail(ctx, TRIDSK_EINVAL, "atom_off / tor_off must be non-decreasing");
+    if (L && b->tor_off[L] > b->tor_off[0] && (!b->tor_a || !b->tor_b || !b->tor_parent)) return fail(ctx, TRIDSK_EINVAL, "torsions without tor_a / tor_b / tor_parent");
+    if (b->pair_off && (!mono(b->pair_off) || (L && b->pair_off[L] > b->pair_off[0] && !b->pair_ab))) return fail(ctx, TRIDSK_EINVAL, "bad pair_off / pair_ab");
+    if (!b->pair_off && L && (!b->bond_off || !mono(b->bond_off) || (b->bond_off[L] > b->bond_off[0] && !b->bond_ab))) return fail(ctx, TRIDSK_EINVAL, "neither pairs nor a valid bond list given");
     std::vector<PackedLig> pk(L);
     // the CTA-per-chain format triples the pair storage: it is the single-dock mapping, so screens do not carry it
     const bool want_cta = L <= TRIDSK_CTA_MAX_LIG;
@@ -669,6 +722,9 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
                                  int pose_stride, float* energy, float* grad, int grad_stride, float* coords, int coord_stride) {
     if (!ctx || !grid || !ligs || !params || !lig_index || !poses || !energy || n_pose < 0)
         return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    NvtxRange nvtx_("tridsk_score_grad");
+    if (int prc = check_params(ctx, params)) return prc;
     if (pose_stride < 7 + ligs->max_tor) return fail(ctx, TRIDSK_EINVAL, "pose_stride < 7 + max torsions");
     if (grad && grad_stride < 6 + ligs->max_tor) return fail(ctx, TRIDSK_EINVAL, "grad_stride < 6 + max torsions");
     if (coords && coord_stride < ligs->max_atoms) return fail(ctx, TRIDSK_EINVAL, "coord_stride < max atoms");
@@ -692,6 +748,7 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
     const size_t b_c = coords ? sizeof(float) * 3 * (size_t)n_pose * coord_stride : 0;
     // inputs: slot 7 holds [lig_index | poses] when they come from the host
     const bool h_li = !is_device_ptr(lig_index), h_po = !is_device_ptr(poses);
+    if (h_po && !host_quats_ok(poses, (size_t)n_pose, pose_stride)) return fail(ctx, TRIDSK_EINVAL, "pose with a zero or non-finite quaternion");
     char* in = nullptr;
     if (h_li || h_po) { int rc = scratch(ctx, 7, b_li + b_po + 64, (void**)&in); if (rc) return rc; }
     const size_t o_po = (b_li + 15) / 16 * 16;
@@ -757,6 +814,9 @@ extern "C" int tridsk_score_direct(tridsk_ctx* ctx, const float* rec_xyz, const 
                                    int n_pose, int pose_stride, float* energy, float* grad, int grad_stride) {
     if (!ctx || !rec_xyz || !rec_type || n_rec < 0 || !params || !ligs || !lig_index || !poses || !energy || n_pose < 0)
         return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    NvtxRange nvtx_("tridsk_score_direct");
+    if (int prc = check_params(ctx, params)) return prc;
     int rc = check_types(ctx, types);
     if (rc) return rc;
     if (!ligs->has_cta) return fail(ctx, TRIDSK_EINVAL, "tridsk_score_direct needs a ligand batch of at most 1024 ligands");
@@ -778,6 +838,7 @@ extern "C" int tridsk_score_direct(tridsk_ctx* ctx, const float* rec_xyz, const 
     if ((h_xyz || h_typ) && (rc = scratch(ctx, 4, b_xyz + sizeof(int) * n_rec, (void**)&stage))) return rc;
     const size_t b_li = sizeof(int) * n_pose, b_po = sizeof(float) * (size_t)n_pose * pose_stride, o_po = (b_li + 15) / 16 * 16;
     const bool h_li = !is_device_ptr(lig_index), h_po = !is_device_ptr(poses);
+    if (h_po && !host_quats_ok(poses, (size_t)n_pose, pose_stride)) return fail(ctx, TRIDSK_EINVAL, "pose with a zero or non-finite quaternion");
     if ((h_li || h_po) && (rc = scratch(ctx, 7, o_po + b_po + 64, (void**)&in))) return rc;
     const size_t b_e = sizeof(float) * 3 * n_pose, b_g = grad ? sizeof(float) * (size_t)n_pose * grad_stride : 0, o_g = (b_e + 15) / 16 * 16;
     const bool h_e = !is_device_ptr(energy), h_g = grad && !is_device_ptr(grad);
@@ -908,6 +969,9 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
                            float* out_energy, float* out_pose, int* out_chain, const tridsk_dock_opts* opts_in) {
     if (!ctx || !grid || !ligs || !params || !box_min || !box_max || !pocket_center)
         return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    NvtxRange nvtx_("tridsk_dock");
+    if (int prc = check_params(ctx, params)) return prc;
     tridsk_dock_opts o;
     memset(&o, 0, sizeof(o));
     if (opts_in) o = *opts_in;
@@ -933,7 +997,9 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     else { int rc = scratch(ctx, 2, sizeof(float) * state_floats, (void**)&state); if (rc) return rc; }
     if (o.resume && state_host) CK(cudaMemcpyAsync(state, o.chain_state, sizeof(float) * state_floats, cudaMemcpyHostToDevice, ctx->stream));
     const void* d_init = nullptr;
-    if (o.init_poses) { int rc = stage_in(ctx, 7, o.init_poses, sizeof(float) * n_pose_f, &d_init); if (rc) return rc; }
+    if (o.init_poses && !is_device_ptr(o.init_poses) && !host_quats_ok(o.init_poses, nch, pose_stride))
+        return fail(ctx, TRIDSK_EINVAL, "init pose with a zero or non-finite quaternion");
+    if (o.init_poses) { int rc = stage_in(ctx, 8, o.init_poses, sizeof(float) * n_pose_f, &d_init); if (rc) return rc; }
     tridsk_trace_rec* d_trace = nullptr;
     const size_t trace_bytes = sizeof(tridsk_trace_rec) * nch * (size_t)n_steps;
     const bool trace_host = o.trace && !is_device_ptr(o.trace);
@@ -1115,6 +1181,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
 
 extern "C" int tridsk_last_dock_ms(tridsk_ctx* ctx, float ms[2]) {
     if (!ctx || !ms) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
     if (!ctx->ev_valid) return fail(ctx, TRIDSK_EINVAL, "no dock has run on this ctx");
     CK(cudaEventSynchronize(ctx->ev[2]));
     CK(cudaEventElapsedTime(&ms[0], ctx->ev[0], ctx->ev[1]));
@@ -1125,14 +1192,45 @@ extern "C" int tridsk_last_dock_ms(tridsk_ctx* ctx, float ms[2]) {
 // ---------------------------------------------------------------------------------------- test hook
 extern "C" int tridsk_debug_philox(tridsk_ctx* ctx, const unsigned int ctr[4], const unsigned int key[2], unsigned int out[4]) {
     if (!ctx || !ctr || !key || !out) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
     unsigned int h[6] = {ctr[0], ctr[1], ctr[2], ctr[3], key[0], key[1]};
     unsigned int* d;
-    int rc = scratch(ctx, 7, 64, (void**)&d);
+    int rc = scratch(ctx, 9, 64, (void**)&d);
     if (rc) return rc;
     CK(cudaMemcpyAsync(d, h, sizeof(h), cudaMemcpyHostToDevice, ctx->stream));
     CK(launch_philox_debug(ctx->stream, d, d + 8));
     ctx->launches += 1;
     CK(cudaMemcpyAsync(out, d + 8, 4 * sizeof(unsigned int), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
+    return TRIDSK_OK;
+}
+
+extern "C" int tridsk_debug_microbench(tridsk_ctx* ctx, int which, unsigned long long bytes, int iters, float* ms, double* work) {
+    if (!ctx || !ms || !work || iters < 1) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    const bool mem = which == TRIDSK_MB_L2_READ || which == TRIDSK_MB_GATHER;
+    if (which < TRIDSK_MB_FFMA || which > TRIDSK_MB_GATHER || (mem && bytes < 4096)) return fail(ctx, TRIDSK_EINVAL, "bad microbenchmark");
+    char* buf = nullptr;
+    float* sink;
+    int rc = scratch(ctx, 9, 64, (void**)&sink);
+    if (rc) return rc;
+    if (mem) {
+        if ((rc = scratch(ctx, 10, bytes, (void**)&buf))) return rc;
+        CK(cudaMemsetAsync(buf, 0, bytes, ctx->stream));
+    }
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    double w = 0.0;
+    cudaError_t e = launch_microbench(ctx->stream, which, ctx->sm_count, buf, bytes, 1, sink, &w);      // warm-up pass (fills L2)
+    if (e == cudaSuccess) e = cudaEventRecord(e0, ctx->stream);
+    if (e == cudaSuccess) e = launch_microbench(ctx->stream, which, ctx->sm_count, buf, bytes, iters, sink, &w);
+    if (e == cudaSuccess) e = cudaEventRecord(e1, ctx->stream);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (e != cudaSuccess) return fail(ctx, TRIDSK_ECUDA, std::string("microbench: ") + cudaGetErrorString(e));
+    ctx->launches += 2;
+    *work = w;
     return TRIDSK_OK;
 }

@@ -73,13 +73,15 @@ __global__ void __launch_bounds__(GB_THREADS) grid_build_kernel(const float4* __
     const float hx = 0.5f * G.h * (float)(GB_BX - 1), hy = 0.5f * G.h * (float)(GB_BY - 1), hz = 0.5f * G.h * (float)(GB_BZ - 1);
     const float cx = G.ox + G.h * (float)(blockIdx.x * GB_BX) + hx, cy = G.oy + G.h * (float)(blockIdx.y * GB_BY) + hy;
     const float cz = G.oz + G.h * (float)(blockIdx.z * GB_BZ) + hz;
-    const float rc = P.long_dmax + sqrtf(hx * hx + hy * hy + hz * hz) + 1e-3f;
+    // the indicators of O2 are independent: cull with the larger of the long-range cut-off and the clash / hydrogen-bond range
+    const float cull = fmaxf(P.long_dmax, dc_max);
+    const float rc = cull + sqrtf(hx * hx + hy * hy + hz * hz) + 1e-3f;
     const float rc2 = rc * rc;
 
     float acc[NT], accx[NT];                       // acc: sum of 2^(...) Gaussians (scaled by -w_long at the end); accx: the rest
 #pragma unroll
     for (int t = 0; t < NT; ++t) { acc[t] = 0.f; accx[t] = 0.f; }
-    const float dmax2 = P.long_dmax * P.long_dmax;
+    const float dmax2 = cull * cull;
     const float nk2 = -P.long_inv_two_sigma2 * 1.4426950408889634f;
 
     for (int base = 0; base < n_rec; base += GB_CHUNK) {
@@ -113,9 +115,10 @@ __global__ void __launch_bounds__(GB_THREADS) grid_build_kernel(const float4* __
             if (d2 >= dmax2) continue;
             const float rinv = rsqrtf(fmaxf(d2, 1e-12f));
             const float d = d2 * rinv;
-            if (!(d < P.long_dmax)) continue;
             const int s = __float_as_int(ra.w);
-            if (LAT) {
+            if (!(d < P.long_dmax)) {               // beyond the long-range cut-off: only the rare terms below can act
+                if (!(d < dc_max)) continue;
+            } else if (LAT) {
                 const float xs = d - s_c[s * NT + lat.order[0]];      // r_s + r_min + mu, as tabulated
                 const float B = exp2f_approx(lat.delta_k * xs);
                 float pw = exp2f_approx(nk2 * xs * xs);

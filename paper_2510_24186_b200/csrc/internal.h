@@ -14,6 +14,7 @@
 #define TRIDSK_MAX_J 4           // atoms per lane (n_atoms <= 32 * MAX_J)
 #define TRIDSK_MAX_TILES 10      // J(J+1)/2 tiles of the pair schedule
 #define TRIDSK_CTA_MAX_LIG 1024  // batches up to this size also carry the CTA-per-chain pair format
+#define TRIDSK_SCRATCH 12       // scratch buffers owned by a ctx (api.cu names the slots)
 #define TRIDSK_BRANCHES 16       // parallel branches of a dock's launch series (ctx stream + side streams)
 
 // ---------------------------------------------------------------- device-side packed formats
@@ -233,8 +234,8 @@ struct tridsk_ctx {
     long long launches = 0;
     int sm_count = 0;
     // scratch owned by the ctx (grown on demand)
-    void* scratch[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    size_t scratch_bytes[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    void* scratch[TRIDSK_SCRATCH] = {};
+    size_t scratch_bytes[TRIDSK_SCRATCH] = {};
     // cached CUDA graph of the last dock launch series
     cudaGraphExec_t graph_exec = nullptr;
     std::vector<unsigned char> graph_key;
@@ -309,4 +310,5 @@ cudaError_t launch_score_direct(cudaStream_t s, const LigHdr* hdr, const float4*
                                 const unsigned char* role, const DParams& P, const int* lig_index, const float* poses, int n_pose,
                                 int pose_stride, float* energy, float* grad, int grad_stride, int max_atoms);
 size_t topk_cluster_smem(int top_k, int max_atoms, int max_tor);
+cudaError_t launch_microbench(cudaStream_t s, int which, int sm_count, void* buf, size_t bytes, int iters, float* sink, double* work);
 cudaError_t launch_philox_debug(cudaStream_t s, const unsigned int* ctr_key /* dev[6] */, unsigned int* out /* dev[4] */);

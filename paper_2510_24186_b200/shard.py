@@ -40,18 +40,47 @@ def merge_ligand_shards(energy, pose, chain, n_lig: int):
     return tuple(outs)
 
 
-def merge_chain_shards(energy, pose, chain, chain_base: int, k: int):
+def merge_chain_shards(energy, pose, chain, chain_base: int, k: int, cluster_rmsd: float = 0.0):
     """Global top-k per ligand from every rank's local top-k candidates: sort by (E_dock, global chain id) (O13).
-    energy [n_lig, k_local, 2], pose [n_lig, k_local, stride], chain [n_lig, k_local] (local ids)."""
+    energy [n_lig, k_local, 2], pose [n_lig, k_local, stride], chain [n_lig, k_local] (local ids; -1 = an empty slot).
+    k_local may differ between ranks (uneven chain shards: a rank with fewer chains than k returns fewer candidates):
+    every rank's block is padded to the largest k_local with (+inf, zero pose, chain -1) before the all_gather, and the
+    fillers sort last; if fewer than k real candidates exist overall the tail of the result is such fillers.
+    Duplicate removal (tridsk_dock_opts.cluster_rmsd, O14) compares poses ACROSS chains, so per-shard filtered candidates
+    cannot be merged by a sort: it is refused here -- shard such a job by ligand, or dock it on one GPU."""
+    if cluster_rmsd > 0.0:
+        raise ValueError("merge_chain_shards: duplicate-removing top-k (cluster_rmsd > 0) cannot be merged across chain "
+                         "shards; shard by ligand or run the dock on one GPU")
     world = dist.get_world_size()
-    g_chain = chain.to(torch.int64) + int(chain_base)
+    k_loc = torch.tensor([energy.shape[1]], dtype=torch.int64, device=energy.device)
+    ks = [torch.zeros_like(k_loc) for _ in range(world)]
+    dist.all_gather(ks, k_loc)
+    k_pad = int(max(int(v) for v in ks))
+    valid = chain >= 0
+    g_chain = torch.where(valid, chain.to(torch.int64) + int(chain_base), torch.full_like(chain, -1, dtype=torch.int64))
+    e_in = energy.clone()
+    e_in[~valid] = float("inf")
+
+    def pad(t, fill):
+        if t.shape[1] == k_pad:
+            return t.contiguous()
+        ext = torch.full((t.shape[0], k_pad - t.shape[1]) + tuple(t.shape[2:]), fill, dtype=t.dtype, device=t.device)
+        return torch.cat([t, ext], dim=1).contiguous()
+
     parts = []
-    for t in (energy, pose, g_chain):
-        buf = [torch.empty_like(t) for _ in range(world)]
-        dist.all_gather(buf, t.contiguous())
+    for t, fill in ((e_in, float("inf")), (pose, 0.0), (g_chain, -1)):
+        tp = pad(t, fill)
+        buf = [torch.empty_like(tp) for _ in range(world)]
+        dist.all_gather(buf, tp)
         parts.append(torch.cat(buf, dim=1))
     e, p, c = parts
-    o1 = torch.argsort(c, dim=1, stable=True)                         # secondary key first
+    if e.shape[1] < k:                                                # fewer candidates than slots asked for
+        short = k - e.shape[1]
+        ext = lambda t, fill: torch.cat([t, torch.full((t.shape[0], short) + tuple(t.shape[2:]), fill, dtype=t.dtype, device=t.device)], dim=1)
+        e, p, c = ext(e, float("inf")), ext(p, 0.0), ext(c, -1)
+    # fillers (chain -1, +inf) must sort after every real candidate, also after a real +inf energy: key them by a huge id
+    ckey = torch.where(c >= 0, c, torch.full_like(c, 2 ** 62))
+    o1 = torch.argsort(ckey, dim=1, stable=True)                      # secondary key first
     e1 = torch.gather(e[..., 0], 1, o1)
     o2 = torch.argsort(e1, dim=1, stable=True)
     order = torch.gather(o1, 1, o2)[:, :k]

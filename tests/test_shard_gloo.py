@@ -41,7 +41,26 @@ def _worker(rank, world, port, q):
     want = [sorted(range(n_ch), key=lambda i: (float(row[i]), i))[:kk] for row in Eb]
     ok2 = mc.tolist() == want and torch.equal(me[..., 0], torch.stack([Eb[r][want[r]] for r in range(3)]))
     ok2 = ok2 and torch.equal(mp_[..., 0], torch.tensor(want).float())
-    q.put((rank, bool(ok1), bool(ok2)))
+    # ---- uneven chain shards: 5 chains over 2 ranks = 3 + 2, local top-3 of a rank with 2 chains has only 2 candidates
+    n_ch = 5
+    Eu = torch.tensor([[4., -1., 2., -1., 0.5]])
+    base, n_local = shard.chain_shard(n_ch, rank, world)
+    loc = Eu[:, base:base + n_local]
+    k_local = min(3, n_local)
+    order = torch.stack([torch.tensor(sorted(range(n_local), key=lambda i: (float(row[i]), i))[:k_local]) for row in loc])
+    le = torch.stack([torch.gather(loc, 1, order), torch.gather(loc, 1, order)], dim=-1)
+    lp = order.float().unsqueeze(-1).repeat(1, 1, stride) + base
+    me, mp_, mc = shard.merge_chain_shards(le, lp, order.to(torch.int32), base, 5)
+    ok3 = mc.tolist() == [[1, 3, 4, 2, 0]] and me[0, :, 0].tolist() == [-1., -1., 0.5, 2., 4.]
+    # more slots asked for than candidates exist: the tail is fillers (chain -1, +inf)
+    me, mp_, mc = shard.merge_chain_shards(le[:, :1], lp[:, :1], order[:, :1].to(torch.int32), base, 3)
+    ok3 = ok3 and mc.tolist() == [[1, 3, -1]] and torch.isinf(me[0, 2, 0]).item()
+    try:
+        shard.merge_chain_shards(le, lp, order.to(torch.int32), base, 2, cluster_rmsd=1.0)
+        ok3 = False
+    except ValueError:
+        pass
+    q.put((rank, bool(ok1), bool(ok2 and ok3)))
     dist.destroy_process_group()
 
 
