@@ -1,9 +1,9 @@
 """oracle/mdn.py -- E_MDN, the mixture-density term of the paper's score, as a plain fp64 definition.
 
 TEST INFRASTRUCTURE (like the rest of oracle/): only tests/ may import it; it shares no code with the CUDA path.
-STATUS: SURVEY 8(f) NEXT-1 groundwork.  This round builds no kernel for E_MDN (w_MDN * E_MDN stays out of the hot path,
-DESIGN.md section 3); the oracle is written and pinned first, as the build order requires, so that the kernels of the
-next round have something to be checked against.  GPU parity for this term: not applicable yet.
+STATUS: the plain Python transcription of O15.  The oracle the kernels are checked against is orc_mdn_energy in
+tridsk_oracle.c (the same definition in C, called from orc_score_grad / orc_mc_step); both run under the same pins in
+tests/test_oracle_pins.py and must agree with each other to rounding.
 
 What is computed (P:N = /root/reference/PAPER.md line N):
   Eq.GMM      p(d | i, j) = sum_k pi_ijk N(d; mu_ijk, sigma_ijk)      K Gaussians per (residue i, ligand atom j)

@@ -47,10 +47,15 @@ class _Grid(C.Structure):
                 ("origin", C.c_double * 3), ("spacing", C.c_double)]
 
 
+class _Mdn(C.Structure):
+    _fields_ = [("n_res", C.c_int), ("K", C.c_int), ("res_off", C.c_void_p), ("res_xyz", C.c_void_p), ("pi", C.c_void_p),
+                ("mu", C.c_void_p), ("sigma", C.c_void_p), ("w_mdn", C.c_double), ("d_cut", C.c_double)]
+
+
 class _Ligand(C.Structure):
     _fields_ = [("n", C.c_int), ("T", C.c_int), ("P", C.c_int), ("ref", C.c_void_p), ("type", C.c_void_p),
                 ("frag", C.c_void_p), ("tor_a", C.c_void_p), ("tor_b", C.c_void_p), ("tor_parent", C.c_void_p),
-                ("pairs", C.c_void_p)]
+                ("pairs", C.c_void_p), ("mdn", C.c_void_p)]
 
 
 class StepRec(C.Structure):
@@ -69,6 +74,7 @@ def lib():
         _lib.orc_derive_pairs.restype = C.c_int
         assert _lib.orc_sizeof_params() == C.sizeof(Params)
         assert _lib.orc_sizeof_step_rec() == C.sizeof(StepRec)
+        assert _lib.orc_sizeof_ligand() == C.sizeof(_Ligand) and _lib.orc_sizeof_mdn() == C.sizeof(_Mdn)
     return _lib
 
 
@@ -121,7 +127,43 @@ class Ligand:
         self.P = len(self.pairs)
         self.c = _Ligand(self.n, self.T, self.P, _p(self.ref).value, _p(self.type).value, _p(self.frag).value,
                          _p(self.tor_a).value, _p(self.tor_b).value, _p(self.tor_parent).value,
-                         _p(self.pairs).value)
+                         _p(self.pairs).value, None)
+        self.mdn = None
+
+    def set_mdn(self, mdn: "Mdn | None"):
+        """Attach (or detach, None) the mixture-density term: every score / MC step of this ligand then uses the paper's
+        full E_dock = w_MDN E_MDN + w_long E_long + w_clash E_clash + w_Hbond E_Hbond."""
+        if mdn is not None:
+            assert mdn.pi.shape[1] == self.n
+        self.mdn = mdn
+        self.c.mdn = C.addressof(mdn.c) if mdn is not None else None
+        return self
+
+
+class Mdn:
+    """O15 inputs for ONE ligand: residues of the receptor (res_off into res_xyz) and the mixture parameters
+    pi, mu, sigma [n_res][n_atoms][K] of every (residue, ligand atom) pair (Eq.GMM)."""
+
+    def __init__(self, res_xyz, res_off, pi, mu, sigma, w_mdn=1.0, d_cut=5.0):
+        self.res_xyz = np.ascontiguousarray(res_xyz, dtype=np.float64)
+        self.res_off = np.ascontiguousarray(res_off, dtype=np.int32)
+        self.pi, self.mu, self.sigma = (np.ascontiguousarray(a, dtype=np.float64) for a in (pi, mu, sigma))
+        n_res, n, K = self.pi.shape
+        assert len(self.res_off) == n_res + 1 and self.mu.shape == self.pi.shape == self.sigma.shape
+        self.c = _Mdn(n_res, K, _p(self.res_off).value, _p(self.res_xyz).value, _p(self.pi).value, _p(self.mu).value,
+                      _p(self.sigma).value, float(w_mdn), float(d_cut))
+
+
+def mdn_energy(res_xyz, res_off, pi, mu, sigma, x, d_cut=5.0):
+    """orc_mdn_energy (O15): -> (E_MDN, dE/dx [n][3], d [n_res][n]).  Same signature as oracle.mdn.mdn_energy."""
+    M = Mdn(res_xyz, res_off, pi, mu, sigma, 1.0, d_cut)
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    n = x.shape[0]
+    e = C.c_double()
+    g = np.zeros((n, 3))
+    dm = np.zeros((M.c.n_res, n))
+    lib().orc_mdn_energy(C.byref(M.c), C.c_int(n), _p(x), C.byref(e), _p(g), _p(dm))
+    return float(e.value), g, dm
 
 
 def ligand_from_batch(batch, i) -> Ligand:

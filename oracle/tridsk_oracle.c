@@ -15,7 +15,8 @@
  * trilinear fields + scipy RegularGridInterpolator; FK vs scipy Rotation / textbook matrices /
  * preserved internal coordinates; intra-ligand rigid invariance + Newton's third law; analytic
  * gradient vs central differences; Philox known answers; Adam vs torch.optim.Adam; Metropolis
- * P(accept | dE = 10) = 0.5016.
+ * P(accept | dE = 10) = 0.5016; E_MDN (orc_mdn_energy): closed forms, scipy.stats.norm, central differences,
+ * the plain Python transcription of the same definition (oracle/mdn.py), and total = physics + w_MDN E_MDN on a hand case.
  * PARITY UNPINNED: the whole stochastic chain (orc_dock) has no external truth -- the paper
  * prints no worked example -- so it is pinned only through its parts plus sanity invariants.
  */
@@ -48,6 +49,17 @@ typedef struct {
     double origin[3], spacing;
 } orc_grid;
 
+/* O15: the mixture-density term of one (receptor, ligand) pair -- Eq.GMM, Eq.E_MDN */
+typedef struct {
+    int n_res, K;
+    const int* res_off;          /* [n_res+1]: the atoms of residue i are res_xyz[res_off[i] .. res_off[i+1]) */
+    const double* res_xyz;       /* [res_off[n_res]][3] */
+    const double* pi;            /* [n_res][n][K] mixture weights of (residue i, ligand atom j) */
+    const double* mu;            /* [n_res][n][K] */
+    const double* sigma;         /* [n_res][n][K] */
+    double w_mdn, d_cut;         /* 1.0, 5.0 A */
+} orc_mdn;
+
 typedef struct {
     int n, T, P;
     const double* ref;           /* [n][3] reference conformer, centred */
@@ -57,6 +69,7 @@ typedef struct {
     const unsigned char* tor_b;
     const signed char* tor_parent; /* [T] -1 = root; parents precede children */
     const unsigned char* pairs;  /* [P][2] */
+    const orc_mdn* mdn;          /* NULL: w_MDN E_MDN absent from the score (the round-1 hot path); else added to E */
 } orc_ligand;
 
 void orc_default_params(orc_params* p) {
@@ -280,6 +293,44 @@ int orc_derive_pairs(int n, const unsigned char* frag, const unsigned char* bond
     return P;
 }
 
+/* ------------------------------------------------------------------ O15: E_MDN */
+/*
+ * E_MDN = - sum_i sum_j [d_ij < d_cut] sum_k pi_ijk N(d_ij; mu_ijk, sigma_ijk)  (Eq.E_MDN, sign G1), with
+ * N the normalised Gaussian density (G17) and d_ij the minimum distance between the atoms of residue i and ligand atom j
+ * (P:93); ties of the minimum go to the lowest atom index, and neither the arg-min switch nor the cut-off indicator is
+ * differentiated (G21): the gradient flows through the arg-min atom.
+ * x [n][3] ligand coordinates.  *e = E_MDN (unweighted); g (may be NULL) [n][3] += nothing -- it is SET to dE_MDN/dx;
+ * dmin (may be NULL) [n_res][n] the minimum distances.
+ */
+void orc_mdn_energy(const orc_mdn* M, int n, const double* x, double* e, double* g, double* dmin) {
+    double E = 0.0;
+    if (g) for (int c = 0; c < 3 * n; ++c) g[c] = 0.0;
+    for (int i = 0; i < M->n_res; ++i) {
+        for (int j = 0; j < n; ++j) {
+            double best = INFINITY;
+            int r_best = -1;
+            for (int r = M->res_off[i]; r < M->res_off[i + 1]; ++r) {
+                double dv[3] = {x[3 * j] - M->res_xyz[3 * r], x[3 * j + 1] - M->res_xyz[3 * r + 1], x[3 * j + 2] - M->res_xyz[3 * r + 2]};
+                double d = sqrt(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2]);
+                if (d < best) { best = d; r_best = r; }
+            }
+            if (dmin) dmin[(size_t)i * n + j] = best;
+            if (!(best < M->d_cut)) continue;
+            double dE_dd = 0.0;
+            for (int k = 0; k < M->K; ++k) {
+                size_t q = ((size_t)i * n + j) * M->K + k;
+                double sg = M->sigma[q], m = M->mu[q], w = M->pi[q];
+                double N = exp(-(best - m) * (best - m) / (2.0 * sg * sg)) / (sg * sqrt(2.0 * M_PI));
+                E -= w * N;
+                dE_dd += w * N * (best - m) / (sg * sg);
+            }
+            if (g && best > 0.0)
+                for (int c = 0; c < 3; ++c) g[3 * j + c] += dE_dd * (x[3 * j + c] - M->res_xyz[3 * r_best + c]) / best;
+        }
+    }
+    *e = E;
+}
+
 /* ------------------------------------------------------------------ O7 + O9: score and gradient */
 /* O9: pose gradient from the per-atom gradient g[n][3] by the direct sums (no tree accumulation), O(N*T). */
 static void pose_gradient(const orc_ligand* L, const double* pose, const double* x, const double* g, double* grad) {
@@ -313,7 +364,8 @@ static void pose_gradient(const orc_ligand* L, const double* pose, const double*
 }
 
 /*
- * E = sum_a [interp(a) + wall(a)] + E_intra.  energy[3] = {total, inter, intra}.
+ * E = sum_a [interp(a) + wall(a)] + E_intra (+ w_MDN E_MDN when L->mdn is set, O15; booked under inter).
+ * energy[3] = {total, inter, intra}.
  * grad (may be NULL) = [dE/dt (3), dE/domega (3, world-frame rotation vector about t), dE/dtheta (T)]
  * by the direct sums of O9; coords (may be NULL) [n][3]; gatom (may be NULL) [n][3] = dE/dx_a.
  */
@@ -342,6 +394,13 @@ void orc_score_grad(const orc_params* p, const orc_types* ty, const orc_grid* G,
                 g[3 * a + c] += de * dv[c] / d;
                 g[3 * b + c] -= de * dv[c] / d;
             }
+    }
+    if (L->mdn) {                              /* E_dock = w_MDN E_MDN + ...; a receptor-ligand term: booked under "inter" */
+        double e_mdn, *gm = (double*)malloc(sizeof(double) * 3 * n);
+        orc_mdn_energy(L->mdn, n, x, &e_mdn, gm, NULL);
+        e_inter += L->mdn->w_mdn * e_mdn;
+        for (int c = 0; c < 3 * n; ++c) g[c] += L->mdn->w_mdn * gm[c];
+        free(gm);
     }
     energy[0] = e_inter + e_intra; energy[1] = e_inter; energy[2] = e_intra;
     if (grad) pose_gradient(L, pose, x, g, grad);
@@ -387,6 +446,13 @@ void orc_score_grad_direct(const orc_params* p, const orc_types* ty, const doubl
                 g[3 * a + c] += de * dv[c] / d;
                 g[3 * b + c] -= de * dv[c] / d;
             }
+    }
+    if (L->mdn) {                              /* E_dock = w_MDN E_MDN + ...; a receptor-ligand term: booked under "inter" */
+        double e_mdn, *gm = (double*)malloc(sizeof(double) * 3 * n);
+        orc_mdn_energy(L->mdn, n, x, &e_mdn, gm, NULL);
+        e_inter += L->mdn->w_mdn * e_mdn;
+        for (int c = 0; c < 3 * n; ++c) g[c] += L->mdn->w_mdn * gm[c];
+        free(gm);
     }
     energy[0] = e_inter + e_intra; energy[1] = e_inter; energy[2] = e_intra;
     if (grad) pose_gradient(L, pose, x, g, grad);
@@ -559,3 +625,5 @@ void orc_score_grad_batch(const orc_params* p, const orc_types* ty, const orc_gr
 
 int orc_sizeof_params(void) { return (int)sizeof(orc_params); }
 int orc_sizeof_step_rec(void) { return (int)sizeof(orc_step_rec); }
+int orc_sizeof_ligand(void) { return (int)sizeof(orc_ligand); }
+int orc_sizeof_mdn(void) { return (int)sizeof(orc_mdn); }

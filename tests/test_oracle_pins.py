@@ -843,9 +843,15 @@ def test_direct_receptor_mode_pins(orc, dock_system):
 
 
 # --------------------------------------------------------------------------- E_MDN (Eq.E_MDN; S:8(f) NEXT-1 groundwork)
-def test_mdn_energy_pins():
+@pytest.mark.parametrize("impl", ["python", "c"])
+def test_mdn_energy_pins(impl, orc):
+    """O15 under two independent transcriptions: oracle/mdn.py (plain Python) and orc_mdn_energy (C, the one orc_score_grad
+    and orc_mc_step call)."""
     from scipy.stats import norm
-    from oracle import mdn
+    if impl == "python":
+        from oracle import mdn
+    else:
+        mdn = type("M", (), {"mdn_energy": staticmethod(orc.mdn_energy)})
     rng = np.random.default_rng(3)
     one = lambda v: np.array([[[v]]], dtype=np.float64)
     # (1) one residue of one atom, one ligand atom, K = 1: E = -N(d; mu, sigma) (closed form + scipy's density)
@@ -914,3 +920,60 @@ def test_mdn_energy_pins():
     t = np.array([1.3, -2.2, 0.7])
     E0 = mdn.mdn_energy(rxyz, res_off, pi, mu, sg, x)[0]
     assert mdn.mdn_energy(rxyz + t, res_off, pi, mu, sg, x + t)[0] == pytest.approx(E0, rel=1e-12)
+
+
+def test_mdn_c_and_python_transcriptions_agree(orc):
+    from oracle import mdn
+    rec_ = synth.receptor(200, 18.0, 8, seed=12, grid_n=49, pocket_radius=5.0)
+    order, res_off = synth.residues(rec_, 8)
+    rxyz = rec_.xyz[order].astype(np.float64)
+    n, K = 9, 5
+    pi, mu, sg = synth.gmm_params(len(res_off) - 1, n, K, seed=2)
+    rng = np.random.default_rng(8)
+    for _ in range(5):
+        x = rec_.pocket_center + rng.uniform(-6.0, 6.0, (n, 3))
+        Ep, gp, dp = mdn.mdn_energy(rxyz, res_off, pi, mu, sg, x)
+        Ec, gc, dcc = orc.mdn_energy(rxyz, res_off, pi, mu, sg, x)
+        assert Ep != 0.0 and Ec == pytest.approx(Ep, rel=1e-12)
+        assert np.allclose(gc, gp, rtol=1e-11, atol=1e-14) and np.allclose(dcc, dp, rtol=1e-13)
+
+
+def test_total_energy_is_physics_plus_w_mdn_times_e_mdn(orc):
+    """Eq.E_dock: E = 1.0 E_MDN + 0.2 E_long + 10 E_clash + 0.6 E_Hbond.  Hand case + a random system:
+    orc_score_grad with the term attached = orc_score_grad without it + w_MDN * orc_mdn_energy at the same coordinates,
+    for the energy, the per-atom gradient and (through the same chain rule) all 6+T pose components."""
+    rec = synth.receptor(150, 15.0, 8, seed=1, grid_n=41, pocket_radius=4.0)
+    radius, role = synth.type_table(8)
+    ty, p = orc.Types(radius, role), orc.default_params()
+    G = orc.build_grid(p, ty, rec.xyz, rec.type, rec.origin, rec.dims, rec.spacing)
+    batch = synth.ligands([14], [3], 8, seed=5)
+    L = orc.ligand_from_batch(batch, 0)
+    order, res_off = synth.residues(rec, 8)
+    rxyz = rec.xyz[order].astype(np.float64)
+    pi, mu, sg = synth.gmm_params(len(res_off) - 1, L.n, 3, seed=9)
+    pose = synth.random_poses(batch, [0], rec, seed=4, spread=0.4)[0, :7 + L.T].astype(np.float64)
+    e0, g0, x0, ga0 = orc.score_grad(p, ty, G, L, pose)
+    for w in (1.0, 0.37):
+        L.set_mdn(orc.Mdn(rxyz, res_off, pi, mu, sg, w_mdn=w))
+        e1, g1, x1, ga1 = orc.score_grad(p, ty, G, L, pose)
+        Em, gm, _ = orc.mdn_energy(rxyz, res_off, pi, mu, sg, x0)
+        assert Em < -0.05                                                      # the term is really there
+        assert np.array_equal(x1, x0)
+        assert e1[0] == pytest.approx(e0[0] + w * Em, rel=1e-13) and e1[1] == pytest.approx(e0[1] + w * Em, rel=1e-13)
+        assert e1[2] == e0[2]
+        assert np.allclose(ga1, ga0 + w * gm, rtol=1e-12, atol=1e-13)
+        # pose gradient: central differences of the full energy on all 6+T components
+        h = 1e-6
+        E = lambda q: orc.score_grad(p, ty, G, L, q, want_grad=False)[0][0]
+        for c in range(3):
+            d = np.zeros_like(pose); d[c] = h
+            assert g1[c] == pytest.approx((E(pose + d) - E(pose - d)) / (2 * h), rel=1e-5, abs=2e-5)
+        for k in range(L.T):
+            d = np.zeros_like(pose); d[7 + k] = h
+            assert g1[6 + k] == pytest.approx((E(pose + d) - E(pose - d)) / (2 * h), rel=1e-5, abs=2e-5)
+    L.set_mdn(None)
+    assert orc.score_grad(p, ty, G, L, pose)[0][0] == e0[0]
+    # hand case: one receptor atom = one residue at the origin, one ligand atom at distance 3 on the x axis, K = 1
+    one = lambda v: np.array([[[v]]], dtype=np.float64)
+    Em, gm, dm = orc.mdn_energy(np.zeros((1, 3)), np.array([0, 1]), one(1.0), one(3.0), one(0.5), np.array([[3.0, 0, 0]]))
+    assert Em == pytest.approx(-1.0 / (0.5 * np.sqrt(2 * np.pi)), rel=1e-14) and gm[0, 0] == 0.0
