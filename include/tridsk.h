@@ -158,6 +158,34 @@ int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* batch, const
 int tridsk_ligand_info(const tridsk_ligands* ligs, int* n_lig, int* max_atoms, int* max_torsions, int* n_pairs_out);
 void tridsk_free_ligands(tridsk_ligands* ligs);
 
+/* ---- the mixture-density term E_MDN (O15) ---------------------------------- */
+/*
+ * The paper's main scoring term (w_MDN = 1.0):  E_MDN = - sum_i sum_j [d_ij < d_cut] sum_k pi_ijk N(d_ij; mu_ijk,
+ * sigma_ijk)  (Eq.E_MDN; Eq.GMM) over pocket residues i and ligand atoms j, d_ij = the minimum distance
+ * between the atoms of residue i and ligand atom j, d_cut = 5 A, N the normalised Gaussian density (G17).
+ * The mixture parameters are the output of the paper's graph transformer, which is NOT part of this library:
+ * the caller supplies them (bench.py and the tests: synthetic ones).
+ *   n_res, res_off[n_res+1], res_xyz[res_off[n_res]][3]: the residues' atoms, [host];
+ *   K; pi, mu, sigma: [host|dev], ligand-major: for ligand l of the batch a block [n_res][n_atoms(l)][K], atoms in the
+ *   caller's order, blocks in batch order; sigma > 0.
+ */
+typedef struct {
+    int n_res;
+    const int* res_off;
+    const float* res_xyz;
+    int K;
+    const float* pi;
+    const float* mu;
+    const float* sigma;
+    float w_mdn;               /* 1.0 */
+    float d_cut;               /* 5.0 */
+} tridsk_mdn;
+/* Attach the term to a ligand batch (NULL detaches it): every later tridsk_score_grad / tridsk_dock on these ligands
+ * evaluates the full Eq.E_dock, E = w_MDN E_MDN + [grid terms] + E_intra; in tridsk_score_grad's energy[3]
+ * the term is booked under "receptor" (it is a receptor-ligand term).  The gradient flows through the arg-min atom;
+ * ties of the minimum go to the lowest atom index; the indicators are not differentiated (G21).  Parameters are copied. */
+int tridsk_load_mdn(tridsk_ctx* ctx, tridsk_ligands* ligs, const tridsk_mdn* mdn);
+
 /* ---- score + analytic gradient of given poses (steps a3..a6; O5..O9) --------------------------- */
 /*
  * For pose i of ligand lig_index[i]: forward kinematics, E = sum_a [trilinear G_type(a)(x_a) + wall] + E_intra,

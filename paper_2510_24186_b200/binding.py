@@ -43,6 +43,12 @@ class _Batch(C.Structure):
         "pair_off", "pair_ab", "bond_off", "bond_ab")]
 
 
+class _Mdn(C.Structure):
+    """tridsk_mdn (include/tridsk.h)."""
+    _fields_ = [("n_res", C.c_int), ("res_off", C.c_void_p), ("res_xyz", C.c_void_p), ("K", C.c_int), ("pi", C.c_void_p),
+                ("mu", C.c_void_p), ("sigma", C.c_void_p), ("w_mdn", C.c_float), ("d_cut", C.c_float)]
+
+
 class _DockOpts(C.Structure):
     _fields_ = [("first_step", C.c_int), ("init_poses", C.c_void_p), ("resume", C.c_int),
                 ("chain_state", C.c_void_p), ("trace", C.c_void_p), ("steps_per_launch", C.c_int),
@@ -254,6 +260,20 @@ class Engine:
         h = C.c_void_p()
         self._ck(lib().tridsk_load_ligands(self.ctx, C.byref(b), C.byref(ty), C.byref(h)))
         return Ligands(self, h)
+
+    def load_mdn(self, ligs: Ligands, res_xyz, res_off, pi, mu, sigma, K, w_mdn=1.0, d_cut=5.0):
+        """Attach the mixture-density term (tridsk_load_mdn) to a ligand batch.  res_xyz [n_at,3], res_off [n_res+1]: host;
+        pi, mu, sigma: flat float32 arrays (numpy, or torch tensors on the host or the device), ligand-major blocks
+        [n_res][n_atoms(l)][K] in the caller's atom order."""
+        A = lambda a, dt: np.ascontiguousarray(a, dt)
+        xyz, off = A(res_xyz, np.float32), A(res_off, np.int32)
+        par = [A(a, np.float32).reshape(-1) if isinstance(a, np.ndarray) else a.contiguous().reshape(-1) for a in (pi, mu, sigma)]
+        m = _Mdn(len(off) - 1, off.ctypes.data, xyz.ctypes.data, int(K), _ptr(par[0]), _ptr(par[1]), _ptr(par[2]), float(w_mdn), float(d_cut))
+        self._sync_in()
+        self._ck(lib().tridsk_load_mdn(self.ctx, ligs.handle, C.byref(m)))
+
+    def unload_mdn(self, ligs: Ligands):
+        self._ck(lib().tridsk_load_mdn(self.ctx, ligs.handle, None))
 
     # ------------------------------------------------------------------ score + gradient
     def score_grad(self, grid: Grid, ligs: Ligands, params, lig_index, poses, want_grad=True, want_coords=True):

@@ -10,8 +10,8 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtridsk.so")
-SOURCES = ["api.cu", "mc_kernel.cu", "mc_lane.cu", "mc_cta.cu", "grid_build.cu", "topk.cu", "score_direct.cu", "microbench.cu"]
-HEADERS = ["internal.h", "chain.cuh", os.path.join("..", "..", "include", "tridsk.h")]
+SOURCES = ["api.cu", "mc_kernel.cu", "mc_lane.cu", "mc_cta.cu", "grid_build.cu", "topk.cu", "score_direct.cu", "microbench.cu", "mdn.cu"]
+HEADERS = ["internal.h", "chain.cuh", "mdn.cuh", os.path.join("..", "..", "include", "tridsk.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC,-fopenmp", "--expt-relaxed-constexpr"]
 

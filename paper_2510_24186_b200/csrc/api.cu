@@ -707,8 +707,74 @@ extern "C" int tridsk_ligand_info(const tridsk_ligands* l, int* n_lig, int* max_
     return TRIDSK_OK;
 }
 
+// ---------------------------------------------------------------------------------------- E_MDN (O15)
+static void free_mdn(tridsk_ligands* l) {
+    for (int i = 0; i < 5; ++i) { if (l->mdn_buf[i]) cudaFree(l->mdn_buf[i]); l->mdn_buf[i] = nullptr; }
+    memset(&l->mdn, 0, sizeof(l->mdn));
+}
+
+extern "C" int tridsk_load_mdn(tridsk_ctx* ctx, tridsk_ligands* ligs, const tridsk_mdn* m) {
+    if (!ctx || !ligs) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    NvtxRange nvtx_("tridsk_load_mdn");
+    CK(cudaStreamSynchronize(ctx->stream));               // earlier work may still read the old term
+    free_mdn(ligs);
+    if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; ctx->graph_key.clear(); }
+    if (!m) return TRIDSK_OK;
+    if (m->n_res < 1 || m->K < 1 || !m->res_off || !m->res_xyz || !m->pi || !m->mu || !m->sigma) return fail(ctx, TRIDSK_EINVAL, "bad mixture-density term");
+    if (!(m->d_cut > 0.f) || !std::isfinite(m->d_cut) || !std::isfinite(m->w_mdn)) return fail(ctx, TRIDSK_EINVAL, "bad w_mdn / d_cut");
+    for (int i = 0; i < m->n_res; ++i) if (m->res_off[i + 1] < m->res_off[i] || m->res_off[0] != 0) return fail(ctx, TRIDSK_EINVAL, "res_off must start at 0 and be non-decreasing");
+    const int L = ligs->n_lig, n_at = m->res_off[m->n_res];
+    if (L == 0) return TRIDSK_OK;
+    std::vector<long long> off(L);
+    long long total = 0;
+    for (int l = 0; l < L; ++l) { off[l] = total; total += (long long)m->n_res * ligs->hdr_h[l].n * m->K; }
+    cudaError_t e = cudaMalloc(&ligs->mdn_buf[0], sizeof(float4) * m->n_res);
+    if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[1], sizeof(int) * (m->n_res + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[2], sizeof(float4) * std::max(n_at, 1));
+    if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[3], sizeof(float4) * (size_t)total);
+    if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[4], sizeof(long long) * L);
+    // staging: residue coordinates, and the three parameter arrays when they live on the host
+    float* d_xyz = nullptr;
+    int* d_bad = nullptr;
+    float* stage[3] = {nullptr, nullptr, nullptr};
+    const float* src[3] = {m->pi, m->mu, m->sigma};
+    if (e == cudaSuccess) e = cudaMalloc((void**)&d_xyz, sizeof(float) * 3 * std::max(n_at, 1) + 16);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&d_bad, sizeof(int));
+    for (int a = 0; a < 3 && e == cudaSuccess; ++a)
+        if (!is_device_ptr(src[a])) {
+            e = cudaMalloc((void**)&stage[a], sizeof(float) * (size_t)total);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(stage[a], src[a], sizeof(float) * (size_t)total, cudaMemcpyHostToDevice, ctx->stream);
+            src[a] = stage[a];
+        }
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_bad, 0, sizeof(int), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_xyz, m->res_xyz, sizeof(float) * 3 * n_at, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ligs->mdn_buf[1], m->res_off, sizeof(int) * (m->n_res + 1), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ligs->mdn_buf[4], off.data(), sizeof(long long) * L, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = launch_mdn_spheres(ctx->stream, d_xyz, (const int*)ligs->mdn_buf[1], m->n_res, m->d_cut, (float4*)ligs->mdn_buf[2], (float4*)ligs->mdn_buf[0]);
+    if (e == cudaSuccess) e = launch_mdn_pack(ctx->stream, ligs->hdr, ligs->atom_i, L, m->n_res, m->K, (const long long*)ligs->mdn_buf[4], src[0], src[1], src[2],
+                                              m->w_mdn, (float4*)ligs->mdn_buf[3], d_bad);
+    int bad = 0;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d_xyz); cudaFree(d_bad);
+    for (int a = 0; a < 3; ++a) if (stage[a]) cudaFree(stage[a]);
+    ctx->launches += 2;
+    if (e != cudaSuccess) {
+        free_mdn(ligs);
+        return fail(ctx, e == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA, std::string("load_mdn: ") + cudaGetErrorString(e));
+    }
+    if (bad) { free_mdn(ligs); return fail(ctx, TRIDSK_EINVAL, "mixture parameters: sigma must be > 0 and every value finite"); }
+    ligs->mdn.n_res = m->n_res; ligs->mdn.K = m->K; ligs->mdn.d_cut = m->d_cut;
+    ligs->mdn.sph = (const float4*)ligs->mdn_buf[0]; ligs->mdn.res_off = (const int*)ligs->mdn_buf[1];
+    ligs->mdn.rec = (const float4*)ligs->mdn_buf[2]; ligs->mdn.par = (const float4*)ligs->mdn_buf[3];
+    ligs->mdn.lig_off = (const long long*)ligs->mdn_buf[4];
+    return TRIDSK_OK;
+}
+
 extern "C" void tridsk_free_ligands(tridsk_ligands* l) {
     if (!l) return;                 // cudaFree waits for the device; l->ctx may already be destroyed
+    free_mdn(l);
     cudaFree(l->hdr); cudaFree(l->atom_f4); cudaFree(l->atom_i); cudaFree(l->frags); cudaFree(l->rounds);
     cudaFree(l->lane_frags); cudaFree(l->lane_stream); cudaFree(l->lane_recs); cudaFree(l->cta_rows); cudaFree(l->cta_recs); cudaFree(l->all_ids);
     for (int k = 0; k < 2; ++k) if (l->cta_bucket_dev[k]) cudaFree(l->cta_bucket_dev[k]);
@@ -741,6 +807,7 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
     a.lane_frags = ligs->lane_frags; a.lane_stream = ligs->lane_stream; a.lane_recs = ligs->lane_recs;
     a.cta_rows = ligs->cta_rows; a.cta_recs = ligs->cta_recs;
     a.grid = grid->d;
+    a.mdn = ligs->mdn;
     to_dparams(params, &a.P);
     a.n_pose = n_pose; a.pose_stride = pose_stride; a.grad_stride = grad_stride; a.coord_stride = coord_stride;
     const size_t b_li = sizeof(int) * n_pose, b_po = sizeof(float) * (size_t)n_pose * pose_stride;
@@ -1021,6 +1088,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     base.lane_frags = ligs->lane_frags; base.lane_stream = ligs->lane_stream; base.lane_recs = ligs->lane_recs;
     base.cta_rows = ligs->cta_rows; base.cta_recs = ligs->cta_recs;
     base.grid = grid->d;
+    base.mdn = ligs->mdn;
     to_dparams(params, &base.P);
     for (int c = 0; c < 3; ++c) { base.box_min[c] = box_min[c]; base.box_max[c] = box_max[c]; base.centre[c] = pocket_center[c]; }
     base.radius = pocket_radius;
@@ -1044,6 +1112,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
             return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
     }
     const bool lane = mode == 2 || mode == 4;
+    if (mode == 4 && ligs->mdn.n_res > 0) return fail(ctx, TRIDSK_EINVAL, "the tensor-memory mapping (4) does not evaluate the mixture-density term");
     ctx->last_kernel = mode;
     tridsk_ligands* lg = const_cast<tridsk_ligands*>(ligs);
     if (lane) { int rc = lane_plan(ctx, lg, n_chains, params->n_refine); if (rc) return rc; }

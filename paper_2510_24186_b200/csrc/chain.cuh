@@ -9,6 +9,7 @@
 // P:N = PAPER.md line N; O*/G* = DESIGN.md section 3.
 #pragma once
 #include "internal.h"
+#include "mdn.cuh"
 
 #define FULL_MASK 0xffffffffu
 #define PI_F 3.14159265358979323846f
@@ -298,8 +299,10 @@ __device__ __forceinline__ float pair_energy(const DParams& P, float d2, float d
 // Out: world coordinates x/y/z[J]; per-lane partial energies e_inter / e_intra (warp_sum them);
 //      GRAD: gt[3] = dE/dt, gw[3] = dE/domega (uniform), gth = dE/dtheta on lane f (O9).
 // sP : per-warp shared scratch, 6 * J * 32 floats.
+// M.n_res > 0: the mixture-density term (mdn.cuh) of every atom is added to its receptor term; mdn_par = the ligand's block.
 template <int J, bool GRAD>
 __device__ __forceinline__ void eval_pose(const Lig<J>& L, const DGrid& G, const DParams& P,
+                                          const MdnDev& M, const float4* __restrict__ mdn_par,
                                           const float t[3], const float q[4], float theta,
                                           float x[J], float y[J], float z[J],
                                           float& e_inter, float& e_intra,
@@ -359,6 +362,7 @@ __device__ __forceinline__ void eval_pose(const Lig<J>& L, const DGrid& G, const
     for (int j = 0; j < J; ++j) {
         fx[j] = fy[j] = fz[j] = 0.f;
         if (L.valid[j]) e_inter += grid_interp<GRAD>(G, P.k_wall, L.typ[j], x[j], y[j], z[j], fx[j], fy[j], fz[j]);
+        if (M.n_res > 0 && L.valid[j]) mdn_atom(M, mdn_par, L.n, j * L.S + lane, x[j], y[j], z[j], 0, 1, GRAD, e_inter, fx[j], fy[j], fz[j]);
     }
 
     // ---- a5 intra-ligand pairs: conflict-free rotation schedule, partner data by shuffle, reaction force shuffled back

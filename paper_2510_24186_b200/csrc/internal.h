@@ -38,6 +38,17 @@ struct DGrid {
     float ox, oy, oz, h, inv_h;
 };
 
+// The mixture-density term (mdn.cuh, O15) attached to a ligand batch; n_res == 0: absent.
+struct MdnDev {
+    int n_res, K;
+    const float4* sph;            // [n_res] bounding sphere of a residue: centre, (radius + d_cut)^2
+    const int* res_off;           // [n_res + 1] into rec
+    const float4* rec;            // residue atoms {x, y, z, 0}
+    const float4* par;            // packed parameters {a, mu, nk2, 1/sigma^2}, ligand-major, [n_res][n][K] per ligand, INTERNAL atom order
+    const long long* lig_off;     // [n_lig] start of a ligand's block in par (float4 units)
+    float d_cut;
+};
+
 // Per-ligand header.  Atoms are stored in an INTERNAL order (depth-first over the torsion tree) so that
 // the atoms of every torsion's subtree are one contiguous index range; lane l of a chain's warp owns
 // atoms a = j*S + l, j < J ("stripes").
@@ -139,6 +150,7 @@ struct McLaunch {
     int trace_stride, trace_off;
     int lane_region, tm_cols;     // tensor-memory lane kernel: shared-memory bytes per warp, TMEM columns per CTA
     int lane_minb;                // shared-memory lane kernel: register budget class (launch_bounds min blocks)
+    MdnDev mdn;                   // n_res == 0: no mixture-density term
 };
 
 struct ScoreLaunch {
@@ -164,6 +176,7 @@ struct ScoreLaunch {
     float* energy;                // [n_pose][3]
     float* grad; int grad_stride;
     float* coords; int coord_stride;
+    MdnDev mdn;
 };
 
 struct TopkLaunch {
@@ -285,6 +298,9 @@ struct tridsk_ligands {
     std::vector<int> lane_ids_h;  // host copy behind all_ids (must outlive the async upload)
     long long lane_plan_key = -1; // n_chains << 8 | (n_refine > 1)
     int* bucket_dev[TRIDSK_MAX_J + 1] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    // the mixture-density term (tridsk_load_mdn); mdn.n_res == 0: absent
+    MdnDev mdn = {};
+    void* mdn_buf[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // sph, res_off, rec, par, lig_off
 };
 
 // ---------------------------------------------------------------- kernel launchers (one per .cu)
@@ -310,5 +326,8 @@ cudaError_t launch_score_direct(cudaStream_t s, const LigHdr* hdr, const float4*
                                 const unsigned char* role, const DParams& P, const int* lig_index, const float* poses, int n_pose,
                                 int pose_stride, float* energy, float* grad, int grad_stride, int max_atoms);
 size_t topk_cluster_smem(int top_k, int max_atoms, int max_tor);
+cudaError_t launch_mdn_spheres(cudaStream_t s, const float* res_xyz, const int* res_off, int n_res, float d_cut, float4* rec, float4* sph);
+cudaError_t launch_mdn_pack(cudaStream_t s, const LigHdr* hdr, const int* atom_i, int n_lig, int n_res, int K, const long long* lig_off,
+                            const float* pi, const float* mu, const float* sigma, float w_mdn, float4* par, int* bad);
 cudaError_t launch_microbench(cudaStream_t s, int which, int sm_count, void* buf, size_t bytes, int iters, float* sink, double* work);
 cudaError_t launch_philox_debug(cudaStream_t s, const unsigned int* ctr_key /* dev[6] */, unsigned int* out /* dev[4] */);

@@ -14,6 +14,7 @@
 //
 // P:N = PAPER.md line N; O*/G* = DESIGN.md section 3.
 #include "chain.cuh"
+#include "mdn.cuh"
 
 struct CtaTopo {
     const float4* ref;      // [n] {ref x, y, z, vdW radius}, internal (depth-first) atom order
@@ -157,8 +158,11 @@ __device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], co
 // In : t[3], unit q[4] (uniform), theta (lane g holds the torsion angle of fragment g).
 // Out: ENERGY: e_inter, e_intra (uniform over the CTA); GRAD: g6 = {dE/dt, dE/domega about t} (uniform), gth = dE/dtheta
 //      on lane g (O9); x, y, z = this thread's atom (valid when `active`).
-template <bool GRAD, bool ENERGY>
+// MDN: the mixture-density term (mdn.cuh); the lanes of an atom share its residues (lane `part` takes residues part,
+// part + lpa, ...), their shares join the pair force / the energy sums before the fixed-order reductions.
+template <bool GRAD, bool ENERGY, bool MDN>
 __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
+                                         const MdnDev& M, const float4* __restrict__ mdn_par,
                                          int max_depth, const float t[3], const float q[4], float theta,
                                          int atom, int part, bool active, float& x, float& y, float& z,
                                          float& e_inter, float& e_intra, float g6[6], float& gth) {
@@ -263,6 +267,11 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     // ---- a4 receptor term of this thread's atom (the gathers were issued before the barrier)
     float ei = 0.f, gx = 0.f, gy = 0.f, gz = 0.f;
     if (lead) ei = grid_blend<GRAD>(G, P.k_wall, cell, glo, ghi, gx, gy, gz);
+    if (MDN && active) {
+        float mx = 0.f, my = 0.f, mz = 0.f;
+        mdn_atom(M, mdn_par, n, atom, x, y, z, part, S.lpa, GRAD, ei, mx, my, mz);
+        if (GRAD) { fx = fmaf(mx, K.inv_kappa, fx); fy = fmaf(my, K.inv_kappa, fy); fz = fmaf(mz, K.inv_kappa, fz); }   // kappa units, like the pair force
+    }
     if (GRAD) {
         for (int o = S.lpa >> 1; o > 0; o >>= 1) {                  // the atom's lanes are adjacent: fixed-order tree
             fx += __shfl_xor_sync(FULL_MASK, fx, o);
@@ -360,6 +369,7 @@ __device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const Ct
 }
 
 // ------------------------------------------------------------------ the fused MC kernel, one CTA per chain
+template <bool MDN>
 __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -371,6 +381,7 @@ __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
     cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.P);
     const DParams& P = a.P;
     const PairK K = make_pairk(P);
+    const float4* mdn_par = MDN ? a.mdn.par + a.mdn.lig_off[lig] : nullptr;
     const int T = S.T, max_depth = h->max_depth;
     const int atom = tid / S.lpa, part = tid % S.lpa;
     const bool active = atom < S.n;
@@ -412,7 +423,7 @@ __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
             const float uu = (k & 3) == 0 ? v0 : (k & 3) == 1 ? v1 : (k & 3) == 2 ? v2 : v3;
             cth = F.tor >= 0 ? PI_F * (2.f * uu - 1.f) : 0.f;
         }
-        cta_eval<false, true>(S, a.grid, P, K, F, max_depth, ct, cq, cth, atom, part, active, x, y, z, ei, ea, g6, gth);
+        cta_eval<false, true, MDN>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, ct, cq, cth, atom, part, active, x, y, z, ei, ea, g6, gth);
         ecur = ei + ea;
         ebest = ecur;
 #pragma unroll
@@ -447,7 +458,7 @@ __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
         float m[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         float b1p = 1.f, b2p = 1.f;
         for (int rf = 0; rf < P.n_refine; ++rf) {
-            cta_eval<true, false>(S, a.grid, P, K, F, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
+            cta_eval<true, false, MDN>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
             b1p *= P.adam_b1; b2p *= P.adam_b2;
             const float c1 = __fdividef(1.f, 1.f - b1p), c2 = __fdividef(1.f, 1.f - b2p);
             float g[7] = {g6[0], g6[1], g6[2], g6[3], g6[4], g6[5], gth}, dl[7];
@@ -468,7 +479,7 @@ __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
         }
 
         // a8: energy of the refined proposal, Metropolis, best tracking
-        cta_eval<false, true>(S, a.grid, P, K, F, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
+        cta_eval<false, true, MDN>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
         const float enew = ei + ea;
         const bool accept = isfinite(enew) && (um < expf(-P.beta * (enew - ecur)));
         if (a.trace != nullptr && tid == 0) {
@@ -500,6 +511,7 @@ __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
 }
 
 // ------------------------------------------------------------------ tridsk_score_grad, CTA form: one CTA per pose
+template <bool MDN>
 __global__ void __launch_bounds__(256) score_cta_kernel(const ScoreLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -510,13 +522,14 @@ __global__ void __launch_bounds__(256) score_cta_kernel(const ScoreLaunch a) {
     CtaFrag F;
     cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.P);
     const PairK K = make_pairk(a.P);
+    const float4* mdn_par = MDN ? a.mdn.par + a.mdn.lig_off[lig] : nullptr;
     const int atom = tid / S.lpa, part = tid % S.lpa;
     const bool active = atom < S.n;
     float t[3], q[4], th, x, y, z, g6[6], gth = 0.f, ei, ea;
     cta_load_pose(a.poses + (size_t)i * a.pose_stride, F, t, q, th);
     quat_normalise(q);
-    if (a.grad != nullptr) cta_eval<true, true>(S, a.grid, a.P, K, F, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
-    else cta_eval<false, true>(S, a.grid, a.P, K, F, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
+    if (a.grad != nullptr) cta_eval<true, true, MDN>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
+    else cta_eval<false, true, MDN>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
     if (tid == 0) { a.energy[3 * (size_t)i] = ei + ea; a.energy[3 * (size_t)i + 1] = ei; a.energy[3 * (size_t)i + 2] = ea; }
     if (a.grad != nullptr && warp == 0) {
         float* g = a.grad + (size_t)i * a.grad_stride;
@@ -536,8 +549,10 @@ __global__ void __launch_bounds__(256) score_cta_kernel(const ScoreLaunch a) {
 
 // per device (function attributes are per device): called by tridsk_create
 cudaError_t mc_cta_prepare() {
-    cudaError_t e = cudaFuncSetAttribute(mc_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(score_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    cudaError_t e = cudaFuncSetAttribute(mc_cta_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(score_cta_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(score_cta_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
     return e;
 }
 
@@ -545,12 +560,14 @@ cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int threads, size_t
     const long long blocks = (long long)a.n_list * a.n_chains;
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL || (threads != 128 && threads != 256)) return cudaErrorInvalidValue;
-    mc_cta_kernel<<<(unsigned)blocks, threads, smem_bytes, s>>>(a);
+    if (a.mdn.n_res > 0) mc_cta_kernel<true><<<(unsigned)blocks, threads, smem_bytes, s>>>(a);
+    else mc_cta_kernel<false><<<(unsigned)blocks, threads, smem_bytes, s>>>(a);
     return cudaGetLastError();
 }
 
 cudaError_t launch_score_cta(cudaStream_t s, const ScoreLaunch& a, size_t smem_bytes) {
     if (a.n_pose <= 0) return cudaSuccess;
-    score_cta_kernel<<<a.n_pose, 256, smem_bytes, s>>>(a);
+    if (a.mdn.n_res > 0) score_cta_kernel<true><<<a.n_pose, 256, smem_bytes, s>>>(a);
+    else score_cta_kernel<false><<<a.n_pose, 256, smem_bytes, s>>>(a);
     return cudaGetLastError();
 }

@@ -20,6 +20,7 @@
 //
 // P:N = PAPER.md line N; O*/G* = DESIGN.md section 3.
 #include "chain.cuh"
+#include "mdn.cuh"
 
 struct LaneTopo {
     const float4* ref;      // [n] {ref x, y, z, vdW radius}
@@ -250,9 +251,10 @@ __device__ __forceinline__ float lane_blend(const DGrid& G, float k_wall, const 
 #ifndef LANE_GD
 #define LANE_GD 2     // measured on C5: 2 in flight 225 ms, 3: 238 ms, 4: 245 ms (8,192 ligands) -- the unrolled copies cost more
 #endif                // instruction-cache misses than the deeper prefetch saves
-template <class XS>
+// MDN: the mixture-density term of every atom (mdn.cuh) is added where its grid value is blended.
+template <bool MDN, class XS>
 __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, float k_wall, bool grad, float wscale,
-                                           const XS& X, float* __restrict__ WR) {
+                                           const MdnDev& M, const float4* __restrict__ mdn_par, const XS& X, float* __restrict__ WR) {
     constexpr int C = XS::kC;
     const LaneGridK Q = {-G.ox * G.inv_h, -G.oy * G.inv_h, -G.oz * G.inv_h};
     float e_inter = 0.f;
@@ -289,6 +291,12 @@ __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, fl
             if (a0 + k < n) {                                   // blend atom a0 + k
                 float gx, gy, gz;
                 e_inter += lane_blend(G, k_wall, c[k], lo[k], hi[k], grad, x[k], y[k], z[k], gx, gy, gz);
+                if (MDN) {
+                    float me = 0.f, mx = 0.f, my = 0.f, mz = 0.f;
+                    mdn_atom(M, mdn_par, n, a0 + k, x[k], y[k], z[k], 0, 1, grad, me, mx, my, mz);
+                    e_inter += me;
+                    if (grad) { gx = fmaf(mx, G.h, gx); gy = fmaf(my, G.h, gy); gz = fmaf(mz, G.h, gz); }   // grid units, like the blend
+                }
                 if (grad) {
                     if ((m[k] & 0x100) && a0 + k > 0) {        // first own atom of the next fragment: the previous one is complete
 #pragma unroll
@@ -466,12 +474,13 @@ __device__ __forceinline__ float lane_pairs(const LaneTopo& S, const PairK& K, c
 // In : t[3], unit q[4] (registers), th[(g-1)*C] torsion angles (shared), grad (warp-uniform).
 // Out: X (world coordinates), e_inter, e_intra (e_intra of a gradient evaluation only if GE); grad: WR[g] = wrench on the
 //      own atoms of fragment g in kappa units (1 / K.kappa of the true wrench).
-template <bool GE, class XS>
+template <bool GE, bool MDN, class XS>
 __device__ __forceinline__ void lane_eval(const LaneTopo& S, const DGrid& G, const DParams& P, const PairK& K, bool grad,
+                                          const MdnDev& M, const float4* __restrict__ mdn_par,
                                           const float t[3], const float q[4], const float* __restrict__ th,
                                           const XS& X, float* __restrict__ WR, float& e_inter, float& e_intra) {
     lane_fk(S, t, q, th, X, WR);
-    e_inter = lane_grid(S, G, P.k_wall, grad, G.inv_h * K.inv_kappa, X, WR);
+    e_inter = lane_grid<MDN>(S, G, P.k_wall, grad, G.inv_h * K.inv_kappa, M, mdn_par, X, WR);
     e_intra = grad ? lane_pairs<true, GE, XS>(S, K, X, WR) : lane_pairs<false, true, XS>(S, K, X, WR);
 }
 
@@ -513,7 +522,7 @@ __device__ __forceinline__ void lane_backward(const LaneTopo& S, const float t[3
 // ------------------------------------------------------------------ one chain, start to finish, by one lane
 // `live` = false for the padding lanes of a partial warp: they run a copy of the last chain (tensor-memory moves are
 // warp-collective) and write nothing.
-template <class XS>
+template <bool MDN, class XS>
 __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S, int lig, int chain, bool live, int max_depth,
                                            const XS& X, float* __restrict__ WR, float* __restrict__ THC, float* __restrict__ THP,
                                            float* __restrict__ MV) {
@@ -521,6 +530,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
     const DParams& P = a.P;
     const PairK K = make_pairk(P);
     const int T = S.T;
+    const float4* mdn_par = MDN ? a.mdn.par + a.mdn.lig_off[lig] : nullptr;
     const size_t cidx = (size_t)lig * a.n_chains + chain;
     const uint2 key = make_uint2((uint32_t)a.seed, (uint32_t)(a.seed >> 32));
     const uint32_t gchain = (uint32_t)(a.chain_base + chain);
@@ -606,7 +616,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
         for (int rf = (s >= 0 ? 0 : P.n_refine); rf <= P.n_refine; ++rf) {
             const bool grad = rf < P.n_refine;
             float ei, ea;
-            lane_eval<false>(S, a.grid, P, K, grad, pt, pq, THP, X, WR, ei, ea);   // the Adam steps need no energy
+            lane_eval<false, MDN>(S, a.grid, P, K, grad, a.mdn, mdn_par, pt, pq, THP, X, WR, ei, ea);   // the Adam steps need no energy
             enew = ei + ea;
             if (!grad) break;
             b1p *= P.adam_b1; b2p *= P.adam_b2;
@@ -682,7 +692,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
 // MINB = resident 128-thread CTAs per SM the register budget must allow (3: 168 registers, 2: 255): the host picks 255 for
 // the size buckets whose shared-memory need keeps at most 8 warps per SM resident anyway, 168 (12 warps) for the rest --
 // measured: 12 warps at 168 registers beat 16 warps at 128 (C5 1885 -> 1824 ms), 8 warps at 255 do not (1917 ms).
-template <int MINB, int C>
+template <int MINB, int C, bool MDN>
 __global__ void __launch_bounds__(128, MINB) mc_lane_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char lane_smem[];
     const int tid = threadIdx.x;
@@ -703,7 +713,7 @@ __global__ void __launch_bounds__(128, MINB) mc_lane_kernel(const McLaunch a) {
     float* THC = WR + lane_wslots(T, max_depth) * C;          // current accepted torsions, by pre-order fragment g - 1
     float* THP = THC + T * C;                                 // proposal
     float* MV = THP + T * C;                                  // torsion Adam moments {m, v} (n_refine > 1 only)
-    lane_chain(a, S, lig, chain, true, max_depth, X, WR, THC, THP, MV);
+    lane_chain<MDN>(a, S, lig, chain, true, max_depth, X, WR, THC, THP, MV);
 }
 
 // Coordinates in tensor memory: one CTA = 4 warps, every WARP takes its own work item (ligand, block of 32 chains) and
@@ -743,7 +753,7 @@ __global__ void __launch_bounds__(128, 3) mc_lane_tm_kernel(const McLaunch a) {
         float* THC = WR + lane_wslots(T, max_depth) * C;
         float* THP = THC + T * C;
         float* MV = THP + T * C;
-        lane_chain(a, S, lig, chain, live, max_depth, X, WR, THC, THP, MV);
+        lane_chain<false>(a, S, lig, chain, live, max_depth, X, WR, THC, THP, MV);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -754,38 +764,43 @@ __global__ void __launch_bounds__(128, 3) mc_lane_tm_kernel(const McLaunch a) {
     }
 }
 
-__global__ void score_lane_kernel(const ScoreLaunch a);
+template <bool MDN> __global__ void score_lane_kernel(const ScoreLaunch a);
 
 // Opt-in shared-memory sizes are per device and per function: done once per device (tridsk_create -> mc_lane_prepare).
-template <int MINB, int C>
+template <int MINB, int C, bool MDN>
 static cudaError_t lane_prepare_one(size_t max_smem_bytes) {
-    cudaError_t e = cudaFuncSetAttribute(mc_lane_kernel<MINB, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
+    cudaError_t e = cudaFuncSetAttribute(mc_lane_kernel<MINB, C, MDN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
     // residency is bound by shared memory (the chains' coordinates): take the whole 228 KB, the grid gathers live in L2 anyway
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<MINB, C>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_kernel<MINB, C, MDN>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     return e;
 }
 cudaError_t mc_lane_prepare(size_t max_smem_bytes) {
-    cudaError_t e = lane_prepare_one<3, 32>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<3, 64>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<3, 96>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<3, 128>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<2, 32>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<2, 64>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<2, 96>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<2, 128>(max_smem_bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(score_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
+    cudaError_t e = lane_prepare_one<3, 32, false>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<3, 64, false>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<3, 96, false>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<3, 128, false>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 32, false>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 64, false>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 96, false>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 128, false>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<3, 32, true>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<3, 64, true>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<3, 96, true>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<3, 128, true>(max_smem_bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(score_lane_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(score_lane_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_tm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes - 1024);   // it has 16 static bytes
     if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_tm_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     return e;
 }
 
-template <int MINB>
+template <int MINB, bool MDN>
 static void lane_launch_c(cudaStream_t s, const McLaunch& a, unsigned blocks, int c, size_t smem_bytes) {
     switch (c) {
-        case 32: mc_lane_kernel<MINB, 32><<<blocks, 32, smem_bytes, s>>>(a); break;
-        case 64: mc_lane_kernel<MINB, 64><<<blocks, 64, smem_bytes, s>>>(a); break;
-        case 96: mc_lane_kernel<MINB, 96><<<blocks, 96, smem_bytes, s>>>(a); break;
-        default: mc_lane_kernel<MINB, 128><<<blocks, 128, smem_bytes, s>>>(a); break;
+        case 32: mc_lane_kernel<MINB, 32, MDN><<<blocks, 32, smem_bytes, s>>>(a); break;
+        case 64: mc_lane_kernel<MINB, 64, MDN><<<blocks, 64, smem_bytes, s>>>(a); break;
+        case 96: mc_lane_kernel<MINB, 96, MDN><<<blocks, 96, smem_bytes, s>>>(a); break;
+        default: mc_lane_kernel<MINB, 128, MDN><<<blocks, 128, smem_bytes, s>>>(a); break;
     }
 }
 cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta, size_t smem_bytes, int minb) {
@@ -793,8 +808,9 @@ cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta
     const long long blocks = (long long)a.n_list * cpl;
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL || chains_per_cta < 32 || chains_per_cta > 128 || (chains_per_cta & 31)) return cudaErrorInvalidValue;
-    if (minb == 2) lane_launch_c<2>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);
-    else lane_launch_c<3>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);
+    if (a.mdn.n_res > 0) lane_launch_c<3, true>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);   // one register class with the term
+    else if (minb == 2) lane_launch_c<2, false>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);
+    else lane_launch_c<3, false>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);
     return cudaGetLastError();
 }
 
@@ -809,6 +825,7 @@ cudaError_t launch_mc_lane_tm(cudaStream_t s, const McLaunch& a) {
 
 // ------------------------------------------------------------------ tridsk_score_grad, lane form: one lane per pose
 // One 32-thread CTA takes up to 32 poses of one ligand (the host groups poses by ligand: seg_*, perm).
+template <bool MDN>
 __global__ void __launch_bounds__(32) score_lane_kernel(const ScoreLaunch a) {
     extern __shared__ __align__(16) unsigned char lane_smem[];
     constexpr int C = 32;
@@ -832,7 +849,7 @@ __global__ void __launch_bounds__(32) score_lane_kernel(const ScoreLaunch a) {
     quat_normalise(q);
     for (int g = 1; g <= T; ++g) TH[(g - 1) * C] = src[7 + S.frag[g].tor];
     float ei, ea;
-    lane_eval<true>(S, a.grid, a.P, K, a.grad != nullptr, t, q, TH, X, WR, ei, ea);
+    lane_eval<true, MDN>(S, a.grid, a.P, K, a.grad != nullptr, a.mdn, MDN ? a.mdn.par + a.mdn.lig_off[lig] : nullptr, t, q, TH, X, WR, ei, ea);
     a.energy[3 * (size_t)i] = ei + ea; a.energy[3 * (size_t)i + 1] = ei; a.energy[3 * (size_t)i + 2] = ea;
     if (a.grad != nullptr) {
         float* gr = a.grad + (size_t)i * a.grad_stride;
@@ -854,6 +871,7 @@ __global__ void __launch_bounds__(32) score_lane_kernel(const ScoreLaunch a) {
 
 cudaError_t launch_score_lane(cudaStream_t s, const ScoreLaunch& a, int n_seg, size_t smem_bytes) {
     if (n_seg <= 0) return cudaSuccess;
-    score_lane_kernel<<<n_seg, 32, smem_bytes, s>>>(a);
+    if (a.mdn.n_res > 0) score_lane_kernel<true><<<n_seg, 32, smem_bytes, s>>>(a);
+    else score_lane_kernel<false><<<n_seg, 32, smem_bytes, s>>>(a);
     return cudaGetLastError();
 }

@@ -761,3 +761,111 @@ def test_extreme_ligand_sizes_under_every_mapping(orc, gp, mode):
                 assert close(r["energy"][l, k, 0], eo, rtol=2e-4, atol=2e-3), (mode, L.n, L.T)
     finally:
         e.close()
+
+
+# ------------------------------------------------------------------------------------------- E_MDN (O15)
+def _mdn_system(orc, eng, S, lig_ids, K, seed):
+    """Synthetic residues (groups of 8 receptor atoms) and mixture parameters for a sub-batch of the test ligands; the term
+    attached on both sides."""
+    rec = S["rec"]
+    order, res_off = synth.residues(rec, 8)
+    rxyz = rec.xyz[order].astype(np.float32)
+    b = S["batch"].subset(lig_ids)
+    ligs = eng.load_ligands(b, S["radius"], S["role"])
+    Ls, blocks = [], [[], [], []]
+    for k, li in enumerate(lig_ids):
+        L = orc.ligand_from_batch(S["batch"], li)
+        pi, mu, sg = synth.gmm_params(len(res_off) - 1, L.n, K, seed=seed + k)
+        L.set_mdn(orc.Mdn(rxyz, res_off, pi, mu, sg, w_mdn=1.0, d_cut=5.0))
+        Ls.append(L)
+        for dst, a in zip(blocks, (pi, mu, sg)):
+            dst.append(a.reshape(-1))
+    pi, mu, sg = (np.concatenate(v) for v in blocks)
+    eng.load_mdn(ligs, rxyz, res_off, pi, mu, sg, K)
+    return b, ligs, Ls
+
+
+def test_mdn_score_grad_matches_oracle(orc, eng, gp, system):
+    """The full Eq.E_dock per pose: energy (rel 1e-4 / abs 1e-3) and gradient against the oracle with the term
+    attached; detaching it gives back the physics-only numbers."""
+    S = system
+    ids = [0, 1, 4, 6, 10, 12]                                   # 12 .. 80 atoms, rigid and deep trees
+    b, ligs, Ls = _mdn_system(orc, eng, S, ids, K=5, seed=100)
+    li = np.repeat(np.arange(len(ids), dtype=np.int32), 8)
+    poses = synth.random_poses(b, li, S["rec"], seed=15, spread=0.6)
+    e, g, x = eng.score_grad(S["g_grid"], ligs, gp, li, poses)
+    w_e = w_g = 0.0
+    n_with = 0
+    for i in range(len(li)):
+        L = Ls[li[i]]
+        eo, go, xo, _ = orc.score_grad(S["p"], S["ty"], S["G"], L, poses[i, :7 + L.T].astype(np.float64))
+        Em = orc.mdn_energy(L.mdn.res_xyz, L.mdn.res_off, L.mdn.pi, L.mdn.mu, L.mdn.sigma, xo)[0]
+        n_with += Em < -1e-3
+        assert close(e[i], eo), (i, li[i], e[i], eo)
+        sc = np.abs(go).max()
+        assert close(g[i, :6 + L.T], go, scale=sc), (i, li[i], worst(g[i, :6 + L.T], go, scale=sc))
+        w_e = max(w_e, worst(e[i], eo)); w_g = max(w_g, worst(g[i, :6 + L.T], go, scale=sc))
+    assert n_with > 0.8 * len(li)                                # the term really contributes on these poses
+    print(f"E_MDN worst/tolerance: energy {w_e:.3f} grad {w_g:.3f}")
+    # detach: physics only
+    eng.unload_mdn(ligs)
+    e2, _, _ = eng.score_grad(S["g_grid"], ligs, gp, li, poses, want_grad=False, want_coords=False)
+    for i in range(0, len(li), 5):
+        L = Ls[li[i]]
+        m = L.mdn
+        L.set_mdn(None)
+        eo = orc.score_grad(S["p"], S["ty"], S["G"], L, poses[i, :7 + L.T].astype(np.float64), want_grad=False)[0]
+        L.set_mdn(m)
+        assert close(e2[i], eo)
+    ligs.free()
+
+
+def test_mdn_teacher_forced_steps_match_oracle(orc, eng, gp, system):
+    """Chains sampled under the full score: teacher-forced MC steps against orc_mc_step with the term attached."""
+    from paper_2510_24186_b200 import split_state
+    S = system
+    ids = [1, 0, 4]
+    b, ligs, Ls = _mdn_system(orc, eng, S, ids, K=4, seed=300)
+    n_chains, seed, stride = 32, 17, 7 + ligs.max_tor
+    r = eng.dock(S["g_grid"], ligs, gp, *_dock_args(S), n_chains, 0, 1, seed=seed, want_state=True)
+    state = r["state"]
+    compared = skipped = 0
+    for s in range(6):
+        pc, _, ec, _ = split_state(state.copy(), len(ids), n_chains, stride)
+        r = eng.dock(S["g_grid"], ligs, gp, *_dock_args(S), n_chains, 1, 1, seed=seed, first_step=s, resume=True,
+                     chain_state=state, want_trace=True)
+        for l, L in enumerate(Ls):
+            for c in range(0, n_chains, 2):
+                tr = r["trace"][l, c, 0]
+                pose = pc[l, c, :7 + L.T].astype(np.float64)
+                e_cur = orc.score_grad(S["p"], S["ty"], S["G"], L, pose, want_grad=False)[0][0]
+                assert close(ec[l, c], e_cur, rtol=1e-4, atol=1e-3), (s, l, c, ec[l, c], e_cur)
+                _, _, rec = orc.mc_step(S["p"], S["ty"], S["G"], L, seed, c, s, l, S["rec"].box_min, S["rec"].box_max, pose, e_cur)
+                assert (tr["flags"] >> 8) == rec.entity and tr["u"] == np.float32(rec.u)
+                if rec.min_abs_g < 1e-3 or abs(rec.u - rec.p_accept) < 1e-4 * max(1.0, rec.p_accept):
+                    skipped += 1
+                    continue
+                compared += 1
+                assert close(tr["e_prop"], rec.e_prop, rtol=1e-3, atol=1e-3), (s, l, c, tr["e_prop"], rec.e_prop)
+                assert (tr["flags"] & 1) == rec.accept, (s, l, c)
+    print(f"E_MDN teacher-forced: compared {compared}, skipped {skipped}")
+    assert compared > 0.85 * 6 * 3 * 16
+    ligs.free()
+
+
+def test_mdn_error_paths(eng, system):
+    from paper_2510_24186_b200 import TridskError
+    S = system
+    b = S["batch"].subset([0])
+    ligs = eng.load_ligands(b, S["radius"], S["role"])
+    order, res_off = synth.residues(S["rec"], 8)
+    rxyz = S["rec"].xyz[order].astype(np.float32)
+    pi, mu, sg = synth.gmm_params(len(res_off) - 1, 12, 3, seed=1)
+    bad = sg.copy(); bad[0, 0, 0] = 0.0
+    with pytest.raises(TridskError) as ei:
+        eng.load_mdn(ligs, rxyz, res_off, pi, mu, bad, 3)
+    assert ei.value.code == -1
+    with pytest.raises(TridskError):
+        eng.load_mdn(ligs, rxyz, res_off, pi, mu, sg, 3, d_cut=0.0)
+    eng.load_mdn(ligs, rxyz, res_off, pi, mu, sg, 3)             # a good one after the failures
+    ligs.free()
