@@ -35,12 +35,12 @@ UNIT = "score+grad pose evals/s"
 KERNEL_NAMES = {1: "mc_kernel<J> (warp per chain)", 2: "mc_lane_kernel (lane per chain)", 3: "mc_cta_kernel (CTA per chain)",
                 4: "mc_lane_tm_kernel (lane per chain, TMEM)"}
 REGIME = {"C1": "latency", "C2": "latency", "C3": "throughput", "C4": "throughput", "C5": "throughput", "C2x32": "throughput",
-          "P1": "latency"}
+          "P1": "latency", "M3": "throughput"}
 MB_FFMA, MB_FFMA2, MB_MUFU, MB_L2_READ, MB_GATHER = range(5)
 
 
 # ----------------------------------------------------------------------------------------- accounting
-def work_of(n_atoms, n_tor, n_pairs, n_chains, n_steps, n_refine):
+def work_of(n_atoms, n_tor, n_pairs, n_chains, n_steps, n_refine, mdn=None):
     """Evaluations and ALGORITHMIC work of one step of a workload.  Two kinds of evaluation:
     G = score gradient (what an Adam step needs: FK, trilinear value + gradient, pair forces, reverse pass) and
     E = energy only (the Metropolis evaluation of a step, and the initial one).  Per MC step and chain: n_refine G
@@ -51,11 +51,18 @@ def work_of(n_atoms, n_tor, n_pairs, n_chains, n_steps, n_refine):
     flop_e = 16 * p + 66 * n + 110 * t         # pair: distance 8, Gaussian 5, clash 3; atom: trilinear value 45, FK 21
     flop_adam = 20 * d
     xu_g, xu_e, xu_step = 2.0 * p, 2.3 * p, 2 * d + 10
+    bytes_eval = 32 * n                        # 8 fp32 grid corners per atom per evaluation
+    if mdn:                                    # E_MDN: per (atom, residue within the cut-off): minimum over the residue's atoms (8 flop each),
+        hits, size, K = mdn["hits_per_atom"], mdn["res_size"], mdn["K"]            # then K Gaussians (value 8 flop, + derivative 4) and one sqrt
+        flop_g = flop_g + n * hits * (8 * size + 12 * K + 8)
+        flop_e = flop_e + n * hits * (8 * size + 8 * K)
+        xu_g, xu_e = xu_g + n * hits * (K + 1), xu_e + n * hits * (K + 1)
+        bytes_eval = bytes_eval + n * hits * (16 * K + 16 * size)
     g_per_chain = n_steps * n_refine
     e_per_chain = n_steps + 1
     per_chain_flop = g_per_chain * (flop_g + flop_adam) + e_per_chain * flop_e
     per_chain_xu = g_per_chain * xu_g + e_per_chain * xu_e + n_steps * xu_step
-    per_chain_bytes = (g_per_chain + e_per_chain) * 32 * n       # 8 fp32 grid corners per atom per evaluation
+    per_chain_bytes = (g_per_chain + e_per_chain) * bytes_eval
     ones = np.ones_like(n)
     return dict(evals=float(np.sum(n_chains * (g_per_chain + e_per_chain) * ones)), sg_evals=float(np.sum(n_chains * g_per_chain * ones)),
                 flop=float(np.sum(n_chains * per_chain_flop)), xu=float(np.sum(n_chains * per_chain_xu)),
@@ -202,7 +209,14 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
     d_xyz = torch.from_numpy(rec.xyz).to(eng.device)
     d_typ = torch.from_numpy(rec.type).to(eng.device)
     ligs = eng.load_ligands(batch, radius, role)
-    w = work_of(np.diff(batch.atom_off), np.diff(batch.tor_off), ligs.n_pairs, n_chains, cfg.n_steps, gp.n_refine)
+    mdn = None
+    if cfg.mdn_K:                                                            # the paper's full score: attach E_MDN (synthetic parameters)
+        res_xyz, res_off = synth.pocket_residues(rec)
+        pi, mu, sg = synth.gmm_batch(len(res_off) - 1, np.diff(batch.atom_off), cfg.mdn_K, seed=cfg.lig_seed + 50000)
+        eng.load_mdn(ligs, res_xyz, res_off, pi, mu, sg, cfg.mdn_K)
+        del pi, mu, sg
+        mdn = dict(K=cfg.mdn_K, n_res=len(res_off) - 1, res_size=float(np.mean(np.diff(res_off))))
+    w = work_of(np.diff(batch.atom_off), np.diff(batch.tor_off), ligs.n_pairs, n_chains, cfg.n_steps, gp.n_refine)   # evaluation counts
     L, k = ligs.n_lig, cfg.top_k
     out = (torch.empty(L, k, 2, device=eng.device), torch.empty(L, k, stride, device=eng.device),
            torch.empty(L, k, dtype=torch.int32, device=eng.device))
@@ -265,6 +279,21 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
         evals_all, sg_all = float(tot[0]), float(tot[1])
     else:
         evals_all, sg_all = w["evals"], w["sg_evals"]
+    if mdn:                                                                  # (atom, residue) pairs inside the cut-off: counted on returned poses
+        sample = list(range(0, L, max(1, L // 48)))[:48]
+        li = np.asarray(sample, np.int32)
+        poses = out[1][li, 0, :].contiguous().cpu().numpy()
+        gtmp = eng.build_grid(d_xyz, d_typ, radius, role, gp, rec.origin, rec.dims, rec.spacing)
+        _, _, xs = eng.score_grad(gtmp, ligs, gp, li, poses, want_grad=False)
+        gtmp.free()
+        hits = atoms = 0
+        for q, l in enumerate(sample):
+            nl = batch.n_atoms(l)
+            dmat = np.linalg.norm(xs[q, :nl, None, :] - res_xyz[None, :, :], axis=2)             # [atom][receptor atom]
+            dres = np.minimum.reduceat(dmat, res_off[:-1], axis=1)
+            hits += int((dres < 5.0).sum()); atoms += nl
+        mdn["hits_per_atom"] = hits / max(atoms, 1)
+        w = work_of(np.diff(batch.atom_off), np.diff(batch.tor_off), ligs.n_pairs, n_chains, cfg.n_steps, gp.n_refine, mdn)
     grid_bytes = 16 * int(np.prod(rec.dims)) * cfg.n_types                  # the xy-packed copy the kernels gather from
     pk = peaks(eng, grid_bytes)
     mc_ms = float(np.mean(t_mc))
@@ -277,6 +306,8 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
         roofline=roofline_of(w, mc_ms, pk, KERNEL_NAMES.get(eng.last_kernel(), "?"), stored_traffic(name) if n_lig is None and world == 1 else None),
         best_energy=float(merged[0][:, 0, 0].min().item()))
     res["roofline"]["mc_kernel_pose_evals_per_s"] = w["evals"] / (mc_ms * 1e-3)
+    if mdn:
+        res["mdn"] = mdn
     if do_e2e:                                                               # host buffers in, host buffers out
         h_out = (np.empty((L, k, 2), np.float32), np.empty((L, k, stride), np.float32), np.empty((L, k), np.int32))
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
@@ -442,6 +473,8 @@ def main():
             extras[name] = {k: r[k] for k in ("title", "evals", "sg_evals", "value", "pose_evals_per_s", "ms_per_step", "ms_per_task",
                                               "ms_grid_build", "ms_mc_kernels", "ms_topk", "launches", "best_energy")}
             rf = r["roofline"]
+            if "mdn" in r:
+                extras[name]["mdn"] = r["mdn"]
             extras[name].update(kernel=rf["kernel"], regime=REGIME.get(name, "?"), bound=rf["bound"], roofline_frac=rf["frac"],
                                 alu_frac=rf["alu_frac"], xu_frac=rf["xu_frac"], l2_frac=rf["l2_frac"],
                                 gather_grid_gbs=rf["peaks"].get("gather_grid_gbs"),
@@ -469,7 +502,7 @@ def main():
         pose_evals_per_s=main_res["pose_evals_per_s"], ms_per_task=main_res["ms_per_task"],
         ms_grid_build=main_res["ms_grid_build"], ms_mc_kernels=main_res["ms_mc_kernels"], ms_topk=main_res["ms_topk"],
         clocks=main_res["clocks"], e2e=main_res.get("e2e"), gpu_launches=main_res["launches"],
-        roofline=main_res["roofline"], cpu_baseline=cpu, best_energy=main_res["best_energy"], other_workloads=extras)
+        roofline=main_res["roofline"], mdn=main_res.get("mdn"), cpu_baseline=cpu, best_energy=main_res["best_energy"], other_workloads=extras)
     print(json.dumps(line))
     eng.close()
     if world > 1:

@@ -709,7 +709,7 @@ extern "C" int tridsk_ligand_info(const tridsk_ligands* l, int* n_lig, int* max_
 
 // ---------------------------------------------------------------------------------------- E_MDN (O15)
 static void free_mdn(tridsk_ligands* l) {
-    for (int i = 0; i < 5; ++i) { if (l->mdn_buf[i]) cudaFree(l->mdn_buf[i]); l->mdn_buf[i] = nullptr; }
+    for (int i = 0; i < 7; ++i) { if (l->mdn_buf[i]) cudaFree(l->mdn_buf[i]); l->mdn_buf[i] = nullptr; }
     memset(&l->mdn, 0, sizeof(l->mdn));
 }
 
@@ -721,19 +721,25 @@ extern "C" int tridsk_load_mdn(tridsk_ctx* ctx, tridsk_ligands* ligs, const trid
     free_mdn(ligs);
     if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; ctx->graph_key.clear(); }
     if (!m) return TRIDSK_OK;
+    if (m->n_res > 65535) return fail(ctx, TRIDSK_ELIMIT, "more than 65535 residues");
     if (m->n_res < 1 || m->K < 1 || !m->res_off || !m->res_xyz || !m->pi || !m->mu || !m->sigma) return fail(ctx, TRIDSK_EINVAL, "bad mixture-density term");
     if (!(m->d_cut > 0.f) || !std::isfinite(m->d_cut) || !std::isfinite(m->w_mdn)) return fail(ctx, TRIDSK_EINVAL, "bad w_mdn / d_cut");
     for (int i = 0; i < m->n_res; ++i) if (m->res_off[i + 1] < m->res_off[i] || m->res_off[0] != 0) return fail(ctx, TRIDSK_EINVAL, "res_off must start at 0 and be non-decreasing");
     const int L = ligs->n_lig, n_at = m->res_off[m->n_res];
     if (L == 0) return TRIDSK_OK;
-    std::vector<long long> off(L);
-    long long total = 0;
-    for (int l = 0; l < L; ++l) { off[l] = total; total += (long long)m->n_res * ligs->hdr_h[l].n * m->K; }
+    const int K4 = (m->K + 3) / 4 * 4;
+    std::vector<long long> off(2 * (size_t)L);             // [0, L): blocks of the packed records; [L, 2L): blocks of the caller's arrays
+    long long total = 0, total_p = 0;
+    for (int l = 0; l < L; ++l) {
+        off[l] = total_p; off[L + l] = total;
+        total += (long long)m->n_res * ligs->hdr_h[l].n * m->K;
+        total_p += (long long)m->n_res * ligs->hdr_h[l].n * K4;
+    }
     cudaError_t e = cudaMalloc(&ligs->mdn_buf[0], sizeof(float4) * m->n_res);
     if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[1], sizeof(int) * (m->n_res + 1));
     if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[2], sizeof(float4) * std::max(n_at, 1));
-    if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[3], sizeof(float4) * (size_t)total);
-    if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[4], sizeof(long long) * L);
+    if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[3], sizeof(float4) * (size_t)total_p);
+    if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[4], sizeof(long long) * 2 * L);
     // staging: residue coordinates, and the three parameter arrays when they live on the host
     float* d_xyz = nullptr;
     int* d_bad = nullptr;
@@ -750,9 +756,9 @@ extern "C" int tridsk_load_mdn(tridsk_ctx* ctx, tridsk_ligands* ligs, const trid
     if (e == cudaSuccess) e = cudaMemsetAsync(d_bad, 0, sizeof(int), ctx->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_xyz, m->res_xyz, sizeof(float) * 3 * n_at, cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(ligs->mdn_buf[1], m->res_off, sizeof(int) * (m->n_res + 1), cudaMemcpyHostToDevice, ctx->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(ligs->mdn_buf[4], off.data(), sizeof(long long) * L, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ligs->mdn_buf[4], off.data(), sizeof(long long) * 2 * L, cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = launch_mdn_spheres(ctx->stream, d_xyz, (const int*)ligs->mdn_buf[1], m->n_res, m->d_cut, (float4*)ligs->mdn_buf[2], (float4*)ligs->mdn_buf[0]);
-    if (e == cudaSuccess) e = launch_mdn_pack(ctx->stream, ligs->hdr, ligs->atom_i, L, m->n_res, m->K, (const long long*)ligs->mdn_buf[4], src[0], src[1], src[2],
+    if (e == cudaSuccess) e = launch_mdn_pack(ctx->stream, ligs->hdr, ligs->atom_i, L, m->n_res, m->K, (const long long*)ligs->mdn_buf[4], (const long long*)ligs->mdn_buf[4] + L, src[0], src[1], src[2],
                                               m->w_mdn, (float4*)ligs->mdn_buf[3], d_bad);
     int bad = 0;
     if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
@@ -765,10 +771,47 @@ extern "C" int tridsk_load_mdn(tridsk_ctx* ctx, tridsk_ligands* ligs, const trid
         return fail(ctx, e == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA, std::string("load_mdn: ") + cudaGetErrorString(e));
     }
     if (bad) { free_mdn(ligs); return fail(ctx, TRIDSK_EINVAL, "mixture parameters: sigma must be > 0 and every value finite"); }
-    ligs->mdn.n_res = m->n_res; ligs->mdn.K = m->K; ligs->mdn.d_cut = m->d_cut;
-    ligs->mdn.sph = (const float4*)ligs->mdn_buf[0]; ligs->mdn.res_off = (const int*)ligs->mdn_buf[1];
-    ligs->mdn.rec = (const float4*)ligs->mdn_buf[2]; ligs->mdn.par = (const float4*)ligs->mdn_buf[3];
-    ligs->mdn.lig_off = (const long long*)ligs->mdn_buf[4];
+    MdnDev M;
+    memset(&M, 0, sizeof(M));
+    M.n_res = m->n_res; M.K = m->K; M.K4 = K4; M.d_cut = m->d_cut;
+    M.sph = (const float4*)ligs->mdn_buf[0]; M.res_off = (const int*)ligs->mdn_buf[1];
+    M.rec = (const float4*)ligs->mdn_buf[2]; M.par = (const float4*)ligs->mdn_buf[3];
+    M.lig_off = (const long long*)ligs->mdn_buf[4];
+    // cell list (an acceleration structure, not arithmetic of the method): a uniform grid over the residues' bounding box
+    // grown by d_cut; the lists are counted and filled on the device, the prefix sum of the counts is taken here
+    {
+        float lo[3] = {1e30f, 1e30f, 1e30f}, hi[3] = {-1e30f, -1e30f, -1e30f};
+        for (int r = 0; r < n_at; ++r)
+            for (int c = 0; c < 3; ++c) { lo[c] = std::min(lo[c], m->res_xyz[3 * r + c]); hi[c] = std::max(hi[c], m->res_xyz[3 * r + c]); }
+        if (n_at == 0) for (int c = 0; c < 3; ++c) lo[c] = hi[c] = 0.f;
+        float cell = 1.5f;
+        long long ncell = 0;
+        for (;; cell *= 1.25f) {                            // at most ~256k cells
+            ncell = 1;
+            for (int c = 0; c < 3; ++c) { M.nc[c] = std::max(1, (int)std::ceil((hi[c] - lo[c] + 2.f * m->d_cut) / cell)); ncell *= M.nc[c]; }
+            if (ncell <= 262144) break;
+        }
+        for (int c = 0; c < 3; ++c) M.glo[c] = lo[c] - m->d_cut;
+        M.inv_cell = 1.f / cell;
+        std::vector<int> cnt((size_t)ncell + 1, 0);
+        e = cudaMalloc(&ligs->mdn_buf[5], sizeof(int) * (ncell + 1));
+        if (e == cudaSuccess) e = launch_mdn_cells(ctx->stream, M, cell, false, (int*)ligs->mdn_buf[5], nullptr);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(cnt.data(), ligs->mdn_buf[5], sizeof(int) * ncell, cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        long long run = 0;
+        for (long long c = 0; c < ncell; ++c) { const int k = cnt[c]; cnt[c] = (int)run; run += k; }
+        cnt[ncell] = (int)run;
+        if (e == cudaSuccess && run > 0x7fffffffLL) e = cudaErrorInvalidValue;
+        if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[6], sizeof(float4) * std::max<long long>(run, 1));
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ligs->mdn_buf[5], cnt.data(), sizeof(int) * (ncell + 1), cudaMemcpyHostToDevice, ctx->stream);
+        if (e == cudaSuccess) e = launch_mdn_cells(ctx->stream, M, cell, true, (int*)ligs->mdn_buf[5], (float4*)ligs->mdn_buf[6]);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        ctx->launches += 2;
+        if (e != cudaSuccess) { free_mdn(ligs); return fail(ctx, e == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA, std::string("load_mdn cell list: ") + cudaGetErrorString(e)); }
+        M.cell_off = (const int*)ligs->mdn_buf[5]; M.cell_at = (const float4*)ligs->mdn_buf[6];
+        if (getenv("TRIDSK_DEBUG")) fprintf(stderr, "tridsk load_mdn: %d residues, %lld cells of %.2f A, %.1f atoms per cell\n", m->n_res, ncell, cell, (double)run / (double)ncell);
+    }
+    ligs->mdn = M;
     return TRIDSK_OK;
 }
 

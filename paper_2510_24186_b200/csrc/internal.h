@@ -40,13 +40,21 @@ struct DGrid {
 
 // The mixture-density term (mdn.cuh, O15) attached to a ligand batch; n_res == 0: absent.
 struct MdnDev {
-    int n_res, K;
+    int n_res, K, K4;             // K4 = K rounded up to a multiple of 4: records per (residue, atom) in par
     const float4* sph;            // [n_res] bounding sphere of a residue: centre, (radius + d_cut)^2
     const int* res_off;           // [n_res + 1] into rec
     const float4* rec;            // residue atoms {x, y, z, 0}
-    const float4* par;            // packed parameters {a, mu, nk2, 1/sigma^2}, ligand-major, [n_res][n][K] per ligand, INTERNAL atom order
+    const float4* par;            // packed parameters {a, mu, nk2, 1/sigma^2}, ligand-major, [n_res][n][K] per ligand, INTERNAL atom order; [n_res][n][K4]
     const long long* lig_off;     // [n_lig] start of a ligand's block in par (float4 units)
     float d_cut;
+    // cell list: a uniform grid over the residues' bounding box grown by d_cut; cell c holds, as ONE contiguous stream
+    // sorted by (residue, atom index), every receptor atom {x, y, z, residue id} within d_cut + half a cell diagonal of the
+    // cell's centre.  For a point of the cell, a residue's minimum over the listed atoms equals its true minimum distance
+    // whenever that is below d_cut (the arg-min atom is then listed), and is >= d_cut otherwise.
+    float glo[3], inv_cell;
+    int nc[3];
+    const int* cell_off;          // [ncells + 1]
+    const float4* cell_at;
 };
 
 // Per-ligand header.  Atoms are stored in an INTERNAL order (depth-first over the torsion tree) so that
@@ -300,7 +308,7 @@ struct tridsk_ligands {
     int* bucket_dev[TRIDSK_MAX_J + 1] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     // the mixture-density term (tridsk_load_mdn); mdn.n_res == 0: absent
     MdnDev mdn = {};
-    void* mdn_buf[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // sph, res_off, rec, par, lig_off
+    void* mdn_buf[7] = {};        // sph, res_off, rec, par, lig_off, cell_off, cell_at
 };
 
 // ---------------------------------------------------------------- kernel launchers (one per .cu)
@@ -327,7 +335,8 @@ cudaError_t launch_score_direct(cudaStream_t s, const LigHdr* hdr, const float4*
                                 int pose_stride, float* energy, float* grad, int grad_stride, int max_atoms);
 size_t topk_cluster_smem(int top_k, int max_atoms, int max_tor);
 cudaError_t launch_mdn_spheres(cudaStream_t s, const float* res_xyz, const int* res_off, int n_res, float d_cut, float4* rec, float4* sph);
-cudaError_t launch_mdn_pack(cudaStream_t s, const LigHdr* hdr, const int* atom_i, int n_lig, int n_res, int K, const long long* lig_off,
+cudaError_t launch_mdn_cells(cudaStream_t s, const MdnDev& M, float cell, bool fill, int* counts_or_off, float4* cell_at);
+cudaError_t launch_mdn_pack(cudaStream_t s, const LigHdr* hdr, const int* atom_i, int n_lig, int n_res, int K, const long long* lig_off, const long long* in_off,
                             const float* pi, const float* mu, const float* sigma, float w_mdn, float4* par, int* bad);
 cudaError_t launch_microbench(cudaStream_t s, int which, int sm_count, void* buf, size_t bytes, int iters, float* sink, double* work);
 cudaError_t launch_philox_debug(cudaStream_t s, const unsigned int* ctr_key /* dev[6] */, unsigned int* out /* dev[4] */);

@@ -26,22 +26,26 @@ __global__ void mdn_sphere_kernel(const float* __restrict__ res_xyz, const int* 
     sph[i] = make_float4(cx, cy, cz, reach > 0.f ? reach * reach : -1.f);
 }
 
-// One CTA per ligand: records [n_res][n][K] in the library's INTERNAL atom order from the caller's arrays in the
-// caller's atom order (atom_i carries the original index of an internal atom).
+// One CTA per ligand: records [n_res][n][K4] (K4 = K rounded up to a multiple of 4, padded with zero-amplitude records) in
+// the library's INTERNAL atom order from the caller's arrays [n_res][n][K] in the caller's atom order (atom_i carries the
+// original index of an internal atom).  lig_off / in_off: start of the ligand's block in par / in the caller's arrays.
 __global__ void mdn_pack_kernel(const LigHdr* __restrict__ hdr, const int* __restrict__ atom_i, int n_res, int K,
-                                const long long* __restrict__ lig_off, const float* __restrict__ pi, const float* __restrict__ mu,
+                                const long long* __restrict__ lig_off, const long long* __restrict__ in_off,
+                                const float* __restrict__ pi, const float* __restrict__ mu,
                                 const float* __restrict__ sigma, float w_mdn, float4* __restrict__ par, int* __restrict__ bad) {
     const int lig = blockIdx.x;
     const LigHdr h = hdr[lig];
-    const long long base = lig_off[lig];
-    const long long total = (long long)n_res * h.n * K;
+    const int K4 = (K + 3) / 4 * 4;
+    const long long base = lig_off[lig], ibase = in_off[lig];
+    const long long total = (long long)n_res * h.n * K4;
     for (long long e = threadIdx.x; e < total; e += blockDim.x) {
-        const int k = (int)(e % K);
-        const long long ip = e / K;
+        const int k = (int)(e % K4);
+        const long long ip = e / K4;
         const int p = (int)(ip % h.n);
         const long long i = ip / h.n;
+        if (k >= K) { par[base + e] = make_float4(0.f, 0.f, 0.f, 0.f); continue; }
         const int orig = (atom_i[h.atom_off + p] >> 16) & 0xff;
-        const long long src = base + (i * h.n + orig) * K + k;
+        const long long src = ibase + (i * h.n + orig) * K + k;
         const float sg = sigma[src], w = pi[src], m = mu[src];
         if (!(sg > 0.f) || !isfinite(sg) || !isfinite(w) || !isfinite(m)) { *bad = 1; par[base + e] = make_float4(0.f, 0.f, 0.f, 0.f); continue; }
         const float inv_s2 = 1.f / (sg * sg);
@@ -56,8 +60,48 @@ cudaError_t launch_mdn_spheres(cudaStream_t s, const float* res_xyz, const int* 
 }
 
 cudaError_t launch_mdn_pack(cudaStream_t s, const LigHdr* hdr, const int* atom_i, int n_lig, int n_res, int K, const long long* lig_off,
-                            const float* pi, const float* mu, const float* sigma, float w_mdn, float4* par, int* bad) {
+                            const long long* in_off, const float* pi, const float* mu, const float* sigma, float w_mdn, float4* par, int* bad) {
     if (n_lig <= 0 || n_res <= 0) return cudaSuccess;
-    mdn_pack_kernel<<<n_lig, 256, 0, s>>>(hdr, atom_i, n_res, K, lig_off, pi, mu, sigma, w_mdn, par, bad);
+    mdn_pack_kernel<<<n_lig, 256, 0, s>>>(hdr, atom_i, n_res, K, lig_off, in_off, pi, mu, sigma, w_mdn, par, bad);
+    return cudaGetLastError();
+}
+
+// One thread per cell of the cell list: the receptor atoms within d_cut + half a cell diagonal of the cell's centre, in
+// (residue, atom index) order; the first entry of a residue's run carries residue id | run length << 16 in w, the others
+// the residue id.  fill = false: counts[c] = how many; fill = true: written to cell_at[off[c] ..].
+__global__ void mdn_cell_kernel(MdnDev M, float cell, bool fill, int* __restrict__ counts_or_off, float4* __restrict__ cell_at) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int ncell = M.nc[0] * M.nc[1] * M.nc[2];
+    if (c >= ncell) return;
+    const int ix = c % M.nc[0], iy = (c / M.nc[0]) % M.nc[1], iz = c / (M.nc[0] * M.nc[1]);
+    const float x = M.glo[0] + cell * ((float)ix + 0.5f), y = M.glo[1] + cell * ((float)iy + 0.5f), z = M.glo[2] + cell * ((float)iz + 0.5f);
+    const float half_diag = 0.8660254f * cell;
+    const float reach = M.d_cut + half_diag * 1.001f + 1e-3f, reach2 = reach * reach;
+    int n = 0;
+    float4* dst = fill ? cell_at + counts_or_off[c] : nullptr;
+    for (int i = 0; i < M.n_res; ++i) {
+        const float4 s = M.sph[i];
+        if (s.w < 0.f) continue;
+        const float sx = x - s.x, sy = y - s.y, sz = z - s.z;
+        const float lim = sqrtf(s.w) + half_diag;                 // grown bounding sphere + the cell's own radius
+        if (sx * sx + sy * sy + sz * sz >= lim * lim) continue;
+        const int first = n;
+        for (int r = M.res_off[i]; r < M.res_off[i + 1]; ++r) {
+            const float4 a = M.rec[r];
+            const float dx = x - a.x, dy = y - a.y, dz = z - a.z;
+            if (dx * dx + dy * dy + dz * dz < reach2) {
+                if (fill) dst[n] = make_float4(a.x, a.y, a.z, __int_as_float(i));
+                ++n;
+            }
+        }
+        if (fill && n > first) dst[first].w = __int_as_float(i | ((n - first) << 16));
+    }
+    if (!fill) counts_or_off[c] = n;
+}
+
+cudaError_t launch_mdn_cells(cudaStream_t s, const MdnDev& M, float cell, bool fill, int* counts_or_off, float4* cell_at) {
+    const int ncell = M.nc[0] * M.nc[1] * M.nc[2];
+    if (ncell <= 0) return cudaSuccess;
+    mdn_cell_kernel<<<(ncell + 127) / 128, 128, 0, s>>>(M, cell, fill, counts_or_off, cell_at);
     return cudaGetLastError();
 }

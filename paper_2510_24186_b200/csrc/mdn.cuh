@@ -4,8 +4,8 @@
 // atom, ties of the minimum go to the lowest atom index, indicators are not differentiated (G21).
 // It is a per-ligand-atom term like the grid lookup (it sees only x_j), so every mapping of the fused kernel calls
 // mdn_atom() at the place where it interpolates the receptor grid for an atom.  This is the paper's own "self-defined
-// kernel function" that skips far pairs (P:353 item 4): a residue is visited only if the atom lies inside its bounding
-// sphere grown by d_cut.
+// kernel function" that skips far pairs (P:353 item 4): a residue is visited only if the cell list (internal.h) names
+// it for the cell the atom is in.
 #pragma once
 #include "internal.h"
 
@@ -13,36 +13,61 @@
 // par = the ligand's parameter block [n_res][n][K] of {a, mu, nk2, 1/sigma^2}, a = w_mdn pi / (sigma sqrt(2 pi)),
 // nk2 = -log2(e) / (2 sigma^2):  N = a 2^(nk2 (d - mu)^2),  dN/dd = -N (d - mu) / sigma^2.
 // e += w_mdn * (this atom's share of E_MDN); grad: (gx, gy, gz) += its gradient.
+// One (residue, atom) pair whose minimum squared distance best2 is inside the cut-off: the K mixture components.  The
+// records are padded to a multiple of four per pair (M.K4; the padding has zero amplitude), four loads in flight.
+__device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __restrict__ q, float best2, float bx, float by, float bz,
+                                           bool grad, float& e, float& gx, float& gy, float& gz) {
+    float rinv;
+    { const float b = fmaxf(best2, 1e-12f); asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(b)); }
+    const float d = best2 * rinv;
+    float de = 0.f;
+    for (int k0 = 0; k0 < M.K4; k0 += 4) {
+        float4 c[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) c[j] = __ldg(q + k0 + j);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float t = d - c[j].y;
+            float N;
+            { const float arg = c[j].z * t * t; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(N) : "f"(arg)); }
+            N *= c[j].x;
+            e -= N;
+            de = fmaf(N * t, c[j].w, de);
+        }
+    }
+    if (grad) {
+        const float sc = de * rinv;
+        gx = fmaf(sc, bx, gx); gy = fmaf(sc, by, gy); gz = fmaf(sc, bz, gz);
+    }
+}
+
 __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restrict__ par, int n, int p, float x, float y, float z,
                                          int i0, int istep, bool grad, float& e, float& gx, float& gy, float& gz) {
-    for (int i = i0; i < M.n_res; i += istep) {
-        const float4 s = __ldg(M.sph + i);                    // centre, (bounding radius + d_cut)^2
-        const float sx = x - s.x, sy = y - s.y, sz = z - s.z;
-        if (!(sx * sx + sy * sy + sz * sz < s.w)) continue;
-        float best2 = 3.0e38f, bx = 0.f, by = 0.f, bz = 0.f;
-        const int r1 = __ldg(M.res_off + i + 1);
-        for (int r = __ldg(M.res_off + i); r < r1; ++r) {     // plain minimum, ties -> lowest index
-            const float4 a = __ldg(M.rec + r);
-            const float dx = x - a.x, dy = y - a.y, dz = z - a.z;
+    // the cell of the atom streams every receptor atom it can be within d_cut of, sorted by residue (outside the grid: none)
+    const float ux = (x - M.glo[0]) * M.inv_cell, uy = (y - M.glo[1]) * M.inv_cell, uz = (z - M.glo[2]) * M.inv_cell;
+    const int ix = __float2int_rd(ux), iy = __float2int_rd(uy), iz = __float2int_rd(uz);
+    if ((unsigned)ix >= (unsigned)M.nc[0] || (unsigned)iy >= (unsigned)M.nc[1] || (unsigned)iz >= (unsigned)M.nc[2]) return;
+    const int cell = (iz * M.nc[1] + iy) * M.nc[0] + ix;
+    const int e0 = __ldg(M.cell_off + cell), e1 = __ldg(M.cell_off + cell + 1);
+    if (e0 >= e1) return;
+    const float cut2 = M.d_cut * M.d_cut;
+    // Residue by residue: the first entry of a run holds residue id | run length << 16.  Lanes of a warp sit in different
+    // cells, so their runs differ in length; the short inner loop diverges, the costly mixture evaluation after it is
+    // reached by all lanes together once per residue.
+    int ord = 0;
+    for (int en = e0; en < e1; ++ord) {
+        const float4 a = __ldg(M.cell_at + en);
+        const int hdr = __float_as_int(a.w), i = hdr & 0xffff, cnt = hdr >> 16;
+        float bx = x - a.x, by = y - a.y, bz = z - a.z;
+        float best2 = bx * bx + by * by + bz * bz;
+        for (int r = 1; r < cnt; ++r) {                       // plain minimum, ties -> lowest atom index
+            const float4 b = __ldg(M.cell_at + en + r);
+            const float dx = x - b.x, dy = y - b.y, dz = z - b.z;
             const float d2 = dx * dx + dy * dy + dz * dz;
             if (d2 < best2) { best2 = d2; bx = dx; by = dy; bz = dz; }
         }
-        const float d = sqrtf(best2);
-        if (!(d < M.d_cut)) continue;
-        const float4* q = par + ((size_t)i * n + p) * M.K;
-        float de = 0.f;
-        for (int k = 0; k < M.K; ++k) {
-            const float4 c = __ldg(q + k);
-            const float t = d - c.y;
-            float N;
-            { const float arg = c.z * t * t; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(N) : "f"(arg)); }
-            N *= c.x;
-            e -= N;
-            de = fmaf(N * t, c.w, de);
-        }
-        if (grad && d > 0.f) {
-            const float sc = de / d;
-            gx = fmaf(sc, bx, gx); gy = fmaf(sc, by, gy); gz = fmaf(sc, bz, gz);
-        }
+        en += cnt;
+        if (best2 < cut2 && ord % istep == i0)
+            mdn_finish(M, par + ((size_t)i * n + p) * M.K4, best2, bx, by, bz, grad, e, gx, gy, gz);
     }
 }

@@ -232,6 +232,7 @@ class Config:
     backbone: int = 0
     sizes: dict = field(default_factory=dict)
     n_refine: int = 1
+    mdn_K: int = 0               # > 0: the workload carries the mixture-density term with K components per (residue, atom)
 
 
 CONFIGS = {
@@ -246,6 +247,10 @@ CONFIGS = {
     # Not a BASELINE.json config: 32 independent copies of the C2 dock in one batch ("C2 run as 32 concurrent
     # independent docks to show the kernel's rate when fed")
     "C2x32": Config("C2x32", "32 concurrent drug-like single docks", 3000, 30.0, 80, 16, 32, 384, 1000, 10, 1002, 2002),
+    # Not a BASELINE.json config: the first 1,024 ligands of C3 sampled under the paper's FULL score, E_MDN included (SURVEY
+    # 8(f) NEXT-1), with synthetic mixture parameters (K = 10) on the pocket residues (pocket_residues below).
+    "M3": Config("M3", "Screening batch under the full score (E_MDN, K = 10), first 1,024 ligands of C3", 3000, 30.0, 80, 16, 1024, 128, 500, 1,
+                 1003, 2003, mdn_K=10),
     "P1": Config("P1", "Paper-shaped run (1,024 copies x 8 loops x 32 Adam steps)", 3000, 30.0, 80, 16, 1, 1024, 8, 8, 1002, 2002,
                  n_refine=32),
 }
@@ -259,10 +264,10 @@ def config_sizes(cfg: Config, n_lig: int | None = None):
         return np.full(L, 12), np.full(L, 2)
     if cfg.name in ("C2", "P1", "C2x32"):
         return np.full(L, 30), np.full(L, 6)
-    if cfg.name == "C3":
-        n = rng.integers(15, 51, size=cfg.n_lig)
+    if cfg.name in ("C3", "M3"):
+        n = rng.integers(15, 51, size=4096)
         t = np.array([rng.integers(0, min(12, k // 4) + 1) for k in n])
-        return n[:L], t[:L]
+        return n[:L], t[:L]                                                  # ligand i is the same in C3 and M3
     if cfg.name == "C4":
         return np.full(L, 80), np.full(L, 20)
     if cfg.name == "C5":
@@ -314,6 +319,31 @@ def residues(rec: "Receptor", size: int = 8):
     n_res = (len(order) + size - 1) // size
     res_off = np.minimum(np.arange(n_res + 1) * size, len(order)).astype(np.int32)
     return order, res_off
+
+
+def pocket_residues(rec: "Receptor", size: int = 8, reach: float = 13.0):
+    """The residues E_MDN runs over: the paper uses the POCKET residues (those near the ligand); here the groups of
+    `size` receptor atoms (residues above) that have an atom within `reach` of the pocket centre (search box 8 A + the 5 A
+    cut-off of the term).  -> (res_xyz [n_at,3] float32, res_off [n_res+1] int32)."""
+    order, off = residues(rec, size)
+    xyz = rec.xyz[order]
+    keep_xyz, keep_off = [], [0]
+    for i in range(len(off) - 1):
+        a = xyz[off[i]:off[i + 1]]
+        if len(a) and np.min(np.linalg.norm(a - rec.pocket_center, axis=1)) < reach:
+            keep_xyz.append(a)
+            keep_off.append(keep_off[-1] + len(a))
+    return np.concatenate(keep_xyz).astype(np.float32), np.asarray(keep_off, np.int32)
+
+
+def gmm_batch(n_res: int, n_atoms, K: int, seed: int):
+    """gmm_params for every ligand of a batch, flat and ligand-major (the layout tridsk_load_mdn takes):
+    -> pi, mu, sigma float32 [sum_l n_res * n_atoms[l] * K]."""
+    out = [[], [], []]
+    for l, n in enumerate(n_atoms):
+        for dst, a in zip(out, gmm_params(n_res, int(n), K, seed + l)):
+            dst.append(a.reshape(-1))
+    return tuple(np.concatenate(v) for v in out)
 
 
 def gmm_params(n_res: int, n_atoms: int, K: int, seed: int):
