@@ -144,6 +144,22 @@ int  tridsk_synchronize(tridsk_ctx* ctx);
 int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const int* rec_type, int n_rec,
                       const tridsk_types* types, const tridsk_params* params,
                       const float origin[3], const int dims[3], float spacing, tridsk_grid** out);
+/*
+ * The same grid through the ctx's per-receptor cache (many-target screens rebuild the same receptors'
+ * grids over and over -- DEKOIS 2.0 has 81 targets; crystallographic waters kept as fixed receptor atoms, are
+ * simply more rec_xyz rows and make a different key).  The key is a 64-bit hash of everything the grid depends on
+ * (receptor coordinates and types, the type table, the pair-function parameters, origin / dims / spacing); a hit returns
+ * the cached grid without launching anything, a miss builds it and keeps it.  The cache holds its own reference: free the
+ * returned handle with tridsk_free_grid as usual.  Least recently used grids are dropped when the byte budget
+ * (tridsk_grid_cache_config; default 4 GiB, 0 disables caching) is exceeded.  Receptor arrays in DEVICE memory are copied
+ * to the host to be hashed.
+ */
+int tridsk_build_grid_cached(tridsk_ctx* ctx, const float* rec_xyz, const int* rec_type, int n_rec,
+                             const tridsk_types* types, const tridsk_params* params,
+                             const float origin[3], const int dims[3], float spacing, tridsk_grid** out);
+/* budget_bytes >= 0 sets the budget (dropping grids beyond it); stats (may be NULL) [host] <- {hits, misses, grids held, bytes held}. */
+int tridsk_grid_cache_config(tridsk_ctx* ctx, long long budget_bytes, long long stats[4]);
+
 /* Adopt a caller-built grid (e.g. the oracle's), copied from `values` [host|dev] [n_types][nz][ny][nx]. */
 int tridsk_grid_from_values(tridsk_ctx* ctx, const float* values, int n_types,
                             const float origin[3], const int dims[3], float spacing, tridsk_grid** out);

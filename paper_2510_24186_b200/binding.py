@@ -230,6 +230,25 @@ class Engine:
         self._sync_out()
         return Grid(self, h, ty.n_types, dims, origin, spacing)
 
+    def build_grid_cached(self, rec_xyz, rec_type, radius, role, params, origin, dims, spacing) -> Grid:
+        """tridsk_build_grid_cached: the grid through the ctx's per-receptor cache (a hit launches nothing)."""
+        ty, keep = self._types(radius, role)
+        xyz = rec_xyz if not isinstance(rec_xyz, np.ndarray) else np.ascontiguousarray(rec_xyz, np.float32)
+        typ = rec_type if not isinstance(rec_type, np.ndarray) else np.ascontiguousarray(rec_type, np.int32)
+        h = C.c_void_p()
+        d = (C.c_int * 3)(*[int(v) for v in dims])
+        self._sync_in()
+        self._ck(lib().tridsk_build_grid_cached(self.ctx, _ptr(xyz), _ptr(typ), C.c_int(int(xyz.shape[0])), C.byref(ty), C.byref(params),
+                                                _f3(origin), d, C.c_float(spacing), C.byref(h)))
+        self._sync_out()
+        return Grid(self, h, ty.n_types, dims, origin, spacing)
+
+    def grid_cache(self, budget_bytes=-1):
+        """Set the cache's byte budget (-1: leave it) -> dict(hits, misses, grids, bytes)."""
+        st = (C.c_longlong * 4)()
+        self._ck(lib().tridsk_grid_cache_config(self.ctx, C.c_longlong(int(budget_bytes)), st))
+        return dict(hits=st[0], misses=st[1], grids=st[2], bytes=st[3])
+
     def grid_from_values(self, values, origin, spacing) -> Grid:
         if isinstance(values, np.ndarray):
             values = np.ascontiguousarray(values, np.float32)

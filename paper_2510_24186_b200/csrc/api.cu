@@ -161,6 +161,8 @@ extern "C" int tridsk_create(tridsk_ctx** out, int device, void* cuda_stream) {
 extern "C" void tridsk_destroy(tridsk_ctx* ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
+    for (auto& ent : ctx->grid_cache) tridsk_free_grid(ent.grid);
+    ctx->grid_cache.clear();
     *ctx->alive = false;
     if (ctx->pool) cudaMemPoolDestroy(ctx->pool);   // outstanding grids keep their memory until they are freed
     if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
@@ -276,6 +278,81 @@ extern "C" int tridsk_build_grid(tridsk_ctx* ctx, const float* rec_xyz, const in
     return TRIDSK_OK;
 }
 
+// ---------------------------------------------------------------------------------------- per-receptor grid cache
+static unsigned long long fnv1a(unsigned long long h, const void* p, size_t n) {
+    const unsigned char* b = (const unsigned char*)p;
+    for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ULL; }
+    return h;
+}
+static void cache_trim(tridsk_ctx* ctx) {
+    while (!ctx->grid_cache.empty() && ctx->cache_bytes > ctx->cache_budget) {
+        ctx->cache_bytes -= ctx->grid_cache.back().bytes;
+        tridsk_free_grid(ctx->grid_cache.back().grid);
+        ctx->grid_cache.pop_back();
+    }
+}
+
+extern "C" int tridsk_build_grid_cached(tridsk_ctx* ctx, const float* rec_xyz, const int* rec_type, int n_rec,
+                                        const tridsk_types* types, const tridsk_params* params,
+                                        const float origin[3], const int dims[3], float spacing, tridsk_grid** out) {
+    if (!ctx || !out || !params || !rec_xyz || !rec_type || n_rec < 0 || !origin || !dims) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    *out = nullptr;
+    int rc = check_types(ctx, types);
+    if (rc) return rc;
+    if (ctx->cache_budget == 0) return tridsk_build_grid(ctx, rec_xyz, rec_type, n_rec, types, params, origin, dims, spacing, out);
+    // host view of the receptor for the key
+    std::vector<float> hx;
+    std::vector<int> ht;
+    const float* kx = rec_xyz;
+    const int* kt = rec_type;
+    if (n_rec && is_device_ptr(rec_xyz)) { hx.resize(3 * (size_t)n_rec); CK(cudaMemcpyAsync(hx.data(), rec_xyz, sizeof(float) * hx.size(), cudaMemcpyDeviceToHost, ctx->stream)); kx = hx.data(); }
+    if (n_rec && is_device_ptr(rec_type)) { ht.resize(n_rec); CK(cudaMemcpyAsync(ht.data(), rec_type, sizeof(int) * n_rec, cudaMemcpyDeviceToHost, ctx->stream)); kt = ht.data(); }
+    if (!hx.empty() || !ht.empty()) CK(cudaStreamSynchronize(ctx->stream));
+    unsigned long long key = 14695981039346656037ULL;
+    key = fnv1a(key, &n_rec, sizeof(int));
+    key = fnv1a(key, kx, sizeof(float) * 3 * (size_t)n_rec);
+    key = fnv1a(key, kt, sizeof(int) * (size_t)n_rec);
+    key = fnv1a(key, &types->n_types, sizeof(int));
+    key = fnv1a(key, types->radius, sizeof(float) * types->n_types);
+    key = fnv1a(key, types->hb_role, types->n_types);
+    const float pf[] = {params->w_long, params->w_clash, params->w_hbond, params->long_mu, params->long_two_sigma2, params->long_dmax,
+                        params->hb_mu, params->hb_sigma, params->hb_dmax, params->hb_dclash, params->d_floor, origin[0], origin[1], origin[2], spacing};
+    key = fnv1a(key, pf, sizeof(pf));
+    key = fnv1a(key, dims, 3 * sizeof(int));
+    for (size_t i = 0; i < ctx->grid_cache.size(); ++i)
+        if (ctx->grid_cache[i].key == key) {
+            tridsk_ctx::CacheEnt ent = ctx->grid_cache[i];
+            ctx->grid_cache.erase(ctx->grid_cache.begin() + i);
+            ctx->grid_cache.insert(ctx->grid_cache.begin(), ent);          // most recently used first
+            ++ent.grid->refs;
+            ++ctx->cache_hits;
+            *out = ent.grid;
+            return TRIDSK_OK;
+        }
+    tridsk_grid* g = nullptr;
+    rc = tridsk_build_grid(ctx, rec_xyz, rec_type, n_rec, types, params, origin, dims, spacing, &g);
+    if (rc) return rc;
+    ++ctx->cache_misses;
+    const size_t bytes = (sizeof(float) + sizeof(float4)) * g->d.plane * g->d.n_types;
+    if (bytes <= ctx->cache_budget) {
+        ++g->refs;
+        ctx->grid_cache.insert(ctx->grid_cache.begin(), {key, bytes, g});
+        ctx->cache_bytes += bytes;
+        cache_trim(ctx);
+    }
+    *out = g;
+    return TRIDSK_OK;
+}
+
+extern "C" int tridsk_grid_cache_config(tridsk_ctx* ctx, long long budget_bytes, long long stats[4]) {
+    if (!ctx) return TRIDSK_EINVAL;
+    ENTER(ctx);
+    if (budget_bytes >= 0) { ctx->cache_budget = (size_t)budget_bytes; cache_trim(ctx); }
+    if (stats) { stats[0] = ctx->cache_hits; stats[1] = ctx->cache_misses; stats[2] = (long long)ctx->grid_cache.size(); stats[3] = (long long)ctx->cache_bytes; }
+    return TRIDSK_OK;
+}
+
 extern "C" int tridsk_grid_from_values(tridsk_ctx* ctx, const float* values, int n_types,
                                        const float origin[3], const int dims[3], float spacing, tridsk_grid** out) {
     if (!ctx || !out || !values) return fail(ctx, TRIDSK_EINVAL, "null argument");
@@ -303,6 +380,7 @@ extern "C" int tridsk_grid_export(tridsk_ctx* ctx, const tridsk_grid* grid, floa
 
 extern "C" void tridsk_free_grid(tridsk_grid* g) {
     if (!g) return;
+    if (--g->refs > 0) return;                       // the grid cache (or the caller) still holds it
     if (g->ctx_alive && *g->ctx_alive) {             // stream-ordered: later work on the ctx stream may reuse the memory
         if (g->g) cudaFreeAsync(g->g, g->ctx->stream);
         if (g->gp) cudaFreeAsync(g->gp, g->ctx->stream);

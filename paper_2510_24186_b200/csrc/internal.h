@@ -270,11 +270,17 @@ struct tridsk_ctx {
     cudaMemPool_t pool = nullptr;
     std::shared_ptr<bool> alive = std::make_shared<bool>(true);   // handles that outlive the ctx free synchronously
     int last_kernel = 0;          // what the last dock used
+    // per-receptor grid cache (tridsk_build_grid_cached): most recently used first
+    struct CacheEnt { unsigned long long key; size_t bytes; tridsk_grid* grid; };
+    std::vector<CacheEnt> grid_cache;
+    size_t cache_budget = (size_t)4 << 30, cache_bytes = 0;
+    long long cache_hits = 0, cache_misses = 0;
 };
 
 struct tridsk_grid {
     tridsk_ctx* ctx;
     std::shared_ptr<bool> ctx_alive;
+    int refs = 1;                 // handles out: the caller's, and the grid cache's if the grid is cached
     float* g = nullptr;
     float4* gp = nullptr;
     DGrid d;

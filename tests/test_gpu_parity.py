@@ -869,3 +869,91 @@ def test_mdn_error_paths(eng, system):
         eng.load_mdn(ligs, rxyz, res_off, pi, mu, sg, 3, d_cut=0.0)
     eng.load_mdn(ligs, rxyz, res_off, pi, mu, sg, 3)             # a good one after the failures
     ligs.free()
+
+
+# ------------------------------------------------------------------------------------------- fixed waters, grid cache
+def test_fixed_waters_are_receptor_atoms(orc, eng, gp, system):
+    """Waters kept as fixed receptor atoms: the grid of receptor + waters against the oracle's plain sums (O3) at
+    sampled nodes and as a whole; poses next to a water score differently with and without it, both ways matching the oracle."""
+    S = system
+    rec = S["rec"]
+    wat = synth.with_waters(rec, 10, seed=5)
+    assert len(wat.xyz) == len(rec.xyz) + 10
+    g_w = eng.build_grid(wat.xyz, wat.type, S["radius"], S["role"], gp, wat.origin, wat.dims, wat.spacing)
+    G_w = orc.build_grid(S["p"], S["ty"], wat.xyz, wat.type, wat.origin, wat.dims, wat.spacing)
+    got = g_w.export()
+    assert close(got, G_w.g), worst(got, G_w.g)
+    assert np.abs(got - S["G"].g).max() > 1.0                                  # the waters are really in the field
+    li = np.zeros(6, np.int32)
+    poses = synth.random_poses(S["batch"], li, rec, seed=44, spread=0.1)
+    poses[:, 0:3] = wat.xyz[-6:] + np.array([2.9, 0.0, 0.0], np.float32)          # ligand centred 2.9 A from a water
+    e_w, _, _ = eng.score_grad(g_w, S["g_ligs"], gp, li, poses, want_coords=False)
+    e_0, _, _ = eng.score_grad(S["g_grid"], S["g_ligs"], gp, li, poses, want_coords=False)
+    L = S["L"][0]
+    for i in range(6):
+        pw = orc.score_grad(S["p"], S["ty"], G_w, L, poses[i, :7 + L.T].astype(np.float64), want_grad=False)[0]
+        p0 = orc.score_grad(S["p"], S["ty"], S["G"], L, poses[i, :7 + L.T].astype(np.float64), want_grad=False)[0]
+        assert close(e_w[i], pw) and close(e_0[i], p0)
+    assert np.abs(e_w[:, 1] - e_0[:, 1]).max() > 0.05
+    g_w.free()
+
+
+def test_grid_cache_per_receptor(orc, gp, system):
+    """tridsk_build_grid_cached: a hit returns the same grid without a launch; waters, another receptor or other parameters
+    make another key; the byte budget evicts least recently used grids; cached and uncached builds are bit-identical."""
+    from paper_2510_24186_b200 import Engine, default_params
+    S = system
+    eng = Engine(0)
+    rec = S["rec"]
+    wat = synth.with_waters(rec, 4, seed=9)
+    other = synth.receptor(250, 20.0, 16, seed=77, grid_n=54)
+    args = lambda r, p=gp: (r.xyz, r.type, S["radius"], S["role"], p, r.origin, r.dims, r.spacing)
+    plain = eng.build_grid(*args(rec)).export()
+    a = eng.build_grid_cached(*args(rec))
+    n0 = eng.launch_count()
+    b = eng.build_grid_cached(*args(rec))
+    assert eng.launch_count() == n0                                             # a hit launches nothing
+    assert b.handle.value == a.handle.value
+    assert np.array_equal(a.export(), plain)
+    import torch
+    c = eng.build_grid_cached(torch.from_numpy(rec.xyz).cuda(), torch.from_numpy(rec.type).cuda(), *args(rec)[2:])
+    assert c.handle.value == a.handle.value                                     # device inputs hash to the same key
+    w = eng.build_grid_cached(*args(wat))
+    o = eng.build_grid_cached(*args(other))
+    p2 = default_params(); p2.w_hbond = 0.3
+    q = eng.build_grid_cached(*args(rec, p2))
+    assert len({a.handle.value, w.handle.value, o.handle.value, q.handle.value}) == 4
+    st = eng.grid_cache()
+    assert (st["hits"], st["misses"], st["grids"]) == (2, 4, 4)
+    one = st["bytes"] // 4
+    for h in (b, c):
+        h.free()                                                                # extra references of the same grid
+    st = eng.grid_cache(budget_bytes=2 * one + 16)                              # room for two grids: the two oldest go
+    assert st["grids"] == 2
+    assert np.array_equal(a.export(), plain)                                    # still alive through the caller's reference
+    a2 = eng.build_grid_cached(*args(rec))                                      # evicted: a rebuild, bit-identical
+    assert a2.handle.value != a.handle.value and np.array_equal(a2.export(), plain)
+    st = eng.grid_cache(budget_bytes=0)                                         # caching off: plain builds
+    assert st["grids"] == 0
+    z = eng.build_grid_cached(*args(rec))
+    assert eng.grid_cache()["grids"] == 0 and np.array_equal(z.export(), plain)
+    for h in (a, a2, w, o, q, z):
+        h.free()
+    eng.close()
+
+
+def test_zero_quaternion_is_rejected(eng, gp, system):
+    """tridsk.h conventions: host poses with a zero / non-finite quaternion -> TRIDSK_EINVAL."""
+    from paper_2510_24186_b200 import TridskError
+    S = system
+    li, poses = _poses(S, 1, seed=3)
+    bad = poses.copy(); bad[2, 3:7] = 0.0
+    with pytest.raises(TridskError) as ei:
+        eng.score_grad(S["g_grid"], S["g_ligs"], gp, li, bad)
+    assert ei.value.code == -1
+    bad = poses.copy(); bad[0, 4] = np.nan
+    with pytest.raises(TridskError):
+        eng.score_grad(S["g_grid"], S["g_ligs"], gp, li, bad)
+    init = np.zeros((S["g_ligs"].n_lig, 4, 7 + S["g_ligs"].max_tor), np.float32)
+    with pytest.raises(TridskError):
+        eng.dock(S["g_grid"], S["g_ligs"], gp, *_dock_args(S), 4, 1, 1, seed=1, init_poses=init)

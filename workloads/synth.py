@@ -305,6 +305,28 @@ def random_poses(batch: LigandBatch, lig_index, rec: Receptor, seed: int, spread
     return poses
 
 
+# --------------------------------------------------------------------------- fixed waters
+def with_waters(rec: "Receptor", n_water: int, seed: int, water_type: int = 6, min_sep: float = 2.6):
+    """The receptor with n_water crystallographic-style waters kept as FIXED receptor atoms (Tables S8/S9 P:567-629):
+    oxygen positions drawn uniformly in the shell 1 A inside the pocket wall, at least min_sep from every receptor atom and
+    from one another; type `water_type` (donor + acceptor in the synthetic table).  -> a new Receptor (same grid geometry)."""
+    rng = np.random.default_rng(seed)
+    xyz, typ = [r for r in rec.xyz], list(rec.type)
+    placed, tries = 0, 0
+    while placed < n_water and tries < 200000:
+        tries += 1
+        v = rng.normal(size=3)
+        v /= np.linalg.norm(v)
+        p = rec.pocket_center + v * rng.uniform(rec.pocket_radius - 2.0, rec.pocket_radius - 0.5)
+        if np.min(np.linalg.norm(np.asarray(xyz) - p, axis=1)) < min_sep:
+            continue
+        xyz.append(p.astype(np.float32)); typ.append(water_type); placed += 1
+    out = Receptor(**{**rec.__dict__})
+    out.xyz = np.asarray(xyz, np.float32)
+    out.type = np.asarray(typ, np.int32)
+    return out
+
+
 # --------------------------------------------------------------------------- inputs of E_MDN (SURVEY 8(f) NEXT-1)
 def residues(rec: "Receptor", size: int = 8):
     """Group the receptor atoms into spatially compact pseudo-residues of `size` atoms (the paper's residues come from
