@@ -404,6 +404,7 @@ struct PackedLig {
     long long w_hist[5] = {0, 0, 0, 0, 0};
     std::vector<int> cta_rows;          // CTA format (internal.h): n + 1 row offsets
     std::vector<uint2> cta_recs;        // CTA format: 2 P row records, then P flat records
+    std::vector<float> cta_rtab;        // CTA format, n > 64: the round table
     int err = 0;
     const char* msg = "";
 };
@@ -639,6 +640,23 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
                     out.cta_recs.push_back(make_uint2((unsigned)x | ((unsigned)y << 8) | (hbq(x, y) ? 0x10000u : 0u),
                                                       fbits(out.f4[x].w + out.f4[y].w)));
         if ((int)out.cta_recs.size() != 3 * P) return bad(TRIDSK_EINVAL, "internal: CTA pair records do not cover the pair set");
+        if (n > TRIDSK_CTA_ROUNDS_N) {                        // round table (internal.h): item l of round k = pair (l, (l + k) mod n)
+            const int nr = n / 2;
+            out.cta_rtab.assign((size_t)nr * n, -1.f);
+            int cov = 0;
+            for (int k = 1; k <= nr; ++k)
+                for (int l = 0; l < n; ++l) {
+                    if (n % 2 == 0 && k == nr && l >= nr) continue;          // that half of the last round repeats pairs
+                    const int y = (l + k) % n;
+                    if (!pm[(size_t)l * n + y]) continue;
+                    unsigned bits = fbits(out.f4[l].w + out.f4[y].w);
+                    bits = (bits & ~1u) | (hbq(l, y) ? 1u : 0u);              // layout: flag in the lowest mantissa bit
+                    float v; memcpy(&v, &bits, sizeof(v));
+                    out.cta_rtab[(size_t)(k - 1) * n + l] = v;
+                    ++cov;
+                }
+            if (cov != P) return bad(TRIDSK_EINVAL, "internal: CTA round table does not cover the pair set");
+        }
     }
     // conflict-free schedule: round (j1, j2, k): lane l <-> pair (j1*S + l, j2*S + (l+k) mod S)
     auto hb = [&](int x, int y) {
@@ -696,22 +714,22 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     tridsk_ligands* lg = new (std::nothrow) tridsk_ligands();
     if (!lg) return fail(ctx, TRIDSK_ENOMEM, "host alloc");
     lg->ctx = ctx; lg->n_lig = L; lg->has_cta = want_cta;
-    size_t na = 0, nf = 0, nr = 0, nls = 0, nrec = 0, ncr = 0, ncc = 0;
+    size_t na = 0, nf = 0, nr = 0, nls = 0, nrec = 0, ncr = 0, ncc = 0, nrt = 0;
     lg->hdr_h.resize(L); lg->n_pairs.resize(L);
     for (int i = 0; i < L; ++i) {
         LigHdr& h = pk[i].h;
         h.atom_off = (int)na; h.frag_off = (int)nf; h.round_off = (int)nr; h.ls_off = (int)nls; h.rec_off = (int)nrec;
-        h.cta_row_off = (int)ncr; h.cta_rec_off = (int)ncc;
+        h.cta_row_off = (int)ncr; h.cta_rec_off = (int)ncc; h.cta_rt_off = pk[i].cta_rtab.empty() ? -1 : (int)nrt;
         na += pk[i].f4.size(); nf += pk[i].fr.size(); nr += pk[i].rounds.size();
         nls += pk[i].lane_stream.size(); nrec += pk[i].lane_recs.size();
-        ncr += pk[i].cta_rows.size(); ncc += pk[i].cta_recs.size();
+        ncr += pk[i].cta_rows.size(); ncc += pk[i].cta_recs.size(); nrt += pk[i].cta_rtab.size();
         lg->hdr_h[i] = h; lg->n_pairs[i] = h.n_pairs;
         lg->max_atoms = std::max(lg->max_atoms, h.n); lg->max_tor = std::max(lg->max_tor, h.T);
         lg->bucket[h.J].push_back(i);
         if (want_cta) {
             int th, lpa;
             cta_shape(h.n, &th, &lpa);
-            const int k = th == 128 ? 0 : 1;
+            const int k = h.n > TRIDSK_CTA_ROUNDS_N ? 1 : 0;       // bucket 1: the round-schedule instance of the kernel
             lg->cta_bucket[k].push_back(i);
             lg->cta_smem[k] = std::max(lg->cta_smem[k], cta_layout(h.n, h.T, h.n_pairs).total);
         }
@@ -725,6 +743,7 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     std::vector<LaneRec> lrv(std::max<size_t>(nrec, 1));
     std::vector<int> crv(std::max<size_t>(ncr, 1));
     std::vector<uint2> ccv(std::max<size_t>(ncc, 1));
+    std::vector<float> crt(std::max<size_t>(nrt, 1));
     for (int i = 0; i < L; ++i) {
         const LigHdr& h = pk[i].h;
         std::copy(pk[i].lane_frags.begin(), pk[i].lane_frags.end(), lf.begin() + h.frag_off);
@@ -732,6 +751,7 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
         std::copy(pk[i].lane_recs.begin(), pk[i].lane_recs.end(), lrv.begin() + h.rec_off);
         std::copy(pk[i].cta_rows.begin(), pk[i].cta_rows.end(), crv.begin() + h.cta_row_off);
         std::copy(pk[i].cta_recs.begin(), pk[i].cta_recs.end(), ccv.begin() + h.cta_rec_off);
+        if (h.cta_rt_off >= 0) std::copy(pk[i].cta_rtab.begin(), pk[i].cta_rtab.end(), crt.begin() + h.cta_rt_off);
         std::copy(pk[i].f4.begin(), pk[i].f4.end(), f4.begin() + h.atom_off);
         std::copy(pk[i].ai.begin(), pk[i].ai.end(), ai.begin() + h.atom_off);
         std::copy(pk[i].fr.begin(), pk[i].fr.end(), fr.begin() + h.frag_off);
@@ -762,6 +782,7 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     up((void**)&lg->lane_recs, lrv.data(), sizeof(LaneRec) * lrv.size());
     up((void**)&lg->cta_rows, crv.data(), sizeof(int) * crv.size());
     up((void**)&lg->cta_recs, ccv.data(), sizeof(uint2) * ccv.size());
+    up((void**)&lg->cta_rtab, crt.data(), sizeof(float) * crt.size());
     for (int k = 0; k < 2; ++k)
         if (!lg->cta_bucket[k].empty()) up((void**)&lg->cta_bucket_dev[k], lg->cta_bucket[k].data(), sizeof(int) * lg->cta_bucket[k].size());
     if (e == cudaSuccess) e = cudaMalloc((void**)&lg->all_ids, sizeof(int) * std::max(L, 1));
@@ -897,7 +918,7 @@ extern "C" void tridsk_free_ligands(tridsk_ligands* l) {
     if (!l) return;                 // cudaFree waits for the device; l->ctx may already be destroyed
     free_mdn(l);
     cudaFree(l->hdr); cudaFree(l->atom_f4); cudaFree(l->atom_i); cudaFree(l->frags); cudaFree(l->rounds);
-    cudaFree(l->lane_frags); cudaFree(l->lane_stream); cudaFree(l->lane_recs); cudaFree(l->cta_rows); cudaFree(l->cta_recs); cudaFree(l->all_ids);
+    cudaFree(l->lane_frags); cudaFree(l->lane_stream); cudaFree(l->lane_recs); cudaFree(l->cta_rows); cudaFree(l->cta_recs); cudaFree(l->cta_rtab); cudaFree(l->all_ids);
     for (int k = 0; k < 2; ++k) if (l->cta_bucket_dev[k]) cudaFree(l->cta_bucket_dev[k]);
     for (int j = 0; j <= TRIDSK_MAX_J; ++j) if (l->bucket_dev[j]) cudaFree(l->bucket_dev[j]);
     delete l;
@@ -926,7 +947,7 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
     memset(&a, 0, sizeof(a));
     a.hdr = ligs->hdr; a.atom_f4 = ligs->atom_f4; a.atom_i = ligs->atom_i; a.frags = ligs->frags; a.rounds = ligs->rounds;
     a.lane_frags = ligs->lane_frags; a.lane_stream = ligs->lane_stream; a.lane_recs = ligs->lane_recs;
-    a.cta_rows = ligs->cta_rows; a.cta_recs = ligs->cta_recs;
+    a.cta_rows = ligs->cta_rows; a.cta_recs = ligs->cta_recs; a.cta_rtab = ligs->cta_rtab;
     a.grid = grid->d;
     a.mdn = ligs->mdn;
     to_dparams(params, &a.P);
@@ -1207,7 +1228,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     memset(&base, 0, sizeof(base));
     base.hdr = ligs->hdr; base.atom_f4 = ligs->atom_f4; base.atom_i = ligs->atom_i; base.frags = ligs->frags; base.rounds = ligs->rounds;
     base.lane_frags = ligs->lane_frags; base.lane_stream = ligs->lane_stream; base.lane_recs = ligs->lane_recs;
-    base.cta_rows = ligs->cta_rows; base.cta_recs = ligs->cta_recs;
+    base.cta_rows = ligs->cta_rows; base.cta_recs = ligs->cta_recs; base.cta_rtab = ligs->cta_rtab;
     base.grid = grid->d;
     base.mdn = ligs->mdn;
     to_dparams(params, &base.P);
@@ -1265,7 +1286,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
                 McLaunch a = base;
                 a.lig_list = ligs->cta_bucket_dev[k]; a.n_list = (int)ligs->cta_bucket[k].size();
                 fill(a);
-                series.push_back({3, k == 0 ? 128 : 256, ligs->cta_smem[k], k, a});
+                series.push_back({3, k, ligs->cta_smem[k], k, a});
             }
         } else {
             for (int j = 1; j <= TRIDSK_MAX_J; ++j) {

@@ -74,6 +74,7 @@ struct LigHdr {
     int n_rec;
     int cta_row_off;              // CTA format: into cta_rows (n + 1 row offsets, relative to the ligand's records)
     int cta_rec_off;              // CTA format: into cta_recs (2 n_pairs row records, then n_pairs flat records)
+    int cta_rt_off;               // CTA format, n > 64: into cta_rtab ((n / 2) * n entries of the round table); -1: none
 };
 
 // Lane format (mc_lane.cu).  Fragments are re-indexed in depth-first PRE-order g = 0..T (0 = root), so that the
@@ -111,6 +112,14 @@ struct LaneRec {
 // force is a sum its own threads own (no scatter, no atomics).  Flat form, for energy-only evaluations: every pair once,
 // {a | b << 8 | hb << 16, dvdw bits}, sorted by (a, b).  Fragments are the LaneFrag records (pre-order).
 
+// Ligands of more than 64 atoms (one lane per atom) evaluate every pair ONCE in the gradient pass, on a conflict-free round
+// schedule: in round k = 1 .. n/2 item l is the pair (l, (l + k) mod n).  The ROUND TABLE cta_rtab[(k - 1) * n + l] holds that
+// pair's dvdw as a float whose lowest mantissa bit is the donor/acceptor flag, or -1 if the pair is not in the set (for even n
+// the items l >= n/2 of round n/2 repeat pairs and are absent).  The two forces of an item go to slots (round, atom) that no
+// other item of a block of TRIDSK_CTA_RB rounds writes: no atomics, bit-reproducible.
+#define TRIDSK_CTA_RB 8
+#define TRIDSK_CTA_ROUNDS_N 64         // ligands above this many atoms use the round schedule
+
 // Per-fragment record; fragment 0 is the root, fragment k+1 hangs off torsion k.
 struct FragRec {
     float ux, uy, uz, ox;         // axis unit vector and axis point (atom b_k), reference frame
@@ -139,6 +148,7 @@ struct McLaunch {
     const LaneRec* lane_recs;     // lane format: the pair records
     const int* cta_rows;          // CTA format
     const uint2* cta_recs;
+    const float* cta_rtab;
     const int* lig_list;          // ligands handled by this launch (one bucket)
     int n_list;
     DGrid grid;
@@ -172,6 +182,7 @@ struct ScoreLaunch {
     const LaneRec* lane_recs;
     const int* cta_rows;
     const uint2* cta_recs;
+    const float* cta_rtab;
     const int* seg_lig;           // lane score kernel: per CTA the ligand, and its poses perm[seg_start .. seg_start + seg_cnt)
     const int* seg_start;
     const int* seg_cnt;
@@ -220,7 +231,7 @@ __host__ __device__ static inline int lane_chain_slots(int n, int T, int max_dep
 
 // CTA-per-chain kernel: shared-memory layout (byte offsets) -- topology {ref, meta, fragments, row offsets, records},
 // the chain's coordinates X[3][n], per-atom (force, moment about t) AF[6][n] and a reduction scratch
-struct CtaLayout { size_t ref, meta, frag, rows, recs, X, AF, PF, red, total; };
+struct CtaLayout { size_t ref, meta, frag, rows, recs, rtab, slots, X, AF, PF, red, total; };
 #define TRIDSK_AL16(x) (((x) + 15) / 16 * 16)
 __host__ __device__ static inline CtaLayout cta_layout(int n, int T, int n_pairs) {
     CtaLayout L;
@@ -229,7 +240,10 @@ __host__ __device__ static inline CtaLayout cta_layout(int n, int T, int n_pairs
     L.meta = o; o = TRIDSK_AL16(o + 4 * (size_t)n);
     L.frag = o; o += sizeof(LaneFrag) * (size_t)(T + 1);
     L.rows = o; o = TRIDSK_AL16(o + 4 * (size_t)(n + 1));
-    L.recs = o; o = TRIDSK_AL16(o + 8 * 3 * (size_t)n_pairs);
+    const bool rounds = n > TRIDSK_CTA_ROUNDS_N;                   // round schedule: flat records only, + table + force slots
+    L.recs = o; o = TRIDSK_AL16(o + 8 * (rounds ? 1 : 3) * (size_t)n_pairs);
+    L.rtab = o; o = TRIDSK_AL16(o + (rounds ? 4 * (size_t)(n / 2) * n : 0));
+    L.slots = o; o = TRIDSK_AL16(o + (rounds ? 2 * 12 * (size_t)TRIDSK_CTA_RB * n : 0));
     L.X = o; o = TRIDSK_AL16(o + 12 * (size_t)n);
     L.AF = o; o = TRIDSK_AL16(o + 32 * (size_t)n);
     L.PF = o; o = TRIDSK_AL16(o + 32 * (size_t)n);
@@ -303,7 +317,8 @@ struct tridsk_ligands {
     bool has_cta = false;
     int* cta_rows = nullptr;
     uint2* cta_recs = nullptr;
-    std::vector<int> cta_bucket[2];              // ligand ids per CTA size (128, 256 threads)
+    float* cta_rtab = nullptr;
+    std::vector<int> cta_bucket[2];              // ligand ids: [0] up to 64 atoms (row form), [1] above (round schedule)
     int* cta_bucket_dev[2] = {nullptr, nullptr};
     size_t cta_smem[2] = {0, 0};                 // largest shared-memory need per bucket
     int* all_ids = nullptr;       // 0..n_lig-1 re-ordered per lane bucket (refilled when the plan key changes)
@@ -332,7 +347,7 @@ cudaError_t mc_lane_prepare(size_t max_smem_bytes);   // the *_prepare functions
 cudaError_t mc_cta_prepare();
 cudaError_t topk_prepare();
 cudaError_t launch_score(cudaStream_t s, const ScoreLaunch& a);
-cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int threads, size_t smem_bytes);
+cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int rounds /* 1: ligands above 64 atoms */, size_t smem_bytes);
 cudaError_t launch_score_cta(cudaStream_t s, const ScoreLaunch& a, size_t smem_bytes);
 cudaError_t launch_topk(cudaStream_t s, const TopkLaunch& a);
 cudaError_t launch_score_direct(cudaStream_t s, const LigHdr* hdr, const float4* atom_f4, const int* atom_i, const LaneFrag* lane_frags,

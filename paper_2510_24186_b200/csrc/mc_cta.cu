@@ -22,8 +22,12 @@ struct CtaTopo {
     const LaneFrag* frag;   // [T + 1] pre-order
     const int* rows;        // [n + 1] row offsets into recs
     const uint2* recs;      // [2P] row records {b | hb << 8, c}, then [P] flat records {a | b << 8 | hb << 16, c}; c = dvdw + mu
+    const uint2* flat;      // the flat records
+    const float* rtab;      // n > 64: round table [(n / 2)][n] of c = dvdw + mu (lowest mantissa bit: donor/acceptor), absent: -1e15
+    float* slots;           // n > 64: force slots [2][TRIDSK_CTA_RB][n][3]
     float *X, *AF, *PF, *red;  // X[3][n], AF[n][8] = {force, 0, moment about t, 0}, PF = its prefix sums, red[64]
     int n, T, P, lpa;
+    bool rounds;            // n > 64: every pair once per gradient pass, on the round schedule (internal.h)
 };
 
 // this lane's fragment (lane g = fragment g in pre-order; lanes beyond T are idle copies of the root)
@@ -36,7 +40,7 @@ struct CtaFrag {
 __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char* smem, const LigHdr* __restrict__ h,
                                           const float4* __restrict__ atom_f4, const int* __restrict__ atom_i,
                                           const LaneFrag* __restrict__ lane_frags, const int* __restrict__ cta_rows,
-                                          const uint2* __restrict__ cta_recs, const DParams& P) {
+                                          const uint2* __restrict__ cta_recs, const float* __restrict__ cta_rtab, const DParams& P) {
     const int n = h->n, T = h->T, np = h->n_pairs, tid = threadIdx.x, nt = blockDim.x, lane = tid & 31;
     const CtaLayout L = cta_layout(n, T, np);
     float4* ref = reinterpret_cast<float4*>(smem + L.ref);
@@ -55,10 +59,28 @@ __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char*
         }
     }
     for (int i = tid; i <= n; i += nt) rows[i] = __ldg(cta_rows + h->cta_row_off + i);
-    for (int i = tid; i < 3 * np; i += nt) {
-        const uint2 r = __ldg(cta_recs + h->cta_rec_off + i);
-        recs[i] = make_uint2(r.x, __float_as_uint(__uint_as_float(r.y) + P.long_mu));
+    const bool rounds = n > TRIDSK_CTA_ROUNDS_N;
+    if (!rounds) {
+        for (int i = tid; i < 3 * np; i += nt) {
+            const uint2 r = __ldg(cta_recs + h->cta_rec_off + i);
+            recs[i] = make_uint2(r.x, __float_as_uint(__uint_as_float(r.y) + P.long_mu));
+        }
+    } else {                                                  // flat records only, + the round table
+        for (int i = tid; i < np; i += nt) {
+            const uint2 r = __ldg(cta_recs + h->cta_rec_off + 2 * np + i);
+            recs[i] = make_uint2(r.x, __float_as_uint(__uint_as_float(r.y) + P.long_mu));
+        }
+        float* rt = reinterpret_cast<float*>(smem + L.rtab);
+        for (int i = tid; i < (n / 2) * n; i += nt) {
+            const float d = __ldg(cta_rtab + h->cta_rt_off + i);
+            const unsigned hbbit = __float_as_uint(d) & 1u;
+            rt[i] = d >= 0.f ? __uint_as_float((__float_as_uint(d + P.long_mu) & ~1u) | hbbit) : -1e15f;
+        }
+        S.rtab = rt;
+        S.slots = reinterpret_cast<float*>(smem + L.slots);
     }
+    S.rounds = rounds;
+    S.flat = rounds ? recs : recs + 2 * np;
     S.ref = ref; S.meta = meta; S.frag = reinterpret_cast<const LaneFrag*>(frag); S.rows = rows; S.recs = recs;
     S.X = reinterpret_cast<float*>(smem + L.X); S.AF = reinterpret_cast<float*>(smem + L.AF);
     S.PF = reinterpret_cast<float*>(smem + L.PF);
@@ -110,10 +132,9 @@ __device__ __forceinline__ void cta_pair(const PairK& K, float dx, float dy, flo
 // otherwise a serial string of shared-memory load -> rsqrt -> ex2 latencies).  A lane without a pair in slot u passes
 // ok[u] = false: its c becomes -1e15 and the slot evaluates to exactly zero.
 template <bool GRAD, bool ENERGY>
-__device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c_in[4],
-                                           const bool hb_in[4], const bool ok[4], float& eL, float& eC, float& eH,
-                                           float& fx, float& fy, float& fz) {
-    float d[4], rinv[4], s[4];
+__device__ __forceinline__ void cta_pairs4s(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c_in[4],
+                                            const bool hb_in[4], const bool ok[4], float& eL, float& eC, float& eH, float s[4]) {
+    float d[4], rinv[4];
     bool hb[4], any_hb = false;
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
@@ -148,6 +169,13 @@ __device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], co
             }
         }
     }
+}
+template <bool GRAD, bool ENERGY>
+__device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c_in[4],
+                                           const bool hb_in[4], const bool ok[4], float& eL, float& eC, float& eH,
+                                           float& fx, float& fy, float& fz) {
+    float s[4];
+    cta_pairs4s<GRAD, ENERGY>(K, dx, dy, dz, c_in, hb_in, ok, eL, eC, eH, s);
     if (GRAD) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) { fx = fmaf(s[u], dx[u], fx); fy = fmaf(s[u], dy[u], fy); fz = fmaf(s[u], dz[u], fz); }
@@ -160,7 +188,8 @@ __device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], co
 //      on lane g (O9); x, y, z = this thread's atom (valid when `active`).
 // MDN: the mixture-density term (mdn.cuh); the lanes of an atom share its residues (lane `part` takes residues part,
 // part + lpa, ...), their shares join the pair force / the energy sums before the fixed-order reductions.
-template <bool GRAD, bool ENERGY, bool MDN>
+// ROUNDS: 0 = row form (ligands of up to 64 atoms), 1 = round schedule (above), 2 = decided at run time (S.rounds).
+template <bool GRAD, bool ENERGY, bool MDN, int ROUNDS>
 __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
                                          const MdnDev& M, const float4* __restrict__ mdn_par,
                                          int max_depth, const float t[3], const float q[4], float theta,
@@ -226,7 +255,55 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
 
     // ---- a5 intra-ligand pairs (O6)
     float eL = 0.f, eC = 0.f, eH = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
-    if (GRAD) {
+    if (GRAD && (ROUNDS == 1 || (ROUNDS == 2 && S.rounds))) {
+        // Every pair once: rounds k = 1 .. n/2, item l of round k = pair (l, (l + k) mod n), TRIDSK_CTA_RB rounds per block spread
+        // over ALL threads of the CTA, four items in flight per thread.  The force of an item goes to slot A[round][l] and its
+        // reaction to slot B[round][(l + k) mod n]; no two items of a block share a slot, a barrier, then every atom's thread adds
+        // its slots in round order.
+        const int nr = n >> 1, nt = (int)blockDim.x;
+        const unsigned magic = ((1u << 20) + (unsigned)n - 1u) / (unsigned)n;      // floor(i / n) = (i * magic) >> 20 for i < 1024
+        float* SA = S.slots;
+        float* SB = S.slots + 3 * TRIDSK_CTA_RB * n;
+        for (int k0 = 1; k0 <= nr; k0 += TRIDSK_CTA_RB) {
+            const int nb = min(TRIDSK_CTA_RB, nr - k0 + 1), items = nb * n;
+            for (int it = tid; it < items; it += 4 * nt) {
+                float dx[4], dy[4], dz[4], c[4], sv[4];
+                bool hb[4], ok[4];
+                int sa[4], sb[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int iu = it + u * nt;
+                    ok[u] = iu < items;
+                    const int ii = ok[u] ? iu : it;
+                    const int kk = (int)(((unsigned)ii * magic) >> 20), l = ii - kk * n;
+                    int b = l + k0 + kk;
+                    b = b >= n ? b - n : b;
+                    const float cv = S.rtab[(k0 - 1 + kk) * n + l];
+                    c[u] = cv; hb[u] = (__float_as_uint(cv) & 1u) != 0u && cv > 0.f;
+                    dx[u] = S.X[l] - S.X[b]; dy[u] = S.X[n + l] - S.X[n + b]; dz[u] = S.X[2 * n + l] - S.X[2 * n + b];
+                    sa[u] = 3 * (kk * n + l); sb[u] = 3 * (kk * n + b);
+                }
+                cta_pairs4s<true, ENERGY>(K, dx, dy, dz, c, hb, ok, eL, eC, eH, sv);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (ok[u]) {
+                        const float px = sv[u] * dx[u], py = sv[u] * dy[u], pz = sv[u] * dz[u];
+                        SA[sa[u]] = px; SA[sa[u] + 1] = py; SA[sa[u] + 2] = pz;
+                        SB[sb[u]] = -px; SB[sb[u] + 1] = -py; SB[sb[u] + 2] = -pz;
+                    }
+                }
+            }
+            __syncthreads();
+            if (active) {
+                for (int kk = 0; kk < nb; ++kk) {
+                    const float* pa = SA + 3 * (kk * n + atom);
+                    const float* pb = SB + 3 * (kk * n + atom);
+                    fx += pa[0] + pb[0]; fy += pa[1] + pb[1]; fz += pa[2] + pb[2];
+                }
+            }
+            __syncthreads();
+        }
+    } else if (GRAD) {
         if (active) {
             const int k1 = S.rows[atom + 1];
             for (int k = S.rows[atom] + part; k < k1; k += 4 * S.lpa) {
@@ -246,7 +323,7 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
         }
         eL *= 0.5f; eC *= 0.5f; eH *= 0.5f;                         // every pair was visited from both ends
     } else {
-        const uint2* flat = S.recs + 2 * S.P;
+        const uint2* flat = S.flat;
         float f0 = 0.f, f1 = 0.f, f2 = 0.f;
         const int nt = (int)blockDim.x;
         for (int k = tid; k < S.P; k += 4 * nt) {
@@ -369,7 +446,7 @@ __device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const Ct
 }
 
 // ------------------------------------------------------------------ the fused MC kernel, one CTA per chain
-template <bool MDN>
+template <bool MDN, int ROUNDS>
 __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -378,7 +455,7 @@ __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
     const LigHdr* h = a.hdr + lig;
     CtaTopo S;
     CtaFrag F;
-    cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.P);
+    cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.cta_rtab, a.P);
     const DParams& P = a.P;
     const PairK K = make_pairk(P);
     const float4* mdn_par = MDN ? a.mdn.par + a.mdn.lig_off[lig] : nullptr;
@@ -423,7 +500,7 @@ __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
             const float uu = (k & 3) == 0 ? v0 : (k & 3) == 1 ? v1 : (k & 3) == 2 ? v2 : v3;
             cth = F.tor >= 0 ? PI_F * (2.f * uu - 1.f) : 0.f;
         }
-        cta_eval<false, true, MDN>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, ct, cq, cth, atom, part, active, x, y, z, ei, ea, g6, gth);
+        cta_eval<false, true, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, ct, cq, cth, atom, part, active, x, y, z, ei, ea, g6, gth);
         ecur = ei + ea;
         ebest = ecur;
 #pragma unroll
@@ -458,7 +535,7 @@ __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
         float m[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         float b1p = 1.f, b2p = 1.f;
         for (int rf = 0; rf < P.n_refine; ++rf) {
-            cta_eval<true, false, MDN>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
+            cta_eval<true, false, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
             b1p *= P.adam_b1; b2p *= P.adam_b2;
             const float c1 = __fdividef(1.f, 1.f - b1p), c2 = __fdividef(1.f, 1.f - b2p);
             float g[7] = {g6[0], g6[1], g6[2], g6[3], g6[4], g6[5], gth}, dl[7];
@@ -479,7 +556,7 @@ __global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
         }
 
         // a8: energy of the refined proposal, Metropolis, best tracking
-        cta_eval<false, true, MDN>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
+        cta_eval<false, true, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
         const float enew = ei + ea;
         const bool accept = isfinite(enew) && (um < expf(-P.beta * (enew - ecur)));
         if (a.trace != nullptr && tid == 0) {
@@ -520,7 +597,7 @@ __global__ void __launch_bounds__(256) score_cta_kernel(const ScoreLaunch a) {
     const LigHdr* h = a.hdr + lig;
     CtaTopo S;
     CtaFrag F;
-    cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.P);
+    cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.cta_rtab, a.P);
     const PairK K = make_pairk(a.P);
     const float4* mdn_par = MDN ? a.mdn.par + a.mdn.lig_off[lig] : nullptr;
     const int atom = tid / S.lpa, part = tid % S.lpa;
@@ -528,8 +605,8 @@ __global__ void __launch_bounds__(256) score_cta_kernel(const ScoreLaunch a) {
     float t[3], q[4], th, x, y, z, g6[6], gth = 0.f, ei, ea;
     cta_load_pose(a.poses + (size_t)i * a.pose_stride, F, t, q, th);
     quat_normalise(q);
-    if (a.grad != nullptr) cta_eval<true, true, MDN>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
-    else cta_eval<false, true, MDN>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
+    if (a.grad != nullptr) cta_eval<true, true, MDN, 2>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
+    else cta_eval<false, true, MDN, 2>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
     if (tid == 0) { a.energy[3 * (size_t)i] = ei + ea; a.energy[3 * (size_t)i + 1] = ei; a.energy[3 * (size_t)i + 2] = ea; }
     if (a.grad != nullptr && warp == 0) {
         float* g = a.grad + (size_t)i * a.grad_stride;
@@ -549,19 +626,22 @@ __global__ void __launch_bounds__(256) score_cta_kernel(const ScoreLaunch a) {
 
 // per device (function attributes are per device): called by tridsk_create
 cudaError_t mc_cta_prepare() {
-    cudaError_t e = cudaFuncSetAttribute(mc_cta_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    cudaError_t e = cudaFuncSetAttribute(mc_cta_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(score_cta_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(score_cta_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
     return e;
 }
 
-cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int threads, size_t smem_bytes) {
+cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int rounds, size_t smem_bytes) {
     const long long blocks = (long long)a.n_list * a.n_chains;
     if (blocks <= 0) return cudaSuccess;
-    if (blocks > 0x7fffffffLL || (threads != 128 && threads != 256)) return cudaErrorInvalidValue;
-    if (a.mdn.n_res > 0) mc_cta_kernel<true><<<(unsigned)blocks, threads, smem_bytes, s>>>(a);
-    else mc_cta_kernel<false><<<(unsigned)blocks, threads, smem_bytes, s>>>(a);
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+    const unsigned nb = (unsigned)blocks;
+    if (a.mdn.n_res > 0) { if (rounds) mc_cta_kernel<true, 1><<<nb, 128, smem_bytes, s>>>(a); else mc_cta_kernel<true, 0><<<nb, 128, smem_bytes, s>>>(a); }
+    else { if (rounds) mc_cta_kernel<false, 1><<<nb, 128, smem_bytes, s>>>(a); else mc_cta_kernel<false, 0><<<nb, 128, smem_bytes, s>>>(a); }
     return cudaGetLastError();
 }
 
