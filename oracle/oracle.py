@@ -44,7 +44,8 @@ class _Types(C.Structure):
 
 class _Grid(C.Structure):
     _fields_ = [("g", C.c_void_p), ("n_types", C.c_int), ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
-                ("origin", C.c_double * 3), ("spacing", C.c_double)]
+                ("origin", C.c_double * 3), ("spacing", C.c_double), ("rec_xyz", C.c_void_p), ("rec_type", C.c_void_p),
+                ("n_rec", C.c_int)]
 
 
 class _Mdn(C.Structure):
@@ -75,6 +76,7 @@ def lib():
         assert _lib.orc_sizeof_params() == C.sizeof(Params)
         assert _lib.orc_sizeof_step_rec() == C.sizeof(StepRec)
         assert _lib.orc_sizeof_ligand() == C.sizeof(_Ligand) and _lib.orc_sizeof_mdn() == C.sizeof(_Mdn)
+        assert _lib.orc_sizeof_grid() == C.sizeof(_Grid)
     return _lib
 
 
@@ -109,7 +111,18 @@ class Grid:
         nt, nz, ny, nx = self.g.shape
         self.origin = np.asarray(origin, dtype=np.float64)
         self.spacing = float(spacing)
-        self.c = _Grid(_p(self.g).value, nt, nx, ny, nz, _d3(origin), float(spacing))
+        self.c = _Grid(_p(self.g).value, nt, nx, ny, nz, _d3(origin), float(spacing), None, None, 0)
+
+
+class DirectReceptor:
+    """Stands where a Grid stands in score_grad / mc_step / dock, but makes the receptor term the paper's own direct sums over
+    the receptor atoms (P:103-125, P:353 item 4): no grid, no interpolation, no wall."""
+
+    def __init__(self, rec_xyz, rec_type, n_types):
+        self.xyz = np.ascontiguousarray(rec_xyz, dtype=np.float64)
+        self.type = np.ascontiguousarray(rec_type, dtype=np.int32)
+        self.g = np.zeros((n_types, 2, 2, 2), np.float32)
+        self.c = _Grid(_p(self.g).value, n_types, 2, 2, 2, _d3([0, 0, 0]), 1.0, _p(self.xyz).value, _p(self.type).value, len(self.type))
 
 
 class Ligand:

@@ -47,6 +47,12 @@ typedef struct {
     const float* g;              /* fp32 [n_types][nz][ny][nx], x fastest (O4) */
     int n_types, nx, ny, nz;
     double origin[3], spacing;
+    /* direct-pair receptor mode (the paper's own evaluation, P:103-125, P:353 item 4): when n_rec >= 0 and
+     * rec_xyz != NULL the receptor term of orc_score_grad (hence of orc_mc_step / orc_dock) is the plain sum over these receptor
+     * atoms -- no grid, no interpolation, no wall -- exactly as in orc_score_grad_direct */
+    const double* rec_xyz;
+    const int* rec_type;
+    int n_rec;
 } orc_grid;
 
 /* O15: the mixture-density term of one (receptor, ligand) pair -- Eq.GMM, Eq.E_MDN */
@@ -377,6 +383,19 @@ void orc_score_grad(const orc_params* p, const orc_types* ty, const orc_grid* G,
     orc_fk(L, pose, x);
     double e_inter = 0.0, e_intra = 0.0;
     for (int a = 0; a < n; ++a) {
+        if (G->rec_xyz) {                      /* direct sums over the receptor atoms (O3 evaluated at the atom itself) */
+            int ta = L->type[a];
+            for (int r = 0; r < G->n_rec; ++r) {
+                double dv[3] = {x[3 * a] - G->rec_xyz[3 * r], x[3 * a + 1] - G->rec_xyz[3 * r + 1], x[3 * a + 2] - G->rec_xyz[3 * r + 2]};
+                double d = sqrt(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2]), e, de;
+                int sr = G->rec_type[r];
+                orc_pair(p, ty->radius[sr], ty->role[sr], ty->radius[ta], ty->role[ta], d, &e, &de);
+                e_inter += e;
+                if (d > 0.0)
+                    for (int c = 0; c < 3; ++c) g[3 * a + c] += de * dv[c] / d;
+            }
+            continue;
+        }
         double e, ga[3];
         orc_interp(p, G, L->type[a], x + 3 * a, &e, ga);
         e_inter += e;
@@ -627,3 +646,4 @@ int orc_sizeof_params(void) { return (int)sizeof(orc_params); }
 int orc_sizeof_step_rec(void) { return (int)sizeof(orc_step_rec); }
 int orc_sizeof_ligand(void) { return (int)sizeof(orc_ligand); }
 int orc_sizeof_mdn(void) { return (int)sizeof(orc_mdn); }
+int orc_sizeof_grid(void) { return (int)sizeof(orc_grid); }

@@ -977,3 +977,30 @@ def test_total_energy_is_physics_plus_w_mdn_times_e_mdn(orc):
     one = lambda v: np.array([[[v]]], dtype=np.float64)
     Em, gm, dm = orc.mdn_energy(np.zeros((1, 3)), np.array([0, 1]), one(1.0), one(3.0), one(0.5), np.array([[3.0, 0, 0]]))
     assert Em == pytest.approx(-1.0 / (0.5 * np.sqrt(2 * np.pi)), rel=1e-14) and gm[0, 0] == 0.0
+
+
+def test_direct_receptor_mode_of_the_step_equals_the_direct_sums(orc):
+    """NEXT-3: orc_score_grad handed a DirectReceptor = orc_score_grad_direct (itself pinned against the grid at nodes, the brute
+    force field and central differences); an MC step under it moves downhill in the DIRECT energy."""
+    rec = synth.receptor(150, 15.0, 8, seed=1, grid_n=41, pocket_radius=4.0)
+    radius, role = synth.type_table(8)
+    ty, p = orc.Types(radius, role), orc.default_params()
+    batch = synth.ligands([14], [3], 8, seed=5)
+    L = orc.ligand_from_batch(batch, 0)
+    D = orc.DirectReceptor(rec.xyz, rec.type, 8)
+    rng = np.random.default_rng(2)
+    for s in range(4):
+        pose = synth.random_poses(batch, [0], rec, seed=40 + s, spread=0.5)[0, :7 + L.T].astype(np.float64)
+        e1, g1, x1, ga1 = orc.score_grad(p, ty, D, L, pose)
+        e2, g2, x2, ga2 = orc.score_grad_direct(p, ty, rec.xyz, rec.type, L, pose)
+        assert np.array_equal(e1, e2) and np.array_equal(g1, g2) and np.array_equal(ga1, ga2)
+    # one accepted Adam step (tiny lr, no perturbation amplitude): first-order descent in the direct energy
+    p2 = orc.default_params(lr=1e-5, pert_trans=0.0, pert_rot=0.0)
+    for chain in range(40):
+        u = orc.uniform4(7, chain, 0, 0, 0)
+        if int(u[0] * (L.T + 2)) <= 1:
+            break
+    e0, g0, _, _ = orc.score_grad(p2, ty, D, L, pose)
+    new, e_new, rec_ = orc.mc_step(p2, ty, D, L, 7, chain, 0, 0, rec.box_min, rec.box_max, pose, 1e9)
+    assert rec_.accept == 1
+    assert e_new - e0[0] == pytest.approx(-1e-5 * np.abs(g0).sum(), rel=2e-3)
