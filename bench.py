@@ -35,12 +35,12 @@ UNIT = "score+grad pose evals/s"
 KERNEL_NAMES = {1: "mc_kernel<J> (warp per chain)", 2: "mc_lane_kernel (lane per chain)", 3: "mc_cta_kernel (CTA per chain)",
                 4: "mc_lane_tm_kernel (lane per chain, TMEM)"}
 REGIME = {"C1": "latency", "C2": "latency", "C3": "throughput", "C4": "throughput", "C5": "throughput", "C2x32": "throughput",
-          "P1": "latency", "M3": "throughput"}
+          "P1": "latency", "M3": "throughput", "D2": "latency"}
 MB_FFMA, MB_FFMA2, MB_MUFU, MB_L2_READ, MB_GATHER = range(5)
 
 
 # ----------------------------------------------------------------------------------------- accounting
-def work_of(n_atoms, n_tor, n_pairs, n_chains, n_steps, n_refine, mdn=None):
+def work_of(n_atoms, n_tor, n_pairs, n_chains, n_steps, n_refine, mdn=None, direct=None):
     """Evaluations and ALGORITHMIC work of one step of a workload.  Two kinds of evaluation:
     G = score gradient (what an Adam step needs: FK, trilinear value + gradient, pair forces, reverse pass) and
     E = energy only (the Metropolis evaluation of a step, and the initial one).  Per MC step and chain: n_refine G
@@ -58,6 +58,12 @@ def work_of(n_atoms, n_tor, n_pairs, n_chains, n_steps, n_refine, mdn=None):
         flop_e = flop_e + n * hits * (8 * size + 8 * K)
         xu_g, xu_e = xu_g + n * hits * (K + 1), xu_e + n * hits * (K + 1)
         bytes_eval = bytes_eval + n * hits * (16 * K + 16 * size)
+    if direct:                                 # receptor term by direct sums: pairs within the range per atom instead of the trilinear lookup
+        ppa = direct["pairs_per_atom"]
+        flop_g = flop_g + n * (28 * ppa - 80)
+        flop_e = flop_e + n * (16 * ppa - 45)
+        xu_g, xu_e = xu_g + 2.0 * n * ppa, xu_e + 2.3 * n * ppa
+        bytes_eval = 16 * n * ppa
     g_per_chain = n_steps * n_refine
     e_per_chain = n_steps + 1
     per_chain_flop = g_per_chain * (flop_g + flop_adam) + e_per_chain * flop_e
@@ -217,6 +223,7 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
         del pi, mu, sg
         mdn = dict(K=cfg.mdn_K, n_res=len(res_off) - 1, res_size=float(np.mean(np.diff(res_off))))
     w = work_of(np.diff(batch.atom_off), np.diff(batch.tor_off), ligs.n_pairs, n_chains, cfg.n_steps, gp.n_refine)   # evaluation counts
+    dock_kw = dict(receptor_direct=True) if cfg.direct else {}
     L, k = ligs.n_lig, cfg.top_k
     out = (torch.empty(L, k, 2, device=eng.device), torch.empty(L, k, stride, device=eng.device),
            torch.empty(L, k, dtype=torch.int32, device=eng.device))
@@ -233,7 +240,9 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
 
     def step():
         grid = eng.build_grid(d_xyz, d_typ, radius, role, gp, rec.origin, rec.dims, rec.spacing)
-        eng.dock(grid, ligs, *dock_args, seed=cfg.philox_seed, pose_stride=stride, out=out, chain_base=chain_base)
+        if cfg.direct:
+            eng.attach_receptor(grid, d_xyz, d_typ, radius, role, gp)
+        eng.dock(grid, ligs, *dock_args, seed=cfg.philox_seed, pose_stride=stride, out=out, chain_base=chain_base, **dock_kw)
         merge()
         return grid
 
@@ -256,8 +265,10 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
             flush.zero_()                                                    # L2 flush, outside the timed events
             ev[0].record(eng.stream)
             grid = eng.build_grid(d_xyz, d_typ, radius, role, gp, rec.origin, rec.dims, rec.spacing)
+            if cfg.direct:
+                eng.attach_receptor(grid, d_xyz, d_typ, radius, role, gp)
             ev[1].record(eng.stream)
-            eng.dock(grid, ligs, *dock_args, seed=cfg.philox_seed, pose_stride=stride, out=out, chain_base=chain_base)
+            eng.dock(grid, ligs, *dock_args, seed=cfg.philox_seed, pose_stride=stride, out=out, chain_base=chain_base, **dock_kw)
             merged = merge()
             ev[2].record(eng.stream)
         ev[2].synchronize()
@@ -294,6 +305,16 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
             hits += int((dres < 5.0).sum()); atoms += nl
         mdn["hits_per_atom"] = hits / max(atoms, 1)
         w = work_of(np.diff(batch.atom_off), np.diff(batch.tor_off), ligs.n_pairs, n_chains, cfg.n_steps, gp.n_refine, mdn)
+    direct = None
+    if cfg.direct:                                                           # receptor atoms inside the pair function's range, per ligand atom
+        li = np.zeros(1, np.int32)
+        gtmp = eng.build_grid(d_xyz, d_typ, radius, role, gp, rec.origin, rec.dims, rec.spacing)
+        _, _, xs = eng.score_grad(gtmp, ligs, gp, li, out[1][0, :1, :].contiguous().cpu().numpy(), want_grad=False)
+        gtmp.free()
+        nl = batch.n_atoms(0)
+        dmat = np.linalg.norm(xs[0, :nl, None, :] - rec.xyz[None, :, :], axis=2)
+        direct = dict(pairs_per_atom=float((dmat < gp.long_dmax).sum() / nl))
+        w = work_of(np.diff(batch.atom_off), np.diff(batch.tor_off), ligs.n_pairs, n_chains, cfg.n_steps, gp.n_refine, None, direct)
     grid_bytes = 16 * int(np.prod(rec.dims)) * cfg.n_types                  # the xy-packed copy the kernels gather from
     pk = peaks(eng, grid_bytes)
     mc_ms = float(np.mean(t_mc))
@@ -308,6 +329,8 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
     res["roofline"]["mc_kernel_pose_evals_per_s"] = w["evals"] / (mc_ms * 1e-3)
     if mdn:
         res["mdn"] = mdn
+    if direct:
+        res["direct"] = direct
     if do_e2e:                                                               # host buffers in, host buffers out
         h_out = (np.empty((L, k, 2), np.float32), np.empty((L, k, stride), np.float32), np.empty((L, k), np.int32))
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
@@ -513,8 +536,9 @@ def main():
             extras[name] = {k: r[k] for k in ("title", "evals", "sg_evals", "value", "pose_evals_per_s", "ms_per_step", "ms_per_task",
                                               "ms_grid_build", "ms_mc_kernels", "ms_topk", "launches", "best_energy")}
             rf = r["roofline"]
-            if "mdn" in r:
-                extras[name]["mdn"] = r["mdn"]
+            for kx in ("mdn", "direct"):
+                if kx in r:
+                    extras[name][kx] = r[kx]
             extras[name].update(kernel=rf["kernel"], regime=REGIME.get(name, "?"), bound=rf["bound"], roofline_frac=rf["frac"],
                                 alu_frac=rf["alu_frac"], xu_frac=rf["xu_frac"], l2_frac=rf["l2_frac"],
                                 gather_grid_gbs=rf["peaks"].get("gather_grid_gbs"),

@@ -52,7 +52,7 @@ class _Mdn(C.Structure):
 class _DockOpts(C.Structure):
     _fields_ = [("first_step", C.c_int), ("init_poses", C.c_void_p), ("resume", C.c_int),
                 ("chain_state", C.c_void_p), ("trace", C.c_void_p), ("steps_per_launch", C.c_int),
-                ("no_graph", C.c_int), ("chain_base", C.c_int), ("cluster_rmsd", C.c_float)]
+                ("no_graph", C.c_int), ("chain_base", C.c_int), ("cluster_rmsd", C.c_float), ("receptor_direct", C.c_int)]
 
 
 TRACE_DTYPE = np.dtype([("e_prop", np.float32), ("e_cur", np.float32), ("u", np.float32), ("flags", np.int32)])
@@ -243,6 +243,15 @@ class Engine:
         self._sync_out()
         return Grid(self, h, ty.n_types, dims, origin, spacing)
 
+    def attach_receptor(self, grid: Grid, rec_xyz, rec_type, radius, role, params):
+        """tridsk_grid_attach_receptor: the receptor for dock(..., receptor_direct=True)."""
+        ty, keep = self._types(radius, role)
+        xyz = rec_xyz if not isinstance(rec_xyz, np.ndarray) else np.ascontiguousarray(rec_xyz, np.float32)
+        typ = rec_type if not isinstance(rec_type, np.ndarray) else np.ascontiguousarray(rec_type, np.int32)
+        self._sync_in()
+        self._ck(lib().tridsk_grid_attach_receptor(self.ctx, grid.handle, _ptr(xyz), _ptr(typ), C.c_int(int(xyz.shape[0])), C.byref(ty),
+                                                   C.byref(params)))
+
     def grid_cache(self, budget_bytes=-1):
         """Set the cache's byte budget (-1: leave it) -> dict(hits, misses, grids, bytes)."""
         st = (C.c_longlong * 4)()
@@ -339,7 +348,7 @@ class Engine:
     def dock(self, grid: Grid, ligs: Ligands, params, box_min, box_max, pocket_center, pocket_radius,
              n_chains, n_steps, top_k, seed=0, pose_stride=None, device_out=False, init_poses=None,
              first_step=0, resume=False, chain_state=None, want_state=False, want_trace=False,
-             steps_per_launch=0, no_graph=False, chain_base=0, out=None, cluster_rmsd=0.0):
+             steps_per_launch=0, no_graph=False, chain_base=0, out=None, cluster_rmsd=0.0, receptor_direct=False):
         """-> dict(energy[n_lig,k,2], pose[n_lig,k,stride], chain[n_lig,k], state?, trace?).
         device_out: outputs are CUDA torch tensors (no D2H, no sync); else numpy (D2H inside the call).
         out: optional pre-allocated (energy, pose, chain) buffers to write into."""
@@ -361,6 +370,7 @@ class Engine:
         o.steps_per_launch, o.no_graph = int(steps_per_launch), int(bool(no_graph))
         o.chain_base = int(chain_base)
         o.cluster_rmsd = float(cluster_rmsd)
+        o.receptor_direct = int(bool(receptor_direct))
         keep = []
         if init_poses is not None:
             if isinstance(init_poses, np.ndarray):

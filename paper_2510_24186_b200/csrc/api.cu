@@ -378,9 +378,73 @@ extern "C" int tridsk_grid_export(tridsk_ctx* ctx, const tridsk_grid* grid, floa
     return TRIDSK_OK;
 }
 
+extern "C" int tridsk_grid_attach_receptor(tridsk_ctx* ctx, tridsk_grid* grid, const float* rec_xyz, const int* rec_type, int n_rec,
+                                           const tridsk_types* types, const tridsk_params* params) {
+    if (!ctx || !grid || !rec_xyz || !rec_type || n_rec < 1 || !params) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    int rc = check_types(ctx, types);
+    if (rc) return rc;
+    if ((rc = check_params(ctx, params))) return rc;
+    if (types->n_types != grid->d.n_types) return fail(ctx, TRIDSK_EINVAL, "type table does not match the grid");
+    // host view of the receptor (the cell sort is layout work, no arithmetic of the method)
+    std::vector<float> hx(3 * (size_t)n_rec);
+    std::vector<int> ht(n_rec);
+    CK(cudaMemcpyAsync(hx.data(), rec_xyz, sizeof(float) * hx.size(), cudaMemcpyDefault, ctx->stream));
+    CK(cudaMemcpyAsync(ht.data(), rec_type, sizeof(int) * n_rec, cudaMemcpyDefault, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    float cut = std::max(params->long_dmax, params->hb_dmax);
+    for (int s = 0; s < types->n_types; ++s)
+        for (int t = 0; t < types->n_types; ++t) {
+            const unsigned char rs = types->hb_role[s], rt = types->hb_role[t];
+            const bool hb = ((rs & 1) && (rt & 2)) || ((rs & 2) && (rt & 1));
+            cut = std::max(cut, hb ? params->hb_dclash : types->radius[s] + types->radius[t]);
+        }
+    float lo[3] = {1e30f, 1e30f, 1e30f}, hi[3] = {-1e30f, -1e30f, -1e30f};
+    for (int r = 0; r < n_rec; ++r) {
+        if (ht[r] < 0 || ht[r] >= types->n_types) return fail(ctx, TRIDSK_EINVAL, "receptor atom type out of range");
+        for (int c = 0; c < 3; ++c) { lo[c] = std::min(lo[c], hx[3 * r + c]); hi[c] = std::max(hi[c], hx[3 * r + c]); }
+    }
+    RecDev R;
+    memset(&R, 0, sizeof(R));
+    long long ncell = 1;
+    for (int c = 0; c < 3; ++c) { R.lo[c] = lo[c]; R.nc[c] = std::max(1, (int)std::floor((hi[c] - lo[c]) / cut) + 1); ncell *= R.nc[c]; }
+    if (ncell > (1 << 22)) return fail(ctx, TRIDSK_ELIMIT, "receptor extent / cut-off gives too many cells");
+    R.inv_cell = 1.f / cut; R.cut2 = cut * cut;
+    auto cell_of = [&](int r) {
+        int ci[3];
+        for (int c = 0; c < 3; ++c) ci[c] = std::min(R.nc[c] - 1, std::max(0, (int)std::floor((hx[3 * r + c] - lo[c]) * R.inv_cell)));
+        return (ci[2] * R.nc[1] + ci[1]) * R.nc[0] + ci[0];
+    };
+    std::vector<int> off((size_t)ncell + 1, 0), fillp;
+    for (int r = 0; r < n_rec; ++r) off[cell_of(r) + 1]++;
+    for (long long c = 0; c < ncell; ++c) off[c + 1] += off[c];
+    fillp.assign(off.begin(), off.end() - 1);
+    std::vector<float4> at(n_rec);
+    for (int r = 0; r < n_rec; ++r) {                      // input order inside a cell
+        float tb; memcpy(&tb, &ht[r], sizeof(tb));
+        at[fillp[cell_of(r)]++] = make_float4(hx[3 * r], hx[3 * r + 1], hx[3 * r + 2], tb);
+    }
+    for (int i = 0; i < 4; ++i) if (grid->rd_buf[i]) { cudaFree(grid->rd_buf[i]); grid->rd_buf[i] = nullptr; }
+    cudaError_t e = cudaMalloc(&grid->rd_buf[0], sizeof(float4) * n_rec);
+    if (e == cudaSuccess) e = cudaMalloc(&grid->rd_buf[1], sizeof(int) * (ncell + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&grid->rd_buf[2], sizeof(float) * types->n_types);
+    if (e == cudaSuccess) e = cudaMalloc(&grid->rd_buf[3], types->n_types);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(grid->rd_buf[0], at.data(), sizeof(float4) * n_rec, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(grid->rd_buf[1], off.data(), sizeof(int) * (ncell + 1), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(grid->rd_buf[2], types->radius, sizeof(float) * types->n_types, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(grid->rd_buf[3], types->hb_role, types->n_types, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return fail(ctx, e == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA, std::string("attach_receptor: ") + cudaGetErrorString(e));
+    R.atoms = (const float4*)grid->rd_buf[0]; R.cell_off = (const int*)grid->rd_buf[1];
+    R.radius = (const float*)grid->rd_buf[2]; R.role = (const unsigned char*)grid->rd_buf[3];
+    grid->rd = R;
+    return TRIDSK_OK;
+}
+
 extern "C" void tridsk_free_grid(tridsk_grid* g) {
     if (!g) return;
     if (--g->refs > 0) return;                       // the grid cache (or the caller) still holds it
+    for (int i = 0; i < 4; ++i) if (g->rd_buf[i]) cudaFree(g->rd_buf[i]);
     if (g->ctx_alive && *g->ctx_alive) {             // stream-ordered: later work on the ctx stream may reuse the memory
         if (g->g) cudaFreeAsync(g->g, g->ctx->stream);
         if (g->gp) cudaFreeAsync(g->gp, g->ctx->stream);
@@ -1252,6 +1316,11 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         if (!ligs->has_cta) return fail(ctx, TRIDSK_EINVAL, "the CTA-per-chain mapping needs a ligand batch of at most 1024 ligands");
         if (std::max(ligs->cta_smem[0], ligs->cta_smem[1]) > TRIDSK_SMEM_MAX_CTA)
             return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
+    }
+    if (o.receptor_direct) {                                        // direct pair sums: the warp-per-chain kernel carries that path
+        if (!grid->rd.atoms) return fail(ctx, TRIDSK_EINVAL, "receptor_direct needs tridsk_grid_attach_receptor on this grid");
+        mode = 1;
+        base.rec = grid->rd;
     }
     const bool lane = mode == 2 || mode == 4;
     if (mode == 4 && ligs->mdn.n_res > 0) return fail(ctx, TRIDSK_EINVAL, "the tensor-memory mapping (4) does not evaluate the mixture-density term");

@@ -294,6 +294,37 @@ __device__ __forceinline__ float pair_energy(const DParams& P, float d2, float d
     return e;
 }
 
+// ------------------------------------------------------------------ receptor term by direct pair sums (S:8(f) NEXT-3)
+// The paper's own evaluation (P:103-125, P:353 item 4): e(s_r, t, |x - r_r|) summed over the receptor atoms within the pair
+// function's range -- the 27 cells around the atom's cell, cells and atoms in a fixed order.  No interpolation, no wall.
+template <bool GRAD>
+__device__ __forceinline__ float rec_direct(const RecDev& R, const DParams& P, int type, float x, float y, float z,
+                                            float& gx, float& gy, float& gz) {
+    const float rt = __ldg(R.radius + type);
+    const unsigned char role_t = __ldg(R.role + type);
+    const int cx = (int)floorf((x - R.lo[0]) * R.inv_cell), cy = (int)floorf((y - R.lo[1]) * R.inv_cell), cz = (int)floorf((z - R.lo[2]) * R.inv_cell);
+    float e = 0.f;
+    for (int kz = max(cz - 1, 0); kz <= min(cz + 1, R.nc[2] - 1); ++kz)
+        for (int ky = max(cy - 1, 0); ky <= min(cy + 1, R.nc[1] - 1); ++ky)
+            for (int kx = max(cx - 1, 0); kx <= min(cx + 1, R.nc[0] - 1); ++kx) {
+                const int c = (kz * R.nc[1] + ky) * R.nc[0] + kx;
+                const int r1 = __ldg(R.cell_off + c + 1);
+                for (int r = __ldg(R.cell_off + c); r < r1; ++r) {
+                    const float4 a = __ldg(R.atoms + r);
+                    const float dx = x - a.x, dy = y - a.y, dz = z - a.z;
+                    const float d2 = dx * dx + dy * dy + dz * dz;
+                    if (d2 >= R.cut2) continue;
+                    const int s = __float_as_int(a.w);
+                    const unsigned char role_s = __ldg(R.role + s);
+                    const bool hb = ((role_s & 1) && (role_t & 2)) || ((role_s & 2) && (role_t & 1));
+                    float sod;
+                    e += pair_energy<GRAD>(P, d2, __ldg(R.radius + s) + rt, hb, sod);
+                    if (GRAD) { gx = fmaf(sod, dx, gx); gy = fmaf(sod, dy, gy); gz = fmaf(sod, dz, gz); }
+                }
+            }
+    return e;
+}
+
 // ------------------------------------------------------------------ a3..a6: one pose evaluation
 // In : t[3], unit q[4] (warp-uniform), theta (lane f holds torsion f-1's angle).
 // Out: world coordinates x/y/z[J]; per-lane partial energies e_inter / e_intra (warp_sum them);
@@ -302,7 +333,7 @@ __device__ __forceinline__ float pair_energy(const DParams& P, float d2, float d
 // M.n_res > 0: the mixture-density term (mdn.cuh) of every atom is added to its receptor term; mdn_par = the ligand's block.
 template <int J, bool GRAD>
 __device__ __forceinline__ void eval_pose(const Lig<J>& L, const DGrid& G, const DParams& P,
-                                          const MdnDev& M, const float4* __restrict__ mdn_par,
+                                          const MdnDev& M, const float4* __restrict__ mdn_par, const RecDev& RD,
                                           const float t[3], const float q[4], float theta,
                                           float x[J], float y[J], float z[J],
                                           float& e_inter, float& e_intra,
@@ -361,7 +392,10 @@ __device__ __forceinline__ void eval_pose(const Lig<J>& L, const DGrid& G, const
 #pragma unroll
     for (int j = 0; j < J; ++j) {
         fx[j] = fy[j] = fz[j] = 0.f;
-        if (L.valid[j]) e_inter += grid_interp<GRAD>(G, P.k_wall, L.typ[j], x[j], y[j], z[j], fx[j], fy[j], fz[j]);
+        if (L.valid[j]) {
+            if (RD.atoms) e_inter += rec_direct<GRAD>(RD, P, L.typ[j], x[j], y[j], z[j], fx[j], fy[j], fz[j]);
+            else e_inter += grid_interp<GRAD>(G, P.k_wall, L.typ[j], x[j], y[j], z[j], fx[j], fy[j], fz[j]);
+        }
         if (M.n_res > 0 && L.valid[j]) mdn_atom(M, mdn_par, L.n, j * L.S + lane, x[j], y[j], z[j], 0, 1, GRAD, e_inter, fx[j], fy[j], fz[j]);
     }
 

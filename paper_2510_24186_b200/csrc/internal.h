@@ -57,6 +57,17 @@ struct MdnDev {
     const float4* cell_at;
 };
 
+// Direct-pair receptor mode: the receptor atoms sorted into cubic cells of edge = the pair function's
+// range; atoms == nullptr: the receptor term comes from the grid.
+struct RecDev {
+    const float4* atoms;          // {x, y, z, type bits}, sorted by cell, input order inside a cell
+    const int* cell_off;          // [ncells + 1]
+    const float* radius;          // [n_types]
+    const unsigned char* role;    // [n_types]
+    int nc[3];
+    float lo[3], inv_cell, cut2;
+};
+
 // Per-ligand header.  Atoms are stored in an INTERNAL order (depth-first over the torsion tree) so that
 // the atoms of every torsion's subtree are one contiguous index range; lane l of a chain's warp owns
 // atoms a = j*S + l, j < J ("stripes").
@@ -169,6 +180,7 @@ struct McLaunch {
     int lane_region, tm_cols;     // tensor-memory lane kernel: shared-memory bytes per warp, TMEM columns per CTA
     int lane_minb;                // shared-memory lane kernel: register budget class (launch_bounds min blocks)
     MdnDev mdn;                   // n_res == 0: no mixture-density term
+    RecDev rec;                   // atoms != nullptr: receptor term by direct pair sums (warp-per-chain mapping only)
 };
 
 struct ScoreLaunch {
@@ -298,6 +310,8 @@ struct tridsk_grid {
     float* g = nullptr;
     float4* gp = nullptr;
     DGrid d;
+    RecDev rd = {};               // tridsk_grid_attach_receptor: the receptor for the direct-pair mode
+    void* rd_buf[4] = {nullptr, nullptr, nullptr, nullptr};   // atoms, cell_off, radius, role
 };
 
 struct tridsk_ligands {

@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(TRIDSK_WARPS_PER_CTA * 32) mc_kernel(const McL
             cth = (lane >= 1 && lane <= T) ? PI_F * (2.f * uu - 1.f) : 0.f;
         }
         float ei, ea;
-        eval_pose<J, false>(L, a.grid, P, a.mdn, mdn_par, ct, cq, cth, x, y, z, ei, ea, gt, gw, gth, sP);
+        eval_pose<J, false>(L, a.grid, P, a.mdn, mdn_par, a.rec, ct, cq, cth, x, y, z, ei, ea, gt, gw, gth, sP);
         ecur = warp_sum(ei + ea);
         ebest = ecur;
 #pragma unroll
@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(TRIDSK_WARPS_PER_CTA * 32) mc_kernel(const McL
         float b1p = 1.f, b2p = 1.f;
         for (int rf = 0; rf < P.n_refine; ++rf) {
             float ei, ea;
-            eval_pose<J, true>(L, a.grid, P, a.mdn, mdn_par, pt, pq, pth, x, y, z, ei, ea, gt, gw, gth, sP);
+            eval_pose<J, true>(L, a.grid, P, a.mdn, mdn_par, a.rec, pt, pq, pth, x, y, z, ei, ea, gt, gw, gth, sP);
             b1p *= P.adam_b1; b2p *= P.adam_b2;
             const float c1 = __fdividef(1.f, 1.f - b1p), c2 = __fdividef(1.f, 1.f - b2p);   // 2-ulp division / square root:
             // far inside the tolerance, and the IEEE forms are slow-path subroutines on the chain's critical path
@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(TRIDSK_WARPS_PER_CTA * 32) mc_kernel(const McL
 
         // a8: energy of the refined proposal, Metropolis, best tracking
         float ei, ea;
-        eval_pose<J, false>(L, a.grid, P, a.mdn, mdn_par, pt, pq, pth, x, y, z, ei, ea, gt, gw, gth, sP);
+        eval_pose<J, false>(L, a.grid, P, a.mdn, mdn_par, a.rec, pt, pq, pth, x, y, z, ei, ea, gt, gw, gth, sP);
         const float enew = warp_sum(ei + ea);
         const bool accept = isfinite(enew) && (um < expf(-P.beta * (enew - ecur)));
         if (a.trace != nullptr && lane == 0) {
@@ -188,8 +188,10 @@ __device__ __forceinline__ void score_one(const ScoreLaunch& a, int i, int lig, 
     load_pose(a.poses + (size_t)i * a.pose_stride, L.T, t, q, th);
     quat_normalise(q);
     const float4* mdn_par = a.mdn.n_res > 0 ? a.mdn.par + a.mdn.lig_off[lig] : nullptr;
-    if (a.grad != nullptr) eval_pose<J, true>(L, a.grid, a.P, a.mdn, mdn_par, t, q, th, x, y, z, ei, ea, gt, gw, gth, sP);
-    else eval_pose<J, false>(L, a.grid, a.P, a.mdn, mdn_par, t, q, th, x, y, z, ei, ea, gt, gw, gth, sP);
+    RecDev no_rec;
+    no_rec.atoms = nullptr;
+    if (a.grad != nullptr) eval_pose<J, true>(L, a.grid, a.P, a.mdn, mdn_par, no_rec, t, q, th, x, y, z, ei, ea, gt, gw, gth, sP);
+    else eval_pose<J, false>(L, a.grid, a.P, a.mdn, mdn_par, no_rec, t, q, th, x, y, z, ei, ea, gt, gw, gth, sP);
     ei = warp_sum(ei); ea = warp_sum(ea);
     if (lane == 0) {
         a.energy[3 * (size_t)i] = ei + ea; a.energy[3 * (size_t)i + 1] = ei; a.energy[3 * (size_t)i + 2] = ea;

@@ -957,3 +957,56 @@ def test_zero_quaternion_is_rejected(eng, gp, system):
     init = np.zeros((S["g_ligs"].n_lig, 4, 7 + S["g_ligs"].max_tor), np.float32)
     with pytest.raises(TridskError):
         eng.dock(S["g_grid"], S["g_ligs"], gp, *_dock_args(S), 4, 1, 1, seed=1, init_poses=init)
+
+
+# ------------------------------------------------------------------------------------------- direct-pair receptor mode (S:8(f) NEXT-3)
+def test_dock_with_direct_receptor_sums_matches_oracle(orc, gp, system):
+    """tridsk_dock with receptor_direct: initial energies and teacher-forced MC steps against the oracle step whose receptor
+    term is the plain sum over receptor atoms (orc.DirectReceptor); the mode needs the receptor attached to the grid."""
+    from paper_2510_24186_b200 import Engine, TridskError, split_state
+    S = system
+    eng = Engine(0)
+    rec = S["rec"]
+    grid = eng.grid_from_values(S["G"].g, rec.origin, rec.spacing)
+    ids = [0, 1, 4]
+    b = S["batch"].subset(ids)
+    ligs = eng.load_ligands(b, S["radius"], S["role"])
+    Ls = [S["L"][i] for i in ids]
+    n_chains, seed, stride = 16, 23, 7 + ligs.max_tor
+    with pytest.raises(TridskError):                                             # receptor not attached yet
+        eng.dock(grid, ligs, gp, *_dock_args(S), n_chains, 1, 1, seed=seed, receptor_direct=True)
+    eng.attach_receptor(grid, rec.xyz, rec.type, S["radius"], S["role"], gp)
+    D = orc.DirectReceptor(rec.xyz, rec.type, 16)
+    r = eng.dock(grid, ligs, gp, *_dock_args(S), n_chains, 0, 1, seed=seed, want_state=True, receptor_direct=True)
+    assert eng.last_kernel() == 1
+    state = r["state"]
+    compared = skipped = 0
+    for s in range(4):
+        pc, _, ec, _ = split_state(state.copy(), len(ids), n_chains, stride)
+        r = eng.dock(grid, ligs, gp, *_dock_args(S), n_chains, 1, 1, seed=seed, first_step=s, resume=True, chain_state=state,
+                     want_trace=True, receptor_direct=True)
+        for l, L in enumerate(Ls):
+            for c in range(0, n_chains, 2):
+                tr = r["trace"][l, c, 0]
+                pose = pc[l, c, :7 + L.T].astype(np.float64)
+                e_cur = orc.score_grad(S["p"], S["ty"], D, L, pose, want_grad=False)[0][0]
+                assert close(ec[l, c], e_cur, rtol=1e-4, atol=1e-3), (s, l, c, ec[l, c], e_cur)
+                _, _, rec_ = orc.mc_step(S["p"], S["ty"], D, L, seed, c, s, l, rec.box_min, rec.box_max, pose, e_cur)
+                assert (tr["flags"] >> 8) == rec_.entity and tr["u"] == np.float32(rec_.u)
+                if rec_.min_abs_g < 1e-3 or abs(rec_.u - rec_.p_accept) < 1e-4 * max(1.0, rec_.p_accept):
+                    skipped += 1
+                    continue
+                compared += 1
+                assert close(tr["e_prop"], rec_.e_prop, rtol=1e-3, atol=1e-3), (s, l, c, tr["e_prop"], rec_.e_prop)
+                assert (tr["flags"] & 1) == rec_.accept, (s, l, c)
+    print(f"direct receptor mode, teacher-forced: compared {compared}, skipped {skipped}")
+    assert compared > 0.85 * 4 * 3 * 8
+    # the grid mode on the same grid still gives the interpolated energies
+    r0 = eng.dock(grid, ligs, gp, *_dock_args(S), n_chains, 0, 1, seed=seed, want_state=True)
+    _, _, ec0, _ = split_state(r0["state"], len(ids), n_chains, stride)
+    pc, _, ecd, _ = split_state(eng.dock(grid, ligs, gp, *_dock_args(S), n_chains, 0, 1, seed=seed, want_state=True, receptor_direct=True)["state"],
+                                len(ids), n_chains, stride)
+    assert not np.array_equal(ec0, ecd)
+    e_grid = orc.score_grad(S["p"], S["ty"], S["G"], Ls[0], pc[0, 3, :7 + Ls[0].T].astype(np.float64), want_grad=False)[0][0]
+    assert close(ec0[0, 3], e_grid)
+    ligs.free(); grid.free(); eng.close()

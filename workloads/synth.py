@@ -232,6 +232,7 @@ class Config:
     backbone: int = 0
     sizes: dict = field(default_factory=dict)
     n_refine: int = 1
+    direct: bool = False         # the receptor term by direct pair sums instead of the grid lookup (S:8(f) NEXT-3)
     mdn_K: int = 0               # > 0: the workload carries the mixture-density term with K components per (residue, atom)
 
 
@@ -251,6 +252,9 @@ CONFIGS = {
     # 8(f) NEXT-1), with synthetic mixture parameters (K = 10) on the pocket residues (pocket_residues below).
     "M3": Config("M3", "Screening batch under the full score (E_MDN, K = 10), first 1,024 ligands of C3", 3000, 30.0, 80, 16, 1024, 128, 500, 1,
                  1003, 2003, mdn_K=10),
+    # Not a BASELINE.json config: C2 docked with the receptor term taken the paper's own way, direct sums over the receptor atoms
+    # within the pair function's range, 200 MC steps
+    "D2": Config("D2", "Drug-like single dock, receptor term by direct pair sums", 3000, 30.0, 80, 16, 1, 384, 200, 10, 1002, 2002, direct=True),
     "P1": Config("P1", "Paper-shaped run (1,024 copies x 8 loops x 32 Adam steps)", 3000, 30.0, 80, 16, 1, 1024, 8, 8, 1002, 2002,
                  n_refine=32),
 }
@@ -262,7 +266,7 @@ def config_sizes(cfg: Config, n_lig: int | None = None):
     rng = np.random.default_rng(cfg.lig_seed)
     if cfg.name == "C1":
         return np.full(L, 12), np.full(L, 2)
-    if cfg.name in ("C2", "P1", "C2x32"):
+    if cfg.name in ("C2", "P1", "C2x32", "D2"):
         return np.full(L, 30), np.full(L, 6)
     if cfg.name in ("C3", "M3"):
         n = rng.integers(15, 51, size=4096)
