@@ -505,6 +505,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
     ap.add_argument("--n-lig", type=int, default=None, help="first n ligands of a screening config (profiling)")
+    ap.add_argument("--mc-steps", type=int, default=None, help="override the config's MC steps per chain (profiling only)")
     ap.add_argument("--kernel", type=int, default=0, help="force a chain-to-thread mapping (tridsk_set_kernel); 0 = automatic")
     args = ap.parse_args()
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
@@ -524,6 +525,9 @@ def main():
         torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local))
     eng = Engine(local)
     eng.set_kernel(args.kernel)
+    if args.mc_steps:
+        import dataclasses
+        synth.CONFIGS[args.workload] = dataclasses.replace(synth.CONFIGS[args.workload], n_steps=args.mc_steps)
     args.warmup = max(args.warmup, 3)
     main_res = run_workload(eng, args.workload, args.steps, args.warmup, rank, world, do_e2e=not args.no_e2e, n_lig=args.n_lig)
     extras = {}

@@ -14,17 +14,22 @@
 // nk2 = -log2(e) / (2 sigma^2):  N = a 2^(nk2 (d - mu)^2),  dN/dd = -N (d - mu) / sigma^2.
 // e += w_mdn * (this atom's share of E_MDN); grad: (gx, gy, gz) += its gradient.
 // One (residue, atom) pair whose minimum squared distance best2 is inside the cut-off: the K mixture components.  The
-// records are padded to a multiple of four per pair (M.K4; the padding has zero amplitude), four loads in flight.
-__device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __restrict__ q, float best2, float bx, float by, float bz,
-                                           bool grad, float& e, float& gx, float& gy, float& gz) {
+// records are padded to a multiple of four per pair (M.K4; the padding has zero amplitude), four loads in flight; the first
+// four (c0) were requested by the caller before it searched the residue's atoms.
+__device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __restrict__ q, const float4 c0[4], float best2,
+                                           float bx, float by, float bz, bool grad, float& e, float& gx, float& gy, float& gz) {
     float rinv;
     { const float b = fmaxf(best2, 1e-12f); asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(b)); }
     const float d = best2 * rinv;
     float de = 0.f;
+    float4 c[4] = {c0[0], c0[1], c0[2], c0[3]};
     for (int k0 = 0; k0 < M.K4; k0 += 4) {
-        float4 c[4];
+        float4 cn[4];
+        const bool more = k0 + 4 < M.K4;
+        if (more) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) c[j] = __ldg(q + k0 + j);
+            for (int j = 0; j < 4; ++j) cn[j] = __ldg(q + k0 + 4 + j);
+        }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const float t = d - c[j].y;
@@ -33,6 +38,10 @@ __device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __rest
             N *= c[j].x;
             e -= N;
             de = fmaf(N * t, c[j].w, de);
+        }
+        if (more) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) c[j] = cn[j];
         }
     }
     if (grad) {
@@ -53,11 +62,17 @@ __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restri
     const float cut2 = M.d_cut * M.d_cut;
     // Residue by residue: the first entry of a run holds residue id | run length << 16.  Lanes of a warp sit in different
     // cells, so their runs differ in length; the short inner loop diverges, the costly mixture evaluation after it is
-    // reached by all lanes together once per residue.
+    // reached by all lanes together once per residue.  The loads are L2 round trips: the first four parameter records of the
+    // residue and the first entry of the NEXT run are requested before the run's atoms are searched.
     int ord = 0;
+    float4 a = __ldg(M.cell_at + e0);
     for (int en = e0; en < e1; ++ord) {
-        const float4 a = __ldg(M.cell_at + en);
         const int hdr = __float_as_int(a.w), i = hdr & 0xffff, cnt = hdr >> 16;
+        const float4* q = par + ((size_t)i * n + p) * M.K4;
+        float4 c0[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) c0[j] = __ldg(q + j);
+        const float4 an = __ldg(M.cell_at + min(en + cnt, e1 - 1));
         float bx = x - a.x, by = y - a.y, bz = z - a.z;
         float best2 = bx * bx + by * by + bz * bz;
         for (int r = 1; r < cnt; ++r) {                       // plain minimum, ties -> lowest atom index
@@ -67,7 +82,7 @@ __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restri
             if (d2 < best2) { best2 = d2; bx = dx; by = dy; bz = dz; }
         }
         en += cnt;
-        if (best2 < cut2 && ord % istep == i0)
-            mdn_finish(M, par + ((size_t)i * n + p) * M.K4, best2, bx, by, bz, grad, e, gx, gy, gz);
+        if (best2 < cut2 && ord % istep == i0) mdn_finish(M, q, c0, best2, bx, by, bz, grad, e, gx, gy, gz);
+        a = an;
     }
 }
