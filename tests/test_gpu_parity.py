@@ -14,8 +14,10 @@ pytestmark = pytest.mark.gpu
 
 RTOL, ATOL = 1e-4, 1e-3
 # free-running chains (100 steps, 64 chains): smallest fraction of chains whose every accept/reject decision must equal the
-# oracle's; the measured fractions are printed by the tests
-FREE_RUN_FLOOR = 0.75
+# oracle's.  Measured on B200 under all three mappings: 63/64 (ligand index 0) and 64/64 (index 1 of a batch); the tests print
+# the fraction.  The floor sits just below: a chain may part from the oracle at a Metropolis near-tie or at a
+# sign-unstable first Adam step, nowhere else.
+FREE_RUN_FLOOR = 0.95
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
 
