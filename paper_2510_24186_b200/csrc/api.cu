@@ -6,6 +6,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <omp.h>
+
 #include <algorithm>
 #include <cmath>
 #include <new>
@@ -173,6 +175,7 @@ extern "C" void tridsk_destroy(tridsk_ctx* ctx) {
         if (ctx->side[i]) cudaStreamDestroy(ctx->side[i]);
     }
     for (int i = 0; i < TRIDSK_SCRATCH; ++i) if (ctx->scratch[i]) cudaFree(ctx->scratch[i]);
+    if (ctx->pin) cudaFreeHost(ctx->pin);
     if (ctx->own_stream) cudaStreamDestroy(ctx->stream);
     delete ctx;
 }
@@ -770,8 +773,11 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     std::vector<PackedLig> pk(L);
     // the CTA-per-chain format triples the pair storage: it is the single-dock mapping, so screens do not carry it
     const bool want_cta = L <= TRIDSK_CTA_MAX_LIG;
+    const bool dbg = getenv("TRIDSK_DEBUG") != nullptr;
+    const double t_a = dbg ? omp_get_wtime() : 0.0;
 #pragma omp parallel for schedule(dynamic, 16)
     for (int i = 0; i < L; ++i) pack_ligand(b, types, i, want_cta, pk[i]);
+    const double t_b = dbg ? omp_get_wtime() : 0.0;
     for (int i = 0; i < L; ++i)
         if (pk[i].err) return fail(ctx, pk[i].err, std::string("ligand ") + std::to_string(i) + ": " + pk[i].msg);
 
@@ -798,28 +804,38 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
             lg->cta_smem[k] = std::max(lg->cta_smem[k], cta_layout(h.n, h.T, h.n_pairs).total);
         }
     }
-    std::vector<float4> f4(na);
-    std::vector<int> ai(na);
-    std::vector<FragRec> fr(nf);
-    std::vector<PairRound> rd(std::max<size_t>(nr, 1));
-    std::vector<LaneFrag> lf(nf);
-    std::vector<uint4> lsv(std::max<size_t>(nls, 1));
-    std::vector<LaneRec> lrv(std::max<size_t>(nrec, 1));
-    std::vector<int> crv(std::max<size_t>(ncr, 1));
-    std::vector<uint2> ccv(std::max<size_t>(ncc, 1));
-    std::vector<float> crt(std::max<size_t>(nrt, 1));
+    // One pinned staging block owned by the ctx (grown on demand, reused by later calls) and one device block hold all the
+    // packed arrays back to back; the per-ligand pieces are gathered into the staging block in parallel and go up in one copy.
+    struct Seg { size_t off, bytes; };
+    size_t blob = 0;
+    auto seg = [&](size_t bytes) { Seg sg{blob, bytes}; blob = (blob + std::max<size_t>(bytes, 16) + 255) / 256 * 256; return sg; };
+    const Seg s_hdr = seg(sizeof(LigHdr) * L), s_f4 = seg(sizeof(float4) * na), s_ai = seg(sizeof(int) * na), s_fr = seg(sizeof(FragRec) * nf),
+              s_rd = seg(sizeof(PairRound) * nr), s_lf = seg(sizeof(LaneFrag) * nf), s_ls = seg(sizeof(uint4) * nls),
+              s_lr = seg(sizeof(LaneRec) * nrec), s_cr = seg(sizeof(int) * ncr), s_cc = seg(sizeof(uint2) * ncc), s_rt = seg(sizeof(float) * nrt);
+    if (blob > ctx->pin_bytes) {
+        if (ctx->pin) { cudaStreamSynchronize(ctx->stream); cudaFreeHost(ctx->pin); ctx->pin = nullptr; ctx->pin_bytes = 0; }
+        const size_t cap = blob + blob / 8;
+        if (cudaHostAlloc(&ctx->pin, cap, cudaHostAllocDefault) != cudaSuccess) { cudaGetLastError(); delete lg; return fail(ctx, TRIDSK_ENOMEM, "pinned staging buffer"); }
+        ctx->pin_bytes = cap;
+    } else {
+        cudaStreamSynchronize(ctx->stream);               // an earlier upload may still read the staging block
+    }
+    char* H = (char*)ctx->pin;
+    memcpy(H + s_hdr.off, lg->hdr_h.data(), s_hdr.bytes);
+#pragma omp parallel for schedule(static, 64)
     for (int i = 0; i < L; ++i) {
         const LigHdr& h = pk[i].h;
-        std::copy(pk[i].lane_frags.begin(), pk[i].lane_frags.end(), lf.begin() + h.frag_off);
-        std::copy(pk[i].lane_stream.begin(), pk[i].lane_stream.end(), lsv.begin() + h.ls_off);
-        std::copy(pk[i].lane_recs.begin(), pk[i].lane_recs.end(), lrv.begin() + h.rec_off);
-        std::copy(pk[i].cta_rows.begin(), pk[i].cta_rows.end(), crv.begin() + h.cta_row_off);
-        std::copy(pk[i].cta_recs.begin(), pk[i].cta_recs.end(), ccv.begin() + h.cta_rec_off);
-        if (h.cta_rt_off >= 0) std::copy(pk[i].cta_rtab.begin(), pk[i].cta_rtab.end(), crt.begin() + h.cta_rt_off);
-        std::copy(pk[i].f4.begin(), pk[i].f4.end(), f4.begin() + h.atom_off);
-        std::copy(pk[i].ai.begin(), pk[i].ai.end(), ai.begin() + h.atom_off);
-        std::copy(pk[i].fr.begin(), pk[i].fr.end(), fr.begin() + h.frag_off);
-        std::copy(pk[i].rounds.begin(), pk[i].rounds.end(), rd.begin() + h.round_off);
+        auto put = [&](const Seg& sg, size_t at, const void* src, size_t bytes) { if (bytes) memcpy(H + sg.off + at, src, bytes); };
+        put(s_lf, sizeof(LaneFrag) * h.frag_off, pk[i].lane_frags.data(), sizeof(LaneFrag) * pk[i].lane_frags.size());
+        put(s_ls, sizeof(uint4) * h.ls_off, pk[i].lane_stream.data(), sizeof(uint4) * pk[i].lane_stream.size());
+        put(s_lr, sizeof(LaneRec) * h.rec_off, pk[i].lane_recs.data(), sizeof(LaneRec) * pk[i].lane_recs.size());
+        put(s_cr, sizeof(int) * h.cta_row_off, pk[i].cta_rows.data(), sizeof(int) * pk[i].cta_rows.size());
+        put(s_cc, sizeof(uint2) * h.cta_rec_off, pk[i].cta_recs.data(), sizeof(uint2) * pk[i].cta_recs.size());
+        if (h.cta_rt_off >= 0) put(s_rt, sizeof(float) * h.cta_rt_off, pk[i].cta_rtab.data(), sizeof(float) * pk[i].cta_rtab.size());
+        put(s_f4, sizeof(float4) * h.atom_off, pk[i].f4.data(), sizeof(float4) * pk[i].f4.size());
+        put(s_ai, sizeof(int) * h.atom_off, pk[i].ai.data(), sizeof(int) * pk[i].ai.size());
+        put(s_fr, sizeof(FragRec) * h.frag_off, pk[i].fr.data(), sizeof(FragRec) * pk[i].fr.size());
+        put(s_rd, sizeof(PairRound) * h.round_off, pk[i].rounds.data(), sizeof(PairRound) * pk[i].rounds.size());
     }
     if (getenv("TRIDSK_DEBUG")) {
         long long np = 0;
@@ -830,29 +846,27 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
         for (int i = 0; i < L; ++i) for (int w = 1; w <= 4; ++w) wh[w] += pk[i].w_hist[w];
         fprintf(stderr, "tridsk load_ligands: records by tile width 1..4: %lld %lld %lld %lld\n", wh[1], wh[2], wh[3], wh[4]);
     }
-    cudaError_t e = cudaSuccess;
+    const double t_c = dbg ? omp_get_wtime() : 0.0;
+    cudaError_t e = cudaMalloc(&lg->blob, std::max<size_t>(blob, 256));
+    if (e == cudaSuccess && blob) e = cudaMemcpyAsync(lg->blob, H, blob, cudaMemcpyHostToDevice, ctx->stream);
+    char* D = (char*)lg->blob;
+    lg->hdr = (LigHdr*)(D + s_hdr.off); lg->atom_f4 = (float4*)(D + s_f4.off); lg->atom_i = (int*)(D + s_ai.off);
+    lg->frags = (FragRec*)(D + s_fr.off); lg->rounds = (PairRound*)(D + s_rd.off); lg->lane_frags = (LaneFrag*)(D + s_lf.off);
+    lg->lane_stream = (uint4*)(D + s_ls.off); lg->lane_recs = (LaneRec*)(D + s_lr.off); lg->cta_rows = (int*)(D + s_cr.off);
+    lg->cta_recs = (uint2*)(D + s_cc.off); lg->cta_rtab = (float*)(D + s_rt.off);
     auto up = [&](void** d, const void* src, size_t bytes) {
         if (e != cudaSuccess) return;
         e = cudaMalloc(d, std::max<size_t>(bytes, 16));
         if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(*d, src, bytes, cudaMemcpyHostToDevice, ctx->stream);
     };
-    up((void**)&lg->hdr, lg->hdr_h.data(), sizeof(LigHdr) * L);
-    up((void**)&lg->atom_f4, f4.data(), sizeof(float4) * na);
-    up((void**)&lg->atom_i, ai.data(), sizeof(int) * na);
-    up((void**)&lg->frags, fr.data(), sizeof(FragRec) * nf);
-    up((void**)&lg->rounds, rd.data(), sizeof(PairRound) * rd.size());
-    up((void**)&lg->lane_frags, lf.data(), sizeof(LaneFrag) * nf);
-    up((void**)&lg->lane_stream, lsv.data(), sizeof(uint4) * lsv.size());
-    up((void**)&lg->lane_recs, lrv.data(), sizeof(LaneRec) * lrv.size());
-    up((void**)&lg->cta_rows, crv.data(), sizeof(int) * crv.size());
-    up((void**)&lg->cta_recs, ccv.data(), sizeof(uint2) * ccv.size());
-    up((void**)&lg->cta_rtab, crt.data(), sizeof(float) * crt.size());
     for (int k = 0; k < 2; ++k)
         if (!lg->cta_bucket[k].empty()) up((void**)&lg->cta_bucket_dev[k], lg->cta_bucket[k].data(), sizeof(int) * lg->cta_bucket[k].size());
     if (e == cudaSuccess) e = cudaMalloc((void**)&lg->all_ids, sizeof(int) * std::max(L, 1));
     for (int j = 1; j <= TRIDSK_MAX_J; ++j)
         if (!lg->bucket[j].empty()) up((void**)&lg->bucket_dev[j], lg->bucket[j].data(), sizeof(int) * lg->bucket[j].size());
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (dbg) fprintf(stderr, "tridsk load_ligands: pack %.1f ms (%d threads), gather %.1f ms, upload %.1f ms\n", (t_b - t_a) * 1e3, omp_get_max_threads(),
+                     (t_c - t_b) * 1e3, (omp_get_wtime() - t_c) * 1e3);
     if (e != cudaSuccess) {
         tridsk_free_ligands(lg);
         return fail(ctx, e == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA, std::string("load_ligands: ") + cudaGetErrorString(e));
@@ -981,8 +995,7 @@ extern "C" int tridsk_load_mdn(tridsk_ctx* ctx, tridsk_ligands* ligs, const trid
 extern "C" void tridsk_free_ligands(tridsk_ligands* l) {
     if (!l) return;                 // cudaFree waits for the device; l->ctx may already be destroyed
     free_mdn(l);
-    cudaFree(l->hdr); cudaFree(l->atom_f4); cudaFree(l->atom_i); cudaFree(l->frags); cudaFree(l->rounds);
-    cudaFree(l->lane_frags); cudaFree(l->lane_stream); cudaFree(l->lane_recs); cudaFree(l->cta_rows); cudaFree(l->cta_recs); cudaFree(l->cta_rtab); cudaFree(l->all_ids);
+    cudaFree(l->blob); cudaFree(l->all_ids);       // the packed arrays are pieces of one block
     for (int k = 0; k < 2; ++k) if (l->cta_bucket_dev[k]) cudaFree(l->cta_bucket_dev[k]);
     for (int j = 0; j <= TRIDSK_MAX_J; ++j) if (l->bucket_dev[j]) cudaFree(l->bucket_dev[j]);
     delete l;

@@ -283,6 +283,8 @@ struct tridsk_ctx {
     // scratch owned by the ctx (grown on demand)
     void* scratch[TRIDSK_SCRATCH] = {};
     size_t scratch_bytes[TRIDSK_SCRATCH] = {};
+    void* pin = nullptr;          // pinned host staging block of tridsk_load_ligands (grown on demand)
+    size_t pin_bytes = 0;
     // cached CUDA graph of the last dock launch series
     cudaGraphExec_t graph_exec = nullptr;
     std::vector<unsigned char> graph_key;
@@ -320,6 +322,7 @@ struct tridsk_ligands {
     std::vector<LigHdr> hdr_h;
     std::vector<int> n_pairs;
     std::vector<int> bucket[TRIDSK_MAX_J + 1];   // ligand ids per J
+    void* blob = nullptr;         // one device block holds all the packed arrays below
     LigHdr* hdr = nullptr;
     float4* atom_f4 = nullptr;
     int* atom_i = nullptr;
