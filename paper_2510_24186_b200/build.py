@@ -12,8 +12,9 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtridsk.so")
 SOURCES = ["api.cu", "mc_kernel.cu", "mc_lane.cu", "mc_cta.cu", "grid_build.cu", "topk.cu", "score_direct.cu", "microbench.cu", "mdn.cu"]
 HEADERS = ["internal.h", "chain.cuh", "mdn.cuh", os.path.join("..", "..", "include", "tridsk.h")]
+# TRIDSK_NVCC_EXTRA: extra nvcc flags for experiments (e.g. "-DLANE_F32X2"); part of the content hash
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC,-fopenmp", "--expt-relaxed-constexpr"]
+              "-Xcompiler", "-fPIC,-fopenmp", "--expt-relaxed-constexpr"] + os.environ.get("TRIDSK_NVCC_EXTRA", "").split()
 
 
 def _digest(paths, extra="") -> str:

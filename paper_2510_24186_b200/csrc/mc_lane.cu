@@ -386,6 +386,90 @@ __device__ __forceinline__ void lane_rec(const PairK& K, const float ax[4], cons
     }
 }
 
+#ifdef LANE_F32X2
+// Experimental: the same record with the FP32 arithmetic of slot pairs (0,1) and (2,3) as packed
+// add / mul / fma.rn.f32x2 on 64-bit register pairs kept from the tile load to the force accumulation.
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk2(float a, float b) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void up2(u64 v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+template <bool GRAD, bool ENERGY>
+__device__ __forceinline__ void lane_rec2(const PairK& K, const u64 ax[2], const u64 ay[2], const u64 az[2],
+                                          float bx, float by, float bz, const float4 c4, unsigned hbmask,
+                                          float& eL, float& eC, float& eH, u64 fx[2], u64 fy[2], u64 fz[2]) {
+    const u64 bxx = pk2(bx, bx), byy = pk2(by, by), bzz = pk2(bz, bz);
+    const u64 eps2 = pk2(1e-12f, 1e-12f), nk22 = pk2(K.nk2, K.nk2), nkc2 = pk2(K.nkc, K.nkc);
+    const float cs[4] = {c4.x, c4.y, c4.z, c4.w};
+    float q[4];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const u64 c = pk2(cs[2 * h], cs[2 * h + 1]);
+        const u64 dx = sub2(ax[h], bxx), dy = sub2(ay[h], byy), dz = sub2(az[h], bzz);
+        const u64 d2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, eps2)));
+        float d2a, d2b;
+        up2(d2, d2a, d2b);
+        const float ra = rsqrt_approx(d2a), rb = rsqrt_approx(d2b);
+        const u64 rinv = pk2(ra, rb);
+        const u64 d = mul2(d2, rinv);
+        const u64 t = sub2(d, c);
+        const u64 u = mul2(t, nk22);
+        const u64 ut = mul2(u, t);
+        float uta, utb, da, db, ta, tb;
+        up2(ut, uta, utb); up2(d, da, db); up2(t, ta, tb);
+        float ga = ex2_approx(uta), gb = ex2_approx(utb);
+        ga = da < K.dmax ? ga : 0.f;
+        gb = db < K.dmax ? gb : 0.f;
+        if (ENERGY) {
+            eL += ga + gb;
+            float dca = cs[2 * h] - K.mu, dcb = cs[2 * h + 1] - K.mu;
+            if (hbmask) {
+                dca = ((hbmask >> (2 * h)) & 1u) ? K.hb_dclash : dca;
+                dcb = ((hbmask >> (2 * h + 1)) & 1u) ? K.hb_dclash : dcb;
+            }
+            q[2 * h] = fmaxf(dca * fminf(ra, K.inv_floor), 1.f);
+            q[2 * h + 1] = fmaxf(dcb * fminf(rb, K.inv_floor), 1.f);
+        }
+        if (GRAD) {
+            const float ina = (ta < K.neg_mu && ra < K.inv_floor) ? 1.f : 0.f, inb = (tb < K.neg_mu && rb < K.inv_floor) ? 1.f : 0.f;
+            u64 s = mul2(rinv, fma2(pk2(ina, inb), mul2(nkc2, rinv), mul2(u, pk2(ga, gb))));
+            if (hbmask) {
+                float sa, sb;
+                up2(s, sa, sb);
+                float sv[2] = {sa, sb};
+                const float dv[2] = {da, db}, tv[2] = {ta, tb}, rv[2] = {ra, rb};
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    if ((hbmask >> (2 * h + j)) & 1u) {
+                        const float th = dv[j] - K.hb_mu;
+                        float gh = ex2_approx(K.hb_nk2 * th * th);
+                        gh = dv[j] < K.hb_dmax ? gh : 0.f;
+                        if (ENERGY) eH += gh;
+                        sv[j] = fmaf(K.kh * th, gh * rv[j], sv[j]);
+                        const bool plain = tv[j] < K.neg_mu, hb = dv[j] < K.hb_dclash;
+                        if (plain != hb && rv[j] < K.inv_floor) sv[j] = fmaf(hb ? K.nkc : -K.nkc, rv[j] * rv[j], sv[j]);
+                    }
+                }
+                s = pk2(sv[0], sv[1]);
+            }
+            fx[h] = fma2(s, dx, fx[h]); fy[h] = fma2(s, dy, fy[h]); fz[h] = fma2(s, dz, fz[h]);
+        } else if (ENERGY && hbmask) {
+            const float dv[2] = {da, db};
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                if ((hbmask >> (2 * h + j)) & 1u) {
+                    const float th = dv[j] - K.hb_mu;
+                    float gh = ex2_approx(K.hb_nk2 * th * th);
+                    eH += dv[j] < K.hb_dmax ? gh : 0.f;
+                }
+            }
+        }
+    }
+    if (ENERGY) eC += lg2_approx((q[0] * q[1]) * (q[2] * q[3]));
+}
+#endif
+
 // The record stream is read one record ahead, across run, tile and fragment boundaries: `mt` / (bx, by, bz) always hold
 // the NEXT record's word and its partner's coordinates (a dependent load), so no run starts with an exposed load.
 struct PairCursor {
@@ -412,6 +496,11 @@ __device__ __forceinline__ void lane_tile(PairCursor& pc, int a0, int w, int n_r
         const uint4 rh = *pc.hp++;
         const int fb = (int)rh.x;
         const uint32_t* const rend = pc.rm + rh.y;
+#ifdef LANE_F32X2
+        const u64 pax[2] = {pk2(ax[0], ax[1]), pk2(ax[2], ax[3])}, pay[2] = {pk2(ay[0], ay[1]), pk2(ay[2], ay[3])},
+                  paz[2] = {pk2(az[0], az[1]), pk2(az[2], az[3])};
+        u64 pfx[2] = {0ull, 0ull}, pfy[2] = {0ull, 0ull}, pfz[2] = {0ull, 0ull};
+#endif
         float fx[4], fy[4], fz[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) fx[i] = fy[i] = fz[i] = 0.f;
@@ -421,9 +510,20 @@ __device__ __forceinline__ void lane_tile(PairCursor& pc, int a0, int w, int n_r
             float nx, ny, nz;
             X.fence(pc.bx, pc.by, pc.bz);
             X.get(mtn & 0xffffu, nx, ny, nz);
+#ifdef LANE_F32X2
+            lane_rec2<GRAD, ENERGY>(K, pax, pay, paz, pc.bx, pc.by, pc.bz, c4, pc.mt >> 16, eL, eC, eH, pfx, pfy, pfz);
+#else
             lane_rec<GRAD, ENERGY>(K, ax, ay, az, pc.bx, pc.by, pc.bz, c4, pc.mt >> 16, eL, eC, eH, fx, fy, fz);
+#endif
             pc.mt = mtn; pc.bx = nx; pc.by = ny; pc.bz = nz;
         } while (pc.rm != rend);
+#ifdef LANE_F32X2
+        if (GRAD) {
+            up2(pfx[0], fx[0], fx[1]); up2(pfx[1], fx[2], fx[3]);
+            up2(pfy[0], fy[0], fy[1]); up2(pfy[1], fy[2], fy[3]);
+            up2(pfz[0], fz[0], fz[1]); up2(pfz[1], fz[2], fz[3]);
+        }
+#endif
         if (GRAD) {
             float wv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
