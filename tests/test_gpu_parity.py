@@ -1012,3 +1012,40 @@ def test_dock_with_direct_receptor_sums_matches_oracle(orc, gp, system):
     e_grid = orc.score_grad(S["p"], S["ty"], S["G"], Ls[0], pc[0, 3, :7 + Ls[0].T].astype(np.float64), want_grad=False)[0][0]
     assert close(ec0[0, 3], e_grid)
     ligs.free(); grid.free(); eng.close()
+
+
+def test_m3_shaped_screen_under_the_full_score_sampled_against_oracle(orc, gp):
+    """The launch configuration bench.py times for M3 (C3 receptor and ligands, GPU-built grid, pocket residues, K = 10, 128 chains,
+    automatic mapping = lane per chain with the E_MDN instance), on the first 96 ligands and 60 MC steps: sampled returned poses are
+    re-scored by the oracle -- receptor term from the paper's plain sums at the touched nodes, E_MDN from orc_mdn_energy."""
+    from paper_2510_24186_b200 import Engine
+    cfg = synth.CONFIGS["M3"]
+    rec = synth.make_receptor(cfg)
+    radius, role = synth.type_table(cfg.n_types)
+    batch = synth.make_ligands(cfg, 96)
+    eng = Engine(0)
+    grid = eng.build_grid(rec.xyz, rec.type, radius, role, gp, rec.origin, rec.dims, rec.spacing)
+    ligs = eng.load_ligands(batch, radius, role)
+    res_xyz, res_off = synth.pocket_residues(rec)
+    n_at = np.diff(batch.atom_off)
+    pi, mu, sg = synth.gmm_batch(len(res_off) - 1, n_at, cfg.mdn_K, seed=cfg.lig_seed + 50000)
+    eng.load_mdn(ligs, res_xyz, res_off, pi, mu, sg, cfg.mdn_K)
+    r = eng.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, cfg.n_chains, 60, 1, seed=cfg.philox_seed)
+    assert eng.last_kernel() == 2
+    ty, p = orc.Types(radius, role), orc.default_params()
+    blk = np.concatenate([[0], np.cumsum((len(res_off) - 1) * n_at * cfg.mdn_K)])
+    with_term = 0
+    for l in range(0, 96, 8):
+        L = orc.ligand_from_batch(batch, l)
+        shp = (len(res_off) - 1, L.n, cfg.mdn_K)
+        M = orc.Mdn(res_xyz, res_off, pi[blk[l]:blk[l + 1]].reshape(shp), mu[blk[l]:blk[l + 1]].reshape(shp), sg[blk[l]:blk[l + 1]].reshape(shp))
+        pose = r["pose"][l, 0, :7 + L.T].astype(np.float64)
+        x = orc.fk(L, pose)
+        G = _sparse_oracle_grid(orc, p, ty, rec, x, L.type)
+        e_phys = orc.score_grad(p, ty, G, L, pose, want_grad=False)[0][0]
+        L.set_mdn(M)
+        eo = orc.score_grad(p, ty, G, L, pose, want_grad=False)[0][0]
+        with_term += (e_phys - eo) > 0.05
+        assert close(r["energy"][l, 0, 0], eo, rtol=2e-4, atol=2e-3), (l, r["energy"][l, 0, 0], eo)
+    assert with_term >= 8                                                       # the docked poses sit in range of pocket residues
+    ligs.free(); grid.free(); eng.close()
