@@ -209,7 +209,7 @@ static int new_grid(tridsk_ctx* ctx, int n_types, const float origin[3], const i
     g->d.h = spacing; g->d.inv_h = 1.0f / spacing;
     cudaError_t e = cudaMallocFromPoolAsync((void**)&g->g, sizeof(float) * g->d.plane * n_types, ctx->pool, ctx->stream);
     if (e == cudaSuccess)                                                                  // xy-packed copy (DGrid::gp)
-        e = cudaMallocFromPoolAsync((void**)&g->gp, sizeof(float4) * g->d.plane * n_types, ctx->pool, ctx->stream);
+        e = cudaMallocFromPoolAsync((void**)&g->gp, 2 * sizeof(float4) * g->d.plane * n_types, ctx->pool, ctx->stream);
     if (e != cudaSuccess) {
         if (g->g) cudaFreeAsync(g->g, ctx->stream);
         delete g;
@@ -337,7 +337,7 @@ extern "C" int tridsk_build_grid_cached(tridsk_ctx* ctx, const float* rec_xyz, c
     rc = tridsk_build_grid(ctx, rec_xyz, rec_type, n_rec, types, params, origin, dims, spacing, &g);
     if (rc) return rc;
     ++ctx->cache_misses;
-    const size_t bytes = (sizeof(float) + sizeof(float4)) * g->d.plane * g->d.n_types;
+    const size_t bytes = (sizeof(float) + 2 * sizeof(float4)) * g->d.plane * g->d.n_types;
     if (bytes <= ctx->cache_budget) {
         ++g->refs;
         ctx->grid_cache.insert(ctx->grid_cache.begin(), {key, bytes, g});

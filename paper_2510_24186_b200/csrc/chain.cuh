@@ -186,8 +186,8 @@ __device__ __forceinline__ float grid_interp(const DGrid& G, float k_wall, int t
     return e;
 }
 
-// The same interpolant read from the xy-packed copy of the grid (DGrid::gp): the 8 corners of a cell are two
-// aligned 16-byte records (z and z+1), i.e. 2 load instructions and 2 cache lines per atom instead of 8 and 4.
+// The same interpolant read from the cell-packed copy of the grid (DGrid::gp): the 8 corners of a cell are one
+// aligned 32-byte record (the quads of z and z+1), i.e. one sector per atom instead of 8 loads over 4 lines.
 // Arithmetic and operation order are those of grid_interp, so both give bit-identical results.
 template <bool GRAD>
 __device__ __forceinline__ float grid_interp_packed(const DGrid& G, float k_wall, int type, float x, float y, float z,
@@ -198,8 +198,8 @@ __device__ __forceinline__ float grid_interp_packed(const DGrid& G, float k_wall
     const float cz = fminf(fmaxf(uz, 0.f), (float)(G.nz - 1));
     const int ix = min((int)cx, G.nx - 2), iy = min((int)cy, G.ny - 2), iz = min((int)cz, G.nz - 2);
     const float fx = cx - (float)ix, fy = cy - (float)iy, fz = cz - (float)iz;
-    const float4* p = G.gp + (size_t)type * G.plane + ((size_t)iz * G.ny + iy) * G.nx + ix;
-    const float4 lo = __ldg(p), hi = __ldg(p + (size_t)G.nx * G.ny);
+    const float4* p = G.gp + 2 * ((size_t)type * G.plane + ((size_t)iz * G.ny + iy) * G.nx + ix);
+    const float4 lo = __ldg(p), hi = __ldg(p + 1);
     const float v000 = lo.x, v001 = lo.y, v010 = lo.z, v011 = lo.w, v100 = hi.x, v101 = hi.y, v110 = hi.z, v111 = hi.w;
     const float d00 = v001 - v000, d01 = v011 - v010, d10 = v101 - v100, d11 = v111 - v110;
     const float a00 = fmaf(fx, d00, v000), a01 = fmaf(fx, d01, v010), a10 = fmaf(fx, d10, v100), a11 = fmaf(fx, d11, v110);
@@ -238,7 +238,7 @@ __device__ __forceinline__ GridCell grid_locate(const DGrid& G, int type, float 
     const float cz = fminf(fmaxf(uz, 0.f), (float)(G.nz - 1));
     const int ix = min((int)cx, G.nx - 2), iy = min((int)cy, G.ny - 2), iz = min((int)cz, G.nz - 2);
     c.fx = cx - (float)ix; c.fy = cy - (float)iy; c.fz = cz - (float)iz;
-    c.p = G.gp + (size_t)type * G.plane + ((size_t)iz * G.ny + iy) * G.nx + ix;
+    c.p = G.gp + 2 * ((size_t)type * G.plane + ((size_t)iz * G.ny + iy) * G.nx + ix);
     c.clx = (cx != ux); c.cly = (cy != uy); c.clz = (cz != uz);
     c.wx = c.clx ? x - (G.ox + cx * G.h) : 0.f;
     c.wy = c.cly ? y - (G.oy + cy * G.h) : 0.f;

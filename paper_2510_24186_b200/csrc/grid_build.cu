@@ -233,15 +233,19 @@ cudaError_t launch_grid_build(cudaStream_t s, const float4* rec, int n_rec, cons
 
 // ------------------------------------------------------------------ xy-packed copy of the grid (DGrid::gp)
 // gp[t][z][y][x] = {g(x,y), g(x+1,y), g(x,y+1), g(x+1,y+1)} at the same (t, z); indices clamped at the upper
-// edges (those records are never the base of a cell: i0 <= n - 2).  The 8 corners of a trilinear cell are then two
-// aligned 16-byte records, which is what the chain kernels gather.
+// edges (those records are never the base of a cell: i0 <= n - 2).  The 8 corners of a trilinear cell -- the xy
+// quad of plane z and the quad of plane z + 1 -- are then ONE aligned 32-byte record (one L2 sector; one 256-bit load on
+// sm_100), which is what the chain kernels gather.
 __global__ void __launch_bounds__(256) grid_pack_kernel(const DGrid G, float4* __restrict__ out) {
     const size_t total = G.plane * (size_t)G.n_types;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int x = (int)(i % G.nx), y = (int)((i / G.nx) % G.ny);
         const int dx = (x + 1 < G.nx) ? 1 : 0;
         const size_t dy = (y + 1 < G.ny) ? (size_t)G.nx : 0;
-        out[i] = make_float4(G.g[i], G.g[i + dx], G.g[i + dy], G.g[i + dy + dx]);
+        const int z = (int)((i / ((size_t)G.nx * G.ny)) % G.nz);
+        const size_t dz = (z + 1 < G.nz) ? (size_t)G.nx * G.ny : 0;         // the record above (clamped at the top plane)
+        out[2 * i] = make_float4(G.g[i], G.g[i + dx], G.g[i + dy], G.g[i + dy + dx]);
+        out[2 * i + 1] = make_float4(G.g[i + dz], G.g[i + dz + dx], G.g[i + dz + dy], G.g[i + dz + dy + dx]);
     }
 }
 

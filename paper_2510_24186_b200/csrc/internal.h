@@ -32,7 +32,8 @@ struct DParams {
 // Receptor grid: fp32 planes [type][z][y][x] (x fastest).
 struct DGrid {
     const float* g;
-    const float4* gp;             // xy-packed copy: gp[t][z][y][x] = {g(x,y), g(x+1,y), g(x,y+1), g(x+1,y+1)} (edges clamped)
+    const float4* gp;             // cell-packed copy, 32 bytes per node: gp[2 * node] = {g(x,y), g(x+1,y), g(x,y+1), g(x+1,y+1)} at z, gp[2 * node + 1]
+                                  // = the same at z + 1 (edges clamped): the 8 corners of the trilinear cell based at the node in one sector
     int nx, ny, nz, n_types;
     size_t plane;                 // nx*ny*nz
     float ox, oy, oz, h, inv_h;

@@ -249,7 +249,7 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     if (lead) {
         S.X[atom] = x; S.X[n + atom] = y; S.X[2 * n + atom] = z;
         cell = grid_locate(G, m & 0xff, x, y, z);
-        glo = __ldg(cell.p); ghi = __ldg(cell.p + (size_t)G.nx * G.ny);
+        glo = __ldg(cell.p); ghi = __ldg(cell.p + 1);
     }
     __syncthreads();
 

@@ -178,10 +178,15 @@ __device__ __forceinline__ void lane_fk(const LaneTopo& S, const float t[3], con
 }
 
 // ------------------------------------------------------------------ a4 receptor energy (O5)
-// Two 16-byte records of the xy-packed grid per atom.  The common case -- the atom lies inside the grid -- takes a short
+// One 32-byte record of the cell-packed grid per atom (a 256-bit load).  The common case -- the atom lies inside the grid -- takes a short
 // path (u = x * inv_h - origin * inv_h by one FMA, floor, fraction, one unsigned range test per axis); an atom on or
 // beyond the boundary takes the general clamp of O5 and raises c.cl (bit i: axis i clamped), which sends the blend
 // through the wall terms (G8).
+// the 32-byte cell record (DGrid::gp) by one 256-bit load
+__device__ __forceinline__ void ldg_cell(const float4* p, float4& lo, float4& hi) {
+    asm("ld.global.nc.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=f"(lo.x), "=f"(lo.y), "=f"(lo.z), "=f"(lo.w), "=f"(hi.x), "=f"(hi.y), "=f"(hi.z), "=f"(hi.w) : "l"(p));
+}
 struct LaneCell {
     const float4* p;
     float fx, fy, fz;
@@ -203,7 +208,7 @@ __device__ __forceinline__ LaneCell lane_locate(const DGrid& G, const LaneGridK&
         c.fx = cx - (float)ix; c.fy = cy - (float)iy; c.fz = cz - (float)iz;
         c.cl = (cx != vx ? 1 : 0) | (cy != vy ? 2 : 0) | (cz != vz ? 4 : 0);
     }
-    c.p = G.gp + (size_t)type * G.plane + ((size_t)iz * G.ny + iy) * G.nx + ix;
+    c.p = G.gp + 2 * ((size_t)type * G.plane + ((size_t)iz * G.ny + iy) * G.nx + ix);
     return c;
 }
 // value, and (grad, warp-uniform) the gradient in GRID units: the caller multiplies by inv_h
@@ -261,7 +266,6 @@ __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, fl
     float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     int gcur = 0;
     const int n = S.n;
-    const size_t zs = (size_t)G.nx * G.ny;
     float x[LANE_GD], y[LANE_GD], z[LANE_GD];
     int m[LANE_GD];
     LaneCell c[LANE_GD];
@@ -273,7 +277,7 @@ __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, fl
         X.get(XS::kScale * (uint32_t)a, x[k], y[k], z[k]);
         X.fence(x[k], y[k], z[k]);
         c[k] = lane_locate(G, Q, m[k] & 0xff, x[k], y[k], z[k]);
-        lo[k] = __ldg(c[k].p); hi[k] = __ldg(c[k].p + zs);
+        ldg_cell(c[k].p, lo[k], hi[k]);
     }
     for (int a0 = 0; a0 < n; a0 += LANE_GD) {
 #pragma unroll
@@ -286,7 +290,7 @@ __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, fl
                 X.get(XS::kScale * (uint32_t)a, x[sl], y[sl], z[sl]);
                 X.fence(x[sl], y[sl], z[sl]);
                 c[sl] = lane_locate(G, Q, m[sl] & 0xff, x[sl], y[sl], z[sl]);
-                lo[sl] = __ldg(c[sl].p); hi[sl] = __ldg(c[sl].p + zs);
+                ldg_cell(c[sl].p, lo[sl], hi[sl]);
             }
             if (a0 + k < n) {                                   // blend atom a0 + k
                 float gx, gy, gz;
