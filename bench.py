@@ -105,7 +105,7 @@ def peaks(eng=None, grid_bytes=None):
     out.update(_PEAKS)
     if grid_bytes:
         ms, work = eng.microbench(MB_GATHER, int(grid_bytes), 400)
-        out["gather_grid_gbs"] = work / (ms * 1e-3) / 1e9                           # random sectors of a buffer of the packed grid's size
+        out["gather_grid_gbs"] = work / (ms * 1e-3) / 1e9                           # random sectors of a buffer of the cell-packed grid's size
         out["gather_grid_bytes"] = int(grid_bytes)
     return out
 
@@ -315,7 +315,7 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
         dmat = np.linalg.norm(xs[0, :nl, None, :] - rec.xyz[None, :, :], axis=2)
         direct = dict(pairs_per_atom=float((dmat < gp.long_dmax).sum() / nl))
         w = work_of(np.diff(batch.atom_off), np.diff(batch.tor_off), ligs.n_pairs, n_chains, cfg.n_steps, gp.n_refine, None, direct)
-    grid_bytes = 16 * int(np.prod(rec.dims)) * cfg.n_types                  # the xy-packed copy the kernels gather from
+    grid_bytes = 32 * int(np.prod(rec.dims)) * cfg.n_types                  # the cell-packed copy the kernels gather from (32 B per node)
     pk = peaks(eng, grid_bytes)
     mc_ms = float(np.mean(t_mc))
     res = dict(
