@@ -50,7 +50,7 @@ struct MdnDev {
     float d_cut;
     // cell list: a uniform grid over the residues' bounding box grown by d_cut; cell c holds, as ONE contiguous stream
     // sorted by (residue, atom index), every receptor atom {x, y, z, residue id} within d_cut + half a cell diagonal of the
-    // cell's centre.  For a point of the cell, a residue's minimum over the listed atoms equals its true minimum distance
+    // cell's centre (runs padded to an even number of entries).  For a point of the cell, a residue's minimum over the listed atoms equals its true minimum distance
     // whenever that is below d_cut (the arg-min atom is then listed), and is >= d_cut otherwise.
     float glo[3], inv_cell;
     int nc[3];

@@ -68,7 +68,7 @@ cudaError_t launch_mdn_pack(cudaStream_t s, const LigHdr* hdr, const int* atom_i
 
 // One thread per cell of the cell list: the receptor atoms within d_cut + half a cell diagonal of the cell's centre, in
 // (residue, atom index) order; the first entry of a residue's run carries residue id | run length << 16 in w, the others
-// the residue id.  fill = false: counts[c] = how many; fill = true: written to cell_at[off[c] ..].
+// the residue id; runs are padded to an even length (32-byte alignment for 256-bit loads).  fill = false: counts[c] = how many; fill = true: written to cell_at[off[c] ..].
 __global__ void mdn_cell_kernel(MdnDev M, float cell, bool fill, int* __restrict__ counts_or_off, float4* __restrict__ cell_at) {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     const int ncell = M.nc[0] * M.nc[1] * M.nc[2];
@@ -93,6 +93,10 @@ __global__ void mdn_cell_kernel(MdnDev M, float cell, bool fill, int* __restrict
                 if (fill) dst[n] = make_float4(a.x, a.y, a.z, __int_as_float(i));
                 ++n;
             }
+        }
+        if ((n - first) & 1) {                                    // pad the run to an even length: an entry that can never be the minimum
+            if (fill) dst[n] = make_float4(1e18f, 1e18f, 1e18f, __int_as_float(i));
+            ++n;
         }
         if (fill && n > first) dst[first].w = __int_as_float(i | ((n - first) << 16));
     }
