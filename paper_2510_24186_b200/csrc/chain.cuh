@@ -394,7 +394,7 @@ __device__ __forceinline__ void eval_pose(const Lig<J>& L, const DGrid& G, const
         fx[j] = fy[j] = fz[j] = 0.f;
         if (L.valid[j]) {
             if (RD.atoms) e_inter += rec_direct<GRAD>(RD, P, L.typ[j], x[j], y[j], z[j], fx[j], fy[j], fz[j]);
-            else e_inter += grid_interp<GRAD>(G, P.k_wall, L.typ[j], x[j], y[j], z[j], fx[j], fy[j], fz[j]);
+            else e_inter += grid_interp_packed<GRAD>(G, P.k_wall, L.typ[j], x[j], y[j], z[j], fx[j], fy[j], fz[j]);
         }
         if (M.n_res > 0 && L.valid[j]) mdn_atom(M, mdn_par, L.n, j * L.S + lane, x[j], y[j], z[j], 0, 1, GRAD, e_inter, fx[j], fy[j], fz[j]);
     }
