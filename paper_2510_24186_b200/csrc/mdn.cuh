@@ -22,7 +22,7 @@ __device__ __forceinline__ void mdn_ldg2(const float4* p, float4& a, float4& b) 
 // One (residue, atom) pair whose minimum squared distance best2 is inside the cut-off: the K mixture components.  The
 // records are padded to a multiple of four per pair (M.K4; the padding has zero amplitude) and fetched four at a time by two
 // 256-bit loads; the first four (c0) were requested by the caller before it searched the residue's atoms.
-__device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __restrict__ q, const float4 c0[4], float best2,
+__device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __restrict__ q, const float4 c0[8], float best2,
                                            float bx, float by, float bz, bool grad, float& e, float& gx, float& gy, float& gz) {
     float rinv;
     { const float b = fmaxf(best2, 1e-12f); asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(b)); }
@@ -32,7 +32,10 @@ __device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __rest
     for (int k0 = 0; k0 < M.K4; k0 += 4) {
         float4 cn[4];
         const bool more = k0 + 4 < M.K4;
-        if (more) { mdn_ldg2(q + k0 + 4, cn[0], cn[1]); mdn_ldg2(q + k0 + 6, cn[2], cn[3]); }
+        if (more) {
+            if (k0 == 0) { cn[0] = c0[4]; cn[1] = c0[5]; cn[2] = c0[6]; cn[3] = c0[7]; }      // the second four came with the first
+            else { mdn_ldg2(q + k0 + 4, cn[0], cn[1]); mdn_ldg2(q + k0 + 6, cn[2], cn[3]); }
+        }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const float t = d - c[j].y;
@@ -74,8 +77,9 @@ __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restri
     for (int en = e0; en < e1; ++ord) {
         const int hdr = __float_as_int(a.w), i = hdr & 0xffff, cnt = hdr >> 16;      // cnt is even
         const float4* q = par + ((size_t)i * n + p) * M.K4;
-        float4 c0[4];
+        float4 c0[8];                                         // K4 >= 8 ? eight records : four (the rest of c0 is unused then)
         mdn_ldg2(q, c0[0], c0[1]); mdn_ldg2(q + 2, c0[2], c0[3]);
+        if (M.K4 > 4) { mdn_ldg2(q + 4, c0[4], c0[5]); mdn_ldg2(q + 6, c0[6], c0[7]); }
         float4 an, an2;
         mdn_ldg2(M.cell_at + min(en + cnt, e1 - 2), an, an2);
         float bx = x - a.x, by = y - a.y, bz = z - a.z;
