@@ -504,13 +504,16 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
         depth[k + 1] = depth[tp[k] + 1] + 1;
     }
     // depth-first preorder over fragments (children in torsion order)
-    std::vector<std::vector<int>> kids(T + 1);
-    for (int f = 1; f <= T; ++f) kids[parent[f]].push_back(f);
-    std::vector<int> order, stack{0};
-    while (!stack.empty()) {
-        int f = stack.back(); stack.pop_back();
-        order.push_back(f);
-        for (int c = (int)kids[f].size() - 1; c >= 0; --c) stack.push_back(kids[f][c]);
+    std::vector<int> order;
+    order.reserve(T + 1);
+    {
+        int stack[TRIDSK_MAX_TORSIONS + 2], sp = 0;
+        stack[sp++] = 0;
+        while (sp > 0) {
+            const int f = stack[--sp];
+            order.push_back(f);
+            for (int c = T; c >= 1; --c) if (parent[c] == f) stack[sp++] = c;       // children pushed last-first: popped in torsion order
+        }
     }
     std::vector<int> count(T + 1, 0), sub(T + 1, 0), lo(T + 1, 0);
     for (int a = 0; a < n; ++a) count[frag[a]]++;
@@ -529,6 +532,7 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
     h.n = n; h.T = T; h.J = J; h.S = S;
     h.max_depth = *std::max_element(depth.begin(), depth.end());
     out.f4.resize(n); out.ai.resize(n);
+    out.lane_recs.reserve(n * 4); out.lane_stream.reserve(4 * (T + 1) + n); out.rounds.reserve(2 * n);
     for (int p = 0; p < n; ++p) {
         const int a = oldidx[p];
         out.f4[p] = make_float4(ref[3 * a], ref[3 * a + 1], ref[3 * a + 2], types->radius[type[a]]);
@@ -568,22 +572,38 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
     } else {
         if (!b->bond_off || !b->bond_ab) return bad(TRIDSK_EINVAL, "neither pairs nor bonds given");
         const int b0 = b->bond_off[i], nb = b->bond_off[i + 1] - b0;
-        std::vector<std::vector<int>> adj(n);
+        // bond graph in CSR form on the stack (n <= 128): no allocation per atom
+        int deg[TRIDSK_MAX_ATOMS + 1] = {0};
         for (int k = 0; k < nb; ++k) {
             const int a = b->bond_ab[2 * (size_t)(b0 + k)], c = b->bond_ab[2 * (size_t)(b0 + k) + 1];
             if (a >= n || c >= n || a == c) return bad(TRIDSK_EINVAL, "bond index out of range");
-            adj[a].push_back(c); adj[c].push_back(a);
+            ++deg[a + 1]; ++deg[c + 1];
+        }
+        for (int a = 0; a < n; ++a) deg[a + 1] += deg[a];
+        std::vector<unsigned char> nbr(2 * (size_t)std::max(nb, 1));
+        {
+            int fillp[TRIDSK_MAX_ATOMS];
+            for (int a = 0; a < n; ++a) fillp[a] = deg[a];
+            for (int k = 0; k < nb; ++k) {
+                const int a = b->bond_ab[2 * (size_t)(b0 + k)], c = b->bond_ab[2 * (size_t)(b0 + k) + 1];
+                nbr[fillp[a]++] = (unsigned char)c; nbr[fillp[c]++] = (unsigned char)a;
+            }
         }
         // O6: pairs = {a<b : bond-graph distance >= 4 and different rigid fragment}
-        std::vector<int> dist(n);
+        int dist[TRIDSK_MAX_ATOMS], cur[TRIDSK_MAX_ATOMS], nxt[TRIDSK_MAX_ATOMS];
         for (int a = 0; a < n; ++a) {
-            std::fill(dist.begin(), dist.end(), 1 << 20);
+            for (int c = 0; c < n; ++c) dist[c] = 1 << 20;
             dist[a] = 0;
-            std::vector<int> cur{a};
-            for (int d = 1; d <= 3 && !cur.empty(); ++d) {
-                std::vector<int> nxt;
-                for (int u : cur) for (int v : adj[u]) if (dist[v] > d) { dist[v] = d; nxt.push_back(v); }
-                cur.swap(nxt);
+            int nc = 1;
+            cur[0] = a;
+            for (int d = 1; d <= 3 && nc > 0; ++d) {
+                int nn = 0;
+                for (int q = 0; q < nc; ++q) {
+                    const int u = cur[q];
+                    for (int e = deg[u]; e < deg[u + 1]; ++e) { const int v = nbr[e]; if (dist[v] > d) { dist[v] = d; nxt[nn++] = v; } }
+                }
+                for (int q = 0; q < nn; ++q) cur[q] = nxt[q];
+                nc = nn;
             }
             for (int c = a + 1; c < n; ++c)
                 if (dist[c] > 3 && frag[a] != frag[c]) {
