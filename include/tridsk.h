@@ -282,7 +282,7 @@ int tridsk_debug_philox(tridsk_ctx* ctx, const unsigned int ctr[4], const unsign
  * operations (TRIDSK_MB_MUFU: ex2.approx chains), bytes read (TRIDSK_MB_L2_READ: coalesced 16-byte loads over a buffer of
  * `bytes`, `iters` passes; below the L2 size the buffer is L2-resident after the first pass), bytes of 32-byte sectors
  * touched (TRIDSK_MB_GATHER: per lane one 16-byte load from a pseudo-random sector of a buffer of `bytes`, the access a
- * trilinear lookup in the xy-packed grid makes twice per atom).  Not on the docking path.
+ * trilinear lookup in the cell-packed grid makes once per atom).  Not on the docking path.
  */
 #define TRIDSK_MB_FFMA    0
 #define TRIDSK_MB_FFMA2   1

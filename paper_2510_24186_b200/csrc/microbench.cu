@@ -8,7 +8,7 @@
 //   TRIDSK_MB_L2_READ coalesced 16-byte reads of a buffer, repeated  -> streaming read rate    work = bytes
 //                     (a buffer below the L2 size is L2-resident after the first pass)
 //   TRIDSK_MB_GATHER  one 16-byte load per lane from a pseudo-random 32-byte sector of the buffer (what a trilinear
-//                     lookup in the xy-packed grid does twice per atom)  -> sector gather rate  work = 32-byte sectors * 32
+//                     lookup in the cell-packed grid does once per atom)  -> sector gather rate  work = 32-byte sectors * 32
 #include "internal.h"
 
 __global__ void __launch_bounds__(256) mb_ffma_kernel(float* out, int iters) {
