@@ -208,7 +208,7 @@ static int new_grid(tridsk_ctx* ctx, int n_types, const float origin[3], const i
     g->d.ox = origin[0]; g->d.oy = origin[1]; g->d.oz = origin[2];
     g->d.h = spacing; g->d.inv_h = 1.0f / spacing;
     cudaError_t e = cudaMallocFromPoolAsync((void**)&g->g, sizeof(float) * g->d.plane * n_types, ctx->pool, ctx->stream);
-    if (e == cudaSuccess)                                                                  // xy-packed copy (DGrid::gp)
+    if (e == cudaSuccess)                                                                  // cell-packed copy (DGrid::gp)
         e = cudaMallocFromPoolAsync((void**)&g->gp, 2 * sizeof(float4) * g->d.plane * n_types, ctx->pool, ctx->stream);
     if (e != cudaSuccess) {
         if (g->g) cudaFreeAsync(g->g, ctx->stream);

@@ -231,7 +231,7 @@ cudaError_t launch_grid_build(cudaStream_t s, const float4* rec, int n_rec, cons
     return cudaGetLastError();
 }
 
-// ------------------------------------------------------------------ xy-packed copy of the grid (DGrid::gp)
+// ------------------------------------------------------------------ cell-packed copy of the grid (DGrid::gp)
 // gp[t][z][y][x] = {g(x,y), g(x+1,y), g(x,y+1), g(x+1,y+1)} at the same (t, z); indices clamped at the upper
 // edges (those records are never the base of a cell: i0 <= n - 2).  The 8 corners of a trilinear cell -- the xy
 // quad of plane z and the quad of plane z + 1 -- are then ONE aligned 32-byte record (one L2 sector; one 256-bit load on
