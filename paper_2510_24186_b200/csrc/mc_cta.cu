@@ -23,11 +23,13 @@ struct CtaTopo {
     const int* rows;        // [n + 1] row offsets into recs
     const uint2* recs;      // [2P] row records {b | hb << 8, c}, then [P] flat records {a | b << 8 | hb << 16, c}; c = dvdw + mu
     const uint2* flat;      // the flat records
-    const float* rtab;      // n > 64: round table [(n / 2)][n] of c = dvdw + mu (lowest mantissa bit: donor/acceptor), absent: -1e15
-    float* slots;           // n > 64: force slots [2][TRIDSK_CTA_RB][n][3]
+    const float* ctab;      // n > 64: [npad][npad] c = dvdw + mu of the pair (row b, column l), -1e15: not in the pair set
+    const unsigned* hbm;    // n > 64: [2][npad / 32][npad] lanes l of chunk that form a donor-acceptor pair with b; [1]: those with l < b
+    float4* part;           // n > 64: per-warp partial forces [warps][npad]
+    float4* X4;             // n > 64: {x, y, z, 0} [npad], entries beyond n stay zero
     float *X, *AF, *PF, *red;  // X[3][n], AF[n][8] = {force, 0, moment about t, 0}, PF = its prefix sums, red[64]
-    int n, T, P, lpa;
-    bool rounds;            // n > 64: every pair once per gradient pass, on the round schedule (internal.h)
+    int n, T, P, lpa, npad;
+    bool rounds;            // n > 64: dense partner sweep instead of pair records (internal.h)
 };
 
 // this lane's fragment (lane g = fragment g in pre-order; lanes beyond T are idle copies of the root)
@@ -60,27 +62,41 @@ __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char*
     }
     for (int i = tid; i <= n; i += nt) rows[i] = __ldg(cta_rows + h->cta_row_off + i);
     const bool rounds = n > TRIDSK_CTA_ROUNDS_N;
+    S.ctab = nullptr; S.hbm = nullptr; S.part = nullptr; S.X4 = nullptr; S.npad = 0;
     if (!rounds) {
         for (int i = tid; i < 3 * np; i += nt) {
             const uint2 r = __ldg(cta_recs + h->cta_rec_off + i);
             recs[i] = make_uint2(r.x, __float_as_uint(__uint_as_float(r.y) + P.long_mu));
         }
-    } else {                                                  // flat records only, + the round table
-        for (int i = tid; i < np; i += nt) {
-            const uint2 r = __ldg(cta_recs + h->cta_rec_off + 2 * np + i);
-            recs[i] = make_uint2(r.x, __float_as_uint(__uint_as_float(r.y) + P.long_mu));
-        }
-        float* rt = reinterpret_cast<float*>(smem + L.rtab);
+    } else {                                                  // no records: the dense table and the masks from the round table
+        const int npad = (n + 31) / 32 * 32, nch = npad / 32;
+        float* ct = reinterpret_cast<float*>(smem + L.ctab);
+        unsigned* mk = reinterpret_cast<unsigned*>(smem + L.masks);
+        float4* x4 = reinterpret_cast<float4*>(smem + L.X);
+        for (int i = tid; i < npad * npad; i += nt) ct[i] = -1e15f;
+        for (int i = tid; i < 2 * npad * nch; i += nt) mk[i] = 0u;
+        for (int i = tid; i < npad; i += nt) x4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        __syncthreads();
         for (int i = tid; i < (n / 2) * n; i += nt) {
             const float d = __ldg(cta_rtab + h->cta_rt_off + i);
-            const unsigned hbbit = __float_as_uint(d) & 1u;
-            rt[i] = d >= 0.f ? __uint_as_float((__float_as_uint(d + P.long_mu) & ~1u) | hbbit) : -1e15f;
+            if (d < 0.f) continue;
+            const int k = i / n + 1, l = i - (k - 1) * n, b = (l + k) % n;
+            const float c = (ref[l].w + ref[b].w) + P.long_mu;
+            ct[b * npad + l] = c; ct[l * npad + b] = c;
+            if (__float_as_uint(d) & 1u) {
+                atomicOr(&mk[(l >> 5) * npad + b], 1u << (l & 31));
+                atomicOr(&mk[(b >> 5) * npad + l], 1u << (b & 31));
+                const int lo = min(l, b), hi = max(l, b);     // the energy-only sweep meets the pair as (lane lo, partner hi)
+                atomicOr(&mk[(nch + (lo >> 5)) * npad + hi], 1u << (lo & 31));
+            }
         }
-        S.rtab = rt;
-        S.slots = reinterpret_cast<float*>(smem + L.slots);
+        S.ctab = ct; S.hbm = mk;
+        S.part = reinterpret_cast<float4*>(smem + L.part);
+        S.X4 = x4;
+        S.npad = npad;
     }
     S.rounds = rounds;
-    S.flat = rounds ? recs : recs + 2 * np;
+    S.flat = recs + 2 * np;
     S.ref = ref; S.meta = meta; S.frag = reinterpret_cast<const LaneFrag*>(frag); S.rows = rows; S.recs = recs;
     S.X = reinterpret_cast<float*>(smem + L.X); S.AF = reinterpret_cast<float*>(smem + L.AF);
     S.PF = reinterpret_cast<float*>(smem + L.PF);
@@ -182,13 +198,72 @@ __device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], co
     }
 }
 
+// Dense partner sweep (internal.h): this lane's atom `me` against four partners, branch-free in the main part (the arithmetic
+// of lane_rec in mc_lane.cu: one lg2 for the product of the four clash ratios, the clash force switched by one compare pair);
+// hw.{x,y,z,w} = the lanes that form a donor/acceptor pair with partner 0..3 -- a partner without any skips that term for the
+// whole warp.  A visit that is not in the pair set has c = -1e15 and adds exactly zero.
+template <bool GRAD, bool ENERGY>
+__device__ __forceinline__ void cta_dense4(const PairK& K, const float4 me, const float4 pb[4], const float c[4], const uint4 hw,
+                                           unsigned lbit, float& eL, float& eC, float& eH, float& ax, float& ay, float& az) {
+    const unsigned hbw[4] = {hw.x, hw.y, hw.z, hw.w};
+    float dx[4], dy[4], dz[4], d[4], rinv[4], s[4], q[4], t[4], dc[4];
+    if (ENERGY) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            dc[u] = c[u] - K.mu;                                      // clash distance dvdw (negative: no pair)
+            if (hbw[u] != 0u) dc[u] = (hbw[u] & lbit) ? K.hb_dclash : dc[u];
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        dx[u] = me.x - pb[u].x; dy[u] = me.y - pb[u].y; dz[u] = me.z - pb[u].z;
+        const float d2 = fmaf(dx[u], dx[u], fmaf(dy[u], dy[u], fmaf(dz[u], dz[u], 1e-12f)));
+        rinv[u] = rsqrt_approx(d2);
+        d[u] = d2 * rinv[u];
+        t[u] = d[u] - c[u];
+        const float w = t[u] * K.nk2;
+        float g = ex2_approx(w * t[u]);
+        g = d[u] < K.dmax ? g : 0.f;
+        if (ENERGY) {
+            eL += g;
+            q[u] = fmaxf(dc[u] * fminf(rinv[u], K.inv_floor), 1.f);
+        }
+        if (GRAD) {
+            const float in = (t[u] < K.neg_mu && rinv[u] < K.inv_floor) ? 1.f : 0.f;
+            s[u] = rinv[u] * fmaf(in, K.nkc * rinv[u], w * g);
+        }
+    }
+    if (ENERGY) eC += lg2_approx((q[0] * q[1]) * (q[2] * q[3]));
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        if (hbw[u] != 0u) {                                          // warp-uniform
+            if (hbw[u] & lbit) {
+                const float th = d[u] - K.hb_mu;
+                float gh = ex2_approx(K.hb_nk2 * th * th);
+                gh = d[u] < K.hb_dmax ? gh : 0.f;
+                if (ENERGY) eH += gh;
+                if (GRAD) {
+                    s[u] = fmaf(K.kh * th, gh * rinv[u], s[u]);
+                    // the clash range of a donor/acceptor pair ends at hb_dclash, not at dvdw: put the term right
+                    const bool plain = t[u] < K.neg_mu, hb = d[u] < K.hb_dclash;
+                    if (plain != hb && rinv[u] < K.inv_floor) s[u] = fmaf(hb ? K.nkc : -K.nkc, rinv[u] * rinv[u], s[u]);
+                }
+            }
+        }
+    }
+    if (GRAD) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { ax = fmaf(s[u], dx[u], ax); ay = fmaf(s[u], dy[u], ay); az = fmaf(s[u], dz[u], az); }
+    }
+}
+
 // ------------------------------------------------------------------ a3..a6: one pose evaluation by the whole CTA
 // In : t[3], unit q[4] (uniform), theta (lane g holds the torsion angle of fragment g).
 // Out: ENERGY: e_inter, e_intra (uniform over the CTA); GRAD: g6 = {dE/dt, dE/domega about t} (uniform), gth = dE/dtheta
 //      on lane g (O9); x, y, z = this thread's atom (valid when `active`).
 // MDN: the mixture-density term (mdn.cuh); the lanes of an atom share its residues (lane `part` takes residues part,
 // part + lpa, ...), their shares join the pair force / the energy sums before the fixed-order reductions.
-// ROUNDS: 0 = row form (ligands of up to 64 atoms), 1 = round schedule (above), 2 = decided at run time (S.rounds).
+// ROUNDS: 0 = pair records (ligands of up to 64 atoms), 1 = dense partner sweep (above), 2 = decided at run time (S.rounds).
 template <bool GRAD, bool ENERGY, bool MDN, int ROUNDS>
 __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
                                          const MdnDev& M, const float4* __restrict__ mdn_par,
@@ -197,35 +272,48 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
                                          float& e_inter, float& e_intra, float g6[6], float& gth) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = S.n;
 
-    // ---- a3 forward kinematics (O8): world frame (R, p) of this lane's fragment, F_g = F_parent o L_g
+    // ---- a3 forward kinematics (O8): world frame (R, p) of this lane's fragment, F_g = F_parent o L_g, by pointer jumping:
+    // every lane starts from its own local transform L_g (the root from the rigid transform) and folds in the accumulated
+    // transform of its current ancestor, whose own ancestor it then adopts -- ceil(log2(depth + 1)) rounds instead of `depth`.
     float R[9], p[3];
     quat_matrix(q, R);
     p[0] = t[0]; p[1] = t[1]; p[2] = t[2];
     if (max_depth > 0) {
-        float sn, cs;
-        __sincosf(theta, &sn, &cs);
-        const float oc = 1.f - cs;
-        float Lm[9];
-        Lm[0] = fmaf(oc * F.ux, F.ux, cs);          Lm[1] = fmaf(oc * F.ux, F.uy, -sn * F.uz);  Lm[2] = fmaf(oc * F.ux, F.uz, sn * F.uy);
-        Lm[3] = fmaf(oc * F.uy, F.ux, sn * F.uz);   Lm[4] = fmaf(oc * F.uy, F.uy, cs);          Lm[5] = fmaf(oc * F.uy, F.uz, -sn * F.ux);
-        Lm[6] = fmaf(oc * F.uz, F.ux, -sn * F.uy);  Lm[7] = fmaf(oc * F.uz, F.uy, sn * F.ux);   Lm[8] = fmaf(oc * F.uz, F.uz, cs);
-        const float c0 = F.ox - (Lm[0] * F.ox + Lm[1] * F.oy + Lm[2] * F.oz);
-        const float c1 = F.oy - (Lm[3] * F.ox + Lm[4] * F.oy + Lm[5] * F.oz);
-        const float c2 = F.oz - (Lm[6] * F.ox + Lm[7] * F.oy + Lm[8] * F.oz);
-        for (int d = 1; d <= max_depth; ++d) {
+        int anc = -1;
+        if (F.valid && lane >= 1) {
+            float sn, cs;
+            __sincosf(theta, &sn, &cs);
+            const float oc = 1.f - cs;
+            R[0] = fmaf(oc * F.ux, F.ux, cs);          R[1] = fmaf(oc * F.ux, F.uy, -sn * F.uz);  R[2] = fmaf(oc * F.ux, F.uz, sn * F.uy);
+            R[3] = fmaf(oc * F.uy, F.ux, sn * F.uz);   R[4] = fmaf(oc * F.uy, F.uy, cs);          R[5] = fmaf(oc * F.uy, F.uz, -sn * F.ux);
+            R[6] = fmaf(oc * F.uz, F.ux, -sn * F.uy);  R[7] = fmaf(oc * F.uz, F.uy, sn * F.ux);   R[8] = fmaf(oc * F.uz, F.uz, cs);
+            p[0] = F.ox - (R[0] * F.ox + R[1] * F.oy + R[2] * F.oz);
+            p[1] = F.oy - (R[3] * F.ox + R[4] * F.oy + R[5] * F.oz);
+            p[2] = F.oz - (R[6] * F.ox + R[7] * F.oy + R[8] * F.oz);
+            anc = F.parent;
+        }
+        for (int span = 1; span <= max_depth; span <<= 1) {          // after the round, `2 * span` transforms are folded
+            const int src = anc < 0 ? lane : anc;
             float PR[9], pp[3];
 #pragma unroll
-            for (int i = 0; i < 9; ++i) PR[i] = __shfl_sync(FULL_MASK, R[i], F.parent);
+            for (int i = 0; i < 9; ++i) PR[i] = __shfl_sync(FULL_MASK, R[i], src);
 #pragma unroll
-            for (int i = 0; i < 3; ++i) pp[i] = __shfl_sync(FULL_MASK, p[i], F.parent);
-            if (F.depth == d) {
+            for (int i = 0; i < 3; ++i) pp[i] = __shfl_sync(FULL_MASK, p[i], src);
+            const int na = __shfl_sync(FULL_MASK, anc, src);
+            if (anc >= 0) {
+                float N[9], np3[3];
 #pragma unroll
                 for (int r = 0; r < 3; ++r) {
-                    R[3 * r + 0] = PR[3 * r] * Lm[0] + PR[3 * r + 1] * Lm[3] + PR[3 * r + 2] * Lm[6];
-                    R[3 * r + 1] = PR[3 * r] * Lm[1] + PR[3 * r + 1] * Lm[4] + PR[3 * r + 2] * Lm[7];
-                    R[3 * r + 2] = PR[3 * r] * Lm[2] + PR[3 * r + 1] * Lm[5] + PR[3 * r + 2] * Lm[8];
-                    p[r] = PR[3 * r] * c0 + PR[3 * r + 1] * c1 + PR[3 * r + 2] * c2 + pp[r];
+                    N[3 * r + 0] = PR[3 * r] * R[0] + PR[3 * r + 1] * R[3] + PR[3 * r + 2] * R[6];
+                    N[3 * r + 1] = PR[3 * r] * R[1] + PR[3 * r + 1] * R[4] + PR[3 * r + 2] * R[7];
+                    N[3 * r + 2] = PR[3 * r] * R[2] + PR[3 * r + 1] * R[5] + PR[3 * r + 2] * R[8];
+                    np3[r] = PR[3 * r] * p[0] + PR[3 * r + 1] * p[1] + PR[3 * r + 2] * p[2] + pp[r];
                 }
+#pragma unroll
+                for (int i = 0; i < 9; ++i) R[i] = N[i];
+#pragma unroll
+                for (int i = 0; i < 3; ++i) p[i] = np3[i];
+                anc = na;
             }
         }
     }
@@ -246,8 +334,11 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     const bool lead = active && part == 0;
     GridCell cell;
     float4 glo = make_float4(0.f, 0.f, 0.f, 0.f), ghi = glo;
+    constexpr bool kMaybeDense = ROUNDS != 0;
+    const bool dense = ROUNDS == 1 || (ROUNDS == 2 && S.rounds);
     if (lead) {
-        S.X[atom] = x; S.X[n + atom] = y; S.X[2 * n + atom] = z;
+        if (kMaybeDense && dense) S.X4[atom] = make_float4(x, y, z, 0.f);
+        else { S.X[atom] = x; S.X[n + atom] = y; S.X[2 * n + atom] = z; }
         cell = grid_locate(G, m & 0xff, x, y, z);
         glo = __ldg(cell.p); ghi = __ldg(cell.p + 1);
     }
@@ -255,53 +346,40 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
 
     // ---- a5 intra-ligand pairs (O6)
     float eL = 0.f, eC = 0.f, eH = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
-    if (GRAD && (ROUNDS == 1 || (ROUNDS == 2 && S.rounds))) {
-        // Every pair once: rounds k = 1 .. n/2, item l of round k = pair (l, (l + k) mod n), TRIDSK_CTA_RB rounds per block spread
-        // over ALL threads of the CTA, four items in flight per thread.  The force of an item goes to slot A[round][l] and its
-        // reaction to slot B[round][(l + k) mod n]; no two items of a block share a slot, a barrier, then every atom's thread adds
-        // its slots in round order.
-        const int nr = n >> 1, nt = (int)blockDim.x;
-        const unsigned magic = ((1u << 20) + (unsigned)n - 1u) / (unsigned)n;      // floor(i / n) = (i * magic) >> 20 for i < 1024
-        float* SA = S.slots;
-        float* SB = S.slots + 3 * TRIDSK_CTA_RB * n;
-        for (int k0 = 1; k0 <= nr; k0 += TRIDSK_CTA_RB) {
-            const int nb = min(TRIDSK_CTA_RB, nr - k0 + 1), items = nb * n;
-            for (int it = tid; it < items; it += 4 * nt) {
-                float dx[4], dy[4], dz[4], c[4], sv[4];
-                bool hb[4], ok[4];
-                int sa[4], sb[4];
+    if (kMaybeDense && dense) {
+        // Dense partner sweep (internal.h): this warp's lanes hold the atoms l = c0 + lane of one 32-atom chunk after another and
+        // meet the partners b = b0 + 4 * warp + u, u = 0..3 (warp-uniform: one broadcast 16-byte load each); the other warps
+        // take the other partners, so a chunk's force is the sum of the warps' partials -- fixed order, after a barrier.
+        // GRAD: all partners (both ends of every pair); energy only: the partners b > l.
+        const int nw = (int)(blockDim.x >> 5), npad = S.npad, nch = npad >> 5;
+        const unsigned lbit = 1u << lane;
+        float4* part = S.part + warp * npad;
+        for (int c0 = 0; c0 < npad; c0 += 32) {
+            const int l = c0 + lane;
+            const float4 me = S.X4[l];
+            const float* crow = S.ctab + l;
+            const unsigned* hrow = S.hbm + ((GRAD ? 0 : nch) + (c0 >> 5)) * npad;
+            float ax = 0.f, ay = 0.f, az = 0.f;
+            for (int b0 = (GRAD ? 0 : c0) + 4 * warp; b0 < n; b0 += 4 * nw) {
+                const uint4 hw = *reinterpret_cast<const uint4*>(hrow + b0);
+                float4 pb[4];
+                float c[4];
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
-                    const int iu = it + u * nt;
-                    ok[u] = iu < items;
-                    const int ii = ok[u] ? iu : it;
-                    const int kk = (int)(((unsigned)ii * magic) >> 20), l = ii - kk * n;
-                    int b = l + k0 + kk;
-                    b = b >= n ? b - n : b;
-                    const float cv = S.rtab[(k0 - 1 + kk) * n + l];
-                    c[u] = cv; hb[u] = (__float_as_uint(cv) & 1u) != 0u && cv > 0.f;
-                    dx[u] = S.X[l] - S.X[b]; dy[u] = S.X[n + l] - S.X[n + b]; dz[u] = S.X[2 * n + l] - S.X[2 * n + b];
-                    sa[u] = 3 * (kk * n + l); sb[u] = 3 * (kk * n + b);
+                    pb[u] = S.X4[b0 + u];
+                    c[u] = crow[(b0 + u) * npad];
+                    if (!GRAD) c[u] = l < b0 + u ? c[u] : -1e15f;
                 }
-                cta_pairs4s<true, ENERGY>(K, dx, dy, dz, c, hb, ok, eL, eC, eH, sv);
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    if (ok[u]) {
-                        const float px = sv[u] * dx[u], py = sv[u] * dy[u], pz = sv[u] * dz[u];
-                        SA[sa[u]] = px; SA[sa[u] + 1] = py; SA[sa[u] + 2] = pz;
-                        SB[sb[u]] = -px; SB[sb[u] + 1] = -py; SB[sb[u] + 2] = -pz;
-                    }
-                }
+                cta_dense4<GRAD, ENERGY>(K, me, pb, c, hw, lbit, eL, eC, eH, ax, ay, az);
             }
+            if (GRAD) part[l] = make_float4(ax, ay, az, 0.f);
+        }
+        if (GRAD) {
+            eL *= 0.5f; eC *= 0.5f; eH *= 0.5f;                     // every pair was visited from both ends
             __syncthreads();
             if (active) {
-                for (int kk = 0; kk < nb; ++kk) {
-                    const float* pa = SA + 3 * (kk * n + atom);
-                    const float* pb = SB + 3 * (kk * n + atom);
-                    fx += pa[0] + pb[0]; fy += pa[1] + pb[1]; fz += pa[2] + pb[2];
-                }
+                for (int w = 0; w < nw; ++w) { const float4 f = S.part[w * npad + atom]; fx += f.x; fy += f.y; fz += f.z; }
             }
-            __syncthreads();
         }
     } else if (GRAD) {
         if (active) {
@@ -447,7 +525,10 @@ __device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const Ct
 
 // ------------------------------------------------------------------ the fused MC kernel, one CTA per chain
 template <bool MDN, int ROUNDS>
-__global__ void __launch_bounds__(128, 3) mc_cta_kernel(const McLaunch a) {
+#ifndef CTA_MINB
+#define CTA_MINB 3
+#endif
+__global__ void __launch_bounds__(128, CTA_MINB) mc_cta_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lig = a.lig_list[blockIdx.x / a.n_chains];
