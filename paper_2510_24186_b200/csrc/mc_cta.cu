@@ -23,7 +23,7 @@ struct CtaTopo {
     const int* rows;        // [n + 1] row offsets into recs
     const uint2* recs;      // [2P] row records {b | hb << 8, c}, then [P] flat records {a | b << 8 | hb << 16, c}; c = dvdw + mu
     const uint2* flat;      // the flat records
-    const float* ctab;      // n > 64: [npad][npad] c = dvdw + mu of the pair (row b, column l), -1e15: not in the pair set
+    const float* ctab;      // n > 64: [n rounded up to 16][npad] c = dvdw + mu of the pair (row b, column l), -1e15: not in the pair set
     const unsigned* hbm;    // n > 64: [2][npad / 32][npad] lanes l of chunk that form a donor-acceptor pair with b; [1]: those with l < b
     float4* part;           // n > 64: per-warp partial forces [warps][npad]
     float4* X4;             // n > 64: {x, y, z, 0} [npad], entries beyond n stay zero
@@ -73,7 +73,8 @@ __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char*
         float* ct = reinterpret_cast<float*>(smem + L.ctab);
         unsigned* mk = reinterpret_cast<unsigned*>(smem + L.masks);
         float4* x4 = reinterpret_cast<float4*>(smem + L.X);
-        for (int i = tid; i < npad * npad; i += nt) ct[i] = -1e15f;
+        const int nrow = (n + 4 * TRIDSK_CTA_WARPS - 1) / (4 * TRIDSK_CTA_WARPS) * (4 * TRIDSK_CTA_WARPS);
+        for (int i = tid; i < nrow * npad; i += nt) ct[i] = -1e15f;
         for (int i = tid; i < 2 * npad * nch; i += nt) mk[i] = 0u;
         for (int i = tid; i < npad; i += nt) x4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         __syncthreads();
@@ -351,7 +352,8 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
         // meet the partners b = b0 + 4 * warp + u, u = 0..3 (warp-uniform: one broadcast 16-byte load each); the other warps
         // take the other partners, so a chunk's force is the sum of the warps' partials -- fixed order, after a barrier.
         // GRAD: all partners (both ends of every pair); energy only: the partners b > l.
-        const int nw = (int)(blockDim.x >> 5), npad = S.npad, nch = npad >> 5;
+        constexpr int nw = TRIDSK_CTA_WARPS;
+        const int npad = S.npad, nch = npad >> 5;
         const unsigned lbit = 1u << lane;
         float4* part = S.part + warp * npad;
         for (int c0 = 0; c0 < npad; c0 += 32) {
@@ -524,11 +526,10 @@ __device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const Ct
 }
 
 // ------------------------------------------------------------------ the fused MC kernel, one CTA per chain
+// resident CTAs per SM the register budget is set for: 4 for the dense-sweep instance (C4 72.8 -> 64.2 ms), 3 for the record
+// instance (with 4, C2 6.0 -> 6.3 ms) and with the mixture-density term (spills at 128 registers)
 template <bool MDN, int ROUNDS>
-#ifndef CTA_MINB
-#define CTA_MINB 3
-#endif
-__global__ void __launch_bounds__(128, CTA_MINB) mc_cta_kernel(const McLaunch a) {
+__global__ void __launch_bounds__(128, (ROUNDS && !MDN) ? 4 : 3) mc_cta_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lig = a.lig_list[blockIdx.x / a.n_chains];
@@ -670,7 +671,7 @@ __global__ void __launch_bounds__(128, CTA_MINB) mc_cta_kernel(const McLaunch a)
 
 // ------------------------------------------------------------------ tridsk_score_grad, CTA form: one CTA per pose
 template <bool MDN>
-__global__ void __launch_bounds__(256) score_cta_kernel(const ScoreLaunch a) {
+__global__ void __launch_bounds__(128) score_cta_kernel(const ScoreLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int i = blockIdx.x;
@@ -728,7 +729,7 @@ cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int rounds, size_t 
 
 cudaError_t launch_score_cta(cudaStream_t s, const ScoreLaunch& a, size_t smem_bytes) {
     if (a.n_pose <= 0) return cudaSuccess;
-    if (a.mdn.n_res > 0) score_cta_kernel<true><<<a.n_pose, 256, smem_bytes, s>>>(a);
-    else score_cta_kernel<false><<<a.n_pose, 256, smem_bytes, s>>>(a);
+    if (a.mdn.n_res > 0) score_cta_kernel<true><<<a.n_pose, 128, smem_bytes, s>>>(a);
+    else score_cta_kernel<false><<<a.n_pose, 128, smem_bytes, s>>>(a);
     return cudaGetLastError();
 }
