@@ -261,8 +261,7 @@ __host__ __device__ static inline CtaLayout cta_layout(int n, int T, int n_pairs
     L.frag = o; o += sizeof(LaneFrag) * (size_t)(T + 1);
     L.rows = o; o = TRIDSK_AL16(o + 4 * (size_t)(n + 1));
     L.recs = o; o = TRIDSK_AL16(o + (dense ? 0 : 8 * 3 * (size_t)n_pairs));
-    const size_t nrow = ((size_t)n + 4 * TRIDSK_CTA_WARPS - 1) / (4 * TRIDSK_CTA_WARPS) * (4 * TRIDSK_CTA_WARPS);   // partner rows the sweep touches
-    L.ctab = o; o = TRIDSK_AL16(o + (dense ? 4 * nrow * npad : 0));             // float [nrow][npad]
+    L.ctab = o; o = TRIDSK_AL16(o + (dense ? 4 * npad * npad : 0));             // float [npad][npad]
     L.masks = o; o = TRIDSK_AL16(o + (dense ? 2 * 4 * npad * (npad / 32) : 0));  // u32 [2][npad / 32][npad]: donor-acceptor lanes, all / l < b only
     L.part = o; o = TRIDSK_AL16(o + (dense ? 16 * npad * TRIDSK_CTA_WARPS : 0));   // per-warp partial forces, float4 [warps][npad]
     L.X = o; o = TRIDSK_AL16(o + (dense ? 16 * npad : 12 * (size_t)n));          // dense: float4 {x, y, z, 0} [npad], zero-padded

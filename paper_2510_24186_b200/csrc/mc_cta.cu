@@ -23,7 +23,7 @@ struct CtaTopo {
     const int* rows;        // [n + 1] row offsets into recs
     const uint2* recs;      // [2P] row records {b | hb << 8, c}, then [P] flat records {a | b << 8 | hb << 16, c}; c = dvdw + mu
     const uint2* flat;      // the flat records
-    const float* ctab;      // n > 64: [n rounded up to 16][npad] c = dvdw + mu of the pair (row b, column l), -1e15: not in the pair set
+    const float* ctab;      // n > 64: [npad][npad] c = dvdw + mu of the pair (row b, column l), -1e15: not in the pair set
     const unsigned* hbm;    // n > 64: [2][npad / 32][npad] lanes l of chunk that form a donor-acceptor pair with b; [1]: those with l < b
     float4* part;           // n > 64: per-warp partial forces [warps][npad]
     float4* X4;             // n > 64: {x, y, z, 0} [npad], entries beyond n stay zero
@@ -73,8 +73,7 @@ __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char*
         float* ct = reinterpret_cast<float*>(smem + L.ctab);
         unsigned* mk = reinterpret_cast<unsigned*>(smem + L.masks);
         float4* x4 = reinterpret_cast<float4*>(smem + L.X);
-        const int nrow = (n + 4 * TRIDSK_CTA_WARPS - 1) / (4 * TRIDSK_CTA_WARPS) * (4 * TRIDSK_CTA_WARPS);
-        for (int i = tid; i < nrow * npad; i += nt) ct[i] = -1e15f;
+        for (int i = tid; i < npad * npad; i += nt) ct[i] = -1e15f;
         for (int i = tid; i < 2 * npad * nch; i += nt) mk[i] = 0u;
         for (int i = tid; i < npad; i += nt) x4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         __syncthreads();
@@ -352,17 +351,20 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
         // meet the partners b = b0 + 4 * warp + u, u = 0..3 (warp-uniform: one broadcast 16-byte load each); the other warps
         // take the other partners, so a chunk's force is the sum of the warps' partials -- fixed order, after a barrier.
         // GRAD: all partners (both ends of every pair); energy only: the partners b > l.
+        // A last chunk of at most 16 atoms is held twice, by the two half-warps, which split the partners between them.
         constexpr int nw = TRIDSK_CTA_WARPS;
         const int npad = S.npad, nch = npad >> 5;
-        const unsigned lbit = 1u << lane;
         float4* part = S.part + warp * npad;
         for (int c0 = 0; c0 < npad; c0 += 32) {
-            const int l = c0 + lane;
+            const bool half = GRAD && n - c0 <= 16;
+            const int l = c0 + (half ? (lane & 15) : lane), bo = half ? (lane >> 4) << 2 : 0, per = half ? 8 : 4;
+            const unsigned lbit = 1u << (l & 31);
             const float4 me = S.X4[l];
             const float* crow = S.ctab + l;
             const unsigned* hrow = S.hbm + ((GRAD ? 0 : nch) + (c0 >> 5)) * npad;
             float ax = 0.f, ay = 0.f, az = 0.f;
-            for (int b0 = (GRAD ? 0 : c0) + 4 * warp; b0 < n; b0 += 4 * nw) {
+            for (int bb = (GRAD ? 0 : c0) + per * warp; bb < n; bb += per * nw) {
+                const int b0 = bb + bo;
                 const uint4 hw = *reinterpret_cast<const uint4*>(hrow + b0);
                 float4 pb[4];
                 float c[4];
@@ -374,7 +376,12 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
                 }
                 cta_dense4<GRAD, ENERGY>(K, me, pb, c, hw, lbit, eL, eC, eH, ax, ay, az);
             }
-            if (GRAD) part[l] = make_float4(ax, ay, az, 0.f);
+            if (GRAD) {
+                if (half) {
+                    ax += __shfl_xor_sync(FULL_MASK, ax, 16); ay += __shfl_xor_sync(FULL_MASK, ay, 16); az += __shfl_xor_sync(FULL_MASK, az, 16);
+                }
+                part[l] = make_float4(ax, ay, az, 0.f);
+            }
         }
         if (GRAD) {
             eL *= 0.5f; eC *= 0.5f; eH *= 0.5f;                     // every pair was visited from both ends
