@@ -124,16 +124,18 @@ struct LaneRec {
 // force is a sum its own threads own (no scatter, no atomics).  Flat form, for energy-only evaluations: every pair once,
 // {a | b << 8 | hb << 16, dvdw bits}, sorted by (a, b).  Fragments are the LaneFrag records (pre-order).
 
-// Ligands of more than 64 atoms (one lane per atom) use a DENSE PARTNER SWEEP instead of pair records: a warp takes 32
-// consecutive atoms l (one per lane) and sweeps the partner b over the ligand, four partners in flight; the partner's
-// coordinates are ONE broadcast 16-byte shared-memory load, c = dvdw + mu comes from a dense table ctab[b][l] in shared memory
-// (-1e15 where (l, b) is not in the pair set: such a visit adds exactly zero), and the donor/acceptor pairs from one 32-bit
-// lane mask per (b, 32-atom chunk), so that the hydrogen-bond term is skipped, warp-uniformly, for the partners that have none.
-// Gradient evaluations visit every pair from both ends (an atom's force is a sum its own lane owns: no scatter, no atomics,
-// bit-reproducible); energy-only evaluations visit the pairs l < b only.  Table and masks are built in shared memory from the
-// ROUND TABLE cta_rtab[(k - 1) * n + l], k = 1 .. n/2: the dvdw of pair (l, (l + k) mod n) as a float whose lowest mantissa
-// bit is the donor/acceptor flag, or -1 if the pair is not in the set (for even n the items l >= n/2 of round n/2 repeat
-// pairs and are absent).
+// Ligands of more than 64 atoms use a DENSE PARTNER SWEEP instead of pair records: a warp takes 32 consecutive atoms l (one
+// per lane) and sweeps the partner b over the ligand, four partners in flight; the partner's coordinates and atom type are ONE
+// broadcast 16-byte shared-memory load, c = dvdw + mu comes from a (type, type) table in shared memory (row stride 33: the
+// lanes' rows fall into different banks), and whether (l, b) is in the pair set / is a donor-acceptor pair from 32-bit lane
+// masks per (b, 32-atom chunk): a visit outside the pair set gets c = -1e15 and adds exactly zero, and the hydrogen-bond term
+// is skipped, warp-uniformly, for the partners that have no such pair.  Gradient evaluations visit every pair from both ends
+// (an atom's force is a sum its own lane owns: no scatter, no atomics, bit-reproducible); energy-only evaluations visit the
+// pairs l < b only (a second set of masks).  The masks are built in shared memory from the ROUND TABLE
+// cta_rtab[(k - 1) * n + l], k = 1 .. n/2: the dvdw of pair (l, (l + k) mod n) as a float whose lowest mantissa bit is the
+// donor/acceptor flag, or -1 if the pair is not in the set (for even n the items l >= n/2 of round n/2 repeat pairs and are
+// absent).  The MC kernel gives such a chain TWO warps (64-thread CTAs, two atoms per thread outside the sweep), so that eight
+// chains stay resident per SM.
 #define TRIDSK_CTA_ROUNDS_N 64         // ligands above this many atoms use the round schedule
 
 // Per-fragment record; fragment 0 is the root, fragment k+1 hangs off torsion k.
@@ -248,21 +250,21 @@ __host__ __device__ static inline int lane_chain_slots(int n, int T, int max_dep
 
 // CTA-per-chain kernel: shared-memory layout (byte offsets) -- topology {ref, meta, fragments, row offsets, records},
 // the chain's coordinates X[3][n], per-atom (force, moment about t) AF[6][n] and a reduction scratch
-struct CtaLayout { size_t ref, meta, frag, rows, recs, ctab, masks, part, X, AF, PF, red, total; };
+struct CtaLayout { size_t ref, meta, frag, rows, recs, tt, masks, part, X, AF, PF, red, total; };
 #define TRIDSK_AL16(x) (((x) + 15) / 16 * 16)
-#define TRIDSK_CTA_WARPS 4             // both CTA kernels run 128 threads (cta_shape)
+#define TRIDSK_CTA_WARPS 4             // the most warps a CTA kernel runs (score kernel, record instance: 128 threads)
 __host__ __device__ static inline CtaLayout cta_layout(int n, int T, int n_pairs) {
     CtaLayout L;
     size_t o = 0;
-    const bool dense = n > TRIDSK_CTA_ROUNDS_N;                    // dense partner sweep: no pair records, a dense table instead
+    const bool dense = n > TRIDSK_CTA_ROUNDS_N;                    // dense partner sweep: no pair records
     const size_t npad = ((size_t)n + 31) / 32 * 32;
     L.ref = o; o += 16 * (size_t)n;
     L.meta = o; o = TRIDSK_AL16(o + 4 * (size_t)n);
     L.frag = o; o += sizeof(LaneFrag) * (size_t)(T + 1);
     L.rows = o; o = TRIDSK_AL16(o + 4 * (size_t)(n + 1));
     L.recs = o; o = TRIDSK_AL16(o + (dense ? 0 : 8 * 3 * (size_t)n_pairs));
-    L.ctab = o; o = TRIDSK_AL16(o + (dense ? 4 * npad * npad : 0));             // float [npad][npad]
-    L.masks = o; o = TRIDSK_AL16(o + (dense ? 2 * 4 * npad * (npad / 32) : 0));  // u32 [2][npad / 32][npad]: donor-acceptor lanes, all / l < b only
+    L.tt = o; o = TRIDSK_AL16(o + (dense ? 4 * 32 * 33 : 0));                     // float [32][33]: c of a pair of atom types
+    L.masks = o; o = TRIDSK_AL16(o + (dense ? 4 * 4 * npad * (npad / 32) : 0));  // u32 [4][npad / 32][npad]: in the pair set, donor-acceptor; the same for l < b only
     L.part = o; o = TRIDSK_AL16(o + (dense ? 16 * npad * TRIDSK_CTA_WARPS : 0));   // per-warp partial forces, float4 [warps][npad]
     L.X = o; o = TRIDSK_AL16(o + (dense ? 16 * npad : 12 * (size_t)n));          // dense: float4 {x, y, z, 0} [npad], zero-padded
     L.AF = o; o = TRIDSK_AL16(o + 32 * (size_t)n);

@@ -23,10 +23,11 @@ struct CtaTopo {
     const int* rows;        // [n + 1] row offsets into recs
     const uint2* recs;      // [2P] row records {b | hb << 8, c}, then [P] flat records {a | b << 8 | hb << 16, c}; c = dvdw + mu
     const uint2* flat;      // the flat records
-    const float* ctab;      // n > 64: [npad][npad] c = dvdw + mu of the pair (row b, column l), -1e15: not in the pair set
-    const unsigned* hbm;    // n > 64: [2][npad / 32][npad] lanes l of chunk that form a donor-acceptor pair with b; [1]: those with l < b
+    const float* tt;        // n > 64: [32][33] c = dvdw + mu of a pair of atom types
+    const unsigned* msk;    // n > 64: [4][npad / 32][npad] lanes l of the chunk that are paired with b / form a donor-acceptor pair with b;
+                            //         [2], [3]: the same restricted to l < b
     float4* part;           // n > 64: per-warp partial forces [warps][npad]
-    float4* X4;             // n > 64: {x, y, z, 0} [npad], entries beyond n stay zero
+    float4* X4;             // n > 64: {x, y, z, atom type as int bits} [npad], entries beyond n stay zero
     float *X, *AF, *PF, *red;  // X[3][n], AF[n][8] = {force, 0, moment about t, 0}, PF = its prefix sums, red[64]
     int n, T, P, lpa, npad;
     bool rounds;            // n > 64: dense partner sweep instead of pair records (internal.h)
@@ -62,35 +63,42 @@ __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char*
     }
     for (int i = tid; i <= n; i += nt) rows[i] = __ldg(cta_rows + h->cta_row_off + i);
     const bool rounds = n > TRIDSK_CTA_ROUNDS_N;
-    S.ctab = nullptr; S.hbm = nullptr; S.part = nullptr; S.X4 = nullptr; S.npad = 0;
+    S.tt = nullptr; S.msk = nullptr; S.part = nullptr; S.X4 = nullptr; S.npad = 0;
     if (!rounds) {
         for (int i = tid; i < 3 * np; i += nt) {
             const uint2 r = __ldg(cta_recs + h->cta_rec_off + i);
             recs[i] = make_uint2(r.x, __float_as_uint(__uint_as_float(r.y) + P.long_mu));
         }
-    } else {                                                  // no records: the dense table and the masks from the round table
+    } else {                                                  // no records: the type-pair table, and the masks from the round table
         const int npad = (n + 31) / 32 * 32, nch = npad / 32;
-        float* ct = reinterpret_cast<float*>(smem + L.ctab);
+        float* tt = reinterpret_cast<float*>(smem + L.tt);
+        float* rad = reinterpret_cast<float*>(smem + L.red);  // scratch until the first evaluation: vdW radius by atom type
         unsigned* mk = reinterpret_cast<unsigned*>(smem + L.masks);
         float4* x4 = reinterpret_cast<float4*>(smem + L.X);
-        for (int i = tid; i < npad * npad; i += nt) ct[i] = -1e15f;
-        for (int i = tid; i < 2 * npad * nch; i += nt) mk[i] = 0u;
+        for (int i = tid; i < 4 * npad * nch; i += nt) mk[i] = 0u;
         for (int i = tid; i < npad; i += nt) x4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int i = tid; i < 32; i += nt) rad[i] = 0.f;
+        __syncthreads();                                      // ref, meta staged; scratch zeroed
+        for (int i = tid; i < n; i += nt) rad[meta[i] & 31] = ref[i].w;
         __syncthreads();
+        for (int i = tid; i < 32 * 32; i += nt) tt[(i >> 5) * 33 + (i & 31)] = (rad[i >> 5] + rad[i & 31]) + P.long_mu;
+        const int plane = nch * npad;
         for (int i = tid; i < (n / 2) * n; i += nt) {
             const float d = __ldg(cta_rtab + h->cta_rt_off + i);
             if (d < 0.f) continue;
             const int k = i / n + 1, l = i - (k - 1) * n, b = (l + k) % n;
-            const float c = (ref[l].w + ref[b].w) + P.long_mu;
-            ct[b * npad + l] = c; ct[l * npad + b] = c;
-            if (__float_as_uint(d) & 1u) {
-                atomicOr(&mk[(l >> 5) * npad + b], 1u << (l & 31));
-                atomicOr(&mk[(b >> 5) * npad + l], 1u << (b & 31));
-                const int lo = min(l, b), hi = max(l, b);     // the energy-only sweep meets the pair as (lane lo, partner hi)
-                atomicOr(&mk[(nch + (lo >> 5)) * npad + hi], 1u << (lo & 31));
+            const int lo = min(l, b), hi = max(l, b);         // the energy-only sweep meets the pair as (lane lo, partner hi)
+            const bool hbp = (__float_as_uint(d) & 1u) != 0u;
+            atomicOr(&mk[(l >> 5) * npad + b], 1u << (l & 31));
+            atomicOr(&mk[(b >> 5) * npad + l], 1u << (b & 31));
+            atomicOr(&mk[2 * plane + (lo >> 5) * npad + hi], 1u << (lo & 31));
+            if (hbp) {
+                atomicOr(&mk[plane + (l >> 5) * npad + b], 1u << (l & 31));
+                atomicOr(&mk[plane + (b >> 5) * npad + l], 1u << (b & 31));
+                atomicOr(&mk[3 * plane + (lo >> 5) * npad + hi], 1u << (lo & 31));
             }
         }
-        S.ctab = ct; S.hbm = mk;
+        S.tt = tt; S.msk = mk;
         S.part = reinterpret_cast<float4*>(smem + L.part);
         S.X4 = x4;
         S.npad = npad;
@@ -257,25 +265,14 @@ __device__ __forceinline__ void cta_dense4(const PairK& K, const float4 me, cons
     }
 }
 
-// ------------------------------------------------------------------ a3..a6: one pose evaluation by the whole CTA
-// In : t[3], unit q[4] (uniform), theta (lane g holds the torsion angle of fragment g).
-// Out: ENERGY: e_inter, e_intra (uniform over the CTA); GRAD: g6 = {dE/dt, dE/domega about t} (uniform), gth = dE/dtheta
-//      on lane g (O9); x, y, z = this thread's atom (valid when `active`).
-// MDN: the mixture-density term (mdn.cuh); the lanes of an atom share its residues (lane `part` takes residues part,
-// part + lpa, ...), their shares join the pair force / the energy sums before the fixed-order reductions.
-// ROUNDS: 0 = pair records (ligands of up to 64 atoms), 1 = dense partner sweep (above), 2 = decided at run time (S.rounds).
-template <bool GRAD, bool ENERGY, bool MDN, int ROUNDS>
-__device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
-                                         const MdnDev& M, const float4* __restrict__ mdn_par,
-                                         int max_depth, const float t[3], const float q[4], float theta,
-                                         int atom, int part, bool active, float& x, float& y, float& z,
-                                         float& e_inter, float& e_intra, float g6[6], float& gth) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = S.n;
-
+// ------------------------------------------------------------------ a3 forward kinematics of the frames (O8)
+// World frame (R, p) of this lane's fragment, F_g = F_parent o L_g, by pointer jumping (every warp the same).
+__device__ __forceinline__ void cta_frames(const CtaFrag& F, int max_depth, const float t[3], const float q[4], float theta,
+                                           float R[9], float p[3]) {
+    const int lane = threadIdx.x & 31;
     // ---- a3 forward kinematics (O8): world frame (R, p) of this lane's fragment, F_g = F_parent o L_g, by pointer jumping:
     // every lane starts from its own local transform L_g (the root from the rigid transform) and folds in the accumulated
     // transform of its current ancestor, whose own ancestor it then adopts -- ceil(log2(depth + 1)) rounds instead of `depth`.
-    float R[9], p[3];
     quat_matrix(q, R);
     p[0] = t[0]; p[1] = t[1]; p[2] = t[2];
     if (max_depth > 0) {
@@ -317,6 +314,82 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
             }
         }
     }
+}
+
+// ------------------------------------------------------------------ a6 reverse mode through the tree (O9)
+// In: the per-atom (force, moment about t) records AF of the whole ligand (visible).  Out: g6, gth as cta_eval.
+__device__ __forceinline__ void cta_reverse(const CtaTopo& S, const CtaFrag& F, const float R[9], const float p[3], const float t[3],
+                                            float g6[6], float& gth) {
+    const int lane = threadIdx.x & 31, n = S.n;
+    // ---- a6 reverse mode through the tree (O9): inclusive prefix sums of the per-atom (force, moment) records over the
+    // depth-first atom order (32 atoms per round, shuffle scan + carry); a fragment's subtree is the contiguous atom range
+    // [lo, sub_hi), so its wrench is a difference of two prefix entries.  Every warp writes the same prefix values to PF.
+    float carry[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    float4* PF = reinterpret_cast<float4*>(S.PF);
+    for (int a0 = 0; a0 < n; a0 += 32) {
+        const int a = a0 + lane;
+        float v[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        if (a < n) {
+            const float4 f = reinterpret_cast<const float4*>(S.AF)[2 * a], mo = reinterpret_cast<const float4*>(S.AF)[2 * a + 1];
+            v[0] = f.x; v[1] = f.y; v[2] = f.z; v[3] = mo.x; v[4] = mo.y; v[5] = mo.z;
+        }
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+#pragma unroll
+            for (int c = 0; c < 6; ++c) {
+                const float u = __shfl_up_sync(FULL_MASK, v[c], o);
+                if (lane >= o) v[c] += u;
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 6; ++c) v[c] += carry[c];
+        if (a < n) { PF[2 * a] = make_float4(v[0], v[1], v[2], 0.f); PF[2 * a + 1] = make_float4(v[3], v[4], v[5], 0.f); }
+#pragma unroll
+        for (int c = 0; c < 6; ++c) carry[c] = __shfl_sync(FULL_MASK, v[c], 31);
+    }
+    __syncwarp();
+    float s[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (F.valid) {
+        const float4 hf = PF[2 * (F.sub_hi - 1)], hm = PF[2 * (F.sub_hi - 1) + 1];
+        s[0] = hf.x; s[1] = hf.y; s[2] = hf.z; s[3] = hm.x; s[4] = hm.y; s[5] = hm.z;
+        if (F.lo > 0) {
+            const float4 lf = PF[2 * (F.lo - 1)], lm = PF[2 * (F.lo - 1) + 1];
+            s[0] -= lf.x; s[1] -= lf.y; s[2] -= lf.z; s[3] -= lm.x; s[4] -= lm.y; s[5] -= lm.z;
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) g6[c] = carry[c];
+    gth = 0.f;
+    if (F.valid && lane >= 1) {
+        const float wx = R[0] * F.ux + R[1] * F.uy + R[2] * F.uz;
+        const float wy = R[3] * F.ux + R[4] * F.uy + R[5] * F.uz;
+        const float wz = R[6] * F.ux + R[7] * F.uy + R[8] * F.uz;
+        const float bx = R[0] * F.ox + R[1] * F.oy + R[2] * F.oz + p[0] - t[0];
+        const float by = R[3] * F.ox + R[4] * F.oy + R[5] * F.oz + p[1] - t[1];
+        const float bz = R[6] * F.ox + R[7] * F.oy + R[8] * F.oz + p[2] - t[2];
+        const float tx = s[3] - (by * s[2] - bz * s[1]);             // torque about b = M_t - (b - t) x F
+        const float ty = s[4] - (bz * s[0] - bx * s[2]);
+        const float tz = s[5] - (bx * s[1] - by * s[0]);
+        gth = wx * tx + wy * ty + wz * tz;
+    }
+}
+
+// ------------------------------------------------------------------ a3..a6: one pose evaluation by the whole CTA
+// In : t[3], unit q[4] (uniform), theta (lane g holds the torsion angle of fragment g).
+// Out: ENERGY: e_inter, e_intra (uniform over the CTA); GRAD: g6 = {dE/dt, dE/domega about t} (uniform), gth = dE/dtheta
+//      on lane g (O9); x, y, z = this thread's atom (valid when `active`).
+// MDN: the mixture-density term (mdn.cuh); the lanes of an atom share its residues (lane `part` takes residues part,
+// part + lpa, ...), their shares join the pair force / the energy sums before the fixed-order reductions.
+template <bool GRAD, bool ENERGY, bool MDN>
+__device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
+                                         const MdnDev& M, const float4* __restrict__ mdn_par,
+                                         int max_depth, const float t[3], const float q[4], float theta,
+                                         int atom, int part, bool active, float& x, float& y, float& z,
+                                         float& e_inter, float& e_intra, float g6[6], float& gth) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = S.n;
+
+    float R[9], p[3];
+    cta_frames(F, max_depth, t, q, theta, R, p);
     // this thread's atom: x_a = R_frag(a) r_a + p_frag(a); the group's first lane publishes it and starts the gathers
     const int m = active ? S.meta[atom] : 0;
     {
@@ -334,11 +407,8 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     const bool lead = active && part == 0;
     GridCell cell;
     float4 glo = make_float4(0.f, 0.f, 0.f, 0.f), ghi = glo;
-    constexpr bool kMaybeDense = ROUNDS != 0;
-    const bool dense = ROUNDS == 1 || (ROUNDS == 2 && S.rounds);
     if (lead) {
-        if (kMaybeDense && dense) S.X4[atom] = make_float4(x, y, z, 0.f);
-        else { S.X[atom] = x; S.X[n + atom] = y; S.X[2 * n + atom] = z; }
+        S.X[atom] = x; S.X[n + atom] = y; S.X[2 * n + atom] = z;
         cell = grid_locate(G, m & 0xff, x, y, z);
         glo = __ldg(cell.p); ghi = __ldg(cell.p + 1);
     }
@@ -346,51 +416,7 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
 
     // ---- a5 intra-ligand pairs (O6)
     float eL = 0.f, eC = 0.f, eH = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
-    if (kMaybeDense && dense) {
-        // Dense partner sweep (internal.h): this warp's lanes hold the atoms l = c0 + lane of one 32-atom chunk after another and
-        // meet the partners b = b0 + 4 * warp + u, u = 0..3 (warp-uniform: one broadcast 16-byte load each); the other warps
-        // take the other partners, so a chunk's force is the sum of the warps' partials -- fixed order, after a barrier.
-        // GRAD: all partners (both ends of every pair); energy only: the partners b > l.
-        // A last chunk of at most 16 atoms is held twice, by the two half-warps, which split the partners between them.
-        constexpr int nw = TRIDSK_CTA_WARPS;
-        const int npad = S.npad, nch = npad >> 5;
-        float4* part = S.part + warp * npad;
-        for (int c0 = 0; c0 < npad; c0 += 32) {
-            const bool half = GRAD && n - c0 <= 16;
-            const int l = c0 + (half ? (lane & 15) : lane), bo = half ? (lane >> 4) << 2 : 0, per = half ? 8 : 4;
-            const unsigned lbit = 1u << (l & 31);
-            const float4 me = S.X4[l];
-            const float* crow = S.ctab + l;
-            const unsigned* hrow = S.hbm + ((GRAD ? 0 : nch) + (c0 >> 5)) * npad;
-            float ax = 0.f, ay = 0.f, az = 0.f;
-            for (int bb = (GRAD ? 0 : c0) + per * warp; bb < n; bb += per * nw) {
-                const int b0 = bb + bo;
-                const uint4 hw = *reinterpret_cast<const uint4*>(hrow + b0);
-                float4 pb[4];
-                float c[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    pb[u] = S.X4[b0 + u];
-                    c[u] = crow[(b0 + u) * npad];
-                    if (!GRAD) c[u] = l < b0 + u ? c[u] : -1e15f;
-                }
-                cta_dense4<GRAD, ENERGY>(K, me, pb, c, hw, lbit, eL, eC, eH, ax, ay, az);
-            }
-            if (GRAD) {
-                if (half) {
-                    ax += __shfl_xor_sync(FULL_MASK, ax, 16); ay += __shfl_xor_sync(FULL_MASK, ay, 16); az += __shfl_xor_sync(FULL_MASK, az, 16);
-                }
-                part[l] = make_float4(ax, ay, az, 0.f);
-            }
-        }
-        if (GRAD) {
-            eL *= 0.5f; eC *= 0.5f; eH *= 0.5f;                     // every pair was visited from both ends
-            __syncthreads();
-            if (active) {
-                for (int w = 0; w < nw; ++w) { const float4 f = S.part[w * npad + atom]; fx += f.x; fy += f.y; fz += f.z; }
-            }
-        }
-    } else if (GRAD) {
+    if (GRAD) {
         if (active) {
             const int k1 = S.rows[atom + 1];
             for (int k = S.rows[atom] + part; k < k1; k += 4 * S.lpa) {
@@ -462,56 +488,154 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     }
     if (!GRAD) return;
 
-    // ---- a6 reverse mode through the tree (O9): inclusive prefix sums of the per-atom (force, moment) records over the
-    // depth-first atom order (32 atoms per round, shuffle scan + carry); a fragment's subtree is the contiguous atom range
-    // [lo, sub_hi), so its wrench is a difference of two prefix entries.  Every warp writes the same prefix values to PF.
-    float carry[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    float4* PF = reinterpret_cast<float4*>(S.PF);
-    for (int a0 = 0; a0 < n; a0 += 32) {
-        const int a = a0 + lane;
-        float v[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        if (a < n) {
-            const float4 f = reinterpret_cast<const float4*>(S.AF)[2 * a], mo = reinterpret_cast<const float4*>(S.AF)[2 * a + 1];
-            v[0] = f.x; v[1] = f.y; v[2] = f.z; v[3] = mo.x; v[4] = mo.y; v[5] = mo.z;
+    cta_reverse(S, F, R, p, t, g6, gth);
+}
+
+// ------------------------------------------------------------------ a3..a6 for ligands above 64 atoms: dense partner sweep
+// The same contract as cta_eval, for a CTA of NW warps (4: score kernel, one atom per thread; 2: MC kernel, two atoms per thread).
+// Sweep (internal.h): this warp's lanes hold the atoms l = c0 + lane of one 32-atom chunk after another and meet the partners
+// b = b0 + 4 * warp + u, u = 0..3 (warp-uniform: one broadcast 16-byte load each); the other warps take the other partners, so a
+// chunk's force is the sum of the warps' partials -- fixed order, after a barrier.  GRAD: all partners (both ends of every
+// pair); energy only: the partners b > l.  A last chunk of at most 16 atoms is held twice, by the two half-warps, which split
+// the partners between them.  x0, y0, z0: the coordinates of atom threadIdx.x.
+template <bool GRAD, bool ENERGY, bool MDN, int NW>
+__device__ __forceinline__ void cta_eval_dense(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
+                                               const MdnDev& M, const float4* __restrict__ mdn_par,
+                                               int max_depth, const float t[3], const float q[4], float theta,
+                                               float& x0, float& y0, float& z0,
+                                               float& e_inter, float& e_intra, float g6[6], float& gth) {
+    constexpr int APT = TRIDSK_CTA_WARPS / NW;                      // atoms per thread: 128 atoms at most
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = S.n;
+    float R[9], p[3];
+    cta_frames(F, max_depth, t, q, theta, R, p);
+
+    // this thread's atoms: x_a = R_frag(a) r_a + p_frag(a), published with the atom type; the gathers start
+    float x[APT], y[APT], z[APT];
+    int m[APT];
+    bool act[APT];
+    GridCell cell[APT];
+    float4 glo[APT], ghi[APT];
+#pragma unroll
+    for (int k = 0; k < APT; ++k) {
+        const int atom = tid + 32 * NW * k;
+        act[k] = atom < n;
+        m[k] = act[k] ? S.meta[atom] : 0;
+        const int fr = (m[k] >> 8) & 0xff;
+        float A[9], b[3];
+#pragma unroll
+        for (int i = 0; i < 9; ++i) A[i] = __shfl_sync(FULL_MASK, R[i], fr);
+#pragma unroll
+        for (int i = 0; i < 3; ++i) b[i] = __shfl_sync(FULL_MASK, p[i], fr);
+        const float4 r = S.ref[act[k] ? atom : 0];
+        x[k] = A[0] * r.x + A[1] * r.y + A[2] * r.z + b[0];
+        y[k] = A[3] * r.x + A[4] * r.y + A[5] * r.z + b[1];
+        z[k] = A[6] * r.x + A[7] * r.y + A[8] * r.z + b[2];
+        glo[k] = make_float4(0.f, 0.f, 0.f, 0.f); ghi[k] = glo[k];
+        if (act[k]) {
+            S.X4[atom] = make_float4(x[k], y[k], z[k], __int_as_float(m[k] & 0xff));
+            cell[k] = grid_locate(G, m[k] & 0xff, x[k], y[k], z[k]);
+            glo[k] = __ldg(cell[k].p); ghi[k] = __ldg(cell[k].p + 1);
         }
+    }
+    x0 = x[0]; y0 = y[0]; z0 = z[0];
+    __syncthreads();
+
+    // ---- a5 intra-ligand pairs (O6)
+    float eL = 0.f, eC = 0.f, eH = 0.f;
+    const int npad = S.npad, plane = (npad >> 5) * npad;
+    float4* part = S.part + warp * npad;
+    for (int c0 = 0; c0 < npad; c0 += 32) {
+        const bool half = GRAD && n - c0 <= 16;
+        const int l = c0 + (half ? (lane & 15) : lane), bo = half ? (lane >> 4) << 2 : 0, per = half ? 8 : 4;
+        const unsigned lbit = 1u << (l & 31);
+        const float4 me = S.X4[l];
+        const float* trow = S.tt + 33 * __float_as_int(me.w);
+        const unsigned* irow = S.msk + (GRAD ? 0 : 2 * plane) + (c0 >> 5) * npad;
+        const unsigned* hrow = irow + plane;
+        float ax = 0.f, ay = 0.f, az = 0.f;
+        for (int bb = (GRAD ? 0 : c0) + per * warp; bb < n; bb += per * NW) {
+            const int b0 = bb + bo;
+            const uint4 iw = *reinterpret_cast<const uint4*>(irow + b0);
+            const uint4 hw = *reinterpret_cast<const uint4*>(hrow + b0);
+            const unsigned in[4] = {iw.x, iw.y, iw.z, iw.w};
+            float4 pb[4];
+            float c[4];
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
+            for (int u = 0; u < 4; ++u) {
+                pb[u] = S.X4[b0 + u];
+                c[u] = trow[__float_as_int(pb[u].w)];
+                c[u] = (in[u] & lbit) ? c[u] : -1e15f;
+            }
+            cta_dense4<GRAD, ENERGY>(K, me, pb, c, hw, lbit, eL, eC, eH, ax, ay, az);
+        }
+        if (GRAD) {
+            if (half) {
+                ax += __shfl_xor_sync(FULL_MASK, ax, 16); ay += __shfl_xor_sync(FULL_MASK, ay, 16); az += __shfl_xor_sync(FULL_MASK, az, 16);
+            }
+            part[l] = make_float4(ax, ay, az, 0.f);
+        }
+    }
+    if (GRAD) {
+        eL *= 0.5f; eC *= 0.5f; eH *= 0.5f;                         // every pair was visited from both ends
+        __syncthreads();
+    }
+
+    // ---- a4 receptor term of this thread's atoms (the gathers were issued before the first barrier), force and moment records
+    float ei = 0.f;
 #pragma unroll
-            for (int c = 0; c < 6; ++c) {
-                const float u = __shfl_up_sync(FULL_MASK, v[c], o);
-                if (lane >= o) v[c] += u;
+    for (int k = 0; k < APT; ++k) {
+        const int atom = tid + 32 * NW * k;
+        float gx = 0.f, gy = 0.f, gz = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
+        if (act[k]) {
+            ei += grid_blend<GRAD>(G, P.k_wall, cell[k], glo[k], ghi[k], gx, gy, gz);
+            if (GRAD) {
+#pragma unroll
+                for (int w = 0; w < NW; ++w) { const float4 f = S.part[w * npad + atom]; fx += f.x; fy += f.y; fz += f.z; }
+            }
+            if (MDN) {
+                float mx = 0.f, my = 0.f, mz = 0.f;
+                mdn_atom(M, mdn_par, n, atom, x[k], y[k], z[k], 0, 1, GRAD, ei, mx, my, mz);
+                if (GRAD) { fx = fmaf(mx, K.inv_kappa, fx); fy = fmaf(my, K.inv_kappa, fy); fz = fmaf(mz, K.inv_kappa, fz); }
+            }
+            if (GRAD) {
+                const float Fx = fmaf(K.kappa, fx, gx), Fy = fmaf(K.kappa, fy, gy), Fz = fmaf(K.kappa, fz, gz);
+                const float rx = x[k] - t[0], ry = y[k] - t[1], rz = z[k] - t[2];
+                float4* af = reinterpret_cast<float4*>(S.AF) + 2 * atom;
+                af[0] = make_float4(Fx, Fy, Fz, 0.f);
+                af[1] = make_float4(ry * Fz - rz * Fy, rz * Fx - rx * Fz, rx * Fy - ry * Fx, 0.f);
             }
         }
-#pragma unroll
-        for (int c = 0; c < 6; ++c) v[c] += carry[c];
-        if (a < n) { PF[2 * a] = make_float4(v[0], v[1], v[2], 0.f); PF[2 * a + 1] = make_float4(v[3], v[4], v[5], 0.f); }
-#pragma unroll
-        for (int c = 0; c < 6; ++c) carry[c] = __shfl_sync(FULL_MASK, v[c], 31);
     }
-    __syncwarp();
-    float s[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    if (F.valid) {
-        const float4 hf = PF[2 * (F.sub_hi - 1)], hm = PF[2 * (F.sub_hi - 1) + 1];
-        s[0] = hf.x; s[1] = hf.y; s[2] = hf.z; s[3] = hm.x; s[4] = hm.y; s[5] = hm.z;
-        if (F.lo > 0) {
-            const float4 lf = PF[2 * (F.lo - 1)], lm = PF[2 * (F.lo - 1) + 1];
-            s[0] -= lf.x; s[1] -= lf.y; s[2] -= lf.z; s[3] -= lm.x; s[4] -= lm.y; s[5] -= lm.z;
-        }
+    if (ENERGY) {
+        const float ea = fmaf(K.w_clash_ln2, eC, -fmaf(K.w_long, eL, K.w_hbond * eH));
+        const float si = warp_sum(ei), sa = warp_sum(ea);
+        if (lane == 0) { S.red[2 * warp] = si; S.red[2 * warp + 1] = sa; }
     }
+    __syncthreads();
+    if (ENERGY) {
+        e_inter = 0.f; e_intra = 0.f;
 #pragma unroll
-    for (int c = 0; c < 6; ++c) g6[c] = carry[c];
-    gth = 0.f;
-    if (F.valid && lane >= 1) {
-        const float wx = R[0] * F.ux + R[1] * F.uy + R[2] * F.uz;
-        const float wy = R[3] * F.ux + R[4] * F.uy + R[5] * F.uz;
-        const float wz = R[6] * F.ux + R[7] * F.uy + R[8] * F.uz;
-        const float bx = R[0] * F.ox + R[1] * F.oy + R[2] * F.oz + p[0] - t[0];
-        const float by = R[3] * F.ox + R[4] * F.oy + R[5] * F.oz + p[1] - t[1];
-        const float bz = R[6] * F.ox + R[7] * F.oy + R[8] * F.oz + p[2] - t[2];
-        const float tx = s[3] - (by * s[2] - bz * s[1]);             // torque about b = M_t - (b - t) x F
-        const float ty = s[4] - (bz * s[0] - bx * s[2]);
-        const float tz = s[5] - (bx * s[1] - by * s[0]);
-        gth = wx * tx + wy * ty + wz * tz;
+        for (int w = 0; w < NW; ++w) { e_inter += S.red[2 * w]; e_intra += S.red[2 * w + 1]; }
+    }
+    if (!GRAD) return;
+    cta_reverse(S, F, R, p, t, g6, gth);
+}
+
+// ROUNDS: 0 = pair records (ligands of up to 64 atoms, 128 threads), 1 = dense partner sweep with two warps per chain (MC kernel),
+// 2 = decided at run time by S.rounds, 128 threads (score kernel).
+template <bool GRAD, bool ENERGY, bool MDN, int ROUNDS>
+__device__ __forceinline__ void cta_eval_any(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
+                                             const MdnDev& M, const float4* __restrict__ mdn_par,
+                                             int max_depth, const float t[3], const float q[4], float theta,
+                                             int atom, int part, bool active, float& x, float& y, float& z,
+                                             float& e_inter, float& e_intra, float g6[6], float& gth) {
+    if constexpr (ROUNDS == 1) {
+        cta_eval_dense<GRAD, ENERGY, MDN, 2>(S, G, P, K, F, M, mdn_par, max_depth, t, q, theta, x, y, z, e_inter, e_intra, g6, gth);
+    } else {
+        if (ROUNDS == 2 && S.rounds)
+            cta_eval_dense<GRAD, ENERGY, MDN, 4>(S, G, P, K, F, M, mdn_par, max_depth, t, q, theta, x, y, z, e_inter, e_intra, g6, gth);
+        else
+            cta_eval<GRAD, ENERGY, MDN>(S, G, P, K, F, M, mdn_par, max_depth, t, q, theta, atom, part, active, x, y, z, e_inter, e_intra, g6, gth);
     }
 }
 
@@ -533,10 +657,10 @@ __device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const Ct
 }
 
 // ------------------------------------------------------------------ the fused MC kernel, one CTA per chain
-// resident CTAs per SM the register budget is set for: 4 for the dense-sweep instance (C4 72.8 -> 64.2 ms), 3 for the record
-// instance (with 4, C2 6.0 -> 6.3 ms) and with the mixture-density term (spills at 128 registers)
+// Record instance: 128 threads, registers for 3 resident CTAs per SM (with 4 x 128 registers, C2 goes 6.0 -> 6.3 ms).  Dense
+// instance: 64 threads and 128 registers, EIGHT chains resident per SM (6 with the mixture-density term, which spills at 128).
 template <bool MDN, int ROUNDS>
-__global__ void __launch_bounds__(128, (ROUNDS && !MDN) ? 4 : 3) mc_cta_kernel(const McLaunch a) {
+__global__ void __launch_bounds__(ROUNDS ? 64 : 128, ROUNDS ? (MDN ? 6 : 8) : 3) mc_cta_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lig = a.lig_list[blockIdx.x / a.n_chains];
@@ -589,7 +713,7 @@ __global__ void __launch_bounds__(128, (ROUNDS && !MDN) ? 4 : 3) mc_cta_kernel(c
             const float uu = (k & 3) == 0 ? v0 : (k & 3) == 1 ? v1 : (k & 3) == 2 ? v2 : v3;
             cth = F.tor >= 0 ? PI_F * (2.f * uu - 1.f) : 0.f;
         }
-        cta_eval<false, true, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, ct, cq, cth, atom, part, active, x, y, z, ei, ea, g6, gth);
+        cta_eval_any<false, true, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, ct, cq, cth, atom, part, active, x, y, z, ei, ea, g6, gth);
         ecur = ei + ea;
         ebest = ecur;
 #pragma unroll
@@ -624,7 +748,7 @@ __global__ void __launch_bounds__(128, (ROUNDS && !MDN) ? 4 : 3) mc_cta_kernel(c
         float m[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         float b1p = 1.f, b2p = 1.f;
         for (int rf = 0; rf < P.n_refine; ++rf) {
-            cta_eval<true, false, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
+            cta_eval_any<true, false, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
             b1p *= P.adam_b1; b2p *= P.adam_b2;
             const float c1 = __fdividef(1.f, 1.f - b1p), c2 = __fdividef(1.f, 1.f - b2p);
             float g[7] = {g6[0], g6[1], g6[2], g6[3], g6[4], g6[5], gth}, dl[7];
@@ -645,7 +769,7 @@ __global__ void __launch_bounds__(128, (ROUNDS && !MDN) ? 4 : 3) mc_cta_kernel(c
         }
 
         // a8: energy of the refined proposal, Metropolis, best tracking
-        cta_eval<false, true, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
+        cta_eval_any<false, true, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
         const float enew = ei + ea;
         const bool accept = isfinite(enew) && (um < expf(-P.beta * (enew - ecur)));
         if (a.trace != nullptr && tid == 0) {
@@ -694,8 +818,8 @@ __global__ void __launch_bounds__(128) score_cta_kernel(const ScoreLaunch a) {
     float t[3], q[4], th, x, y, z, g6[6], gth = 0.f, ei, ea;
     cta_load_pose(a.poses + (size_t)i * a.pose_stride, F, t, q, th);
     quat_normalise(q);
-    if (a.grad != nullptr) cta_eval<true, true, MDN, 2>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
-    else cta_eval<false, true, MDN, 2>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
+    if (a.grad != nullptr) cta_eval_any<true, true, MDN, 2>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
+    else cta_eval_any<false, true, MDN, 2>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
     if (tid == 0) { a.energy[3 * (size_t)i] = ei + ea; a.energy[3 * (size_t)i + 1] = ei; a.energy[3 * (size_t)i + 2] = ea; }
     if (a.grad != nullptr && warp == 0) {
         float* g = a.grad + (size_t)i * a.grad_stride;
@@ -729,8 +853,8 @@ cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int rounds, size_t 
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const unsigned nb = (unsigned)blocks;
-    if (a.mdn.n_res > 0) { if (rounds) mc_cta_kernel<true, 1><<<nb, 128, smem_bytes, s>>>(a); else mc_cta_kernel<true, 0><<<nb, 128, smem_bytes, s>>>(a); }
-    else { if (rounds) mc_cta_kernel<false, 1><<<nb, 128, smem_bytes, s>>>(a); else mc_cta_kernel<false, 0><<<nb, 128, smem_bytes, s>>>(a); }
+    if (a.mdn.n_res > 0) { if (rounds) mc_cta_kernel<true, 1><<<nb, 64, smem_bytes, s>>>(a); else mc_cta_kernel<true, 0><<<nb, 128, smem_bytes, s>>>(a); }
+    else { if (rounds) mc_cta_kernel<false, 1><<<nb, 64, smem_bytes, s>>>(a); else mc_cta_kernel<false, 0><<<nb, 128, smem_bytes, s>>>(a); }
     return cudaGetLastError();
 }
 
