@@ -819,7 +819,7 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
         if (want_cta) {
             int th, lpa;
             cta_shape(h.n, &th, &lpa);
-            const int k = h.n > TRIDSK_CTA_ROUNDS_N ? 1 : 0;       // bucket 1: the round-schedule instance of the kernel
+            const int k = h.n > TRIDSK_CTA_ROUNDS_N ? 1 : 0;       // bucket 1: the dense-sweep instance of the kernel
             lg->cta_bucket[k].push_back(i);
             lg->cta_smem[k] = std::max(lg->cta_smem[k], cta_layout(h.n, h.T, h.n_pairs).total);
         }

@@ -136,7 +136,7 @@ struct LaneRec {
 // donor/acceptor flag, or -1 if the pair is not in the set (for even n the items l >= n/2 of round n/2 repeat pairs and are
 // absent).  The MC kernel gives such a chain TWO warps (64-thread CTAs, two atoms per thread outside the sweep), so that eight
 // chains stay resident per SM.
-#define TRIDSK_CTA_ROUNDS_N 64         // ligands above this many atoms use the round schedule
+#define TRIDSK_CTA_ROUNDS_N 64         // ligands above this many atoms use the dense partner sweep
 
 // Per-fragment record; fragment 0 is the root, fragment k+1 hangs off torsion k.
 struct FragRec {
@@ -345,7 +345,7 @@ struct tridsk_ligands {
     int* cta_rows = nullptr;
     uint2* cta_recs = nullptr;
     float* cta_rtab = nullptr;
-    std::vector<int> cta_bucket[2];              // ligand ids: [0] up to 64 atoms (row form), [1] above (round schedule)
+    std::vector<int> cta_bucket[2];              // ligand ids: [0] up to 64 atoms (row form), [1] above (dense partner sweep)
     int* cta_bucket_dev[2] = {nullptr, nullptr};
     size_t cta_smem[2] = {0, 0};                 // largest shared-memory need per bucket
     int* all_ids = nullptr;       // 0..n_lig-1 re-ordered per lane bucket (refilled when the plan key changes)

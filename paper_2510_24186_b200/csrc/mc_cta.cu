@@ -11,6 +11,8 @@
 //     its own lanes -- no scatter, no atomics, bit-reproducible; the energy-only evaluation walks the flat pair list;
 //   * the receptor term of an atom is two 16-byte gathers whose L2 latency hides behind the pair loop;
 //   * two __syncthreads per evaluation: coordinates visible, per-atom (force, moment) / energy partials visible.
+// Ligands above 64 atoms: two warps per chain and a dense partner sweep instead of pair records (cta_eval_dense, internal.h),
+// so that eight such chains stay resident per SM.
 //
 // P:N = PAPER.md line N; O*/G* = DESIGN.md section 3.
 #include "chain.cuh"
