@@ -125,98 +125,16 @@ __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char*
     F.sub_hi = F.valid ? S.frag[e - 1].own_hi : 1;
 }
 
-// ------------------------------------------------------------------ O2: one pair, scalar (same arithmetic as lane_rec)
+// ------------------------------------------------------------------ O2: four pairs at a time (the arithmetic of lane_rec)
+// Branch-free in the main part so that the four dependency chains interleave (a thread's pairs are otherwise a serial string of
+// shared-memory load -> rsqrt -> ex2 latencies): one lg2 for the product of the four clash ratios, the clash force switched by
+// one compare pair.  d* = x_a - x_b; c = dvdw + mu, or -1e15 for a slot without a pair, which then adds exactly zero;
+// hbw[u] & lbit != 0: slot u is a donor/acceptor pair (a slot group without any skips that term).  Out: s[u] = (de/dd) / d /
+// kappa, so that f_a += s (x_a - x_b).
 template <bool GRAD, bool ENERGY>
-__device__ __forceinline__ void cta_pair(const PairK& K, float dx, float dy, float dz, float c, bool hb,
-                                         float& eL, float& eC, float& eH, float& fx, float& fy, float& fz) {
-    const float d2 = fmaxf(fmaf(dx, dx, fmaf(dy, dy, dz * dz)), 1e-12f);
-    const float rinv = rsqrt_approx(d2);
-    const float d = d2 * rinv;
-    const float t = d - c;
-    const float u = t * K.nk2;
-    float g = ex2_approx(u * t);
-    g = d < K.dmax ? g : 0.f;
-    const float dc = hb ? K.hb_dclash : c - K.mu;
-    const float q = dc * fminf(rinv, K.inv_floor);
-    float s = 0.f;
-    if (ENERGY) { eL += g; eC += lg2_approx(fmaxf(q, 1.f)); }
-    if (GRAD) {
-        s = u * g * rinv;
-        if (q > 1.f && rinv < K.inv_floor) s = fmaf(-K.kc * rinv, rinv, s);
-    }
-    if (hb) {
-        const float th = d - K.hb_mu;
-        float gh = ex2_approx(K.hb_nk2 * th * th);
-        gh = d < K.hb_dmax ? gh : 0.f;
-        if (ENERGY) eH += gh;
-        if (GRAD) s = fmaf(K.kh * th, gh * rinv, s);
-    }
-    if (GRAD) { fx = fmaf(s, dx, fx); fy = fmaf(s, dy, fy); fz = fmaf(s, dz, fz); }
-}
-
-// Four pairs at a time, branch-free in the main part so that the four dependency chains interleave (a thread's pairs are
-// otherwise a serial string of shared-memory load -> rsqrt -> ex2 latencies).  A lane without a pair in slot u passes
-// ok[u] = false: its c becomes -1e15 and the slot evaluates to exactly zero.
-template <bool GRAD, bool ENERGY>
-__device__ __forceinline__ void cta_pairs4s(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c_in[4],
-                                            const bool hb_in[4], const bool ok[4], float& eL, float& eC, float& eH, float s[4]) {
-    float d[4], rinv[4];
-    bool hb[4], any_hb = false;
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const float c = ok[u] ? c_in[u] : -1e15f;
-        hb[u] = ok[u] && hb_in[u];
-        any_hb = any_hb || hb[u];
-        const float d2 = fmaxf(fmaf(dx[u], dx[u], fmaf(dy[u], dy[u], dz[u] * dz[u])), 1e-12f);
-        rinv[u] = rsqrt_approx(d2);
-        d[u] = d2 * rinv[u];
-        const float t = d[u] - c;
-        const float w = t * K.nk2;
-        float g = ex2_approx(w * t);
-        g = d[u] < K.dmax ? g : 0.f;
-        const float dc = hb[u] ? K.hb_dclash : c - K.mu;
-        const float q = dc * fminf(rinv[u], K.inv_floor);
-        s[u] = 0.f;
-        if (ENERGY) { eL += g; eC += lg2_approx(fmaxf(q, 1.f)); }
-        if (GRAD) {
-            s[u] = w * g * rinv[u];
-            if (q > 1.f && rinv[u] < K.inv_floor) s[u] = fmaf(-K.kc * rinv[u], rinv[u], s[u]);
-        }
-    }
-    if (any_hb) {
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (hb[u]) {
-                const float th = d[u] - K.hb_mu;
-                float gh = ex2_approx(K.hb_nk2 * th * th);
-                gh = d[u] < K.hb_dmax ? gh : 0.f;
-                if (ENERGY) eH += gh;
-                if (GRAD) s[u] = fmaf(K.kh * th, gh * rinv[u], s[u]);
-            }
-        }
-    }
-}
-template <bool GRAD, bool ENERGY>
-__device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c_in[4],
-                                           const bool hb_in[4], const bool ok[4], float& eL, float& eC, float& eH,
-                                           float& fx, float& fy, float& fz) {
-    float s[4];
-    cta_pairs4s<GRAD, ENERGY>(K, dx, dy, dz, c_in, hb_in, ok, eL, eC, eH, s);
-    if (GRAD) {
-#pragma unroll
-        for (int u = 0; u < 4; ++u) { fx = fmaf(s[u], dx[u], fx); fy = fmaf(s[u], dy[u], fy); fz = fmaf(s[u], dz[u], fz); }
-    }
-}
-
-// Dense partner sweep (internal.h): this lane's atom `me` against four partners, branch-free in the main part (the arithmetic
-// of lane_rec in mc_lane.cu: one lg2 for the product of the four clash ratios, the clash force switched by one compare pair);
-// hw.{x,y,z,w} = the lanes that form a donor/acceptor pair with partner 0..3 -- a partner without any skips that term for the
-// whole warp.  A visit that is not in the pair set has c = -1e15 and adds exactly zero.
-template <bool GRAD, bool ENERGY>
-__device__ __forceinline__ void cta_dense4(const PairK& K, const float4 me, const float4 pb[4], const float c[4], const uint4 hw,
-                                           unsigned lbit, float& eL, float& eC, float& eH, float& ax, float& ay, float& az) {
-    const unsigned hbw[4] = {hw.x, hw.y, hw.z, hw.w};
-    float dx[4], dy[4], dz[4], d[4], rinv[4], s[4], q[4], t[4], dc[4];
+__device__ __forceinline__ void cta_quad(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c[4],
+                                         const unsigned hbw[4], unsigned lbit, float& eL, float& eC, float& eH, float s[4]) {
+    float d[4], rinv[4], q[4], t[4], dc[4];
     if (ENERGY) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
@@ -226,7 +144,6 @@ __device__ __forceinline__ void cta_dense4(const PairK& K, const float4 me, cons
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-        dx[u] = me.x - pb[u].x; dy[u] = me.y - pb[u].y; dz[u] = me.z - pb[u].z;
         const float d2 = fmaf(dx[u], dx[u], fmaf(dy[u], dy[u], fmaf(dz[u], dz[u], 1e-12f)));
         rinv[u] = rsqrt_approx(d2);
         d[u] = d2 * rinv[u];
@@ -234,6 +151,7 @@ __device__ __forceinline__ void cta_dense4(const PairK& K, const float4 me, cons
         const float w = t[u] * K.nk2;
         float g = ex2_approx(w * t[u]);
         g = d[u] < K.dmax ? g : 0.f;
+        s[u] = 0.f;
         if (ENERGY) {
             eL += g;
             q[u] = fmaxf(dc[u] * fminf(rinv[u], K.inv_floor), 1.f);
@@ -246,7 +164,7 @@ __device__ __forceinline__ void cta_dense4(const PairK& K, const float4 me, cons
     if (ENERGY) eC += lg2_approx((q[0] * q[1]) * (q[2] * q[3]));
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-        if (hbw[u] != 0u) {                                          // warp-uniform
+        if (hbw[u] != 0u) {
             if (hbw[u] & lbit) {
                 const float th = d[u] - K.hb_mu;
                 float gh = ex2_approx(K.hb_nk2 * th * th);
@@ -261,6 +179,32 @@ __device__ __forceinline__ void cta_dense4(const PairK& K, const float4 me, cons
             }
         }
     }
+}
+// record form: per-slot flags; a lane without a pair in slot u passes ok[u] = false
+template <bool GRAD, bool ENERGY>
+__device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c_in[4],
+                                           const bool hb_in[4], const bool ok[4], float& eL, float& eC, float& eH,
+                                           float& fx, float& fy, float& fz) {
+    float c[4], s[4];
+    unsigned hbw[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { c[u] = ok[u] ? c_in[u] : -1e15f; hbw[u] = (ok[u] && hb_in[u]) ? 1u : 0u; }
+    cta_quad<GRAD, ENERGY>(K, dx, dy, dz, c, hbw, 1u, eL, eC, eH, s);
+    if (GRAD) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { fx = fmaf(s[u], dx[u], fx); fy = fmaf(s[u], dy[u], fy); fz = fmaf(s[u], dz[u], fz); }
+    }
+}
+// dense partner sweep (internal.h): this lane's atom `me` against four partners; hw.{x,y,z,w} = the lanes that form a
+// donor/acceptor pair with partner 0..3 -- a partner without any skips that term for the whole warp
+template <bool GRAD, bool ENERGY>
+__device__ __forceinline__ void cta_dense4(const PairK& K, const float4 me, const float4 pb[4], const float c[4], const uint4 hw,
+                                           unsigned lbit, float& eL, float& eC, float& eH, float& ax, float& ay, float& az) {
+    const unsigned hbw[4] = {hw.x, hw.y, hw.z, hw.w};
+    float dx[4], dy[4], dz[4], s[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { dx[u] = me.x - pb[u].x; dy[u] = me.y - pb[u].y; dz[u] = me.z - pb[u].z; }
+    cta_quad<GRAD, ENERGY>(K, dx, dy, dz, c, hbw, lbit, eL, eC, eH, s);
     if (GRAD) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) { ax = fmaf(s[u], dx[u], ax); ay = fmaf(s[u], dy[u], ay); az = fmaf(s[u], dz[u], az); }
