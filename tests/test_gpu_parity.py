@@ -826,7 +826,7 @@ def test_mdn_teacher_forced_steps_match_oracle(orc, eng, gp, system):
     """Chains sampled under the full score: teacher-forced MC steps against orc_mc_step with the term attached."""
     from paper_2510_24186_b200 import split_state
     S = system
-    ids = [1, 0, 4]
+    ids = [1, 0, 4, 12]                                          # 12: 80 atoms, the CTA kernel's dense-sweep instance
     b, ligs, Ls = _mdn_system(orc, eng, S, ids, K=4, seed=300)
     n_chains, seed, stride = 32, 17, 7 + ligs.max_tor
     r = eng.dock(S["g_grid"], ligs, gp, *_dock_args(S), n_chains, 0, 1, seed=seed, want_state=True)
@@ -851,7 +851,7 @@ def test_mdn_teacher_forced_steps_match_oracle(orc, eng, gp, system):
                 assert close(tr["e_prop"], rec.e_prop, rtol=1e-3, atol=1e-3), (s, l, c, tr["e_prop"], rec.e_prop)
                 assert (tr["flags"] & 1) == rec.accept, (s, l, c)
     print(f"E_MDN teacher-forced: compared {compared}, skipped {skipped}")
-    assert compared > 0.85 * 6 * 3 * 16
+    assert compared > 0.85 * 6 * len(ids) * 16
     ligs.free()
 
 
