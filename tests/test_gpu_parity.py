@@ -765,6 +765,39 @@ def test_extreme_ligand_sizes_under_every_mapping(orc, gp, mode):
         e.close()
 
 
+def test_thirty_two_atom_types_under_every_mapping(orc, gp):
+    """The type-table limit (32 atom types): the CTA kernel's dense sweep reads c = dvdw + mu from a (type, type) table of that
+    size; ligands on both sides of its 64-atom switch, per-pose energy and gradient and a short dock re-scored by the oracle."""
+    from paper_2510_24186_b200 import Engine
+    rec = synth.receptor(200, 16.0, 32, seed=1234, grid_n=44)
+    radius, role = synth.type_table(32)
+    ty, p = orc.Types(radius, role), orc.default_params()
+    G = orc.build_grid(p, ty, rec.xyz, rec.type, rec.origin, rec.dims, rec.spacing)
+    batch = synth.ligands([40, 70, 80, 113], [6, 12, 20, 25], 32, seed=321)
+    assert len(np.unique(batch.atom_type)) >= 30
+    Ls = [orc.ligand_from_batch(batch, l) for l in range(batch.n_lig)]
+    li = np.repeat(np.arange(batch.n_lig, dtype=np.int32), 3)
+    poses = synth.random_poses(batch, li, rec, seed=8, spread=0.5)
+    for mode in (1, 2, 3):
+        e = Engine(0)
+        try:
+            e.set_kernel(mode)
+            grid = e.grid_from_values(G.g, rec.origin, rec.spacing)
+            ligs = e.load_ligands(batch, radius, role)
+            en, gr, _ = e.score_grad(grid, ligs, gp, li, poses)
+            for i in range(len(li)):
+                L = Ls[int(li[i])]
+                eo, go, _, _ = orc.score_grad(p, ty, G, L, poses[i, :7 + L.T].astype(np.float64))
+                assert worst(en[i], eo) <= 1.0, (mode, L.n, en[i], eo)
+                assert worst(gr[i, :6 + L.T], go, scale=np.abs(go).max()) <= 1.0, (mode, L.n)
+            r = e.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, 16, 10, 1, seed=3)
+            for l, L in enumerate(Ls):
+                eo = orc.score_grad(p, ty, G, L, r["pose"][l, 0, :7 + L.T].astype(np.float64), want_grad=False)[0][0]
+                assert close(r["energy"][l, 0, 0], eo, rtol=2e-4, atol=2e-3), (mode, L.n)
+        finally:
+            e.close()
+
+
 # ------------------------------------------------------------------------------------------- E_MDN (O15; SURVEY 8(f) NEXT-1)
 def _mdn_system(orc, eng, S, lig_ids, K, seed):
     """Synthetic residues (groups of 8 receptor atoms) and mixture parameters for a sub-batch of the test ligands; the term
