@@ -252,6 +252,29 @@ int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* 
                 float* out_energy, float* out_pose, int* out_chain, const tridsk_dock_opts* opts);
 
 /*
+ * tridsk_dock for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the same docking run (a CTA per chain, Philox initialisation, plain top-k) whose only
+ * scratch -- the per-chain state {pose_cur, pose_best, e_cur, e_best}, n_lig * n_chains * (2 * pose_stride + 2) floats --
+ * lives in ONE array of TRIDSK_STATIC_SCRATCH_BYTES (4 MiB) that is part of the library image: every GPU that loads the
+ * library holds it until the process exits.  The call makes no cudaMalloc / cudaFree / graph / event / stream creation;
+ * it enqueues the fused MC kernel(s) and the top-k kernel on the ctx stream and returns without synchronising.
+ *   - out_energy / out_pose / out_chain must be DEVICE memory (layout as tridsk_dock); TRIDSK_EINVAL otherwise.
+ *   - TRIDSK_ELIMIT with a message naming both sizes when the chain state exceeds the 4 MiB (e.g. 1,024 chains of a
+ *     20-torsion ligand need 0.22 MiB, 32 ligands x 384 chains x 6 torsions 1.3 MiB) or when the batch has more than
+ *     1024 ligands (it needs the CTA-per-chain pair format); nothing is launched then.
+ *   - The array is SHARED by every such call on that GPU, from any ctx or thread, and keeps the previous call's contents:
+ *     two calls whose kernels overlap on the GPU (different streams, no ordering between them) race on it.  Calls on one
+ *     stream are ordered and safe.  Nothing in it has to start at zero: the MC kernel writes every chain's state before
+ *     the top-k kernel reads it.
+ * Results are bit-identical to tridsk_dock under mapping 3 with the same arguments and no options.
+ */
+#define TRIDSK_STATIC_SCRATCH_BYTES (4u << 20)
+int tridsk_dock_static(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* ligs, const tridsk_params* params,
+                       const float box_min[3], const float box_max[3], const float pocket_center[3], float pocket_radius,
+                       int n_chains, int n_steps, int top_k, unsigned long long seed, int pose_stride,
+                       float* out_energy, float* out_pose, int* out_chain);
+
+/*
  * Chain-to-thread mapping of the fused kernel: 0 = automatic (a CTA per chain for a single dock with
  * at most 8 chains per SM, a lane per chain when n_lig * n_chains >= 64 per SM, a warp per chain in between), 1 = always
  * a warp per chain, 2 = always a lane per chain, 3 = always a CTA per chain (batches of at most 1024 ligands),

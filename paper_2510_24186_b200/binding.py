@@ -400,6 +400,20 @@ class Engine:
             res["trace"] = trace
         return res
 
+    def dock_static(self, grid: Grid, ligs: Ligands, params, box_min, box_max, pocket_center, pocket_radius,
+                    n_chains, n_steps, top_k, out, seed=0, pose_stride=None):
+        """tridsk_dock_static: the docking run without any allocation (chain state in the library's 4 MiB static device
+        array); `out` = caller-allocated CUDA tensors (energy[n_lig,k,2], pose[n_lig,k,stride], chain[n_lig,k] int32)."""
+        stride = int(pose_stride or (7 + ligs.max_tor))
+        energy, pose, chain = out
+        self._sync_in()
+        self._ck(lib().tridsk_dock_static(self.ctx, grid.handle, ligs.handle, C.byref(params), _f3(box_min), _f3(box_max),
+                                          _f3(pocket_center), C.c_float(pocket_radius), C.c_int(n_chains), C.c_int(n_steps),
+                                          C.c_int(top_k), C.c_ulonglong(seed), C.c_int(stride), _ptr(energy), _ptr(pose),
+                                          _ptr(chain)))
+        self._sync_out()
+        return dict(energy=energy, pose=pose, chain=chain)
+
     def last_dock_ms(self):
         """(MC kernel series, top-k) device milliseconds of the last dock, from CUDA events on the ctx stream."""
         ms = (C.c_float * 2)()

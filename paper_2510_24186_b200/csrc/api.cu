@@ -15,6 +15,7 @@
 #include <nvtx3/nvToolsExt.h>
 
 #include "internal.h"
+#include <mutex>
 
 // ---------------------------------------------------------------------------------------- helpers
 // NVTX range around a C-ABI call: captures under nsys / ncu name the four hot-path calls.
@@ -42,6 +43,9 @@ static int fail(tridsk_ctx* ctx, int code, const std::string& msg) {
             return fail(ctx, e_ == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA,       \
                         std::string(#call) + ": " + cudaGetErrorString(e_));                       \
     } while (0)
+
+// tridsk_dock_static (end of this file): resolves the device address of its static scratch array on the current device
+static cudaError_t dock_static_prepare(int device);
 
 static bool is_device_ptr(const void* p) {
     cudaPointerAttributes at;
@@ -137,6 +141,7 @@ extern "C" int tridsk_create(tridsk_ctx** out, int device, void* cuda_stream) {
     e = mc_lane_prepare(TRIDSK_SMEM_MAX_CTA);
     if (e == cudaSuccess) e = mc_cta_prepare();
     if (e == cudaSuccess) e = topk_prepare();
+    if (e == cudaSuccess) e = dock_static_prepare(device);
     if (e != cudaSuccess) { fprintf(stderr, "tridsk_create: %s\n", cudaGetErrorString(e)); delete ctx; return TRIDSK_ECUDA; }
     if (!ctx->stream) {               // the legacy default stream cannot be captured into a graph: own one
         e = cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking);
@@ -1545,5 +1550,88 @@ extern "C" int tridsk_debug_microbench(tridsk_ctx* ctx, int which, unsigned long
     if (e != cudaSuccess) return fail(ctx, TRIDSK_ECUDA, std::string("microbench: ") + cudaGetErrorString(e));
     ctx->launches += 2;
     *work = w;
+    return TRIDSK_OK;
+}
+
+// ---------------------------------------------------------------------------------------- tridsk_dock_static
+// The docking run for callers that may not allocate (tridsk.h): the chain state lives in a file-scope device array instead
+// of ctx scratch.  In host code `g_dock_scratch` is a host-side stand-in for the symbol, NOT a device address; the address
+// is taken with cudaGetSymbolAddress once per device, with that device current (tridsk_create), and handed to the kernels.
+#define TRIDSK_MAX_DEVICES 64
+static __device__ __align__(256) unsigned char g_dock_scratch[TRIDSK_STATIC_SCRATCH_BYTES];
+static float* g_dock_scratch_ptr[TRIDSK_MAX_DEVICES] = {};
+static std::mutex g_dock_scratch_mu;
+
+static cudaError_t dock_static_prepare(int device) {
+    if (device < 0 || device >= TRIDSK_MAX_DEVICES) return cudaSuccess;          // tridsk_dock_static reports it
+    std::lock_guard<std::mutex> lk(g_dock_scratch_mu);
+    if (g_dock_scratch_ptr[device]) return cudaSuccess;
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_dock_scratch);
+    if (e == cudaSuccess) g_dock_scratch_ptr[device] = (float*)ptr;
+    return e;
+}
+
+extern "C" int tridsk_dock_static(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* ligs, const tridsk_params* params,
+                                  const float box_min[3], const float box_max[3], const float pocket_center[3], float pocket_radius,
+                                  int n_chains, int n_steps, int top_k, unsigned long long seed, int pose_stride,
+                                  float* out_energy, float* out_pose, int* out_chain) {
+    if (!ctx || !grid || !ligs || !params || !box_min || !box_max || !pocket_center)
+        return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    NvtxRange nvtx_("tridsk_dock_static");
+    if (int prc = check_params(ctx, params)) return prc;
+    if (n_chains < 1 || n_steps < 0 || top_k < 0 || top_k > n_chains) return fail(ctx, TRIDSK_EINVAL, "bad n_chains / n_steps / top_k");
+    if (top_k > 0 && (!out_energy || !out_pose || !out_chain)) return fail(ctx, TRIDSK_EINVAL, "null output");
+    if (top_k > 0 && (!is_device_ptr(out_energy) || !is_device_ptr(out_pose) || !is_device_ptr(out_chain)))
+        return fail(ctx, TRIDSK_EINVAL, "tridsk_dock_static writes device memory only (a host output would need a staging allocation)");
+    if (pose_stride < 7 + ligs->max_tor) return fail(ctx, TRIDSK_EINVAL, "pose_stride < 7 + max torsions");
+    for (int c = 0; c < 3; ++c) if (!(box_min[c] <= box_max[c])) return fail(ctx, TRIDSK_EINVAL, "box_min > box_max");
+    const int L = ligs->n_lig;
+    if (L == 0) return TRIDSK_OK;
+    if (!ligs->has_cta) return fail(ctx, TRIDSK_ELIMIT, "tridsk_dock_static needs a ligand batch of at most 1024 ligands (CTA-per-chain pair format)");
+    if (std::max(ligs->cta_smem[0], ligs->cta_smem[1]) > TRIDSK_SMEM_MAX_CTA)
+        return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
+    const size_t nch = (size_t)L * n_chains, n_pose_f = nch * pose_stride;
+    const size_t state_bytes = sizeof(float) * (2 * n_pose_f + 2 * nch);
+    if (state_bytes > TRIDSK_STATIC_SCRATCH_BYTES)
+        return fail(ctx, TRIDSK_ELIMIT, "tridsk_dock_static: the chain state of " + std::to_string(nch) + " chains x pose_stride " +
+                    std::to_string(pose_stride) + " needs " + std::to_string(state_bytes) + " bytes, the static scratch array holds " +
+                    std::to_string((size_t)TRIDSK_STATIC_SCRATCH_BYTES) + " (use tridsk_dock)");
+    float* state = (ctx->device >= 0 && ctx->device < TRIDSK_MAX_DEVICES) ? g_dock_scratch_ptr[ctx->device] : nullptr;
+    if (!state) return fail(ctx, TRIDSK_ECUDA, "tridsk_dock_static: no static scratch address for this device");
+
+    McLaunch base;
+    memset(&base, 0, sizeof(base));
+    base.hdr = ligs->hdr; base.atom_f4 = ligs->atom_f4; base.atom_i = ligs->atom_i; base.frags = ligs->frags; base.rounds = ligs->rounds;
+    base.lane_frags = ligs->lane_frags; base.lane_stream = ligs->lane_stream; base.lane_recs = ligs->lane_recs;
+    base.cta_rows = ligs->cta_rows; base.cta_recs = ligs->cta_recs; base.cta_rtab = ligs->cta_rtab;
+    base.grid = grid->d;
+    base.mdn = ligs->mdn;
+    to_dparams(params, &base.P);
+    for (int c = 0; c < 3; ++c) { base.box_min[c] = box_min[c]; base.box_max[c] = box_max[c]; base.centre[c] = pocket_center[c]; }
+    base.radius = pocket_radius;
+    base.n_chains = n_chains; base.pose_stride = pose_stride; base.seed = seed;
+    base.pose_cur = state; base.pose_best = state + n_pose_f; base.e_cur = state + 2 * n_pose_f; base.e_best = state + 2 * n_pose_f + nch;
+    base.first_step = 0; base.n_steps = n_steps; base.init_mode = 0;             // a1: Philox initialisation writes every chain's state
+    ctx->last_kernel = 3;
+    for (int k = 0; k < 2; ++k) {                                                // the two instances of the CTA kernel (internal.h)
+        if (ligs->cta_bucket[k].empty()) continue;
+        McLaunch a = base;
+        a.lig_list = ligs->cta_bucket_dev[k]; a.n_list = (int)ligs->cta_bucket[k].size();
+        CK(launch_mc_cta(ctx->stream, a, k, ligs->cta_smem[k]));
+        ctx->launches += 1;
+    }
+    if (top_k > 0) {
+        TopkLaunch tk;
+        memset(&tk, 0, sizeof(tk));
+        tk.hdr = ligs->hdr; tk.e_best = base.e_best; tk.pose_best = base.pose_best;
+        tk.n_lig = L; tk.n_chains = n_chains; tk.pose_stride = pose_stride; tk.top_k = top_k; tk.w_tor = params->w_tor;
+        tk.atom_f4 = ligs->atom_f4; tk.lane_frags = ligs->lane_frags; tk.cluster_rmsd = 0.f;
+        tk.max_atoms = ligs->max_atoms; tk.max_tor = ligs->max_tor;
+        tk.out_energy = out_energy; tk.out_pose = out_pose; tk.out_chain = out_chain;
+        CK(launch_topk(ctx->stream, tk));
+        ctx->launches += 1;
+    }
     return TRIDSK_OK;
 }
