@@ -929,7 +929,7 @@ extern "C" int tridsk_load_mdn(tridsk_ctx* ctx, tridsk_ligands* ligs, const trid
     for (int i = 0; i < m->n_res; ++i) if (m->res_off[i + 1] < m->res_off[i] || m->res_off[0] != 0) return fail(ctx, TRIDSK_EINVAL, "res_off must start at 0 and be non-decreasing");
     const int L = ligs->n_lig, n_at = m->res_off[m->n_res];
     if (L == 0) return TRIDSK_OK;
-    const int K4 = (m->K + 3) / 4 * 4;
+    const int K4 = mdn_slot_f4(m->K);
     std::vector<long long> off(2 * (size_t)L);             // [0, L): blocks of the packed records; [L, 2L): blocks of the caller's arrays
     long long total = 0, total_p = 0;
     for (int l = 0; l < L; ++l) {
@@ -1189,10 +1189,11 @@ extern "C" int tridsk_score_direct(tridsk_ctx* ctx, const float* rec_xyz, const 
 // shared memory is the group's largest need, the groups run concurrently as parallel branches of the CUDA graph, and
 // inside a group the costliest ligands go first (short tail).
 static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_refine) {
-    const long long key = ((long long)n_chains << 8) | (n_refine > 1 ? 1 : 0) | (ctx->kernel == 4 ? 2 : 0);
+    const long long key = ((long long)n_chains << 8) | (n_refine > 1 ? 1 : 0) | (ctx->kernel == 4 ? 2 : 0) | (lg->mdn.n_res > 0 ? 4 : 0);
     if (lg->lane_plan_key == key) return TRIDSK_OK;
     const int L = lg->n_lig;
     const int cmax = std::min(128, (n_chains + 31) / 32 * 32);
+    const int wmax = lg->mdn.n_res > 0 ? 8 : 12;               // resident warps per SM the register budget allows (mc_lane.cu)
     struct Ent { int cls; long long cost; int lig; size_t need; };
     const bool use_tm = ctx->kernel == 4;
     std::vector<Ent> ent(L);
@@ -1201,7 +1202,7 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
         const size_t topo = lane_topo_bytes(h.n, h.T, h.ls_len, h.n_rec);
         const size_t per_chain = 4 * (size_t)lane_chain_slots(h.n, h.T, h.max_depth, n_refine);
         // chains per CTA: the multiple of a warp that keeps the most warps resident per SM (ties: the larger CTA, which
-        // stages the topology fewer times); 168 registers per thread allow 12 warps per SM
+        // stages the topology fewer times); 168 registers per thread allow 12 warps per SM (255 with E_MDN: 8)
         int c = 0, r = 0;
         size_t need = 0;
         long long best_live = -1;
@@ -1209,7 +1210,7 @@ static int lane_plan(tridsk_ctx* ctx, tridsk_ligands* lg, int n_chains, int n_re
             const size_t nd = (topo + per_chain * cc + 15) / 16 * 16;
             if (nd > TRIDSK_SMEM_MAX_CTA) continue;
             int rr = (int)(TRIDSK_SMEM_PER_SM / ((nd + 1023) / 1024 * 1024 + TRIDSK_SMEM_RESERVED));   // allocated in KB units
-            rr = std::max(1, std::min(std::min(rr, 32), 12 * 32 / cc));
+            rr = std::max(1, std::min(std::min(rr, 32), wmax * 32 / cc));
             // live chains resident per SM: a ligand's last CTA may be partly empty (128 chains in CTAs of 96 = 96 + 32)
             const int cpl_ = (n_chains + cc - 1) / cc;
             const long long live = (long long)rr * n_chains / cpl_;

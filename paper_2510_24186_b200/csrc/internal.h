@@ -40,16 +40,22 @@ struct DGrid {
 };
 
 // The mixture-density term (mdn.cuh, O15) attached to a ligand batch; n_res == 0: absent.
+// Parameters: a (residue, atom) pair owns a SLOT of blocks; a block holds up to ten components as {a, mu, nk2} x 10 (30 floats
+// + 2 unused = 128 bytes); the last block is cut to whole 32-byte chunks.  K = 10: one 128-byte cache line per pair.
+__host__ __device__ static inline int mdn_slot_f4(int K) {          // float4 units per slot
+    const int nb = (K + 9) / 10, kl = K - 10 * (nb - 1);
+    return 2 * (4 * (nb - 1) + (3 * kl + 7) / 8);
+}
 struct MdnDev {
-    int n_res, K, K4;             // K4 = K rounded up to a multiple of 4: records per (residue, atom) in par
+    int n_res, K, K4;             // K4 = mdn_slot_f4(K): float4 units per (residue, atom) slot in par
     const float4* sph;            // [n_res] bounding sphere of a residue: centre, (radius + d_cut)^2
     const int* res_off;           // [n_res + 1] into rec
     const float4* rec;            // residue atoms {x, y, z, 0}
-    const float4* par;            // packed parameters {a, mu, nk2, 1/sigma^2}, ligand-major, [n_res][n][K] per ligand, INTERNAL atom order; [n_res][n][K4]
+    const float4* par;            // packed parameter slots, ligand-major, [n_res][n][K4] per ligand, INTERNAL atom order
     const long long* lig_off;     // [n_lig] start of a ligand's block in par (float4 units)
     float d_cut;
     // cell list: a uniform grid over the residues' bounding box grown by d_cut; cell c holds, as ONE contiguous stream
-    // sorted by (residue, atom index), every receptor atom {x, y, z, residue id} within d_cut + half a cell diagonal of the
+    // sorted by (residue, atom index), every receptor atom {x, y, z, w} within d_cut + half a cell diagonal of the
     // cell's centre (runs padded to an even number of entries).  For a point of the cell, a residue's minimum over the listed atoms equals its true minimum distance
     // whenever that is below d_cut (the arg-min atom is then listed), and is >= d_cut otherwise.
     float glo[3], inv_cell;

@@ -796,6 +796,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
 // MINB = resident 128-thread CTAs per SM the register budget must allow (3: 168 registers, 2: 255): the host picks 255 for
 // the size buckets whose shared-memory need keeps at most 8 warps per SM resident anyway, 168 (12 warps) for the rest --
 // measured: 12 warps at 168 registers beat 16 warps at 128 (C5 1885 -> 1824 ms), 8 warps at 255 do not (1917 ms).
+// With the mixture-density term: always 255 (8 warps) -- at 168 the term's prefetch buffers spill (M3 4.9 s against 3.6 s).
 template <int MINB, int C, bool MDN>
 __global__ void __launch_bounds__(128, MINB) mc_lane_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char lane_smem[];
@@ -887,10 +888,10 @@ cudaError_t mc_lane_prepare(size_t max_smem_bytes) {
     if (e == cudaSuccess) e = lane_prepare_one<2, 64, false>(max_smem_bytes);
     if (e == cudaSuccess) e = lane_prepare_one<2, 96, false>(max_smem_bytes);
     if (e == cudaSuccess) e = lane_prepare_one<2, 128, false>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<3, 32, true>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<3, 64, true>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<3, 96, true>(max_smem_bytes);
-    if (e == cudaSuccess) e = lane_prepare_one<3, 128, true>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 32, true>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 64, true>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 96, true>(max_smem_bytes);
+    if (e == cudaSuccess) e = lane_prepare_one<2, 128, true>(max_smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(score_lane_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(score_lane_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_lane_tm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem_bytes - 1024);   // it has 16 static bytes
@@ -912,7 +913,7 @@ cudaError_t launch_mc_lane(cudaStream_t s, const McLaunch& a, int chains_per_cta
     const long long blocks = (long long)a.n_list * cpl;
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL || chains_per_cta < 32 || chains_per_cta > 128 || (chains_per_cta & 31)) return cudaErrorInvalidValue;
-    if (a.mdn.n_res > 0) lane_launch_c<3, true>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);   // one register class with the term
+    if (a.mdn.n_res > 0) lane_launch_c<2, true>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);   // with the term: 255 registers (mdn_atom's one-ahead pipeline holds two parameter blocks)
     else if (minb == 2) lane_launch_c<2, false>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);
     else lane_launch_c<3, false>(s, a, (unsigned)blocks, chains_per_cta, smem_bytes);
     return cudaGetLastError();

@@ -1,6 +1,6 @@
 // mdn.cu -- device-side preparation of the mixture-density term (tridsk_load_mdn; O15): bounding spheres of the residues
 // and the packed parameter records.  Every value that the term's arithmetic uses is formed here, on the device, from the
-// caller's plain (pi, mu, sigma): a = w_mdn pi / (sigma sqrt(2 pi)), nk2 = -log2(e) / (2 sigma^2), 1 / sigma^2 (mdn.cuh).
+// caller's plain (pi, mu, sigma): a = w_mdn pi / (sigma sqrt(2 pi)), nk2 = -log2(e) / (2 sigma^2) (mdn.cuh).
 #include "internal.h"
 
 // One thread per residue: copy its atoms into float4 records and take the bounding sphere about their centroid.
@@ -26,30 +26,36 @@ __global__ void mdn_sphere_kernel(const float* __restrict__ res_xyz, const int* 
     sph[i] = make_float4(cx, cy, cz, reach > 0.f ? reach * reach : -1.f);
 }
 
-// One CTA per ligand: records [n_res][n][K4] (K4 = K rounded up to a multiple of 4, padded with zero-amplitude records) in
-// the library's INTERNAL atom order from the caller's arrays [n_res][n][K] in the caller's atom order (atom_i carries the
-// original index of an internal atom).  lig_off / in_off: start of the ligand's block in par / in the caller's arrays.
+// One CTA per ligand: parameter slots [n_res][n][K4 float4] (internal.h: blocks of ten components {a, mu, nk2}, unused floats
+// zero) in the library's INTERNAL atom order from the caller's arrays [n_res][n][K] in the caller's atom order (atom_i carries
+// the original index of an internal atom).  lig_off / in_off: start of the ligand's block in par / in the caller's arrays.
 __global__ void mdn_pack_kernel(const LigHdr* __restrict__ hdr, const int* __restrict__ atom_i, int n_res, int K,
                                 const long long* __restrict__ lig_off, const long long* __restrict__ in_off,
                                 const float* __restrict__ pi, const float* __restrict__ mu,
                                 const float* __restrict__ sigma, float w_mdn, float4* __restrict__ par, int* __restrict__ bad) {
     const int lig = blockIdx.x;
     const LigHdr h = hdr[lig];
-    const int K4 = (K + 3) / 4 * 4;
+    const int K4 = mdn_slot_f4(K);
     const long long base = lig_off[lig], ibase = in_off[lig];
     const long long total = (long long)n_res * h.n * K4;
     for (long long e = threadIdx.x; e < total; e += blockDim.x) {
-        const int k = (int)(e % K4);
+        const int f4 = (int)(e % K4);
         const long long ip = e / K4;
         const int p = (int)(ip % h.n);
         const long long i = ip / h.n;
-        if (k >= K) { par[base + e] = make_float4(0.f, 0.f, 0.f, 0.f); continue; }
         const int orig = (atom_i[h.atom_off + p] >> 16) & 0xff;
-        const long long src = ibase + (i * h.n + orig) * K + k;
-        const float sg = sigma[src], w = pi[src], m = mu[src];
-        if (!(sg > 0.f) || !isfinite(sg) || !isfinite(w) || !isfinite(m)) { *bad = 1; par[base + e] = make_float4(0.f, 0.f, 0.f, 0.f); continue; }
-        const float inv_s2 = 1.f / (sg * sg);
-        par[base + e] = make_float4(w_mdn * w / (sg * 2.5066282746310002f), m, -0.7213475204444817f * inv_s2, inv_s2);
+        float v[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int f = 4 * f4 + c, w = f & 31, k = 10 * (f >> 5) + w / 3, fld = w % 3;
+            v[c] = 0.f;
+            if (w >= 30 || k >= K) continue;
+            const long long src = ibase + (i * h.n + orig) * K + k;
+            const float sg = sigma[src], wt = pi[src], m = mu[src];
+            if (!(sg > 0.f) || !isfinite(sg) || !isfinite(wt) || !isfinite(m)) { *bad = 1; continue; }
+            v[c] = fld == 0 ? w_mdn * wt / (sg * 2.5066282746310002f) : fld == 1 ? m : -0.7213475204444817f / (sg * sg);
+        }
+        par[base + e] = make_float4(v[0], v[1], v[2], v[3]);
     }
 }
 
@@ -67,8 +73,8 @@ cudaError_t launch_mdn_pack(cudaStream_t s, const LigHdr* hdr, const int* atom_i
 }
 
 // One thread per cell of the cell list: the receptor atoms within d_cut + half a cell diagonal of the cell's centre, in
-// (residue, atom index) order; the first entry of a residue's run carries residue id | run length << 16 in w, the others
-// the residue id; runs are padded to an even length (32-byte alignment for 256-bit loads).  fill = false: counts[c] = how many; fill = true: written to cell_at[off[c] ..].
+// (residue, atom index) order; the first entry of a residue's run carries residue id | run length << 16 in w, the second
+// the same header of the NEXT run of the cell (-1: none), the others the residue id; runs are padded to an even length (32-byte alignment for 256-bit loads).  fill = false: counts[c] = how many; fill = true: written to cell_at[off[c] ..].
 __global__ void mdn_cell_kernel(MdnDev M, float cell, bool fill, int* __restrict__ counts_or_off, float4* __restrict__ cell_at) {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     const int ncell = M.nc[0] * M.nc[1] * M.nc[2];
@@ -77,7 +83,7 @@ __global__ void mdn_cell_kernel(MdnDev M, float cell, bool fill, int* __restrict
     const float x = M.glo[0] + cell * ((float)ix + 0.5f), y = M.glo[1] + cell * ((float)iy + 0.5f), z = M.glo[2] + cell * ((float)iz + 0.5f);
     const float half_diag = 0.8660254f * cell;
     const float reach = M.d_cut + half_diag * 1.001f + 1e-3f, reach2 = reach * reach;
-    int n = 0;
+    int n = 0, prev = -1;
     float4* dst = fill ? cell_at + counts_or_off[c] : nullptr;
     for (int i = 0; i < M.n_res; ++i) {
         const float4 s = M.sph[i];
@@ -98,7 +104,13 @@ __global__ void mdn_cell_kernel(MdnDev M, float cell, bool fill, int* __restrict
             if (fill) dst[n] = make_float4(1e18f, 1e18f, 1e18f, __int_as_float(i));
             ++n;
         }
-        if (fill && n > first) dst[first].w = __int_as_float(i | ((n - first) << 16));
+        if (fill && n > first) {
+            const int hdr = i | ((n - first) << 16);
+            dst[first].w = __int_as_float(hdr);
+            dst[first + 1].w = __int_as_float(-1);                  // the next run's header goes here (-1: this is the last run)
+            if (prev >= 0) dst[prev + 1].w = __int_as_float(hdr);
+            prev = first;
+        }
     }
     if (!fill) counts_or_off[c] = n;
 }

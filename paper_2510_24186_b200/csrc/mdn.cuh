@@ -9,53 +9,66 @@
 #pragma once
 #include "internal.h"
 
-// One ligand atom (internal index p of a ligand with n atoms) at (x, y, z) against residues i0, i0 + istep, ...
-// par = the ligand's parameter block [n_res][n][K] of {a, mu, nk2, 1/sigma^2}, a = w_mdn pi / (sigma sqrt(2 pi)),
-// nk2 = -log2(e) / (2 sigma^2):  N = a 2^(nk2 (d - mu)^2),  dN/dd = -N (d - mu) / sigma^2.
-// e += w_mdn * (this atom's share of E_MDN); grad: (gx, gy, gz) += its gradient.
-// two adjacent 16-byte records by one 256-bit load (p 32-byte aligned)
-__device__ __forceinline__ void mdn_ldg2(const float4* p, float4& a, float4& b) {
+// Parameter layout (internal.h, mdn_slot_f4): a (residue, atom) pair owns one SLOT of blocks; a block holds up to ten
+// components as {a, mu, nk2} x 10 (30 floats + 2 unused = 128 bytes, one cache line), a = w_mdn pi / (sigma sqrt(2 pi)),
+// nk2 = -log2(e) / (2 sigma^2):  N = a 2^(nk2 (d - mu)^2),  dN/dd = -N (d - mu) / sigma^2 = 2 ln 2 N (d - mu) nk2.
+// The last block is cut to whole 32-byte chunks; unused components have zero amplitude.  K <= 10 (the paper's mixture
+// sizes): one block, fetched whole by the caller one residue AHEAD of its use.
+__device__ __forceinline__ void mdn_ldg2(const float4* p, float4& a, float4& b) {     // two adjacent 16-byte records, p 32-byte aligned
     asm("ld.global.nc.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
         : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w) : "l"(p));
 }
+__device__ __forceinline__ void mdn_ldg8(const float4* p, float* v) {                  // one 32-byte chunk
+    asm("ld.global.nc.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+        : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]) : "l"(p));
+}
+// the first nch (1..4, warp-uniform) chunks of the block at q
+__device__ __forceinline__ void mdn_load_block(const float4* q, int nch, float v[32]) {
+    mdn_ldg8(q, v);
+    if (nch > 1) mdn_ldg8(q + 2, v + 8);
+    if (nch > 2) mdn_ldg8(q + 4, v + 16);
+    if (nch > 3) mdn_ldg8(q + 6, v + 24);
+}
+// the components that lie wholly inside the first nch chunks of a block: e -= sum N, dn += sum N (d - mu) nk2
+__device__ __forceinline__ void mdn_block(const float v[32], int nch, float d, float& e, float& dn) {
+#pragma unroll
+    for (int j = 0; j < 10; ++j) {
+        if (3 * j + 2 < 8 * nch) {
+            const float t = d - v[3 * j + 1];
+            float N;
+            { const float arg = v[3 * j + 2] * t * t; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(N) : "f"(arg)); }
+            N *= v[3 * j];
+            e -= N;
+            dn = fmaf(N * t, v[3 * j + 2], dn);
+        }
+    }
+}
 
-// One (residue, atom) pair whose minimum squared distance best2 is inside the cut-off: the K mixture components.  The
-// records are padded to a multiple of four per pair (M.K4; the padding has zero amplitude) and fetched four at a time by two
-// 256-bit loads; the first four (c0) were requested by the caller before it searched the residue's atoms.
-__device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __restrict__ q, const float4 c0[8], float best2,
+// One (residue, atom) pair whose minimum squared distance best2 is inside the cut-off: the K mixture components.  c0 = the
+// slot's first block (requested by the caller one residue ahead); further blocks (K > 10) are fetched here.
+__device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __restrict__ q, const float c0[32], float best2,
                                            float bx, float by, float bz, bool grad, float& e, float& gx, float& gy, float& gz) {
     float rinv;
     { const float b = fmaxf(best2, 1e-12f); asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(b)); }
     const float d = best2 * rinv;
-    float de = 0.f;
-    float4 c[4] = {c0[0], c0[1], c0[2], c0[3]};
-    for (int k0 = 0; k0 < M.K4; k0 += 4) {
-        float4 cn[4];
-        const bool more = k0 + 4 < M.K4;
-        if (more) {
-            if (k0 == 0) { cn[0] = c0[4]; cn[1] = c0[5]; cn[2] = c0[6]; cn[3] = c0[7]; }      // the second four came with the first
-            else { mdn_ldg2(q + k0 + 4, cn[0], cn[1]); mdn_ldg2(q + k0 + 6, cn[2], cn[3]); }
-        }
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const float t = d - c[j].y;
-            float N;
-            { const float arg = c[j].z * t * t; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(N) : "f"(arg)); }
-            N *= c[j].x;
-            e -= N;
-            de = fmaf(N * t, c[j].w, de);
-        }
-        if (more) {
-#pragma unroll
-            for (int j = 0; j < 4; ++j) c[j] = cn[j];
-        }
+    float dn = 0.f;
+    const int nch0 = min(M.K4 >> 1, 4);
+    mdn_block(c0, nch0, d, e, dn);
+    for (int c = 4; 2 * c < M.K4; c += 4) {                     // K > 10
+        float v[32];
+        const int nch = min((M.K4 >> 1) - c, 4);
+        mdn_load_block(q + 2 * c, nch, v);
+        mdn_block(v, nch, d, e, dn);
     }
     if (grad) {
-        const float sc = de * rinv;
+        const float sc = -1.3862943611198906f * dn * rinv;      // de/dd / d,  1 / sigma^2 = -2 ln 2 nk2
         gx = fmaf(sc, bx, gx); gy = fmaf(sc, by, gy); gz = fmaf(sc, bz, gz);
     }
 }
 
+// One ligand atom (internal index p of a ligand with n atoms) at (x, y, z) against residues i0, i0 + istep, ...
+// par = the ligand's parameter block [n_res][n] of slots (M.K4 float4 each).
+// e += w_mdn * (this atom's share of E_MDN); grad: (gx, gy, gz) += its gradient.
 __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restrict__ par, int n, int p, float x, float y, float z,
                                          int i0, int istep, bool grad, float& e, float& gx, float& gy, float& gz) {
     // the cell of the atom streams every receptor atom it can be within d_cut of, sorted by residue (outside the grid: none)
@@ -66,26 +79,33 @@ __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restri
     const int e0 = __ldg(M.cell_off + cell), e1 = __ldg(M.cell_off + cell + 1);
     if (e0 >= e1) return;
     const float cut2 = M.d_cut * M.d_cut;
-    // Residue by residue: the first entry of a run holds residue id | run length << 16; runs are padded to an even number of
-    // entries (a padding entry lies 1e18 away) so that every run starts 32-byte aligned and is read two entries per 256-bit
-    // load.  Lanes of a warp sit in different cells, so their runs differ in length; the short inner loop diverges, the costly
-    // mixture evaluation after it is reached by all lanes together once per residue.  The loads are L2 round trips: the first
-    // four parameter records of the residue and the first entries of the NEXT run are requested before the run is searched.
-    int ord = 0;
-    float4 a, a2;
+    const int nch0 = min(M.K4 >> 1, 4);
+    // Residue by residue.  The FIRST entry of a run holds residue id | run length << 16 in w, the SECOND the same header of the
+    // NEXT run of the cell (-1: none); runs are padded to an even number of entries (a padding entry lies 1e18 away), so every
+    // run starts 32-byte aligned and is read two entries per 256-bit load.  Everything a run needs -- its entries and the first
+    // parameter block of its residue -- is requested while the run BEFORE it is being worked on: the loop is a one-ahead
+    // software pipeline over L2 round trips.  Lanes of a warp sit in different cells, so their runs differ in length; the short
+    // inner loop diverges, the costly mixture evaluation after it is reached by all lanes together once per residue.
+    // The loop body is written once and instantiated twice with the two buffer sets swapped, so that no register copy touches
+    // a load that is still in flight.
+    int ord = 0, en = e0;
+    float4 a, a2, b, b2;
+    float cur[32], nxt[32];
     mdn_ldg2(M.cell_at + e0, a, a2);
-    for (int en = e0; en < e1; ++ord) {
-        const int hdr = __float_as_int(a.w), i = hdr & 0xffff, cnt = hdr >> 16;      // cnt is even
+    int hdr = __float_as_int(a.w);
+    mdn_load_block(par + ((size_t)(hdr & 0xffff) * n + p) * M.K4, nch0, cur);
+    auto step = [&](const float4& ra, const float4& ra2, const float (&rc)[32], float4& na, float4& na2, float (&nc)[32]) {
+        const int i = hdr & 0xffff, cnt = hdr >> 16;             // cnt is even
         const float4* q = par + ((size_t)i * n + p) * M.K4;
-        float4 c0[8];                                         // K4 >= 8 ? eight records : four (the rest of c0 is unused then)
-        mdn_ldg2(q, c0[0], c0[1]); mdn_ldg2(q + 2, c0[2], c0[3]);
-        if (M.K4 > 4) { mdn_ldg2(q + 4, c0[4], c0[5]); mdn_ldg2(q + 6, c0[6], c0[7]); }
-        float4 an, an2;
-        mdn_ldg2(M.cell_at + min(en + cnt, e1 - 2), an, an2);
-        float bx = x - a.x, by = y - a.y, bz = z - a.z;
+        const int nh = __float_as_int(ra2.w);                    // the next run's header
+        if (nh >= 0) {
+            mdn_ldg2(M.cell_at + en + cnt, na, na2);
+            mdn_load_block(par + ((size_t)(nh & 0xffff) * n + p) * M.K4, nch0, nc);
+        }
+        float bx = x - ra.x, by = y - ra.y, bz = z - ra.z;
         float best2 = bx * bx + by * by + bz * bz;
         {
-            const float dx = x - a2.x, dy = y - a2.y, dz = z - a2.z;
+            const float dx = x - ra2.x, dy = y - ra2.y, dz = z - ra2.z;
             const float d2 = dx * dx + dy * dy + dz * dz;
             if (d2 < best2) { best2 = d2; bx = dx; by = dy; bz = dz; }
         }
@@ -99,8 +119,13 @@ __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restri
             d2 = dx * dx + dy * dy + dz * dz;
             if (d2 < best2) { best2 = d2; bx = dx; by = dy; bz = dz; }
         }
-        en += cnt;
-        if (best2 < cut2 && ord % istep == i0) mdn_finish(M, q, c0, best2, bx, by, bz, grad, e, gx, gy, gz);
-        a = an; a2 = an2;
+        if (best2 < cut2 && ord % istep == i0) mdn_finish(M, q, rc, best2, bx, by, bz, grad, e, gx, gy, gz);
+        en += cnt; hdr = nh; ++ord;
+    };
+    for (;;) {
+        step(a, a2, cur, b, b2, nxt);
+        if (en >= e1) break;
+        step(b, b2, nxt, a, a2, cur);
+        if (en >= e1) break;
     }
 }
