@@ -986,12 +986,12 @@ extern "C" int tridsk_load_mdn(tridsk_ctx* ctx, tridsk_ligands* ligs, const trid
         for (int r = 0; r < n_at; ++r)
             for (int c = 0; c < 3; ++c) { lo[c] = std::min(lo[c], m->res_xyz[3 * r + c]); hi[c] = std::max(hi[c], m->res_xyz[3 * r + c]); }
         if (n_at == 0) for (int c = 0; c < 3; ++c) lo[c] = hi[c] = 0.f;
-        float cell = 1.5f;
+        float cell = 0.6f;                                  // measured on M3: 1.5 A 3.64 s, 1.0 A 2.95 s, 0.75 A 2.61 s, 0.6 A 2.44 s, 0.5 A 2.38 s
         long long ncell = 0;
-        for (;; cell *= 1.25f) {                            // at most ~256k cells
+        for (;; cell *= 1.25f) {                            // at most ~1M cells
             ncell = 1;
             for (int c = 0; c < 3; ++c) { M.nc[c] = std::max(1, (int)std::ceil((hi[c] - lo[c] + 2.f * m->d_cut) / cell)); ncell *= M.nc[c]; }
-            if (ncell <= 262144) break;
+            if (ncell <= 1048576) break;
         }
         for (int c = 0; c < 3; ++c) M.glo[c] = lo[c] - m->d_cut;
         M.inv_cell = 1.f / cell;
