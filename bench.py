@@ -57,7 +57,7 @@ def work_of(n_atoms, n_tor, n_pairs, n_chains, n_steps, n_refine, mdn=None, dire
         flop_g = flop_g + n * hits * (8 * size + 12 * K + 8)
         flop_e = flop_e + n * hits * (8 * size + 8 * K)
         xu_g, xu_e = xu_g + n * hits * (K + 1), xu_e + n * hits * (K + 1)
-        bytes_eval = bytes_eval + n * hits * (16 * K + 16 * size)
+        bytes_eval = bytes_eval + n * hits * (12 * K + 16 * size)   # three fp32 parameters per component, 16-byte atom records
     if direct:                                 # receptor term by direct sums: pairs within the range per atom instead of the trilinear lookup
         ppa = direct["pairs_per_atom"]
         flop_g = flop_g + n * (28 * ppa - 80)

@@ -604,9 +604,10 @@ __device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const Ct
 
 // ------------------------------------------------------------------ the fused MC kernel, one CTA per chain
 // Record instance: 128 threads, registers for 3 resident CTAs per SM (with 4 x 128 registers, C2 goes 6.0 -> 6.3 ms).  Dense
-// instance: 64 threads and 128 registers, EIGHT chains resident per SM (6 with the mixture-density term, which spills at 128).
+// instance: 64 threads and 128 registers, EIGHT chains resident per SM (with the mixture-density term: 255 registers, four chains --
+// an 80-atom dock under the full score 490 -> 345 ms; the record instance with the term is faster at 168 than at 255: 60.5 / 71.3 ms).
 template <bool MDN, int ROUNDS>
-__global__ void __launch_bounds__(ROUNDS ? 64 : 128, ROUNDS ? (MDN ? 6 : 8) : 3) mc_cta_kernel(const McLaunch a) {
+__global__ void __launch_bounds__(ROUNDS ? 64 : 128, ROUNDS ? (MDN ? 4 : 8) : 3) mc_cta_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lig = a.lig_list[blockIdx.x / a.n_chains];
