@@ -855,6 +855,28 @@ def test_mdn_score_grad_matches_oracle(orc, eng, gp, system):
     ligs.free()
 
 
+@pytest.mark.parametrize("K", [1, 3, 8, 13, 23])
+def test_mdn_mixture_sizes_across_the_parameter_blocks(orc, eng, gp, system, K):
+    """Mixture sizes on every shape of the packed parameter slot (blocks of ten components, the last cut to 1..4 chunks of 32
+    bytes; K > 10 takes more than one block): energy and gradient against the oracle."""
+    S = system
+    ids = [1, 6]
+    b, ligs, Ls = _mdn_system(orc, eng, S, ids, K=K, seed=500 + K)
+    li = np.repeat(np.arange(len(ids), dtype=np.int32), 6)
+    poses = synth.random_poses(b, li, S["rec"], seed=21, spread=0.6)
+    e, g, _ = eng.score_grad(S["g_grid"], ligs, gp, li, poses)
+    n_with = 0
+    for i in range(len(li)):
+        L = Ls[li[i]]
+        eo, go, xo, _ = orc.score_grad(S["p"], S["ty"], S["G"], L, poses[i, :7 + L.T].astype(np.float64))
+        n_with += orc.mdn_energy(L.mdn.res_xyz, L.mdn.res_off, L.mdn.pi, L.mdn.mu, L.mdn.sigma, xo)[0] < -1e-3
+        assert close(e[i], eo), (K, i, e[i], eo)
+        sc = np.abs(go).max()
+        assert close(g[i, :6 + L.T], go, scale=sc), (K, i, worst(g[i, :6 + L.T], go, scale=sc))
+    assert n_with > 0.7 * len(li)
+    ligs.free()
+
+
 def test_mdn_teacher_forced_steps_match_oracle(orc, eng, gp, system):
     """Chains sampled under the full score: teacher-forced MC steps against orc_mc_step with the term attached."""
     from paper_2510_24186_b200 import split_state
