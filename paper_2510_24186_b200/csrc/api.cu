@@ -1356,9 +1356,9 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         if (std::max(ligs->cta_smem[0], ligs->cta_smem[1]) > TRIDSK_SMEM_MAX_CTA)
             return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
     }
-    if (o.receptor_direct) {                                        // direct pair sums: the warp-per-chain kernel carries that path
+    if (o.receptor_direct) {                                        // direct pair sums: the CTA- and the warp-per-chain kernels carry that path
         if (!grid->rd.atoms) return fail(ctx, TRIDSK_EINVAL, "receptor_direct needs tridsk_grid_attach_receptor on this grid");
-        mode = 1;
+        if (mode != 3 || ligs->mdn.n_res > 0) mode = 1;             // (the CTA instances with direct sums leave out E_MDN)
         base.rec = grid->rd;
     }
     const bool lane = mode == 2 || mode == 4;

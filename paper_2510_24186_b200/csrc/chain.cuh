@@ -298,8 +298,9 @@ __device__ __forceinline__ float pair_energy(const DParams& P, float d2, float d
 // The paper's own evaluation (P:103-125, P:353 item 4): e(s_r, t, |x - r_r|) summed over the receptor atoms within the pair
 // function's range -- the 27 cells around the atom's cell, cells and atoms in a fixed order.  No interpolation, no wall.
 template <bool GRAD>
+// i0, istep: the caller's share of every cell's atoms (the CTA mapping spreads an atom's partners over its lanes).
 __device__ __forceinline__ float rec_direct(const RecDev& R, const DParams& P, int type, float x, float y, float z,
-                                            float& gx, float& gy, float& gz) {
+                                            float& gx, float& gy, float& gz, int i0 = 0, int istep = 1) {
     const float rt = __ldg(R.radius + type);
     const unsigned char role_t = __ldg(R.role + type);
     const int cx = (int)floorf((x - R.lo[0]) * R.inv_cell), cy = (int)floorf((y - R.lo[1]) * R.inv_cell), cz = (int)floorf((z - R.lo[2]) * R.inv_cell);
@@ -309,7 +310,7 @@ __device__ __forceinline__ float rec_direct(const RecDev& R, const DParams& P, i
             for (int kx = max(cx - 1, 0); kx <= min(cx + 1, R.nc[0] - 1); ++kx) {
                 const int c = (kz * R.nc[1] + ky) * R.nc[0] + kx;
                 const int r1 = __ldg(R.cell_off + c + 1);
-                for (int r = __ldg(R.cell_off + c); r < r1; ++r) {
+                for (int r = __ldg(R.cell_off + c) + i0; r < r1; r += istep) {
                     const float4 a = __ldg(R.atoms + r);
                     const float dx = x - a.x, dy = y - a.y, dz = z - a.z;
                     const float d2 = dx * dx + dy * dy + dz * dz;

@@ -193,7 +193,7 @@ struct McLaunch {
     int lane_region, tm_cols;     // tensor-memory lane kernel: shared-memory bytes per warp, TMEM columns per CTA
     int lane_minb;                // shared-memory lane kernel: register budget class (launch_bounds min blocks)
     MdnDev mdn;                   // n_res == 0: no mixture-density term
-    RecDev rec;                   // atoms != nullptr: receptor term by direct pair sums (warp-per-chain mapping only)
+    RecDev rec;                   // atoms != nullptr: receptor term by direct pair sums (warp- and CTA-per-chain mappings)
 };
 
 struct ScoreLaunch {

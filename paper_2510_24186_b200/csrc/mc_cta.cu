@@ -326,9 +326,11 @@ __device__ __forceinline__ void cta_reverse(const CtaTopo& S, const CtaFrag& F, 
 //      on lane g (O9); x, y, z = this thread's atom (valid when `active`).
 // MDN: the mixture-density term (mdn.cuh); the lanes of an atom share its residues (lane `part` takes residues part,
 // part + lpa, ...), their shares join the pair force / the energy sums before the fixed-order reductions.
-template <bool GRAD, bool ENERGY, bool MDN>
+// DIRECT: the receptor term by direct pair sums over the receptor atoms (rec_direct, chain.cuh) instead of the grid lookup; the
+// lanes of an atom share the atoms of every cell, their shares join the pair force like the mixture-density term's.
+template <bool GRAD, bool ENERGY, bool MDN, bool DIRECT>
 __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
-                                         const MdnDev& M, const float4* __restrict__ mdn_par,
+                                         const MdnDev& M, const float4* __restrict__ mdn_par, const RecDev& RD,
                                          int max_depth, const float t[3], const float q[4], float theta,
                                          int atom, int part, bool active, float& x, float& y, float& z,
                                          float& e_inter, float& e_intra, float g6[6], float& gth) {
@@ -355,8 +357,10 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     float4 glo = make_float4(0.f, 0.f, 0.f, 0.f), ghi = glo;
     if (lead) {
         S.X[atom] = x; S.X[n + atom] = y; S.X[2 * n + atom] = z;
-        cell = grid_locate(G, m & 0xff, x, y, z);
-        glo = __ldg(cell.p); ghi = __ldg(cell.p + 1);
+        if (!DIRECT) {
+            cell = grid_locate(G, m & 0xff, x, y, z);
+            glo = __ldg(cell.p); ghi = __ldg(cell.p + 1);
+        }
     }
     __syncthreads();
 
@@ -402,7 +406,12 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     }
     // ---- a4 receptor term of this thread's atom (the gathers were issued before the barrier)
     float ei = 0.f, gx = 0.f, gy = 0.f, gz = 0.f;
-    if (lead) ei = grid_blend<GRAD>(G, P.k_wall, cell, glo, ghi, gx, gy, gz);
+    if (!DIRECT && lead) ei = grid_blend<GRAD>(G, P.k_wall, cell, glo, ghi, gx, gy, gz);
+    if (DIRECT && active) {
+        float mx = 0.f, my = 0.f, mz = 0.f;
+        ei += rec_direct<GRAD>(RD, P, m & 0xff, x, y, z, mx, my, mz, part, S.lpa);
+        if (GRAD) { fx = fmaf(mx, K.inv_kappa, fx); fy = fmaf(my, K.inv_kappa, fy); fz = fmaf(mz, K.inv_kappa, fz); }
+    }
     if (MDN && active) {
         float mx = 0.f, my = 0.f, mz = 0.f;
         mdn_atom(M, mdn_par, n, atom, x, y, z, part, S.lpa, GRAD, ei, mx, my, mz);
@@ -444,9 +453,9 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
 // chunk's force is the sum of the warps' partials -- fixed order, after a barrier.  GRAD: all partners (both ends of every
 // pair); energy only: the partners b > l.  A last chunk of at most 16 atoms is held twice, by the two half-warps, which split
 // the partners between them.  x0, y0, z0: the coordinates of atom threadIdx.x.
-template <bool GRAD, bool ENERGY, bool MDN, int NW>
+template <bool GRAD, bool ENERGY, bool MDN, bool DIRECT, int NW>
 __device__ __forceinline__ void cta_eval_dense(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
-                                               const MdnDev& M, const float4* __restrict__ mdn_par,
+                                               const MdnDev& M, const float4* __restrict__ mdn_par, const RecDev& RD,
                                                int max_depth, const float t[3], const float q[4], float theta,
                                                float& x0, float& y0, float& z0,
                                                float& e_inter, float& e_intra, float g6[6], float& gth) {
@@ -479,8 +488,10 @@ __device__ __forceinline__ void cta_eval_dense(const CtaTopo& S, const DGrid& G,
         glo[k] = make_float4(0.f, 0.f, 0.f, 0.f); ghi[k] = glo[k];
         if (act[k]) {
             S.X4[atom] = make_float4(x[k], y[k], z[k], __int_as_float(m[k] & 0xff));
-            cell[k] = grid_locate(G, m[k] & 0xff, x[k], y[k], z[k]);
-            glo[k] = __ldg(cell[k].p); ghi[k] = __ldg(cell[k].p + 1);
+            if (!DIRECT) {
+                cell[k] = grid_locate(G, m[k] & 0xff, x[k], y[k], z[k]);
+                glo[k] = __ldg(cell[k].p); ghi[k] = __ldg(cell[k].p + 1);
+            }
         }
     }
     x0 = x[0]; y0 = y[0]; z0 = z[0];
@@ -533,7 +544,8 @@ __device__ __forceinline__ void cta_eval_dense(const CtaTopo& S, const DGrid& G,
         const int atom = tid + 32 * NW * k;
         float gx = 0.f, gy = 0.f, gz = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
         if (act[k]) {
-            ei += grid_blend<GRAD>(G, P.k_wall, cell[k], glo[k], ghi[k], gx, gy, gz);
+            if (DIRECT) ei += rec_direct<GRAD>(RD, P, m[k] & 0xff, x[k], y[k], z[k], gx, gy, gz);
+            else ei += grid_blend<GRAD>(G, P.k_wall, cell[k], glo[k], ghi[k], gx, gy, gz);
             if (GRAD) {
 #pragma unroll
                 for (int w = 0; w < NW; ++w) { const float4 f = S.part[w * npad + atom]; fx += f.x; fy += f.y; fz += f.z; }
@@ -569,19 +581,19 @@ __device__ __forceinline__ void cta_eval_dense(const CtaTopo& S, const DGrid& G,
 
 // ROUNDS: 0 = pair records (ligands of up to 64 atoms, 128 threads), 1 = dense partner sweep with two warps per chain (MC kernel),
 // 2 = decided at run time by S.rounds, 128 threads (score kernel).
-template <bool GRAD, bool ENERGY, bool MDN, int ROUNDS>
+template <bool GRAD, bool ENERGY, bool MDN, int ROUNDS, bool DIRECT>
 __device__ __forceinline__ void cta_eval_any(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
-                                             const MdnDev& M, const float4* __restrict__ mdn_par,
+                                             const MdnDev& M, const float4* __restrict__ mdn_par, const RecDev& RD,
                                              int max_depth, const float t[3], const float q[4], float theta,
                                              int atom, int part, bool active, float& x, float& y, float& z,
                                              float& e_inter, float& e_intra, float g6[6], float& gth) {
     if constexpr (ROUNDS == 1) {
-        cta_eval_dense<GRAD, ENERGY, MDN, 2>(S, G, P, K, F, M, mdn_par, max_depth, t, q, theta, x, y, z, e_inter, e_intra, g6, gth);
+        cta_eval_dense<GRAD, ENERGY, MDN, DIRECT, 2>(S, G, P, K, F, M, mdn_par, RD, max_depth, t, q, theta, x, y, z, e_inter, e_intra, g6, gth);
     } else {
         if (ROUNDS == 2 && S.rounds)
-            cta_eval_dense<GRAD, ENERGY, MDN, 4>(S, G, P, K, F, M, mdn_par, max_depth, t, q, theta, x, y, z, e_inter, e_intra, g6, gth);
+            cta_eval_dense<GRAD, ENERGY, MDN, DIRECT, 4>(S, G, P, K, F, M, mdn_par, RD, max_depth, t, q, theta, x, y, z, e_inter, e_intra, g6, gth);
         else
-            cta_eval<GRAD, ENERGY, MDN>(S, G, P, K, F, M, mdn_par, max_depth, t, q, theta, atom, part, active, x, y, z, e_inter, e_intra, g6, gth);
+            cta_eval<GRAD, ENERGY, MDN, DIRECT>(S, G, P, K, F, M, mdn_par, RD, max_depth, t, q, theta, atom, part, active, x, y, z, e_inter, e_intra, g6, gth);
     }
 }
 
@@ -606,7 +618,8 @@ __device__ __forceinline__ void cta_store_pose(float* __restrict__ dst, const Ct
 // Record instance: 128 threads, registers for 3 resident CTAs per SM (with 4 x 128 registers, C2 goes 6.0 -> 6.3 ms).  Dense
 // instance: 64 threads and 128 registers, EIGHT chains resident per SM (with the mixture-density term: 255 registers, four chains --
 // an 80-atom dock under the full score 490 -> 345 ms; the record instance with the term is faster at 168 than at 255: 60.5 / 71.3 ms).
-template <bool MDN, int ROUNDS>
+// DIRECT: the receptor term by direct pair sums (tridsk_dock_opts.receptor_direct), without the mixture-density term.
+template <bool MDN, int ROUNDS, bool DIRECT>
 __global__ void __launch_bounds__(ROUNDS ? 64 : 128, ROUNDS ? (MDN ? 4 : 8) : 3) mc_cta_kernel(const McLaunch a) {
     extern __shared__ __align__(16) unsigned char cta_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -660,7 +673,7 @@ __global__ void __launch_bounds__(ROUNDS ? 64 : 128, ROUNDS ? (MDN ? 4 : 8) : 3)
             const float uu = (k & 3) == 0 ? v0 : (k & 3) == 1 ? v1 : (k & 3) == 2 ? v2 : v3;
             cth = F.tor >= 0 ? PI_F * (2.f * uu - 1.f) : 0.f;
         }
-        cta_eval_any<false, true, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, ct, cq, cth, atom, part, active, x, y, z, ei, ea, g6, gth);
+        cta_eval_any<false, true, MDN, ROUNDS, DIRECT>(S, a.grid, P, K, F, a.mdn, mdn_par, a.rec, max_depth, ct, cq, cth, atom, part, active, x, y, z, ei, ea, g6, gth);
         ecur = ei + ea;
         ebest = ecur;
 #pragma unroll
@@ -695,7 +708,7 @@ __global__ void __launch_bounds__(ROUNDS ? 64 : 128, ROUNDS ? (MDN ? 4 : 8) : 3)
         float m[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         float b1p = 1.f, b2p = 1.f;
         for (int rf = 0; rf < P.n_refine; ++rf) {
-            cta_eval_any<true, false, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
+            cta_eval_any<true, false, MDN, ROUNDS, DIRECT>(S, a.grid, P, K, F, a.mdn, mdn_par, a.rec, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
             b1p *= P.adam_b1; b2p *= P.adam_b2;
             const float c1 = __fdividef(1.f, 1.f - b1p), c2 = __fdividef(1.f, 1.f - b2p);
             float g[7] = {g6[0], g6[1], g6[2], g6[3], g6[4], g6[5], gth}, dl[7];
@@ -716,7 +729,7 @@ __global__ void __launch_bounds__(ROUNDS ? 64 : 128, ROUNDS ? (MDN ? 4 : 8) : 3)
         }
 
         // a8: energy of the refined proposal, Metropolis, best tracking
-        cta_eval_any<false, true, MDN, ROUNDS>(S, a.grid, P, K, F, a.mdn, mdn_par, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
+        cta_eval_any<false, true, MDN, ROUNDS, DIRECT>(S, a.grid, P, K, F, a.mdn, mdn_par, a.rec, max_depth, pt, pq, pth, atom, part, active, x, y, z, ei, ea, g6, gth);
         const float enew = ei + ea;
         const bool accept = isfinite(enew) && (um < expf(-P.beta * (enew - ecur)));
         if (a.trace != nullptr && tid == 0) {
@@ -763,10 +776,12 @@ __global__ void __launch_bounds__(128) score_cta_kernel(const ScoreLaunch a) {
     const int atom = tid / S.lpa, part = tid % S.lpa;
     const bool active = atom < S.n;
     float t[3], q[4], th, x, y, z, g6[6], gth = 0.f, ei, ea;
+    RecDev no_rec;
+    no_rec.atoms = nullptr;
     cta_load_pose(a.poses + (size_t)i * a.pose_stride, F, t, q, th);
     quat_normalise(q);
-    if (a.grad != nullptr) cta_eval_any<true, true, MDN, 2>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
-    else cta_eval_any<false, true, MDN, 2>(S, a.grid, a.P, K, F, a.mdn, mdn_par, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
+    if (a.grad != nullptr) cta_eval_any<true, true, MDN, 2, false>(S, a.grid, a.P, K, F, a.mdn, mdn_par, no_rec, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
+    else cta_eval_any<false, true, MDN, 2, false>(S, a.grid, a.P, K, F, a.mdn, mdn_par, no_rec, h->max_depth, t, q, th, atom, part, active, x, y, z, ei, ea, g6, gth);
     if (tid == 0) { a.energy[3 * (size_t)i] = ei + ea; a.energy[3 * (size_t)i + 1] = ei; a.energy[3 * (size_t)i + 2] = ea; }
     if (a.grad != nullptr && warp == 0) {
         float* g = a.grad + (size_t)i * a.grad_stride;
@@ -786,10 +801,12 @@ __global__ void __launch_bounds__(128) score_cta_kernel(const ScoreLaunch a) {
 
 // per device (function attributes are per device): called by tridsk_create
 cudaError_t mc_cta_prepare() {
-    cudaError_t e = cudaFuncSetAttribute(mc_cta_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    cudaError_t e = cudaFuncSetAttribute(mc_cta_kernel<false, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<true, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<false, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<true, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mc_cta_kernel<false, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(score_cta_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(score_cta_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TRIDSK_SMEM_MAX_CTA);
     return e;
@@ -800,8 +817,14 @@ cudaError_t launch_mc_cta(cudaStream_t s, const McLaunch& a, int rounds, size_t 
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const unsigned nb = (unsigned)blocks;
-    if (a.mdn.n_res > 0) { if (rounds) mc_cta_kernel<true, 1><<<nb, 64, smem_bytes, s>>>(a); else mc_cta_kernel<true, 0><<<nb, 128, smem_bytes, s>>>(a); }
-    else { if (rounds) mc_cta_kernel<false, 1><<<nb, 64, smem_bytes, s>>>(a); else mc_cta_kernel<false, 0><<<nb, 128, smem_bytes, s>>>(a); }
+    if (a.rec.atoms) {                                            // direct receptor sums (the host does not pair them with E_MDN)
+        if (a.mdn.n_res > 0) return cudaErrorInvalidValue;
+        if (rounds) mc_cta_kernel<false, 1, true><<<nb, 64, smem_bytes, s>>>(a); else mc_cta_kernel<false, 0, true><<<nb, 128, smem_bytes, s>>>(a);
+    } else if (a.mdn.n_res > 0) {
+        if (rounds) mc_cta_kernel<true, 1, false><<<nb, 64, smem_bytes, s>>>(a); else mc_cta_kernel<true, 0, false><<<nb, 128, smem_bytes, s>>>(a);
+    } else {
+        if (rounds) mc_cta_kernel<false, 1, false><<<nb, 64, smem_bytes, s>>>(a); else mc_cta_kernel<false, 0, false><<<nb, 128, smem_bytes, s>>>(a);
+    }
     return cudaGetLastError();
 }
 

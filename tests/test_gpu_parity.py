@@ -1017,15 +1017,18 @@ def test_zero_quaternion_is_rejected(eng, gp, system):
 
 
 # ------------------------------------------------------------------------------------------- direct-pair receptor mode (S:8(f) NEXT-3)
-def test_dock_with_direct_receptor_sums_matches_oracle(orc, gp, system):
-    """tridsk_dock with receptor_direct: initial energies and teacher-forced MC steps against the oracle step whose receptor
-    term is the plain sum over receptor atoms (orc.DirectReceptor); the mode needs the receptor attached to the grid."""
+@pytest.mark.parametrize("mode", [1, 3])
+def test_dock_with_direct_receptor_sums_matches_oracle(orc, gp, system, mode):
+    """tridsk_dock with receptor_direct under the two mappings that carry it (a warp / a CTA per chain, the latter with both of
+    its instances: ligands up to 64 atoms and above): initial energies and teacher-forced MC steps against the oracle step whose
+    receptor term is the plain sum over receptor atoms (orc.DirectReceptor); the mode needs the receptor attached to the grid."""
     from paper_2510_24186_b200 import Engine, TridskError, split_state
     S = system
     eng = Engine(0)
+    eng.set_kernel(mode)
     rec = S["rec"]
     grid = eng.grid_from_values(S["G"].g, rec.origin, rec.spacing)
-    ids = [0, 1, 4]
+    ids = [0, 1, 4, 12]
     b = S["batch"].subset(ids)
     ligs = eng.load_ligands(b, S["radius"], S["role"])
     Ls = [S["L"][i] for i in ids]
@@ -1035,7 +1038,7 @@ def test_dock_with_direct_receptor_sums_matches_oracle(orc, gp, system):
     eng.attach_receptor(grid, rec.xyz, rec.type, S["radius"], S["role"], gp)
     D = orc.DirectReceptor(rec.xyz, rec.type, 16)
     r = eng.dock(grid, ligs, gp, *_dock_args(S), n_chains, 0, 1, seed=seed, want_state=True, receptor_direct=True)
-    assert eng.last_kernel() == 1
+    assert eng.last_kernel() == mode
     state = r["state"]
     compared = skipped = 0
     for s in range(4):
@@ -1057,7 +1060,7 @@ def test_dock_with_direct_receptor_sums_matches_oracle(orc, gp, system):
                 assert close(tr["e_prop"], rec_.e_prop, rtol=1e-3, atol=1e-3), (s, l, c, tr["e_prop"], rec_.e_prop)
                 assert (tr["flags"] & 1) == rec_.accept, (s, l, c)
     print(f"direct receptor mode, teacher-forced: compared {compared}, skipped {skipped}")
-    assert compared > 0.85 * 4 * 3 * 8
+    assert compared > 0.85 * 4 * len(ids) * 8
     # the grid mode on the same grid still gives the interpolated energies
     r0 = eng.dock(grid, ligs, gp, *_dock_args(S), n_chains, 0, 1, seed=seed, want_state=True)
     _, _, ec0, _ = split_state(r0["state"], len(ids), n_chains, stride)
