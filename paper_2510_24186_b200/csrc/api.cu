@@ -896,6 +896,10 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
         tridsk_free_ligands(lg);
         return fail(ctx, e == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA, std::string("load_ligands: ") + cudaGetErrorString(e));
     }
+    // the per-ligand pieces (a dozen small vectors each) are released by all threads, not one after the other by pk's destructor
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < L; ++i) pk[i] = PackedLig();
+    if (dbg) fprintf(stderr, "tridsk load_ligands: total %.1f ms\n", (omp_get_wtime() - t_a) * 1e3);
     *out = lg;
     return TRIDSK_OK;
 }
