@@ -415,9 +415,13 @@ extern "C" int tridsk_grid_attach_receptor(tridsk_ctx* ctx, tridsk_grid* grid, c
     RecDev R;
     memset(&R, 0, sizeof(R));
     long long ncell = 1;
-    for (int c = 0; c < 3; ++c) { R.lo[c] = lo[c]; R.nc[c] = std::max(1, (int)std::floor((hi[c] - lo[c]) / cut) + 1); ncell *= R.nc[c]; }
+    // cells of a third of the range, x fastest: the atoms of a row of cells adjacent in x are one contiguous slice, so a ligand
+    // atom visits, per (y, z) row within range, ONE slice trimmed to the x interval that can still lie inside the cut-off
+    R.span = 3;                                             // measured on D2: span 1 81 ms, 2 49 ms, 3 42 ms, 4 43 ms, 5 46 ms
+    const float cell = cut / (float)R.span;
+    for (int c = 0; c < 3; ++c) { R.lo[c] = lo[c]; R.nc[c] = std::max(1, (int)std::floor((hi[c] - lo[c]) / cell) + 1); ncell *= R.nc[c]; }
     if (ncell > (1 << 22)) return fail(ctx, TRIDSK_ELIMIT, "receptor extent / cut-off gives too many cells");
-    R.inv_cell = 1.f / cut; R.cut2 = cut * cut;
+    R.inv_cell = 1.f / cell; R.cell = cell; R.cut2 = cut * cut;
     auto cell_of = [&](int r) {
         int ci[3];
         for (int c = 0; c < 3; ++c) ci[c] = std::min(R.nc[c] - 1, std::max(0, (int)std::floor((hx[3 * r + c] - lo[c]) * R.inv_cell)));

@@ -296,7 +296,7 @@ __device__ __forceinline__ float pair_energy(const DParams& P, float d2, float d
 
 // ------------------------------------------------------------------ receptor term by direct pair sums (S:8(f) NEXT-3)
 // The paper's own evaluation (P:103-125, P:353 item 4): e(s_r, t, |x - r_r|) summed over the receptor atoms within the pair
-// function's range -- the 27 cells around the atom's cell, cells and atoms in a fixed order.  No interpolation, no wall.
+// function's range -- the cells within R.span of the atom's cell, cells and atoms in a fixed order.  No interpolation, no wall.
 template <bool GRAD>
 // i0, istep: the caller's share of every cell's atoms (the CTA mapping spreads an atom's partners over its lanes).
 __device__ __forceinline__ float rec_direct(const RecDev& R, const DParams& P, int type, float x, float y, float z,
@@ -305,9 +305,9 @@ __device__ __forceinline__ float rec_direct(const RecDev& R, const DParams& P, i
     const unsigned char role_t = __ldg(R.role + type);
     const int cx = (int)floorf((x - R.lo[0]) * R.inv_cell), cy = (int)floorf((y - R.lo[1]) * R.inv_cell), cz = (int)floorf((z - R.lo[2]) * R.inv_cell);
     float e = 0.f;
-    for (int kz = max(cz - 1, 0); kz <= min(cz + 1, R.nc[2] - 1); ++kz)
-        for (int ky = max(cy - 1, 0); ky <= min(cy + 1, R.nc[1] - 1); ++ky)
-            for (int kx = max(cx - 1, 0); kx <= min(cx + 1, R.nc[0] - 1); ++kx) {
+    for (int kz = max(cz - R.span, 0); kz <= min(cz + R.span, R.nc[2] - 1); ++kz)
+        for (int ky = max(cy - R.span, 0); ky <= min(cy + R.span, R.nc[1] - 1); ++ky)
+            for (int kx = max(cx - R.span, 0); kx <= min(cx + R.span, R.nc[0] - 1); ++kx) {
                 const int c = (kz * R.nc[1] + ky) * R.nc[0] + kx;
                 const int r1 = __ldg(R.cell_off + c + 1);
                 for (int r = __ldg(R.cell_off + c) + i0; r < r1; r += istep) {

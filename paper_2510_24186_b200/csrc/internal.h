@@ -71,8 +71,8 @@ struct RecDev {
     const int* cell_off;          // [ncells + 1]
     const float* radius;          // [n_types]
     const unsigned char* role;    // [n_types]
-    int nc[3];
-    float lo[3], inv_cell, cut2;
+    int nc[3], span;              // cells per axis; the cut-off spans `span` cells
+    float lo[3], inv_cell, cell, cut2;
 };
 
 // Per-ligand header.  Atoms are stored in an INTERNAL order (depth-first over the torsion tree) so that

@@ -211,6 +211,82 @@ __device__ __forceinline__ void cta_dense4(const PairK& K, const float4 me, cons
     }
 }
 
+// ------------------------------------------------------------------ receptor term by direct pair sums, CTA form (S:8(f) NEXT-3)
+// e(s_r, t, |x - r_r|) summed over the receptor atoms within the pair function's range (P:103-125, P:353 item 4), for this
+// thread's share (i0, i0 + istep, ... of every slice) of the partners of the ligand atom at (x, y, z).  The receptor's cells
+// (RecDev) are sorted x fastest, so per (y, z) row of cells within range the candidates are ONE contiguous slice, trimmed to
+// the x interval that can still lie inside the cut-off.  The warp walks the rows in lockstep, every lane its own slice of the
+// row, one atom per iteration; an atom inside the cut-off goes to a four-slot queue, and when any lane's queue is full all lanes
+// evaluate theirs with the branch-free four-pair arithmetic (cta_quad) -- the costly part runs with most lanes busy although
+// only one scanned atom in four to ten is in range.  ALL 32 lanes of a warp must call (work = false: nothing to do).
+// e += this share of the energy; (fx, fy, fz) += its force in kappa units, like the intra-ligand pair force.
+template <bool GRAD, bool ENERGY>
+__device__ __forceinline__ void cta_rec_direct(const RecDev& R, const PairK& K, bool work, int type, float x, float y, float z,
+                                               int i0, int istep, float& e, float& fx, float& fy, float& fz) {
+    const float rt = work ? __ldg(R.radius + type) : 0.f;
+    const unsigned role_t = work ? __ldg(R.role + type) : 0u;
+    float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f), q1 = q0, q2 = q0, q3 = q0;
+    int cnt = 0;
+    float eL = 0.f, eC = 0.f, eH = 0.f;
+    auto flush = [&]() {
+        const float4 qa[4] = {q0, q1, q2, q3};
+        float dx[4], dy[4], dz[4], c[4], sv[4];
+        unsigned hbw[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const bool valid = u < cnt;
+            const int st = valid ? __float_as_int(qa[u].w) : 0;
+            const unsigned role_s = __ldg(R.role + st);
+            dx[u] = x - qa[u].x; dy[u] = y - qa[u].y; dz[u] = z - qa[u].z;
+            c[u] = valid ? (__ldg(R.radius + st) + rt) + K.mu : -1e15f;
+            hbw[u] = (valid && (((role_s & 1u) && (role_t & 2u)) || ((role_s & 2u) && (role_t & 1u)))) ? 1u : 0u;
+        }
+        cta_quad<GRAD, ENERGY>(K, dx, dy, dz, c, hbw, 1u, eL, eC, eH, sv);
+        if (GRAD) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { fx = fmaf(sv[u], dx[u], fx); fy = fmaf(sv[u], dy[u], fy); fz = fmaf(sv[u], dz[u], fz); }
+        }
+        cnt = 0;
+    };
+    // the rows are walked in lockstep (row offsets -span .. span about every lane's own cell: uniform control flow), the slice of a
+    // row differs per lane
+    const int cy = __float2int_rd((y - R.lo[1]) * R.inv_cell), cz = __float2int_rd((z - R.lo[2]) * R.inv_cell);
+    for (int oz = -R.span; oz <= R.span; ++oz)
+        for (int oy = -R.span; oy <= R.span; ++oy) {
+            const int ky = cy + oy, kz = cz + oz;
+            int r = 0, r1 = 0;
+            if (work && (unsigned)ky < (unsigned)R.nc[1] && (unsigned)kz < (unsigned)R.nc[2]) {
+                const float y0 = R.lo[1] + R.cell * (float)ky, z0 = R.lo[2] + R.cell * (float)kz;
+                const float dy = fmaxf(0.f, fmaxf(y0 - y, y - (y0 + R.cell))), dz = fmaxf(0.f, fmaxf(z0 - z, z - (z0 + R.cell)));
+                const float rem = R.cut2 - dy * dy - dz * dz;
+                if (rem > 0.f) {
+                    const float hx = sqrt_approx(rem) + 1e-3f;       // (a hair wider: the cut-off test below is the exact one)
+                    const int kx0 = max(0, __float2int_rd((x - hx - R.lo[0]) * R.inv_cell));
+                    const int kx1 = min(R.nc[0] - 1, __float2int_rd((x + hx - R.lo[0]) * R.inv_cell));
+                    if (kx0 <= kx1) {
+                        const int base = (kz * R.nc[1] + ky) * R.nc[0];
+                        r = __ldg(R.cell_off + base + kx0) + i0;
+                        r1 = __ldg(R.cell_off + base + kx1 + 1);
+                    }
+                }
+            }
+            while (__any_sync(FULL_MASK, r < r1)) {
+                if (r < r1) {
+                    const float4 a = __ldg(R.atoms + r);
+                    r += istep;
+                    const float dx = x - a.x, dy = y - a.y, dz = z - a.z;
+                    if (dx * dx + dy * dy + dz * dz < R.cut2) {
+                        if (cnt == 0) q0 = a; else if (cnt == 1) q1 = a; else if (cnt == 2) q2 = a; else q3 = a;
+                        ++cnt;
+                    }
+                }
+                if (__any_sync(FULL_MASK, cnt == 4)) flush();
+            }
+        }
+    if (__any_sync(FULL_MASK, cnt > 0)) flush();
+    if (ENERGY) e += fmaf(K.w_clash_ln2, eC, -fmaf(K.w_long, eL, K.w_hbond * eH));
+}
+
 // ------------------------------------------------------------------ a3 forward kinematics of the frames (O8)
 // World frame (R, p) of this lane's fragment, F_g = F_parent o L_g, by pointer jumping (every warp the same).
 __device__ __forceinline__ void cta_frames(const CtaFrag& F, int max_depth, const float t[3], const float q[4], float theta,
@@ -326,8 +402,8 @@ __device__ __forceinline__ void cta_reverse(const CtaTopo& S, const CtaFrag& F, 
 //      on lane g (O9); x, y, z = this thread's atom (valid when `active`).
 // MDN: the mixture-density term (mdn.cuh); the lanes of an atom share its residues (lane `part` takes residues part,
 // part + lpa, ...), their shares join the pair force / the energy sums before the fixed-order reductions.
-// DIRECT: the receptor term by direct pair sums over the receptor atoms (rec_direct, chain.cuh) instead of the grid lookup; the
-// lanes of an atom share the atoms of every cell, their shares join the pair force like the mixture-density term's.
+// DIRECT: the receptor term by direct pair sums over the receptor atoms (cta_rec_direct) instead of the grid lookup; the lanes
+// of an atom share the atoms of every slice, their shares join the pair force.
 template <bool GRAD, bool ENERGY, bool MDN, bool DIRECT>
 __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const DParams& P, const PairK& K, const CtaFrag& F,
                                          const MdnDev& M, const float4* __restrict__ mdn_par, const RecDev& RD,
@@ -407,11 +483,7 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     // ---- a4 receptor term of this thread's atom (the gathers were issued before the barrier)
     float ei = 0.f, gx = 0.f, gy = 0.f, gz = 0.f;
     if (!DIRECT && lead) ei = grid_blend<GRAD>(G, P.k_wall, cell, glo, ghi, gx, gy, gz);
-    if (DIRECT && active) {
-        float mx = 0.f, my = 0.f, mz = 0.f;
-        ei += rec_direct<GRAD>(RD, P, m & 0xff, x, y, z, mx, my, mz, part, S.lpa);
-        if (GRAD) { fx = fmaf(mx, K.inv_kappa, fx); fy = fmaf(my, K.inv_kappa, fy); fz = fmaf(mz, K.inv_kappa, fz); }
-    }
+    if (DIRECT) cta_rec_direct<GRAD, ENERGY>(RD, K, active, m & 0xff, x, y, z, part, S.lpa, ei, fx, fy, fz);
     if (MDN && active) {
         float mx = 0.f, my = 0.f, mz = 0.f;
         mdn_atom(M, mdn_par, n, atom, x, y, z, part, S.lpa, GRAD, ei, mx, my, mz);
@@ -543,9 +615,9 @@ __device__ __forceinline__ void cta_eval_dense(const CtaTopo& S, const DGrid& G,
     for (int k = 0; k < APT; ++k) {
         const int atom = tid + 32 * NW * k;
         float gx = 0.f, gy = 0.f, gz = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
+        if (DIRECT) cta_rec_direct<GRAD, ENERGY>(RD, K, act[k], m[k] & 0xff, x[k], y[k], z[k], 0, 1, ei, fx, fy, fz);   // (the whole warp calls)
         if (act[k]) {
-            if (DIRECT) ei += rec_direct<GRAD>(RD, P, m[k] & 0xff, x[k], y[k], z[k], gx, gy, gz);
-            else ei += grid_blend<GRAD>(G, P.k_wall, cell[k], glo[k], ghi[k], gx, gy, gz);
+            if (!DIRECT) ei += grid_blend<GRAD>(G, P.k_wall, cell[k], glo[k], ghi[k], gx, gy, gz);
             if (GRAD) {
 #pragma unroll
                 for (int w = 0; w < NW; ++w) { const float4 f = S.part[w * npad + atom]; fx += f.x; fy += f.y; fz += f.z; }
