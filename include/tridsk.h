@@ -125,7 +125,8 @@ typedef struct {
     int receptor_direct;       /* 1: the receptor term of every evaluation is the paper's own direct sum over the receptor atoms
                                   within the pair function's range (P:103-125, P:353 item 4) instead of the
                                   trilinear grid lookup: no interpolation error, no wall, ~500 pair evaluations per ligand atom.
-                                  Needs tridsk_grid_attach_receptor on the grid; runs under the warp-per-chain mapping          */
+                                  Needs tridsk_grid_attach_receptor on the grid; runs under the CTA-per-chain mapping (single
+                                  docks, without E_MDN) and the warp-per-chain mapping (everything else)                     */
 } tridsk_dock_opts;
 
 /* ---- lifetime ------------------------------------------------------------------------------ */
@@ -164,8 +165,8 @@ int tridsk_build_grid_cached(tridsk_ctx* ctx, const float* rec_xyz, const int* r
 /* budget_bytes >= 0 sets the budget (dropping grids beyond it); stats (may be NULL) [host] <- {hits, misses, grids held, bytes held}. */
 int tridsk_grid_cache_config(tridsk_ctx* ctx, long long budget_bytes, long long stats[4]);
 
-/* Give a grid the receptor it tabulates, for tridsk_dock's receptor_direct mode: the atoms are sorted into cells of the pair
- * function's range (max of long_dmax, hb_dmax and the largest clash distance).  rec_xyz, rec_type: [host|dev]. */
+/* Give a grid the receptor it tabulates, for tridsk_dock's receptor_direct mode: the atoms are sorted into cells of a third of
+ * the pair function's range (max of long_dmax, hb_dmax and the largest clash distance).  rec_xyz, rec_type: [host|dev]. */
 int tridsk_grid_attach_receptor(tridsk_ctx* ctx, tridsk_grid* grid, const float* rec_xyz, const int* rec_type, int n_rec,
                                 const tridsk_types* types, const tridsk_params* params);
 
