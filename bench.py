@@ -341,12 +341,16 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
             grid = eng.build_grid(h_xyz, h_typ, radius, role, gp, rec.origin, rec.dims, rec.spacing)
             eng.dock(grid, lg, *dock_args, seed=cfg.philox_seed, pose_stride=stride, out=h_out, chain_base=chain_base)
             grid.free(); lg.free()
-        e2e_step()
+        e2e_step()                                                           # two untimed passes: the first one also pays first-touch
+        e2e_step()                                                           # costs (pinned staging, allocator arenas, graph instantiation)
         barrier()
         n_e2e = max(1, min(steps, 3))
         t0 = time.perf_counter()
         for _ in range(n_e2e):
+            ts = time.perf_counter()
             e2e_step()
+            if os.environ.get("TRIDSK_BENCH_DEBUG"):
+                print(f"e2e step {1e3 * (time.perf_counter() - ts):.1f} ms", file=sys.stderr)
         barrier()
         e2e_s = (time.perf_counter() - t0) / n_e2e
         if world > 1:
