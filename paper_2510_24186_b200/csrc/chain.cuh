@@ -332,7 +332,8 @@ __device__ __forceinline__ float rec_direct(const RecDev& R, const DParams& P, i
 //      GRAD: gt[3] = dE/dt, gw[3] = dE/domega (uniform), gth = dE/dtheta on lane f (O9).
 // sP : per-warp shared scratch, 6 * J * 32 floats.
 // M.n_res > 0: the mixture-density term (mdn.cuh) of every atom is added to its receptor term; mdn_par = the ligand's block.
-template <int J, bool GRAD>
+// MDN: the instance that carries the mixture-density term (its prefetch buffers cost ~90 registers: kept out of the other one)
+template <int J, bool GRAD, bool MDN>
 __device__ __forceinline__ void eval_pose(const Lig<J>& L, const DGrid& G, const DParams& P,
                                           const MdnDev& M, const float4* __restrict__ mdn_par, const RecDev& RD,
                                           const float t[3], const float q[4], float theta,
@@ -397,7 +398,7 @@ __device__ __forceinline__ void eval_pose(const Lig<J>& L, const DGrid& G, const
             if (RD.atoms) e_inter += rec_direct<GRAD>(RD, P, L.typ[j], x[j], y[j], z[j], fx[j], fy[j], fz[j]);
             else e_inter += grid_interp_packed<GRAD>(G, P.k_wall, L.typ[j], x[j], y[j], z[j], fx[j], fy[j], fz[j]);
         }
-        if (M.n_res > 0 && L.valid[j]) mdn_atom(M, mdn_par, L.n, j * L.S + lane, x[j], y[j], z[j], 0, 1, GRAD, e_inter, fx[j], fy[j], fz[j]);
+        if (MDN && L.valid[j]) mdn_atom(M, mdn_par, L.n, j * L.S + lane, x[j], y[j], z[j], 0, 1, GRAD, e_inter, fx[j], fy[j], fz[j]);
     }
 
     // ---- a5 intra-ligand pairs: conflict-free rotation schedule, partner data by shuffle, reaction force shuffled back

@@ -19,7 +19,7 @@ __device__ __forceinline__ void store_pose(float* __restrict__ dst, int T, int s
 }
 
 // ------------------------------------------------------------------ the fused MC kernel
-template <int J>
+template <int J, bool MDN>
 __global__ void __launch_bounds__(TRIDSK_WARPS_PER_CTA * 32) mc_kernel(const McLaunch a) {
     __shared__ float sP_all[TRIDSK_WARPS_PER_CTA][6 * J * 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(TRIDSK_WARPS_PER_CTA * 32) mc_kernel(const McL
             cth = (lane >= 1 && lane <= T) ? PI_F * (2.f * uu - 1.f) : 0.f;
         }
         float ei, ea;
-        eval_pose<J, false>(L, a.grid, P, a.mdn, mdn_par, a.rec, ct, cq, cth, x, y, z, ei, ea, gt, gw, gth, sP);
+        eval_pose<J, false, MDN>(L, a.grid, P, a.mdn, mdn_par, a.rec, ct, cq, cth, x, y, z, ei, ea, gt, gw, gth, sP);
         ecur = warp_sum(ei + ea);
         ebest = ecur;
 #pragma unroll
@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(TRIDSK_WARPS_PER_CTA * 32) mc_kernel(const McL
         float b1p = 1.f, b2p = 1.f;
         for (int rf = 0; rf < P.n_refine; ++rf) {
             float ei, ea;
-            eval_pose<J, true>(L, a.grid, P, a.mdn, mdn_par, a.rec, pt, pq, pth, x, y, z, ei, ea, gt, gw, gth, sP);
+            eval_pose<J, true, MDN>(L, a.grid, P, a.mdn, mdn_par, a.rec, pt, pq, pth, x, y, z, ei, ea, gt, gw, gth, sP);
             b1p *= P.adam_b1; b2p *= P.adam_b2;
             const float c1 = __fdividef(1.f, 1.f - b1p), c2 = __fdividef(1.f, 1.f - b2p);   // 2-ulp division / square root:
             // far inside the tolerance, and the IEEE forms are slow-path subroutines on the chain's critical path
@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(TRIDSK_WARPS_PER_CTA * 32) mc_kernel(const McL
 
         // a8: energy of the refined proposal, Metropolis, best tracking
         float ei, ea;
-        eval_pose<J, false>(L, a.grid, P, a.mdn, mdn_par, a.rec, pt, pq, pth, x, y, z, ei, ea, gt, gw, gth, sP);
+        eval_pose<J, false, MDN>(L, a.grid, P, a.mdn, mdn_par, a.rec, pt, pq, pth, x, y, z, ei, ea, gt, gw, gth, sP);
         const float enew = warp_sum(ei + ea);
         const bool accept = isfinite(enew) && (um < expf(-P.beta * (enew - ecur)));
         if (a.trace != nullptr && lane == 0) {
@@ -168,18 +168,28 @@ cudaError_t launch_mc(cudaStream_t s, int J, const McLaunch& a) {
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const dim3 grid((unsigned)blocks), block(TRIDSK_WARPS_PER_CTA * 32);
-    switch (J) {
-        case 1: mc_kernel<1><<<grid, block, 0, s>>>(a); break;
-        case 2: mc_kernel<2><<<grid, block, 0, s>>>(a); break;
-        case 3: mc_kernel<3><<<grid, block, 0, s>>>(a); break;
-        case 4: mc_kernel<4><<<grid, block, 0, s>>>(a); break;
-        default: return cudaErrorInvalidValue;
+    if (a.mdn.n_res > 0) {
+        switch (J) {
+            case 1: mc_kernel<1, true><<<grid, block, 0, s>>>(a); break;
+            case 2: mc_kernel<2, true><<<grid, block, 0, s>>>(a); break;
+            case 3: mc_kernel<3, true><<<grid, block, 0, s>>>(a); break;
+            case 4: mc_kernel<4, true><<<grid, block, 0, s>>>(a); break;
+            default: return cudaErrorInvalidValue;
+        }
+    } else {
+        switch (J) {
+            case 1: mc_kernel<1, false><<<grid, block, 0, s>>>(a); break;
+            case 2: mc_kernel<2, false><<<grid, block, 0, s>>>(a); break;
+            case 3: mc_kernel<3, false><<<grid, block, 0, s>>>(a); break;
+            case 4: mc_kernel<4, false><<<grid, block, 0, s>>>(a); break;
+            default: return cudaErrorInvalidValue;
+        }
     }
     return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------ tridsk_score_grad: one warp per pose
-template <int J>
+template <int J, bool MDN>
 __device__ __forceinline__ void score_one(const ScoreLaunch& a, int i, int lig, float* sP) {
     const int lane = threadIdx.x & 31;
     Lig<J> L;
@@ -190,8 +200,8 @@ __device__ __forceinline__ void score_one(const ScoreLaunch& a, int i, int lig, 
     const float4* mdn_par = a.mdn.n_res > 0 ? a.mdn.par + a.mdn.lig_off[lig] : nullptr;
     RecDev no_rec;
     no_rec.atoms = nullptr;
-    if (a.grad != nullptr) eval_pose<J, true>(L, a.grid, a.P, a.mdn, mdn_par, no_rec, t, q, th, x, y, z, ei, ea, gt, gw, gth, sP);
-    else eval_pose<J, false>(L, a.grid, a.P, a.mdn, mdn_par, no_rec, t, q, th, x, y, z, ei, ea, gt, gw, gth, sP);
+    if (a.grad != nullptr) eval_pose<J, true, MDN>(L, a.grid, a.P, a.mdn, mdn_par, no_rec, t, q, th, x, y, z, ei, ea, gt, gw, gth, sP);
+    else eval_pose<J, false, MDN>(L, a.grid, a.P, a.mdn, mdn_par, no_rec, t, q, th, x, y, z, ei, ea, gt, gw, gth, sP);
     ei = warp_sum(ei); ea = warp_sum(ea);
     if (lane == 0) {
         a.energy[3 * (size_t)i] = ei + ea; a.energy[3 * (size_t)i + 1] = ei; a.energy[3 * (size_t)i + 2] = ea;
@@ -211,6 +221,7 @@ __device__ __forceinline__ void score_one(const ScoreLaunch& a, int i, int lig, 
     }
 }
 
+template <bool MDN>
 __global__ void __launch_bounds__(TRIDSK_WARPS_PER_CTA * 32) score_kernel(const ScoreLaunch a) {
     __shared__ float sP_all[TRIDSK_WARPS_PER_CTA][6 * TRIDSK_MAX_J * 32];
     const int warp = threadIdx.x >> 5;
@@ -218,17 +229,18 @@ __global__ void __launch_bounds__(TRIDSK_WARPS_PER_CTA * 32) score_kernel(const 
     if (i >= a.n_pose) return;
     const int lig = a.lig_index[i];
     switch (a.hdr[lig].J) {                 // warp-uniform
-        case 1: score_one<1>(a, i, lig, sP_all[warp]); break;
-        case 2: score_one<2>(a, i, lig, sP_all[warp]); break;
-        case 3: score_one<3>(a, i, lig, sP_all[warp]); break;
-        default: score_one<4>(a, i, lig, sP_all[warp]); break;
+        case 1: score_one<1, MDN>(a, i, lig, sP_all[warp]); break;
+        case 2: score_one<2, MDN>(a, i, lig, sP_all[warp]); break;
+        case 3: score_one<3, MDN>(a, i, lig, sP_all[warp]); break;
+        default: score_one<4, MDN>(a, i, lig, sP_all[warp]); break;
     }
 }
 
 cudaError_t launch_score(cudaStream_t s, const ScoreLaunch& a) {
     if (a.n_pose <= 0) return cudaSuccess;
     const int blocks = (a.n_pose + TRIDSK_WARPS_PER_CTA - 1) / TRIDSK_WARPS_PER_CTA;
-    score_kernel<<<blocks, TRIDSK_WARPS_PER_CTA * 32, 0, s>>>(a);
+    if (a.mdn.n_res > 0) score_kernel<true><<<blocks, TRIDSK_WARPS_PER_CTA * 32, 0, s>>>(a);
+    else score_kernel<false><<<blocks, TRIDSK_WARPS_PER_CTA * 32, 0, s>>>(a);
     return cudaGetLastError();
 }
 
