@@ -1355,7 +1355,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     // tridsk_set_kernel overrides.
     int mode = ctx->kernel;
     if (mode == 0) {
-        if (nch >= (size_t)ctx->sm_count * 64) mode = 2;            // measured crossover with the warp form: ~64 chains per SM
+        if (nch >= (size_t)ctx->sm_count * 44) mode = 2;            // measured crossover with the warp form: ~43 chains per SM (16 C2 docks)
         else if (ligs->has_cta && nch <= (size_t)ctx->sm_count * 8) mode = 3;
         else mode = 1;
     }
