@@ -127,6 +127,8 @@ typedef struct {
                                   trilinear grid lookup: no interpolation error, no wall, ~500 pair evaluations per ligand atom.
                                   Needs tridsk_grid_attach_receptor on the grid; runs under the CTA-per-chain mapping (single
                                   docks, without E_MDN) and the warp-per-chain mapping (everything else)                     */
+    int lig_base;              /* Philox ligand id of the handle's ligand 0: a batch docked in parts (tridsk_screen) draws the
+                                  same random streams as the whole batch in one call                                         */
 } tridsk_dock_opts;
 
 /* ---- lifetime ------------------------------------------------------------------------------ */
@@ -251,6 +253,20 @@ int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligands* 
                 const float box_min[3], const float box_max[3], const float pocket_center[3], float pocket_radius,
                 int n_chains, int n_steps, int top_k, unsigned long long seed, int pose_stride,
                 float* out_energy, float* out_pose, int* out_chain, const tridsk_dock_opts* opts);
+
+/*
+ * A whole screen in one call, from the caller's HOST ligand arrays: tridsk_load_ligands + tridsk_dock + tridsk_free_ligands,
+ * but the batch goes in two parts and the host-side packing of the second (most of the batch) runs while the first is
+ * docking on the GPU.  Results are identical to the three calls on the whole batch (the second part docks with
+ * tridsk_dock_opts.lig_base = size of the first, so every chain draws the same Philox streams; "each of which was
+ * individually tackled": ligands are independent).  Batches below 8,192 ligands go in one part.  Outputs [host|dev] as in
+ * tridsk_dock, pose_stride >= 7 + the largest torsion count of the batch; the call returns when they are complete.  The
+ * physics terms only: the mixture-density term is attached to a loaded batch (tridsk_load_mdn), which this call never exposes.
+ */
+int tridsk_screen(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligand_batch* batch, const tridsk_types* types,
+                  const tridsk_params* params, const float box_min[3], const float box_max[3],
+                  const float pocket_center[3], float pocket_radius, int n_chains, int n_steps, int top_k,
+                  unsigned long long seed, int pose_stride, float* out_energy, float* out_pose, int* out_chain);
 
 /*
  * tridsk_dock for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that

@@ -52,7 +52,8 @@ class _Mdn(C.Structure):
 class _DockOpts(C.Structure):
     _fields_ = [("first_step", C.c_int), ("init_poses", C.c_void_p), ("resume", C.c_int),
                 ("chain_state", C.c_void_p), ("trace", C.c_void_p), ("steps_per_launch", C.c_int),
-                ("no_graph", C.c_int), ("chain_base", C.c_int), ("cluster_rmsd", C.c_float), ("receptor_direct", C.c_int)]
+                ("no_graph", C.c_int), ("chain_base", C.c_int), ("cluster_rmsd", C.c_float), ("receptor_direct", C.c_int),
+                ("lig_base", C.c_int)]
 
 
 TRACE_DTYPE = np.dtype([("e_prop", np.float32), ("e_cur", np.float32), ("u", np.float32), ("flags", np.int32)])
@@ -273,6 +274,14 @@ class Engine:
         """batch: any object with the arrays of tridsk_ligand_batch (e.g. workloads.synth.LigandBatch).
         pairs: optional (pair_off, pair_ab); otherwise the library derives them from the bonds."""
         ty, keep = self._types(radius, role)
+        b, arrs = self._batch(batch, pairs)
+        h = C.c_void_p()
+        self._ck(lib().tridsk_load_ligands(self.ctx, C.byref(b), C.byref(ty), C.byref(h)))
+        return Ligands(self, h)
+
+    @staticmethod
+    def _batch(batch, pairs=None):
+        """tridsk_ligand_batch over the arrays of `batch` (no copies when they already have the ABI's dtypes)."""
         A = lambda a, dt: np.ascontiguousarray(a, dt)
         arrs = dict(atom_off=A(batch.atom_off, np.int32), ref_xyz=A(batch.ref_xyz, np.float32),
                     atom_type=A(batch.atom_type, np.uint8), atom_frag=A(batch.atom_frag, np.uint8),
@@ -285,9 +294,29 @@ class Engine:
         b = _Batch(n_lig=int(batch.n_lig))
         for k, v in arrs.items():
             setattr(b, k, v.ctypes.data)
-        h = C.c_void_p()
-        self._ck(lib().tridsk_load_ligands(self.ctx, C.byref(b), C.byref(ty), C.byref(h)))
-        return Ligands(self, h)
+        return b, arrs
+
+    def screen(self, grid: Grid, batch, radius, role, params, box_min, box_max, pocket_center, pocket_radius,
+               n_chains, n_steps, top_k, seed=0, pose_stride=None, out=None, pairs=None):
+        """tridsk_screen: load + dock + free of a host ligand batch in one call (the packing of most of the batch overlaps the
+        docking of its first part).  -> dict(energy[n_lig,k,2], pose[n_lig,k,stride], chain[n_lig,k]); `out`: optional
+        pre-allocated buffers (numpy or CUDA tensors)."""
+        ty, keep = self._types(radius, role)
+        b, arrs = self._batch(batch, pairs)
+        L = int(batch.n_lig)
+        stride = int(pose_stride or (7 + int(np.max(np.diff(arrs["tor_off"])) if L else 0)))
+        if out is not None:
+            energy, pose, chain = out
+        else:
+            energy = np.empty((L, top_k, 2), np.float32)
+            pose = np.empty((L, top_k, stride), np.float32)
+            chain = np.empty((L, top_k), np.int32)
+        self._sync_in()
+        self._ck(lib().tridsk_screen(self.ctx, grid.handle, C.byref(b), C.byref(ty), C.byref(params), _f3(box_min), _f3(box_max),
+                                     _f3(pocket_center), C.c_float(pocket_radius), C.c_int(n_chains), C.c_int(n_steps),
+                                     C.c_int(top_k), C.c_ulonglong(seed), C.c_int(stride), _ptr(energy), _ptr(pose), _ptr(chain)))
+        self._sync_out()
+        return dict(energy=energy, pose=pose, chain=chain)
 
     def load_mdn(self, ligs: Ligands, res_xyz, res_off, pi, mu, sigma, K, w_mdn=1.0, d_cut=5.0):
         """Attach the mixture-density term (tridsk_load_mdn) to a ligand batch.  res_xyz [n_at,3], res_off [n_res+1]: host;
@@ -348,7 +377,7 @@ class Engine:
     def dock(self, grid: Grid, ligs: Ligands, params, box_min, box_max, pocket_center, pocket_radius,
              n_chains, n_steps, top_k, seed=0, pose_stride=None, device_out=False, init_poses=None,
              first_step=0, resume=False, chain_state=None, want_state=False, want_trace=False,
-             steps_per_launch=0, no_graph=False, chain_base=0, out=None, cluster_rmsd=0.0, receptor_direct=False):
+             steps_per_launch=0, no_graph=False, chain_base=0, out=None, cluster_rmsd=0.0, receptor_direct=False, lig_base=0):
         """-> dict(energy[n_lig,k,2], pose[n_lig,k,stride], chain[n_lig,k], state?, trace?).
         device_out: outputs are CUDA torch tensors (no D2H, no sync); else numpy (D2H inside the call).
         out: optional pre-allocated (energy, pose, chain) buffers to write into."""
@@ -371,6 +400,7 @@ class Engine:
         o.chain_base = int(chain_base)
         o.cluster_rmsd = float(cluster_rmsd)
         o.receptor_direct = int(bool(receptor_direct))
+        o.lig_base = int(lig_base)
         keep = []
         if init_poses is not None:
             if isinstance(init_poses, np.ndarray):

@@ -1345,7 +1345,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     to_dparams(params, &base.P);
     for (int c = 0; c < 3; ++c) { base.box_min[c] = box_min[c]; base.box_max[c] = box_max[c]; base.centre[c] = pocket_center[c]; }
     base.radius = pocket_radius;
-    base.n_chains = n_chains; base.pose_stride = pose_stride; base.seed = seed; base.chain_base = o.chain_base;
+    base.n_chains = n_chains; base.pose_stride = pose_stride; base.seed = seed; base.chain_base = o.chain_base; base.lig_base = o.lig_base;
     base.init_poses = (const float*)d_init;
     base.pose_cur = state; base.pose_best = state + n_pose_f; base.e_cur = state + 2 * n_pose_f; base.e_best = state + 2 * n_pose_f + nch;
     base.trace = d_trace; base.trace_stride = n_steps;
@@ -1560,6 +1560,77 @@ extern "C" int tridsk_debug_microbench(tridsk_ctx* ctx, int which, unsigned long
     ctx->launches += 2;
     *work = w;
     return TRIDSK_OK;
+}
+
+// ---------------------------------------------------------------------------------------- tridsk_screen
+// load + dock + free of a screen given as host arrays, with the host-side packing of most of the batch overlapped with the
+// docking of its first part (tridsk.h).  The two parts are sub-batch VIEWS of the caller's arrays (the offset tables hold
+// absolute positions); the second part docks with lig_base = size of the first, so every chain draws the Philox streams it
+// would draw in one tridsk_dock over the whole batch.
+extern "C" int tridsk_screen(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_ligand_batch* batch, const tridsk_types* types,
+                             const tridsk_params* params, const float box_min[3], const float box_max[3],
+                             const float pocket_center[3], float pocket_radius, int n_chains, int n_steps, int top_k,
+                             unsigned long long seed, int pose_stride, float* out_energy, float* out_pose, int* out_chain) {
+    if (!ctx || !grid || !batch || !types || !params) return fail(ctx, TRIDSK_EINVAL, "null argument");
+    ENTER(ctx);
+    NvtxRange nvtx_("tridsk_screen");
+    const int L = batch->n_lig;
+    if (L < 0 || top_k < 0) return fail(ctx, TRIDSK_EINVAL, "bad n_lig / top_k");
+    if (L == 0) return TRIDSK_OK;
+    if (top_k > 0 && (!out_energy || !out_pose || !out_chain)) return fail(ctx, TRIDSK_EINVAL, "null output");
+    // first part: large enough that its docking outlasts the packing of the rest, small enough that its own packing is short
+    const int l1 = L >= 8192 ? std::max(2048, L / 16) : L;      // measured on C5 (65,536 ligands): 1/8 1641 ms, 1/12 1630, 1/16 1626, 1/24 1624 per pass
+    const size_t per_e = 2 * (size_t)top_k, per_p = (size_t)top_k * pose_stride, per_c = (size_t)top_k;
+    const bool h_oe = top_k && !is_device_ptr(out_energy), h_op = top_k && !is_device_ptr(out_pose), h_oc = top_k && !is_device_ptr(out_chain);
+    float* d_e = out_energy; float* d_p = out_pose; int* d_c = out_chain;
+    if (l1 < L && (h_oe || h_op || h_oc)) {                      // the parts write device memory; one copy back at the end
+        char* ob = nullptr;
+        const size_t b_e = sizeof(float) * per_e * L, b_p = sizeof(float) * per_p * L, b_c = sizeof(int) * per_c * L;
+        const size_t o_p = (b_e + 255) / 256 * 256, o_c = o_p + (b_p + 255) / 256 * 256;
+        int rc = scratch(ctx, 11, o_c + b_c + 256, (void**)&ob);
+        if (rc) return rc;
+        if (h_oe) d_e = (float*)ob;
+        if (h_op) d_p = (float*)(ob + o_p);
+        if (h_oc) d_c = (int*)(ob + o_c);
+    }
+    auto view = [&](int a, int b) {
+        tridsk_ligand_batch v = *batch;
+        v.n_lig = b - a;
+        v.atom_off = batch->atom_off + a; v.tor_off = batch->tor_off + a;
+        if (batch->pair_off) v.pair_off = batch->pair_off + a;
+        if (batch->bond_off) v.bond_off = batch->bond_off + a;
+        return v;
+    };
+    tridsk_ligands* part[2] = {nullptr, nullptr};
+    auto cleanup = [&](int rc) { for (auto* p : part) if (p) tridsk_free_ligands(p); return rc; };
+    if (!batch->atom_off || !batch->tor_off) return fail(ctx, TRIDSK_EINVAL, "bad ligand batch");
+    tridsk_dock_opts o;
+    memset(&o, 0, sizeof(o));
+    if (l1 == L) {                                               // small batch: nothing to overlap
+        int rc = tridsk_load_ligands(ctx, batch, types, &part[0]);
+        if (rc) return rc;
+        rc = tridsk_dock(ctx, grid, part[0], params, box_min, box_max, pocket_center, pocket_radius, n_chains, n_steps, top_k, seed,
+                         pose_stride, out_energy, out_pose, out_chain, &o);
+        return cleanup(rc);
+    }
+    o.no_graph = 1;                                              // two launch series that run once each
+    const tridsk_ligand_batch va = view(0, l1), vb = view(l1, L);
+    int rc = tridsk_load_ligands(ctx, &va, types, &part[0]);
+    if (rc) return cleanup(rc);
+    rc = tridsk_dock(ctx, grid, part[0], params, box_min, box_max, pocket_center, pocket_radius, n_chains, n_steps, top_k, seed,
+                     pose_stride, d_e, d_p, d_c, &o);            // device outputs: enqueued, not waited for
+    if (rc) return cleanup(rc);
+    rc = tridsk_load_ligands(ctx, &vb, types, &part[1]);         // packs on the host while the first part docks
+    if (rc) return cleanup(rc);
+    o.lig_base = l1;
+    rc = tridsk_dock(ctx, grid, part[1], params, box_min, box_max, pocket_center, pocket_radius, n_chains, n_steps, top_k, seed,
+                     pose_stride, d_e + per_e * l1, d_p + per_p * l1, d_c + per_c * l1, &o);
+    if (rc) return cleanup(rc);
+    if (h_oe) CK(cudaMemcpyAsync(out_energy, d_e, sizeof(float) * per_e * L, cudaMemcpyDeviceToHost, ctx->stream));
+    if (h_op) CK(cudaMemcpyAsync(out_pose, d_p, sizeof(float) * per_p * L, cudaMemcpyDeviceToHost, ctx->stream));
+    if (h_oc) CK(cudaMemcpyAsync(out_chain, d_c, sizeof(int) * per_c * L, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));                      // the handles are released below: their kernels must be done
+    return cleanup(TRIDSK_OK);
 }
 
 // ---------------------------------------------------------------------------------------- tridsk_dock_static

@@ -180,6 +180,7 @@ struct McLaunch {
     float box_min[3], box_max[3], centre[3], radius;
     int n_chains, pose_stride;
     int chain_base;               // global id of local chain 0 in the Philox counter (multi-GPU chain sharding)
+    int lig_base;                 // global id of the handle's ligand 0 in the Philox counter (tridsk_screen docks a batch in two parts)
     unsigned long long seed;
     int first_step, n_steps;
     int init_mode;                // 0 Philox init, 1 from init_poses, 2 resume from state

@@ -724,7 +724,7 @@ __global__ void __launch_bounds__(ROUNDS ? 64 : 128, ROUNDS ? (MDN ? 4 : 8) : 3)
             cta_load_pose(a.init_poses + cidx * a.pose_stride, F, ct, cq, cth);
             quat_normalise(cq);
         } else {                            // a1 / O11: Philox initialisation; lane l computes block purpose 2 + l
-            const uint4 r = philox4x32_10(make_uint4(gchain, 0u, (uint32_t)lig, 2u + (uint32_t)lane), key);
+            const uint4 r = philox4x32_10(make_uint4(gchain, 0u, (uint32_t)(a.lig_base + lig), 2u + (uint32_t)lane), key);
             const float u0 = u01(r.x), u1 = u01(r.y), u2 = u01(r.z), u3 = u01(r.w);
             const float a0 = __shfl_sync(FULL_MASK, u0, 0), a1 = __shfl_sync(FULL_MASK, u1, 0), a2 = __shfl_sync(FULL_MASK, u2, 0);
             const float b0 = __shfl_sync(FULL_MASK, u0, 1), b1 = __shfl_sync(FULL_MASK, u1, 1), b2 = __shfl_sync(FULL_MASK, u2, 1);
@@ -758,7 +758,7 @@ __global__ void __launch_bounds__(ROUNDS ? 64 : 128, ROUNDS ? (MDN ? 4 : 8) : 3)
     for (int s = 0; s < a.n_steps; ++s) {
         const uint32_t step = (uint32_t)(a.first_step + s);
         // O10: even lanes draw the perturbation block (purpose 0), odd lanes the Metropolis block (purpose 1)
-        const uint4 r = philox4x32_10(make_uint4(gchain, step, (uint32_t)lig, (uint32_t)(lane & 1)), key);
+        const uint4 r = philox4x32_10(make_uint4(gchain, step, (uint32_t)(a.lig_base + lig), (uint32_t)(lane & 1)), key);
         const float u0 = __shfl_sync(FULL_MASK, u01(r.x), 0), u1 = __shfl_sync(FULL_MASK, u01(r.y), 0);
         const float u2 = __shfl_sync(FULL_MASK, u01(r.z), 0), u3 = __shfl_sync(FULL_MASK, u01(r.w), 0);
         const float um = __shfl_sync(FULL_MASK, u01(r.x), 1);

@@ -655,13 +655,13 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
             quat_normalise(cq);
             for (int g = 1; g <= T; ++g) THC[(g - 1) * C] = src[7 + S.frag[g].tor];
         } else {                                              // a1 / O11: Philox initialisation
-            const uint4 r2 = philox4x32_10(make_uint4(gchain, 0u, (uint32_t)lig, 2u), key);
+            const uint4 r2 = philox4x32_10(make_uint4(gchain, 0u, (uint32_t)(a.lig_base + lig), 2u), key);
             const float a0 = u01(r2.x), a1 = u01(r2.y), a2 = u01(r2.z);
             const float rr = a.radius * cbrtf(a0), zz = 2.f * a1 - 1.f, sq = sqrtf(fmaxf(1.f - zz * zz, 0.f));
             float sn, cs;
             sincosf(2.f * PI_F * a2, &sn, &cs);
             ct[0] = a.centre[0] + rr * sq * cs; ct[1] = a.centre[1] + rr * sq * sn; ct[2] = a.centre[2] + rr * zz;
-            const uint4 r3 = philox4x32_10(make_uint4(gchain, 0u, (uint32_t)lig, 3u), key);
+            const uint4 r3 = philox4x32_10(make_uint4(gchain, 0u, (uint32_t)(a.lig_base + lig), 3u), key);
             const float b0 = u01(r3.x), b1 = u01(r3.y), b2 = u01(r3.z);
             const float s1 = sqrtf(1.f - b0), s2 = sqrtf(b0);
             float sn1, cs1, sn2, cs2;
@@ -671,7 +671,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
             quat_normalise(cq);
             for (int g = 1; g <= T; ++g) {                    // torsion k takes element k % 4 of block 4 + k / 4
                 const int k = S.frag[g].tor;
-                const uint4 r = philox4x32_10(make_uint4(gchain, 0u, (uint32_t)lig, 4u + (uint32_t)(k >> 2)), key);
+                const uint4 r = philox4x32_10(make_uint4(gchain, 0u, (uint32_t)(a.lig_base + lig), 4u + (uint32_t)(k >> 2)), key);
                 const uint32_t w = (k & 3) == 0 ? r.x : (k & 3) == 1 ? r.y : (k & 3) == 2 ? r.z : r.w;
                 THC[(g - 1) * C] = PI_F * (2.f * u01(w) - 1.f);
             }
@@ -691,7 +691,7 @@ __device__ __forceinline__ void lane_chain(const McLaunch& a, const LaneTopo& S,
             uint4 r = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll 1
             for (uint32_t pz = 0; pz < 2; ++pz) {
-                const uint4 v = philox4x32_10(make_uint4(gchain, step, (uint32_t)lig, 1u - pz), key);
+                const uint4 v = philox4x32_10(make_uint4(gchain, step, (uint32_t)(a.lig_base + lig), 1u - pz), key);
                 if (pz == 0) um = u01(v.x);
                 else r = v;
             }

@@ -555,6 +555,47 @@ def test_full_size_configs_auto_mapping_sampled_against_oracle(orc, gp, name, n_
     assert np.median(en[:, 0, 0]) < 0.0                                                       # the search found bound poses
 
 
+def test_screen_in_one_call_equals_load_and_dock(gp):
+    """tridsk_screen (the batch in two parts, the second packed on the host while the first docks, lig_base carrying the global
+    ligand id into the Philox counter) returns exactly what tridsk_load_ligands + tridsk_dock return on the whole batch: host
+    and device outputs, a batch large enough for two parts and one that goes in one; and lig_base on its own."""
+    import torch
+    from paper_2510_24186_b200 import Engine
+    cfg = synth.CONFIGS["C5"]
+    rec = synth.make_receptor(cfg)
+    radius, role = synth.type_table(cfg.n_types)
+    e = Engine(0)
+    try:
+        grid = e.build_grid(rec.xyz, rec.type, radius, role, gp, rec.origin, rec.dims, rec.spacing)
+        box = (rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius)
+        for n_lig in (9000, 700):
+            batch = synth.make_ligands(cfg, n_lig)
+            stride = 7 + int(np.max(np.diff(batch.tor_off)))
+            ligs = e.load_ligands(batch, radius, role)
+            want = e.dock(grid, ligs, gp, *box, 32, 6, 2, seed=77, pose_stride=stride)
+            got = e.screen(grid, batch, radius, role, gp, *box, 32, 6, 2, seed=77, pose_stride=stride)
+            for k in ("chain", "energy", "pose"):
+                assert np.array_equal(got[k], want[k]), (n_lig, k)
+            dev = (torch.empty(n_lig, 2, 2, device=e.device), torch.empty(n_lig, 2, stride, device=e.device),
+                   torch.empty(n_lig, 2, dtype=torch.int32, device=e.device))
+            e.screen(grid, batch, radius, role, gp, *box, 32, 6, 2, seed=77, pose_stride=stride, out=dev)
+            torch.cuda.synchronize()
+            assert np.array_equal(dev[2].cpu().numpy(), want["chain"]) and np.array_equal(dev[0].cpu().numpy(), want["energy"])
+            if n_lig == 700:                                       # lig_base alone: the last 200 ligands as a batch of their own
+                sub = batch.subset(np.arange(500, 700))
+                ls = e.load_ligands(sub, radius, role)
+                e.set_kernel(2)                                    # (6,400 chains alone would go to the warp mapping: other summation order)
+                r = e.dock(grid, ls, gp, *box, 32, 6, 2, seed=77, pose_stride=stride, lig_base=500)
+                assert np.array_equal(r["energy"], want["energy"][500:]) and np.array_equal(r["pose"], want["pose"][500:])
+                r0 = e.dock(grid, ls, gp, *box, 32, 6, 2, seed=77, pose_stride=stride)
+                assert not np.array_equal(r0["energy"], want["energy"][500:])
+                e.set_kernel(0)
+                ls.free()
+            ligs.free()
+    finally:
+        e.close()
+
+
 def test_tensor_memory_lane_kernel_is_bit_identical_to_shared_memory_lane_kernel(gp):
     """Mapping 4 keeps the chains' coordinates in tensor memory (tcgen05.st / tcgen05.ld) instead of shared memory; the
     arithmetic and its order are those of mapping 2, so a screen gives bit-identical energies, poses and chain ids."""
