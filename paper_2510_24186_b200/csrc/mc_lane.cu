@@ -261,17 +261,18 @@ template <bool MDN, class XS>
 __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, float k_wall, bool grad, float wscale,
                                            const MdnDev& M, const float4* __restrict__ mdn_par, const XS& X, float* __restrict__ WR) {
     constexpr int C = XS::kC;
+    constexpr int GD = MDN ? 1 : LANE_GD;                       // with the term: one copy of mdn_atom, and its registers
     const LaneGridK Q = {-G.ox * G.inv_h, -G.oy * G.inv_h, -G.oz * G.inv_h};
     float e_inter = 0.f;
     float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     int gcur = 0;
     const int n = S.n;
-    float x[LANE_GD], y[LANE_GD], z[LANE_GD];
-    int m[LANE_GD];
-    LaneCell c[LANE_GD];
-    float4 lo[LANE_GD], hi[LANE_GD];
+    float x[GD], y[GD], z[GD];
+    int m[GD];
+    LaneCell c[GD];
+    float4 lo[GD], hi[GD];
 #pragma unroll
-    for (int k = 0; k < LANE_GD - 1; ++k) {                    // prologue: atoms 0 .. LANE_GD-2 (the tail repeats the last atom)
+    for (int k = 0; k < GD - 1; ++k) {                    // prologue: atoms 0 .. GD-2 (the tail repeats the last atom)
         const int a = min(k, n - 1);
         m[k] = S.meta[a];
         X.get(XS::kScale * (uint32_t)a, x[k], y[k], z[k]);
@@ -279,12 +280,12 @@ __device__ __forceinline__ float lane_grid(const LaneTopo& S, const DGrid& G, fl
         c[k] = lane_locate(G, Q, m[k] & 0xff, x[k], y[k], z[k]);
         ldg_cell(c[k].p, lo[k], hi[k]);
     }
-    for (int a0 = 0; a0 < n; a0 += LANE_GD) {
+    for (int a0 = 0; a0 < n; a0 += GD) {
 #pragma unroll
-        for (int k = 0; k < LANE_GD; ++k) {
-            {                                                   // request atom a0 + k + LANE_GD - 1 into the slot freed last
-                constexpr int D1 = LANE_GD - 1;
-                const int sl = (k + D1) % LANE_GD;
+        for (int k = 0; k < GD; ++k) {
+            {                                                   // request atom a0 + k + GD - 1 into the slot freed last
+                constexpr int D1 = GD - 1;
+                const int sl = (k + D1) % GD;
                 const int a = min(a0 + k + D1, n - 1);
                 m[sl] = S.meta[a];
                 X.get(XS::kScale * (uint32_t)a, x[sl], y[sl], z[sl]);
