@@ -1355,7 +1355,12 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     // tridsk_set_kernel overrides.
     int mode = ctx->kernel;
     if (mode == 0) {
-        if (nch >= (size_t)ctx->sm_count * 44) mode = 2;            // measured crossover with the warp form: ~43 chains per SM (16 C2 docks)
+        // batches of ligands above 64 atoms only: the CTA kernel's dense-sweep instance (two warps per chain) beats the warp form at
+        // every size and the lane form up to ~80 chains per SM (80-atom docks of 1,024 chains, 2 / 4 / 8 / 12 at once: CTA 107 / 207 /
+        // 394 / 586 ms, warp 413 / 632 / - / -, lane - / - / 565 / 566)
+        const bool all_dense = ligs->has_cta && ligs->cta_bucket[0].empty() && !ligs->cta_bucket[1].empty();
+        if (all_dense) mode = nch <= (size_t)ctx->sm_count * 76 ? 3 : 2;
+        else if (nch >= (size_t)ctx->sm_count * 44) mode = 2;       // measured crossover with the warp form: ~43 chains per SM (16 C2 docks)
         else if (ligs->has_cta && nch <= (size_t)ctx->sm_count * 8) mode = 3;
         else mode = 1;
     }
