@@ -823,7 +823,7 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
         nls += pk[i].lane_stream.size(); nrec += pk[i].lane_recs.size();
         ncr += pk[i].cta_rows.size(); ncc += pk[i].cta_recs.size(); nrt += pk[i].cta_rtab.size();
         lg->hdr_h[i] = h; lg->n_pairs[i] = h.n_pairs;
-        lg->max_atoms = std::max(lg->max_atoms, h.n); lg->max_tor = std::max(lg->max_tor, h.T);
+        lg->max_atoms = std::max(lg->max_atoms, h.n); lg->max_tor = std::max(lg->max_tor, h.T); lg->min_atoms = std::min(lg->min_atoms, h.n);
         lg->bucket[h.J].push_back(i);
         if (want_cta) {
             int th, lpa;
@@ -1360,6 +1360,10 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         // 394 / 586 ms, warp 413 / 632 / - / -, lane - / - / 565 / 566)
         const bool all_dense = ligs->has_cta && ligs->cta_bucket[0].empty() && !ligs->cta_bucket[1].empty();
         if (all_dense) mode = nch <= (size_t)ctx->sm_count * 76 ? 3 : 2;
+        // batches without a ligand of 32 atoms or fewer: the warp form (two or more atoms per lane) is never the fastest; the CTA form
+        // until the lane form's latency floor is reached (384-chain docks, 500 steps, 1 / 4 / 16 at once: 48 atoms CTA 3.6 / 13.3 / 49 ms,
+        // warp 16.7 / 18.2 / 72, lane 51 / 52 / 54; 64 atoms CTA 4.5 / 17.2 / 63, warp 19.8 / 24.0 / 94, lane 79 / 87 / 91)
+        else if (ligs->has_cta && ligs->min_atoms > 32) mode = nch <= (size_t)ctx->sm_count * 40 ? 3 : 2;
         else if (nch >= (size_t)ctx->sm_count * 44) mode = 2;       // measured crossover with the warp form: ~43 chains per SM (16 C2 docks)
         else if (ligs->has_cta && nch <= (size_t)ctx->sm_count * 8) mode = 3;
         else mode = 1;

@@ -335,7 +335,7 @@ struct tridsk_grid {
 
 struct tridsk_ligands {
     tridsk_ctx* ctx;
-    int n_lig = 0, max_atoms = 0, max_tor = 0;
+    int n_lig = 0, max_atoms = 0, max_tor = 0, min_atoms = 1 << 30;
     std::vector<LigHdr> hdr_h;
     std::vector<int> n_pairs;
     std::vector<int> bucket[TRIDSK_MAX_J + 1];   // ligand ids per J
