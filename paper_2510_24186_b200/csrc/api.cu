@@ -1361,8 +1361,8 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         const bool all_dense = ligs->has_cta && ligs->cta_bucket[0].empty() && !ligs->cta_bucket[1].empty();
         if (all_dense) mode = nch <= (size_t)ctx->sm_count * 76 ? 3 : 2;
         // batches without a ligand of 32 atoms or fewer: the warp form (two or more atoms per lane) is never the fastest; the CTA form
-        // until the lane form's latency floor is reached (384-chain docks, 500 steps, 1 / 4 / 16 at once: 48 atoms CTA 3.6 / 13.3 / 49 ms,
-        // warp 16.7 / 18.2 / 72, lane 51 / 52 / 54; 64 atoms CTA 4.5 / 17.2 / 63, warp 19.8 / 24.0 / 94, lane 79 / 87 / 91)
+        // until the lane form's latency floor is reached (384-chain docks, 500 steps, 48 atoms, 2 / 4 / 16 at once: CTA 7.0 / 13.3 / 49 ms,
+        // warp 16.7 / 18.2 / 72, lane 51 / 52 / 54; 64 atoms, 1 / 4 / 16 at once: CTA 4.5 / 17.2 / 63, warp 19.8 / 24.0 / 94, lane 79 / 87 / 91)
         else if (ligs->has_cta && ligs->min_atoms > 32) mode = nch <= (size_t)ctx->sm_count * 40 ? 3 : 2;
         else if (nch >= (size_t)ctx->sm_count * 44) mode = 2;       // measured crossover with the warp form: ~43 chains per SM (16 C2 docks)
         else if (ligs->has_cta && nch <= (size_t)ctx->sm_count * 8) mode = 3;
