@@ -1365,7 +1365,7 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         // warp 16.7 / 18.2 / 72, lane 51 / 52 / 54; 64 atoms, 1 / 4 / 16 at once: CTA 4.5 / 17.2 / 63, warp 19.8 / 24.0 / 94, lane 79 / 87 / 91)
         else if (ligs->has_cta && ligs->min_atoms > 32) mode = nch <= (size_t)ctx->sm_count * 40 ? 3 : 2;
         else if (nch >= (size_t)ctx->sm_count * 44) mode = 2;       // measured crossover with the warp form: ~43 chains per SM (16 C2 docks)
-        else if (ligs->has_cta && nch <= (size_t)ctx->sm_count * 8) mode = 3;
+        else if (ligs->has_cta && nch <= (size_t)ctx->sm_count * 5) mode = 3;   // small ligands: the warp form catches up at two 384-chain docks
         else mode = 1;
     }
     if (mode == 3) {
