@@ -736,7 +736,7 @@ static void pack_ligand(const tridsk_ligand_batch* b, const tridsk_types* types,
                     out.cta_recs.push_back(make_uint2((unsigned)x | ((unsigned)y << 8) | (hbq(x, y) ? 0x10000u : 0u),
                                                       fbits(out.f4[x].w + out.f4[y].w)));
         if ((int)out.cta_recs.size() != 3 * P) return bad(TRIDSK_EINVAL, "internal: CTA pair records do not cover the pair set");
-        if (n > TRIDSK_CTA_ROUNDS_N) {                        // round table (internal.h): item l of round k = pair (l, (l + k) mod n)
+        if (n > TRIDSK_CTA_DENSE_MIN) {                       // round table (internal.h): item l of round k = pair (l, (l + k) mod n)
             const int nr = n / 2;
             out.cta_rtab.assign((size_t)nr * n, -1.f);
             int cov = 0;
@@ -828,9 +828,11 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
         if (want_cta) {
             int th, lpa;
             cta_shape(h.n, &th, &lpa);
-            const int k = h.n > TRIDSK_CTA_ROUNDS_N ? 1 : 0;       // bucket 1: the dense-sweep instance of the kernel
-            lg->cta_bucket[k].push_back(i);
-            lg->cta_smem[k] = std::max(lg->cta_smem[k], cta_layout(h.n, h.T, h.n_pairs).total);
+            for (int v = 0; v < 2; ++v) {                       // bucket 1: the dense-sweep instance of the kernel
+                const int k = h.n > (v ? TRIDSK_CTA_DENSE_MIN : TRIDSK_CTA_ROUNDS_N) ? 1 : 0;
+                lg->cta_bucket[v][k].push_back(i);
+                lg->cta_smem[v][k] = std::max(lg->cta_smem[v][k], cta_layout(h.n, h.T, h.n_pairs, k == 1).total);
+            }
         }
     }
     // One pinned staging block owned by the ctx (grown on demand, reused by later calls) and one device block hold all the
@@ -889,7 +891,8 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
         if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(*d, src, bytes, cudaMemcpyHostToDevice, ctx->stream);
     };
     for (int k = 0; k < 2; ++k)
-        if (!lg->cta_bucket[k].empty()) up((void**)&lg->cta_bucket_dev[k], lg->cta_bucket[k].data(), sizeof(int) * lg->cta_bucket[k].size());
+        for (int v = 0; v < 2; ++v)
+            if (!lg->cta_bucket[v][k].empty()) up((void**)&lg->cta_bucket_dev[v][k], lg->cta_bucket[v][k].data(), sizeof(int) * lg->cta_bucket[v][k].size());
     if (e == cudaSuccess) e = cudaMalloc((void**)&lg->all_ids, sizeof(int) * std::max(L, 1));
     for (int j = 1; j <= TRIDSK_MAX_J; ++j)
         if (!lg->bucket[j].empty()) up((void**)&lg->bucket_dev[j], lg->bucket[j].data(), sizeof(int) * lg->bucket[j].size());
@@ -1029,7 +1032,7 @@ extern "C" void tridsk_free_ligands(tridsk_ligands* l) {
     if (!l) return;                 // cudaFree waits for the device; l->ctx may already be destroyed
     free_mdn(l);
     cudaFree(l->blob); cudaFree(l->all_ids);       // the packed arrays are pieces of one block
-    for (int k = 0; k < 2; ++k) if (l->cta_bucket_dev[k]) cudaFree(l->cta_bucket_dev[k]);
+    for (int v = 0; v < 2; ++v) for (int k = 0; k < 2; ++k) if (l->cta_bucket_dev[v][k]) cudaFree(l->cta_bucket_dev[v][k]);
     for (int j = 0; j <= TRIDSK_MAX_J; ++j) if (l->bucket_dev[j]) cudaFree(l->bucket_dev[j]);
     delete l;
 }
@@ -1112,7 +1115,7 @@ extern "C" int tridsk_score_grad(tridsk_ctx* ctx, const tridsk_grid* grid, const
         CK(launch_score_lane(ctx->stream, a, ns, smem));
     } else if (ctx->kernel == 3) {
         if (!ligs->has_cta) return fail(ctx, TRIDSK_EINVAL, "the CTA-per-chain mapping needs a ligand batch of at most 1024 ligands");
-        const size_t smem = std::max(ligs->cta_smem[0], ligs->cta_smem[1]);
+        const size_t smem = std::max(ligs->cta_smem[0][0], ligs->cta_smem[0][1]);
         if (smem > TRIDSK_SMEM_MAX_CTA) return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
         CK(launch_score_cta(ctx->stream, a, smem));
     } else {
@@ -1358,21 +1361,27 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         // batches of ligands above 64 atoms only: the CTA kernel's dense-sweep instance (two warps per chain) beats the warp form at
         // every size and the lane form up to ~80 chains per SM (80-atom docks of 1,024 chains, 2 / 4 / 8 / 12 at once: CTA 107 / 207 /
         // 394 / 586 ms, warp 413 / 632 / - / -, lane - / - / 565 / 566)
-        const bool all_dense = ligs->has_cta && ligs->cta_bucket[0].empty() && !ligs->cta_bucket[1].empty();
+        const bool all_dense = ligs->has_cta && ligs->cta_bucket[0][0].empty() && !ligs->cta_bucket[0][1].empty();
         if (all_dense) mode = nch <= (size_t)ctx->sm_count * 76 ? 3 : 2;
         // batches without a ligand of 32 atoms or fewer: the warp form (two or more atoms per lane) is never the fastest; the CTA form
         // until the lane form's latency floor is reached (384-chain docks, 500 steps, 48 atoms, 2 / 4 / 16 at once: CTA 7.0 / 13.3 / 49 ms,
         // warp 16.7 / 18.2 / 72, lane 51 / 52 / 54; 64 atoms, 1 / 4 / 16 at once: CTA 4.5 / 17.2 / 63, warp 19.8 / 24.0 / 94, lane 79 / 87 / 91)
-        else if (ligs->has_cta && ligs->min_atoms > 32) mode = nch <= (size_t)ctx->sm_count * 40 ? 3 : 2;
+        // (with the dense sweep for 33 .. 64 atoms beyond 3 chains per SM, 16 docks at once: 48 atoms 35.9 ms, 64 atoms 52.0 ms)
+        else if (ligs->has_cta && ligs->min_atoms > 32) mode = nch <= (size_t)ctx->sm_count * 60 ? 3 : 2;
         else if (nch >= (size_t)ctx->sm_count * 44) mode = 2;       // measured crossover with the warp form: ~43 chains per SM (16 C2 docks)
         else if (ligs->has_cta && nch <= (size_t)ctx->sm_count * 5) mode = 3;   // small ligands: the warp form catches up at two 384-chain docks
         else mode = 1;
     }
     if (mode == 3) {
         if (!ligs->has_cta) return fail(ctx, TRIDSK_EINVAL, "the CTA-per-chain mapping needs a ligand batch of at most 1024 ligands");
-        if (std::max(ligs->cta_smem[0], ligs->cta_smem[1]) > TRIDSK_SMEM_MAX_CTA)
-            return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
+        for (int v = 0; v < 2; ++v)
+            if (std::max(ligs->cta_smem[v][0], ligs->cta_smem[v][1]) > TRIDSK_SMEM_MAX_CTA)
+                return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
     }
+    // CTA form: which ligands take the dense sweep (two warps per chain) -- with more chains than the SMs hold at once (3 record-
+    // instance CTAs each) also those of 33 .. 64 atoms
+    const int cv = nch > (size_t)ctx->sm_count * 3 ? 1 : 0;
+    base.cta_dense_n = cv ? TRIDSK_CTA_DENSE_MIN : TRIDSK_CTA_ROUNDS_N;
     if (o.receptor_direct) {                                        // direct pair sums: the CTA- and the warp-per-chain kernels carry that path
         if (!grid->rd.atoms) return fail(ctx, TRIDSK_EINVAL, "receptor_direct needs tridsk_grid_attach_receptor on this grid");
         if (mode != 3 || ligs->mdn.n_res > 0) mode = 1;             // (the CTA instances with direct sums leave out E_MDN)
@@ -1407,11 +1416,11 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
             }
         } else if (mode == 3) {
             for (int k = 0; k < 2; ++k) {
-                if (ligs->cta_bucket[k].empty()) continue;
+                if (ligs->cta_bucket[cv][k].empty()) continue;
                 McLaunch a = base;
-                a.lig_list = ligs->cta_bucket_dev[k]; a.n_list = (int)ligs->cta_bucket[k].size();
+                a.lig_list = ligs->cta_bucket_dev[cv][k]; a.n_list = (int)ligs->cta_bucket[cv][k].size();
                 fill(a);
-                series.push_back({3, k, ligs->cta_smem[k], k, a});
+                series.push_back({3, k, ligs->cta_smem[cv][k], k, a});
             }
         } else {
             for (int j = 1; j <= TRIDSK_MAX_J; ++j) {
@@ -1679,9 +1688,10 @@ extern "C" int tridsk_dock_static(tridsk_ctx* ctx, const tridsk_grid* grid, cons
     const int L = ligs->n_lig;
     if (L == 0) return TRIDSK_OK;
     if (!ligs->has_cta) return fail(ctx, TRIDSK_ELIMIT, "tridsk_dock_static needs a ligand batch of at most 1024 ligands (CTA-per-chain pair format)");
-    if (std::max(ligs->cta_smem[0], ligs->cta_smem[1]) > TRIDSK_SMEM_MAX_CTA)
-        return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
     const size_t nch = (size_t)L * n_chains, n_pose_f = nch * pose_stride;
+    const int cv = nch > (size_t)ctx->sm_count * 3 ? 1 : 0;          // as tridsk_dock: which ligands take the dense sweep
+    if (std::max(ligs->cta_smem[cv][0], ligs->cta_smem[cv][1]) > TRIDSK_SMEM_MAX_CTA)
+        return fail(ctx, TRIDSK_ELIMIT, "ligand does not fit the CTA kernel's shared memory");
     const size_t state_bytes = sizeof(float) * (2 * n_pose_f + 2 * nch);
     if (state_bytes > TRIDSK_STATIC_SCRATCH_BYTES)
         return fail(ctx, TRIDSK_ELIMIT, "tridsk_dock_static: the chain state of " + std::to_string(nch) + " chains x pose_stride " +
@@ -1702,13 +1712,14 @@ extern "C" int tridsk_dock_static(tridsk_ctx* ctx, const tridsk_grid* grid, cons
     base.radius = pocket_radius;
     base.n_chains = n_chains; base.pose_stride = pose_stride; base.seed = seed;
     base.pose_cur = state; base.pose_best = state + n_pose_f; base.e_cur = state + 2 * n_pose_f; base.e_best = state + 2 * n_pose_f + nch;
+    base.cta_dense_n = cv ? TRIDSK_CTA_DENSE_MIN : TRIDSK_CTA_ROUNDS_N;
     base.first_step = 0; base.n_steps = n_steps; base.init_mode = 0;             // a1: Philox initialisation writes every chain's state
     ctx->last_kernel = 3;
     for (int k = 0; k < 2; ++k) {                                                // the two instances of the CTA kernel (internal.h)
-        if (ligs->cta_bucket[k].empty()) continue;
+        if (ligs->cta_bucket[cv][k].empty()) continue;
         McLaunch a = base;
-        a.lig_list = ligs->cta_bucket_dev[k]; a.n_list = (int)ligs->cta_bucket[k].size();
-        CK(launch_mc_cta(ctx->stream, a, k, ligs->cta_smem[k]));
+        a.lig_list = ligs->cta_bucket_dev[cv][k]; a.n_list = (int)ligs->cta_bucket[cv][k].size();
+        CK(launch_mc_cta(ctx->stream, a, k, ligs->cta_smem[cv][k]));
         ctx->launches += 1;
     }
     if (top_k > 0) {

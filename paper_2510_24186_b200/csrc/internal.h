@@ -142,7 +142,9 @@ struct LaneRec {
 // donor/acceptor flag, or -1 if the pair is not in the set (for even n the items l >= n/2 of round n/2 repeat pairs and are
 // absent).  The MC kernel gives such a chain TWO warps (64-thread CTAs, two atoms per thread outside the sweep), so that eight
 // chains stay resident per SM.
-#define TRIDSK_CTA_ROUNDS_N 64         // ligands above this many atoms use the dense partner sweep
+#define TRIDSK_CTA_ROUNDS_N 64         // ligands above this many atoms always use the dense partner sweep (two warps per chain)
+#define TRIDSK_CTA_DENSE_MIN 32        // ... and those above this many when the dock has more chains than the SMs hold at once (throughput
+                                       // over latency: 48 atoms, 4 x 384 chains 13.3 -> 11.2 ms, but one dock of 64 atoms 4.5 -> 7.3 ms)
 
 // Per-fragment record; fragment 0 is the root, fragment k+1 hangs off torsion k.
 struct FragRec {
@@ -181,6 +183,7 @@ struct McLaunch {
     int n_chains, pose_stride;
     int chain_base;               // global id of local chain 0 in the Philox counter (multi-GPU chain sharding)
     int lig_base;                 // global id of the handle's ligand 0 in the Philox counter (tridsk_screen docks a batch in two parts)
+    int cta_dense_n;              // CTA kernel: ligands above this many atoms take the dense partner sweep
     unsigned long long seed;
     int first_step, n_steps;
     int init_mode;                // 0 Philox init, 1 from init_poses, 2 resume from state
@@ -260,10 +263,9 @@ __host__ __device__ static inline int lane_chain_slots(int n, int T, int max_dep
 struct CtaLayout { size_t ref, meta, frag, rows, recs, tt, masks, part, X, AF, PF, red, total; };
 #define TRIDSK_AL16(x) (((x) + 15) / 16 * 16)
 #define TRIDSK_CTA_WARPS 4             // the most warps a CTA kernel runs (score kernel, record instance: 128 threads)
-__host__ __device__ static inline CtaLayout cta_layout(int n, int T, int n_pairs) {
+__host__ __device__ static inline CtaLayout cta_layout(int n, int T, int n_pairs, bool dense) {
     CtaLayout L;
     size_t o = 0;
-    const bool dense = n > TRIDSK_CTA_ROUNDS_N;                    // dense partner sweep: no pair records
     const size_t npad = ((size_t)n + 31) / 32 * 32;
     L.ref = o; o += 16 * (size_t)n;
     L.meta = o; o = TRIDSK_AL16(o + 4 * (size_t)n);
@@ -352,9 +354,12 @@ struct tridsk_ligands {
     int* cta_rows = nullptr;
     uint2* cta_recs = nullptr;
     float* cta_rtab = nullptr;
-    std::vector<int> cta_bucket[2];              // ligand ids: [0] up to 64 atoms (row form), [1] above (dense partner sweep)
-    int* cta_bucket_dev[2] = {nullptr, nullptr};
-    size_t cta_smem[2] = {0, 0};                 // largest shared-memory need per bucket
+    // ligand ids by instance of the CTA kernel, [v][k]: k = 0 pair records, 1 dense partner sweep; v = which ligands are dense:
+    // v = 0 those above TRIDSK_CTA_ROUNDS_N atoms (single docks: latency), v = 1 those above TRIDSK_CTA_DENSE_MIN (more chains
+    // than the SMs hold at once: throughput)
+    std::vector<int> cta_bucket[2][2];
+    int* cta_bucket_dev[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
+    size_t cta_smem[2][2] = {{0, 0}, {0, 0}};    // largest shared-memory need per bucket
     int* all_ids = nullptr;       // 0..n_lig-1 re-ordered per lane bucket (refilled when the plan key changes)
     struct LaneBucket { int chains_per_cta; size_t smem; int first, count; int tm_cols; long long work = 0; int minb = 3; };   // tm_cols > 0: tensor-memory form, smem = bytes per warp
     std::vector<LaneBucket> lane_plan;

@@ -45,9 +45,11 @@ struct CtaFrag {
 __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char* smem, const LigHdr* __restrict__ h,
                                           const float4* __restrict__ atom_f4, const int* __restrict__ atom_i,
                                           const LaneFrag* __restrict__ lane_frags, const int* __restrict__ cta_rows,
-                                          const uint2* __restrict__ cta_recs, const float* __restrict__ cta_rtab, const DParams& P) {
+                                          const uint2* __restrict__ cta_recs, const float* __restrict__ cta_rtab, const DParams& P,
+                                          int dense_n) {
     const int n = h->n, T = h->T, np = h->n_pairs, tid = threadIdx.x, nt = blockDim.x, lane = tid & 31;
-    const CtaLayout L = cta_layout(n, T, np);
+    const bool rounds = n > dense_n;                             // dense partner sweep (internal.h)
+    const CtaLayout L = cta_layout(n, T, np, rounds);
     float4* ref = reinterpret_cast<float4*>(smem + L.ref);
     int* meta = reinterpret_cast<int*>(smem + L.meta);
     int* frag = reinterpret_cast<int*>(smem + L.frag);
@@ -64,7 +66,6 @@ __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char*
         }
     }
     for (int i = tid; i <= n; i += nt) rows[i] = __ldg(cta_rows + h->cta_row_off + i);
-    const bool rounds = n > TRIDSK_CTA_ROUNDS_N;
     S.tt = nullptr; S.msk = nullptr; S.part = nullptr; S.X4 = nullptr; S.npad = 0;
     if (!rounds) {
         for (int i = tid; i < 3 * np; i += nt) {
@@ -700,7 +701,7 @@ __global__ void __launch_bounds__(ROUNDS ? 64 : 128, ROUNDS ? (MDN ? 4 : 8) : 3)
     const LigHdr* h = a.hdr + lig;
     CtaTopo S;
     CtaFrag F;
-    cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.cta_rtab, a.P);
+    cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.cta_rtab, a.P, a.cta_dense_n);
     const DParams& P = a.P;
     const PairK K = make_pairk(P);
     const float4* mdn_par = MDN ? a.mdn.par + a.mdn.lig_off[lig] : nullptr;
@@ -842,7 +843,7 @@ __global__ void __launch_bounds__(128) score_cta_kernel(const ScoreLaunch a) {
     const LigHdr* h = a.hdr + lig;
     CtaTopo S;
     CtaFrag F;
-    cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.cta_rtab, a.P);
+    cta_stage(S, F, cta_smem, h, a.atom_f4, a.atom_i, a.lane_frags, a.cta_rows, a.cta_recs, a.cta_rtab, a.P, TRIDSK_CTA_ROUNDS_N);
     const PairK K = make_pairk(a.P);
     const float4* mdn_par = MDN ? a.mdn.par + a.mdn.lig_off[lig] : nullptr;
     const int atom = tid / S.lpa, part = tid % S.lpa;

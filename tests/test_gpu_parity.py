@@ -555,6 +555,45 @@ def test_full_size_configs_auto_mapping_sampled_against_oracle(orc, gp, name, n_
     assert np.median(en[:, 0, 0]) < 0.0                                                       # the search found bound poses
 
 
+def test_cta_mapping_dense_sweep_for_mid_size_ligands_when_chains_exceed_the_sms(orc, gp):
+    """CTA-per-chain mapping with more chains than the SMs hold at once: ligands of 33 .. 64 atoms then take the dense partner
+    sweep (two warps per chain) instead of the pair records; smaller ones keep the records, larger ones the sweep.  Per-chain
+    initial energies and the returned poses of a short dock are re-scored by the oracle, and the two instances agree with
+    each other on the initial energies to fp32 summation order."""
+    from paper_2510_24186_b200 import Engine, split_state
+    rec = synth.receptor(300, 20.0, 16, seed=1001, grid_n=54)
+    radius, role = synth.type_table(16)
+    ty, p = orc.Types(radius, role), orc.default_params()
+    G = orc.build_grid(p, ty, rec.xyz, rec.type, rec.origin, rec.dims, rec.spacing)
+    batch = synth.ligands([20, 33, 48, 64, 65], [3, 6, 9, 12, 12], 16, seed=909)
+    Ls = [orc.ligand_from_batch(batch, l) for l in range(batch.n_lig)]
+    box = (rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius)
+    e = Engine(0)
+    try:
+        e.set_kernel(3)
+        grid = e.grid_from_values(G.g, rec.origin, rec.spacing)
+        ligs = e.load_ligands(batch, radius, role)
+        stride = 7 + ligs.max_tor
+        n_many, n_few = 160, 16                                      # 5 x 160 = 800 chains > 3 per SM; 5 x 16 = 80 are not
+        init = e.dock(grid, ligs, gp, *box, n_many, 0, 1, seed=41, want_state=True)
+        pc, _, ec, _ = split_state(init["state"], batch.n_lig, n_many, stride)
+        few = e.dock(grid, ligs, gp, *box, n_few, 0, 1, seed=41, want_state=True)
+        _, _, ec_few, _ = split_state(few["state"], batch.n_lig, n_few, stride)
+        for l, L in enumerate(Ls):
+            for c in (0, 7, 15, 100, 159):
+                eo = orc.score_grad(p, ty, G, L, pc[l, c, :7 + L.T].astype(np.float64), want_grad=False)[0][0]
+                assert close(ec[l, c], eo, rtol=1e-4, atol=1e-3), (L.n, c, ec[l, c], eo)
+            assert close(ec[l, :n_few], ec_few[l], rtol=1e-5, atol=1e-3), L.n     # same chains, the other instance for 33 .. 64 atoms
+        r = e.dock(grid, ligs, gp, *box, n_many, 12, 3, seed=41)
+        assert e.last_kernel() == 3
+        for l, L in enumerate(Ls):
+            for k in range(3):
+                eo = orc.score_grad(p, ty, G, L, r["pose"][l, k, :7 + L.T].astype(np.float64), want_grad=False)[0][0]
+                assert close(r["energy"][l, k, 0], eo, rtol=2e-4, atol=2e-3), (L.n, k)
+    finally:
+        e.close()
+
+
 def test_screen_in_one_call_equals_load_and_dock(gp):
     """tridsk_screen (the batch in two parts, the second packed on the host while the first docks, lig_base carrying the global
     ligand id into the Philox counter) returns exactly what tridsk_load_ligands + tridsk_dock return on the whole batch: host
