@@ -69,6 +69,9 @@ __device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __rest
 // One ligand atom (internal index p of a ligand with n atoms) at (x, y, z) against residues i0, i0 + istep, ...
 // par = the ligand's parameter block [n_res][n] of slots (M.K4 float4 each).
 // e += w_mdn * (this atom's share of E_MDN); grad: (gx, gy, gz) += its gradient.
+// PIPE = false: the parameter block is requested when its run comes up (one buffer instead of two: for the instances whose
+// register budget cannot hold both).
+template <bool PIPE = true>
 __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restrict__ par, int n, int p, float x, float y, float z,
                                          int i0, int istep, bool grad, float& e, float& gx, float& gy, float& gz) {
     // the cell of the atom streams every receptor atom it can be within d_cut of, sorted by residue (outside the grid: none)
@@ -93,14 +96,15 @@ __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restri
     float cur[32], nxt[32];
     mdn_ldg2(M.cell_at + e0, a, a2);
     int hdr = __float_as_int(a.w);
-    mdn_load_block(par + ((size_t)(hdr & 0xffff) * n + p) * M.K4, nch0, cur);
+    if (PIPE) mdn_load_block(par + ((size_t)(hdr & 0xffff) * n + p) * M.K4, nch0, cur);
     auto step = [&](const float4& ra, const float4& ra2, const float (&rc)[32], float4& na, float4& na2, float (&nc)[32]) {
         const int i = hdr & 0xffff, cnt = hdr >> 16;             // cnt is even
         const float4* q = par + ((size_t)i * n + p) * M.K4;
         const int nh = __float_as_int(ra2.w);                    // the next run's header
+        if (!PIPE) mdn_load_block(q, nch0, nc);                 // (nc and rc are the same buffer then)
         if (nh >= 0) {
             mdn_ldg2(M.cell_at + en + cnt, na, na2);
-            mdn_load_block(par + ((size_t)(nh & 0xffff) * n + p) * M.K4, nch0, nc);
+            if (PIPE) mdn_load_block(par + ((size_t)(nh & 0xffff) * n + p) * M.K4, nch0, nc);
         }
         float bx = x - ra.x, by = y - ra.y, bz = z - ra.z;
         float best2 = bx * bx + by * by + bz * bz;
@@ -123,9 +127,9 @@ __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restri
         en += cnt; hdr = nh; ++ord;
     };
     for (;;) {
-        step(a, a2, cur, b, b2, nxt);
+        step(a, a2, cur, b, b2, PIPE ? nxt : cur);
         if (en >= e1) break;
-        step(b, b2, nxt, a, a2, cur);
+        step(b, b2, PIPE ? nxt : cur, a, a2, cur);
         if (en >= e1) break;
     }
 }
