@@ -35,7 +35,7 @@ UNIT = "score+grad pose evals/s"
 KERNEL_NAMES = {1: "mc_kernel<J> (warp per chain)", 2: "mc_lane_kernel (lane per chain)", 3: "mc_cta_kernel (CTA per chain)",
                 4: "mc_lane_tm_kernel (lane per chain, TMEM)"}
 REGIME = {"C1": "latency", "C2": "latency", "C3": "throughput", "C4": "throughput", "C5": "throughput", "C2x32": "throughput",
-          "P1": "latency", "M3": "throughput", "D2": "latency"}
+          "P1": "latency", "M3": "throughput", "D2": "latency", "M2": "latency"}
 MB_FFMA, MB_FFMA2, MB_MUFU, MB_L2_READ, MB_GATHER = range(5)
 
 
@@ -220,6 +220,7 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
         res_xyz, res_off = synth.pocket_residues(rec)
         pi, mu, sg = synth.gmm_batch(len(res_off) - 1, np.diff(batch.atom_off), cfg.mdn_K, seed=cfg.lig_seed + 50000)
         eng.load_mdn(ligs, res_xyz, res_off, pi, mu, sg, cfg.mdn_K)
+        mdn_host = (res_xyz, res_off, pi, mu, sg) if do_e2e else None       # the end-to-end leg attaches the term again
         del pi, mu, sg
         mdn = dict(K=cfg.mdn_K, n_res=len(res_off) - 1, res_size=float(np.mean(np.diff(res_off))))
     w = work_of(np.diff(batch.atom_off), np.diff(batch.tor_off), ligs.n_pairs, n_chains, cfg.n_steps, gp.n_refine)   # evaluation counts
@@ -340,11 +341,15 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
 
         def e2e_step():
             grid = eng.build_grid(h_xyz, h_typ, radius, role, gp, rec.origin, rec.dims, rec.spacing)
+            if cfg.direct:
+                eng.attach_receptor(grid, h_xyz, h_typ, radius, role, gp)
             if one_call:
                 eng.screen(grid, batch, radius, role, *dock_args, seed=cfg.philox_seed, pose_stride=stride, out=h_out)
             else:
                 lg = eng.load_ligands(batch, radius, role)
-                eng.dock(grid, lg, *dock_args, seed=cfg.philox_seed, pose_stride=stride, out=h_out, chain_base=chain_base)
+                if cfg.mdn_K:
+                    eng.load_mdn(lg, *mdn_host, cfg.mdn_K)
+                eng.dock(grid, lg, *dock_args, seed=cfg.philox_seed, pose_stride=stride, out=h_out, chain_base=chain_base, **dock_kw)
                 lg.free()
             grid.free()
         e2e_step()                                                           # two untimed passes: the first one also pays first-touch
@@ -365,11 +370,14 @@ def run_workload(eng, name, steps, warmup, rank=0, world=1, do_e2e=True, sample_
             e2e_s = float(tt[0])
         h2d = rec.xyz.nbytes + rec.type.nbytes + sum(getattr(batch, f).nbytes for f in (
             "atom_off", "ref_xyz", "atom_type", "atom_frag", "tor_off", "tor_a", "tor_b", "tor_parent", "bond_off", "bond_ab"))
+        if cfg.mdn_K:
+            h2d += sum(np.asarray(a).nbytes for a in mdn_host)
         res["e2e"] = dict(value=sg_all / e2e_s, unit=UNIT, h2d_bytes_per_step=int(h2d),
                           d2h_bytes_per_step=int(sum(a.nbytes for a in h_out)), ms_per_step=e2e_s * 1e3, steps=n_e2e,
                           note=("tridsk_build_grid + tridsk_screen (host packing of the batch, upload, dock, results to host buffers; the packing of most "
                                 "of the batch overlaps the docking of its first part)" if one_call else
-                                "tridsk_load_ligands (host packing of the batch + upload) + tridsk_build_grid + tridsk_dock with host buffers"))
+                                "tridsk_load_ligands (host packing of the batch + upload)" + (" + tridsk_load_mdn" if cfg.mdn_K else "") +
+                                " + tridsk_build_grid + tridsk_dock with host buffers"))
         assert np.array_equal(h_out[2], out[2].cpu().numpy()), "e2e and device-resident legs disagree"
     ligs.free()
     return res

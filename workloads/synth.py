@@ -252,6 +252,10 @@ CONFIGS = {
     # 8(f) NEXT-1), with synthetic mixture parameters (K = 10) on the pocket residues (pocket_residues below).
     "M3": Config("M3", "Screening batch under the full score (E_MDN, K = 10), first 1,024 ligands of C3", 3000, 30.0, 80, 16, 1024, 128, 500, 1,
                  1003, 2003, mdn_K=10),
+    # Not a BASELINE.json config: the C2 dock under the paper's FULL score (E_MDN, K = 10, pocket residues): the paper's own use
+    # case for "ms per docking task"
+    "M2": Config("M2", "Drug-like single dock under the full score (E_MDN, K = 10)", 3000, 30.0, 80, 16, 1, 384, 1000, 10, 1002, 2002,
+                 mdn_K=10),
     # Not a BASELINE.json config: C2 docked with the receptor term taken the paper's own way, direct sums over the receptor atoms
     # within the pair function's range, 200 MC steps
     "D2": Config("D2", "Drug-like single dock, receptor term by direct pair sums", 3000, 30.0, 80, 16, 1, 384, 200, 10, 1002, 2002, direct=True),
@@ -266,7 +270,7 @@ def config_sizes(cfg: Config, n_lig: int | None = None):
     rng = np.random.default_rng(cfg.lig_seed)
     if cfg.name == "C1":
         return np.full(L, 12), np.full(L, 2)
-    if cfg.name in ("C2", "P1", "C2x32", "D2"):
+    if cfg.name in ("C2", "P1", "C2x32", "D2", "M2"):
         return np.full(L, 30), np.full(L, 6)
     if cfg.name in ("C3", "M3"):
         n = rng.integers(15, 51, size=4096)
