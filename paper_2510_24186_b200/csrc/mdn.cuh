@@ -69,8 +69,8 @@ __device__ __forceinline__ void mdn_finish(const MdnDev& M, const float4* __rest
 // One ligand atom (internal index p of a ligand with n atoms) at (x, y, z) against residues i0, i0 + istep, ...
 // par = the ligand's parameter block [n_res][n] of slots (M.K4 float4 each).
 // e += w_mdn * (this atom's share of E_MDN); grad: (gx, gy, gz) += its gradient.
-// PIPE = false: the parameter block is requested when its run comes up (one buffer instead of two: for the instances whose
-// register budget cannot hold both).
+// PIPE = false: the parameter block is requested only once its run has passed the cut-off test, by the lane that evaluates it
+// (one buffer, no speculative loads: for the instances whose register budget cannot hold two).
 template <bool PIPE = true>
 __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restrict__ par, int n, int p, float x, float y, float z,
                                          int i0, int istep, bool grad, float& e, float& gx, float& gy, float& gz) {
@@ -101,7 +101,6 @@ __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restri
         const int i = hdr & 0xffff, cnt = hdr >> 16;             // cnt is even
         const float4* q = par + ((size_t)i * n + p) * M.K4;
         const int nh = __float_as_int(ra2.w);                    // the next run's header
-        if (!PIPE) mdn_load_block(q, nch0, nc);                 // (nc and rc are the same buffer then)
         if (nh >= 0) {
             mdn_ldg2(M.cell_at + en + cnt, na, na2);
             if (PIPE) mdn_load_block(par + ((size_t)(nh & 0xffff) * n + p) * M.K4, nch0, nc);
@@ -123,7 +122,10 @@ __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restri
             d2 = dx * dx + dy * dy + dz * dz;
             if (d2 < best2) { best2 = d2; bx = dx; by = dy; bz = dz; }
         }
-        if (best2 < cut2 && ord % istep == i0) mdn_finish(M, q, rc, best2, bx, by, bz, grad, e, gx, gy, gz);
+        if (best2 < cut2 && ord % istep == i0) {
+            if (!PIPE) mdn_load_block(q, nch0, nc);             // (nc and rc are the same buffer then)
+            mdn_finish(M, q, rc, best2, bx, by, bz, grad, e, gx, gy, gz);
+        }
         en += cnt; hdr = nh; ++ord;
     };
     for (;;) {
