@@ -922,7 +922,7 @@ extern "C" int tridsk_ligand_info(const tridsk_ligands* l, int* n_lig, int* max_
 
 // ---------------------------------------------------------------------------------------- E_MDN (O15)
 static void free_mdn(tridsk_ligands* l) {
-    for (int i = 0; i < 7; ++i) { if (l->mdn_buf[i]) cudaFree(l->mdn_buf[i]); l->mdn_buf[i] = nullptr; }
+    for (int i = 0; i < 9; ++i) { if (l->mdn_buf[i]) cudaFree(l->mdn_buf[i]); l->mdn_buf[i] = nullptr; }
     memset(&l->mdn, 0, sizeof(l->mdn));
 }
 
@@ -1022,6 +1022,22 @@ extern "C" int tridsk_load_mdn(tridsk_ctx* ctx, tridsk_ligands* ligs, const trid
         ctx->launches += 2;
         if (e != cudaSuccess) { free_mdn(ligs); return fail(ctx, e == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA, std::string("load_mdn cell list: ") + cudaGetErrorString(e)); }
         M.cell_off = (const int*)ligs->mdn_buf[5]; M.cell_at = (const float4*)ligs->mdn_buf[6];
+        // run directory: counted and filled the same way
+        e = cudaMalloc(&ligs->mdn_buf[7], sizeof(int) * (ncell + 1));
+        if (e == cudaSuccess) e = launch_mdn_dir(ctx->stream, M, false, (int*)ligs->mdn_buf[7], nullptr);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(cnt.data(), ligs->mdn_buf[7], sizeof(int) * ncell, cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        long long nrun = 0;
+        for (long long c = 0; c < ncell; ++c) { const int k = cnt[c]; cnt[c] = (int)nrun; nrun += k; }
+        cnt[ncell] = (int)nrun;
+        if (e == cudaSuccess && nrun > 0x7fffffffLL) e = cudaErrorInvalidValue;
+        if (e == cudaSuccess) e = cudaMalloc(&ligs->mdn_buf[8], sizeof(int2) * std::max<long long>(nrun, 1));
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ligs->mdn_buf[7], cnt.data(), sizeof(int) * (ncell + 1), cudaMemcpyHostToDevice, ctx->stream);
+        if (e == cudaSuccess) e = launch_mdn_dir(ctx->stream, M, true, (int*)ligs->mdn_buf[7], (int2*)ligs->mdn_buf[8]);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        ctx->launches += 2;
+        if (e != cudaSuccess) { free_mdn(ligs); return fail(ctx, e == cudaErrorMemoryAllocation ? TRIDSK_ENOMEM : TRIDSK_ECUDA, std::string("load_mdn run directory: ") + cudaGetErrorString(e)); }
+        M.dir_off = (const int*)ligs->mdn_buf[7]; M.dir = (const int2*)ligs->mdn_buf[8];
         if (getenv("TRIDSK_DEBUG")) fprintf(stderr, "tridsk load_mdn: %d residues, %lld cells of %.2f A, %.1f atoms per cell\n", m->n_res, ncell, cell, (double)run / (double)ncell);
     }
     ligs->mdn = M;

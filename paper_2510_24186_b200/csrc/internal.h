@@ -62,6 +62,10 @@ struct MdnDev {
     int nc[3];
     const int* cell_off;          // [ncells + 1]
     const float4* cell_at;
+    // run directory (for the mapping whose lanes SHARE an atom's candidate runs): the runs of cell c are dir[dir_off[c] .. dir_off[c + 1]),
+    // each {header = residue id | run length << 16, position of the run in cell_at}
+    const int* dir_off;           // [ncells + 1]
+    const int2* dir;
 };
 
 // Direct-pair receptor mode: the receptor atoms sorted into cubic cells of edge = the pair function's
@@ -368,7 +372,7 @@ struct tridsk_ligands {
     int* bucket_dev[TRIDSK_MAX_J + 1] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     // the mixture-density term (tridsk_load_mdn); mdn.n_res == 0: absent
     MdnDev mdn = {};
-    void* mdn_buf[7] = {};        // sph, res_off, rec, par, lig_off, cell_off, cell_at
+    void* mdn_buf[9] = {};        // sph, res_off, rec, par, lig_off, cell_off, cell_at, dir_off, dir
 };
 
 // ---------------------------------------------------------------- kernel launchers (one per .cu)
@@ -396,6 +400,7 @@ cudaError_t launch_score_direct(cudaStream_t s, const LigHdr* hdr, const float4*
 size_t topk_cluster_smem(int top_k, int max_atoms, int max_tor);
 cudaError_t launch_mdn_spheres(cudaStream_t s, const float* res_xyz, const int* res_off, int n_res, float d_cut, float4* rec, float4* sph);
 cudaError_t launch_mdn_cells(cudaStream_t s, const MdnDev& M, float cell, bool fill, int* counts_or_off, float4* cell_at);
+cudaError_t launch_mdn_dir(cudaStream_t s, const MdnDev& M, bool fill, int* counts_or_off, int2* dir);
 cudaError_t launch_mdn_pack(cudaStream_t s, const LigHdr* hdr, const int* atom_i, int n_lig, int n_res, int K, const long long* lig_off, const long long* in_off,
                             const float* pi, const float* mu, const float* sigma, float w_mdn, float4* par, int* bad);
 cudaError_t launch_microbench(cudaStream_t s, int which, int sm_count, void* buf, size_t bytes, int iters, float* sink, double* work);

@@ -487,7 +487,7 @@ __device__ __forceinline__ void cta_eval(const CtaTopo& S, const DGrid& G, const
     if (DIRECT) cta_rec_direct<GRAD, ENERGY>(RD, K, active, m & 0xff, x, y, z, part, S.lpa, ei, fx, fy, fz);
     if (MDN && active) {
         float mx = 0.f, my = 0.f, mz = 0.f;
-        mdn_atom<false>(M, mdn_par, n, atom, x, y, z, part, S.lpa, GRAD, ei, mx, my, mz);   // 168 registers here: one parameter buffer
+        mdn_atom_shared(M, mdn_par, n, atom, x, y, z, part, S.lpa, GRAD, ei, mx, my, mz);   // the atom's lanes split its candidate runs
         if (GRAD) { fx = fmaf(mx, K.inv_kappa, fx); fy = fmaf(my, K.inv_kappa, fy); fz = fmaf(mz, K.inv_kappa, fz); }   // kappa units, like the pair force
     }
     if (GRAD) {

@@ -121,3 +121,28 @@ cudaError_t launch_mdn_cells(cudaStream_t s, const MdnDev& M, float cell, bool f
     mdn_cell_kernel<<<(ncell + 127) / 128, 128, 0, s>>>(M, cell, fill, counts_or_off, cell_at);
     return cudaGetLastError();
 }
+
+// One thread per cell: walk the cell's stream run by run.  fill = false: counts[c] = number of runs; fill = true: the
+// directory entries {header, position in cell_at} written to dir[off[c] ..].
+__global__ void mdn_dir_kernel(MdnDev M, bool fill, int* __restrict__ counts_or_off, int2* __restrict__ dir) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int ncell = M.nc[0] * M.nc[1] * M.nc[2];
+    if (c >= ncell) return;
+    const int e1 = M.cell_off[c + 1];
+    int n = 0;
+    int2* dst = fill ? dir + counts_or_off[c] : nullptr;
+    for (int en = M.cell_off[c]; en < e1;) {
+        const int hdr = __float_as_int(M.cell_at[en].w);
+        if (fill) dst[n] = make_int2(hdr, en);
+        ++n;
+        en += hdr >> 16;
+    }
+    if (!fill) counts_or_off[c] = n;
+}
+
+cudaError_t launch_mdn_dir(cudaStream_t s, const MdnDev& M, bool fill, int* counts_or_off, int2* dir) {
+    const int ncell = M.nc[0] * M.nc[1] * M.nc[2];
+    if (ncell <= 0) return cudaSuccess;
+    mdn_dir_kernel<<<(ncell + 127) / 128, 128, 0, s>>>(M, fill, counts_or_off, dir);
+    return cudaGetLastError();
+}

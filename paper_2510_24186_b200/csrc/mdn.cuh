@@ -135,3 +135,52 @@ __device__ __forceinline__ void mdn_atom(const MdnDev& M, const float4* __restri
         if (en >= e1) break;
     }
 }
+
+// The same term for the mapping whose lanes SHARE an atom (CTA per chain, pair-record instance): lane i0 of the atom's istep
+// lanes takes the candidate runs i0, i0 + istep, ... of the cell through the run directory (internal.h) instead of walking
+// the whole stream -- the same assignment as mdn_atom's `ord % istep == i0`, so every lane's partial sum is the same, in a
+// quarter (an eighth, a half) of the dependent L2 round trips.  One buffer: the parameter block is requested once the run has
+// passed the cut-off test; the directory entry of the lane's next run is requested one run ahead.
+__device__ __forceinline__ void mdn_atom_shared(const MdnDev& M, const float4* __restrict__ par, int n, int p, float x, float y, float z,
+                                                int i0, int istep, bool grad, float& e, float& gx, float& gy, float& gz) {
+    const float ux = (x - M.glo[0]) * M.inv_cell, uy = (y - M.glo[1]) * M.inv_cell, uz = (z - M.glo[2]) * M.inv_cell;
+    const int ix = __float2int_rd(ux), iy = __float2int_rd(uy), iz = __float2int_rd(uz);
+    if ((unsigned)ix >= (unsigned)M.nc[0] || (unsigned)iy >= (unsigned)M.nc[1] || (unsigned)iz >= (unsigned)M.nc[2]) return;
+    const int cell = (iz * M.nc[1] + iy) * M.nc[0] + ix;
+    const int d1 = __ldg(M.dir_off + cell + 1);
+    int k = __ldg(M.dir_off + cell) + i0;
+    if (k >= d1) return;
+    const float cut2 = M.d_cut * M.d_cut;
+    const int nch0 = min(M.K4 >> 1, 4);
+    int2 de = __ldg(M.dir + k);
+    for (; k < d1; k += istep) {
+        const int hdr = de.x, en = de.y, cnt = hdr >> 16;         // cnt is even
+        float4 a, a2;
+        mdn_ldg2(M.cell_at + en, a, a2);
+        const int2 dn = __ldg(M.dir + min(k + istep, d1 - 1));    // this lane's next run (or a harmless re-read)
+        float bx = x - a.x, by = y - a.y, bz = z - a.z;
+        float best2 = bx * bx + by * by + bz * bz;
+        {
+            const float dx = x - a2.x, dy = y - a2.y, dz = z - a2.z;
+            const float d2 = dx * dx + dy * dy + dz * dz;
+            if (d2 < best2) { best2 = d2; bx = dx; by = dy; bz = dz; }
+        }
+        for (int r = 2; r < cnt; r += 2) {                        // plain minimum, ties -> lowest atom index
+            float4 b0, b1;
+            mdn_ldg2(M.cell_at + en + r, b0, b1);
+            float dx = x - b0.x, dy = y - b0.y, dz = z - b0.z;
+            float d2 = dx * dx + dy * dy + dz * dz;
+            if (d2 < best2) { best2 = d2; bx = dx; by = dy; bz = dz; }
+            dx = x - b1.x; dy = y - b1.y; dz = z - b1.z;
+            d2 = dx * dx + dy * dy + dz * dz;
+            if (d2 < best2) { best2 = d2; bx = dx; by = dy; bz = dz; }
+        }
+        if (best2 < cut2) {
+            const float4* q = par + ((size_t)(hdr & 0xffff) * n + p) * M.K4;
+            float v[32];
+            mdn_load_block(q, nch0, v);
+            mdn_finish(M, q, v, best2, bx, by, bz, grad, e, gx, gy, gz);
+        }
+        de = dn;
+    }
+}
