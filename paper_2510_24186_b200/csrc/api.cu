@@ -1378,7 +1378,11 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
         // every size and the lane form up to ~80 chains per SM (80-atom docks of 1,024 chains, 2 / 4 / 8 / 12 at once: CTA 107 / 207 /
         // 394 / 586 ms, warp 413 / 632 / - / -, lane - / - / 565 / 566)
         const bool all_dense = ligs->has_cta && ligs->cta_bucket[0][0].empty() && !ligs->cta_bucket[0][1].empty();
-        if (all_dense) mode = nch <= (size_t)ctx->sm_count * 76 ? 3 : 2;
+        // with the mixture-density term the CTA form -- the lanes of an atom split its candidate residues (mdn_atom_shared) -- holds
+        // ~49 M pose evaluations/s from one dock up; the lane form passes it at ~330 chains per SM (C2-sized ligands, K = 10, 8 / 32 /
+        // 128 / 256 docks of 384 chains: CTA 46.7 / 48.9 / 49.9 / 50.2 M/s, lane 7.0 / 26.8 / 50.4 / 66.1 M/s)
+        if (ligs->mdn.n_res > 0 && ligs->has_cta) mode = nch <= (size_t)ctx->sm_count * 330 ? 3 : 2;
+        else if (all_dense) mode = nch <= (size_t)ctx->sm_count * 76 ? 3 : 2;
         // batches without a ligand of 32 atoms or fewer: the warp form (two or more atoms per lane) is never the fastest; the CTA form
         // until the lane form's latency floor is reached (384-chain docks, 500 steps, 48 atoms, 2 / 4 / 16 at once: CTA 7.0 / 13.3 / 49 ms,
         // warp 16.7 / 18.2 / 72, lane 51 / 52 / 54; 64 atoms, 1 / 4 / 16 at once: CTA 4.5 / 17.2 / 63, warp 19.8 / 24.0 / 94, lane 79 / 87 / 91)

@@ -1168,22 +1168,29 @@ def test_m3_shaped_screen_under_the_full_score_sampled_against_oracle(orc, gp):
     n_at = np.diff(batch.atom_off)
     pi, mu, sg = synth.gmm_batch(len(res_off) - 1, n_at, cfg.mdn_K, seed=cfg.lig_seed + 50000)
     eng.load_mdn(ligs, res_xyz, res_off, pi, mu, sg, cfg.mdn_K)
-    r = eng.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, cfg.n_chains, 60, 1, seed=cfg.philox_seed)
-    assert eng.last_kernel() == 2
     ty, p = orc.Types(radius, role), orc.default_params()
     blk = np.concatenate([[0], np.cumsum((len(res_off) - 1) * n_at * cfg.mdn_K)])
-    with_term = 0
-    for l in range(0, 96, 8):
-        L = orc.ligand_from_batch(batch, l)
-        shp = (len(res_off) - 1, L.n, cfg.mdn_K)
-        M = orc.Mdn(res_xyz, res_off, pi[blk[l]:blk[l + 1]].reshape(shp), mu[blk[l]:blk[l + 1]].reshape(shp), sg[blk[l]:blk[l + 1]].reshape(shp))
-        pose = r["pose"][l, 0, :7 + L.T].astype(np.float64)
-        x = orc.fk(L, pose)
-        G = _sparse_oracle_grid(orc, p, ty, rec, x, L.type)
-        e_phys = orc.score_grad(p, ty, G, L, pose, want_grad=False)[0][0]
-        L.set_mdn(M)
-        eo = orc.score_grad(p, ty, G, L, pose, want_grad=False)[0][0]
-        with_term += (e_phys - eo) > 0.05
-        assert close(r["energy"][l, 0, 0], eo, rtol=2e-4, atol=2e-3), (l, r["energy"][l, 0, 0], eo)
-    assert with_term >= 8                                                       # the docked poses sit in range of pocket residues
+    # M3's 1,024 ligands x 128 chains go to the lane form; these 96 alone would go to the CTA form (fewer than 330 chains per SM
+    # with the term attached): both are run, the lane form forced
+    def rescore(r, forced):
+        with_term = 0
+        for l in range(0, 96, 8):
+            L = orc.ligand_from_batch(batch, l)
+            shp = (len(res_off) - 1, L.n, cfg.mdn_K)
+            M = orc.Mdn(res_xyz, res_off, pi[blk[l]:blk[l + 1]].reshape(shp), mu[blk[l]:blk[l + 1]].reshape(shp), sg[blk[l]:blk[l + 1]].reshape(shp))
+            pose = r["pose"][l, 0, :7 + L.T].astype(np.float64)
+            x = orc.fk(L, pose)
+            G = _sparse_oracle_grid(orc, p, ty, rec, x, L.type)
+            e_phys = orc.score_grad(p, ty, G, L, pose, want_grad=False)[0][0]
+            L.set_mdn(M)
+            eo = orc.score_grad(p, ty, G, L, pose, want_grad=False)[0][0]
+            with_term += (e_phys - eo) > 0.05
+            assert close(r["energy"][l, 0, 0], eo, rtol=2e-4, atol=2e-3), (forced, l, r["energy"][l, 0, 0], eo)
+        assert with_term >= 8                                                   # the docked poses sit in range of pocket residues
+
+    for forced, want_kernel in ((2, 2), (0, 3)):
+        eng.set_kernel(forced)
+        r = eng.dock(grid, ligs, gp, rec.box_min, rec.box_max, rec.pocket_center, rec.pocket_radius, cfg.n_chains, 60, 1, seed=cfg.philox_seed)
+        assert eng.last_kernel() == want_kernel
+        rescore(r, forced)
     ligs.free(); grid.free(); eng.close()
