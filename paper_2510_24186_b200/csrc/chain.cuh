@@ -294,6 +294,61 @@ __device__ __forceinline__ float pair_energy(const DParams& P, float d2, float d
     return e;
 }
 
+// ------------------------------------------------------------------ O2: four pairs at a time (the arithmetic of lane_rec)
+// Branch-free in the main part so that the four dependency chains interleave (a thread's pairs are otherwise a serial string of
+// shared-memory load -> rsqrt -> ex2 latencies): one lg2 for the product of the four clash ratios, the clash force switched by
+// one compare pair.  d* = x_a - x_b; c = dvdw + mu, or -1e15 for a slot without a pair, which then adds exactly zero;
+// hbw[u] & lbit != 0: slot u is a donor/acceptor pair (a slot group without any skips that term).  Out: s[u] = (de/dd) / d /
+// kappa, so that f_a += s (x_a - x_b).
+template <bool GRAD, bool ENERGY>
+__device__ __forceinline__ void pair_quad(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c[4],
+                                         const unsigned hbw[4], unsigned lbit, float& eL, float& eC, float& eH, float s[4]) {
+    float d[4], rinv[4], q[4], t[4], dc[4];
+    if (ENERGY) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            dc[u] = c[u] - K.mu;                                      // clash distance dvdw (negative: no pair)
+            if (hbw[u] != 0u) dc[u] = (hbw[u] & lbit) ? K.hb_dclash : dc[u];
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const float d2 = fmaf(dx[u], dx[u], fmaf(dy[u], dy[u], fmaf(dz[u], dz[u], 1e-12f)));
+        rinv[u] = rsqrt_approx(d2);
+        d[u] = d2 * rinv[u];
+        t[u] = d[u] - c[u];
+        const float w = t[u] * K.nk2;
+        float g = ex2_approx(w * t[u]);
+        g = d[u] < K.dmax ? g : 0.f;
+        s[u] = 0.f;
+        if (ENERGY) {
+            eL += g;
+            q[u] = fmaxf(dc[u] * fminf(rinv[u], K.inv_floor), 1.f);
+        }
+        if (GRAD) {
+            const float in = (t[u] < K.neg_mu && rinv[u] < K.inv_floor) ? 1.f : 0.f;
+            s[u] = rinv[u] * fmaf(in, K.nkc * rinv[u], w * g);
+        }
+    }
+    if (ENERGY) eC += lg2_approx((q[0] * q[1]) * (q[2] * q[3]));
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        if (hbw[u] != 0u) {
+            if (hbw[u] & lbit) {
+                const float th = d[u] - K.hb_mu;
+                float gh = ex2_approx(K.hb_nk2 * th * th);
+                gh = d[u] < K.hb_dmax ? gh : 0.f;
+                if (ENERGY) eH += gh;
+                if (GRAD) {
+                    s[u] = fmaf(K.kh * th, gh * rinv[u], s[u]);
+                    // the clash range of a donor/acceptor pair ends at hb_dclash, not at dvdw: put the term right
+                    const bool plain = t[u] < K.neg_mu, hb = d[u] < K.hb_dclash;
+                    if (plain != hb && rinv[u] < K.inv_floor) s[u] = fmaf(hb ? K.nkc : -K.nkc, rinv[u] * rinv[u], s[u]);
+                }
+            }
+        }
+    }
+}
 // ------------------------------------------------------------------ receptor term by direct pair sums (S:8(f) NEXT-3)
 // The paper's own evaluation (P:103-125, P:353 item 4): e(s_r, t, |x - r_r|) summed over the receptor atoms within the pair
 // function's range -- the cells within R.span of the atom's cell, cells and atoms in a fixed order.  No interpolation, no wall.
@@ -401,42 +456,54 @@ __device__ __forceinline__ void eval_pose(const Lig<J>& L, const DGrid& G, const
         if (MDN && L.valid[j]) mdn_atom(M, mdn_par, L.n, j * L.S + lane, x[j], y[j], z[j], 0, 1, GRAD, e_inter, fx[j], fy[j], fz[j]);
     }
 
-    // ---- a5 intra-ligand pairs: conflict-free rotation schedule, partner data by shuffle, reaction force shuffled back
+    // ---- a5 intra-ligand pairs: conflict-free rotation schedule, partner data by shuffle, reaction force shuffled back; four
+    // rounds at a time through the branch-free four-pair arithmetic (pair_quad), so that their dependency chains interleave
     {
+        const PairK K = make_pairk(P);
+        float eL = 0.f, eC = 0.f, eH = 0.f;
         int tile = 0;
 #pragma unroll
         for (int j1 = 0; j1 < J; ++j1) {
 #pragma unroll
             for (int j2 = j1; j2 < J; ++j2, ++tile) {
                 const int rb = L.tile_off[tile], re = L.tile_off[tile + 1];
-#pragma unroll 2
-                for (int r = rb; r < re; ++r) {
-                    const uint4 rd = __ldg(reinterpret_cast<const uint4*>(L.rounds + r));
-                    const int k = (int)rd.z;
-                    int src = lane + k; if (src >= L.S) src -= L.S;
-                    const float bx = __shfl_sync(FULL_MASK, x[j2], src);
-                    const float by = __shfl_sync(FULL_MASK, y[j2], src);
-                    const float bz = __shfl_sync(FULL_MASK, z[j2], src);
-                    const float br = __shfl_sync(FULL_MASK, L.rad[j2], src);
-                    float px = 0.f, py = 0.f, pz = 0.f;
-                    if ((rd.x >> lane) & 1u) {
-                        const float dx = x[j1] - bx, dy = y[j1] - by, dz = z[j1] - bz;
-                        float s;
-                        e_intra += pair_energy<GRAD>(P, dx * dx + dy * dy + dz * dz, L.rad[j1] + br, (rd.y >> lane) & 1u, s);
-                        if (GRAD) {
-                            px = s * dx; py = s * dy; pz = s * dz;
-                            fx[j1] += px; fy[j1] += py; fz[j1] += pz;
-                        }
+                for (int r = rb; r < re; r += 4) {
+                    float dx[4], dy[4], dz[4], c[4], sv[4];
+                    unsigned hbw[4];
+                    int kk[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const bool in = r + u < re;                // (a round past the end: empty masks)
+                        const uint4 rd = __ldg(reinterpret_cast<const uint4*>(L.rounds + (in ? r + u : rb)));
+                        const int k = (int)rd.z;
+                        kk[u] = k;
+                        int src = lane + k; if (src >= L.S) src -= L.S;
+                        const float bx = __shfl_sync(FULL_MASK, x[j2], src);
+                        const float by = __shfl_sync(FULL_MASK, y[j2], src);
+                        const float bz = __shfl_sync(FULL_MASK, z[j2], src);
+                        const float br = __shfl_sync(FULL_MASK, L.rad[j2], src);
+                        const bool on = in && ((rd.x >> lane) & 1u);
+                        dx[u] = x[j1] - bx; dy[u] = y[j1] - by; dz[u] = z[j1] - bz;
+                        c[u] = on ? (L.rad[j1] + br) + K.mu : -1e15f;
+                        hbw[u] = (on && ((rd.y >> lane) & 1u)) ? 1u : 0u;
                     }
+                    pair_quad<GRAD, true>(K, dx, dy, dz, c, hbw, 1u, eL, eC, eH, sv);
                     if (GRAD) {
-                        int dst = lane - k; if (dst < 0) dst += L.S;
-                        fx[j2] -= __shfl_sync(FULL_MASK, px, dst);
-                        fy[j2] -= __shfl_sync(FULL_MASK, py, dst);
-                        fz[j2] -= __shfl_sync(FULL_MASK, pz, dst);
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            const float s = K.kappa * sv[u];
+                            const float px = s * dx[u], py = s * dy[u], pz = s * dz[u];
+                            fx[j1] += px; fy[j1] += py; fz[j1] += pz;
+                            int dst = lane - kk[u]; if (dst < 0) dst += L.S;
+                            fx[j2] -= __shfl_sync(FULL_MASK, px, dst);
+                            fy[j2] -= __shfl_sync(FULL_MASK, py, dst);
+                            fz[j2] -= __shfl_sync(FULL_MASK, pz, dst);
+                        }
                     }
                 }
             }
         }
+        e_intra += fmaf(K.w_clash_ln2, eC, -fmaf(K.w_long, eL, K.w_hbond * eH));
     }
 
     if (!GRAD) return;

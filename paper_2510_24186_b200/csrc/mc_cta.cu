@@ -126,61 +126,6 @@ __device__ __forceinline__ void cta_stage(CtaTopo& S, CtaFrag& F, unsigned char*
     F.sub_hi = F.valid ? S.frag[e - 1].own_hi : 1;
 }
 
-// ------------------------------------------------------------------ O2: four pairs at a time (the arithmetic of lane_rec)
-// Branch-free in the main part so that the four dependency chains interleave (a thread's pairs are otherwise a serial string of
-// shared-memory load -> rsqrt -> ex2 latencies): one lg2 for the product of the four clash ratios, the clash force switched by
-// one compare pair.  d* = x_a - x_b; c = dvdw + mu, or -1e15 for a slot without a pair, which then adds exactly zero;
-// hbw[u] & lbit != 0: slot u is a donor/acceptor pair (a slot group without any skips that term).  Out: s[u] = (de/dd) / d /
-// kappa, so that f_a += s (x_a - x_b).
-template <bool GRAD, bool ENERGY>
-__device__ __forceinline__ void cta_quad(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c[4],
-                                         const unsigned hbw[4], unsigned lbit, float& eL, float& eC, float& eH, float s[4]) {
-    float d[4], rinv[4], q[4], t[4], dc[4];
-    if (ENERGY) {
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            dc[u] = c[u] - K.mu;                                      // clash distance dvdw (negative: no pair)
-            if (hbw[u] != 0u) dc[u] = (hbw[u] & lbit) ? K.hb_dclash : dc[u];
-        }
-    }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const float d2 = fmaf(dx[u], dx[u], fmaf(dy[u], dy[u], fmaf(dz[u], dz[u], 1e-12f)));
-        rinv[u] = rsqrt_approx(d2);
-        d[u] = d2 * rinv[u];
-        t[u] = d[u] - c[u];
-        const float w = t[u] * K.nk2;
-        float g = ex2_approx(w * t[u]);
-        g = d[u] < K.dmax ? g : 0.f;
-        s[u] = 0.f;
-        if (ENERGY) {
-            eL += g;
-            q[u] = fmaxf(dc[u] * fminf(rinv[u], K.inv_floor), 1.f);
-        }
-        if (GRAD) {
-            const float in = (t[u] < K.neg_mu && rinv[u] < K.inv_floor) ? 1.f : 0.f;
-            s[u] = rinv[u] * fmaf(in, K.nkc * rinv[u], w * g);
-        }
-    }
-    if (ENERGY) eC += lg2_approx((q[0] * q[1]) * (q[2] * q[3]));
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        if (hbw[u] != 0u) {
-            if (hbw[u] & lbit) {
-                const float th = d[u] - K.hb_mu;
-                float gh = ex2_approx(K.hb_nk2 * th * th);
-                gh = d[u] < K.hb_dmax ? gh : 0.f;
-                if (ENERGY) eH += gh;
-                if (GRAD) {
-                    s[u] = fmaf(K.kh * th, gh * rinv[u], s[u]);
-                    // the clash range of a donor/acceptor pair ends at hb_dclash, not at dvdw: put the term right
-                    const bool plain = t[u] < K.neg_mu, hb = d[u] < K.hb_dclash;
-                    if (plain != hb && rinv[u] < K.inv_floor) s[u] = fmaf(hb ? K.nkc : -K.nkc, rinv[u] * rinv[u], s[u]);
-                }
-            }
-        }
-    }
-}
 // record form: per-slot flags; a lane without a pair in slot u passes ok[u] = false
 template <bool GRAD, bool ENERGY>
 __device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], const float dy[4], const float dz[4], const float c_in[4],
@@ -190,7 +135,7 @@ __device__ __forceinline__ void cta_pairs4(const PairK& K, const float dx[4], co
     unsigned hbw[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) { c[u] = ok[u] ? c_in[u] : -1e15f; hbw[u] = (ok[u] && hb_in[u]) ? 1u : 0u; }
-    cta_quad<GRAD, ENERGY>(K, dx, dy, dz, c, hbw, 1u, eL, eC, eH, s);
+    pair_quad<GRAD, ENERGY>(K, dx, dy, dz, c, hbw, 1u, eL, eC, eH, s);
     if (GRAD) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) { fx = fmaf(s[u], dx[u], fx); fy = fmaf(s[u], dy[u], fy); fz = fmaf(s[u], dz[u], fz); }
@@ -205,7 +150,7 @@ __device__ __forceinline__ void cta_dense4(const PairK& K, const float4 me, cons
     float dx[4], dy[4], dz[4], s[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) { dx[u] = me.x - pb[u].x; dy[u] = me.y - pb[u].y; dz[u] = me.z - pb[u].z; }
-    cta_quad<GRAD, ENERGY>(K, dx, dy, dz, c, hbw, lbit, eL, eC, eH, s);
+    pair_quad<GRAD, ENERGY>(K, dx, dy, dz, c, hbw, lbit, eL, eC, eH, s);
     if (GRAD) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) { ax = fmaf(s[u], dx[u], ax); ay = fmaf(s[u], dy[u], ay); az = fmaf(s[u], dz[u], az); }
@@ -242,7 +187,7 @@ __device__ __forceinline__ void cta_rec_direct(const RecDev& R, const PairK& K, 
             c[u] = valid ? (__ldg(R.radius + st) + rt) + K.mu : -1e15f;
             hbw[u] = (valid && (((role_s & 1u) && (role_t & 2u)) || ((role_s & 2u) && (role_t & 1u)))) ? 1u : 0u;
         }
-        cta_quad<GRAD, ENERGY>(K, dx, dy, dz, c, hbw, 1u, eL, eC, eH, sv);
+        pair_quad<GRAD, ENERGY>(K, dx, dy, dz, c, hbw, 1u, eL, eC, eH, sv);
         if (GRAD) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) { fx = fmaf(sv[u], dx[u], fx); fy = fmaf(sv[u], dy[u], fy); fz = fmaf(sv[u], dz[u], fz); }
