@@ -292,9 +292,10 @@ int tridsk_dock_static(tridsk_ctx* ctx, const tridsk_grid* grid, const tridsk_li
                        float* out_energy, float* out_pose, int* out_chain);
 
 /*
- * Chain-to-thread mapping of the fused kernel: 0 = automatic (a CTA per chain for a single dock with
- * at most 5 chains per SM, a lane per chain when n_lig * n_chains >= 44 per SM, a warp per chain in between; batches without a ligand of 32 atoms or fewer: a CTA
- * per chain up to 60 chains per SM -- 76 when every ligand has more than 64 atoms --, a lane per chain beyond; with the mixture-density term attached: a CTA per chain up to 330 chains per SM), 1 = always
+ * Chain-to-thread mapping of the fused kernel: 0 = automatic (measured crossovers: a CTA per chain for a single
+ * dock -- up to 3 chains per SM, 5 when no ligand has 32 atoms or fewer --, a lane per chain from 64 chains per SM, a warp per
+ * chain in between; batches of ligands above 64 atoms only: a CTA per chain up to 76 chains per SM, a lane per chain beyond; with
+ * the mixture-density term attached: a CTA per chain up to 330 chains per SM, a lane per chain beyond), 1 = always
  * a warp per chain, 2 = always a lane per chain, 3 = always a CTA per chain (batches of at most 1024 ligands),
  * 4 = a lane per chain with the chains' coordinates in tensor memory (tcgen05.st/ld) for ligands of at most 42 atoms
  * where that keeps more warps resident -- same arithmetic and results as 2; experimental, never chosen automatically.

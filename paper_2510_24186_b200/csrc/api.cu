@@ -1374,22 +1374,20 @@ extern "C" int tridsk_dock(tridsk_ctx* ctx, const tridsk_grid* grid, const trids
     // tridsk_set_kernel overrides.
     int mode = ctx->kernel;
     if (mode == 0) {
-        // batches of ligands above 64 atoms only: the CTA kernel's dense-sweep instance (two warps per chain) beats the warp form at
-        // every size and the lane form up to ~80 chains per SM (80-atom docks of 1,024 chains, 2 / 4 / 8 / 12 at once: CTA 107 / 207 /
-        // 394 / 586 ms, warp 413 / 632 / - / -, lane - / - / 565 / 566)
+        // Measured on the final kernels (docks of 384 chains x 500 steps, 1 / 2 / 4 / 8 / 16 at once, ms):
+        //   20 atoms: CTA 2.2 / 4.2 / 7.9 / 14.5 / 28.6, warp 2.2 / 2.6 / 3.2 / 6.3 / 11.9, lane 12.6 / 13.1 / 13.1 / 13.1 / 13.3
+        //   30 atoms: CTA - / 5.0 / 9.2 / 16.7 / 32.9, warp - / 3.4 / 4.0 / 8.0 / 14.5, lane - / 24 / 24 / 26 / 26  (one C2 dock of 1,000 steps: CTA 5.7, warp 6.4)
+        //   48 atoms: CTA 3.5 / 5.8 / 11.1 / 19.0 / 35.7, warp 6.3 / 7.1 / 9.4 / 18.3 / 33.9, lane 51 / 51 / 52 / 52 / 53
+        //   64 atoms: CTA 4.5 / 8.3 / 16.3 / 27.1 / 51.8, warp - / 9.2 / 12.7 / 23.7 / 44.3, lane 79 / 79 / 87 / 87 / 91
+        //   80 atoms: CTA 10.7 / 12.6 / 24.4 / 40.0 / 76.5, warp 18.0 / 21.5 / 28.2 / 53.2 / 98.9, lane 134 / 134 / 136 / 136 / 136
+        // with the mixture-density term (C2-sized ligands, K = 10, 8 / 32 / 128 / 256 docks, M pose evaluations/s): CTA 46.7 / 48.9 /
+        // 49.9 / 50.2 (the lanes of an atom split its candidate residues), lane 7.0 / 26.8 / 50.4 / 66.1
         const bool all_dense = ligs->has_cta && ligs->cta_bucket[0][0].empty() && !ligs->cta_bucket[0][1].empty();
-        // with the mixture-density term the CTA form -- the lanes of an atom split its candidate residues (mdn_atom_shared) -- holds
-        // ~49 M pose evaluations/s from one dock up; the lane form passes it at ~330 chains per SM (C2-sized ligands, K = 10, 8 / 32 /
-        // 128 / 256 docks of 384 chains: CTA 46.7 / 48.9 / 49.9 / 50.2 M/s, lane 7.0 / 26.8 / 50.4 / 66.1 M/s)
-        if (ligs->mdn.n_res > 0 && ligs->has_cta) mode = nch <= (size_t)ctx->sm_count * 330 ? 3 : 2;
-        else if (all_dense) mode = nch <= (size_t)ctx->sm_count * 76 ? 3 : 2;
-        // batches without a ligand of 32 atoms or fewer: the warp form (two or more atoms per lane) is never the fastest; the CTA form
-        // until the lane form's latency floor is reached (384-chain docks, 500 steps, 48 atoms, 2 / 4 / 16 at once: CTA 7.0 / 13.3 / 49 ms,
-        // warp 16.7 / 18.2 / 72, lane 51 / 52 / 54; 64 atoms, 1 / 4 / 16 at once: CTA 4.5 / 17.2 / 63, warp 19.8 / 24.0 / 94, lane 79 / 87 / 91)
-        // (with the dense sweep for 33 .. 64 atoms beyond 3 chains per SM, 16 docks at once: 48 atoms 35.9 ms, 64 atoms 52.0 ms)
-        else if (ligs->has_cta && ligs->min_atoms > 32) mode = nch <= (size_t)ctx->sm_count * 60 ? 3 : 2;
-        else if (nch >= (size_t)ctx->sm_count * 44) mode = 2;       // measured crossover with the warp form: ~43 chains per SM (16 C2 docks)
-        else if (ligs->has_cta && nch <= (size_t)ctx->sm_count * 5) mode = 3;   // small ligands: the warp form catches up at two 384-chain docks
+        const size_t per_sm = (size_t)ctx->sm_count;
+        if (ligs->mdn.n_res > 0 && ligs->has_cta) mode = nch <= per_sm * 330 ? 3 : 2;
+        else if (all_dense) mode = nch <= per_sm * 76 ? 3 : 2;       // above 64 atoms (dense sweep): the CTA form beats the warp form at every size
+        else if (nch >= per_sm * 64) mode = 2;
+        else if (ligs->has_cta && nch <= per_sm * (ligs->min_atoms > 32 ? 5 : 3)) mode = 3;
         else mode = 1;
     }
     if (mode == 3) {
