@@ -181,6 +181,7 @@ extern "C" void tridsk_destroy(tridsk_ctx* ctx) {
     }
     for (int i = 0; i < TRIDSK_SCRATCH; ++i) if (ctx->scratch[i]) cudaFree(ctx->scratch[i]);
     if (ctx->pin) cudaFreeHost(ctx->pin);
+    if (ctx->pin_ev) cudaEventDestroy(ctx->pin_ev);
     if (ctx->own_stream) cudaStreamDestroy(ctx->stream);
     delete ctx;
 }
@@ -843,13 +844,14 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     const Seg s_hdr = seg(sizeof(LigHdr) * L), s_f4 = seg(sizeof(float4) * na), s_ai = seg(sizeof(int) * na), s_fr = seg(sizeof(FragRec) * nf),
               s_rd = seg(sizeof(PairRound) * nr), s_lf = seg(sizeof(LaneFrag) * nf), s_ls = seg(sizeof(uint4) * nls),
               s_lr = seg(sizeof(LaneRec) * nrec), s_cr = seg(sizeof(int) * ncr), s_cc = seg(sizeof(uint2) * ncc), s_rt = seg(sizeof(float) * nrt);
+    // the staging block is free once the last upload from it is done (an event, not the stream: kernels of an earlier dock may
+    // still be running there, and tridsk_screen wants this gather to overlap them)
+    if (ctx->pin_ev) cudaEventSynchronize(ctx->pin_ev);
     if (blob > ctx->pin_bytes) {
-        if (ctx->pin) { cudaStreamSynchronize(ctx->stream); cudaFreeHost(ctx->pin); ctx->pin = nullptr; ctx->pin_bytes = 0; }
+        if (ctx->pin) { cudaFreeHost(ctx->pin); ctx->pin = nullptr; ctx->pin_bytes = 0; }
         const size_t cap = blob + blob / 8;
         if (cudaHostAlloc(&ctx->pin, cap, cudaHostAllocDefault) != cudaSuccess) { cudaGetLastError(); delete lg; return fail(ctx, TRIDSK_ENOMEM, "pinned staging buffer"); }
         ctx->pin_bytes = cap;
-    } else {
-        cudaStreamSynchronize(ctx->stream);               // an earlier upload may still read the staging block
     }
     char* H = (char*)ctx->pin;
     memcpy(H + s_hdr.off, lg->hdr_h.data(), s_hdr.bytes);
@@ -880,6 +882,8 @@ extern "C" int tridsk_load_ligands(tridsk_ctx* ctx, const tridsk_ligand_batch* b
     const double t_c = dbg ? omp_get_wtime() : 0.0;
     cudaError_t e = cudaMalloc(&lg->blob, std::max<size_t>(blob, 256));
     if (e == cudaSuccess && blob) e = cudaMemcpyAsync(lg->blob, H, blob, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess && !ctx->pin_ev) e = cudaEventCreateWithFlags(&ctx->pin_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->pin_ev, ctx->stream);
     char* D = (char*)lg->blob;
     lg->hdr = (LigHdr*)(D + s_hdr.off); lg->atom_f4 = (float4*)(D + s_f4.off); lg->atom_i = (int*)(D + s_ai.off);
     lg->frags = (FragRec*)(D + s_fr.off); lg->rounds = (PairRound*)(D + s_rd.off); lg->lane_frags = (LaneFrag*)(D + s_lf.off);

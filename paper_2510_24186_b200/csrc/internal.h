@@ -307,6 +307,7 @@ struct tridsk_ctx {
     void* scratch[TRIDSK_SCRATCH] = {};
     size_t scratch_bytes[TRIDSK_SCRATCH] = {};
     void* pin = nullptr;          // pinned host staging block of tridsk_load_ligands (grown on demand)
+    cudaEvent_t pin_ev = nullptr; // recorded after the last upload from the staging block
     size_t pin_bytes = 0;
     // cached CUDA graph of the last dock launch series
     cudaGraphExec_t graph_exec = nullptr;
